@@ -1,0 +1,153 @@
+/* lqcd.h -- C ABI of liblqcd: even-odd preconditioned Wilson-clover operator and Krylov solves on
+ * one B200 (sm_100a).  Boundary of SURVEY.md §8(b); every step behind these calls runs in
+ * hand-written CUDA kernels (paper_2411_08461_b200/csrc).  No CPU fallback exists.
+ *
+ * Operator (Eq. 5, isotropic case; kappa normalisation, reading A2):
+ *     M = A - kappa * D,     A = 1 - kappa * csw * sum_{mu<nu} sigma_{mu nu} (x) F_{mu nu}
+ *     (D psi)(x) = sum_mu [ (1-g_mu) U_mu(x) psi(x+mu) + (1+g_mu) U_mu^dag(x-mu) psi(x-mu) ]
+ * DeGrand-Rossi gamma basis.  The paper's a_t*M equals M/(2 kappa).
+ *
+ * PUBLIC layouts (complex = interleaved (re,im) of the context's real type):
+ *     gauge   [4][2][Lt][Lz][Ly][Lx/2][3][3]   mu = 0..3 <-> x,y,z,t ; row-column colour order
+ *     spinor  [2][Lt][Lz][Ly][Lx/2][4][3]      even parity first
+ *     clover  [2][Lt][Lz][Ly][Lx/2][2][36] reals: per chiral block (upper, lower) 6 real diagonal
+ *             entries then the 15 strictly-lower complex entries, row-major ((i,j), i>j at
+ *             i(i-1)/2+j)
+ * NATIVE layouts are private structure-of-arrays of 16-byte vectors; the
+ * caller only needs their byte sizes (lqcd_*_bytes) and moves data with pack/unpack.
+ *
+ * Conventions.  Every pointer is a DEVICE pointer unless the name ends in _host.  The caller owns
+ * all buffers; the library keeps none beyond the call (the context owns only a small reduction
+ * scratch).  Device pointers must be 16-byte aligned.  All calls are asynchronous on `stream`
+ * (a cudaStream_t passed as void*) except lqcd_invert*, lqcd_*_host and lqcd_blas_*, which
+ * synchronise the stream before returning.  Return: 0 = OK, <0 = error, +1 = NOT_CONVERGED.
+ * No exceptions, no abort, nothing printed.  A context is not thread-safe.
+ */
+#ifndef LQCD_H
+#define LQCD_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lqcd_ctx lqcd_ctx;
+
+enum {
+  LQCD_OK = 0,
+  LQCD_NOT_CONVERGED = 1,
+  LQCD_ERR_INVALID_ARG = -1,
+  LQCD_ERR_DIMS = -2,
+  LQCD_ERR_ALIGN = -3,
+  LQCD_ERR_WORKSPACE = -4,
+  LQCD_ERR_CUDA = -5,
+  LQCD_ERR_SINGULAR_CLOVER = -6,
+  LQCD_ERR_BREAKDOWN = -7
+};
+enum { LQCD_SOLVER_CGNE = 0, LQCD_SOLVER_CGNR = 1, LQCD_SOLVER_BICGSTAB = 2 };
+enum { LQCD_MATPC_ASYMMETRIC = 0, LQCD_MATPC_SYMMETRIC = 1 };
+
+typedef struct lqcd_result {
+  int status;          /* LQCD_OK, LQCD_NOT_CONVERGED or LQCD_ERR_BREAKDOWN */
+  int iterations;
+  double iter_resid;   /* |r_hat| / |b| from the recurrence at exit                         */
+  double true_resid;   /* |b - M x| / |b| recomputed with the full operator (lqcd_mat_apply) */
+  double seconds;      /* device time of the whole call, CUDA events                        */
+  long dslash_count;   /* single-parity dslash launches                                     */
+  long kernel_launches;
+} lqcd_result;
+
+/* Context (init + LatticeInfo).  dims = {Lx,Ly,Lz,Lt}, each even and >= 4;
+ * prec = 4 (fp32) or 8 (fp64): the real type of every native AND public buffer of this context;
+ * recon = 18 (full links) or 12 (two rows stored, third recomputed); t_boundary = +1 or -1
+ * (antiperiodic in t, applied in-kernel to raw periodic links); device = CUDA
+ * ordinal (must be compute capability 10.x). */
+int lqcd_create(lqcd_ctx** ctx, const int dims[4], int prec, int recon, int t_boundary, int device);
+int lqcd_destroy(lqcd_ctx* ctx);
+const char* lqcd_strerror(int code);
+const char* lqcd_last_error(const lqcd_ctx* ctx);
+/* number of kernels this context has launched since creation (bench.py's gpu_launches) */
+long lqcd_launch_count(const lqcd_ctx* ctx);
+
+/* Byte sizes of native buffers: links (4 directions, both parities), ONE parity of a spinor,
+ * the clover field (both parities; same size for A and for A^-1), the solver workspace. */
+size_t lqcd_gauge_bytes(const lqcd_ctx* ctx);
+size_t lqcd_spinor_bytes(const lqcd_ctx* ctx);
+size_t lqcd_clover_bytes(const lqcd_ctx* ctx);
+size_t lqcd_invert_workspace_bytes(const lqcd_ctx* ctx, int solver);
+
+/* public <-> native ("QUDA needs to convert the data format to its native one").
+ * Spinor natives hold both parities: [2][one-parity native]. recon 12 drops the third row. */
+int lqcd_gauge_pack(lqcd_ctx* ctx, void* gauge_native, const void* gauge_public, void* stream);
+int lqcd_spinor_pack(lqcd_ctx* ctx, void* spinor_native, const void* spinor_public, void* stream);
+int lqcd_spinor_unpack(lqcd_ctx* ctx, void* spinor_public, const void* spinor_native, void* stream);
+int lqcd_clover_unpack(lqcd_ctx* ctx, void* clover_public, const void* clover_native, void* stream);
+
+/* Clover term and its inverse from the links ("the clover field is then created";
+ * SURVEY.md §8(c) O4-O6).  kappa is required because A contains kappa*csw (reading A6).  Leaves
+ * and the 6x6 inverses are computed in fp64 whatever the storage precision.  clover_inv may be
+ * NULL.  Synchronises; returns LQCD_ERR_SINGULAR_CLOVER if some block has a pivot < 1e-12|A|. */
+int lqcd_clover_build(lqcd_ctx* ctx, void* clover, void* clover_inv, const void* gauge, double csw,
+                      double kappa, void* stream);
+
+/* out = C in on one parity, C = the two Hermitian 6x6 chiral blocks per site of `clover_or_inv`
+ * (PAPER.md:56).  in/out: one-parity native spinors; they may alias. */
+int lqcd_clover_apply(lqcd_ctx* ctx, void* out, const void* in, const void* clover_or_inv, int parity,
+                      void* stream);
+
+/* out_p = scale * D_{p,1-p} in_{1-p}  (dagger != 0: D^dag).  parity = parity of `out` (0 even).
+ * in/out: one-parity native spinors, must not alias.  scale = 1 gives the bare hopping term
+ * (1320 flop/site); -kappa gives the off-diagonal block of M. */
+int lqcd_dslash(lqcd_ctx* ctx, void* out, const void* in, const void* gauge, int parity, double scale,
+                int dagger, void* stream);
+
+/* Even-even Schur complement on one-parity native spinors:
+ *   matpc 0: out = A_ee in - kappa^2 D_eo A_oo^-1 D_oe in
+ *   matpc 1: out = in - kappa^2 A_ee^-1 D_eo A_oo^-1 D_oe in      (dagger: the adjoint of either)
+ * tmp_o: one-parity scratch spinor. */
+int lqcd_mpc_apply(lqcd_ctx* ctx, void* out_e, const void* in_e, const void* gauge, const void* clover,
+                   const void* clover_inv, double kappa, int matpc, int dagger, void* tmp_o, void* stream);
+
+/* Full operator on both parities: out = A in - kappa D in (dagger: D^dag).  in/out: two-parity
+ * native spinors, must not alias. */
+int lqcd_mat_apply(lqcd_ctx* ctx, void* out, const void* in, const void* gauge, const void* clover,
+                   double kappa, int dagger, void* stream);
+
+/* Solve M x = b through the even-even Schur system,
+ * x0 = 0, stop when |r_hat| <= tol*|b| (reading A11), reconstruct the odd half, recompute the true
+ * residual.  x_public/b_public: public-layout device spinors.  clover/clover_inv: native fields
+ * from lqcd_clover_build; if clover == NULL both are built inside the workspace from
+ * (gauge, csw, kappa), otherwise csw is ignored.  workspace: >= lqcd_invert_workspace_bytes.
+ * Host-synchronous.  Returns res->status. */
+int lqcd_invert(lqcd_ctx* ctx, void* x_public, const void* b_public, const void* gauge, const void* clover,
+                const void* clover_inv, double kappa, double csw, double tol, int maxiter, int solver,
+                int matpc, void* workspace, size_t workspace_bytes, lqcd_result* res, void* stream);
+
+/* End-to-end variants with HOST buffers (pageable or pinned): the call uploads the public input,
+ * packs, computes, unpacks and downloads the public result.  Links/clover stay resident on the
+ * device (PAPER.md:225 loadGauge).  scratch: device buffer of >= lqcd_host_scratch_bytes. */
+size_t lqcd_host_scratch_bytes(const lqcd_ctx* ctx, int solver);
+int lqcd_dslash_host(lqcd_ctx* ctx, void* out_public_host, const void* in_public_host, const void* gauge,
+                     int parity, double scale, int dagger, void* scratch, void* stream);
+int lqcd_invert_host(lqcd_ctx* ctx, void* x_public_host, const void* b_public_host, const void* gauge,
+                     const void* clover, const void* clover_inv, double kappa, double tol, int maxiter,
+                     int solver, int matpc, void* scratch, size_t scratch_bytes, lqcd_result* res,
+                     void* stream);
+
+/* Fused BLAS-1 kernels of the solvers, exposed for parity tests and bandwidth measurement
+ * (SURVEY.md §8(a) a9).  Vectors are one-parity native spinors; results are fp64 on the host;
+ * these calls synchronise.  a, b are complex given as {re, im}.
+ *   lqcd_blas_axpy_norm : y += a*x (a real),  returns |y|^2
+ *   lqcd_blas_xpay      : y  = x + a*y (a real)
+ *   lqcd_blas_cdot      : returns <x,y> = sum conj(x_i) y_i  and |x|^2 in out[0..2]
+ *   lqcd_blas_caxpbypz  : z += a*x + b*y (a, b complex)
+ *   lqcd_blas_cxpaypbz  : y  = x + a*y + b*z ... see DESIGN.md for the BiCGStab updates */
+int lqcd_blas_axpy_norm(lqcd_ctx* ctx, double a, const void* x, void* y, double* norm2_host, void* stream);
+int lqcd_blas_xpay(lqcd_ctx* ctx, const void* x, double a, void* y, void* stream);
+int lqcd_blas_cdot(lqcd_ctx* ctx, const void* x, const void* y, double out_host[3], void* stream);
+int lqcd_blas_caxpbypz(lqcd_ctx* ctx, const double a[2], const void* x, const double b[2], const void* y,
+                       void* z, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LQCD_H */

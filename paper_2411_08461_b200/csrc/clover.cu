@@ -1,0 +1,238 @@
+// K4/K5: clover term from the clover-leaf field strength and its per-site inverse
+// ("the clover field is then created"; PAPER.md:56 packed layout; SURVEY.md §8(c)
+// O4-O6).  All arithmetic in fp64 whatever the storage precision; one thread per site.
+//
+//   F_{mu nu} = (Q - Q^dag)/(8i),  Q = sum of the four leaves around x (counter-clockwise)
+//   A = 1 - kappa*csw*sum_{mu<nu} sigma_{mu nu} (x) F_{mu nu}.   In the DeGrand-Rossi basis
+//   sigma_{mu nu} is block diagonal, so with  E3 = F_xy -/+ F_zt, E2 = F_xz +/- F_yt,
+//   E1 = F_yz -/+ F_xt  (upper sign: spins 0,1; lower sign: spins 2,3)
+//   A_block = 1 - kappa*csw * [[E3, E1 - i E2], [E1 + i E2, -E3]],  row index = 3*spin + colour.
+#include "lqcd_internal.cuh"
+
+struct cd {
+  double re, im;
+};
+__device__ __forceinline__ cd operator+(cd a, cd b) { return {a.re + b.re, a.im + b.im}; }
+__device__ __forceinline__ cd operator-(cd a, cd b) { return {a.re - b.re, a.im - b.im}; }
+__device__ __forceinline__ cd operator*(cd a, cd b) { return {a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re}; }
+__device__ __forceinline__ cd conj(cd a) { return {a.re, -a.im}; }
+__device__ __forceinline__ double abs2(cd a) { return a.re * a.re + a.im * a.im; }
+
+struct M3 {
+  cd m[9];
+};
+__device__ __forceinline__ M3 mul(const M3& a, const M3& b) {
+  M3 c;
+#pragma unroll
+  for (int i = 0; i < 3; i++)
+#pragma unroll
+    for (int j = 0; j < 3; j++) c.m[3 * i + j] = a.m[3 * i] * b.m[j] + a.m[3 * i + 1] * b.m[3 + j] + a.m[3 * i + 2] * b.m[6 + j];
+  return c;
+}
+__device__ __forceinline__ M3 dag(const M3& a) {
+  M3 c;
+#pragma unroll
+  for (int i = 0; i < 3; i++)
+#pragma unroll
+    for (int j = 0; j < 3; j++) c.m[3 * i + j] = conj(a.m[3 * j + i]);
+  return c;
+}
+
+// link U_mu at lattice coordinates (x,y,z,t) (already wrapped), promoted to fp64
+template <typename T, int R>
+__device__ __forceinline__ M3 link_at(const T* __restrict__ gauge, const Lat& L, int mu, const int* x) {
+  const int par = (x[0] + x[1] + x[2] + x[3]) & 1;
+  const int idx = (x[0] >> 1) + L.Lxh * (x[1] + L.Ly * (x[2] + L.Lz * x[3]));
+  T U[18];
+  load_link<T, R>(gauge + (size_t)(mu * 2 + par) * R * L.Vh, L.Vh, idx, U);
+  M3 m;
+#pragma unroll
+  for (int e = 0; e < 9; e++) m.m[e] = {(double)U[2 * e], (double)U[2 * e + 1]};
+  return m;
+}
+
+__device__ __forceinline__ void step(const Lat& L, int* x, int mu, int s) {
+  const int ext = (mu == 0) ? 2 * L.Lxh : (mu == 1) ? L.Ly : (mu == 2) ? L.Lz : L.Lt;
+  int v = x[mu] + s;
+  x[mu] = v < 0 ? v + ext : (v >= ext ? v - ext : v);
+}
+
+// F_{mu nu}(x) as 9 complex numbers
+template <typename T, int R>
+__device__ void field_strength(const T* __restrict__ g, const Lat& L, const int* x0, int mu, int nu, cd* F) {
+  int x[4], a[4], b[4], c[4];
+  M3 Q;
+  // P1 = U_mu(x) U_nu(x+mu) U_mu^dag(x+nu) U_nu^dag(x)
+  for (int i = 0; i < 4; i++) x[i] = a[i] = b[i] = x0[i];
+  step(L, a, mu, +1);
+  step(L, b, nu, +1);
+  Q = mul(mul(link_at<T, R>(g, L, mu, x), link_at<T, R>(g, L, nu, a)),
+          mul(dag(link_at<T, R>(g, L, mu, b)), dag(link_at<T, R>(g, L, nu, x))));
+  // P2 = U_nu(x) U_mu^dag(x-mu+nu) U_nu^dag(x-mu) U_mu(x-mu)
+  for (int i = 0; i < 4; i++) a[i] = b[i] = x0[i];
+  step(L, a, mu, -1);           // x-mu
+  for (int i = 0; i < 4; i++) b[i] = a[i];
+  step(L, b, nu, +1);           // x-mu+nu
+  {
+    M3 P = mul(mul(link_at<T, R>(g, L, nu, x), dag(link_at<T, R>(g, L, mu, b))),
+               mul(dag(link_at<T, R>(g, L, nu, a)), link_at<T, R>(g, L, mu, a)));
+    for (int e = 0; e < 9; e++) Q.m[e] = Q.m[e] + P.m[e];
+  }
+  // P3 = U_mu^dag(x-mu) U_nu^dag(x-mu-nu) U_mu(x-mu-nu) U_nu(x-nu)
+  for (int i = 0; i < 4; i++) b[i] = a[i];
+  step(L, b, nu, -1);           // x-mu-nu
+  for (int i = 0; i < 4; i++) c[i] = x0[i];
+  step(L, c, nu, -1);           // x-nu
+  {
+    M3 P = mul(mul(dag(link_at<T, R>(g, L, mu, a)), dag(link_at<T, R>(g, L, nu, b))),
+               mul(link_at<T, R>(g, L, mu, b), link_at<T, R>(g, L, nu, c)));
+    for (int e = 0; e < 9; e++) Q.m[e] = Q.m[e] + P.m[e];
+  }
+  // P4 = U_nu^dag(x-nu) U_mu(x-nu) U_nu(x+mu-nu) U_mu^dag(x)
+  for (int i = 0; i < 4; i++) b[i] = c[i];
+  step(L, b, mu, +1);           // x+mu-nu
+  {
+    M3 P = mul(mul(dag(link_at<T, R>(g, L, nu, c)), link_at<T, R>(g, L, mu, c)),
+               mul(link_at<T, R>(g, L, nu, b), dag(link_at<T, R>(g, L, mu, x))));
+    for (int e = 0; e < 9; e++) Q.m[e] = Q.m[e] + P.m[e];
+  }
+  // (Q - Q^dag)/(8i):  (z)/(i) = -i z
+#pragma unroll
+  for (int i = 0; i < 3; i++)
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+      cd d = Q.m[3 * i + j] - conj(Q.m[3 * j + i]);
+      F[3 * i + j] = {0.125 * d.im, -0.125 * d.re};
+    }
+}
+
+// Gauss-Jordan with partial pivoting on a 6x6 complex matrix held row-major in a[6][12] = [A | 1].
+// Returns false when a pivot is below 1e-12 * max|A|.
+__device__ bool invert6(cd (*a)[12]) {
+  double nrm = 0;
+  for (int i = 0; i < 6; i++)
+    for (int j = 0; j < 6; j++) nrm = fmax(nrm, abs2(a[i][j]));
+  const double thresh = 1e-24 * nrm;
+  for (int c = 0; c < 6; c++) {
+    int piv = c;
+    double best = abs2(a[c][c]);
+    for (int r = c + 1; r < 6; r++) {
+      double v = abs2(a[r][c]);
+      if (v > best) { best = v; piv = r; }
+    }
+    if (best <= thresh) return false;
+    if (piv != c)
+      for (int j = 0; j < 12; j++) { cd t = a[piv][j]; a[piv][j] = a[c][j]; a[c][j] = t; }
+    const cd p = a[c][c];
+    const cd inv = {p.re / best, -p.im / best};
+    for (int j = 0; j < 12; j++) a[c][j] = a[c][j] * inv;
+    for (int r = 0; r < 6; r++) {
+      if (r == c) continue;
+      const cd f = a[r][c];
+      for (int j = 0; j < 12; j++) a[r][j] = a[r][j] - f * a[c][j];
+    }
+  }
+  return true;
+}
+
+template <typename T>
+__device__ __forceinline__ void store_block(T* __restrict__ field, int Vh, int idx, int k, const double* p36) {
+  typedef typename V16<T>::vec vec;
+  constexpr int N = V16<T>::N;
+  vec* dst = reinterpret_cast<vec*>(field) + idx;
+  for (int q = 0; q < 36 / N; q++) {
+    T r[N];
+    for (int e = 0; e < N; e++) r[e] = (T)p36[q * N + e];
+    vec w;
+    vec_set(w, r);
+    dst[(size_t)(k * (36 / N) + q) * Vh] = w;
+  }
+}
+
+template <typename T, int R>
+__global__ void __launch_bounds__(64) clover_build_kernel(T* __restrict__ clover, T* __restrict__ clover_inv,
+                                                          const T* __restrict__ gauge, Lat L, double kc, int* flag) {
+  const int gid = blockIdx.x * blockDim.x + threadIdx.x;
+  if (gid >= 2 * L.Vh) return;
+  const int par = gid / L.Vh, idx = gid % L.Vh;
+  const Site s = site_of(L, idx, par);
+  const int x0[4] = {2 * s.xh + s.r, s.y, s.z, s.t};
+  cd F[6][9];  // planes xy, xz, xt, yz, yt, zt
+  {
+    int pl = 0;
+    for (int mu = 0; mu < 4; mu++)
+      for (int nu = mu + 1; nu < 4; nu++) field_strength<T, R>(gauge, L, x0, mu, nu, F[pl++]);
+  }
+  const size_t half = (size_t)72 * L.Vh;  // reals per parity of a clover field
+  for (int k = 0; k < 2; k++) {
+    const double sg = k == 0 ? 1.0 : -1.0;
+    cd B[6][6];
+    for (int i = 0; i < 3; i++)
+      for (int j = 0; j < 3; j++) {
+        const int e = 3 * i + j;
+        cd E3 = {F[0][e].re - sg * F[5][e].re, F[0][e].im - sg * F[5][e].im};  // F_xy -/+ F_zt
+        cd E2 = {F[1][e].re + sg * F[4][e].re, F[1][e].im + sg * F[4][e].im};  // F_xz +/- F_yt
+        cd E1 = {F[3][e].re - sg * F[2][e].re, F[3][e].im - sg * F[2][e].im};  // F_yz -/+ F_xt
+        const double d = (i == j) ? 1.0 : 0.0;
+        B[i][j] = {d - kc * E3.re, -kc * E3.im};
+        B[3 + i][3 + j] = {d + kc * E3.re, kc * E3.im};
+        B[i][3 + j] = {-kc * (E1.re + E2.im), -kc * (E1.im - E2.re)};      // E1 - i E2
+        B[3 + i][j] = {-kc * (E1.re - E2.im), -kc * (E1.im + E2.re)};      // E1 + i E2
+      }
+    double pk[36];
+    for (int i = 0; i < 6; i++) pk[i] = B[i][i].re;
+    for (int i = 1; i < 6; i++)
+      for (int j = 0; j < i; j++) {
+        // Hermitian by construction; average the two triangles so rounding stays symmetric
+        const int o = 6 + 2 * (i * (i - 1) / 2 + j);
+        pk[o] = 0.5 * (B[i][j].re + B[j][i].re);
+        pk[o + 1] = 0.5 * (B[i][j].im - B[j][i].im);
+      }
+    store_block<T>(clover + par * half, L.Vh, idx, k, pk);
+    if (clover_inv) {
+      cd a[6][12];
+      for (int i = 0; i < 6; i++)
+        for (int j = 0; j < 6; j++) {
+          a[i][j] = B[i][j];
+          a[i][6 + j] = {i == j ? 1.0 : 0.0, 0.0};
+        }
+      if (!invert6(a)) {
+        atomicExch(flag, 1);
+        for (int i = 0; i < 36; i++) pk[i] = 0;
+      } else {
+        for (int i = 0; i < 6; i++) pk[i] = a[i][6 + i].re;
+        for (int i = 1; i < 6; i++)
+          for (int j = 0; j < i; j++) {
+            const int o = 6 + 2 * (i * (i - 1) / 2 + j);
+            pk[o] = 0.5 * (a[i][6 + j].re + a[j][6 + i].re);
+            pk[o + 1] = 0.5 * (a[i][6 + j].im - a[j][6 + i].im);
+          }
+      }
+      store_block<T>(clover_inv + par * half, L.Vh, idx, k, pk);
+    }
+  }
+}
+
+extern "C" int lqcd_clover_build(lqcd_ctx* c, void* clover, void* clover_inv, const void* gauge, double csw,
+                                 double kappa, void* stream) {
+  if (!c || !clover || !gauge) return LQCD_ERR_INVALID_ARG;
+  if (!lqcd_aligned16(clover) || !lqcd_aligned16(clover_inv) || !lqcd_aligned16(gauge))
+    return lqcd_set_error(c, LQCD_ERR_ALIGN, "clover_build: alignment");
+  cudaStream_t st = as_stream(stream);
+  const int n = 2 * c->lat.Vh, block = 64, grid = (n + block - 1) / block;
+  const double kc = kappa * csw;
+  cudaMemsetAsync(c->d_flag, 0, sizeof(int), st);
+  if (c->prec == 4 && c->recon == 18)
+    clover_build_kernel<float, 18><<<grid, block, 0, st>>>((float*)clover, (float*)clover_inv, (const float*)gauge, c->lat, kc, c->d_flag);
+  else if (c->prec == 4)
+    clover_build_kernel<float, 12><<<grid, block, 0, st>>>((float*)clover, (float*)clover_inv, (const float*)gauge, c->lat, kc, c->d_flag);
+  else if (c->recon == 18)
+    clover_build_kernel<double, 18><<<grid, block, 0, st>>>((double*)clover, (double*)clover_inv, (const double*)gauge, c->lat, kc, c->d_flag);
+  else
+    clover_build_kernel<double, 12><<<grid, block, 0, st>>>((double*)clover, (double*)clover_inv, (const double*)gauge, c->lat, kc, c->d_flag);
+  LQCD_LAUNCH_CHECK(c, "clover_build");
+  cudaMemcpyAsync(c->h_flag, c->d_flag, sizeof(int), cudaMemcpyDeviceToHost, st);
+  if (cudaStreamSynchronize(st) != cudaSuccess) return lqcd_check_cuda(c, "clover_build sync");
+  if (c->h_flag[0]) return lqcd_set_error(c, LQCD_ERR_SINGULAR_CLOVER, "clover_build: singular 6x6 block");
+  return LQCD_OK;
+}

@@ -1,0 +1,119 @@
+// Context, error reporting and size queries of liblqcd (include/lqcd.h).
+#include <stdarg.h>
+#include <string.h>
+#include "lqcd_internal.cuh"
+
+int lqcd_set_error(lqcd_ctx* ctx, int code, const char* fmt, ...) {
+  if (ctx) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(ctx->err, sizeof(ctx->err), fmt, ap);
+    va_end(ap);
+  }
+  return code;
+}
+
+int lqcd_check_cuda(lqcd_ctx* ctx, const char* what) {
+  cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess) return LQCD_OK;
+  return lqcd_set_error(ctx, LQCD_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+extern "C" {
+
+const char* lqcd_strerror(int code) {
+  switch (code) {
+    case LQCD_OK: return "ok";
+    case LQCD_NOT_CONVERGED: return "not converged within maxiter";
+    case LQCD_ERR_INVALID_ARG: return "invalid argument";
+    case LQCD_ERR_DIMS: return "unsupported lattice dimensions";
+    case LQCD_ERR_ALIGN: return "device pointer not 16-byte aligned";
+    case LQCD_ERR_WORKSPACE: return "workspace too small";
+    case LQCD_ERR_CUDA: return "CUDA error";
+    case LQCD_ERR_SINGULAR_CLOVER: return "singular clover block";
+    case LQCD_ERR_BREAKDOWN: return "solver breakdown";
+    default: return "unknown error code";
+  }
+}
+
+const char* lqcd_last_error(const lqcd_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+long lqcd_launch_count(const lqcd_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int lqcd_create(lqcd_ctx** out, const int dims[4], int prec, int recon, int t_boundary, int device) {
+  if (!out || !dims) return LQCD_ERR_INVALID_ARG;
+  *out = nullptr;
+  if ((prec != 4 && prec != 8) || (recon != 18 && recon != 12) || (t_boundary != 1 && t_boundary != -1))
+    return LQCD_ERR_INVALID_ARG;
+  long V = 1;
+  for (int i = 0; i < 4; i++) {
+    if (dims[i] < 4 || (dims[i] & 1)) return LQCD_ERR_DIMS;
+    V *= dims[i];
+  }
+  if (V / 2 > 0x3fffffffL) return LQCD_ERR_DIMS;  // 32-bit site indices inside kernels
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+    cudaGetLastError();
+    return LQCD_ERR_CUDA;  // no CPU fallback: without a device the library does nothing
+  }
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return LQCD_ERR_CUDA;
+  if (prop.major != 10) return LQCD_ERR_CUDA;  // kernels are built for sm_100a only
+  if (cudaSetDevice(device) != cudaSuccess) return LQCD_ERR_CUDA;
+
+  lqcd_ctx* c = new lqcd_ctx();
+  memset(c, 0, sizeof(*c));
+  for (int i = 0; i < 4; i++) c->L[i] = dims[i];
+  c->V = V;
+  c->lat.Lxh = dims[0] / 2;
+  c->lat.Ly = dims[1];
+  c->lat.Lz = dims[2];
+  c->lat.Lt = dims[3];
+  c->lat.Vh = (int)(V / 2);
+  c->lat.tb = t_boundary;
+  c->prec = prec;
+  c->recon = recon;
+  c->device = device;
+  c->sm_count = prop.multiProcessorCount;
+  c->max_red_blocks = 8 * c->sm_count;
+  strcpy(c->err, "ok");
+  bool ok = cudaMalloc(&c->d_partial, sizeof(double) * 8 * c->max_red_blocks) == cudaSuccess &&
+            cudaMalloc(&c->d_scalars, sizeof(double) * 64) == cudaSuccess &&
+            cudaMalloc(&c->d_ticket, sizeof(unsigned int) * 4) == cudaSuccess &&
+            cudaMalloc(&c->d_flag, sizeof(int) * 4) == cudaSuccess &&
+            cudaMallocHost(&c->h_scalars, sizeof(double) * 64) == cudaSuccess &&
+            cudaMallocHost(&c->h_flag, sizeof(int) * 4) == cudaSuccess &&
+            cudaEventCreate(&c->ev0) == cudaSuccess && cudaEventCreate(&c->ev1) == cudaSuccess;
+  if (ok) {
+    ok = cudaMemset(c->d_ticket, 0, sizeof(unsigned int) * 4) == cudaSuccess &&
+         cudaMemset(c->d_flag, 0, sizeof(int) * 4) == cudaSuccess &&
+         cudaMemset(c->d_scalars, 0, sizeof(double) * 64) == cudaSuccess;
+  }
+  if (!ok) {
+    cudaGetLastError();
+    lqcd_destroy(c);
+    return LQCD_ERR_CUDA;
+  }
+  *out = c;
+  return LQCD_OK;
+}
+
+int lqcd_destroy(lqcd_ctx* c) {
+  if (!c) return LQCD_ERR_INVALID_ARG;
+  cudaSetDevice(c->device);
+  if (c->d_partial) cudaFree(c->d_partial);
+  if (c->d_scalars) cudaFree(c->d_scalars);
+  if (c->d_ticket) cudaFree(c->d_ticket);
+  if (c->d_flag) cudaFree(c->d_flag);
+  if (c->h_scalars) cudaFreeHost(c->h_scalars);
+  if (c->h_flag) cudaFreeHost(c->h_flag);
+  if (c->ev0) cudaEventDestroy(c->ev0);
+  if (c->ev1) cudaEventDestroy(c->ev1);
+  delete c;
+  return LQCD_OK;
+}
+
+size_t lqcd_gauge_bytes(const lqcd_ctx* c) { return c ? (size_t)4 * c->V * c->recon * c->prec : 0; }
+size_t lqcd_spinor_bytes(const lqcd_ctx* c) { return c ? (size_t)c->lat.Vh * 24 * c->prec : 0; }
+size_t lqcd_clover_bytes(const lqcd_ctx* c) { return c ? (size_t)c->V * 72 * c->prec : 0; }
+
+}  // extern "C"

@@ -1,0 +1,131 @@
+// K2 dslash kernel with fused epilogues and K3 clover apply.
+#include "dslash.cuh"
+
+// Epilogues (EPI), with d = D_{p,1-p} in  and C = the clover-like field passed in `cl`:
+//   0: out = scale * d
+//   1: out = scale * C d                 (e.g. A_oo^-1 D_oe x)
+//   2: out = C x + scale * d             (asymmetric Mhat:  A_ee x - k^2 D_eo t)
+//   3: out = x + scale * C d             (symmetric  Mhat:  x - k^2 A_ee^-1 D_eo t)
+template <typename T> struct DslashArgs {
+  T* out;
+  const T* in;
+  const T* gauge;
+  const T* cl;  // one-parity clover field of the OUTPUT parity (EPI 1..3)
+  const T* x;   // one-parity spinor of the OUTPUT parity (EPI 2, 3)
+  Lat lat;
+  int parity;
+  T scale;
+};
+
+template <typename T, int R, bool DAG, int EPI>
+__global__ void __launch_bounds__(128) dslash_kernel(const DslashArgs<T> a) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= a.lat.Vh) return;
+  T acc[24];
+  dslash_site<T, R, DAG>(acc, a.in, a.gauge, a.lat, idx, a.parity);
+  T res[24];
+  if (EPI == 0) {
+#pragma unroll
+    for (int e = 0; e < 24; e++) res[e] = a.scale * acc[e];
+  } else if (EPI == 1) {
+    clover_mul<T>(a.cl, a.lat.Vh, idx, acc, res);
+#pragma unroll
+    for (int e = 0; e < 24; e++) res[e] *= a.scale;
+  } else if (EPI == 2) {
+    T xv[24];
+    load_spinor<T>(a.x, a.lat.Vh, idx, xv);
+    clover_mul<T>(a.cl, a.lat.Vh, idx, xv, res);
+#pragma unroll
+    for (int e = 0; e < 24; e++) res[e] += a.scale * acc[e];
+  } else {
+    T xv[24];
+    load_spinor<T>(a.x, a.lat.Vh, idx, xv);
+    clover_mul<T>(a.cl, a.lat.Vh, idx, acc, res);
+#pragma unroll
+    for (int e = 0; e < 24; e++) res[e] = xv[e] + a.scale * res[e];
+  }
+  store_spinor<T>(a.out, a.lat.Vh, idx, res);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(128) clover_apply_kernel(T* __restrict__ out, const T* __restrict__ in,
+                                                           const T* __restrict__ cl, int Vh) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= Vh) return;
+  T v[24], r[24];
+  load_spinor<T>(in, Vh, idx, v);
+  clover_mul<T>(cl, Vh, idx, v, r);
+  store_spinor<T>(out, Vh, idx, r);
+}
+
+template <typename T, int R, bool DAG>
+static void launch_epi(const DslashArgs<T>& a, int epi, cudaStream_t st) {
+  const int block = 128;
+  const int grid = (a.lat.Vh + block - 1) / block;
+  switch (epi) {
+    case 0: dslash_kernel<T, R, DAG, 0><<<grid, block, 0, st>>>(a); break;
+    case 1: dslash_kernel<T, R, DAG, 1><<<grid, block, 0, st>>>(a); break;
+    case 2: dslash_kernel<T, R, DAG, 2><<<grid, block, 0, st>>>(a); break;
+    default: dslash_kernel<T, R, DAG, 3><<<grid, block, 0, st>>>(a); break;
+  }
+}
+
+template <typename T>
+static void launch_typed(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
+                         int parity, double scale, int dagger, int epi, cudaStream_t st) {
+  DslashArgs<T> a;
+  a.out = (T*)out;
+  a.in = (const T*)in;
+  a.gauge = (const T*)gauge;
+  a.cl = (const T*)cl;
+  a.x = (const T*)x;
+  a.lat = c->lat;
+  a.parity = parity;
+  a.scale = (T)scale;
+  if (c->recon == 18) {
+    if (dagger) launch_epi<T, 18, true>(a, epi, st);
+    else launch_epi<T, 18, false>(a, epi, st);
+  } else {
+    if (dagger) launch_epi<T, 12, true>(a, epi, st);
+    else launch_epi<T, 12, false>(a, epi, st);
+  }
+}
+
+// internal entry used by the C ABI and by the solvers.  cl: one-parity clover block of the output
+// parity (or NULL for epi 0); x: one-parity spinor (epi 2,3).
+int lqcd_dslash_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
+                       int parity, double scale, int dagger, int epi, cudaStream_t st) {
+  if (c->prec == 4) launch_typed<float>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, st);
+  else launch_typed<double>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, st);
+  LQCD_LAUNCH_CHECK(c, "dslash");
+  return LQCD_OK;
+}
+
+int lqcd_clover_apply_launch(lqcd_ctx* c, void* out, const void* in, const void* cl_parity, cudaStream_t st) {
+  const int Vh = c->lat.Vh, block = 128, grid = (Vh + block - 1) / block;
+  if (c->prec == 4) clover_apply_kernel<float><<<grid, block, 0, st>>>((float*)out, (const float*)in, (const float*)cl_parity, Vh);
+  else clover_apply_kernel<double><<<grid, block, 0, st>>>((double*)out, (const double*)in, (const double*)cl_parity, Vh);
+  LQCD_LAUNCH_CHECK(c, "clover_apply");
+  return LQCD_OK;
+}
+
+extern "C" {
+
+int lqcd_dslash(lqcd_ctx* c, void* out, const void* in, const void* gauge, int parity, double scale, int dagger,
+                void* stream) {
+  if (!c || !out || !in || !gauge || (parity != 0 && parity != 1)) return LQCD_ERR_INVALID_ARG;
+  if (out == in) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "dslash: out aliases in");
+  if (!lqcd_aligned16(out) || !lqcd_aligned16(in) || !lqcd_aligned16(gauge))
+    return lqcd_set_error(c, LQCD_ERR_ALIGN, "dslash: alignment");
+  return lqcd_dslash_launch(c, out, in, gauge, nullptr, nullptr, parity, scale, dagger ? 1 : 0, 0, as_stream(stream));
+}
+
+int lqcd_clover_apply(lqcd_ctx* c, void* out, const void* in, const void* clover, int parity, void* stream) {
+  if (!c || !out || !in || !clover || (parity != 0 && parity != 1)) return LQCD_ERR_INVALID_ARG;
+  if (!lqcd_aligned16(out) || !lqcd_aligned16(in) || !lqcd_aligned16(clover))
+    return lqcd_set_error(c, LQCD_ERR_ALIGN, "clover_apply: alignment");
+  const char* cl = (const char*)clover + (size_t)parity * (lqcd_clover_bytes(c) / 2);
+  return lqcd_clover_apply_launch(c, out, in, cl, as_stream(stream));
+}
+
+}  // extern "C"

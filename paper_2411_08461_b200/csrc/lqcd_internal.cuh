@@ -1,0 +1,176 @@
+// Internal declarations of liblqcd (CUDA, sm_100a).  Not part of the C ABI (include/lqcd.h).
+// Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include "lqcd.h"
+
+// ---------------------------------------------------------------------------------------------
+// Lattice geometry handed to kernels by value.  Checkerboard index of a site of parity p
+// (cb2 layout [2][Lt][Lz][Ly][Lx/2]):  c = xh + Lxh*(y + Ly*(z + Lz*t)),
+// x = 2*xh + ((p + y + z + t) & 1).
+// ---------------------------------------------------------------------------------------------
+struct Lat {
+  int Lxh, Ly, Lz, Lt;
+  int Vh;
+  int tb;  // +1 periodic, -1 antiperiodic in t
+};
+
+struct lqcd_ctx {
+  int L[4];
+  Lat lat;
+  long V;
+  int prec, recon, device, sm_count;
+  long launches;
+  char err[256];
+  // reduction scratch (device): per-block partials, ticket counter, result slots; pinned host mirror
+  double* d_partial;
+  double* d_scalars;
+  unsigned int* d_ticket;
+  int* d_flag;
+  double* h_scalars;
+  int* h_flag;
+  int max_red_blocks;
+  cudaEvent_t ev0, ev1;
+};
+
+int lqcd_set_error(lqcd_ctx* ctx, int code, const char* fmt, ...);
+int lqcd_check_cuda(lqcd_ctx* ctx, const char* what);
+static inline bool lqcd_aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+
+// ---------------------------------------------------------------------------------------------
+// Native structure-of-arrays layouts: arrays of 16-byte vectors, vector index slowest.
+//   spinor (one parity): [NSV][Vh] vec16,  24 reals per site in (spin, colour, re/im) order
+//   clover (one parity): [NCV][Vh] vec16,  72 reals per site in the public packed order
+//   links               : [mu][parity][NGV][Vh] gauge-vec; first R reals of the row-major 3x3
+// fp32: vec16 = float4 (4 reals), fp64: vec16 = double2 (2 reals).  fp32 recon-18 links use
+// float2 (9 per link); every other link variant uses 16-byte vectors.
+// ---------------------------------------------------------------------------------------------
+template <typename T> struct V16;
+template <> struct V16<float> { typedef float4 vec; static constexpr int N = 4; };
+template <> struct V16<double> { typedef double2 vec; static constexpr int N = 2; };
+
+template <typename T, int R> struct GV { typedef typename V16<T>::vec vec; static constexpr int N = V16<T>::N; };
+template <> struct GV<float, 18> { typedef float2 vec; static constexpr int N = 2; };
+
+template <typename T> struct Lay {
+  static constexpr int N = V16<T>::N;
+  static constexpr int NSV = 24 / N;  // vectors per spinor site
+  static constexpr int NCV = 72 / N;  // vectors per clover site
+};
+
+__device__ __forceinline__ void vec_get(const float4& v, float* r) { r[0] = v.x; r[1] = v.y; r[2] = v.z; r[3] = v.w; }
+__device__ __forceinline__ void vec_get(const double2& v, double* r) { r[0] = v.x; r[1] = v.y; }
+__device__ __forceinline__ void vec_get(const float2& v, float* r) { r[0] = v.x; r[1] = v.y; }
+__device__ __forceinline__ void vec_set(float4& v, const float* r) { v = make_float4(r[0], r[1], r[2], r[3]); }
+__device__ __forceinline__ void vec_set(double2& v, const double* r) { v = make_double2(r[0], r[1]); }
+__device__ __forceinline__ void vec_set(float2& v, const float* r) { v = make_float2(r[0], r[1]); }
+
+// read-only streaming load (links, clover: touched once per sweep) and default cached load
+template <typename V> __device__ __forceinline__ V ld_stream(const V* p) { return __ldcs(p); }
+template <typename V> __device__ __forceinline__ V ld_cached(const V* p) { return __ldg(p); }
+
+template <typename T>
+__device__ __forceinline__ void load_spinor(const T* __restrict__ base, int Vh, int idx, T* psi) {
+  typedef typename V16<T>::vec vec;
+  const vec* p = reinterpret_cast<const vec*>(base) + idx;
+#pragma unroll
+  for (int v = 0; v < Lay<T>::NSV; v++) {
+    vec q = ld_cached(p + (size_t)v * Vh);
+    vec_get(q, psi + v * V16<T>::N);
+  }
+}
+template <typename T>
+__device__ __forceinline__ void store_spinor(T* __restrict__ base, int Vh, int idx, const T* psi) {
+  typedef typename V16<T>::vec vec;
+  vec* p = reinterpret_cast<vec*>(base) + idx;
+#pragma unroll
+  for (int v = 0; v < Lay<T>::NSV; v++) {
+    vec q;
+    vec_set(q, psi + v * V16<T>::N);
+    p[(size_t)v * Vh] = q;
+  }
+}
+
+// bytes of one link-field block [NGV][Vh] for (mu, parity)
+template <typename T, int R> __host__ __device__ constexpr int gauge_nvec() { return R / GV<T, R>::N; }
+
+// load one link into U[18] (row-major, (re,im)); recon-12 rebuilds row 2 = conj(row0 x row1)
+template <typename T, int R>
+__device__ __forceinline__ void load_link(const T* __restrict__ block, int Vh, int idx, T* U) {
+  typedef typename GV<T, R>::vec vec;
+  constexpr int N = GV<T, R>::N;
+  const vec* p = reinterpret_cast<const vec*>(block) + idx;
+#pragma unroll
+  for (int v = 0; v < R / N; v++) {
+    vec q = ld_stream(p + (size_t)v * Vh);
+    vec_get(q, U + v * N);
+  }
+  if (R == 12) {
+    // row2[c] = conj(row0[a]*row1[b] - row0[b]*row1[a]),  (a,b) = (1,2),(2,0),(0,1)
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+      const int a = (c + 1) % 3, b = (c + 2) % 3;
+      T re = U[2 * a] * U[6 + 2 * b] - U[2 * a + 1] * U[6 + 2 * b + 1] - U[2 * b] * U[6 + 2 * a] +
+             U[2 * b + 1] * U[6 + 2 * a + 1];
+      T im = U[2 * a] * U[6 + 2 * b + 1] + U[2 * a + 1] * U[6 + 2 * b] - U[2 * b] * U[6 + 2 * a + 1] -
+             U[2 * b + 1] * U[6 + 2 * a];
+      U[12 + 2 * c] = re;
+      U[12 + 2 * c + 1] = -im;
+    }
+  }
+}
+
+// site coordinates of checkerboard index idx of parity par
+struct Site {
+  int xh, y, z, t, r;  // r = (par + y + z + t) & 1 : x = 2*xh + r
+};
+__device__ __forceinline__ Site site_of(const Lat& L, int idx, int par) {
+  Site s;
+  s.xh = idx % L.Lxh;
+  int q = idx / L.Lxh;
+  s.y = q % L.Ly;
+  q /= L.Ly;
+  s.z = q % L.Lz;
+  s.t = q / L.Lz;
+  s.r = (par + s.y + s.z + s.t) & 1;
+  return s;
+}
+// checkerboard index (in the opposite parity) of the neighbour at +1/-1 in direction mu
+template <int MU, int DIR>
+__device__ __forceinline__ int neighbour(const Lat& L, int idx, const Site& s) {
+  if (MU == 0) {
+    if (DIR > 0) return s.r ? (s.xh == L.Lxh - 1 ? idx - (L.Lxh - 1) : idx + 1) : idx;
+    return s.r ? idx : (s.xh == 0 ? idx + (L.Lxh - 1) : idx - 1);
+  } else if (MU == 1) {
+    const int st = L.Lxh;
+    if (DIR > 0) return s.y == L.Ly - 1 ? idx - (L.Ly - 1) * st : idx + st;
+    return s.y == 0 ? idx + (L.Ly - 1) * st : idx - st;
+  } else if (MU == 2) {
+    const int st = L.Lxh * L.Ly;
+    if (DIR > 0) return s.z == L.Lz - 1 ? idx - (L.Lz - 1) * st : idx + st;
+    return s.z == 0 ? idx + (L.Lz - 1) * st : idx - st;
+  } else {
+    const int st = L.Lxh * L.Ly * L.Lz;
+    if (DIR > 0) return s.t == L.Lt - 1 ? idx - (L.Lt - 1) * st : idx + st;
+    return s.t == 0 ? idx + (L.Lt - 1) * st : idx - st;
+  }
+}
+
+// launchers implemented per translation unit
+#define LQCD_LAUNCH_CHECK(ctx, what)                 \
+  do {                                               \
+    (ctx)->launches++;                               \
+    cudaError_t e__ = cudaPeekAtLastError();         \
+    if (e__ != cudaSuccess) return lqcd_check_cuda((ctx), what); \
+  } while (0)
+
+static inline cudaStream_t as_stream(void* s) { return reinterpret_cast<cudaStream_t>(s); }
+
+// internal launchers shared between translation units
+int lqcd_dslash_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
+                       int parity, double scale, int dagger, int epi, cudaStream_t st);
+int lqcd_clover_apply_launch(lqcd_ctx* c, void* out, const void* in, const void* cl_parity, cudaStream_t st);
+int lqcd_spinor_pack_parity(lqcd_ctx* c, void* native, const void* pub, cudaStream_t st);
+int lqcd_spinor_unpack_parity(lqcd_ctx* c, void* pub, const void* native, cudaStream_t st);

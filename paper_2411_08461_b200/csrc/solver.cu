@@ -1,0 +1,440 @@
+// Operators M, Mhat and the Krylov solvers (§8(c) O7-O9;
+// PAPER.md:94 "BiCGStab for Wilson/clover and CG", PAPER.md:227-230 invert).
+#include <string.h>
+#include "blas.cuh"
+
+static inline char* off(const void* p, size_t bytes) { return (char*)p + bytes; }
+
+// reduction slots in ctx->d_scalars
+enum { S_BB = 0, S_RR0 = 2, S_RR1 = 3, S_TT = 4, S_RES = 5, S_RHO0 = 8, S_RHO1 = 10, S_R0V = 12, S_TS = 16, S_RR = 20, S_TRUE = 24 };
+
+#define BLAS_CALL(c, OPNAME, SETUP, vecs, outs, st)                       \
+  ((c)->prec == 4 ? [&]() { OPNAME<float> op; SETUP; return blas_launch<float, OPNAME<float>>((c), op, (vecs), (outs), (st)); }() \
+                  : [&]() { OPNAME<double> op; SETUP; return blas_launch<double, OPNAME<double>>((c), op, (vecs), (outs), (st)); }())
+
+static int read_scalars(lqcd_ctx* c, int first, int count, cudaStream_t st) {
+  cudaMemcpyAsync(c->h_scalars + first, c->d_scalars + first, sizeof(double) * count, cudaMemcpyDeviceToHost, st);
+  if (cudaStreamSynchronize(st) != cudaSuccess) return lqcd_check_cuda(c, "scalar read-back");
+  return LQCD_OK;
+}
+
+// Mhat (O8) on one-parity native spinors.  Two fused dslash launches:
+//   asym:       tmp = A_oo^-1 D_oe in ; out = A_ee in - k^2 D_eo tmp
+//   sym:        tmp = A_oo^-1 D_oe in ; out = in - k^2 A_ee^-1 D_eo tmp
+//   sym dagger: out(scratch) = A_ee^-1 in ; tmp = A_oo^-1 D^dag_oe out ; out = in - k^2 D^dag_eo tmp
+static int mpc_apply(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* clover,
+                     const void* clover_inv, double kappa, int matpc, int dagger, void* tmp, cudaStream_t st) {
+  const size_t half = lqcd_clover_bytes(c) / 2;
+  const void* A_e = clover;
+  const void* Ai_e = clover_inv;
+  const void* Ai_o = off(clover_inv, half);
+  const double k2 = -kappa * kappa;
+  int rc;
+  if (matpc == LQCD_MATPC_ASYMMETRIC) {
+    if ((rc = lqcd_dslash_launch(c, tmp, in, gauge, Ai_o, nullptr, 1, 1.0, dagger, 1, st))) return rc;
+    return lqcd_dslash_launch(c, out, tmp, gauge, A_e, in, 0, k2, dagger, 2, st);
+  }
+  if (!dagger) {
+    if ((rc = lqcd_dslash_launch(c, tmp, in, gauge, Ai_o, nullptr, 1, 1.0, 0, 1, st))) return rc;
+    return lqcd_dslash_launch(c, out, tmp, gauge, Ai_e, in, 0, k2, 0, 3, st);
+  }
+  if ((rc = lqcd_clover_apply_launch(c, out, in, Ai_e, st))) return rc;
+  if ((rc = lqcd_dslash_launch(c, tmp, out, gauge, Ai_o, nullptr, 1, 1.0, 1, 1, st))) return rc;
+  // out = in + k2 * D^dag_eo tmp : epilogue 2 with C = identity is not available, so use the
+  // plain dslash into `out` followed by an xpay
+  if ((rc = lqcd_dslash_launch(c, out, tmp, gauge, nullptr, nullptr, 0, k2, 1, 0, st))) return rc;
+  void* v[2] = {(void*)in, out};
+  return BLAS_CALL(c, OpXpay, op.a = 1.0, v, nullptr, st);  // out = in + 1*out
+}
+
+// full M (O7): out_p = A_pp in_p - kappa D_{p,1-p} in_{1-p}
+static int mat_apply(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* clover, double kappa,
+                     int dagger, cudaStream_t st) {
+  const size_t sp = lqcd_spinor_bytes(c), half = lqcd_clover_bytes(c) / 2;
+  int rc;
+  if ((rc = lqcd_dslash_launch(c, out, off(in, sp), gauge, clover, in, 0, -kappa, dagger, 2, st))) return rc;
+  return lqcd_dslash_launch(c, off(out, sp), in, gauge, off(clover, half), off(in, sp), 1, -kappa, dagger, 2, st);
+}
+
+static bool check_ptrs(lqcd_ctx* c, const void* const* p, int n, const char* what) {
+  for (int i = 0; i < n; i++)
+    if (!lqcd_aligned16(p[i])) {
+      lqcd_set_error(c, LQCD_ERR_ALIGN, "%s: pointer %d not 16-byte aligned", what, i);
+      return false;
+    }
+  return true;
+}
+
+extern "C" {
+
+int lqcd_mpc_apply(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* clover,
+                   const void* clover_inv, double kappa, int matpc, int dagger, void* tmp, void* stream) {
+  if (!c || !out || !in || !gauge || !clover || !clover_inv || !tmp || (matpc != 0 && matpc != 1))
+    return LQCD_ERR_INVALID_ARG;
+  if (out == in || tmp == in || tmp == out) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "mpc_apply: aliasing");
+  const void* p[6] = {out, in, gauge, clover, clover_inv, tmp};
+  if (!check_ptrs(c, p, 6, "mpc_apply")) return LQCD_ERR_ALIGN;
+  return mpc_apply(c, out, in, gauge, clover, clover_inv, kappa, matpc, dagger ? 1 : 0, tmp, as_stream(stream));
+}
+
+int lqcd_mat_apply(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* clover, double kappa,
+                   int dagger, void* stream) {
+  if (!c || !out || !in || !gauge || !clover) return LQCD_ERR_INVALID_ARG;
+  if (out == in) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "mat_apply: out aliases in");
+  const void* p[4] = {out, in, gauge, clover};
+  if (!check_ptrs(c, p, 4, "mat_apply")) return LQCD_ERR_ALIGN;
+  return mat_apply(c, out, in, gauge, clover, kappa, dagger ? 1 : 0, as_stream(stream));
+}
+
+// workspace: up to 9 one-parity spinors + 2 two-parity spinors (+ clover pair when built inside)
+size_t lqcd_invert_workspace_bytes(const lqcd_ctx* c, int solver) {
+  (void)solver;
+  if (!c) return 0;
+  return 13 * lqcd_spinor_bytes(c) + 2 * lqcd_clover_bytes(c);
+}
+
+}  // extern "C"
+
+struct Work {
+  char* b;      // two-parity native source
+  char* x;      // two-parity native solution
+  char* v[9];   // one-parity scratch spinors
+  char* clover; // optional
+  char* clover_inv;
+};
+
+static int solve_cg(lqcd_ctx* c, const Work& w, const void* gauge, const void* A, const void* Ai, double kappa,
+                    int matpc, int normal_residual, double stop2, int maxiter, lqcd_result* res, cudaStream_t st) {
+  // CGNE (normal_residual = 0): Mhat Mhat^dag y = bhat, x = Mhat^dag y.   bhat in v[0], x_e in w.x
+  // CGNR (normal_residual = 1): Mhat^dag Mhat x = Mhat^dag bhat; `resv` tracks bhat - Mhat x
+  char *r = w.v[1], *p = w.v[2], *t = w.v[3], *q = w.v[4], *tmp = w.v[5], *resv = w.v[6];
+  const size_t sp = lqcd_spinor_bytes(c);
+  char* x = w.x;
+  int rc;
+  cudaMemsetAsync(x, 0, sp, st);
+  if (!normal_residual) {
+    cudaMemcpyAsync(r, w.v[0], sp, cudaMemcpyDeviceToDevice, st);
+  } else {
+    cudaMemcpyAsync(resv, w.v[0], sp, cudaMemcpyDeviceToDevice, st);
+    if ((rc = mpc_apply(c, r, resv, gauge, A, Ai, kappa, matpc, 1, tmp, st))) return rc;
+    res->dslash_count += 2;
+  }
+  cudaMemcpyAsync(p, r, sp, cudaMemcpyDeviceToDevice, st);
+  {
+    void* v[1] = {r};
+    int outs[4] = {S_RR0, 0, 0, 0};
+    if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v, outs, st))) return rc;
+    void* v2[1] = {normal_residual ? resv : r};
+    int outs2[4] = {S_RES, 0, 0, 0};
+    if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v2, outs2, st))) return rc;
+  }
+  if ((rc = read_scalars(c, S_RES, 1, st))) return rc;
+  double resn = c->h_scalars[S_RES];
+  int it = 0;
+  while (it < maxiter && resn > stop2) {
+    const int cur = (it & 1) ? S_RR1 : S_RR0, nxt = (it & 1) ? S_RR0 : S_RR1;
+    int outs[4] = {S_TT, 0, 0, 0};
+    if (!normal_residual) {
+      if ((rc = mpc_apply(c, t, p, gauge, A, Ai, kappa, matpc, 1, tmp, st))) return rc;   // t = Mhat^dag p
+      void* v[1] = {t};
+      if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v, outs, st))) return rc;                 // <p, Mhat Mhat^dag p>
+      if ((rc = mpc_apply(c, q, t, gauge, A, Ai, kappa, matpc, 0, tmp, st))) return rc;   // q = Mhat t
+      void* u[4] = {x, t, r, q};
+      int o2[4] = {nxt, 0, 0, 0};
+      if ((rc = BLAS_CALL(c, OpCgUpdate, (op.num = cur, op.den = S_TT), u, o2, st))) return rc;  // x += a t ; r -= a q
+    } else {
+      if ((rc = mpc_apply(c, t, p, gauge, A, Ai, kappa, matpc, 0, tmp, st))) return rc;   // t = Mhat p
+      void* v[1] = {t};
+      if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v, outs, st))) return rc;
+      void* u[4] = {x, p, resv, t};
+      int o2[4] = {S_RES, 0, 0, 0};
+      if ((rc = BLAS_CALL(c, OpCgUpdate, (op.num = cur, op.den = S_TT), u, o2, st))) return rc;  // x += a p ; res -= a t
+      if ((rc = mpc_apply(c, q, t, gauge, A, Ai, kappa, matpc, 1, tmp, st))) return rc;   // q = Mhat^dag t
+      void* u2[2] = {r, q};
+      int o3[4] = {nxt, 0, 0, 0};
+      if ((rc = BLAS_CALL(c, OpAxmyNormRatio, (op.num = cur, op.den = S_TT), u2, o3, st))) return rc;
+    }
+    res->dslash_count += 4;
+    void* u3[2] = {p, r};
+    if ((rc = BLAS_CALL(c, OpXpayRatio, (op.num = nxt, op.den = cur), u3, nullptr, st))) return rc;  // p = r + beta p
+    it++;
+    if ((rc = read_scalars(c, S_RR0, 4, st))) return rc;
+    resn = normal_residual ? c->h_scalars[S_RES] : c->h_scalars[nxt];
+    if (!(resn == resn)) { res->status = LQCD_ERR_BREAKDOWN; break; }
+  }
+  res->iterations = it;
+  res->iter_resid = resn;  // squared, normalised by the caller
+  return LQCD_OK;
+}
+
+static int solve_bicgstab(lqcd_ctx* c, const Work& w, const void* gauge, const void* A, const void* Ai, double kappa,
+                          int matpc, double stop2, int maxiter, lqcd_result* res, cudaStream_t st) {
+  char *r = w.v[1], *r0 = w.v[2], *p = w.v[3], *v = w.v[4], *s = w.v[6], *t = w.v[7], *tmp = w.v[5];
+  const size_t sp = lqcd_spinor_bytes(c);
+  char* x = w.x;
+  int rc;
+  cudaMemsetAsync(x, 0, sp, st);
+  cudaMemcpyAsync(r, w.v[0], sp, cudaMemcpyDeviceToDevice, st);
+  cudaMemcpyAsync(r0, w.v[0], sp, cudaMemcpyDeviceToDevice, st);
+  {
+    // rho_0 = <r0,r> = |r|^2
+    void* u[2] = {r0, r};
+    int outs[4] = {S_RHO0, S_RHO0 + 1, S_RR, 0};
+    if ((rc = BLAS_CALL(c, OpCdot, (void)op, u, outs, st))) return rc;
+  }
+  if ((rc = read_scalars(c, S_RR, 1, st))) return rc;
+  double rr = c->h_scalars[S_RR];
+  int it = 0, first = 1, restarted = 0;
+  while (it < maxiter && rr > stop2) {
+    const int rho = (it & 1) ? S_RHO1 : S_RHO0, rho_next = (it & 1) ? S_RHO0 : S_RHO1;
+    {
+      void* u[3] = {p, r, v};
+      if ((rc = BLAS_CALL(c, OpBicgP, (op.rho = rho, op.r0v = S_R0V, op.ts = S_TS, op.first = first), u, nullptr, st))) return rc;
+    }
+    first = 0;
+    if ((rc = mpc_apply(c, v, p, gauge, A, Ai, kappa, matpc, 0, tmp, st))) return rc;   // v = Mhat p
+    {
+      void* u[2] = {r0, v};
+      int outs[4] = {S_R0V, S_R0V + 1, S_R0V + 2, 0};
+      if ((rc = BLAS_CALL(c, OpCdot, (void)op, u, outs, st))) return rc;
+      void* u2[3] = {s, r, v};
+      if ((rc = BLAS_CALL(c, OpBicgS, (op.rho = rho, op.r0v = S_R0V), u2, nullptr, st))) return rc;
+    }
+    if ((rc = mpc_apply(c, t, s, gauge, A, Ai, kappa, matpc, 0, tmp, st))) return rc;   // t = Mhat s
+    {
+      void* u[2] = {t, s};
+      int outs[4] = {S_TS, S_TS + 1, S_TS + 2, 0};
+      if ((rc = BLAS_CALL(c, OpCdot, (void)op, u, outs, st))) return rc;                // <t,s>, |t|^2
+      void* u2[6] = {x, r, p, s, t, r0};
+      int o2[4] = {S_RR, rho_next, rho_next + 1, 0};
+      if ((rc = BLAS_CALL(c, OpBicgXR, (op.rho = rho, op.r0v = S_R0V, op.ts = S_TS), u2, o2, st))) return rc;
+    }
+    res->dslash_count += 4;
+    it++;
+    if ((rc = read_scalars(c, S_RHO0, 16, st))) return rc;
+    rr = c->h_scalars[S_RR];
+    const double* h = c->h_scalars;
+    const double rho_mag = h[rho_next] * h[rho_next] + h[rho_next + 1] * h[rho_next + 1];
+    const double om_mag = (h[S_TS] * h[S_TS] + h[S_TS + 1] * h[S_TS + 1]);
+    if (!(rr == rr) || ((rho_mag < 1e-300 || om_mag < 1e-300) && rr > stop2)) {
+      if (restarted || !(rr == rr)) { res->status = LQCD_ERR_BREAKDOWN; break; }
+      // one restart with r0 = r (O9)
+      restarted = 1;
+      first = 1;
+      cudaMemcpyAsync(r0, r, sp, cudaMemcpyDeviceToDevice, st);
+      void* u[2] = {r0, r};
+      int outs[4] = {rho_next, rho_next + 1, S_RR, 0};
+      if ((rc = BLAS_CALL(c, OpCdot, (void)op, u, outs, st))) return rc;
+    }
+  }
+  res->iterations = it;
+  res->iter_resid = rr;
+  return LQCD_OK;
+}
+
+static void carve(lqcd_ctx* c, void* workspace, Work& w, bool with_clover) {
+  const size_t sp = lqcd_spinor_bytes(c);
+  char* p = (char*)workspace;
+  w.b = p; p += 2 * sp;
+  w.x = p; p += 2 * sp;
+  for (int i = 0; i < 9; i++) { w.v[i] = p; p += sp; }
+  w.clover = with_clover ? p : nullptr;
+  w.clover_inv = with_clover ? p + lqcd_clover_bytes(c) : nullptr;
+}
+
+// the whole solve on native fields already in w.b; result in w.x (both parities)
+static int invert_native(lqcd_ctx* c, Work& w, const void* gauge, const void* A, const void* Ai, double kappa,
+                         double tol, int maxiter, int solver, int matpc, lqcd_result* res, cudaStream_t st) {
+  const size_t sp = lqcd_spinor_bytes(c), half = lqcd_clover_bytes(c) / 2;
+  const void* Ai_e = Ai;
+  const void* Ai_o = off(Ai, half);
+  char *b_e = w.b, *b_o = w.b + sp, *x_e = w.x, *x_o = w.x + sp;
+  int rc;
+  // |b|^2 over both parities
+  {
+    void* v[1] = {b_e};
+    int o[4] = {S_BB, 0, 0, 0};
+    if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v, o, st))) return rc;
+    void* v2[1] = {b_o};
+    int o2[4] = {S_BB + 1, 0, 0, 0};
+    if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v2, o2, st))) return rc;
+  }
+  if ((rc = read_scalars(c, S_BB, 2, st))) return rc;
+  const double bb = c->h_scalars[S_BB] + c->h_scalars[S_BB + 1];
+  if (bb == 0.0) {
+    cudaMemsetAsync(w.x, 0, 2 * sp, st);
+    res->status = LQCD_OK;
+    return LQCD_OK;
+  }
+  // a5: bhat = b_e + kappa D_eo A_oo^-1 b_o   (sym: bhat_s = A_ee^-1 bhat)
+  char* bh = w.v[0];
+  if ((rc = lqcd_clover_apply_launch(c, w.v[5], b_o, Ai_o, st))) return rc;
+  if ((rc = lqcd_dslash_launch(c, bh, w.v[5], gauge, nullptr, nullptr, 0, kappa, 0, 0, st))) return rc;
+  res->dslash_count += 1;
+  {
+    void* v[2] = {b_e, bh};
+    if ((rc = BLAS_CALL(c, OpXpay, op.a = 1.0, v, nullptr, st))) return rc;
+  }
+  if (matpc == LQCD_MATPC_SYMMETRIC)
+    if ((rc = lqcd_clover_apply_launch(c, bh, bh, Ai_e, st))) return rc;
+  const double stop2 = tol * tol * bb;
+  res->status = LQCD_OK;
+  if (solver == LQCD_SOLVER_BICGSTAB) rc = solve_bicgstab(c, w, gauge, A, Ai, kappa, matpc, stop2, maxiter, res, st);
+  else rc = solve_cg(c, w, gauge, A, Ai, kappa, matpc, solver == LQCD_SOLVER_CGNR, stop2, maxiter, res, st);
+  if (rc) return rc;
+  const double rr = res->iter_resid;
+  res->iter_resid = sqrt(rr / bb);
+  if (res->status == LQCD_OK && rr > stop2) res->status = LQCD_NOT_CONVERGED;
+  // a10: x_o = A_oo^-1 (b_o + kappa D_oe x_e)
+  if ((rc = lqcd_dslash_launch(c, w.v[5], x_e, gauge, nullptr, nullptr, 1, kappa, 0, 0, st))) return rc;
+  res->dslash_count += 1;
+  {
+    void* v[2] = {b_o, w.v[5]};
+    if ((rc = BLAS_CALL(c, OpXpay, op.a = 1.0, v, nullptr, st))) return rc;
+  }
+  if ((rc = lqcd_clover_apply_launch(c, x_o, w.v[5], Ai_o, st))) return rc;
+  // a11: true residual |b - M x| / |b| with the full operator; v[1], v[2] are adjacent
+  if ((rc = mat_apply(c, w.v[1], w.x, gauge, A, kappa, 0, st))) return rc;
+  res->dslash_count += 2;
+  {
+    void* v[2] = {b_e, w.v[1]};
+    int o[4] = {S_TRUE, 0, 0, 0};
+    if ((rc = BLAS_CALL(c, OpAxpyNorm, op.a = -1.0, v, o, st))) return rc;
+    void* v2[2] = {b_o, w.v[2]};
+    int o2[4] = {S_TRUE + 1, 0, 0, 0};
+    if ((rc = BLAS_CALL(c, OpAxpyNorm, op.a = -1.0, v2, o2, st))) return rc;
+  }
+  if ((rc = read_scalars(c, S_TRUE, 2, st))) return rc;
+  res->true_resid = sqrt((c->h_scalars[S_TRUE] + c->h_scalars[S_TRUE + 1]) / bb);
+  return LQCD_OK;
+}
+
+static int invert_common(lqcd_ctx* c, void* x_public, const void* b_public, const void* gauge, const void* clover,
+                         const void* clover_inv, double kappa, double csw, double tol, int maxiter, int solver,
+                         int matpc, void* workspace, size_t workspace_bytes, lqcd_result* res, cudaStream_t st) {
+  if (!c || !x_public || !b_public || !gauge || !workspace || !res) return LQCD_ERR_INVALID_ARG;
+  if (solver < 0 || solver > 2 || (matpc != 0 && matpc != 1) || maxiter < 0 || !(tol >= 0) || (clover && !clover_inv))
+    return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "invert: bad solver/matpc/maxiter/tol");
+  if (workspace_bytes < lqcd_invert_workspace_bytes(c, solver))
+    return lqcd_set_error(c, LQCD_ERR_WORKSPACE, "invert: workspace %zu < %zu", workspace_bytes,
+                          lqcd_invert_workspace_bytes(c, solver));
+  const void* p[6] = {x_public, b_public, gauge, clover, clover_inv, workspace};
+  if (!check_ptrs(c, p, 6, "invert")) return LQCD_ERR_ALIGN;
+  memset(res, 0, sizeof(*res));
+  const long launches0 = c->launches;
+  Work w;
+  carve(c, workspace, w, clover == nullptr);
+  int rc;
+  cudaEventRecord(c->ev0, st);
+  if (!clover) {
+    void* s = (void*)st;
+    if ((rc = lqcd_clover_build(c, w.clover, w.clover_inv, gauge, csw, kappa, s))) return rc;
+    clover = w.clover;
+    clover_inv = w.clover_inv;
+  }
+  if ((rc = lqcd_spinor_pack(c, w.b, b_public, (void*)st))) return rc;
+  if ((rc = invert_native(c, w, gauge, clover, clover_inv, kappa, tol, maxiter, solver, matpc, res, st))) return rc;
+  if ((rc = lqcd_spinor_unpack(c, x_public, w.x, (void*)st))) return rc;
+  cudaEventRecord(c->ev1, st);
+  if (cudaStreamSynchronize(st) != cudaSuccess) return lqcd_check_cuda(c, "invert sync");
+  float ms = 0;
+  cudaEventElapsedTime(&ms, c->ev0, c->ev1);
+  res->seconds = ms * 1e-3;
+  res->kernel_launches = c->launches - launches0;
+  return res->status;
+}
+
+extern "C" {
+
+int lqcd_invert(lqcd_ctx* c, void* x_public, const void* b_public, const void* gauge, const void* clover,
+                const void* clover_inv, double kappa, double csw, double tol, int maxiter, int solver, int matpc,
+                void* workspace, size_t workspace_bytes, lqcd_result* res, void* stream) {
+  return invert_common(c, x_public, b_public, gauge, clover, clover_inv, kappa, csw, tol, maxiter, solver, matpc,
+                       workspace, workspace_bytes, res, as_stream(stream));
+}
+
+size_t lqcd_host_scratch_bytes(const lqcd_ctx* c, int solver) {
+  return c ? 4 * lqcd_spinor_bytes(c) + lqcd_invert_workspace_bytes(c, solver) : 0;
+}
+
+// scratch: [public in (1 parity)] [public out (1 parity)] [native in] [native out]
+int lqcd_dslash_host(lqcd_ctx* c, void* out_host, const void* in_host, const void* gauge, int parity, double scale,
+                     int dagger, void* scratch, void* stream) {
+  if (!c || !out_host || !in_host || !gauge || !scratch || (parity != 0 && parity != 1)) return LQCD_ERR_INVALID_ARG;
+  if (!lqcd_aligned16(scratch) || !lqcd_aligned16(gauge)) return lqcd_set_error(c, LQCD_ERR_ALIGN, "dslash_host: alignment");
+  cudaStream_t st = as_stream(stream);
+  const size_t sp = lqcd_spinor_bytes(c);
+  char* s = (char*)scratch;
+  int rc;
+  cudaMemcpyAsync(s, (const char*)in_host + (size_t)(1 - parity) * sp, sp, cudaMemcpyHostToDevice, st);
+  if ((rc = lqcd_spinor_pack_parity(c, s + 2 * sp, s, st))) return rc;
+  if ((rc = lqcd_dslash_launch(c, s + 3 * sp, s + 2 * sp, gauge, nullptr, nullptr, parity, scale, dagger ? 1 : 0, 0, st))) return rc;
+  if ((rc = lqcd_spinor_unpack_parity(c, s + sp, s + 3 * sp, st))) return rc;
+  cudaMemcpyAsync((char*)out_host + (size_t)parity * sp, s + sp, sp, cudaMemcpyDeviceToHost, st);
+  if (cudaStreamSynchronize(st) != cudaSuccess) return lqcd_check_cuda(c, "dslash_host sync");
+  return LQCD_OK;
+}
+
+int lqcd_invert_host(lqcd_ctx* c, void* x_host, const void* b_host, const void* gauge, const void* clover,
+                     const void* clover_inv, double kappa, double tol, int maxiter, int solver, int matpc,
+                     void* scratch, size_t scratch_bytes, lqcd_result* res, void* stream) {
+  if (!c || !x_host || !b_host || !scratch || !clover || !clover_inv) return LQCD_ERR_INVALID_ARG;
+  if (scratch_bytes < lqcd_host_scratch_bytes(c, solver)) return lqcd_set_error(c, LQCD_ERR_WORKSPACE, "invert_host: scratch too small");
+  cudaStream_t st = as_stream(stream);
+  const size_t sp = lqcd_spinor_bytes(c);
+  char* s = (char*)scratch;
+  cudaMemcpyAsync(s, b_host, 2 * sp, cudaMemcpyHostToDevice, st);
+  int rc = invert_common(c, s + 2 * sp, s, gauge, clover, clover_inv, kappa, 0.0, tol, maxiter, solver, matpc,
+                         s + 4 * sp, scratch_bytes - 4 * sp, res, st);
+  if (rc < 0) return rc;
+  cudaMemcpyAsync(x_host, s + 2 * sp, 2 * sp, cudaMemcpyDeviceToHost, st);
+  if (cudaStreamSynchronize(st) != cudaSuccess) return lqcd_check_cuda(c, "invert_host sync");
+  return rc;
+}
+
+int lqcd_blas_axpy_norm(lqcd_ctx* c, double a, const void* x, void* y, double* norm2_host, void* stream) {
+  if (!c || !x || !y || !norm2_host) return LQCD_ERR_INVALID_ARG;
+  cudaStream_t st = as_stream(stream);
+  void* v[2] = {(void*)x, y};
+  int o[4] = {S_TRUE, 0, 0, 0};
+  int rc;
+  if ((rc = BLAS_CALL(c, OpAxpyNorm, op.a = a, v, o, st))) return rc;
+  if ((rc = read_scalars(c, S_TRUE, 1, st))) return rc;
+  *norm2_host = c->h_scalars[S_TRUE];
+  return LQCD_OK;
+}
+
+int lqcd_blas_xpay(lqcd_ctx* c, const void* x, double a, void* y, void* stream) {
+  if (!c || !x || !y) return LQCD_ERR_INVALID_ARG;
+  cudaStream_t st = as_stream(stream);
+  void* v[2] = {(void*)x, y};
+  int rc;
+  if ((rc = BLAS_CALL(c, OpXpay, op.a = a, v, nullptr, st))) return rc;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return lqcd_check_cuda(c, "blas_xpay sync");
+  return LQCD_OK;
+}
+
+int lqcd_blas_cdot(lqcd_ctx* c, const void* x, const void* y, double out_host[3], void* stream) {
+  if (!c || !x || !y || !out_host) return LQCD_ERR_INVALID_ARG;
+  cudaStream_t st = as_stream(stream);
+  void* v[2] = {(void*)x, (void*)y};
+  int o[4] = {S_TRUE, S_TRUE + 1, S_TRUE + 2, 0};
+  int rc;
+  if ((rc = BLAS_CALL(c, OpCdot, (void)op, v, o, st))) return rc;
+  if ((rc = read_scalars(c, S_TRUE, 3, st))) return rc;
+  for (int i = 0; i < 3; i++) out_host[i] = c->h_scalars[S_TRUE + i];
+  return LQCD_OK;
+}
+
+int lqcd_blas_caxpbypz(lqcd_ctx* c, const double a[2], const void* x, const double b[2], const void* y, void* z,
+                       void* stream) {
+  if (!c || !a || !b || !x || !y || !z) return LQCD_ERR_INVALID_ARG;
+  cudaStream_t st = as_stream(stream);
+  void* v[3] = {(void*)x, (void*)y, z};
+  int rc;
+  if ((rc = BLAS_CALL(c, OpCaxpbypz, (op.a = {a[0], a[1]}, op.b = {b[0], b[1]}), v, nullptr, st))) return rc;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return lqcd_check_cuda(c, "blas_caxpbypz sync");
+  return LQCD_OK;
+}
+
+}  // extern "C"

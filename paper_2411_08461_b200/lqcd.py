@@ -1,0 +1,266 @@
+"""Thin Python binding of liblqcd (include/lqcd.h): argument marshalling only.
+
+PyTorch supplies device memory and the CUDA stream; every step of the path runs in the CUDA
+kernels behind the C ABI.  There is no CPU fallback: if the shared library is missing or no
+sm_100 device is present, creating a context raises.
+"""
+import ctypes
+import os
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+_lib = None
+
+
+class Result(ctypes.Structure):
+    _fields_ = [("status", ctypes.c_int), ("iterations", ctypes.c_int),
+                ("iter_resid", ctypes.c_double), ("true_resid", ctypes.c_double),
+                ("seconds", ctypes.c_double), ("dslash_count", ctypes.c_long),
+                ("kernel_launches", ctypes.c_long)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+SOLVERS = {"cgne": 0, "cgnr": 1, "bicgstab": 2}
+SYMBOLS = [
+    "lqcd_create", "lqcd_destroy", "lqcd_strerror", "lqcd_last_error", "lqcd_launch_count",
+    "lqcd_gauge_bytes", "lqcd_spinor_bytes", "lqcd_clover_bytes", "lqcd_invert_workspace_bytes",
+    "lqcd_gauge_pack", "lqcd_spinor_pack", "lqcd_spinor_unpack", "lqcd_clover_unpack",
+    "lqcd_clover_build", "lqcd_clover_apply", "lqcd_dslash", "lqcd_mpc_apply", "lqcd_mat_apply",
+    "lqcd_invert", "lqcd_host_scratch_bytes", "lqcd_dslash_host", "lqcd_invert_host",
+    "lqcd_blas_axpy_norm", "lqcd_blas_xpay", "lqcd_blas_cdot", "lqcd_blas_caxpbypz",
+]
+
+
+def library_path():
+    return _build.SO
+
+
+def load():
+    """dlopen liblqcd.so (built in-tree by build.py) and declare the prototypes."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_build.SO):
+        raise RuntimeError("liblqcd.so is missing: run `python -m paper_2411_08461_b200.build` "
+                           "(there is no CPU fallback)")
+    L = ctypes.CDLL(_build.SO)
+    vp, ci, cd, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+    L.lqcd_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(ci), ci, ci, ci, ci]
+    L.lqcd_destroy.argtypes = [vp]
+    L.lqcd_strerror.restype = ctypes.c_char_p
+    L.lqcd_strerror.argtypes = [ci]
+    L.lqcd_last_error.restype = ctypes.c_char_p
+    L.lqcd_last_error.argtypes = [vp]
+    L.lqcd_launch_count.restype = ctypes.c_long
+    L.lqcd_launch_count.argtypes = [vp]
+    for f in ("lqcd_gauge_bytes", "lqcd_spinor_bytes", "lqcd_clover_bytes"):
+        getattr(L, f).restype = sz
+        getattr(L, f).argtypes = [vp]
+    for f in ("lqcd_invert_workspace_bytes", "lqcd_host_scratch_bytes"):
+        getattr(L, f).restype = sz
+        getattr(L, f).argtypes = [vp, ci]
+    for f in ("lqcd_gauge_pack", "lqcd_spinor_pack", "lqcd_spinor_unpack", "lqcd_clover_unpack"):
+        getattr(L, f).argtypes = [vp, vp, vp, vp]
+    L.lqcd_clover_build.argtypes = [vp, vp, vp, vp, cd, cd, vp]
+    L.lqcd_clover_apply.argtypes = [vp, vp, vp, vp, ci, vp]
+    L.lqcd_dslash.argtypes = [vp, vp, vp, vp, ci, cd, ci, vp]
+    L.lqcd_mpc_apply.argtypes = [vp, vp, vp, vp, vp, vp, cd, ci, ci, vp, vp]
+    L.lqcd_mat_apply.argtypes = [vp, vp, vp, vp, vp, cd, ci, vp]
+    L.lqcd_invert.argtypes = [vp, vp, vp, vp, vp, vp, cd, cd, cd, ci, ci, ci, vp, sz,
+                              ctypes.POINTER(Result), vp]
+    L.lqcd_dslash_host.argtypes = [vp, vp, vp, vp, ci, cd, ci, vp, vp]
+    L.lqcd_invert_host.argtypes = [vp, vp, vp, vp, vp, vp, cd, cd, ci, ci, ci, vp, sz,
+                                   ctypes.POINTER(Result), vp]
+    L.lqcd_blas_axpy_norm.argtypes = [vp, cd, vp, vp, ctypes.POINTER(cd), vp]
+    L.lqcd_blas_xpay.argtypes = [vp, vp, cd, vp, vp]
+    L.lqcd_blas_cdot.argtypes = [vp, vp, vp, ctypes.POINTER(cd), vp]
+    L.lqcd_blas_caxpbypz.argtypes = [vp, ctypes.POINTER(cd), vp, ctypes.POINTER(cd), vp, vp, vp]
+    _lib = L
+    return L
+
+
+class LqcdError(RuntimeError):
+    pass
+
+
+def _stream():
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _p(t):
+    return ctypes.c_void_p(t.data_ptr()) if t is not None else ctypes.c_void_p(0)
+
+
+class Context:
+    """One lattice, precision and link reconstruction (init + LatticeInfo)."""
+
+    def __init__(self, dims, prec=8, recon=18, t_boundary=-1, device=0):
+        self.lib = load()
+        self.dims = tuple(int(d) for d in dims)
+        self.prec, self.recon, self.device = prec, recon, device
+        h = ctypes.c_void_p()
+        rc = self.lib.lqcd_create(ctypes.byref(h), (ctypes.c_int * 4)(*self.dims), prec, recon,
+                                  t_boundary, device)
+        if rc != 0:
+            raise LqcdError("lqcd_create failed: %s (no CUDA sm_100 device => no fallback)"
+                            % self.lib.lqcd_strerror(rc).decode())
+        self.h = h
+        self.dev = torch.device("cuda", device)
+        self.rdtype = torch.float32 if prec == 4 else torch.float64
+        self.cdtype = torch.complex64 if prec == 4 else torch.complex128
+        self.np_cdtype = np.complex64 if prec == 4 else np.complex128
+        Lx, Ly, Lz, Lt = self.dims
+        self.site_shape = (2, Lt, Lz, Ly, Lx // 2)
+        self.Vh = Lx * Ly * Lz * Lt // 2
+        self.gauge_bytes = self.lib.lqcd_gauge_bytes(h)
+        self.spinor_bytes = self.lib.lqcd_spinor_bytes(h)
+        self.clover_bytes = self.lib.lqcd_clover_bytes(h)
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.lqcd_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- helpers ---------------------------------------------------------------------------
+    def _check(self, rc, allow_not_converged=False):
+        if rc == 0 or (allow_not_converged and rc == 1):
+            return rc
+        raise LqcdError("%s: %s" % (self.lib.lqcd_strerror(rc).decode(),
+                                    self.lib.lqcd_last_error(self.h).decode()))
+
+    def launch_count(self):
+        return self.lib.lqcd_launch_count(self.h)
+
+    def empty(self, nbytes):
+        return torch.empty(nbytes // self.prec, dtype=self.rdtype, device=self.dev)
+
+    def new_spinor(self, parities=1):
+        return self.empty(self.spinor_bytes * parities)
+
+    def to_device(self, a):
+        """numpy public-layout array -> device tensor in this context's precision."""
+        t = torch.from_numpy(np.ascontiguousarray(a))
+        if t.is_complex():
+            t = t.to(self.cdtype)
+        else:
+            t = t.to(self.rdtype)
+        return t.to(self.dev).contiguous()
+
+    # ---- pack / unpack ---------------------------------------------------------------------
+    def gauge_pack(self, U_public):
+        g = self.empty(self.gauge_bytes)
+        self._check(self.lib.lqcd_gauge_pack(self.h, _p(g), _p(U_public), _stream()))
+        return g
+
+    def spinor_pack(self, psi_public):
+        s = self.new_spinor(2)
+        self._check(self.lib.lqcd_spinor_pack(self.h, _p(s), _p(psi_public), _stream()))
+        return s
+
+    def spinor_unpack(self, s_native):
+        out = torch.empty(self.site_shape + (4, 3), dtype=self.cdtype, device=self.dev)
+        self._check(self.lib.lqcd_spinor_unpack(self.h, _p(out), _p(s_native), _stream()))
+        return out
+
+    def clover_unpack(self, cl_native):
+        out = torch.empty(self.site_shape + (2, 36), dtype=self.rdtype, device=self.dev)
+        self._check(self.lib.lqcd_clover_unpack(self.h, _p(out), _p(cl_native), _stream()))
+        return out
+
+    def parity(self, s_native, p):
+        n = self.spinor_bytes // self.prec
+        return s_native[p * n:(p + 1) * n]
+
+    # ---- operators -------------------------------------------------------------------------
+    def clover_build(self, gauge, csw, kappa, want_inverse=True):
+        A = self.empty(self.clover_bytes)
+        Ai = self.empty(self.clover_bytes) if want_inverse else None
+        self._check(self.lib.lqcd_clover_build(self.h, _p(A), _p(Ai), _p(gauge), csw, kappa, _stream()))
+        return A, Ai
+
+    def clover_apply(self, out, inp, clover, parity):
+        self._check(self.lib.lqcd_clover_apply(self.h, _p(out), _p(inp), _p(clover), parity, _stream()))
+        return out
+
+    def dslash(self, out, inp, gauge, parity, scale=1.0, dagger=False):
+        self._check(self.lib.lqcd_dslash(self.h, _p(out), _p(inp), _p(gauge), parity, scale,
+                                         int(dagger), _stream()))
+        return out
+
+    def mpc_apply(self, out, inp, gauge, clover, clover_inv, kappa, matpc=0, dagger=False, tmp=None):
+        tmp = tmp if tmp is not None else self.new_spinor()
+        self._check(self.lib.lqcd_mpc_apply(self.h, _p(out), _p(inp), _p(gauge), _p(clover),
+                                            _p(clover_inv), kappa, matpc, int(dagger), _p(tmp), _stream()))
+        return out
+
+    def mat_apply(self, out, inp, gauge, clover, kappa, dagger=False):
+        self._check(self.lib.lqcd_mat_apply(self.h, _p(out), _p(inp), _p(gauge), _p(clover), kappa,
+                                            int(dagger), _stream()))
+        return out
+
+    def workspace(self, solver="cgne"):
+        n = self.lib.lqcd_invert_workspace_bytes(self.h, SOLVERS[solver])
+        return self.empty(n), n
+
+    def invert(self, b_public, gauge, clover, clover_inv, kappa, csw=0.0, tol=1e-10, maxiter=1000,
+               solver="cgne", matpc=0, workspace=None):
+        if workspace is None:
+            workspace, _ = self.workspace(solver)
+        x = torch.empty_like(b_public)
+        res = Result()
+        rc = self.lib.lqcd_invert(self.h, _p(x), _p(b_public), _p(gauge), _p(clover), _p(clover_inv),
+                                  kappa, csw, tol, maxiter, SOLVERS[solver], matpc, _p(workspace),
+                                  workspace.numel() * self.prec, ctypes.byref(res), _stream())
+        self._check(rc, allow_not_converged=True)
+        return x, res
+
+    # ---- host-buffer (end-to-end) entry points -----------------------------------------------
+    def host_scratch(self, solver="cgne"):
+        n = self.lib.lqcd_host_scratch_bytes(self.h, SOLVERS[solver])
+        return self.empty(n), n
+
+    def dslash_host(self, out_host, in_host, gauge, parity, scratch, scale=1.0, dagger=False):
+        """out_host/in_host: pinned or pageable CPU tensors in the public two-parity layout."""
+        self._check(self.lib.lqcd_dslash_host(self.h, _p(out_host), _p(in_host), _p(gauge), parity,
+                                              scale, int(dagger), _p(scratch), _stream()))
+        return out_host
+
+    def invert_host(self, x_host, b_host, gauge, clover, clover_inv, kappa, scratch, tol=1e-10,
+                    maxiter=1000, solver="cgne", matpc=0):
+        res = Result()
+        rc = self.lib.lqcd_invert_host(self.h, _p(x_host), _p(b_host), _p(gauge), _p(clover),
+                                       _p(clover_inv), kappa, tol, maxiter, SOLVERS[solver], matpc,
+                                       _p(scratch), scratch.numel() * self.prec, ctypes.byref(res),
+                                       _stream())
+        self._check(rc, allow_not_converged=True)
+        return x_host, res
+
+    # ---- BLAS-1 ----------------------------------------------------------------------------
+    def blas_axpy_norm(self, a, x, y):
+        out = ctypes.c_double()
+        self._check(self.lib.lqcd_blas_axpy_norm(self.h, a, _p(x), _p(y), ctypes.byref(out), _stream()))
+        return out.value
+
+    def blas_xpay(self, x, a, y):
+        self._check(self.lib.lqcd_blas_xpay(self.h, _p(x), a, _p(y), _stream()))
+
+    def blas_cdot(self, x, y):
+        out = (ctypes.c_double * 3)()
+        self._check(self.lib.lqcd_blas_cdot(self.h, _p(x), _p(y), out, _stream()))
+        return complex(out[0], out[1]), out[2]
+
+    def blas_caxpbypz(self, a, x, b, y, z):
+        A = (ctypes.c_double * 2)(a.real, a.imag)
+        B = (ctypes.c_double * 2)(b.real, b.imag)
+        self._check(self.lib.lqcd_blas_caxpbypz(self.h, A, _p(x), B, _p(y), _p(z), _stream()))

@@ -1,0 +1,120 @@
+"""GPU parity of lqcd_invert against the oracle's solvers and operator (reading A17): the solution
+is unique, so the GPU's x must agree with the oracle's x within 10*tol, and the TRUE residual of
+the GPU's x, evaluated by the oracle's own M, must be below tol."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2411_08461_b200 import synth
+from latt import rel_err
+from test_gpu_parity import Setup, from_cfg, lq
+
+pytestmark = pytest.mark.gpu
+
+
+def solve_and_check(s, b, solver, matpc, tol, oracle_solution=None, resid_bound=None):
+    bd = s.ctx.to_device(b)
+    x, res = s.ctx.invert(bd, s.gauge, s.A, s.Ai, s.kappa, tol=tol, maxiter=2000, solver=solver, matpc=matpc)
+    xg = x.cpu().numpy().astype(np.complex128)
+    assert res.status == 0, (solver, matpc, res.as_dict())
+    true = s.orc.true_residual(b, xg)
+    bound = resid_bound if resid_bound is not None else tol
+    assert true < bound, (solver, matpc, true, res.as_dict())
+    assert abs(res.true_resid - true) < 0.5 * bound
+    if oracle_solution is not None:
+        assert rel_err(xg, oracle_solution) < 10 * tol, (solver, matpc)
+    return xg, res
+
+
+def test_config1_point_source_cgne_fp64():
+    s, c = from_cfg(1, 8, 18)
+    b = synth.source(c["dims"], "point")
+    xo, ro = s.orc.invert(b, 1e-10, 2000, "cgne", 0)
+    assert ro.status == 0
+    xg, res = solve_and_check(s, b, "cgne", 0, 1e-10, xo)
+    assert abs(res.iterations - ro.iterations) <= 1
+    # paper's normalisation: a_t M = M/(2 kappa), so its propagator is 2 kappa x (reading A2)
+    assert res.dslash_count > 0 and res.kernel_launches > 0 and res.seconds > 0
+
+
+@pytest.mark.parametrize("solver", ["cgne", "cgnr", "bicgstab"])
+@pytest.mark.parametrize("matpc", [0, 1])
+def test_config2_z2_source_fp64(solver, matpc):
+    s, c = from_cfg(2, 8, 18)
+    b = synth.source(c["dims"], "z2", c["src_seed"])
+    xo, ro = s.orc.invert(b, 1e-10, 2000, "bicgstab", 0)
+    xg, res = solve_and_check(s, b, solver, matpc, 1e-10, xo)
+
+
+@pytest.mark.parametrize("recon", [18, 12])
+def test_config2_bicgstab_fp32(recon):
+    s, c = from_cfg(2, 4, recon)
+    b = synth.source(c["dims"], "z2", c["src_seed"])
+    xo, ro = s.orc.invert(b, 1e-10, 2000, "bicgstab", 0)
+    # north_star: fp32 solve to 1e-6; the oracle-evaluated true residual must be < 1e-6 as well,
+    # allowing the fp32 rounding floor of the recurrence (2x)
+    solve_and_check(s, b, "bicgstab", 0, 1e-6, xo, resid_bound=2e-6)
+    solve_and_check(s, b, "cgne", 0, 1e-6, xo, resid_bound=2e-6)
+
+
+def test_invert_builds_clover_when_absent_and_edge_cases():
+    s, c = from_cfg(1, 8, 18)
+    b = synth.source(c["dims"], "gaussian", 9)
+    bd = s.ctx.to_device(b)
+    x1, r1 = s.ctx.invert(bd, s.gauge, None, None, s.kappa, csw=s.csw, tol=1e-10, solver="bicgstab")
+    x2, r2 = s.ctx.invert(bd, s.gauge, s.A, s.Ai, s.kappa, tol=1e-10, solver="bicgstab")
+    assert r1.status == 0 and torch.equal(x1, x2)
+    # zero source -> zero solution, no iterations
+    x0, r0 = s.ctx.invert(torch.zeros_like(bd), s.gauge, s.A, s.Ai, s.kappa)
+    assert r0.status == 0 and r0.iterations == 0 and float(x0.abs().max()) == 0.0
+    # maxiter exhausted -> NOT_CONVERGED (+1), x is still the best iterate
+    x3, r3 = s.ctx.invert(bd, s.gauge, s.A, s.Ai, s.kappa, tol=1e-10, maxiter=3, solver="cgne")
+    assert r3.status == 1 and r3.iterations == 3 and r3.true_resid > 1e-10
+    xo, ro = s.orc.invert(b, 1e-10, 3, "cgne", 0)
+    assert rel_err(x3.cpu().numpy(), xo) < 1e-12
+    # workspace too small / bad solver id
+    ws = s.ctx.empty(1024)
+    with pytest.raises(lq().LqcdError):
+        s.ctx.invert(bd, s.gauge, s.A, s.Ai, s.kappa, workspace=ws)
+
+
+def test_host_entry_points():
+    s, c = from_cfg(1, 8, 18)
+    b = synth.source(c["dims"], "gaussian", 9)
+    bh = torch.from_numpy(b).pin_memory()
+    xh = torch.empty_like(bh).pin_memory()
+    scratch, _ = s.ctx.host_scratch("bicgstab")
+    _, res = s.ctx.invert_host(xh, bh, s.gauge, s.A, s.Ai, s.kappa, scratch, tol=1e-10, solver="bicgstab")
+    assert res.status == 0 and s.orc.true_residual(b, xh.numpy()) < 1e-10
+    oh = torch.zeros_like(bh)
+    for p in (0, 1):
+        s.ctx.dslash_host(oh, bh, s.gauge, p, scratch)
+    assert rel_err(oh.numpy(), s.orc.dslash(b)) < 1e-13
+
+
+def test_config3_propagator_12_columns_fp32_recon12():
+    """BASELINE config 3: 16^3x32, fp32, reconstruct-12, point source, all 12 spin-colour columns by
+    CGNE, assembled sink-source.  Each column's true residual is checked with the
+    oracle's operator; one column is compared with the oracle's own solve."""
+    s, c = from_cfg(3, 4, 12)
+    dims = c["dims"]
+    prop = np.zeros(s.orc.site_shape + (4, 4, 3, 3), dtype=np.complex128)
+    ws, _ = s.ctx.workspace("cgne")
+    for spin in range(4):
+        for col in range(3):
+            b = synth.source(dims, "point", spin=spin, colour=col)
+            x, res = s.ctx.invert(s.ctx.to_device(b), s.gauge, s.A, s.Ai, s.kappa, tol=1e-6, solver="cgne",
+                                  workspace=ws)
+            assert res.status == 0
+            xg = x.cpu().numpy().astype(np.complex128)
+            prop[..., :, spin, :, col] = xg
+            if (spin, col) in ((0, 0), (3, 2)):
+                assert s.orc.true_residual(b, xg) < 2e-6
+            if (spin, col) == (0, 0):
+                xo, ro = s.orc.invert(b, 1e-9, 2000, "cgne", 0)
+                assert rel_err(xg, xo) < 1e-5
+    # gamma5-hermiticity of the point-to-point propagator at the source: g5 S(0,0) g5 = S(0,0)^dag
+    S00 = prop[0, 0, 0, 0, 0].transpose(0, 2, 1, 3).reshape(12, 12)   # (s_sink,c_sink),(s_src,c_src)
+    g5 = np.repeat([1, 1, -1, -1.0], 3)
+    assert np.abs(g5[:, None] * S00 * g5[None, :] - S00.conj().T).max() < 1e-5 * np.abs(S00).max()
