@@ -1,0 +1,338 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the driver.
+
+Workload: BASELINE.json configs[3], 32^3x64 (2.1M sites), eps=0.8 warm links, kappa=0.1248,
+csw=1.8, Gaussian source.  One STEP is one pass of the whole hot path
+in fp64 with 18-real links:
+    gauge pack -> clover build + inverse -> source pack -> prepare -> even-odd CGNE to 1e-10
+    (dslash with fused clover epilogues + fused BLAS-1) -> reconstruct -> true residual -> unpack.
+value  = algorithmic HBM bytes of every kernel of the step / step time (GB/s), whole job.
+roofline = the dominant kernel (dslash with fused clover epilogue), timed per launch with CUDA
+events on the launching stream inside the timed region.
+Also reported (extra keys): the standalone dslash sweep (fp32/fp64 x 18/12 reals) that the
+headline target is stated on, and the solve's iterations / seconds / residuals.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+N > 1: one replica per GPU under torchrun ("replicas only": the path has no exchange step).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+WORKLOAD = 4  # BASELINE.json configs[3] (1-based numbering in synth.CONFIGS)
+METRIC = "Wilson-clover dslash GB/s (whole even-odd CGNE solve, algorithmic bytes / time)"
+FLOPS_PER_SITE = 1320.0
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(max(mx)) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def dslash_alg_bytes(recon, prec, Vh):
+    return (8 * recon + 48) * prec * Vh
+
+
+# ------------------------------------------------------------------------------------------------
+# reference arm / cpu_baseline: the oracle as it stands, on the host cores, bounded sample
+# ------------------------------------------------------------------------------------------------
+def oracle_sample(steps, warmup):
+    """Each step = one full-lattice hopping-term application (two parity sweeps) at the workload's
+    size in fp64 by the CPU oracle.  Returns (GB/s with the dslash algorithmic bytes, ms/step)."""
+    import oracle
+    from paper_2411_08461_b200 import synth
+    cfg = synth.CONFIGS[WORKLOAD]
+    dims = cfg["dims"]
+    U = synth.gauge(dims, cfg["eps"], cfg["seed"])
+    psi = synth.source(dims, "gaussian", cfg["src_seed"])
+    orc = oracle.Oracle(dims, U, -1)
+    del U
+    for _ in range(warmup):
+        orc.dslash(psi)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        orc.dslash(psi)
+    dt = (time.perf_counter() - t0) / steps
+    Vh = int(np.prod(dims)) // 2
+    gbs = 2 * dslash_alg_bytes(18, 8, Vh) / dt / 1e9
+    return gbs, dt * 1e3, oracle.threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    gbs, ms, cores = oracle_sample(max(1, args.steps), min(args.warmup, 1))
+    sample = "per step: one full-lattice fp64 hopping-term application (2 parity sweeps) at 32^3x64 by the CPU oracle"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": gbs, "unit": "GB/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "configs[3]: 32^3x64, eps=0.8 links seed 4, Gaussian source seed 104",
+                   "sample": sample},
+        "cpu_baseline": {"value": gbs, "unit": "GB/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": gbs, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------
+# GPU arm
+# ------------------------------------------------------------------------------------------------
+def dslash_sweep(torch, lqcd, U, psi, dims, device, peak):
+    """Standalone dslash (bare hopping term, scale 1) at the workload size for the four
+    (precision, reconstruction) variants.  Inputs (links 0.4-1.2 GB) exceed L2 (126 MB)."""
+    out = {}
+    for prec, recon in ((4, 18), (4, 12), (8, 18), (8, 12)):
+        ctx = lqcd.Context(dims, prec, recon, -1, device)
+        g = ctx.gauge_pack(ctx.to_device(U))
+        nat = ctx.spinor_pack(ctx.to_device(psi))
+        dst = ctx.new_spinor(2)
+        for i in range(10):
+            ctx.dslash(ctx.parity(dst, i & 1), ctx.parity(nat, 1 - (i & 1)), g, i & 1)
+        torch.cuda.synchronize()
+        ts = []
+        for i in range(40):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ctx.dslash(ctx.parity(dst, i & 1), ctx.parity(nat, 1 - (i & 1)), g, i & 1)
+            e1.record()
+            e1.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e-3)
+        t = float(np.median(ts))
+        by = dslash_alg_bytes(recon, prec, ctx.Vh)
+        out["fp%d_recon%d" % (8 * prec, recon)] = {
+            "us": t * 1e6, "GBps": by / t / 1e9, "frac_of_measured_peak": by / t / 1e9 / peak,
+            "frac_of_8TBps": by / t / 8e12, "GFLOPs": FLOPS_PER_SITE * ctx.Vh / t / 1e9,
+            "bytes_per_site": by // ctx.Vh}
+        ctx.close()
+        del g, nat, dst
+    return out
+
+
+def run_gpu(args):
+    import torch
+    from paper_2411_08461_b200 import lqcd, synth
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    peak, peak_src = measured_peaks()
+
+    cfg = synth.CONFIGS[WORKLOAD]
+    dims = cfg["dims"]
+    kappa, csw, tol = cfg["kappa"], cfg["csw"], 1e-10
+    U = synth.gauge(dims, cfg["eps"], cfg["seed"])            # same seeded field on every replica
+    b = synth.source(dims, cfg["source"], cfg["src_seed"] + rank)
+    ctx = lqcd.Context(dims, 8, 18, -1, local)
+    U_dev, b_dev = ctx.to_device(U), ctx.to_device(b)
+    gauge = ctx.empty(ctx.gauge_bytes)
+    ws, _ = ctx.workspace("cgne")
+    lib, P, S = ctx.lib, lqcd._p, lqcd._stream
+    results = []
+
+    def step():
+        ctx._check(lib.lqcd_gauge_pack(ctx.h, P(gauge), P(U_dev), S()))
+        x, res = ctx.invert(b_dev, gauge, None, None, kappa, csw=csw, tol=tol, maxiter=2000,
+                            solver="cgne", matpc=0, workspace=ws)
+        results.append(res)
+        return x
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    results.clear()
+    sampler = ClockSampler(local)
+    ctx.profile_enable(True)
+    ctx.profile_read()
+    barrier()
+    sampler.start()
+    l0, a0 = ctx.launch_count(), ctx.algorithmic_bytes()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    ctx.profile_enable(False)
+    dt = e0.elapsed_time(e1) * 1e-3
+    launches = ctx.launch_count() - l0
+    alg = ctx.algorithmic_bytes() - a0
+    n_ds, ds_ms, ds_bytes = ctx.profile_read()
+    if dist is not None:
+        t = torch.tensor([dt], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dt = float(t.item())
+        s = torch.tensor([alg, float(launches)], device="cuda", dtype=torch.float64)
+        dist.all_reduce(s, op=dist.ReduceOp.SUM)
+        alg, launches = float(s[0].item()), int(s[1].item())
+    value = alg / dt / 1e9
+    res = results[-1]
+
+    # ---- end to end through the host-buffer entry points (pinned host inputs, result read back)
+    U_h = torch.from_numpy(U).pin_memory()
+    b_h = torch.from_numpy(b).pin_memory()
+    x_h = torch.empty_like(b_h).pin_memory()
+    g_scr = ctx.empty(U_h.numel() * 16)
+    h_scr, _ = ctx.host_scratch("cgne")
+    A, Ai = ctx.empty(ctx.clover_bytes), ctx.empty(ctx.clover_bytes)
+
+    def step_e2e():
+        ctx.gauge_pack_host(gauge, U_h, g_scr)
+        ctx._check(lib.lqcd_clover_build(ctx.h, P(A), P(Ai), P(gauge), csw, kappa, S()))
+        return ctx.invert_host(x_h, b_h, gauge, A, Ai, kappa, h_scr, tol=tol, maxiter=2000, solver="cgne")[1]
+
+    step_e2e()
+    barrier()
+    a0 = ctx.algorithmic_bytes()
+    e0.record()
+    n_e2e = max(1, min(args.steps, 3))
+    for _ in range(n_e2e):
+        r2 = step_e2e()
+    e1.record()
+    barrier()
+    dt2 = e0.elapsed_time(e1) * 1e-3
+    alg2 = ctx.algorithmic_bytes() - a0
+    if dist is not None:
+        t = torch.tensor([dt2], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dt2 = float(t.item())
+        alg2 *= world
+    e2e = {"value": alg2 / dt2 / 1e9, "unit": "GB/s",
+           "h2d_bytes_per_step": int(U_h.numel() * 16 + b_h.numel() * 16),
+           "d2h_bytes_per_step": int(x_h.numel() * 16), "ms_per_step": dt2 / n_e2e * 1e3,
+           "true_resid": r2.true_resid}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "configs[3]: 32^3x64 (2.1M sites), eps=0.8 links seed 4, kappa=0.1248, "
+                               "csw=1.8, Gaussian source seed 104; fp64, 18-real links, antiperiodic t",
+                   "step": "gauge pack + clover build/inverse + even-odd CGNE to 1e-10 + reconstruct + true residual",
+                   "l2": "inputs larger than L2 (links 1.2 GB, clover 2x1.2 GB, spinors 0.2 GB each)",
+                   "parallelism": "replicas only (one independent solve per GPU)",
+                   "value_definition": "sum over all kernels of the step of their algorithmic HBM bytes / step time"},
+        "roofline": {"bound": "hbm", "achieved": ds_bytes / (ds_ms * 1e-3) / 1e9 if ds_ms > 0 else None,
+                     "peak": peak, "unit": "GB/s",
+                     "frac": (ds_bytes / (ds_ms * 1e-3) / 1e9 / peak) if ds_ms > 0 else None,
+                     "traffic": TRAFFIC_BYTES_PER_LAUNCH, "kernel": "dslash_kernel<double,18,*,EPI 1|2> (fused clover epilogues)",
+                     "launches_timed": n_ds, "avg_launch_us": ds_ms * 1e3 / max(n_ds, 1),
+                     "alg_bytes_per_launch": ds_bytes / max(n_ds, 1), "peak_source": peak_src,
+                     "frac_of_8TBps": (ds_bytes / (ds_ms * 1e-3) / 8e12) if ds_ms > 0 else None},
+        "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        "solve": {"solver": "cgne", "tol": tol, "iterations": res.iterations, "seconds": res.seconds,
+                  "iter_resid": res.iter_resid, "true_resid": res.true_resid, "status": res.status,
+                  "dslash_count": res.dslash_count, "kernel_launches": res.kernel_launches},
+    }
+    if rank == 0 and not args.no_sweep:
+        line["dslash"] = dslash_sweep(torch, lqcd, U, b, dims, local, peak)
+    if rank == 0 and world == 1 and not args.no_cpu:
+        gbs, ms, cores = oracle_sample(12, 0)
+        line["cpu_baseline"] = {"value": gbs, "unit": "GB/s", "cores": cores, "kind": "oracle",
+                                "sample": "12 full-lattice fp64 hopping-term applications (24 parity sweeps) at 32^3x64; "
+                                          "algorithmic dslash bytes / time", "ms_per_application": ms}
+    if rank == 0:
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
+# ncu --set full capture (profiles/), or None until one exists
+TRAFFIC_BYTES_PER_LAUNCH = None
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-sweep", action="store_true", help="skip the standalone dslash sweep")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the CPU-oracle baseline leg")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_gpu(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

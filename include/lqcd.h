@@ -68,6 +68,16 @@ const char* lqcd_last_error(const lqcd_ctx* ctx);
 /* number of kernels this context has launched since creation (bench.py's gpu_launches) */
 long lqcd_launch_count(const lqcd_ctx* ctx);
 
+/* Algorithmic HBM bytes (compulsory reads + writes of each kernel) summed over
+ * every kernel this context has launched since creation (bench.py's whole-step throughput). */
+double lqcd_algorithmic_bytes(const lqcd_ctx* ctx);
+/* Per-launch device timing of the dslash kernels (all epilogues) with CUDA events on the launching
+ * stream.  enable != 0 starts recording (up to 8192 launches), 0 stops.  lqcd_profile_read
+ * synchronises the recorded events, returns the number of launches, their summed duration in ms
+ * and their summed algorithmic bytes, and clears the record. */
+int lqcd_profile_enable(lqcd_ctx* ctx, int enable);
+int lqcd_profile_read(lqcd_ctx* ctx, long* launches, double* total_ms, double* total_bytes);
+
 /* Byte sizes of native buffers: links (4 directions, both parities), ONE parity of a spinor,
  * the clover field (both parities; same size for A and for A^-1), the solver workspace. */
 size_t lqcd_gauge_bytes(const lqcd_ctx* ctx);
@@ -126,6 +136,8 @@ int lqcd_invert(lqcd_ctx* ctx, void* x_public, const void* b_public, const void*
  * packs, computes, unpacks and downloads the public result.  Links/clover stay resident on the
  * device (PAPER.md:225 loadGauge).  scratch: device buffer of >= lqcd_host_scratch_bytes. */
 size_t lqcd_host_scratch_bytes(const lqcd_ctx* ctx, int solver);
+int lqcd_gauge_pack_host(lqcd_ctx* ctx, void* gauge_native, const void* gauge_public_host, void* scratch,
+                         void* stream); /* scratch: >= 4*V*18*prec bytes (the public link field) */
 int lqcd_dslash_host(lqcd_ctx* ctx, void* out_public_host, const void* in_public_host, const void* gauge,
                      int parity, double scale, int dagger, void* scratch, void* stream);
 int lqcd_invert_host(lqcd_ctx* ctx, void* x_public_host, const void* b_public_host, const void* gauge,

@@ -282,6 +282,7 @@ static inline int blas_launch(lqcd_ctx* c, const Op& op, void* const* v, const i
   red.ticket = c->d_ticket;
   red.max_blocks = c->max_red_blocks;
   for (int k = 0; k < 4; k++) red.out[k] = out_slots ? out_slots[k] : 0;
+  c->alg_bytes += (double)(__builtin_popcount(Op::LOAD) + __builtin_popcount(Op::STORE)) * 24.0 * sizeof(T) * c->lat.Vh;
   blas_kernel<T, Op><<<grid, BLAS_BLOCK, 0, st>>>(op, vecs, nvec, red);
   LQCD_LAUNCH_CHECK(c, "blas");
   return LQCD_OK;

@@ -222,6 +222,7 @@ extern "C" int lqcd_clover_build(lqcd_ctx* c, void* clover, void* clover_inv, co
   const int n = 2 * c->lat.Vh, block = 64, grid = (n + block - 1) / block;
   const double kc = kappa * csw;
   cudaMemsetAsync(c->d_flag, 0, sizeof(int), st);
+  c->alg_bytes += (double)lqcd_gauge_bytes(c) + (clover_inv ? 2.0 : 1.0) * (double)lqcd_clover_bytes(c);
   if (c->prec == 4 && c->recon == 18)
     clover_build_kernel<float, 18><<<grid, block, 0, st>>>((float*)clover, (float*)clover_inv, (const float*)gauge, c->lat, kc, c->d_flag);
   else if (c->prec == 4)

@@ -108,7 +108,42 @@ int lqcd_destroy(lqcd_ctx* c) {
   if (c->h_flag) cudaFreeHost(c->h_flag);
   if (c->ev0) cudaEventDestroy(c->ev0);
   if (c->ev1) cudaEventDestroy(c->ev1);
+  if (c->prof_ev) {
+    for (int i = 0; i < 2 * c->prof_cap; i++) cudaEventDestroy(c->prof_ev[i]);
+    delete[] c->prof_ev;
+  }
   delete c;
+  return LQCD_OK;
+}
+
+double lqcd_algorithmic_bytes(const lqcd_ctx* c) { return c ? c->alg_bytes : 0.0; }
+
+int lqcd_profile_enable(lqcd_ctx* c, int enable) {
+  if (!c) return LQCD_ERR_INVALID_ARG;
+  if (enable && !c->prof_ev) {
+    c->prof_cap = 8192;
+    c->prof_ev = new cudaEvent_t[2 * c->prof_cap];
+    for (int i = 0; i < 2 * c->prof_cap; i++)
+      if (cudaEventCreate(&c->prof_ev[i]) != cudaSuccess) return lqcd_check_cuda(c, "profile events");
+  }
+  c->prof_on = enable ? 1 : 0;
+  return LQCD_OK;
+}
+
+int lqcd_profile_read(lqcd_ctx* c, long* launches, double* total_ms, double* total_bytes) {
+  if (!c || !launches || !total_ms || !total_bytes) return LQCD_ERR_INVALID_ARG;
+  double ms = 0;
+  for (int i = 0; i < c->prof_n; i++) {
+    if (cudaEventSynchronize(c->prof_ev[2 * i + 1]) != cudaSuccess) return lqcd_check_cuda(c, "profile sync");
+    float t = 0;
+    cudaEventElapsedTime(&t, c->prof_ev[2 * i], c->prof_ev[2 * i + 1]);
+    ms += t;
+  }
+  *launches = c->prof_n;
+  *total_ms = ms;
+  *total_bytes = c->prof_bytes;
+  c->prof_n = 0;
+  c->prof_bytes = 0;
   return LQCD_OK;
 }
 

@@ -95,14 +95,26 @@ static void launch_typed(lqcd_ctx* c, void* out, const void* in, const void* gau
 // parity (or NULL for epi 0); x: one-parity spinor (epi 2,3).
 int lqcd_dslash_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
                        int parity, double scale, int dagger, int epi, cudaStream_t st) {
+  // algorithmic bytes: every link once, input spinor once, output once (+ clover, + x)
+  const double bytes = (double)c->lat.Vh * c->prec *
+                       (8.0 * c->recon + 48.0 + (epi >= 1 ? 72.0 : 0.0) + (epi >= 2 ? 24.0 : 0.0));
+  c->alg_bytes += bytes;
+  const bool rec = c->prof_on && c->prof_n < c->prof_cap;
+  if (rec) cudaEventRecord(c->prof_ev[2 * c->prof_n], st);
   if (c->prec == 4) launch_typed<float>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, st);
   else launch_typed<double>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, st);
+  if (rec) {
+    cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], st);
+    c->prof_n++;
+    c->prof_bytes += bytes;
+  }
   LQCD_LAUNCH_CHECK(c, "dslash");
   return LQCD_OK;
 }
 
 int lqcd_clover_apply_launch(lqcd_ctx* c, void* out, const void* in, const void* cl_parity, cudaStream_t st) {
   const int Vh = c->lat.Vh, block = 128, grid = (Vh + block - 1) / block;
+  c->alg_bytes += (double)Vh * c->prec * (72.0 + 48.0);
   if (c->prec == 4) clover_apply_kernel<float><<<grid, block, 0, st>>>((float*)out, (const float*)in, (const float*)cl_parity, Vh);
   else clover_apply_kernel<double><<<grid, block, 0, st>>>((double*)out, (const double*)in, (const double*)cl_parity, Vh);
   LQCD_LAUNCH_CHECK(c, "clover_apply");

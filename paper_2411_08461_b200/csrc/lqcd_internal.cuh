@@ -33,6 +33,11 @@ struct lqcd_ctx {
   int* h_flag;
   int max_red_blocks;
   cudaEvent_t ev0, ev1;
+  // accounting: algorithmic bytes of every launch; optional per-launch event timing of dslash
+  double alg_bytes;
+  int prof_on, prof_n, prof_cap;
+  cudaEvent_t* prof_ev;  // 2 events per recorded launch
+  double prof_bytes;
 };
 
 int lqcd_set_error(lqcd_ctx* ctx, int code, const char* fmt, ...);

@@ -57,6 +57,7 @@ int lqcd_gauge_pack(lqcd_ctx* c, void* native, const void* pub, void* stream) {
   else if (c->prec == 4) launch_to_soa<float, float4, 4, 18, 3>(native, pub, Vh, 8, st);
   else if (c->recon == 18) launch_to_soa<double, double2, 2, 18, 9>(native, pub, Vh, 8, st);
   else launch_to_soa<double, double2, 2, 18, 6>(native, pub, Vh, 8, st);
+  c->alg_bytes += (double)4 * c->V * 18 * c->prec + (double)lqcd_gauge_bytes(c);
   LQCD_LAUNCH_CHECK(c, "gauge_pack");
   return LQCD_OK;
 }
@@ -67,6 +68,7 @@ int lqcd_spinor_pack(lqcd_ctx* c, void* native, const void* pub, void* stream) {
   cudaStream_t st = as_stream(stream);
   if (c->prec == 4) launch_to_soa<float, float4, 4, 24, 6>(native, pub, c->lat.Vh, 2, st);
   else launch_to_soa<double, double2, 2, 24, 12>(native, pub, c->lat.Vh, 2, st);
+  c->alg_bytes += 4.0 * (double)lqcd_spinor_bytes(c);
   LQCD_LAUNCH_CHECK(c, "spinor_pack");
   return LQCD_OK;
 }
@@ -77,6 +79,7 @@ int lqcd_spinor_unpack(lqcd_ctx* c, void* pub, const void* native, void* stream)
   cudaStream_t st = as_stream(stream);
   if (c->prec == 4) launch_to_aos<float, float4, 4, 24, 6>(pub, native, c->lat.Vh, 2, st);
   else launch_to_aos<double, double2, 2, 24, 12>(pub, native, c->lat.Vh, 2, st);
+  c->alg_bytes += 4.0 * (double)lqcd_spinor_bytes(c);
   LQCD_LAUNCH_CHECK(c, "spinor_unpack");
   return LQCD_OK;
 }
@@ -87,6 +90,7 @@ int lqcd_clover_unpack(lqcd_ctx* c, void* pub, const void* native, void* stream)
   cudaStream_t st = as_stream(stream);
   if (c->prec == 4) launch_to_aos<float, float4, 4, 72, 18>(pub, native, c->lat.Vh, 2, st);
   else launch_to_aos<double, double2, 2, 72, 36>(pub, native, c->lat.Vh, 2, st);
+  c->alg_bytes += 2.0 * (double)lqcd_clover_bytes(c);
   LQCD_LAUNCH_CHECK(c, "clover_unpack");
   return LQCD_OK;
 }
@@ -97,12 +101,14 @@ int lqcd_clover_unpack(lqcd_ctx* c, void* pub, const void* native, void* stream)
 int lqcd_spinor_pack_parity(lqcd_ctx* c, void* native, const void* pub, cudaStream_t st) {
   if (c->prec == 4) launch_to_soa<float, float4, 4, 24, 6>(native, pub, c->lat.Vh, 1, st);
   else launch_to_soa<double, double2, 2, 24, 12>(native, pub, c->lat.Vh, 1, st);
+  c->alg_bytes += 2.0 * (double)lqcd_spinor_bytes(c);
   LQCD_LAUNCH_CHECK(c, "spinor_pack_parity");
   return LQCD_OK;
 }
 int lqcd_spinor_unpack_parity(lqcd_ctx* c, void* pub, const void* native, cudaStream_t st) {
   if (c->prec == 4) launch_to_aos<float, float4, 4, 24, 6>(pub, native, c->lat.Vh, 1, st);
   else launch_to_aos<double, double2, 2, 24, 12>(pub, native, c->lat.Vh, 1, st);
+  c->alg_bytes += 2.0 * (double)lqcd_spinor_bytes(c);
   LQCD_LAUNCH_CHECK(c, "spinor_unpack_parity");
   return LQCD_OK;
 }

@@ -357,6 +357,13 @@ size_t lqcd_host_scratch_bytes(const lqcd_ctx* c, int solver) {
   return c ? 4 * lqcd_spinor_bytes(c) + lqcd_invert_workspace_bytes(c, solver) : 0;
 }
 
+int lqcd_gauge_pack_host(lqcd_ctx* c, void* native, const void* pub_host, void* scratch, void* stream) {
+  if (!c || !native || !pub_host || !scratch) return LQCD_ERR_INVALID_ARG;
+  cudaStream_t st = as_stream(stream);
+  cudaMemcpyAsync(scratch, pub_host, (size_t)4 * c->V * 18 * c->prec, cudaMemcpyHostToDevice, st);
+  return lqcd_gauge_pack(c, native, scratch, stream);
+}
+
 // scratch: [public in (1 parity)] [public out (1 parity)] [native in] [native out]
 int lqcd_dslash_host(lqcd_ctx* c, void* out_host, const void* in_host, const void* gauge, int parity, double scale,
                      int dagger, void* scratch, void* stream) {

@@ -28,6 +28,7 @@ class Result(ctypes.Structure):
 SOLVERS = {"cgne": 0, "cgnr": 1, "bicgstab": 2}
 SYMBOLS = [
     "lqcd_create", "lqcd_destroy", "lqcd_strerror", "lqcd_last_error", "lqcd_launch_count",
+    "lqcd_algorithmic_bytes", "lqcd_profile_enable", "lqcd_profile_read", "lqcd_gauge_pack_host",
     "lqcd_gauge_bytes", "lqcd_spinor_bytes", "lqcd_clover_bytes", "lqcd_invert_workspace_bytes",
     "lqcd_gauge_pack", "lqcd_spinor_pack", "lqcd_spinor_unpack", "lqcd_clover_unpack",
     "lqcd_clover_build", "lqcd_clover_apply", "lqcd_dslash", "lqcd_mpc_apply", "lqcd_mat_apply",
@@ -58,6 +59,11 @@ def load():
     L.lqcd_last_error.argtypes = [vp]
     L.lqcd_launch_count.restype = ctypes.c_long
     L.lqcd_launch_count.argtypes = [vp]
+    L.lqcd_algorithmic_bytes.restype = cd
+    L.lqcd_algorithmic_bytes.argtypes = [vp]
+    L.lqcd_profile_enable.argtypes = [vp, ci]
+    L.lqcd_profile_read.argtypes = [vp, ctypes.POINTER(ctypes.c_long), ctypes.POINTER(cd), ctypes.POINTER(cd)]
+    L.lqcd_gauge_pack_host.argtypes = [vp, vp, vp, vp, vp]
     for f in ("lqcd_gauge_bytes", "lqcd_spinor_bytes", "lqcd_clover_bytes"):
         getattr(L, f).restype = sz
         getattr(L, f).argtypes = [vp]
@@ -141,6 +147,22 @@ class Context:
 
     def launch_count(self):
         return self.lib.lqcd_launch_count(self.h)
+
+    def algorithmic_bytes(self):
+        return self.lib.lqcd_algorithmic_bytes(self.h)
+
+    def profile_enable(self, on=True):
+        self._check(self.lib.lqcd_profile_enable(self.h, int(on)))
+
+    def profile_read(self):
+        """(launches, total ms, total algorithmic bytes) of the dslash kernels recorded so far."""
+        n, ms, by = ctypes.c_long(), ctypes.c_double(), ctypes.c_double()
+        self._check(self.lib.lqcd_profile_read(self.h, ctypes.byref(n), ctypes.byref(ms), ctypes.byref(by)))
+        return n.value, ms.value, by.value
+
+    def gauge_pack_host(self, gauge_native, U_host, scratch):
+        self._check(self.lib.lqcd_gauge_pack_host(self.h, _p(gauge_native), _p(U_host), _p(scratch), _stream()))
+        return gauge_native
 
     def empty(self, nbytes):
         return torch.empty(nbytes // self.prec, dtype=self.rdtype, device=self.dev)
