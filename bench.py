@@ -177,6 +177,19 @@ def dslash_sweep(torch, lqcd, U, psi, dims, device, peak):
     return out
 
 
+def reduce_over_ranks(dist, dt, sums, device):
+    """Multi-replica aggregation: MAX of the device time over ranks, SUM of the work counters.
+    dist = torch.distributed (initialised) or None for a single process."""
+    if dist is None:
+        return dt, list(sums)
+    import torch
+    t = torch.tensor([dt], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    s = torch.tensor(list(sums), device=device, dtype=torch.float64)
+    dist.all_reduce(s, op=dist.ReduceOp.SUM)
+    return float(t.item()), [float(v) for v in s.tolist()]
+
+
 def run_gpu(args):
     import torch
     from paper_2411_08461_b200 import lqcd, synth
@@ -235,13 +248,7 @@ def run_gpu(args):
     launches = ctx.launch_count() - l0
     alg = ctx.algorithmic_bytes() - a0
     n_ds, ds_ms, ds_bytes = ctx.profile_read()
-    if dist is not None:
-        t = torch.tensor([dt], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dt = float(t.item())
-        s = torch.tensor([alg, float(launches)], device="cuda", dtype=torch.float64)
-        dist.all_reduce(s, op=dist.ReduceOp.SUM)
-        alg, launches = float(s[0].item()), int(s[1].item())
+    dt, (alg, launches) = reduce_over_ranks(dist, dt, [alg, float(launches)], "cuda")
     value = alg / dt / 1e9
     res = results[-1]
 
@@ -269,11 +276,7 @@ def run_gpu(args):
     barrier()
     dt2 = e0.elapsed_time(e1) * 1e-3
     alg2 = ctx.algorithmic_bytes() - a0
-    if dist is not None:
-        t = torch.tensor([dt2], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dt2 = float(t.item())
-        alg2 *= world
+    dt2, (alg2,) = reduce_over_ranks(dist, dt2, [alg2], "cuda")
     e2e = {"value": alg2 / dt2 / 1e9, "unit": "GB/s",
            "h2d_bytes_per_step": int(U_h.numel() * 16 + b_h.numel() * 16),
            "d2h_bytes_per_step": int(x_h.numel() * 16), "ms_per_step": dt2 / n_e2e * 1e3,
