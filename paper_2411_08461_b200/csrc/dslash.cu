@@ -17,12 +17,42 @@ template <typename T> struct DslashArgs {
   T scale;
 };
 
+// Launch shape per precision (threads per block, minimum resident blocks per SM = register budget).
+// The kernel is latency bound: what matters is how many independent loads ptxas can hoist per
+// thread, which the register budget controls; values chosen by the sweep in profiles/r01_tuning.md.
+#ifndef DSLASH_BLOCK_F32
+#define DSLASH_BLOCK_F32 128
+#endif
+#ifndef DSLASH_MINB_F32
+#define DSLASH_MINB_F32 4
+#endif
+#ifndef DSLASH_BLOCK_F64
+#define DSLASH_BLOCK_F64 64
+#endif
+#ifndef DSLASH_MINB_F64
+#define DSLASH_MINB_F64 5
+#endif
+#ifndef DSLASH_STAGE_F32
+#define DSLASH_STAGE_F32 0
+#endif
+#ifndef DSLASH_STAGE_F64
+#define DSLASH_STAGE_F64 0
+#endif
+template <typename T> struct Tune;
+template <> struct Tune<float> { static constexpr int BLOCK = DSLASH_BLOCK_F32, MINB = DSLASH_MINB_F32; static constexpr bool STAGE = DSLASH_STAGE_F32; };
+template <> struct Tune<double> { static constexpr int BLOCK = DSLASH_BLOCK_F64, MINB = DSLASH_MINB_F64; static constexpr bool STAGE = DSLASH_STAGE_F64; };
+
 template <typename T, int R, bool DAG, int EPI>
-__global__ void __launch_bounds__(128) dslash_kernel(const DslashArgs<T> a) {
+__global__ void __launch_bounds__(Tune<T>::BLOCK, Tune<T>::MINB) dslash_kernel(const DslashArgs<T> a) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= a.lat.Vh) return;
   T acc[24];
-  dslash_site<T, R, DAG>(acc, a.in, a.gauge, a.lat, idx, a.parity);
+  if (Tune<T>::STAGE) {
+    extern __shared__ __align__(16) unsigned char dslash_smem[];
+    dslash_site_staged<T, R, DAG, Tune<T>::BLOCK>(acc, a.in, a.gauge, a.lat, idx, a.parity, dslash_smem);
+  } else {
+    dslash_site<T, R, DAG>(acc, a.in, a.gauge, a.lat, idx, a.parity);
+  }
   T res[24];
   if (EPI == 0) {
 #pragma unroll
@@ -60,13 +90,22 @@ __global__ void __launch_bounds__(128) clover_apply_kernel(T* __restrict__ out, 
 
 template <typename T, int R, bool DAG>
 static void launch_epi(const DslashArgs<T>& a, int epi, cudaStream_t st) {
-  const int block = 128;
+  const int block = Tune<T>::BLOCK;
   const int grid = (a.lat.Vh + block - 1) / block;
+  const size_t smem = Tune<T>::STAGE ? (size_t)8 * R * sizeof(T) * block : 0;  // eight links per thread
+  static bool configured = false;  // one flag per (T, R, DAG) instantiation
+  if (!configured && smem > 48 * 1024) {
+    cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  }
+  configured = true;
   switch (epi) {
-    case 0: dslash_kernel<T, R, DAG, 0><<<grid, block, 0, st>>>(a); break;
-    case 1: dslash_kernel<T, R, DAG, 1><<<grid, block, 0, st>>>(a); break;
-    case 2: dslash_kernel<T, R, DAG, 2><<<grid, block, 0, st>>>(a); break;
-    default: dslash_kernel<T, R, DAG, 3><<<grid, block, 0, st>>>(a); break;
+    case 0: dslash_kernel<T, R, DAG, 0><<<grid, block, smem, st>>>(a); break;
+    case 1: dslash_kernel<T, R, DAG, 1><<<grid, block, smem, st>>>(a); break;
+    case 2: dslash_kernel<T, R, DAG, 2><<<grid, block, smem, st>>>(a); break;
+    default: dslash_kernel<T, R, DAG, 3><<<grid, block, smem, st>>>(a); break;
   }
 }
 

@@ -142,6 +142,106 @@ __device__ __forceinline__ void dslash_site(T* acc, const T* __restrict__ in, co
   hop<T, R, 3, false, DAG>(acc, in, gauge + (3 * 2 + 1 - par) * blk, Vh, n, n, sb);
 }
 
+// ---------------------------------------------------------------------------------------------
+// Link staging through shared memory with cp.async (LDGSTS).  Links are 67-75 % of the bytes, are
+// streamed exactly once and need no sharing between threads, so each thread copies ITS OWN eight
+// links global->shared asynchronously at kernel entry (one commit group per hop): all link bytes of
+// a block are in flight at once without holding a single register, independently of how ptxas
+// schedules the arithmetic.  Layout in shared memory: [slot = hop][vector][thread] (conflict free).
+// A thread only reads what it copied itself, so cp.async.wait_group is the only synchronisation.
+// ---------------------------------------------------------------------------------------------
+template <int BYTES>
+__device__ __forceinline__ void cp_async(void* smem_dst, const void* gsrc) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  if (BYTES == 16) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+  else asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+template <typename T, int R, int BLOCK>
+__device__ __forceinline__ void stage_link(void* smem, int slot, const T* __restrict__ block, int Vh, int lidx) {
+  typedef typename GV<T, R>::vec vec;
+  constexpr int NGV = R / GV<T, R>::N;
+  vec* sl = reinterpret_cast<vec*>(smem) + (size_t)slot * NGV * BLOCK + threadIdx.x;
+  const vec* g = reinterpret_cast<const vec*>(block) + lidx;
+#pragma unroll
+  for (int v = 0; v < NGV; v++) cp_async<sizeof(vec)>(sl + v * BLOCK, g + (size_t)v * Vh);
+  cp_async_commit();
+}
+template <typename T, int R, int BLOCK>
+__device__ __forceinline__ void fetch_link(const void* smem, int slot, T* U) {
+  typedef typename GV<T, R>::vec vec;
+  constexpr int N = GV<T, R>::N, NGV = R / N;
+  const vec* sl = reinterpret_cast<const vec*>(smem) + (size_t)slot * NGV * BLOCK + threadIdx.x;
+#pragma unroll
+  for (int v = 0; v < NGV; v++) {
+    vec q = sl[v * BLOCK];
+    vec_get(q, U + v * N);
+  }
+  if (R == 12) {
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+      const int a = (c + 1) % 3, b = (c + 2) % 3;
+      T re = U[2 * a] * U[6 + 2 * b] - U[2 * a + 1] * U[6 + 2 * b + 1] - U[2 * b] * U[6 + 2 * a] +
+             U[2 * b + 1] * U[6 + 2 * a + 1];
+      T im = U[2 * a] * U[6 + 2 * b + 1] + U[2 * a + 1] * U[6 + 2 * b] - U[2 * b] * U[6 + 2 * a + 1] -
+             U[2 * b + 1] * U[6 + 2 * a];
+      U[12 + 2 * c] = re;
+      U[12 + 2 * c + 1] = -im;
+    }
+  }
+}
+
+template <typename T, int R, int MU, bool FWD, bool DAG, int BLOCK, int SLOT>
+__device__ __forceinline__ void hop_staged(T* acc, const T* __restrict__ in, const void* smem, int Vh, int nidx, T bsign) {
+  constexpr int S = (FWD != DAG) ? -1 : +1;
+  T psi[24], U[18], h[12], chi[12];
+  load_spinor<T>(in, Vh, nidx, psi);
+  project<T, MU, S>(psi, h);
+  if (MU == 3) {
+#pragma unroll
+    for (int e = 0; e < 12; e++) h[e] *= bsign;
+  }
+  cp_async_wait<7 - SLOT>();
+  fetch_link<T, R, BLOCK>(smem, SLOT, U);
+  su3_mul<T, !FWD>(U, h, chi);
+  reconstruct<T, MU, S>(acc, chi);
+}
+
+template <typename T, int R, bool DAG, int BLOCK>
+__device__ __forceinline__ void dslash_site_staged(T* acc, const T* __restrict__ in, const T* __restrict__ gauge,
+                                                   const Lat& L, int idx, int par, void* smem) {
+  const Site s = site_of(L, idx, par);
+  const int Vh = L.Vh;
+  const size_t blk = (size_t)R * Vh;
+  const int n0 = neighbour<0, +1>(L, idx, s), n1 = neighbour<0, -1>(L, idx, s);
+  const int n2 = neighbour<1, +1>(L, idx, s), n3 = neighbour<1, -1>(L, idx, s);
+  const int n4 = neighbour<2, +1>(L, idx, s), n5 = neighbour<2, -1>(L, idx, s);
+  const int n6 = neighbour<3, +1>(L, idx, s), n7 = neighbour<3, -1>(L, idx, s);
+  stage_link<T, R, BLOCK>(smem, 0, gauge + (0 * 2 + par) * blk, Vh, idx);
+  stage_link<T, R, BLOCK>(smem, 1, gauge + (0 * 2 + 1 - par) * blk, Vh, n1);
+  stage_link<T, R, BLOCK>(smem, 2, gauge + (1 * 2 + par) * blk, Vh, idx);
+  stage_link<T, R, BLOCK>(smem, 3, gauge + (1 * 2 + 1 - par) * blk, Vh, n3);
+  stage_link<T, R, BLOCK>(smem, 4, gauge + (2 * 2 + par) * blk, Vh, idx);
+  stage_link<T, R, BLOCK>(smem, 5, gauge + (2 * 2 + 1 - par) * blk, Vh, n5);
+  stage_link<T, R, BLOCK>(smem, 6, gauge + (3 * 2 + par) * blk, Vh, idx);
+  stage_link<T, R, BLOCK>(smem, 7, gauge + (3 * 2 + 1 - par) * blk, Vh, n7);
+#pragma unroll
+  for (int e = 0; e < 24; e++) acc[e] = 0;
+  const T one = 1;
+  const T sf = (L.tb < 0 && s.t == L.Lt - 1) ? -one : one;
+  const T sb = (L.tb < 0 && s.t == 0) ? -one : one;
+  hop_staged<T, R, 0, true, DAG, BLOCK, 0>(acc, in, smem, Vh, n0, one);
+  hop_staged<T, R, 0, false, DAG, BLOCK, 1>(acc, in, smem, Vh, n1, one);
+  hop_staged<T, R, 1, true, DAG, BLOCK, 2>(acc, in, smem, Vh, n2, one);
+  hop_staged<T, R, 1, false, DAG, BLOCK, 3>(acc, in, smem, Vh, n3, one);
+  hop_staged<T, R, 2, true, DAG, BLOCK, 4>(acc, in, smem, Vh, n4, one);
+  hop_staged<T, R, 2, false, DAG, BLOCK, 5>(acc, in, smem, Vh, n5, one);
+  hop_staged<T, R, 3, true, DAG, BLOCK, 6>(acc, in, smem, Vh, n6, sf);
+  hop_staged<T, R, 3, false, DAG, BLOCK, 7>(acc, in, smem, Vh, n7, sb);
+}
+
 // out = C v for the two Hermitian 6x6 chiral blocks of one site.  cl = one-parity clover field
 // [NCV][Vh]; packed order per block: 6 real diagonal, then 15 complex lower entries row-major.
 // v and out are 24-real spinors (block k acts on reals 12k..12k+11); they must not alias.
