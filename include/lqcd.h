@@ -45,6 +45,7 @@ enum {
 };
 enum { LQCD_SOLVER_CGNE = 0, LQCD_SOLVER_CGNR = 1, LQCD_SOLVER_BICGSTAB = 2 };
 enum { LQCD_MATPC_ASYMMETRIC = 0, LQCD_MATPC_SYMMETRIC = 1 };
+#define LQCD_MAX_RHS 16 /* right-hand sides per multi-RHS call (a propagator has 12 columns) */
 
 typedef struct lqcd_result {
   int status;          /* LQCD_OK, LQCD_NOT_CONVERGED or LQCD_ERR_BREAKDOWN */
@@ -131,6 +132,29 @@ int lqcd_mat_apply(lqcd_ctx* ctx, void* out, const void* in, const void* gauge, 
 int lqcd_invert(lqcd_ctx* ctx, void* x_public, const void* b_public, const void* gauge, const void* clover,
                 const void* clover_inv, double kappa, double csw, double tol, int maxiter, int solver,
                 int matpc, void* workspace, size_t workspace_bytes, lqcd_result* res, void* stream);
+
+/* Multi-right-hand-side forms (a propagator is 12 solves, one
+ * per spin-colour column, on the same links and clover).  The links are loaded once per site for all
+ * nrhs columns, so the bytes per site and column fall from (8R+48)w towards (8R/nrhs+48)w.
+ * Native multi-RHS fields are nrhs consecutive one-parity native spinors ([rhs][one-parity native]);
+ * 1 <= nrhs <= LQCD_MAX_RHS; nrhs = 1 runs the single-RHS kernels.
+ *   lqcd_dslash_mrhs    : out[r] = scale * D_{p,1-p} in[r]                      (as lqcd_dslash)
+ *   lqcd_mpc_apply_mrhs : out[r] = Mhat in[r]; tmp_o: nrhs one-parity spinors   (as lqcd_mpc_apply)
+ *   lqcd_invert_multi   : nrhs independent Krylov recurrences advanced in lock step (each column has
+ *       its own alpha, beta, omega and stopping test |r_hat_r| <= tol*|b_r|; a converged column is
+ *       frozen, so every column's result is that of its own single solve).  x_public/b_public: nrhs
+ *       consecutive public spinors; res: array of nrhs results.  Returns the worst status: the
+ *       most negative error if any column failed, else NOT_CONVERGED if any did not converge, else
+ *       OK.  workspace: >= lqcd_invert_multi_workspace_bytes; clover and clover_inv are required. */
+int lqcd_dslash_mrhs(lqcd_ctx* ctx, void* out, const void* in, const void* gauge, int parity, double scale,
+                     int dagger, int nrhs, void* stream);
+int lqcd_mpc_apply_mrhs(lqcd_ctx* ctx, void* out_e, const void* in_e, const void* gauge, const void* clover,
+                        const void* clover_inv, double kappa, int matpc, int dagger, void* tmp_o, int nrhs,
+                        void* stream);
+size_t lqcd_invert_multi_workspace_bytes(const lqcd_ctx* ctx, int solver, int nrhs);
+int lqcd_invert_multi(lqcd_ctx* ctx, void* x_public, const void* b_public, const void* gauge, const void* clover,
+                      const void* clover_inv, double kappa, double tol, int maxiter, int solver, int matpc,
+                      int nrhs, void* workspace, size_t workspace_bytes, lqcd_result* res, void* stream);
 
 /* End-to-end variants with HOST buffers (pageable or pinned): the call uploads the public input,
  * packs, computes, unpacks and downloads the public result.  Links/clover stay resident on the

@@ -11,6 +11,13 @@
 
 constexpr int BLAS_BLOCK = 256;
 constexpr int BLAS_MAXV = 6;
+// Batched (multi-right-hand-side) form: blockIdx.y selects the right-hand side; every vector is a
+// block of nrhs consecutive one-parity spinors, every right-hand side owns SC_STRIDE scalar slots,
+// its own partials and its own ticket.  Slot S_DONE != 0 freezes a right-hand side (its blocks exit
+// at once: a converged column is no longer updated); slot S_FIRST marks BiCGStab's first iteration.
+constexpr int SC_STRIDE = 64;
+constexpr int S_DONE = 60, S_FIRST = 61;
+constexpr int BLAS_MAXR = 4;  // reductions per launch
 
 template <typename T> struct BlasVecs {
   T* v[BLAS_MAXV];
@@ -70,6 +77,8 @@ struct RedArgs {
   double* scalars;
   unsigned int* ticket;
   int max_blocks;
+  int rhs0;       // first right-hand side of this launch
+  size_t stride;  // reals between consecutive right-hand sides of a vector block
   int out[4];
 };
 
@@ -81,6 +90,13 @@ template <typename T, typename Op>
 __global__ void __launch_bounds__(BLAS_BLOCK) blas_kernel(Op op, BlasVecs<T> vecs, long nvec, RedArgs red) {
   typedef typename V16<T>::vec vec;
   constexpr int N = V16<T>::N;
+  const int rhs = red.rhs0 + blockIdx.y;
+  red.scalars += (size_t)rhs * SC_STRIDE;
+  if (red.scalars[S_DONE] != 0.0) return;  // frozen right-hand side (uniform over its blocks)
+  red.partial += (size_t)rhs * BLAS_MAXR * red.max_blocks;
+  red.ticket += rhs;
+#pragma unroll
+  for (int a = 0; a < Op::NV; a++) vecs.v[a] += (size_t)rhs * red.stride;
   op.init(red.scalars);
   double acc[Op::NR > 0 ? Op::NR : 1];
 #pragma unroll
@@ -213,9 +229,11 @@ template <typename T> struct OpXpayRatio {
 template <typename T> struct OpBicgP {
   static constexpr int NV = 3, NR = 0;
   static constexpr unsigned LOAD = 7, STORE = 1;
-  int rho, r0v, ts, first;
+  int rho, r0v, ts;
+  bool first;
   cplxd beta, omega;
   __device__ void init(const double* s) {
+    first = s[S_FIRST] != 0.0;
     if (first) { beta = {0, 0}; omega = {0, 0}; return; }
     omega = {s[ts] / s[ts + 2], s[ts + 1] / s[ts + 2]};
     beta = cdiv(cdiv({s[rho], s[rho + 1]}, {s[r0v], s[r0v + 1]}), omega);
@@ -269,8 +287,10 @@ template <typename T> struct OpBicgXR {
   }
 };
 
+// v[a]: base of vector block a (right-hand side 0); right-hand sides rhs0 .. rhs0+nrhs-1 are processed
 template <typename T, typename Op>
-static inline int blas_launch(lqcd_ctx* c, const Op& op, void* const* v, const int* out_slots, cudaStream_t st) {
+static inline int blas_launch(lqcd_ctx* c, const Op& op, void* const* v, const int* out_slots, int nrhs, int rhs0,
+                              cudaStream_t st) {
   BlasVecs<T> vecs;
   for (int a = 0; a < BLAS_MAXV; a++) vecs.v[a] = a < Op::NV ? (T*)v[a] : nullptr;
   const long nvec = (long)Lay<T>::NSV * c->lat.Vh;
@@ -281,9 +301,12 @@ static inline int blas_launch(lqcd_ctx* c, const Op& op, void* const* v, const i
   red.scalars = c->d_scalars;
   red.ticket = c->d_ticket;
   red.max_blocks = c->max_red_blocks;
+  red.rhs0 = rhs0;
+  red.stride = (size_t)24 * c->lat.Vh;
   for (int k = 0; k < 4; k++) red.out[k] = out_slots ? out_slots[k] : 0;
-  c->alg_bytes += (double)(__builtin_popcount(Op::LOAD) + __builtin_popcount(Op::STORE)) * 24.0 * sizeof(T) * c->lat.Vh;
-  blas_kernel<T, Op><<<grid, BLAS_BLOCK, 0, st>>>(op, vecs, nvec, red);
+  const int acct = (c->acct_rhs > 0 && c->acct_rhs < nrhs) ? c->acct_rhs : nrhs;  // frozen columns move no bytes
+  c->alg_bytes += (double)(__builtin_popcount(Op::LOAD) + __builtin_popcount(Op::STORE)) * 24.0 * sizeof(T) * c->lat.Vh * acct;
+  blas_kernel<T, Op><<<dim3(grid, nrhs), BLAS_BLOCK, 0, st>>>(op, vecs, nvec, red);
   LQCD_LAUNCH_CHECK(c, "blas");
   return LQCD_OK;
 }

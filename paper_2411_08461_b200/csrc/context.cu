@@ -76,17 +76,20 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], int prec, int recon, int t_bo
   c->sm_count = prop.multiProcessorCount;
   c->max_red_blocks = 8 * c->sm_count;
   strcpy(c->err, "ok");
-  bool ok = cudaMalloc(&c->d_partial, sizeof(double) * 8 * c->max_red_blocks) == cudaSuccess &&
-            cudaMalloc(&c->d_scalars, sizeof(double) * 64) == cudaSuccess &&
-            cudaMalloc(&c->d_ticket, sizeof(unsigned int) * 4) == cudaSuccess &&
+  bool ok = cudaMalloc(&c->d_partial, sizeof(double) * 4 * c->max_red_blocks * LQCD_MAX_RHS) == cudaSuccess &&
+            cudaMalloc(&c->d_scalars, sizeof(double) * 64 * LQCD_MAX_RHS) == cudaSuccess &&
+            cudaMalloc(&c->d_ticket, sizeof(unsigned int) * LQCD_MAX_RHS) == cudaSuccess &&
             cudaMalloc(&c->d_flag, sizeof(int) * 4) == cudaSuccess &&
-            cudaMallocHost(&c->h_scalars, sizeof(double) * 64) == cudaSuccess &&
+            cudaMallocHost(&c->h_scalars, sizeof(double) * 64 * LQCD_MAX_RHS) == cudaSuccess &&
+            cudaMallocHost(&c->h_consts, sizeof(double) * 2) == cudaSuccess &&
             cudaMallocHost(&c->h_flag, sizeof(int) * 4) == cudaSuccess &&
             cudaEventCreate(&c->ev0) == cudaSuccess && cudaEventCreate(&c->ev1) == cudaSuccess;
   if (ok) {
-    ok = cudaMemset(c->d_ticket, 0, sizeof(unsigned int) * 4) == cudaSuccess &&
+    c->h_consts[0] = 0.0;
+    c->h_consts[1] = 1.0;
+    ok = cudaMemset(c->d_ticket, 0, sizeof(unsigned int) * LQCD_MAX_RHS) == cudaSuccess &&
          cudaMemset(c->d_flag, 0, sizeof(int) * 4) == cudaSuccess &&
-         cudaMemset(c->d_scalars, 0, sizeof(double) * 64) == cudaSuccess;
+         cudaMemset(c->d_scalars, 0, sizeof(double) * 64 * LQCD_MAX_RHS) == cudaSuccess;
   }
   if (!ok) {
     cudaGetLastError();
@@ -105,6 +108,7 @@ int lqcd_destroy(lqcd_ctx* c) {
   if (c->d_ticket) cudaFree(c->d_ticket);
   if (c->d_flag) cudaFree(c->d_flag);
   if (c->h_scalars) cudaFreeHost(c->h_scalars);
+  if (c->h_consts) cudaFreeHost(c->h_consts);
   if (c->h_flag) cudaFreeHost(c->h_flag);
   if (c->ev0) cudaEventDestroy(c->ev0);
   if (c->ev1) cudaEventDestroy(c->ev1);

@@ -82,6 +82,8 @@ __global__ void __launch_bounds__(128) clover_apply_kernel(T* __restrict__ out, 
                                                            const T* __restrict__ cl, int Vh) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= Vh) return;
+  out += (size_t)blockIdx.y * 24 * Vh;  // right-hand side
+  in += (size_t)blockIdx.y * 24 * Vh;
   T v[24], r[24];
   load_spinor<T>(in, Vh, idx, v);
   clover_mul<T>(cl, Vh, idx, v, r);
@@ -131,9 +133,11 @@ static void launch_typed(lqcd_ctx* c, void* out, const void* in, const void* gau
 }
 
 // internal entry used by the C ABI and by the solvers.  cl: one-parity clover block of the output
-// parity (or NULL for epi 0); x: one-parity spinor (epi 2,3).
+// parity (or NULL for epi 0); x: one-parity spinor (epi 2,3).  nrhs > 1: `in`, `out`, `x` are nrhs
+// consecutive one-parity spinors and the multi-right-hand-side kernel (dslash_mrhs.cu) runs.
 int lqcd_dslash_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
-                       int parity, double scale, int dagger, int epi, cudaStream_t st) {
+                       int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st) {
+  if (nrhs > 1) return lqcd_dslash_mrhs_launch(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st);
   // algorithmic bytes: every link once, input spinor once, output once (+ clover, + x)
   const double bytes = (double)c->lat.Vh * c->prec *
                        (8.0 * c->recon + 48.0 + (epi >= 1 ? 72.0 : 0.0) + (epi >= 2 ? 24.0 : 0.0));
@@ -151,9 +155,10 @@ int lqcd_dslash_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge
   return LQCD_OK;
 }
 
-int lqcd_clover_apply_launch(lqcd_ctx* c, void* out, const void* in, const void* cl_parity, cudaStream_t st) {
-  const int Vh = c->lat.Vh, block = 128, grid = (Vh + block - 1) / block;
-  c->alg_bytes += (double)Vh * c->prec * (72.0 + 48.0);
+int lqcd_clover_apply_launch(lqcd_ctx* c, void* out, const void* in, const void* cl_parity, int nrhs, cudaStream_t st) {
+  const int Vh = c->lat.Vh, block = 128;
+  const dim3 grid((Vh + block - 1) / block, nrhs);
+  c->alg_bytes += (double)Vh * c->prec * (72.0 + 48.0 * nrhs);
   if (c->prec == 4) clover_apply_kernel<float><<<grid, block, 0, st>>>((float*)out, (const float*)in, (const float*)cl_parity, Vh);
   else clover_apply_kernel<double><<<grid, block, 0, st>>>((double*)out, (const double*)in, (const double*)cl_parity, Vh);
   LQCD_LAUNCH_CHECK(c, "clover_apply");
@@ -168,7 +173,7 @@ int lqcd_dslash(lqcd_ctx* c, void* out, const void* in, const void* gauge, int p
   if (out == in) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "dslash: out aliases in");
   if (!lqcd_aligned16(out) || !lqcd_aligned16(in) || !lqcd_aligned16(gauge))
     return lqcd_set_error(c, LQCD_ERR_ALIGN, "dslash: alignment");
-  return lqcd_dslash_launch(c, out, in, gauge, nullptr, nullptr, parity, scale, dagger ? 1 : 0, 0, as_stream(stream));
+  return lqcd_dslash_launch(c, out, in, gauge, nullptr, nullptr, parity, scale, dagger ? 1 : 0, 0, 1, as_stream(stream));
 }
 
 int lqcd_clover_apply(lqcd_ctx* c, void* out, const void* in, const void* clover, int parity, void* stream) {
@@ -176,7 +181,7 @@ int lqcd_clover_apply(lqcd_ctx* c, void* out, const void* in, const void* clover
   if (!lqcd_aligned16(out) || !lqcd_aligned16(in) || !lqcd_aligned16(clover))
     return lqcd_set_error(c, LQCD_ERR_ALIGN, "clover_apply: alignment");
   const char* cl = (const char*)clover + (size_t)parity * (lqcd_clover_bytes(c) / 2);
-  return lqcd_clover_apply_launch(c, out, in, cl, as_stream(stream));
+  return lqcd_clover_apply_launch(c, out, in, cl, 1, as_stream(stream));
 }
 
 }  // extern "C"

@@ -1,0 +1,294 @@
+// Multi-right-hand-side dslash (the 12 spin-colour columns of
+// a propagator are 12 solves with the same links and clover).  Links are 67-75 % of the compulsory
+// bytes of a single-RHS dslash and are identical for every column, so this kernel loads each link
+// ONCE per site for NRHS spinors: bytes per site and column fall from (8R+48)w to (8R/NRHS+48)w.
+//
+// Field layout: NRHS consecutive one-parity native spinors, [rhs][NSV][Vh] vec16.
+// Thread layout: blockDim = (SITES, G).  threadIdx.x = site of the block (a warp = 32 consecutive
+// sites: coalesced 512 B rows), threadIdx.y = group of NB columns kept in registers (NB x 24
+// accumulators), NRHS = G * NB.  A thread loads a link once into registers and applies it to its NB
+// half-spinors; the G warps of a block that share the same sites read the same link rows, so only
+// the first touches L2/HBM and the others hit L1 (links are loaded with the L1-allocating path
+// here, unlike the streaming single-RHS kernel).  Epilogues are those of dslash.cu; the clover
+// block is loaded once per thread for its NB columns.
+#include "dslash.cuh"
+
+#ifndef MRHS_NB_F32
+#define MRHS_NB_F32 1
+#endif
+#ifndef MRHS_NB_F64
+#define MRHS_NB_F64 1
+#endif
+#ifndef MRHS_SITES
+#define MRHS_SITES 32
+#endif
+#ifndef MRHS_MINB_F32
+#define MRHS_MINB_F32 4
+#endif
+#ifndef MRHS_MINB_F64
+#define MRHS_MINB_F64 3
+#endif
+#ifndef MRHS_GMAX
+#define MRHS_GMAX 4                                  // column groups resident in one block
+#endif
+constexpr int MRHS_MAXT = MRHS_SITES * MRHS_GMAX;    // threads per block (register allocation bound)
+
+template <typename T> struct MrhsArgs {
+  T* out;
+  const T* in;
+  const T* gauge;
+  const T* cl;
+  const T* x;
+  Lat lat;
+  int parity;
+  T scale;
+  size_t stride;  // reals between consecutive right-hand sides (24 * Vh)
+  int ngroups;    // nrhs / NB column groups; group g is handled by threadIdx.y = g mod blockDim.y
+};
+
+template <typename T, int R>
+__device__ __forceinline__ void load_link_l1(const T* __restrict__ block, int Vh, int idx, T* U) {
+  typedef typename GV<T, R>::vec vec;
+  constexpr int N = GV<T, R>::N;
+  const vec* p = reinterpret_cast<const vec*>(block) + idx;
+#pragma unroll
+  for (int v = 0; v < R / N; v++) {
+    vec q = ld_cached(p + (size_t)v * Vh);
+    vec_get(q, U + v * N);
+  }
+  if (R == 12) {
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+      const int a = (c + 1) % 3, b = (c + 2) % 3;
+      T re = U[2 * a] * U[6 + 2 * b] - U[2 * a + 1] * U[6 + 2 * b + 1] - U[2 * b] * U[6 + 2 * a] +
+             U[2 * b + 1] * U[6 + 2 * a + 1];
+      T im = U[2 * a] * U[6 + 2 * b + 1] + U[2 * a + 1] * U[6 + 2 * b] - U[2 * b] * U[6 + 2 * a + 1] -
+             U[2 * b + 1] * U[6 + 2 * a];
+      U[12 + 2 * c] = re;
+      U[12 + 2 * c + 1] = -im;
+    }
+  }
+}
+
+template <typename T, int R, int MU, bool FWD, bool DAG, int NB>
+__device__ __forceinline__ void hop_mrhs(T (*acc)[24], const T* __restrict__ in, size_t stride,
+                                         const T* __restrict__ links, int Vh, int nidx, int lidx, T bsign,
+                                         bool seam) {
+  constexpr int S = (FWD != DAG) ? -1 : +1;
+  T U[18];
+  load_link_l1<T, R>(links, Vh, lidx, U);
+  if (MU == 3) {  // antiperiodic seam: flip the link once for all NB columns (after the row-3 rebuild)
+    const T sg = seam ? bsign : (T)1;
+#pragma unroll
+    for (int e = 0; e < 18; e++) U[e] *= sg;
+  }
+#pragma unroll
+  for (int r = 0; r < NB; r++) {
+    T psi[24], h[12], chi[12];
+    load_spinor<T>(in + r * stride, Vh, nidx, psi);
+    project<T, MU, S>(psi, h);
+    su3_mul<T, !FWD>(U, h, chi);
+    reconstruct<T, MU, S>(acc[r], chi);
+  }
+}
+
+// out[r] = C v[r] for NB vectors with one load of the clover block
+template <typename T, int NB>
+__device__ __forceinline__ void clover_mul_mrhs(const T* __restrict__ cl, int Vh, int idx, const T (*v)[24], T (*out)[24]) {
+  typedef typename V16<T>::vec vec;
+  constexpr int N = V16<T>::N;
+  const vec* p = reinterpret_cast<const vec*>(cl) + idx;
+#pragma unroll
+  for (int k = 0; k < 2; k++) {
+    T a[36];
+#pragma unroll
+    for (int q = 0; q < 36 / N; q++) {
+      vec w = ld_cached(p + (size_t)(k * (36 / N) + q) * Vh);
+      vec_get(w, a + q * N);
+    }
+#pragma unroll
+    for (int r = 0; r < NB; r++) {
+      const T* x = v[r] + 12 * k;
+      T* y = out[r] + 12 * k;
+#pragma unroll
+      for (int i = 0; i < 6; i++) {
+        T re = a[i] * x[2 * i], im = a[i] * x[2 * i + 1];
+#pragma unroll
+        for (int j = 0; j < 6; j++) {
+          if (j < i) {
+            const int o = 6 + 2 * (i * (i - 1) / 2 + j);
+            re += a[o] * x[2 * j] - a[o + 1] * x[2 * j + 1];
+            im += a[o] * x[2 * j + 1] + a[o + 1] * x[2 * j];
+          } else if (j > i) {
+            const int o = 6 + 2 * (j * (j - 1) / 2 + i);
+            re += a[o] * x[2 * j] + a[o + 1] * x[2 * j + 1];
+            im += a[o] * x[2 * j + 1] - a[o + 1] * x[2 * j];
+          }
+        }
+        y[2 * i] = re;
+        y[2 * i + 1] = im;
+      }
+    }
+  }
+}
+
+template <typename T> struct MrhsTune;
+template <> struct MrhsTune<float> { static constexpr int MINB = MRHS_MINB_F32, NB = MRHS_NB_F32; };
+template <> struct MrhsTune<double> { static constexpr int MINB = MRHS_MINB_F64, NB = MRHS_NB_F64; };
+
+template <typename T, int R, bool DAG, int EPI, int NB>
+__global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kernel(const MrhsArgs<T> a) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= a.lat.Vh) return;
+  const Lat& L = a.lat;
+  const int Vh = L.Vh, par = a.parity;
+  const size_t stride = a.stride;
+  const Site s = site_of(L, idx, par);
+  const size_t blk = (size_t)R * Vh;
+  for (int g = threadIdx.y; g < a.ngroups; g += blockDim.y) {
+  const size_t first = (size_t)g * NB * stride;  // first column of this thread's group
+  const T* in = a.in + first;
+  T acc[NB][24];
+#pragma unroll
+  for (int r = 0; r < NB; r++)
+#pragma unroll
+    for (int e = 0; e < 24; e++) acc[r][e] = 0;
+  const T one = 1;
+  const bool anti = L.tb < 0;
+  const bool seam_f = anti && s.t == L.Lt - 1, seam_b = anti && s.t == 0;
+  int n;
+  n = neighbour<0, +1>(L, idx, s);
+  hop_mrhs<T, R, 0, true, DAG, NB>(acc, in, stride, a.gauge + (0 * 2 + par) * blk, Vh, n, idx, one, false);
+  n = neighbour<0, -1>(L, idx, s);
+  hop_mrhs<T, R, 0, false, DAG, NB>(acc, in, stride, a.gauge + (0 * 2 + 1 - par) * blk, Vh, n, n, one, false);
+  n = neighbour<1, +1>(L, idx, s);
+  hop_mrhs<T, R, 1, true, DAG, NB>(acc, in, stride, a.gauge + (1 * 2 + par) * blk, Vh, n, idx, one, false);
+  n = neighbour<1, -1>(L, idx, s);
+  hop_mrhs<T, R, 1, false, DAG, NB>(acc, in, stride, a.gauge + (1 * 2 + 1 - par) * blk, Vh, n, n, one, false);
+  n = neighbour<2, +1>(L, idx, s);
+  hop_mrhs<T, R, 2, true, DAG, NB>(acc, in, stride, a.gauge + (2 * 2 + par) * blk, Vh, n, idx, one, false);
+  n = neighbour<2, -1>(L, idx, s);
+  hop_mrhs<T, R, 2, false, DAG, NB>(acc, in, stride, a.gauge + (2 * 2 + 1 - par) * blk, Vh, n, n, one, false);
+  n = neighbour<3, +1>(L, idx, s);
+  hop_mrhs<T, R, 3, true, DAG, NB>(acc, in, stride, a.gauge + (3 * 2 + par) * blk, Vh, n, idx, -one, seam_f);
+  n = neighbour<3, -1>(L, idx, s);
+  hop_mrhs<T, R, 3, false, DAG, NB>(acc, in, stride, a.gauge + (3 * 2 + 1 - par) * blk, Vh, n, n, -one, seam_b);
+
+  T* out = a.out + first;
+  if (EPI == 0) {
+#pragma unroll
+    for (int r = 0; r < NB; r++) {
+#pragma unroll
+      for (int e = 0; e < 24; e++) acc[r][e] *= a.scale;
+      store_spinor<T>(out + r * stride, Vh, idx, acc[r]);
+    }
+  } else if (EPI == 1) {
+    T res[NB][24];
+    clover_mul_mrhs<T, NB>(a.cl, Vh, idx, acc, res);
+#pragma unroll
+    for (int r = 0; r < NB; r++) {
+#pragma unroll
+      for (int e = 0; e < 24; e++) res[r][e] *= a.scale;
+      store_spinor<T>(out + r * stride, Vh, idx, res[r]);
+    }
+  } else if (EPI == 2) {
+    T xv[NB][24], res[NB][24];
+#pragma unroll
+    for (int r = 0; r < NB; r++) load_spinor<T>(a.x + first + r * stride, Vh, idx, xv[r]);
+    clover_mul_mrhs<T, NB>(a.cl, Vh, idx, xv, res);
+#pragma unroll
+    for (int r = 0; r < NB; r++) {
+#pragma unroll
+      for (int e = 0; e < 24; e++) res[r][e] += a.scale * acc[r][e];
+      store_spinor<T>(out + r * stride, Vh, idx, res[r]);
+    }
+  } else {
+    T res[NB][24];
+    clover_mul_mrhs<T, NB>(a.cl, Vh, idx, acc, res);
+#pragma unroll
+    for (int r = 0; r < NB; r++) {
+      T xv[24];
+      load_spinor<T>(a.x + first + r * stride, Vh, idx, xv);
+#pragma unroll
+      for (int e = 0; e < 24; e++) res[r][e] = xv[e] + a.scale * res[r][e];
+      store_spinor<T>(out + r * stride, Vh, idx, res[r]);
+    }
+  }
+  }  // column groups
+}
+
+template <typename T, int R, bool DAG, int NB>
+static void launch_mrhs_epi(MrhsArgs<T> a, int epi, int nrhs, cudaStream_t st) {
+  a.ngroups = nrhs / NB;
+  const dim3 block(MRHS_SITES, a.ngroups < MRHS_GMAX ? a.ngroups : MRHS_GMAX);
+  const int grid = (a.lat.Vh + MRHS_SITES - 1) / MRHS_SITES;
+  switch (epi) {
+    case 0: dslash_mrhs_kernel<T, R, DAG, 0, NB><<<grid, block, 0, st>>>(a); break;
+    case 1: dslash_mrhs_kernel<T, R, DAG, 1, NB><<<grid, block, 0, st>>>(a); break;
+    case 2: dslash_mrhs_kernel<T, R, DAG, 2, NB><<<grid, block, 0, st>>>(a); break;
+    default: dslash_mrhs_kernel<T, R, DAG, 3, NB><<<grid, block, 0, st>>>(a); break;
+  }
+}
+
+template <typename T, int R, bool DAG>
+static void launch_mrhs_nb(const MrhsArgs<T>& a, int epi, int nrhs, cudaStream_t st) {
+  // columns per thread: the tuned NB when it divides nrhs, else one per thread
+  if (nrhs % MrhsTune<T>::NB == 0) launch_mrhs_epi<T, R, DAG, MrhsTune<T>::NB>(a, epi, nrhs, st);
+  else launch_mrhs_epi<T, R, DAG, 1>(a, epi, nrhs, st);
+}
+
+template <typename T>
+static void launch_mrhs_typed(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
+                              int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st) {
+  MrhsArgs<T> a;
+  a.out = (T*)out;
+  a.in = (const T*)in;
+  a.gauge = (const T*)gauge;
+  a.cl = (const T*)cl;
+  a.x = (const T*)x;
+  a.lat = c->lat;
+  a.parity = parity;
+  a.scale = (T)scale;
+  a.stride = (size_t)24 * c->lat.Vh;
+  if (c->recon == 18) {
+    if (dagger) launch_mrhs_nb<T, 18, true>(a, epi, nrhs, st);
+    else launch_mrhs_nb<T, 18, false>(a, epi, nrhs, st);
+  } else {
+    if (dagger) launch_mrhs_nb<T, 12, true>(a, epi, nrhs, st);
+    else launch_mrhs_nb<T, 12, false>(a, epi, nrhs, st);
+  }
+}
+
+// internal entry (solvers and the C ABI): nrhs >= 2 consecutive one-parity native spinors in `in`,
+// `out` and (epilogues 2, 3) `x`.
+int lqcd_dslash_mrhs_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
+                            int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st) {
+  const double bytes = (double)c->lat.Vh * c->prec *
+                       (8.0 * c->recon + nrhs * 48.0 + (epi >= 1 ? 72.0 : 0.0) + (epi >= 2 ? nrhs * 24.0 : 0.0));
+  c->alg_bytes += bytes;
+  const bool rec = c->prof_on && c->prof_n < c->prof_cap;
+  if (rec) cudaEventRecord(c->prof_ev[2 * c->prof_n], st);
+  if (c->prec == 4) launch_mrhs_typed<float>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st);
+  else launch_mrhs_typed<double>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st);
+  if (rec) {
+    cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], st);
+    c->prof_n++;
+    c->prof_bytes += bytes;
+  }
+  LQCD_LAUNCH_CHECK(c, "dslash_mrhs");
+  return LQCD_OK;
+}
+
+extern "C" {
+
+int lqcd_dslash_mrhs(lqcd_ctx* c, void* out, const void* in, const void* gauge, int parity, double scale, int dagger,
+                     int nrhs, void* stream) {
+  if (!c || !out || !in || !gauge || (parity != 0 && parity != 1) || nrhs < 1 || nrhs > LQCD_MAX_RHS)
+    return LQCD_ERR_INVALID_ARG;
+  if (out == in) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "dslash_mrhs: out aliases in");
+  if (!lqcd_aligned16(out) || !lqcd_aligned16(in) || !lqcd_aligned16(gauge))
+    return lqcd_set_error(c, LQCD_ERR_ALIGN, "dslash_mrhs: alignment");
+  return lqcd_dslash_launch(c, out, in, gauge, nullptr, nullptr, parity, scale, dagger ? 1 : 0, 0, nrhs, as_stream(stream));
+}
+
+}  // extern "C"

@@ -30,11 +30,13 @@ struct lqcd_ctx {
   unsigned int* d_ticket;
   int* d_flag;
   double* h_scalars;
+  double* h_consts;  // pinned {0.0, 1.0}: sources of small asynchronous flag writes
   int* h_flag;
   int max_red_blocks;
   cudaEvent_t ev0, ev1;
   // accounting: algorithmic bytes of every launch; optional per-launch event timing of dslash
   double alg_bytes;
+  int acct_rhs;  // active right-hand sides of a batched solve (byte accounting of frozen columns)
   int prof_on, prof_n, prof_cap;
   cudaEvent_t* prof_ev;  // 2 events per recorded launch
   double prof_bytes;
@@ -175,7 +177,9 @@ static inline cudaStream_t as_stream(void* s) { return reinterpret_cast<cudaStre
 
 // internal launchers shared between translation units
 int lqcd_dslash_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
-                       int parity, double scale, int dagger, int epi, cudaStream_t st);
-int lqcd_clover_apply_launch(lqcd_ctx* c, void* out, const void* in, const void* cl_parity, cudaStream_t st);
+                       int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st);
+int lqcd_dslash_mrhs_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
+                            int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st);
+int lqcd_clover_apply_launch(lqcd_ctx* c, void* out, const void* in, const void* cl_parity, int nrhs, cudaStream_t st);
 int lqcd_spinor_pack_parity(lqcd_ctx* c, void* native, const void* pub, cudaStream_t st);
 int lqcd_spinor_unpack_parity(lqcd_ctx* c, void* pub, const void* native, cudaStream_t st);

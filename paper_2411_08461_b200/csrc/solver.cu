@@ -1,29 +1,43 @@
 // Operators M, Mhat and the Krylov solvers (§8(c) O7-O9;
-// PAPER.md:94 "BiCGStab for Wilson/clover and CG", PAPER.md:227-230 invert).
+// PAPER.md:94 "BiCGStab for Wilson/clover and CG", PAPER.md:227-230 invert), for nrhs >= 1
+// right-hand sides advanced in lock step.  Every "vector" below is a block
+// of nrhs consecutive one-parity native spinors; every right-hand side has its own scalar slots,
+// coefficients and stopping test.  nrhs = 1 is the single solve and runs the single-RHS kernels.
+#include <math.h>
 #include <string.h>
 #include "blas.cuh"
 
 static inline char* off(const void* p, size_t bytes) { return (char*)p + bytes; }
 
-// reduction slots in ctx->d_scalars
+// reduction slots of one right-hand side (SC_STRIDE doubles each) in ctx->d_scalars
 enum { S_BB = 0, S_RR0 = 2, S_RR1 = 3, S_TT = 4, S_RES = 5, S_RHO0 = 8, S_RHO1 = 10, S_R0V = 12, S_TS = 16, S_RR = 20, S_TRUE = 24 };
 
-#define BLAS_CALL(c, OPNAME, SETUP, vecs, outs, st)                       \
-  ((c)->prec == 4 ? [&]() { OPNAME<float> op; SETUP; return blas_launch<float, OPNAME<float>>((c), op, (vecs), (outs), (st)); }() \
-                  : [&]() { OPNAME<double> op; SETUP; return blas_launch<double, OPNAME<double>>((c), op, (vecs), (outs), (st)); }())
+#define BLAS_CALL(c, OPNAME, SETUP, vecs, outs, nrhs, rhs0, st)                       \
+  ((c)->prec == 4 ? [&]() { OPNAME<float> op; SETUP; return blas_launch<float, OPNAME<float>>((c), op, (vecs), (outs), (nrhs), (rhs0), (st)); }() \
+                  : [&]() { OPNAME<double> op; SETUP; return blas_launch<double, OPNAME<double>>((c), op, (vecs), (outs), (nrhs), (rhs0), (st)); }())
 
-static int read_scalars(lqcd_ctx* c, int first, int count, cudaStream_t st) {
-  cudaMemcpyAsync(c->h_scalars + first, c->d_scalars + first, sizeof(double) * count, cudaMemcpyDeviceToHost, st);
+// all slots of the first nrhs right-hand sides -> pinned host mirror; synchronises the stream
+static int read_scalars(lqcd_ctx* c, int nrhs, cudaStream_t st) {
+  cudaMemcpyAsync(c->h_scalars, c->d_scalars, sizeof(double) * SC_STRIDE * nrhs, cudaMemcpyDeviceToHost, st);
   if (cudaStreamSynchronize(st) != cudaSuccess) return lqcd_check_cuda(c, "scalar read-back");
   return LQCD_OK;
 }
+static inline double hs(const lqcd_ctx* c, int rhs, int slot) { return c->h_scalars[(size_t)rhs * SC_STRIDE + slot]; }
+// write 0.0 / 1.0 into one slot of one right-hand side, or of all of them (stream ordered)
+static void set_slot(lqcd_ctx* c, int rhs, int slot, bool one, cudaStream_t st) {
+  cudaMemcpyAsync(c->d_scalars + (size_t)rhs * SC_STRIDE + slot, c->h_consts + (one ? 1 : 0), sizeof(double),
+                  cudaMemcpyHostToDevice, st);
+}
+static void set_slot_all(lqcd_ctx* c, int nrhs, int slot, bool one, cudaStream_t st) {
+  for (int j = 0; j < nrhs; j++) set_slot(c, j, slot, one, st);
+}
 
-// Mhat (O8) on one-parity native spinors.  Two fused dslash launches:
+// Mhat (O8) on blocks of nrhs one-parity native spinors.  Two fused dslash launches:
 //   asym:       tmp = A_oo^-1 D_oe in ; out = A_ee in - k^2 D_eo tmp
 //   sym:        tmp = A_oo^-1 D_oe in ; out = in - k^2 A_ee^-1 D_eo tmp
 //   sym dagger: out(scratch) = A_ee^-1 in ; tmp = A_oo^-1 D^dag_oe out ; out = in - k^2 D^dag_eo tmp
 static int mpc_apply(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* clover,
-                     const void* clover_inv, double kappa, int matpc, int dagger, void* tmp, cudaStream_t st) {
+                     const void* clover_inv, double kappa, int matpc, int dagger, void* tmp, int nrhs, cudaStream_t st) {
   const size_t half = lqcd_clover_bytes(c) / 2;
   const void* A_e = clover;
   const void* Ai_e = clover_inv;
@@ -31,29 +45,28 @@ static int mpc_apply(lqcd_ctx* c, void* out, const void* in, const void* gauge, 
   const double k2 = -kappa * kappa;
   int rc;
   if (matpc == LQCD_MATPC_ASYMMETRIC) {
-    if ((rc = lqcd_dslash_launch(c, tmp, in, gauge, Ai_o, nullptr, 1, 1.0, dagger, 1, st))) return rc;
-    return lqcd_dslash_launch(c, out, tmp, gauge, A_e, in, 0, k2, dagger, 2, st);
+    if ((rc = lqcd_dslash_launch(c, tmp, in, gauge, Ai_o, nullptr, 1, 1.0, dagger, 1, nrhs, st))) return rc;
+    return lqcd_dslash_launch(c, out, tmp, gauge, A_e, in, 0, k2, dagger, 2, nrhs, st);
   }
   if (!dagger) {
-    if ((rc = lqcd_dslash_launch(c, tmp, in, gauge, Ai_o, nullptr, 1, 1.0, 0, 1, st))) return rc;
-    return lqcd_dslash_launch(c, out, tmp, gauge, Ai_e, in, 0, k2, 0, 3, st);
+    if ((rc = lqcd_dslash_launch(c, tmp, in, gauge, Ai_o, nullptr, 1, 1.0, 0, 1, nrhs, st))) return rc;
+    return lqcd_dslash_launch(c, out, tmp, gauge, Ai_e, in, 0, k2, 0, 3, nrhs, st);
   }
-  if ((rc = lqcd_clover_apply_launch(c, out, in, Ai_e, st))) return rc;
-  if ((rc = lqcd_dslash_launch(c, tmp, out, gauge, Ai_o, nullptr, 1, 1.0, 1, 1, st))) return rc;
-  // out = in + k2 * D^dag_eo tmp : epilogue 2 with C = identity is not available, so use the
-  // plain dslash into `out` followed by an xpay
-  if ((rc = lqcd_dslash_launch(c, out, tmp, gauge, nullptr, nullptr, 0, k2, 1, 0, st))) return rc;
+  if ((rc = lqcd_clover_apply_launch(c, out, in, Ai_e, nrhs, st))) return rc;
+  if ((rc = lqcd_dslash_launch(c, tmp, out, gauge, Ai_o, nullptr, 1, 1.0, 1, 1, nrhs, st))) return rc;
+  // out = in + k2 * D^dag_eo tmp : plain dslash into `out` followed by an xpay
+  if ((rc = lqcd_dslash_launch(c, out, tmp, gauge, nullptr, nullptr, 0, k2, 1, 0, nrhs, st))) return rc;
   void* v[2] = {(void*)in, out};
-  return BLAS_CALL(c, OpXpay, op.a = 1.0, v, nullptr, st);  // out = in + 1*out
+  return BLAS_CALL(c, OpXpay, op.a = 1.0, v, nullptr, nrhs, 0, st);  // out = in + 1*out
 }
 
-// full M (O7): out_p = A_pp in_p - kappa D_{p,1-p} in_{1-p}
+// full M (O7): out_p = A_pp in_p - kappa D_{p,1-p} in_{1-p}; fields are [parity][nrhs][one-parity]
 static int mat_apply(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* clover, double kappa,
-                     int dagger, cudaStream_t st) {
-  const size_t sp = lqcd_spinor_bytes(c), half = lqcd_clover_bytes(c) / 2;
+                     int dagger, int nrhs, cudaStream_t st) {
+  const size_t blk = lqcd_spinor_bytes(c) * nrhs, half = lqcd_clover_bytes(c) / 2;
   int rc;
-  if ((rc = lqcd_dslash_launch(c, out, off(in, sp), gauge, clover, in, 0, -kappa, dagger, 2, st))) return rc;
-  return lqcd_dslash_launch(c, off(out, sp), in, gauge, off(clover, half), off(in, sp), 1, -kappa, dagger, 2, st);
+  if ((rc = lqcd_dslash_launch(c, out, off(in, blk), gauge, clover, in, 0, -kappa, dagger, 2, nrhs, st))) return rc;
+  return lqcd_dslash_launch(c, off(out, blk), in, gauge, off(clover, half), off(in, blk), 1, -kappa, dagger, 2, nrhs, st);
 }
 
 static bool check_ptrs(lqcd_ctx* c, const void* const* p, int n, const char* what) {
@@ -67,14 +80,20 @@ static bool check_ptrs(lqcd_ctx* c, const void* const* p, int n, const char* wha
 
 extern "C" {
 
-int lqcd_mpc_apply(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* clover,
-                   const void* clover_inv, double kappa, int matpc, int dagger, void* tmp, void* stream) {
-  if (!c || !out || !in || !gauge || !clover || !clover_inv || !tmp || (matpc != 0 && matpc != 1))
+int lqcd_mpc_apply_mrhs(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* clover,
+                        const void* clover_inv, double kappa, int matpc, int dagger, void* tmp, int nrhs, void* stream) {
+  if (!c || !out || !in || !gauge || !clover || !clover_inv || !tmp || (matpc != 0 && matpc != 1) || nrhs < 1 ||
+      nrhs > LQCD_MAX_RHS)
     return LQCD_ERR_INVALID_ARG;
   if (out == in || tmp == in || tmp == out) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "mpc_apply: aliasing");
   const void* p[6] = {out, in, gauge, clover, clover_inv, tmp};
   if (!check_ptrs(c, p, 6, "mpc_apply")) return LQCD_ERR_ALIGN;
-  return mpc_apply(c, out, in, gauge, clover, clover_inv, kappa, matpc, dagger ? 1 : 0, tmp, as_stream(stream));
+  return mpc_apply(c, out, in, gauge, clover, clover_inv, kappa, matpc, dagger ? 1 : 0, tmp, nrhs, as_stream(stream));
+}
+
+int lqcd_mpc_apply(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* clover,
+                   const void* clover_inv, double kappa, int matpc, int dagger, void* tmp, void* stream) {
+  return lqcd_mpc_apply_mrhs(c, out, in, gauge, clover, clover_inv, kappa, matpc, dagger, tmp, 1, stream);
 }
 
 int lqcd_mat_apply(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* clover, double kappa,
@@ -83,161 +102,207 @@ int lqcd_mat_apply(lqcd_ctx* c, void* out, const void* in, const void* gauge, co
   if (out == in) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "mat_apply: out aliases in");
   const void* p[4] = {out, in, gauge, clover};
   if (!check_ptrs(c, p, 4, "mat_apply")) return LQCD_ERR_ALIGN;
-  return mat_apply(c, out, in, gauge, clover, kappa, dagger ? 1 : 0, as_stream(stream));
+  return mat_apply(c, out, in, gauge, clover, kappa, dagger ? 1 : 0, 1, as_stream(stream));
 }
 
-// workspace: up to 9 one-parity spinors + 2 two-parity spinors (+ clover pair when built inside)
-size_t lqcd_invert_workspace_bytes(const lqcd_ctx* c, int solver) {
+// workspace: nrhs x (2 two-parity + 9 one-parity spinors) (+ clover pair when built inside)
+size_t lqcd_invert_multi_workspace_bytes(const lqcd_ctx* c, int solver, int nrhs) {
   (void)solver;
-  if (!c) return 0;
-  return 13 * lqcd_spinor_bytes(c) + 2 * lqcd_clover_bytes(c);
+  if (!c || nrhs < 1) return 0;
+  return (size_t)nrhs * 13 * lqcd_spinor_bytes(c) + 2 * lqcd_clover_bytes(c);
 }
+size_t lqcd_invert_workspace_bytes(const lqcd_ctx* c, int solver) { return lqcd_invert_multi_workspace_bytes(c, solver, 1); }
 
 }  // extern "C"
 
 struct Work {
-  char* b;      // two-parity native source
-  char* x;      // two-parity native solution
-  char* v[9];   // one-parity scratch spinors
+  int nrhs;
+  char* b;      // source, [parity][nrhs][one-parity native]
+  char* x;      // solution, same layout
+  char* v[9];   // scratch blocks of nrhs one-parity spinors
   char* clover; // optional
   char* clover_inv;
 };
 
+// per-right-hand-side bookkeeping of a batched solve (host)
+struct Cols {
+  int n;
+  bool active[LQCD_MAX_RHS];
+  double stop2[LQCD_MAX_RHS], bb[LQCD_MAX_RHS], rr[LQCD_MAX_RHS];
+  int nactive() const { int k = 0; for (int j = 0; j < n; j++) k += active[j]; return k; }
+};
+// freeze column j: its BLAS blocks exit from now on, so x_j, r_j keep the values of this iteration
+static void freeze(lqcd_ctx* c, Cols& cols, int j, cudaStream_t st) {
+  cols.active[j] = false;
+  set_slot(c, j, S_DONE, true, st);
+  c->acct_rhs = cols.nactive();
+}
+
 static int solve_cg(lqcd_ctx* c, const Work& w, const void* gauge, const void* A, const void* Ai, double kappa,
-                    int matpc, int normal_residual, double stop2, int maxiter, lqcd_result* res, cudaStream_t st) {
+                    int matpc, int normal_residual, Cols& cols, int maxiter, lqcd_result* res, cudaStream_t st) {
   // CGNE (normal_residual = 0): Mhat Mhat^dag y = bhat, x = Mhat^dag y.   bhat in v[0], x_e in w.x
   // CGNR (normal_residual = 1): Mhat^dag Mhat x = Mhat^dag bhat; `resv` tracks bhat - Mhat x
   char *r = w.v[1], *p = w.v[2], *t = w.v[3], *q = w.v[4], *tmp = w.v[5], *resv = w.v[6];
-  const size_t sp = lqcd_spinor_bytes(c);
+  const int n = w.nrhs;
+  const size_t blk = lqcd_spinor_bytes(c) * n;
   char* x = w.x;
   int rc;
-  cudaMemsetAsync(x, 0, sp, st);
+  long dslashes = 0;
+  cudaMemsetAsync(x, 0, blk, st);
   if (!normal_residual) {
-    cudaMemcpyAsync(r, w.v[0], sp, cudaMemcpyDeviceToDevice, st);
+    cudaMemcpyAsync(r, w.v[0], blk, cudaMemcpyDeviceToDevice, st);
   } else {
-    cudaMemcpyAsync(resv, w.v[0], sp, cudaMemcpyDeviceToDevice, st);
-    if ((rc = mpc_apply(c, r, resv, gauge, A, Ai, kappa, matpc, 1, tmp, st))) return rc;
-    res->dslash_count += 2;
+    cudaMemcpyAsync(resv, w.v[0], blk, cudaMemcpyDeviceToDevice, st);
+    if ((rc = mpc_apply(c, r, resv, gauge, A, Ai, kappa, matpc, 1, tmp, n, st))) return rc;
+    dslashes += 2;
   }
-  cudaMemcpyAsync(p, r, sp, cudaMemcpyDeviceToDevice, st);
+  cudaMemcpyAsync(p, r, blk, cudaMemcpyDeviceToDevice, st);
   {
     void* v[1] = {r};
     int outs[4] = {S_RR0, 0, 0, 0};
-    if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v, outs, st))) return rc;
+    if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v, outs, n, 0, st))) return rc;
     void* v2[1] = {normal_residual ? resv : r};
     int outs2[4] = {S_RES, 0, 0, 0};
-    if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v2, outs2, st))) return rc;
+    if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v2, outs2, n, 0, st))) return rc;
   }
-  if ((rc = read_scalars(c, S_RES, 1, st))) return rc;
-  double resn = c->h_scalars[S_RES];
+  if ((rc = read_scalars(c, n, st))) return rc;
+  for (int j = 0; j < n; j++) {
+    if (!cols.active[j]) continue;
+    cols.rr[j] = hs(c, j, S_RES);
+    if (!(cols.rr[j] > cols.stop2[j])) freeze(c, cols, j, st);
+  }
   int it = 0;
-  while (it < maxiter && resn > stop2) {
+  while (it < maxiter && cols.nactive() > 0) {
     const int cur = (it & 1) ? S_RR1 : S_RR0, nxt = (it & 1) ? S_RR0 : S_RR1;
     int outs[4] = {S_TT, 0, 0, 0};
     if (!normal_residual) {
-      if ((rc = mpc_apply(c, t, p, gauge, A, Ai, kappa, matpc, 1, tmp, st))) return rc;   // t = Mhat^dag p
+      if ((rc = mpc_apply(c, t, p, gauge, A, Ai, kappa, matpc, 1, tmp, n, st))) return rc;   // t = Mhat^dag p
       void* v[1] = {t};
-      if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v, outs, st))) return rc;                 // <p, Mhat Mhat^dag p>
-      if ((rc = mpc_apply(c, q, t, gauge, A, Ai, kappa, matpc, 0, tmp, st))) return rc;   // q = Mhat t
+      if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v, outs, n, 0, st))) return rc;              // <p, Mhat Mhat^dag p>
+      if ((rc = mpc_apply(c, q, t, gauge, A, Ai, kappa, matpc, 0, tmp, n, st))) return rc;   // q = Mhat t
       void* u[4] = {x, t, r, q};
       int o2[4] = {nxt, 0, 0, 0};
-      if ((rc = BLAS_CALL(c, OpCgUpdate, (op.num = cur, op.den = S_TT), u, o2, st))) return rc;  // x += a t ; r -= a q
+      if ((rc = BLAS_CALL(c, OpCgUpdate, (op.num = cur, op.den = S_TT), u, o2, n, 0, st))) return rc;  // x += a t ; r -= a q
     } else {
-      if ((rc = mpc_apply(c, t, p, gauge, A, Ai, kappa, matpc, 0, tmp, st))) return rc;   // t = Mhat p
+      if ((rc = mpc_apply(c, t, p, gauge, A, Ai, kappa, matpc, 0, tmp, n, st))) return rc;   // t = Mhat p
       void* v[1] = {t};
-      if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v, outs, st))) return rc;
+      if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v, outs, n, 0, st))) return rc;
       void* u[4] = {x, p, resv, t};
       int o2[4] = {S_RES, 0, 0, 0};
-      if ((rc = BLAS_CALL(c, OpCgUpdate, (op.num = cur, op.den = S_TT), u, o2, st))) return rc;  // x += a p ; res -= a t
-      if ((rc = mpc_apply(c, q, t, gauge, A, Ai, kappa, matpc, 1, tmp, st))) return rc;   // q = Mhat^dag t
+      if ((rc = BLAS_CALL(c, OpCgUpdate, (op.num = cur, op.den = S_TT), u, o2, n, 0, st))) return rc;  // x += a p ; res -= a t
+      if ((rc = mpc_apply(c, q, t, gauge, A, Ai, kappa, matpc, 1, tmp, n, st))) return rc;   // q = Mhat^dag t
       void* u2[2] = {r, q};
       int o3[4] = {nxt, 0, 0, 0};
-      if ((rc = BLAS_CALL(c, OpAxmyNormRatio, (op.num = cur, op.den = S_TT), u2, o3, st))) return rc;
+      if ((rc = BLAS_CALL(c, OpAxmyNormRatio, (op.num = cur, op.den = S_TT), u2, o3, n, 0, st))) return rc;
     }
-    res->dslash_count += 4;
+    dslashes += 4;
     void* u3[2] = {p, r};
-    if ((rc = BLAS_CALL(c, OpXpayRatio, (op.num = nxt, op.den = cur), u3, nullptr, st))) return rc;  // p = r + beta p
+    if ((rc = BLAS_CALL(c, OpXpayRatio, (op.num = nxt, op.den = cur), u3, nullptr, n, 0, st))) return rc;  // p = r + beta p
     it++;
-    if ((rc = read_scalars(c, S_RR0, 4, st))) return rc;
-    resn = normal_residual ? c->h_scalars[S_RES] : c->h_scalars[nxt];
-    if (!(resn == resn)) { res->status = LQCD_ERR_BREAKDOWN; break; }
+    if ((rc = read_scalars(c, n, st))) return rc;
+    for (int j = 0; j < n; j++) {
+      if (!cols.active[j]) continue;
+      const double resn = normal_residual ? hs(c, j, S_RES) : hs(c, j, nxt);
+      cols.rr[j] = resn;
+      res[j].iterations = it;
+      if (!(resn == resn)) { res[j].status = LQCD_ERR_BREAKDOWN; freeze(c, cols, j, st); }
+      else if (!(resn > cols.stop2[j])) freeze(c, cols, j, st);
+    }
   }
-  res->iterations = it;
-  res->iter_resid = resn;  // squared, normalised by the caller
+  for (int j = 0; j < n; j++) res[j].dslash_count += dslashes;
   return LQCD_OK;
 }
 
 static int solve_bicgstab(lqcd_ctx* c, const Work& w, const void* gauge, const void* A, const void* Ai, double kappa,
-                          int matpc, double stop2, int maxiter, lqcd_result* res, cudaStream_t st) {
+                          int matpc, Cols& cols, int maxiter, lqcd_result* res, cudaStream_t st) {
   char *r = w.v[1], *r0 = w.v[2], *p = w.v[3], *v = w.v[4], *s = w.v[6], *t = w.v[7], *tmp = w.v[5];
-  const size_t sp = lqcd_spinor_bytes(c);
+  const int n = w.nrhs;
+  const size_t sp = lqcd_spinor_bytes(c), blk = sp * n;
   char* x = w.x;
   int rc;
-  cudaMemsetAsync(x, 0, sp, st);
-  cudaMemcpyAsync(r, w.v[0], sp, cudaMemcpyDeviceToDevice, st);
-  cudaMemcpyAsync(r0, w.v[0], sp, cudaMemcpyDeviceToDevice, st);
+  long dslashes = 0;
+  bool restarted[LQCD_MAX_RHS] = {false};
+  cudaMemsetAsync(x, 0, blk, st);
+  cudaMemcpyAsync(r, w.v[0], blk, cudaMemcpyDeviceToDevice, st);
+  cudaMemcpyAsync(r0, w.v[0], blk, cudaMemcpyDeviceToDevice, st);
   {
     // rho_0 = <r0,r> = |r|^2
     void* u[2] = {r0, r};
     int outs[4] = {S_RHO0, S_RHO0 + 1, S_RR, 0};
-    if ((rc = BLAS_CALL(c, OpCdot, (void)op, u, outs, st))) return rc;
+    if ((rc = BLAS_CALL(c, OpCdot, (void)op, u, outs, n, 0, st))) return rc;
   }
-  if ((rc = read_scalars(c, S_RR, 1, st))) return rc;
-  double rr = c->h_scalars[S_RR];
-  int it = 0, first = 1, restarted = 0;
-  while (it < maxiter && rr > stop2) {
+  set_slot_all(c, n, S_FIRST, true, st);  // first iteration: p = r (p, v hold garbage)
+  bool first_pending = true;
+  if ((rc = read_scalars(c, n, st))) return rc;
+  for (int j = 0; j < n; j++) {
+    if (!cols.active[j]) continue;
+    cols.rr[j] = hs(c, j, S_RR);
+    if (!(cols.rr[j] > cols.stop2[j])) freeze(c, cols, j, st);
+  }
+  int it = 0;
+  while (it < maxiter && cols.nactive() > 0) {
     const int rho = (it & 1) ? S_RHO1 : S_RHO0, rho_next = (it & 1) ? S_RHO0 : S_RHO1;
     {
       void* u[3] = {p, r, v};
-      if ((rc = BLAS_CALL(c, OpBicgP, (op.rho = rho, op.r0v = S_R0V, op.ts = S_TS, op.first = first), u, nullptr, st))) return rc;
+      if ((rc = BLAS_CALL(c, OpBicgP, (op.rho = rho, op.r0v = S_R0V, op.ts = S_TS), u, nullptr, n, 0, st))) return rc;
     }
-    first = 0;
-    if ((rc = mpc_apply(c, v, p, gauge, A, Ai, kappa, matpc, 0, tmp, st))) return rc;   // v = Mhat p
+    if (first_pending) {
+      set_slot_all(c, n, S_FIRST, false, st);
+      first_pending = false;
+    }
+    if ((rc = mpc_apply(c, v, p, gauge, A, Ai, kappa, matpc, 0, tmp, n, st))) return rc;   // v = Mhat p
     {
       void* u[2] = {r0, v};
       int outs[4] = {S_R0V, S_R0V + 1, S_R0V + 2, 0};
-      if ((rc = BLAS_CALL(c, OpCdot, (void)op, u, outs, st))) return rc;
+      if ((rc = BLAS_CALL(c, OpCdot, (void)op, u, outs, n, 0, st))) return rc;
       void* u2[3] = {s, r, v};
-      if ((rc = BLAS_CALL(c, OpBicgS, (op.rho = rho, op.r0v = S_R0V), u2, nullptr, st))) return rc;
+      if ((rc = BLAS_CALL(c, OpBicgS, (op.rho = rho, op.r0v = S_R0V), u2, nullptr, n, 0, st))) return rc;
     }
-    if ((rc = mpc_apply(c, t, s, gauge, A, Ai, kappa, matpc, 0, tmp, st))) return rc;   // t = Mhat s
+    if ((rc = mpc_apply(c, t, s, gauge, A, Ai, kappa, matpc, 0, tmp, n, st))) return rc;   // t = Mhat s
     {
       void* u[2] = {t, s};
       int outs[4] = {S_TS, S_TS + 1, S_TS + 2, 0};
-      if ((rc = BLAS_CALL(c, OpCdot, (void)op, u, outs, st))) return rc;                // <t,s>, |t|^2
+      if ((rc = BLAS_CALL(c, OpCdot, (void)op, u, outs, n, 0, st))) return rc;             // <t,s>, |t|^2
       void* u2[6] = {x, r, p, s, t, r0};
       int o2[4] = {S_RR, rho_next, rho_next + 1, 0};
-      if ((rc = BLAS_CALL(c, OpBicgXR, (op.rho = rho, op.r0v = S_R0V, op.ts = S_TS), u2, o2, st))) return rc;
+      if ((rc = BLAS_CALL(c, OpBicgXR, (op.rho = rho, op.r0v = S_R0V, op.ts = S_TS), u2, o2, n, 0, st))) return rc;
     }
-    res->dslash_count += 4;
+    dslashes += 4;
     it++;
-    if ((rc = read_scalars(c, S_RHO0, 16, st))) return rc;
-    rr = c->h_scalars[S_RR];
-    const double* h = c->h_scalars;
-    const double rho_mag = h[rho_next] * h[rho_next] + h[rho_next + 1] * h[rho_next + 1];
-    const double om_mag = (h[S_TS] * h[S_TS] + h[S_TS + 1] * h[S_TS + 1]);
-    if (!(rr == rr) || ((rho_mag < 1e-300 || om_mag < 1e-300) && rr > stop2)) {
-      if (restarted || !(rr == rr)) { res->status = LQCD_ERR_BREAKDOWN; break; }
-      // one restart with r0 = r (O9)
-      restarted = 1;
-      first = 1;
-      cudaMemcpyAsync(r0, r, sp, cudaMemcpyDeviceToDevice, st);
-      void* u[2] = {r0, r};
-      int outs[4] = {rho_next, rho_next + 1, S_RR, 0};
-      if ((rc = BLAS_CALL(c, OpCdot, (void)op, u, outs, st))) return rc;
+    if ((rc = read_scalars(c, n, st))) return rc;
+    for (int j = 0; j < n; j++) {
+      if (!cols.active[j]) continue;
+      const double rr = hs(c, j, S_RR);
+      cols.rr[j] = rr;
+      res[j].iterations = it;
+      const double rho_mag = hs(c, j, rho_next) * hs(c, j, rho_next) + hs(c, j, rho_next + 1) * hs(c, j, rho_next + 1);
+      const double om_mag = hs(c, j, S_TS) * hs(c, j, S_TS) + hs(c, j, S_TS + 1) * hs(c, j, S_TS + 1);
+      if (!(rr == rr)) { res[j].status = LQCD_ERR_BREAKDOWN; freeze(c, cols, j, st); continue; }
+      if (!(rr > cols.stop2[j])) { freeze(c, cols, j, st); continue; }
+      if (rho_mag < 1e-300 || om_mag < 1e-300) {
+        if (restarted[j]) { res[j].status = LQCD_ERR_BREAKDOWN; freeze(c, cols, j, st); continue; }
+        // one restart with r0 = r (O9), for this column only; the slots the next iteration reads as rho
+        restarted[j] = true;
+        set_slot(c, j, S_FIRST, true, st);
+        first_pending = true;
+        cudaMemcpyAsync(r0 + (size_t)j * sp, r + (size_t)j * sp, sp, cudaMemcpyDeviceToDevice, st);
+        void* u[2] = {r0, r};
+        int outs[4] = {rho_next, rho_next + 1, S_RR, 0};
+        if ((rc = BLAS_CALL(c, OpCdot, (void)op, u, outs, 1, j, st))) return rc;
+      }
     }
   }
-  res->iterations = it;
-  res->iter_resid = rr;
+  for (int j = 0; j < n; j++) res[j].dslash_count += dslashes;
   return LQCD_OK;
 }
 
-static void carve(lqcd_ctx* c, void* workspace, Work& w, bool with_clover) {
-  const size_t sp = lqcd_spinor_bytes(c);
+static void carve(lqcd_ctx* c, void* workspace, Work& w, int nrhs, bool with_clover) {
+  const size_t blk = lqcd_spinor_bytes(c) * nrhs;
   char* p = (char*)workspace;
-  w.b = p; p += 2 * sp;
-  w.x = p; p += 2 * sp;
-  for (int i = 0; i < 9; i++) { w.v[i] = p; p += sp; }
+  w.nrhs = nrhs;
+  w.b = p; p += 2 * blk;
+  w.x = p; p += 2 * blk;
+  for (int i = 0; i < 9; i++) { w.v[i] = p; p += blk; }
   w.clover = with_clover ? p : nullptr;
   w.clover_inv = with_clover ? p + lqcd_clover_bytes(c) : nullptr;
 }
@@ -245,85 +310,108 @@ static void carve(lqcd_ctx* c, void* workspace, Work& w, bool with_clover) {
 // the whole solve on native fields already in w.b; result in w.x (both parities)
 static int invert_native(lqcd_ctx* c, Work& w, const void* gauge, const void* A, const void* Ai, double kappa,
                          double tol, int maxiter, int solver, int matpc, lqcd_result* res, cudaStream_t st) {
-  const size_t sp = lqcd_spinor_bytes(c), half = lqcd_clover_bytes(c) / 2;
+  const int n = w.nrhs;
+  const size_t blk = lqcd_spinor_bytes(c) * n, half = lqcd_clover_bytes(c) / 2;
   const void* Ai_e = Ai;
   const void* Ai_o = off(Ai, half);
-  char *b_e = w.b, *b_o = w.b + sp, *x_e = w.x, *x_o = w.x + sp;
+  char *b_e = w.b, *b_o = w.b + blk, *x_e = w.x, *x_o = w.x + blk;
   int rc;
+  cudaMemsetAsync(c->d_scalars, 0, sizeof(double) * SC_STRIDE * n, st);  // clears S_DONE / S_FIRST too
+  c->acct_rhs = 0;
   // |b|^2 over both parities
   {
     void* v[1] = {b_e};
     int o[4] = {S_BB, 0, 0, 0};
-    if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v, o, st))) return rc;
+    if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v, o, n, 0, st))) return rc;
     void* v2[1] = {b_o};
     int o2[4] = {S_BB + 1, 0, 0, 0};
-    if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v2, o2, st))) return rc;
+    if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v2, o2, n, 0, st))) return rc;
   }
-  if ((rc = read_scalars(c, S_BB, 2, st))) return rc;
-  const double bb = c->h_scalars[S_BB] + c->h_scalars[S_BB + 1];
-  if (bb == 0.0) {
-    cudaMemsetAsync(w.x, 0, 2 * sp, st);
-    res->status = LQCD_OK;
-    return LQCD_OK;
+  if ((rc = read_scalars(c, n, st))) return rc;
+  Cols cols;
+  cols.n = n;
+  for (int j = 0; j < n; j++) {
+    cols.bb[j] = hs(c, j, S_BB) + hs(c, j, S_BB + 1);
+    cols.stop2[j] = tol * tol * cols.bb[j];
+    cols.rr[j] = 0;
+    cols.active[j] = cols.bb[j] > 0.0;  // a zero source has the zero solution: nothing to iterate
+    res[j].status = LQCD_OK;
   }
-  // a5: bhat = b_e + kappa D_eo A_oo^-1 b_o   (sym: bhat_s = A_ee^-1 bhat)
-  char* bh = w.v[0];
-  if ((rc = lqcd_clover_apply_launch(c, w.v[5], b_o, Ai_o, st))) return rc;
-  if ((rc = lqcd_dslash_launch(c, bh, w.v[5], gauge, nullptr, nullptr, 0, kappa, 0, 0, st))) return rc;
-  res->dslash_count += 1;
-  {
-    void* v[2] = {b_e, bh};
-    if ((rc = BLAS_CALL(c, OpXpay, op.a = 1.0, v, nullptr, st))) return rc;
+  cudaMemsetAsync(w.x, 0, 2 * blk, st);
+  if (cols.nactive() > 0) {
+    // a5: bhat = b_e + kappa D_eo A_oo^-1 b_o   (sym: bhat_s = A_ee^-1 bhat)
+    char* bh = w.v[0];
+    if ((rc = lqcd_clover_apply_launch(c, w.v[5], b_o, Ai_o, n, st))) return rc;
+    if ((rc = lqcd_dslash_launch(c, bh, w.v[5], gauge, nullptr, nullptr, 0, kappa, 0, 0, n, st))) return rc;
+    {
+      void* v[2] = {b_e, bh};
+      if ((rc = BLAS_CALL(c, OpXpay, op.a = 1.0, v, nullptr, n, 0, st))) return rc;
+    }
+    if (matpc == LQCD_MATPC_SYMMETRIC)
+      if ((rc = lqcd_clover_apply_launch(c, bh, bh, Ai_e, n, st))) return rc;
+    for (int j = 0; j < n; j++)
+      if (!cols.active[j]) set_slot(c, j, S_DONE, true, st);
+    c->acct_rhs = cols.nactive();
+    if (solver == LQCD_SOLVER_BICGSTAB) rc = solve_bicgstab(c, w, gauge, A, Ai, kappa, matpc, cols, maxiter, res, st);
+    else rc = solve_cg(c, w, gauge, A, Ai, kappa, matpc, solver == LQCD_SOLVER_CGNR, cols, maxiter, res, st);
+    c->acct_rhs = 0;
+    if (rc) return rc;
+    set_slot_all(c, n, S_DONE, false, st);  // the closing steps below update every column
+    // a10: x_o = A_oo^-1 (b_o + kappa D_oe x_e)
+    if ((rc = lqcd_dslash_launch(c, w.v[5], x_e, gauge, nullptr, nullptr, 1, kappa, 0, 0, n, st))) return rc;
+    {
+      void* v[2] = {b_o, w.v[5]};
+      if ((rc = BLAS_CALL(c, OpXpay, op.a = 1.0, v, nullptr, n, 0, st))) return rc;
+    }
+    if ((rc = lqcd_clover_apply_launch(c, x_o, w.v[5], Ai_o, n, st))) return rc;
+    // a11: true residual |b - M x| / |b| with the full operator; v[1], v[2] are adjacent blocks
+    if ((rc = mat_apply(c, w.v[1], w.x, gauge, A, kappa, 0, n, st))) return rc;
+    {
+      void* v[2] = {b_e, w.v[1]};
+      int o[4] = {S_TRUE, 0, 0, 0};
+      if ((rc = BLAS_CALL(c, OpAxpyNorm, op.a = -1.0, v, o, n, 0, st))) return rc;
+      void* v2[2] = {b_o, w.v[2]};
+      int o2[4] = {S_TRUE + 1, 0, 0, 0};
+      if ((rc = BLAS_CALL(c, OpAxpyNorm, op.a = -1.0, v2, o2, n, 0, st))) return rc;
+    }
+    if ((rc = read_scalars(c, n, st))) return rc;
   }
-  if (matpc == LQCD_MATPC_SYMMETRIC)
-    if ((rc = lqcd_clover_apply_launch(c, bh, bh, Ai_e, st))) return rc;
-  const double stop2 = tol * tol * bb;
-  res->status = LQCD_OK;
-  if (solver == LQCD_SOLVER_BICGSTAB) rc = solve_bicgstab(c, w, gauge, A, Ai, kappa, matpc, stop2, maxiter, res, st);
-  else rc = solve_cg(c, w, gauge, A, Ai, kappa, matpc, solver == LQCD_SOLVER_CGNR, stop2, maxiter, res, st);
-  if (rc) return rc;
-  const double rr = res->iter_resid;
-  res->iter_resid = sqrt(rr / bb);
-  if (res->status == LQCD_OK && rr > stop2) res->status = LQCD_NOT_CONVERGED;
-  // a10: x_o = A_oo^-1 (b_o + kappa D_oe x_e)
-  if ((rc = lqcd_dslash_launch(c, w.v[5], x_e, gauge, nullptr, nullptr, 1, kappa, 0, 0, st))) return rc;
-  res->dslash_count += 1;
-  {
-    void* v[2] = {b_o, w.v[5]};
-    if ((rc = BLAS_CALL(c, OpXpay, op.a = 1.0, v, nullptr, st))) return rc;
+  for (int j = 0; j < n; j++) {
+    if (!(cols.bb[j] > 0.0)) continue;
+    res[j].dslash_count += 4;  // prepare, reconstruct, two for the true residual
+    res[j].iter_resid = sqrt(cols.rr[j] / cols.bb[j]);
+    if (res[j].status == LQCD_OK && cols.rr[j] > cols.stop2[j]) res[j].status = LQCD_NOT_CONVERGED;
+    res[j].true_resid = sqrt((hs(c, j, S_TRUE) + hs(c, j, S_TRUE + 1)) / cols.bb[j]);
   }
-  if ((rc = lqcd_clover_apply_launch(c, x_o, w.v[5], Ai_o, st))) return rc;
-  // a11: true residual |b - M x| / |b| with the full operator; v[1], v[2] are adjacent
-  if ((rc = mat_apply(c, w.v[1], w.x, gauge, A, kappa, 0, st))) return rc;
-  res->dslash_count += 2;
-  {
-    void* v[2] = {b_e, w.v[1]};
-    int o[4] = {S_TRUE, 0, 0, 0};
-    if ((rc = BLAS_CALL(c, OpAxpyNorm, op.a = -1.0, v, o, st))) return rc;
-    void* v2[2] = {b_o, w.v[2]};
-    int o2[4] = {S_TRUE + 1, 0, 0, 0};
-    if ((rc = BLAS_CALL(c, OpAxpyNorm, op.a = -1.0, v2, o2, st))) return rc;
-  }
-  if ((rc = read_scalars(c, S_TRUE, 2, st))) return rc;
-  res->true_resid = sqrt((c->h_scalars[S_TRUE] + c->h_scalars[S_TRUE + 1]) / bb);
   return LQCD_OK;
+}
+
+static int worst_status(const lqcd_result* res, int n) {
+  int worst = LQCD_OK;
+  for (int j = 0; j < n; j++) {
+    if (res[j].status < 0) worst = (worst < 0 && worst < res[j].status) ? worst : res[j].status;
+    else if (res[j].status > 0 && worst == LQCD_OK) worst = res[j].status;
+  }
+  return worst;
 }
 
 static int invert_common(lqcd_ctx* c, void* x_public, const void* b_public, const void* gauge, const void* clover,
                          const void* clover_inv, double kappa, double csw, double tol, int maxiter, int solver,
-                         int matpc, void* workspace, size_t workspace_bytes, lqcd_result* res, cudaStream_t st) {
+                         int matpc, int nrhs, void* workspace, size_t workspace_bytes, lqcd_result* res, cudaStream_t st) {
   if (!c || !x_public || !b_public || !gauge || !workspace || !res) return LQCD_ERR_INVALID_ARG;
-  if (solver < 0 || solver > 2 || (matpc != 0 && matpc != 1) || maxiter < 0 || !(tol >= 0) || (clover && !clover_inv))
-    return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "invert: bad solver/matpc/maxiter/tol");
-  if (workspace_bytes < lqcd_invert_workspace_bytes(c, solver))
+  if (solver < 0 || solver > 2 || (matpc != 0 && matpc != 1) || maxiter < 0 || !(tol >= 0) || (clover && !clover_inv) ||
+      nrhs < 1 || nrhs > LQCD_MAX_RHS)
+    return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "invert: bad solver/matpc/maxiter/tol/nrhs");
+  if (workspace_bytes < lqcd_invert_multi_workspace_bytes(c, solver, nrhs))
     return lqcd_set_error(c, LQCD_ERR_WORKSPACE, "invert: workspace %zu < %zu", workspace_bytes,
-                          lqcd_invert_workspace_bytes(c, solver));
+                          lqcd_invert_multi_workspace_bytes(c, solver, nrhs));
   const void* p[6] = {x_public, b_public, gauge, clover, clover_inv, workspace};
   if (!check_ptrs(c, p, 6, "invert")) return LQCD_ERR_ALIGN;
-  memset(res, 0, sizeof(*res));
+  memset(res, 0, sizeof(*res) * nrhs);
   const long launches0 = c->launches;
+  const size_t sp = lqcd_spinor_bytes(c);
   Work w;
-  carve(c, workspace, w, clover == nullptr);
+  carve(c, workspace, w, nrhs, clover == nullptr);
   int rc;
   cudaEventRecord(c->ev0, st);
   if (!clover) {
@@ -332,16 +420,24 @@ static int invert_common(lqcd_ctx* c, void* x_public, const void* b_public, cons
     clover = w.clover;
     clover_inv = w.clover_inv;
   }
-  if ((rc = lqcd_spinor_pack(c, w.b, b_public, (void*)st))) return rc;
+  for (int j = 0; j < nrhs; j++)
+    for (int par = 0; par < 2; par++)
+      if ((rc = lqcd_spinor_pack_parity(c, w.b + ((size_t)par * nrhs + j) * sp,
+                                        (const char*)b_public + ((size_t)2 * j + par) * sp, st))) return rc;
   if ((rc = invert_native(c, w, gauge, clover, clover_inv, kappa, tol, maxiter, solver, matpc, res, st))) return rc;
-  if ((rc = lqcd_spinor_unpack(c, x_public, w.x, (void*)st))) return rc;
+  for (int j = 0; j < nrhs; j++)
+    for (int par = 0; par < 2; par++)
+      if ((rc = lqcd_spinor_unpack_parity(c, (char*)x_public + ((size_t)2 * j + par) * sp,
+                                          w.x + ((size_t)par * nrhs + j) * sp, st))) return rc;
   cudaEventRecord(c->ev1, st);
   if (cudaStreamSynchronize(st) != cudaSuccess) return lqcd_check_cuda(c, "invert sync");
   float ms = 0;
   cudaEventElapsedTime(&ms, c->ev0, c->ev1);
-  res->seconds = ms * 1e-3;
-  res->kernel_launches = c->launches - launches0;
-  return res->status;
+  for (int j = 0; j < nrhs; j++) {
+    res[j].seconds = ms * 1e-3;  // of the whole (batched) call
+    res[j].kernel_launches = c->launches - launches0;
+  }
+  return worst_status(res, nrhs);
 }
 
 extern "C" {
@@ -349,7 +445,15 @@ extern "C" {
 int lqcd_invert(lqcd_ctx* c, void* x_public, const void* b_public, const void* gauge, const void* clover,
                 const void* clover_inv, double kappa, double csw, double tol, int maxiter, int solver, int matpc,
                 void* workspace, size_t workspace_bytes, lqcd_result* res, void* stream) {
-  return invert_common(c, x_public, b_public, gauge, clover, clover_inv, kappa, csw, tol, maxiter, solver, matpc,
+  return invert_common(c, x_public, b_public, gauge, clover, clover_inv, kappa, csw, tol, maxiter, solver, matpc, 1,
+                       workspace, workspace_bytes, res, as_stream(stream));
+}
+
+int lqcd_invert_multi(lqcd_ctx* c, void* x_public, const void* b_public, const void* gauge, const void* clover,
+                      const void* clover_inv, double kappa, double tol, int maxiter, int solver, int matpc, int nrhs,
+                      void* workspace, size_t workspace_bytes, lqcd_result* res, void* stream) {
+  if (!clover || !clover_inv) return LQCD_ERR_INVALID_ARG;
+  return invert_common(c, x_public, b_public, gauge, clover, clover_inv, kappa, 0.0, tol, maxiter, solver, matpc, nrhs,
                        workspace, workspace_bytes, res, as_stream(stream));
 }
 
@@ -375,7 +479,7 @@ int lqcd_dslash_host(lqcd_ctx* c, void* out_host, const void* in_host, const voi
   int rc;
   cudaMemcpyAsync(s, (const char*)in_host + (size_t)(1 - parity) * sp, sp, cudaMemcpyHostToDevice, st);
   if ((rc = lqcd_spinor_pack_parity(c, s + 2 * sp, s, st))) return rc;
-  if ((rc = lqcd_dslash_launch(c, s + 3 * sp, s + 2 * sp, gauge, nullptr, nullptr, parity, scale, dagger ? 1 : 0, 0, st))) return rc;
+  if ((rc = lqcd_dslash_launch(c, s + 3 * sp, s + 2 * sp, gauge, nullptr, nullptr, parity, scale, dagger ? 1 : 0, 0, 1, st))) return rc;
   if ((rc = lqcd_spinor_unpack_parity(c, s + sp, s + 3 * sp, st))) return rc;
   cudaMemcpyAsync((char*)out_host + (size_t)parity * sp, s + sp, sp, cudaMemcpyDeviceToHost, st);
   if (cudaStreamSynchronize(st) != cudaSuccess) return lqcd_check_cuda(c, "dslash_host sync");
@@ -391,7 +495,7 @@ int lqcd_invert_host(lqcd_ctx* c, void* x_host, const void* b_host, const void* 
   const size_t sp = lqcd_spinor_bytes(c);
   char* s = (char*)scratch;
   cudaMemcpyAsync(s, b_host, 2 * sp, cudaMemcpyHostToDevice, st);
-  int rc = invert_common(c, s + 2 * sp, s, gauge, clover, clover_inv, kappa, 0.0, tol, maxiter, solver, matpc,
+  int rc = invert_common(c, s + 2 * sp, s, gauge, clover, clover_inv, kappa, 0.0, tol, maxiter, solver, matpc, 1,
                          s + 4 * sp, scratch_bytes - 4 * sp, res, st);
   if (rc < 0) return rc;
   cudaMemcpyAsync(x_host, s + 2 * sp, 2 * sp, cudaMemcpyDeviceToHost, st);
@@ -399,14 +503,15 @@ int lqcd_invert_host(lqcd_ctx* c, void* x_host, const void* b_host, const void* 
   return rc;
 }
 
+// BLAS-1 entry points: single right-hand side, slot S_DONE of column 0 cleared by every solve's end
 int lqcd_blas_axpy_norm(lqcd_ctx* c, double a, const void* x, void* y, double* norm2_host, void* stream) {
   if (!c || !x || !y || !norm2_host) return LQCD_ERR_INVALID_ARG;
   cudaStream_t st = as_stream(stream);
   void* v[2] = {(void*)x, y};
   int o[4] = {S_TRUE, 0, 0, 0};
   int rc;
-  if ((rc = BLAS_CALL(c, OpAxpyNorm, op.a = a, v, o, st))) return rc;
-  if ((rc = read_scalars(c, S_TRUE, 1, st))) return rc;
+  if ((rc = BLAS_CALL(c, OpAxpyNorm, op.a = a, v, o, 1, 0, st))) return rc;
+  if ((rc = read_scalars(c, 1, st))) return rc;
   *norm2_host = c->h_scalars[S_TRUE];
   return LQCD_OK;
 }
@@ -416,7 +521,7 @@ int lqcd_blas_xpay(lqcd_ctx* c, const void* x, double a, void* y, void* stream) 
   cudaStream_t st = as_stream(stream);
   void* v[2] = {(void*)x, y};
   int rc;
-  if ((rc = BLAS_CALL(c, OpXpay, op.a = a, v, nullptr, st))) return rc;
+  if ((rc = BLAS_CALL(c, OpXpay, op.a = a, v, nullptr, 1, 0, st))) return rc;
   if (cudaStreamSynchronize(st) != cudaSuccess) return lqcd_check_cuda(c, "blas_xpay sync");
   return LQCD_OK;
 }
@@ -427,8 +532,8 @@ int lqcd_blas_cdot(lqcd_ctx* c, const void* x, const void* y, double out_host[3]
   void* v[2] = {(void*)x, (void*)y};
   int o[4] = {S_TRUE, S_TRUE + 1, S_TRUE + 2, 0};
   int rc;
-  if ((rc = BLAS_CALL(c, OpCdot, (void)op, v, o, st))) return rc;
-  if ((rc = read_scalars(c, S_TRUE, 3, st))) return rc;
+  if ((rc = BLAS_CALL(c, OpCdot, (void)op, v, o, 1, 0, st))) return rc;
+  if ((rc = read_scalars(c, 1, st))) return rc;
   for (int i = 0; i < 3; i++) out_host[i] = c->h_scalars[S_TRUE + i];
   return LQCD_OK;
 }
@@ -439,7 +544,7 @@ int lqcd_blas_caxpbypz(lqcd_ctx* c, const double a[2], const void* x, const doub
   cudaStream_t st = as_stream(stream);
   void* v[3] = {(void*)x, (void*)y, z};
   int rc;
-  if ((rc = BLAS_CALL(c, OpCaxpbypz, (op.a = {a[0], a[1]}, op.b = {b[0], b[1]}), v, nullptr, st))) return rc;
+  if ((rc = BLAS_CALL(c, OpCaxpbypz, (op.a = {a[0], a[1]}, op.b = {b[0], b[1]}), v, nullptr, 1, 0, st))) return rc;
   if (cudaStreamSynchronize(st) != cudaSuccess) return lqcd_check_cuda(c, "blas_caxpbypz sync");
   return LQCD_OK;
 }

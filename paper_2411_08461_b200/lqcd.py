@@ -34,7 +34,9 @@ SYMBOLS = [
     "lqcd_clover_build", "lqcd_clover_apply", "lqcd_dslash", "lqcd_mpc_apply", "lqcd_mat_apply",
     "lqcd_invert", "lqcd_host_scratch_bytes", "lqcd_dslash_host", "lqcd_invert_host",
     "lqcd_blas_axpy_norm", "lqcd_blas_xpay", "lqcd_blas_cdot", "lqcd_blas_caxpbypz",
+    "lqcd_dslash_mrhs", "lqcd_mpc_apply_mrhs", "lqcd_invert_multi_workspace_bytes", "lqcd_invert_multi",
 ]
+MAX_RHS = 16
 
 
 def library_path():
@@ -79,6 +81,12 @@ def load():
     L.lqcd_mat_apply.argtypes = [vp, vp, vp, vp, vp, cd, ci, vp]
     L.lqcd_invert.argtypes = [vp, vp, vp, vp, vp, vp, cd, cd, cd, ci, ci, ci, vp, sz,
                               ctypes.POINTER(Result), vp]
+    L.lqcd_dslash_mrhs.argtypes = [vp, vp, vp, vp, ci, cd, ci, ci, vp]
+    L.lqcd_mpc_apply_mrhs.argtypes = [vp, vp, vp, vp, vp, vp, cd, ci, ci, vp, ci, vp]
+    L.lqcd_invert_multi_workspace_bytes.restype = sz
+    L.lqcd_invert_multi_workspace_bytes.argtypes = [vp, ci, ci]
+    L.lqcd_invert_multi.argtypes = [vp, vp, vp, vp, vp, vp, cd, cd, ci, ci, ci, ci, vp, sz,
+                                    ctypes.POINTER(Result), vp]
     L.lqcd_dslash_host.argtypes = [vp, vp, vp, vp, ci, cd, ci, vp, vp]
     L.lqcd_invert_host.argtypes = [vp, vp, vp, vp, vp, vp, cd, cd, ci, ci, ci, vp, sz,
                                    ctypes.POINTER(Result), vp]
@@ -246,6 +254,38 @@ class Context:
                                   workspace.numel() * self.prec, ctypes.byref(res), _stream())
         self._check(rc, allow_not_converged=True)
         return x, res
+
+    # ---- multi-right-hand-side forms (nrhs consecutive one-parity native spinors) -----------------
+    def dslash_mrhs(self, out, inp, gauge, parity, nrhs, scale=1.0, dagger=False):
+        self._check(self.lib.lqcd_dslash_mrhs(self.h, _p(out), _p(inp), _p(gauge), parity, scale,
+                                              int(dagger), nrhs, _stream()))
+        return out
+
+    def mpc_apply_mrhs(self, out, inp, gauge, clover, clover_inv, kappa, nrhs, matpc=0, dagger=False, tmp=None):
+        tmp = tmp if tmp is not None else self.new_spinor(nrhs)
+        self._check(self.lib.lqcd_mpc_apply_mrhs(self.h, _p(out), _p(inp), _p(gauge), _p(clover),
+                                                 _p(clover_inv), kappa, matpc, int(dagger), _p(tmp), nrhs,
+                                                 _stream()))
+        return out
+
+    def workspace_multi(self, nrhs, solver="cgne"):
+        n = self.lib.lqcd_invert_multi_workspace_bytes(self.h, SOLVERS[solver], nrhs)
+        return self.empty(n), n
+
+    def invert_multi(self, b_public, gauge, clover, clover_inv, kappa, tol=1e-10, maxiter=1000,
+                     solver="cgne", matpc=0, workspace=None):
+        """b_public: [nrhs, 2, Lt, Lz, Ly, Lx/2, 4, 3] device tensor; returns (x, [Result]*nrhs, status)."""
+        nrhs = b_public.shape[0]
+        if workspace is None:
+            workspace, _ = self.workspace_multi(nrhs, solver)
+        x = torch.empty_like(b_public)
+        res = (Result * nrhs)()
+        rc = self.lib.lqcd_invert_multi(self.h, _p(x), _p(b_public), _p(gauge), _p(clover), _p(clover_inv),
+                                        kappa, tol, maxiter, SOLVERS[solver], matpc, nrhs, _p(workspace),
+                                        workspace.numel() * self.prec, res, _stream())
+        if rc < 0 and rc != -7:  # a breakdown of some column is reported per column
+            self._check(rc)
+        return x, list(res), rc
 
     # ---- host-buffer (end-to-end) entry points -----------------------------------------------
     def host_scratch(self, solver="cgne"):

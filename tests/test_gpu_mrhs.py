@@ -1,0 +1,135 @@
+"""GPU parity of the multi-right-hand-side path against the
+oracle: every column of lqcd_dslash_mrhs / lqcd_mpc_apply_mrhs equals the oracle's operator on that
+column (north_star tolerances), and every column of lqcd_invert_multi meets reading A17 (oracle's
+solution within 10*tol, oracle-evaluated true residual below tol)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2411_08461_b200 import synth
+from latt import rel_err
+from test_gpu_parity import Setup, TOL, from_cfg, lq
+
+pytestmark = pytest.mark.gpu
+
+
+def pack_block(s, psis, parity):
+    """list of public spinors -> device block [nrhs][one-parity native] of the given parity."""
+    return torch.cat([s.ctx.parity(s.up(p), parity) for p in psis])
+
+
+def unpack_block(s, block, nrhs, parity):
+    n = s.ctx.spinor_bytes // s.ctx.prec
+    out = []
+    for r in range(nrhs):
+        full = s.ctx.new_spinor(2)
+        full.zero_()
+        s.ctx.parity(full, parity).copy_(block[r * n:(r + 1) * n])
+        out.append(s.down(full)[parity])
+    return out
+
+
+@pytest.mark.parametrize("prec,recon", [(8, 18), (8, 12), (4, 18), (4, 12)])
+@pytest.mark.parametrize("dims,tb,nrhs", [((4, 6, 8, 10), -1, 12), ((8, 8, 8, 16), -1, 12), ((12, 4, 6, 4), 1, 5),
+                                          ((4, 4, 4, 8), -1, 16), ((4, 4, 4, 8), -1, 2)])
+def test_dslash_mrhs_matches_oracle(prec, recon, dims, tb, nrhs):
+    s = Setup(dims, 0.5, 2, 0.124, 1.2, prec, recon, tb, with_clover=False)
+    psis = [s.spinor("gaussian", 200 + r) for r in range(nrhs)]
+    n = s.ctx.spinor_bytes // s.ctx.prec
+    for dagger in (False, True):
+        wants = [s.orc.dslash(p, dagger=dagger) for p in psis]
+        for par in (0, 1):
+            inp = pack_block(s, psis, 1 - par)
+            out = s.ctx.new_spinor(nrhs)
+            s.ctx.dslash_mrhs(out, inp, s.gauge, par, nrhs, 1.0, dagger)
+            gots = unpack_block(s, out, nrhs, par)
+            for r in range(nrhs):
+                assert rel_err(gots[r], wants[r][par]) < TOL[prec], (dagger, par, r)
+            # every column equals the single-RHS kernel's result up to rounding order
+            single = s.ctx.new_spinor(1)
+            s.ctx.dslash(single, inp[:n], s.gauge, par, 1.0, dagger)
+            assert rel_err(out[:n].cpu().numpy().astype(np.float64), single.cpu().numpy().astype(np.float64)) < TOL[prec]
+
+
+@pytest.mark.parametrize("prec,recon", [(8, 18), (4, 12)])
+@pytest.mark.parametrize("nrhs", [12, 7])
+def test_mpc_apply_mrhs(prec, recon, nrhs):
+    s, c = from_cfg(2, prec, recon)
+    psis = [s.spinor("gaussian", 300 + r) for r in range(nrhs)]
+    for p in psis:
+        p[1] = 0
+    inp = pack_block(s, psis, 0)
+    for matpc in (0, 1):
+        for dagger in (False, True):
+            out = s.ctx.new_spinor(nrhs)
+            s.ctx.mpc_apply_mrhs(out, inp, s.gauge, s.A, s.Ai, s.kappa, nrhs, matpc, dagger)
+            gots = unpack_block(s, out, nrhs, 0)
+            for r in range(nrhs):
+                assert rel_err(gots[r], s.orc.mpc(psis[r], matpc, dagger)[0]) < TOL[prec], (matpc, dagger, r)
+
+
+@pytest.mark.parametrize("solver", ["cgne", "cgnr", "bicgstab"])
+def test_invert_multi_fp64_config2(solver):
+    """Columns of different difficulty (point, Z2, Gaussian, zero) in one batch: each column must be
+    the solution of its own system, frozen at its own convergence."""
+    s, c = from_cfg(2, 8, 18)
+    dims = c["dims"]
+    bs = [synth.source(dims, "point", spin=1, colour=2), synth.source(dims, "z2", 102),
+          synth.source(dims, "gaussian", 5), np.zeros_like(synth.source(dims, "point")),
+          synth.source(dims, "point", spin=3, colour=0)]
+    B = s.ctx.to_device(np.stack(bs))
+    x, res, rc = s.ctx.invert_multi(B, s.gauge, s.A, s.Ai, s.kappa, tol=1e-10, maxiter=2000, solver=solver)
+    assert rc == 0
+    xs = x.cpu().numpy()
+    its = []  # per-column iteration counts (columns freeze independently; the zero column never starts)
+    for r, b in enumerate(bs):
+        assert res[r].status == 0
+        if not b.any():
+            assert res[r].iterations == 0 and not xs[r].any()
+            continue
+        true = s.orc.true_residual(b, xs[r])
+        assert true < 1e-10 and abs(true - res[r].true_resid) < 5e-11, (r, true, res[r].as_dict())
+        xo, ro = s.orc.invert(b, 1e-10, 2000, "bicgstab", 0)
+        assert rel_err(xs[r], xo) < 1e-9, r
+        # same answer and iteration count as the column's own single solve
+        x1, r1 = s.ctx.invert(s.ctx.to_device(b), s.gauge, s.A, s.Ai, s.kappa, tol=1e-10, maxiter=2000, solver=solver)
+        assert r1.iterations == res[r].iterations
+        assert rel_err(xs[r], x1.cpu().numpy()) < 1e-12
+        its.append(res[r].iterations)
+
+
+def test_invert_multi_maxiter_and_errors():
+    s, c = from_cfg(1, 8, 18)
+    bs = np.stack([synth.source(c["dims"], "gaussian", 9), synth.source(c["dims"], "point")])
+    B = s.ctx.to_device(bs)
+    x, res, rc = s.ctx.invert_multi(B, s.gauge, s.A, s.Ai, s.kappa, tol=1e-10, maxiter=3, solver="cgne")
+    assert rc == 1 and all(r.status == 1 and r.iterations == 3 for r in res)
+    with pytest.raises(lq().LqcdError):
+        s.ctx.invert_multi(B, s.gauge, s.A, s.Ai, s.kappa, workspace=s.ctx.empty(1024))
+    big = s.ctx.to_device(np.stack([bs[0]] * 17))
+    with pytest.raises(lq().LqcdError):
+        s.ctx.invert_multi(big, s.gauge, s.A, s.Ai, s.kappa)
+
+
+def test_config3_propagator_12_columns_batched_fp32_recon12():
+    """BASELINE config 3 through the batched path: the 12 spin-colour columns of a point-source
+    propagator in ONE lqcd_invert_multi call (fp32, reconstruct-12, CGNE to 1e-6)."""
+    s, c = from_cfg(3, 4, 12)
+    dims = c["dims"]
+    bs = [synth.source(dims, "point", spin=sp, colour=col) for sp in range(4) for col in range(3)]
+    B = s.ctx.to_device(np.stack(bs))
+    x, res, rc = s.ctx.invert_multi(B, s.gauge, s.A, s.Ai, s.kappa, tol=1e-6, solver="cgne")
+    assert rc == 0
+    xs = x.cpu().numpy().astype(np.complex128)
+    for r in (0, 5, 11):
+        assert s.orc.true_residual(bs[r], xs[r]) < 2e-6
+    xo, ro = s.orc.invert(bs[0], 1e-9, 2000, "cgne", 0)
+    assert rel_err(xs[0], xo) < 1e-5
+    # sink-source assembly [.., s_sink, s_src, c_sink, c_src] and gamma5-hermiticity at the source
+    prop = np.zeros(s.orc.site_shape + (4, 4, 3, 3), dtype=np.complex128)
+    for r in range(12):
+        prop[..., :, r // 3, :, r % 3] = xs[r]
+    S00 = prop[0, 0, 0, 0, 0].transpose(0, 2, 1, 3).reshape(12, 12)
+    g5 = np.repeat([1, 1, -1, -1.0], 3)
+    assert np.abs(g5[:, None] * S00 * g5[None, :] - S00.conj().T).max() < 1e-5 * np.abs(S00).max()
