@@ -156,6 +156,20 @@ int lqcd_invert_multi(lqcd_ctx* ctx, void* x_public, const void* b_public, const
                       const void* clover_inv, double kappa, double tol, int maxiter, int solver, int matpc,
                       int nrhs, void* workspace, size_t workspace_bytes, lqcd_result* res, void* stream);
 
+/* Mixed precision: the same system solved to the same fp64 stopping test
+ * |r_hat| <= tol*|b| by fp64 defect correction around fp32 Krylov solves:
+ *     x = 0, r = b_hat;  repeat { e = Mhat^-1 (r/|r|) in fp32 to tol_k;  x += |r| e;  r = b_hat - Mhat x (fp64) }
+ * with tol_k = max(inner_tol, 0.25*tol*|b|/|r|).  ctx: fp64 context owning x, b, gauge, clover,
+ * clover_inv, workspace (as lqcd_invert); ctx_lo: fp32 context of the same lattice/boundary/device
+ * owning gauge_lo, clover_lo, clover_inv_lo (its own pack/clover_build of the same links; the
+ * reconstructions may differ) and workspace_lo (>= lqcd_invert_workspace_bytes(ctx_lo)).
+ * res->iterations counts inner iterations; true_resid is recomputed in fp64.  Host-synchronous. */
+int lqcd_invert_mixed(lqcd_ctx* ctx, lqcd_ctx* ctx_lo, void* x_public, const void* b_public, const void* gauge,
+                      const void* clover, const void* clover_inv, const void* gauge_lo, const void* clover_lo,
+                      const void* clover_inv_lo, double kappa, double tol, double inner_tol, int maxiter, int solver,
+                      int matpc, void* workspace, size_t workspace_bytes, void* workspace_lo,
+                      size_t workspace_lo_bytes, lqcd_result* res, void* stream);
+
 /* End-to-end variants with HOST buffers (pageable or pinned): the call uploads the public input,
  * packs, computes, unpacks and downloads the public result.  Links/clover stay resident on the
  * device (PAPER.md:225 loadGauge).  scratch: device buffer of >= lqcd_host_scratch_bytes. */

@@ -307,9 +307,122 @@ static void carve(lqcd_ctx* c, void* workspace, Work& w, int nrhs, bool with_clo
   w.clover_inv = with_clover ? p + lqcd_clover_bytes(c) : nullptr;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Mixed precision: fp64 defect correction around fp32 Krylov solves.
+//   x = 0, r = bhat;  repeat { e = Mhat^-1 (r/|r|) in fp32 to tol_k ; x += |r| e ; r = bhat - Mhat x in fp64 }
+// The fp64 residual is recomputed from x every outer step, so the result meets the same stopping
+// test |r_hat| <= tol |b| as the pure fp64 solve; the fp32 inner solves carry ~all the bytes at half
+// the width.  tol_k = max(inner_tol, 0.25 * tol|b| / |r|): the last inner solve is not over-solved.
+// ---------------------------------------------------------------------------------------------
+struct Mixed {
+  lqcd_ctx* ci;  // fp32 context (same lattice, boundary, device)
+  Work wi;
+  const void *gauge, *A, *Ai;  // fp32 natives
+  double inner_tol;
+};
+
+__global__ void __launch_bounds__(256) spinor_down_kernel(float4* __restrict__ out, const double2* __restrict__ in, int Vh,
+                                                          double scale) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= Vh) return;
+#pragma unroll
+  for (int u = 0; u < 6; u++) {
+    const double2 a = in[(size_t)(2 * u) * Vh + i], b = in[(size_t)(2 * u + 1) * Vh + i];
+    out[(size_t)u * Vh + i] = make_float4((float)(scale * a.x), (float)(scale * a.y), (float)(scale * b.x), (float)(scale * b.y));
+  }
+}
+__global__ void __launch_bounds__(256) spinor_up_axpy_kernel(double2* __restrict__ x, const float4* __restrict__ e, int Vh,
+                                                             double a) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= Vh) return;
+#pragma unroll
+  for (int u = 0; u < 6; u++) {
+    const float4 v = e[(size_t)u * Vh + i];
+    double2 p = x[(size_t)(2 * u) * Vh + i], q = x[(size_t)(2 * u + 1) * Vh + i];
+    p.x += a * v.x; p.y += a * v.y; q.x += a * v.z; q.y += a * v.w;
+    x[(size_t)(2 * u) * Vh + i] = p;
+    x[(size_t)(2 * u + 1) * Vh + i] = q;
+  }
+}
+
+static int solve_cg(lqcd_ctx* c, const Work& w, const void* gauge, const void* A, const void* Ai, double kappa,
+                    int matpc, int normal_residual, Cols& cols, int maxiter, lqcd_result* res, cudaStream_t st);
+static int solve_bicgstab(lqcd_ctx* c, const Work& w, const void* gauge, const void* A, const void* Ai, double kappa,
+                          int matpc, Cols& cols, int maxiter, lqcd_result* res, cudaStream_t st);
+
+// single right-hand side; bhat in w.v[0], x_e (zeroed) in w.x; fills cols.rr[0], res->iterations
+static int solve_mixed(lqcd_ctx* c, const Work& w, const void* gauge, const void* A, const void* Ai, double kappa,
+                       int matpc, int solver, Cols& cols, int maxiter, lqcd_result* res, Mixed& m, cudaStream_t st) {
+  lqcd_ctx* ci = m.ci;
+  char *bh = w.v[0], *r = w.v[1], *mx = w.v[2], *tmp = w.v[5], *x = w.x;
+  const size_t sp = lqcd_spinor_bytes(c);
+  const int Vh = c->lat.Vh, grid = (Vh + 255) / 256;
+  int rc;
+  cudaMemcpyAsync(r, bh, sp, cudaMemcpyDeviceToDevice, st);
+  double rr = 0;
+  {
+    void* v[1] = {r};
+    int o[4] = {S_RES, 0, 0, 0};
+    if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v, o, 1, 0, st))) return rc;
+    if ((rc = read_scalars(c, 1, st))) return rc;
+    rr = hs(c, 0, S_RES);
+  }
+  int total = 0, outer = 0;
+  while (rr > cols.stop2[0] && total < maxiter && outer < 64) {
+    const double rn = sqrt(rr);
+    spinor_down_kernel<<<grid, 256, 0, st>>>((float4*)m.wi.v[0], (const double2*)r, Vh, 1.0 / rn);
+    c->alg_bytes += (double)Vh * 24 * 12;
+    LQCD_LAUNCH_CHECK(c, "spinor_down");
+    // inner fp32 solve of Mhat e = r/|r|, relative tolerance tol_k
+    const double need = 0.25 * sqrt(cols.stop2[0] / rr);
+    const double tol_k = need > m.inner_tol ? need : m.inner_tol;
+    Cols ic;
+    ic.n = 1;
+    ic.active[0] = true;
+    ic.bb[0] = 1.0;
+    ic.stop2[0] = tol_k * tol_k;
+    ic.rr[0] = 1.0;
+    cudaMemsetAsync(ci->d_scalars, 0, sizeof(double) * SC_STRIDE, st);
+    lqcd_result ri;
+    memset(&ri, 0, sizeof(ri));
+    ci->acct_rhs = 0;
+    if (solver == LQCD_SOLVER_BICGSTAB) rc = solve_bicgstab(ci, m.wi, m.gauge, m.A, m.Ai, kappa, matpc, ic, maxiter - total, &ri, st);
+    else rc = solve_cg(ci, m.wi, m.gauge, m.A, m.Ai, kappa, matpc, solver == LQCD_SOLVER_CGNR, ic, maxiter - total, &ri, st);
+    if (rc) return lqcd_set_error(c, rc, "invert_mixed: inner solve: %s", ci->err);
+    total += ri.iterations;
+    res->dslash_count += ri.dslash_count;
+    if (ri.status < 0) { res->status = ri.status; break; }
+    // x += |r| e ; r = bhat - Mhat x (fp64)
+    spinor_up_axpy_kernel<<<grid, 256, 0, st>>>((double2*)x, (const float4*)m.wi.x, Vh, rn);
+    c->alg_bytes += (double)Vh * 24 * 20;
+    LQCD_LAUNCH_CHECK(c, "spinor_up_axpy");
+    if ((rc = mpc_apply(c, mx, x, gauge, A, Ai, kappa, matpc, 0, tmp, 1, st))) return rc;
+    res->dslash_count += 2;
+    {
+      void* v[2] = {bh, mx};
+      if ((rc = BLAS_CALL(c, OpXpay, op.a = -1.0, v, nullptr, 1, 0, st))) return rc;  // mx = bhat - Mhat x
+      void* v2[1] = {mx};
+      int o[4] = {S_RES, 0, 0, 0};
+      if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v2, o, 1, 0, st))) return rc;
+      if ((rc = read_scalars(c, 1, st))) return rc;
+    }
+    char* sw = r; r = mx; mx = sw;
+    const double rr_new = hs(c, 0, S_RES);
+    outer++;
+    if (!(rr_new == rr_new)) { res->status = LQCD_ERR_BREAKDOWN; rr = rr_new; break; }
+    if (rr_new > 0.81 * rr) { rr = rr_new; break; }  // fp32 inner solves no longer reduce the fp64 residual
+    rr = rr_new;
+  }
+  cols.rr[0] = rr;
+  res->iterations = total;
+  c->launches += 0;
+  return LQCD_OK;
+}
+
 // the whole solve on native fields already in w.b; result in w.x (both parities)
 static int invert_native(lqcd_ctx* c, Work& w, const void* gauge, const void* A, const void* Ai, double kappa,
-                         double tol, int maxiter, int solver, int matpc, lqcd_result* res, cudaStream_t st) {
+                         double tol, int maxiter, int solver, int matpc, lqcd_result* res, cudaStream_t st,
+                         Mixed* mixed = nullptr) {
   const int n = w.nrhs;
   const size_t blk = lqcd_spinor_bytes(c) * n, half = lqcd_clover_bytes(c) / 2;
   const void* Ai_e = Ai;
@@ -352,7 +465,8 @@ static int invert_native(lqcd_ctx* c, Work& w, const void* gauge, const void* A,
     for (int j = 0; j < n; j++)
       if (!cols.active[j]) set_slot(c, j, S_DONE, true, st);
     c->acct_rhs = cols.nactive();
-    if (solver == LQCD_SOLVER_BICGSTAB) rc = solve_bicgstab(c, w, gauge, A, Ai, kappa, matpc, cols, maxiter, res, st);
+    if (mixed) rc = solve_mixed(c, w, gauge, A, Ai, kappa, matpc, solver, cols, maxiter, res, *mixed, st);
+    else if (solver == LQCD_SOLVER_BICGSTAB) rc = solve_bicgstab(c, w, gauge, A, Ai, kappa, matpc, cols, maxiter, res, st);
     else rc = solve_cg(c, w, gauge, A, Ai, kappa, matpc, solver == LQCD_SOLVER_CGNR, cols, maxiter, res, st);
     c->acct_rhs = 0;
     if (rc) return rc;
@@ -397,7 +511,8 @@ static int worst_status(const lqcd_result* res, int n) {
 
 static int invert_common(lqcd_ctx* c, void* x_public, const void* b_public, const void* gauge, const void* clover,
                          const void* clover_inv, double kappa, double csw, double tol, int maxiter, int solver,
-                         int matpc, int nrhs, void* workspace, size_t workspace_bytes, lqcd_result* res, cudaStream_t st) {
+                         int matpc, int nrhs, void* workspace, size_t workspace_bytes, lqcd_result* res, cudaStream_t st,
+                         Mixed* mixed = nullptr) {
   if (!c || !x_public || !b_public || !gauge || !workspace || !res) return LQCD_ERR_INVALID_ARG;
   if (solver < 0 || solver > 2 || (matpc != 0 && matpc != 1) || maxiter < 0 || !(tol >= 0) || (clover && !clover_inv) ||
       nrhs < 1 || nrhs > LQCD_MAX_RHS)
@@ -408,7 +523,7 @@ static int invert_common(lqcd_ctx* c, void* x_public, const void* b_public, cons
   const void* p[6] = {x_public, b_public, gauge, clover, clover_inv, workspace};
   if (!check_ptrs(c, p, 6, "invert")) return LQCD_ERR_ALIGN;
   memset(res, 0, sizeof(*res) * nrhs);
-  const long launches0 = c->launches;
+  const long launches0 = c->launches, mixed_launches0 = mixed ? mixed->ci->launches : 0;
   const size_t sp = lqcd_spinor_bytes(c);
   Work w;
   carve(c, workspace, w, nrhs, clover == nullptr);
@@ -424,7 +539,7 @@ static int invert_common(lqcd_ctx* c, void* x_public, const void* b_public, cons
     for (int par = 0; par < 2; par++)
       if ((rc = lqcd_spinor_pack_parity(c, w.b + ((size_t)par * nrhs + j) * sp,
                                         (const char*)b_public + ((size_t)2 * j + par) * sp, st))) return rc;
-  if ((rc = invert_native(c, w, gauge, clover, clover_inv, kappa, tol, maxiter, solver, matpc, res, st))) return rc;
+  if ((rc = invert_native(c, w, gauge, clover, clover_inv, kappa, tol, maxiter, solver, matpc, res, st, mixed))) return rc;
   for (int j = 0; j < nrhs; j++)
     for (int par = 0; par < 2; par++)
       if ((rc = lqcd_spinor_unpack_parity(c, (char*)x_public + ((size_t)2 * j + par) * sp,
@@ -435,7 +550,7 @@ static int invert_common(lqcd_ctx* c, void* x_public, const void* b_public, cons
   cudaEventElapsedTime(&ms, c->ev0, c->ev1);
   for (int j = 0; j < nrhs; j++) {
     res[j].seconds = ms * 1e-3;  // of the whole (batched) call
-    res[j].kernel_launches = c->launches - launches0;
+    res[j].kernel_launches = c->launches - launches0 + (mixed ? mixed->ci->launches - mixed_launches0 : 0);
   }
   return worst_status(res, nrhs);
 }
@@ -455,6 +570,31 @@ int lqcd_invert_multi(lqcd_ctx* c, void* x_public, const void* b_public, const v
   if (!clover || !clover_inv) return LQCD_ERR_INVALID_ARG;
   return invert_common(c, x_public, b_public, gauge, clover, clover_inv, kappa, 0.0, tol, maxiter, solver, matpc, nrhs,
                        workspace, workspace_bytes, res, as_stream(stream));
+}
+
+int lqcd_invert_mixed(lqcd_ctx* c, lqcd_ctx* ci, void* x_public, const void* b_public, const void* gauge,
+                      const void* clover, const void* clover_inv, const void* gauge_lo, const void* clover_lo,
+                      const void* clover_inv_lo, double kappa, double tol, double inner_tol, int maxiter, int solver,
+                      int matpc, void* workspace, size_t workspace_bytes, void* workspace_lo, size_t workspace_lo_bytes,
+                      lqcd_result* res, void* stream) {
+  if (!c || !ci || !clover || !clover_inv || !gauge_lo || !clover_lo || !clover_inv_lo || !workspace_lo)
+    return LQCD_ERR_INVALID_ARG;
+  if (c->prec != 8 || ci->prec != 4 || c->device != ci->device || c->lat.tb != ci->lat.tb || c->L[0] != ci->L[0] ||
+      c->L[1] != ci->L[1] || c->L[2] != ci->L[2] || c->L[3] != ci->L[3] || !(inner_tol > 0) || !(inner_tol < 1))
+    return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "invert_mixed: needs an fp64 and an fp32 context of the same lattice");
+  if (workspace_lo_bytes < lqcd_invert_workspace_bytes(ci, solver))
+    return lqcd_set_error(c, LQCD_ERR_WORKSPACE, "invert_mixed: low-precision workspace too small");
+  const void* p[4] = {gauge_lo, clover_lo, clover_inv_lo, workspace_lo};
+  if (!check_ptrs(c, p, 4, "invert_mixed")) return LQCD_ERR_ALIGN;
+  Mixed m;
+  m.ci = ci;
+  carve(ci, workspace_lo, m.wi, 1, false);
+  m.gauge = gauge_lo;
+  m.A = clover_lo;
+  m.Ai = clover_inv_lo;
+  m.inner_tol = inner_tol;
+  return invert_common(c, x_public, b_public, gauge, clover, clover_inv, kappa, 0.0, tol, maxiter, solver, matpc, 1,
+                       workspace, workspace_bytes, res, as_stream(stream), &m);
 }
 
 size_t lqcd_host_scratch_bytes(const lqcd_ctx* c, int solver) {

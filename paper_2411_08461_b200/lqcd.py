@@ -35,6 +35,7 @@ SYMBOLS = [
     "lqcd_invert", "lqcd_host_scratch_bytes", "lqcd_dslash_host", "lqcd_invert_host",
     "lqcd_blas_axpy_norm", "lqcd_blas_xpay", "lqcd_blas_cdot", "lqcd_blas_caxpbypz",
     "lqcd_dslash_mrhs", "lqcd_mpc_apply_mrhs", "lqcd_invert_multi_workspace_bytes", "lqcd_invert_multi",
+    "lqcd_invert_mixed",
 ]
 MAX_RHS = 16
 
@@ -86,6 +87,8 @@ def load():
     L.lqcd_invert_multi_workspace_bytes.restype = sz
     L.lqcd_invert_multi_workspace_bytes.argtypes = [vp, ci, ci]
     L.lqcd_invert_multi.argtypes = [vp, vp, vp, vp, vp, vp, cd, cd, ci, ci, ci, ci, vp, sz,
+                                    ctypes.POINTER(Result), vp]
+    L.lqcd_invert_mixed.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, cd, cd, cd, ci, ci, ci, vp, sz, vp, sz,
                                     ctypes.POINTER(Result), vp]
     L.lqcd_dslash_host.argtypes = [vp, vp, vp, vp, ci, cd, ci, vp, vp]
     L.lqcd_invert_host.argtypes = [vp, vp, vp, vp, vp, vp, cd, cd, ci, ci, ci, vp, sz,
@@ -286,6 +289,24 @@ class Context:
         if rc < 0 and rc != -7:  # a breakdown of some column is reported per column
             self._check(rc)
         return x, list(res), rc
+
+    def invert_mixed(self, lo, b_public, gauge, clover, clover_inv, gauge_lo, clover_lo, clover_inv_lo, kappa,
+                     tol=1e-10, inner_tol=1e-4, maxiter=1000, solver="cgne", matpc=0, workspace=None,
+                     workspace_lo=None):
+        """self: fp64 context, lo: fp32 context of the same lattice (its own natives *_lo)."""
+        if workspace is None:
+            workspace, _ = self.workspace(solver)
+        if workspace_lo is None:
+            workspace_lo, _ = lo.workspace(solver)
+        x = torch.empty_like(b_public)
+        res = Result()
+        rc = self.lib.lqcd_invert_mixed(self.h, lo.h, _p(x), _p(b_public), _p(gauge), _p(clover), _p(clover_inv),
+                                        _p(gauge_lo), _p(clover_lo), _p(clover_inv_lo), kappa, tol, inner_tol,
+                                        maxiter, SOLVERS[solver], matpc, _p(workspace),
+                                        workspace.numel() * self.prec, _p(workspace_lo),
+                                        workspace_lo.numel() * lo.prec, ctypes.byref(res), _stream())
+        self._check(rc, allow_not_converged=True)
+        return x, res
 
     # ---- host-buffer (end-to-end) entry points -----------------------------------------------
     def host_scratch(self, solver="cgne"):

@@ -107,6 +107,20 @@ def test_config4_cgne_fp64_true_residual():
     assert true < 1e-10 and abs(true - res.true_resid) < 1e-11, (true, res.as_dict())
 
 
+def test_config4_mixed_precision_cgne():
+    """fp64-accurate solve at 32^3x64 by fp64 defect correction around fp32 reconstruct-12 CGNE
+    (SURVEY.md §8(f) rank 2); same bar as the pure fp64 solve."""
+    d = Dev(4, 8, 18)
+    lo = lq().Context(d.c["dims"], 4, 12, -1)
+    g_lo = lo.gauge_pack(lo.to_device(d.U))
+    A_lo, Ai_lo = lo.clover_build(g_lo, d.c["csw"], d.c["kappa"])
+    x, res = d.ctx.invert_mixed(lo, d.ctx.to_device(d.b), d.gauge, d.A, d.Ai, g_lo, A_lo, Ai_lo, d.c["kappa"],
+                                tol=1e-10, inner_tol=1e-4, solver="cgne")
+    assert res.status == 0, res.as_dict()
+    true = d.orc.true_residual(d.b, x.cpu().numpy())
+    assert true < 1e-10 and abs(true - res.true_resid) < 1e-11, (true, res.as_dict())
+
+
 @pytest.mark.parametrize("recon", [18, 12])
 def test_config4_operators_every_site_fp32(recon):
     check_operators(Dev(4, 4, recon))

@@ -118,3 +118,30 @@ def test_config3_propagator_12_columns_fp32_recon12():
     S00 = prop[0, 0, 0, 0, 0].transpose(0, 2, 1, 3).reshape(12, 12)   # (s_sink,c_sink),(s_src,c_src)
     g5 = np.repeat([1, 1, -1, -1.0], 3)
     assert np.abs(g5[:, None] * S00 * g5[None, :] - S00.conj().T).max() < 1e-5 * np.abs(S00).max()
+
+
+@pytest.mark.parametrize("solver", ["cgne", "bicgstab"])
+@pytest.mark.parametrize("recon_lo", [18, 12])
+def test_config2_mixed_precision_reaches_fp64_tolerance(solver, recon_lo):
+    """fp64 defect correction around fp32 solves must meet the SAME bar as the
+    pure fp64 solve (reading A17): oracle solution within 10*tol, oracle-evaluated true residual < tol."""
+    s, c = from_cfg(2, 8, 18)
+    lo = lq().Context(c["dims"], 4, recon_lo, -1)
+    g_lo = lo.gauge_pack(lo.to_device(s.U))
+    A_lo, Ai_lo = lo.clover_build(g_lo, c["csw"], c["kappa"])
+    b = synth.source(c["dims"], "z2", c["src_seed"])
+    xo, ro = s.orc.invert(b, 1e-12, 2000, "bicgstab", 0)
+    x, res = s.ctx.invert_mixed(lo, s.ctx.to_device(b), s.gauge, s.A, s.Ai, g_lo, A_lo, Ai_lo, s.kappa,
+                                tol=1e-10, inner_tol=1e-4, maxiter=2000, solver=solver)
+    assert res.status == 0, res.as_dict()
+    xg = x.cpu().numpy()
+    true = s.orc.true_residual(b, xg)
+    assert true < 1e-10 and abs(true - res.true_resid) < 5e-11, (true, res.as_dict())
+    assert rel_err(xg, xo) < 1e-9
+    # a tolerance below the fp32 floor of the inner solver is still reached (more outer steps)
+    x2, res2 = s.ctx.invert_mixed(lo, s.ctx.to_device(b), s.gauge, s.A, s.Ai, g_lo, A_lo, Ai_lo, s.kappa,
+                                  tol=1e-13, inner_tol=1e-3, maxiter=4000, solver=solver)
+    assert res2.status == 0 and s.orc.true_residual(b, x2.cpu().numpy()) < 1e-13
+    # argument checks: contexts swapped / same precision
+    with pytest.raises(lq().LqcdError):
+        s.ctx.invert_mixed(s.ctx, s.ctx.to_device(b), s.gauge, s.A, s.Ai, s.gauge, s.A, s.Ai, s.kappa)
