@@ -46,6 +46,8 @@ def lib():
         L.orc_create.argtypes = [ctypes.POINTER(ci), ci, vp]
         L.orc_destroy.argtypes = [vp]
         L.orc_set_clover.argtypes = [vp, cd, cd]
+        L.orc_set_anisotropy.argtypes = [vp, cd]
+        L.orc_set_clover_aniso.argtypes = [vp, cd, cd, cd]
         L.orc_clover_defect.restype = cd
         L.orc_clover_defect.argtypes = [vp]
         L.orc_get_clover.argtypes = [vp, vp, vp]
@@ -115,6 +117,18 @@ class Oracle:
 
     def set_clover(self, kappa, csw):
         rc = lib().orc_set_clover(self._h, float(kappa), float(csw))
+        if rc != 0:
+            raise ArithmeticError("singular clover block")
+        return self
+
+    def set_anisotropy(self, nu_over_xi0):
+        """Spatial hop weight nu/xi_0 of Eq. 5; the temporal weight is 1."""
+        lib().orc_set_anisotropy(self._h, float(nu_over_xi0))
+        return self
+
+    def set_clover_aniso(self, kappa, csw_s, csw_t):
+        """A with csw_s = c_SW^r/xi_0 on the spatial planes and csw_t = c_SW^t on the temporal ones."""
+        rc = lib().orc_set_clover_aniso(self._h, float(kappa), float(csw_s), float(csw_t))
         if rc != 0:
             raise ArithmeticError("singular clover block")
         return self

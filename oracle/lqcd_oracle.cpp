@@ -2,7 +2,8 @@
 //
 // A plain, slow, obviously-correct fp64 implementation of the Wilson-clover operator
 //     M = A - kappa*D,   A = 1 - kappa*csw*sum_{mu<nu} sigma_{mu nu} (x) F_{mu nu}
-// (Eq. 5, isotropic case xi_0 = nu = 1, c_SW^t = c_SW^r, kappa normalisation:
+// (Eq. 5; isotropic by default, the anisotropic weights nu/xi_0, c_SW^t, c_SW^r/xi_0
+// through orc_set_anisotropy / orc_set_clover_aniso; kappa normalisation:
 // the paper's a_t*M is this M/(2 kappa)), its even-odd Schur forms and CG / BiCGStab, written
 // from the definitions in SURVEY.md §8(c) O1-O9 (the paper states conventions only:
 // DeGrand-Rossi basis and cb2 layouts; BiCGStab/CG).
@@ -177,7 +178,10 @@ static void m3_path(const cplx* a, bool da, const cplx* b, bool db, const cplx* 
 // (both use U_t(., Lt-1)) get a factor -1.  only_parity = 0/1 restricts the OUTPUT sites to that
 // parity (other output sites are set to zero); -1 = all sites.
 // ---------------------------------------------------------------------------------------------
-static void hop(const Geom& g, int tb, const cplx* U, const cplx* in, cplx* out, int dagger, int only_parity) {
+// w[mu]: weight of the hops in direction mu (Eq. 5: gamma_4 W_4 + (nu/xi_0) sum_i
+// gamma_i W_i, i.e. w = (nu/xi_0, nu/xi_0, nu/xi_0, 1); isotropic: all 1).
+static void hop(const Geom& g, int tb, const cplx* U, const cplx* in, cplx* out, int dagger, int only_parity,
+                const double* w) {
   const double sgn = dagger ? -1.0 : 1.0;
 #pragma omp parallel for schedule(static)
   for (long l = 0; l < g.V; l++) {
@@ -206,7 +210,7 @@ static void hop(const Geom& g, int tb, const cplx* U, const cplx* in, cplx* out,
               cplx v = up[s][a];
               for (int s2 = 0; s2 < 4; s2++)
                 if (GM.g[mu][s][s2] != 0.0) v -= sgn * GM.g[mu][s][s2] * up[s2][a];
-              acc[s][a] += bsign * v;
+              acc[s][a] += w[mu] * bsign * v;
             }
         }
         // backward: (1 + sgn*g_mu) U_mu^dag(x-mu) psi(x-mu)
@@ -227,7 +231,7 @@ static void hop(const Geom& g, int tb, const cplx* U, const cplx* in, cplx* out,
               cplx v = up[s][a];
               for (int s2 = 0; s2 < 4; s2++)
                 if (GM.g[mu][s][s2] != 0.0) v += sgn * GM.g[mu][s][s2] * up[s2][a];
-              acc[s][a] += bsign * v;
+              acc[s][a] += w[mu] * bsign * v;
             }
         }
       }
@@ -267,7 +271,10 @@ static void field_strength(const Geom& g, const cplx* U, long l, int mu, int nu,
 }
 
 // O5: dense 12x12 clover matrix at one site, row/col index = 3*spin + colour
-static void clover_dense_site(const Geom& g, const cplx* U, long l, double kappa, double csw, cplx* A /*144*/) {
+// csw = coefficient of the spatial planes (Eq. 5: c_SW^r/xi_0), csw_t = of the temporal planes
+// (c_SW^t); isotropic: csw_t = csw.
+static void clover_dense_site(const Geom& g, const cplx* U, long l, double kappa, double csw, double csw_t,
+                              cplx* A /*144*/) {
   for (int e = 0; e < 144; e++) A[e] = 0;
   for (int i = 0; i < 12; i++) A[13 * i] = 1.0;
   for (int mu = 0; mu < 4; mu++)
@@ -279,7 +286,8 @@ static void clover_dense_site(const Geom& g, const cplx* U, long l, double kappa
           cplx sg = GM.sig[mu][nu][s][s2];
           if (sg == 0.0) continue;
           for (int a = 0; a < 3; a++)
-            for (int b = 0; b < 3; b++) A[(3 * s + a) * 12 + (3 * s2 + b)] -= kappa * csw * sg * F[3 * a + b];
+            for (int b = 0; b < 3; b++)
+              A[(3 * s + a) * 12 + (3 * s2 + b)] -= kappa * (nu == 3 ? csw_t : csw) * sg * F[3 * a + b];
         }
     }
 }
@@ -307,12 +315,12 @@ static void unpack_block(const double* p, cplx* B) {
 
 // Build the packed clover field in lex order: [V][2][36].  Returns the largest magnitude found in
 // the off-diagonal chiral 6x6 blocks and the largest anti-Hermitian part (both must be ~0).
-static double clover_build_lex(const Geom& g, const cplx* U, double kappa, double csw, double* Apk) {
+static double clover_build_lex(const Geom& g, const cplx* U, double kappa, double csw, double csw_t, double* Apk) {
   double worst = 0;
 #pragma omp parallel for schedule(static) reduction(max : worst)
   for (long l = 0; l < g.V; l++) {
     cplx A[144], B[36];
-    clover_dense_site(g, U, l, kappa, csw, A);
+    clover_dense_site(g, U, l, kappa, csw, csw_t, A);
     for (int i = 0; i < 6; i++)
       for (int j = 0; j < 6; j++) {
         worst = std::max(worst, std::abs(A[i * 12 + 6 + j]));
@@ -406,6 +414,7 @@ struct Problem {
   Geom g;
   int tb;
   double kappa, csw, defect;
+  double w[4];                     // hop weights per direction (anisotropy); 1 = isotropic
   std::vector<cplx> U;             // [4][V][9]
   std::vector<double> A, Ainv;     // [V][2][36]
   long hops;                       // number of single-parity hop sweeps executed (full = 2)
@@ -414,7 +423,7 @@ struct Problem {
 typedef std::vector<cplx> Field;
 
 static void op_hop(Problem& P, const Field& in, Field& out, int dagger, int only_parity) {
-  hop(P.g, P.tb, P.U.data(), in.data(), out.data(), dagger, only_parity);
+  hop(P.g, P.tb, P.U.data(), in.data(), out.data(), dagger, only_parity, P.w);
   P.hops += (only_parity < 0) ? 2 : 1;
 }
 
@@ -646,6 +655,7 @@ void* orc_create(const int* dims, int t_boundary, const double* U_public) {
   }
   P->tb = t_boundary;
   P->kappa = 0; P->csw = 0; P->defect = 0; P->hops = 0;
+  for (int mu = 0; mu < 4; mu++) P->w[mu] = 1.0;
   P->U.resize((size_t)4 * P->g.V * 9);
   gauge_to_lex(P->g, reinterpret_cast<const cplx*>(U_public), P->U.data());
   return P;
@@ -660,7 +670,25 @@ int orc_set_clover(void* h, double kappa, double csw) {
   P.csw = csw;
   P.A.assign((size_t)P.g.V * 72, 0.0);
   P.Ainv.assign((size_t)P.g.V * 72, 0.0);
-  P.defect = clover_build_lex(P.g, P.U.data(), kappa, csw, P.A.data());
+  P.defect = clover_build_lex(P.g, P.U.data(), kappa, csw, csw, P.A.data());
+  return clover_invert_lex(P.g, P.A.data(), P.Ainv.data()) ? 0 : -6;
+}
+// Anisotropic operator of Eq. 5 in kappa normalisation:
+//   M = 1 - kappa [ D_t + (nu/xi_0) sum_i D_i ] - kappa [ c_SW^t sum_i sigma_i4 F_i4 + (c_SW^r/xi_0) sum_{i<j} sigma_ij F_ij ]
+// orc_set_anisotropy fixes the spatial hop weight nu/xi_0 for every later operator call;
+// orc_set_clover_aniso builds A with separate spatial (csw_s = c_SW^r/xi_0) and temporal (csw_t) coefficients.
+void orc_set_anisotropy(void* h, double nu_over_xi0) {
+  Problem& P = *static_cast<Problem*>(h);
+  P.w[0] = P.w[1] = P.w[2] = nu_over_xi0;
+  P.w[3] = 1.0;
+}
+int orc_set_clover_aniso(void* h, double kappa, double csw_s, double csw_t) {
+  Problem& P = *static_cast<Problem*>(h);
+  P.kappa = kappa;
+  P.csw = csw_s;
+  P.A.assign((size_t)P.g.V * 72, 0.0);
+  P.Ainv.assign((size_t)P.g.V * 72, 0.0);
+  P.defect = clover_build_lex(P.g, P.U.data(), kappa, csw_s, csw_t, P.A.data());
   return clover_invert_lex(P.g, P.A.data(), P.Ainv.data()) ? 0 : -6;
 }
 // largest |entry| of the off-diagonal chiral blocks / anti-Hermitian part seen by the last build
@@ -693,14 +721,14 @@ void orc_clover_dense(void* h, double kappa, double csw, double* out) {
   Problem& P = *static_cast<Problem*>(h);
   cplx* o = reinterpret_cast<cplx*>(out);
 #pragma omp parallel for schedule(static)
-  for (long l = 0; l < P.g.V; l++) clover_dense_site(P.g, P.U.data(), l, kappa, csw, o + P.g.cb(l) * 144);
+  for (long l = 0; l < P.g.V; l++) clover_dense_site(P.g, P.U.data(), l, kappa, csw, csw, o + P.g.cb(l) * 144);
 }
 // dense clover at ONE site given by its public index (parity*Vh + cb); for sampled checks at size
 void orc_clover_dense_site(void* h, double kappa, double csw, long public_index, double* out) {
   Problem& P = *static_cast<Problem*>(h);
   long par = public_index / P.g.Vh, c = public_index % P.g.Vh;
   for (long l = 2 * c; l < 2 * c + 2; l++)
-    if (P.g.parity(l) == par) clover_dense_site(P.g, P.U.data(), l, kappa, csw, reinterpret_cast<cplx*>(out));
+    if (P.g.parity(l) == par) clover_dense_site(P.g, P.U.data(), l, kappa, csw, csw, reinterpret_cast<cplx*>(out));
 }
 
 // F_{mu nu}(x) for all sites: [2][Vh][3][3] complex
@@ -751,7 +779,7 @@ void orc_dslash_site(void* h, const double* in_public, long public_index, int da
         for (int a = 0; a < 3; a++) {
           cplx v = up[s][a];
           for (int s2 = 0; s2 < 4; s2++) v += gs * GM.g[mu][s][s2] * up[s2][a];
-          acc[3 * s + a] += bs * v;
+          acc[3 * s + a] += P.w[mu] * bs * v;
         }
     }
   std::memcpy(out, acc, sizeof(acc));
