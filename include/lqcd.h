@@ -100,6 +100,19 @@ int lqcd_clover_unpack(lqcd_ctx* ctx, void* clover_public, const void* clover_na
 int lqcd_clover_build(lqcd_ctx* ctx, void* clover, void* clover_inv, const void* gauge, double csw,
                       double kappa, void* stream);
 
+/* Anisotropic operator of PAPER.md:218-221, Eq. 5, in kappa normalisation:
+ *     M = 1 - kappa [ D_t + (nu/xi_0) sum_i D_i ]
+ *           - kappa [ c_SW^t sum_i sigma_i4 F_i4 + (c_SW^r/xi_0) sum_{i<j} sigma_ij F_ij ],   1/kappa = 2(m0 + 1 + 3 nu/xi_0)
+ * lqcd_set_anisotropy fixes the weight nu/xi_0 (> 0; default 1 = isotropic) of the spatial hops for
+ * every later dslash / mpc_apply / mat_apply / invert* call of this context (the temporal hops keep
+ * weight 1 and the boundary sign).  lqcd_clover_build_aniso is lqcd_clover_build with
+ * csw_s = c_SW^r/xi_0 on the planes xy, xz, yz and csw_t = c_SW^t on xt, yt, zt.  Raw (unscaled)
+ * SU(3) links are passed in both cases: no "fake anisotropy" is applied to the gauge field
+ * (PAPER.md:100-102 describes that workaround for QUDA). */
+int lqcd_set_anisotropy(lqcd_ctx* ctx, double nu_over_xi0);
+int lqcd_clover_build_aniso(lqcd_ctx* ctx, void* clover, void* clover_inv, const void* gauge, double csw_s,
+                            double csw_t, double kappa, void* stream);
+
 /* out = C in on one parity, C = the two Hermitian 6x6 chiral blocks per site of `clover_or_inv`
  * (PAPER.md:56).  in/out: one-parity native spinors; they may alias. */
 int lqcd_clover_apply(lqcd_ctx* ctx, void* out, const void* in, const void* clover_or_inv, int parity,

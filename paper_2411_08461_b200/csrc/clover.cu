@@ -7,6 +7,7 @@
 //   sigma_{mu nu} is block diagonal, so with  E3 = F_xy -/+ F_zt, E2 = F_xz +/- F_yt,
 //   E1 = F_yz -/+ F_xt  (upper sign: spins 0,1; lower sign: spins 2,3)
 //   A_block = 1 - kappa*csw * [[E3, E1 - i E2], [E1 + i E2, -E3]],  row index = 3*spin + colour.
+//   Anisotropic form (Eq. 5): csw -> c_SW^r/xi_0 on the planes xy, xz, yz and c_SW^t on xt, yt, zt.
 #include "lqcd_internal.cuh"
 
 struct cd {
@@ -151,7 +152,7 @@ __device__ __forceinline__ void store_block(T* __restrict__ field, int Vh, int i
 
 template <typename T, int R>
 __global__ void __launch_bounds__(64) clover_build_kernel(T* __restrict__ clover, T* __restrict__ clover_inv,
-                                                          const T* __restrict__ gauge, Lat L, double kc, int* flag) {
+                                                          const T* __restrict__ gauge, Lat L, double kc, double kt, int* flag) {
   const int gid = blockIdx.x * blockDim.x + threadIdx.x;
   if (gid >= 2 * L.Vh) return;
   const int par = gid / L.Vh, idx = gid % L.Vh;
@@ -170,14 +171,16 @@ __global__ void __launch_bounds__(64) clover_build_kernel(T* __restrict__ clover
     for (int i = 0; i < 3; i++)
       for (int j = 0; j < 3; j++) {
         const int e = 3 * i + j;
-        cd E3 = {F[0][e].re - sg * F[5][e].re, F[0][e].im - sg * F[5][e].im};  // F_xy -/+ F_zt
-        cd E2 = {F[1][e].re + sg * F[4][e].re, F[1][e].im + sg * F[4][e].im};  // F_xz +/- F_yt
-        cd E1 = {F[3][e].re - sg * F[2][e].re, F[3][e].im - sg * F[2][e].im};  // F_yz -/+ F_xt
+        // kc = kappa*csw on the spatial planes, kt = kappa*csw_t on the temporal ones (Eq. 5)
+        const double st = sg * kt;
+        cd E3 = {kc * F[0][e].re - st * F[5][e].re, kc * F[0][e].im - st * F[5][e].im};  // kc F_xy -/+ kt F_zt
+        cd E2 = {kc * F[1][e].re + st * F[4][e].re, kc * F[1][e].im + st * F[4][e].im};  // kc F_xz +/- kt F_yt
+        cd E1 = {kc * F[3][e].re - st * F[2][e].re, kc * F[3][e].im - st * F[2][e].im};  // kc F_yz -/+ kt F_xt
         const double d = (i == j) ? 1.0 : 0.0;
-        B[i][j] = {d - kc * E3.re, -kc * E3.im};
-        B[3 + i][3 + j] = {d + kc * E3.re, kc * E3.im};
-        B[i][3 + j] = {-kc * (E1.re + E2.im), -kc * (E1.im - E2.re)};      // E1 - i E2
-        B[3 + i][j] = {-kc * (E1.re - E2.im), -kc * (E1.im + E2.re)};      // E1 + i E2
+        B[i][j] = {d - E3.re, -E3.im};
+        B[3 + i][3 + j] = {d + E3.re, E3.im};
+        B[i][3 + j] = {-(E1.re + E2.im), -(E1.im - E2.re)};      // E1 - i E2
+        B[3 + i][j] = {-(E1.re - E2.im), -(E1.im + E2.re)};      // E1 + i E2
       }
     double pk[36];
     for (int i = 0; i < 6; i++) pk[i] = B[i][i].re;
@@ -213,27 +216,32 @@ __global__ void __launch_bounds__(64) clover_build_kernel(T* __restrict__ clover
   }
 }
 
-extern "C" int lqcd_clover_build(lqcd_ctx* c, void* clover, void* clover_inv, const void* gauge, double csw,
-                                 double kappa, void* stream) {
+extern "C" int lqcd_clover_build_aniso(lqcd_ctx* c, void* clover, void* clover_inv, const void* gauge, double csw_s,
+                                       double csw_t, double kappa, void* stream) {
   if (!c || !clover || !gauge) return LQCD_ERR_INVALID_ARG;
   if (!lqcd_aligned16(clover) || !lqcd_aligned16(clover_inv) || !lqcd_aligned16(gauge))
     return lqcd_set_error(c, LQCD_ERR_ALIGN, "clover_build: alignment");
   cudaStream_t st = as_stream(stream);
   const int n = 2 * c->lat.Vh, block = 64, grid = (n + block - 1) / block;
-  const double kc = kappa * csw;
+  const double kc = kappa * csw_s, kt = kappa * csw_t;
   cudaMemsetAsync(c->d_flag, 0, sizeof(int), st);
   c->alg_bytes += (double)lqcd_gauge_bytes(c) + (clover_inv ? 2.0 : 1.0) * (double)lqcd_clover_bytes(c);
   if (c->prec == 4 && c->recon == 18)
-    clover_build_kernel<float, 18><<<grid, block, 0, st>>>((float*)clover, (float*)clover_inv, (const float*)gauge, c->lat, kc, c->d_flag);
+    clover_build_kernel<float, 18><<<grid, block, 0, st>>>((float*)clover, (float*)clover_inv, (const float*)gauge, c->lat, kc, kt, c->d_flag);
   else if (c->prec == 4)
-    clover_build_kernel<float, 12><<<grid, block, 0, st>>>((float*)clover, (float*)clover_inv, (const float*)gauge, c->lat, kc, c->d_flag);
+    clover_build_kernel<float, 12><<<grid, block, 0, st>>>((float*)clover, (float*)clover_inv, (const float*)gauge, c->lat, kc, kt, c->d_flag);
   else if (c->recon == 18)
-    clover_build_kernel<double, 18><<<grid, block, 0, st>>>((double*)clover, (double*)clover_inv, (const double*)gauge, c->lat, kc, c->d_flag);
+    clover_build_kernel<double, 18><<<grid, block, 0, st>>>((double*)clover, (double*)clover_inv, (const double*)gauge, c->lat, kc, kt, c->d_flag);
   else
-    clover_build_kernel<double, 12><<<grid, block, 0, st>>>((double*)clover, (double*)clover_inv, (const double*)gauge, c->lat, kc, c->d_flag);
+    clover_build_kernel<double, 12><<<grid, block, 0, st>>>((double*)clover, (double*)clover_inv, (const double*)gauge, c->lat, kc, kt, c->d_flag);
   LQCD_LAUNCH_CHECK(c, "clover_build");
   cudaMemcpyAsync(c->h_flag, c->d_flag, sizeof(int), cudaMemcpyDeviceToHost, st);
   if (cudaStreamSynchronize(st) != cudaSuccess) return lqcd_check_cuda(c, "clover_build sync");
   if (c->h_flag[0]) return lqcd_set_error(c, LQCD_ERR_SINGULAR_CLOVER, "clover_build: singular 6x6 block");
   return LQCD_OK;
+}
+
+extern "C" int lqcd_clover_build(lqcd_ctx* c, void* clover, void* clover_inv, const void* gauge, double csw,
+                                 double kappa, void* stream) {
+  return lqcd_clover_build_aniso(c, clover, clover_inv, gauge, csw, csw, kappa, stream);
 }

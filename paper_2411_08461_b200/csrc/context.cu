@@ -71,6 +71,7 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], int prec, int recon, int t_bo
   c->lat.Vh = (int)(V / 2);
   c->lat.tb = t_boundary;
   c->prec = prec;
+  c->ws = 1.0;
   c->recon = recon;
   c->device = device;
   c->sm_count = prop.multiProcessorCount;
@@ -117,6 +118,12 @@ int lqcd_destroy(lqcd_ctx* c) {
     delete[] c->prof_ev;
   }
   delete c;
+  return LQCD_OK;
+}
+
+int lqcd_set_anisotropy(lqcd_ctx* c, double nu_over_xi0) {
+  if (!c || !(nu_over_xi0 > 0)) return LQCD_ERR_INVALID_ARG;
+  c->ws = nu_over_xi0;
   return LQCD_OK;
 }
 

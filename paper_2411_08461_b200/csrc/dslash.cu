@@ -15,6 +15,7 @@ template <typename T> struct DslashArgs {
   Lat lat;
   int parity;
   T scale;
+  T ws;  // weight of the spatial hops (anisotropy nu/xi_0; 1 = isotropic)
 };
 
 // Launch shape per precision (threads per block, minimum resident blocks per SM = register budget).
@@ -49,9 +50,9 @@ __global__ void __launch_bounds__(Tune<T>::BLOCK, Tune<T>::MINB) dslash_kernel(c
   T acc[24];
   if (Tune<T>::STAGE) {
     extern __shared__ __align__(16) unsigned char dslash_smem[];
-    dslash_site_staged<T, R, DAG, Tune<T>::BLOCK>(acc, a.in, a.gauge, a.lat, idx, a.parity, dslash_smem);
+    dslash_site_staged<T, R, DAG, Tune<T>::BLOCK>(acc, a.in, a.gauge, a.lat, idx, a.parity, dslash_smem, a.ws);
   } else {
-    dslash_site<T, R, DAG>(acc, a.in, a.gauge, a.lat, idx, a.parity);
+    dslash_site<T, R, DAG>(acc, a.in, a.gauge, a.lat, idx, a.parity, a.ws);
   }
   T res[24];
   if (EPI == 0) {
@@ -123,6 +124,7 @@ static void launch_typed(lqcd_ctx* c, void* out, const void* in, const void* gau
   a.lat = c->lat;
   a.parity = parity;
   a.scale = (T)scale;
+  a.ws = (T)c->ws;
   if (c->recon == 18) {
     if (dagger) launch_epi<T, 18, true>(a, epi, st);
     else launch_epi<T, 18, false>(a, epi, st);

@@ -103,10 +103,8 @@ __device__ __forceinline__ void hop(T* acc, const T* __restrict__ in, const T* _
   load_spinor<T>(in, Vh, nidx, psi);
   load_link<T, R>(links, Vh, lidx, U);
   project<T, MU, S>(psi, h);
-  if (MU == 3) {
 #pragma unroll
-    for (int e = 0; e < 12; e++) h[e] *= bsign;
-  }
+  for (int e = 0; e < 12; e++) h[e] *= bsign;  // t: boundary sign; x,y,z: hop weight nu/xi_0 (1 if isotropic)
   su3_mul<T, !FWD>(U, h, chi);
   reconstruct<T, MU, S>(acc, chi);
 }
@@ -114,15 +112,15 @@ __device__ __forceinline__ void hop(T* acc, const T* __restrict__ in, const T* _
 // all eight hops for output site idx of parity par.  gauge = native links [mu][parity][NGV][Vh].
 template <typename T, int R, bool DAG>
 __device__ __forceinline__ void dslash_site(T* acc, const T* __restrict__ in, const T* __restrict__ gauge,
-                                            const Lat& L, int idx, int par) {
+                                            const Lat& L, int idx, int par, T ws) {
   const Site s = site_of(L, idx, par);
   const int Vh = L.Vh;
   const size_t blk = (size_t)R * Vh;  // reals per (mu, parity) link block
 #pragma unroll
   for (int e = 0; e < 24; e++) acc[e] = 0;
-  const T one = 1;
-  const T sf = (L.tb < 0 && s.t == L.Lt - 1) ? -one : one;
-  const T sb = (L.tb < 0 && s.t == 0) ? -one : one;
+  const T one = ws;  // weight of the spatial hops (Eq. 5: nu/xi_0); the temporal hops carry the boundary sign
+  const T sf = (L.tb < 0 && s.t == L.Lt - 1) ? (T)-1 : (T)1;
+  const T sb = (L.tb < 0 && s.t == 0) ? (T)-1 : (T)1;
   int n;
   n = neighbour<0, +1>(L, idx, s);
   hop<T, R, 0, true, DAG>(acc, in, gauge + (0 * 2 + par) * blk, Vh, n, idx, one);
@@ -199,10 +197,8 @@ __device__ __forceinline__ void hop_staged(T* acc, const T* __restrict__ in, con
   T psi[24], U[18], h[12], chi[12];
   load_spinor<T>(in, Vh, nidx, psi);
   project<T, MU, S>(psi, h);
-  if (MU == 3) {
 #pragma unroll
-    for (int e = 0; e < 12; e++) h[e] *= bsign;
-  }
+  for (int e = 0; e < 12; e++) h[e] *= bsign;
   cp_async_wait<7 - SLOT>();
   fetch_link<T, R, BLOCK>(smem, SLOT, U);
   su3_mul<T, !FWD>(U, h, chi);
@@ -211,7 +207,7 @@ __device__ __forceinline__ void hop_staged(T* acc, const T* __restrict__ in, con
 
 template <typename T, int R, bool DAG, int BLOCK>
 __device__ __forceinline__ void dslash_site_staged(T* acc, const T* __restrict__ in, const T* __restrict__ gauge,
-                                                   const Lat& L, int idx, int par, void* smem) {
+                                                   const Lat& L, int idx, int par, void* smem, T ws) {
   const Site s = site_of(L, idx, par);
   const int Vh = L.Vh;
   const size_t blk = (size_t)R * Vh;
@@ -229,9 +225,9 @@ __device__ __forceinline__ void dslash_site_staged(T* acc, const T* __restrict__
   stage_link<T, R, BLOCK>(smem, 7, gauge + (3 * 2 + 1 - par) * blk, Vh, n7);
 #pragma unroll
   for (int e = 0; e < 24; e++) acc[e] = 0;
-  const T one = 1;
-  const T sf = (L.tb < 0 && s.t == L.Lt - 1) ? -one : one;
-  const T sb = (L.tb < 0 && s.t == 0) ? -one : one;
+  const T one = ws;  // weight of the spatial hops (Eq. 5: nu/xi_0); the temporal hops carry the boundary sign
+  const T sf = (L.tb < 0 && s.t == L.Lt - 1) ? (T)-1 : (T)1;
+  const T sb = (L.tb < 0 && s.t == 0) ? (T)-1 : (T)1;
   hop_staged<T, R, 0, true, DAG, BLOCK, 0>(acc, in, smem, Vh, n0, one);
   hop_staged<T, R, 0, false, DAG, BLOCK, 1>(acc, in, smem, Vh, n1, one);
   hop_staged<T, R, 1, true, DAG, BLOCK, 2>(acc, in, smem, Vh, n2, one);

@@ -42,6 +42,7 @@ template <typename T> struct MrhsArgs {
   Lat lat;
   int parity;
   T scale;
+  T ws;           // weight of the spatial hops (anisotropy nu/xi_0)
   size_t stride;  // reals between consecutive right-hand sides (24 * Vh)
   int ngroups;    // nrhs / NB column groups; group g is handled by threadIdx.y = g mod blockDim.y
 };
@@ -77,8 +78,8 @@ __device__ __forceinline__ void hop_mrhs(T (*acc)[24], const T* __restrict__ in,
   constexpr int S = (FWD != DAG) ? -1 : +1;
   T U[18];
   load_link_l1<T, R>(links, Vh, lidx, U);
-  if (MU == 3) {  // antiperiodic seam: flip the link once for all NB columns (after the row-3 rebuild)
-    const T sg = seam ? bsign : (T)1;
+  {  // t: antiperiodic seam; x,y,z: hop weight.  Scale the link once for all NB columns (after the row-3 rebuild)
+    const T sg = (MU == 3) ? (seam ? (T)-1 : (T)1) : bsign;
 #pragma unroll
     for (int e = 0; e < 18; e++) U[e] *= sg;
   }
@@ -153,7 +154,7 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kern
   for (int r = 0; r < NB; r++)
 #pragma unroll
     for (int e = 0; e < 24; e++) acc[r][e] = 0;
-  const T one = 1;
+  const T one = a.ws;
   const bool anti = L.tb < 0;
   const bool seam_f = anti && s.t == L.Lt - 1, seam_b = anti && s.t == 0;
   int n;
@@ -249,6 +250,7 @@ static void launch_mrhs_typed(lqcd_ctx* c, void* out, const void* in, const void
   a.lat = c->lat;
   a.parity = parity;
   a.scale = (T)scale;
+  a.ws = (T)c->ws;
   a.stride = (size_t)24 * c->lat.Vh;
   if (c->recon == 18) {
     if (dagger) launch_mrhs_nb<T, 18, true>(a, epi, nrhs, st);

@@ -22,6 +22,7 @@ struct lqcd_ctx {
   Lat lat;
   long V;
   int prec, recon, device, sm_count;
+  double ws;  // weight of the spatial hops: nu/xi_0 of Eq. 5; 1 = isotropic
   long launches;
   char err[256];
   // reduction scratch (device): per-block partials, ticket counter, result slots; pinned host mirror

@@ -35,7 +35,7 @@ SYMBOLS = [
     "lqcd_invert", "lqcd_host_scratch_bytes", "lqcd_dslash_host", "lqcd_invert_host",
     "lqcd_blas_axpy_norm", "lqcd_blas_xpay", "lqcd_blas_cdot", "lqcd_blas_caxpbypz",
     "lqcd_dslash_mrhs", "lqcd_mpc_apply_mrhs", "lqcd_invert_multi_workspace_bytes", "lqcd_invert_multi",
-    "lqcd_invert_mixed",
+    "lqcd_invert_mixed", "lqcd_set_anisotropy", "lqcd_clover_build_aniso",
 ]
 MAX_RHS = 16
 
@@ -76,6 +76,8 @@ def load():
     for f in ("lqcd_gauge_pack", "lqcd_spinor_pack", "lqcd_spinor_unpack", "lqcd_clover_unpack"):
         getattr(L, f).argtypes = [vp, vp, vp, vp]
     L.lqcd_clover_build.argtypes = [vp, vp, vp, vp, cd, cd, vp]
+    L.lqcd_set_anisotropy.argtypes = [vp, cd]
+    L.lqcd_clover_build_aniso.argtypes = [vp, vp, vp, vp, cd, cd, cd, vp]
     L.lqcd_clover_apply.argtypes = [vp, vp, vp, vp, ci, vp]
     L.lqcd_dslash.argtypes = [vp, vp, vp, vp, ci, cd, ci, vp]
     L.lqcd_mpc_apply.argtypes = [vp, vp, vp, vp, vp, vp, cd, ci, ci, vp, vp]
@@ -220,6 +222,16 @@ class Context:
         A = self.empty(self.clover_bytes)
         Ai = self.empty(self.clover_bytes) if want_inverse else None
         self._check(self.lib.lqcd_clover_build(self.h, _p(A), _p(Ai), _p(gauge), csw, kappa, _stream()))
+        return A, Ai
+
+    def set_anisotropy(self, nu_over_xi0):
+        self._check(self.lib.lqcd_set_anisotropy(self.h, nu_over_xi0))
+        return self
+
+    def clover_build_aniso(self, gauge, csw_s, csw_t, kappa, want_inverse=True):
+        A = self.empty(self.clover_bytes)
+        Ai = self.empty(self.clover_bytes) if want_inverse else None
+        self._check(self.lib.lqcd_clover_build_aniso(self.h, _p(A), _p(Ai), _p(gauge), csw_s, csw_t, kappa, _stream()))
         return A, Ai
 
     def clover_apply(self, out, inp, clover, parity):
