@@ -177,6 +177,58 @@ def dslash_sweep(torch, lqcd, U, psi, dims, device, peak):
     return out
 
 
+def extras(torch, lqcd, synth, U, b, ctx, gauge, device):
+    """SURVEY.md §8(f) rows measured beside the headline (not part of `value`):
+    mixed   : the same 32^3x64 system to the same fp64 tolerance by fp64 defect correction around fp32
+              reconstruct-12 solves (lqcd_invert_mixed), CGNE and BiCGStab;
+    propagator : BASELINE configs[2] (16^3x32, fp32, reconstruct-12): the 12 spin-colour columns of a
+              point-source propagator by CGNE to 1e-6, 12 single solves vs one lqcd_invert_multi."""
+    out = {}
+    cfg = synth.CONFIGS[WORKLOAD]
+    kappa, csw = cfg["kappa"], cfg["csw"]
+    A, Ai = ctx.clover_build(gauge, csw, kappa)
+    lo = lqcd.Context(cfg["dims"], 4, 12, -1, device)
+    g_lo = lo.gauge_pack(lo.to_device(U))
+    A_lo, Ai_lo = lo.clover_build(g_lo, csw, kappa)
+    b_dev = ctx.to_device(b)
+    mixed = {}
+    for solver in ("cgne", "bicgstab"):
+        for _ in range(2):
+            _, r64 = ctx.invert(b_dev, gauge, A, Ai, kappa, tol=1e-10, maxiter=2000, solver=solver)
+            _, rmx = ctx.invert_mixed(lo, b_dev, gauge, A, Ai, g_lo, A_lo, Ai_lo, kappa, tol=1e-10,
+                                      inner_tol=1e-5, maxiter=2000, solver=solver)
+        mixed[solver] = {"fp64_seconds": r64.seconds, "fp64_iterations": r64.iterations,
+                         "mixed_seconds": rmx.seconds, "mixed_inner_iterations": rmx.iterations,
+                         "mixed_true_resid": rmx.true_resid, "fp64_true_resid": r64.true_resid,
+                         "speedup": r64.seconds / rmx.seconds}
+    out["mixed_precision_32x64"] = mixed
+    lo.close()
+    del A, Ai, g_lo, A_lo, Ai_lo
+    c3 = synth.CONFIGS[3]
+    dims = c3["dims"]
+    U3 = synth.gauge(dims, c3["eps"], c3["seed"])
+    p = lqcd.Context(dims, 4, 12, -1, device)
+    g3 = p.gauge_pack(p.to_device(U3))
+    A3, Ai3 = p.clover_build(g3, c3["csw"], c3["kappa"])
+    cols = np.stack([synth.source(dims, "point", spin=sp, colour=c) for sp in range(4) for c in range(3)])
+    B = p.to_device(cols)
+    for _ in range(2):
+        e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        e0.record()
+        its = [p.invert(B[j], g3, A3, Ai3, c3["kappa"], tol=1e-6, solver="cgne")[1].iterations for j in range(12)]
+        e1.record()
+        _, rs, rc = p.invert_multi(B, g3, A3, Ai3, c3["kappa"], tol=1e-6, solver="cgne")
+        e2.record()
+        torch.cuda.synchronize()
+    out["propagator_16x32_fp32_recon12"] = {
+        "single_solves_ms": e0.elapsed_time(e1), "batched_ms": e1.elapsed_time(e2),
+        "speedup": e0.elapsed_time(e1) / e1.elapsed_time(e2), "iterations_single": its,
+        "iterations_batched": [r.iterations for r in rs], "status": rc,
+        "worst_true_resid": max(r.true_resid for r in rs)}
+    p.close()
+    return out
+
+
 def reduce_over_ranks(dist, dt, sums, device):
     """Multi-replica aggregation: MAX of the device time over ranks, SUM of the work counters.
     dist = torch.distributed (initialised) or None for a single process."""
@@ -295,7 +347,7 @@ def run_gpu(args):
         "roofline": {"bound": "hbm", "achieved": ds_bytes / (ds_ms * 1e-3) / 1e9 if ds_ms > 0 else None,
                      "peak": peak, "unit": "GB/s",
                      "frac": (ds_bytes / (ds_ms * 1e-3) / 1e9 / peak) if ds_ms > 0 else None,
-                     "traffic": TRAFFIC_BYTES_PER_LAUNCH, "kernel": "dslash_kernel<double,18,*,EPI 1|2> (fused clover epilogues)",
+                     "traffic": traffic_from_profile(), "kernel": "dslash_kernel<double,18,*,EPI 1|2> (fused clover epilogues)",
                      "launches_timed": n_ds, "avg_launch_us": ds_ms * 1e3 / max(n_ds, 1),
                      "alg_bytes_per_launch": ds_bytes / max(n_ds, 1), "peak_source": peak_src,
                      "frac_of_8TBps": (ds_bytes / (ds_ms * 1e-3) / 8e12) if ds_ms > 0 else None},
@@ -306,6 +358,8 @@ def run_gpu(args):
     }
     if rank == 0 and not args.no_sweep:
         line["dslash"] = dslash_sweep(torch, lqcd, U, b, dims, local, peak)
+    if rank == 0 and world == 1 and not args.no_extras:
+        line["next_rows"] = extras(torch, lqcd, synth, U, b, ctx, gauge, local)
     if rank == 0 and world == 1 and not args.no_cpu:
         gbs, ms, cores = oracle_sample(12, 0)
         line["cpu_baseline"] = {"value": gbs, "unit": "GB/s", "cores": cores, "kind": "oracle",
@@ -318,9 +372,25 @@ def run_gpu(args):
     return 0
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
-# ncu --set full capture (profiles/), or None until one exists
-TRAFFIC_BYTES_PER_LAUNCH = None
+def traffic_from_profile():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (fp64 dslash
+    with fused clover epilogue) from the committed `ncu --set full` raw page under profiles/
+    (newest round first), averaged over the captured launches; None if no capture is committed."""
+    import csv
+    import glob
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_dslash_full_raw.csv")), reverse=True):
+        try:
+            rows = list(csv.reader(open(path)))
+            hdr, units = rows[0], rows[1]
+            ik, ir, iw = hdr.index("Kernel Name"), hdr.index("dram__bytes_read.sum"), hdr.index("dram__bytes_write.sum")
+            scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+            tot = [float(r[ir]) * scale[units[ir]] + float(r[iw]) * scale[units[iw]]
+                   for r in rows[2:] if r[ik].startswith("void dslash_kernel<double, 18")]
+            if tot:
+                return sum(tot) / len(tot)
+        except Exception:
+            continue
+    return None
 
 
 def main():
@@ -330,6 +400,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-sweep", action="store_true", help="skip the standalone dslash sweep")
+    ap.add_argument("--no-extras", action="store_true", help="skip the SURVEY 8(f) rows (mixed precision, batched propagator)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the CPU-oracle baseline leg")
     args = ap.parse_args()
     if args.impl == "reference":
