@@ -177,6 +177,40 @@ def dslash_sweep(torch, lqcd, U, psi, dims, device, peak):
     return out
 
 
+def mrhs_sweep(torch, lqcd, U, psi, dims, device, peak, nrhs=12):
+    """Standalone multi-RHS dslash (lqcd_dslash_mrhs, 12 columns) at the workload size.  Algorithmic
+    bytes per site: links once for all columns, every column's input and output once:
+    (8R + nrhs*48)*w.  Reported per column beside the single-RHS time of the same variant."""
+    out = {}
+    for prec, recon in ((4, 18), (4, 12), (8, 18), (8, 12)):
+        ctx = lqcd.Context(dims, prec, recon, -1, device)
+        g = ctx.gauge_pack(ctx.to_device(U))
+        nat = ctx.spinor_pack(ctx.to_device(psi))
+        n = ctx.spinor_bytes // prec
+        src = [torch.cat([ctx.parity(nat, p)] * nrhs) for p in (0, 1)]
+        dst = ctx.new_spinor(nrhs)
+        for i in range(4):
+            ctx.dslash_mrhs(dst, src[1 - (i & 1)], g, i & 1, nrhs)
+        torch.cuda.synchronize()
+        ts = []
+        for i in range(20):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ctx.dslash_mrhs(dst, src[1 - (i & 1)], g, i & 1, nrhs)
+            e1.record()
+            e1.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e-3)
+        t = float(np.median(ts))
+        by = (8 * recon + nrhs * 48) * prec * ctx.Vh
+        out["fp%d_recon%d" % (8 * prec, recon)] = {
+            "nrhs": nrhs, "us": t * 1e6, "us_per_column": t * 1e6 / nrhs, "GBps": by / t / 1e9,
+            "frac_of_measured_peak": by / t / 1e9 / peak, "GFLOPs": FLOPS_PER_SITE * ctx.Vh * nrhs / t / 1e9,
+            "bytes_per_site_and_column": by / ctx.Vh / nrhs}
+        ctx.close()
+        del g, nat, src, dst
+    return out
+
+
 def extras(torch, lqcd, synth, U, b, ctx, gauge, device):
     """SURVEY.md §8(f) rows measured beside the headline (not part of `value`):
     mixed   : the same 32^3x64 system to the same fp64 tolerance by fp64 defect correction around fp32
@@ -360,6 +394,7 @@ def run_gpu(args):
         line["dslash"] = dslash_sweep(torch, lqcd, U, b, dims, local, peak)
     if rank == 0 and world == 1 and not args.no_extras:
         line["next_rows"] = extras(torch, lqcd, synth, U, b, ctx, gauge, local)
+        line["next_rows"]["dslash_mrhs_32x64"] = mrhs_sweep(torch, lqcd, U, b, dims, local, peak)
     if rank == 0 and world == 1 and not args.no_cpu:
         gbs, ms, cores = oracle_sample(12, 0)
         line["cpu_baseline"] = {"value": gbs, "unit": "GB/s", "cores": cores, "kind": "oracle",

@@ -107,33 +107,71 @@ __device__ void field_strength(const T* __restrict__ g, const Lat& L, const int*
     }
 }
 
-// Gauss-Jordan with partial pivoting on a 6x6 complex matrix held row-major in a[6][12] = [A | 1].
-// Returns false when a pivot is below 1e-12 * max|A|.
-__device__ bool invert6(cd (*a)[12]) {
+// In-place Gauss-Jordan inverse with partial (row) pivoting of a 6x6 complex matrix (SURVEY.md §8(c)
+// O6: no positive-definiteness assumed).  Every loop is unrolled with compile-time indices and the
+// run-time pivot row only enters comparisons, so the 36 complex numbers stay in registers (the first
+// version kept [A | 1] in local memory and spent 60 % of the build there).  Row swaps are recorded and
+// undone as column swaps at the end.  Returns false when a pivot is below 1e-12 * max|A|.
+__device__ __forceinline__ bool invert6(cd (&a)[6][6]) {
   double nrm = 0;
+#pragma unroll
   for (int i = 0; i < 6; i++)
+#pragma unroll
     for (int j = 0; j < 6; j++) nrm = fmax(nrm, abs2(a[i][j]));
   const double thresh = 1e-24 * nrm;
+  int perm[6];
+  bool ok = true;
+#pragma unroll
   for (int c = 0; c < 6; c++) {
     int piv = c;
     double best = abs2(a[c][c]);
+#pragma unroll
     for (int r = c + 1; r < 6; r++) {
-      double v = abs2(a[r][c]);
+      const double v = abs2(a[r][c]);
       if (v > best) { best = v; piv = r; }
     }
-    if (best <= thresh) return false;
-    if (piv != c)
-      for (int j = 0; j < 12; j++) { cd t = a[piv][j]; a[piv][j] = a[c][j]; a[c][j] = t; }
+    ok = ok && (best > thresh);
+    perm[c] = piv;
+#pragma unroll
+    for (int r = c + 1; r < 6; r++) {
+      const bool sw = (piv == r);
+#pragma unroll
+      for (int j = 0; j < 6; j++) {
+        const cd t = a[c][j], u = a[r][j];
+        a[c][j] = sw ? u : t;
+        a[r][j] = sw ? t : u;
+      }
+    }
     const cd p = a[c][c];
-    const cd inv = {p.re / best, -p.im / best};
-    for (int j = 0; j < 12; j++) a[c][j] = a[c][j] * inv;
+    const double ib = best > 0.0 ? 1.0 / best : 0.0;
+    const cd inv = {p.re * ib, -p.im * ib};
+    a[c][c] = {1.0, 0.0};
+#pragma unroll
+    for (int j = 0; j < 6; j++) a[c][j] = a[c][j] * inv;
+#pragma unroll
     for (int r = 0; r < 6; r++) {
       if (r == c) continue;
       const cd f = a[r][c];
-      for (int j = 0; j < 12; j++) a[r][j] = a[r][j] - f * a[c][j];
+      a[r][c] = {0.0, 0.0};
+#pragma unroll
+      for (int j = 0; j < 6; j++) a[r][j] = a[r][j] - f * a[c][j];
     }
   }
-  return true;
+  // (P A)^-1 = A^-1 P^T: undo the row swaps as column swaps, last first
+#pragma unroll
+  for (int c = 5; c >= 0; c--) {
+#pragma unroll
+    for (int r = c + 1; r < 6; r++) {
+      const bool sw = (perm[c] == r);
+#pragma unroll
+      for (int i = 0; i < 6; i++) {
+        const cd t = a[i][c], u = a[i][r];
+        a[i][c] = sw ? u : t;
+        a[i][r] = sw ? t : u;
+      }
+    }
+  }
+  return ok;
 }
 
 template <typename T>
@@ -150,22 +188,38 @@ __device__ __forceinline__ void store_block(T* __restrict__ field, int Vh, int i
   }
 }
 
+// Thread layout: blockDim = (CB_SITES sites, 6 planes).  Phase 1: thread (s, pl) computes F of plane pl
+// at site s (4 leaves, 12 matrix products, 16 link loads) and parks it in shared memory, so the six
+// planes of a site run in parallel and no thread holds more than one F.  Phase 2: threads (s, k < 2)
+// assemble chiral block k, pack it, invert it by Gauss-Jordan and store both.
+constexpr int CB_SITES = 32;
+#ifndef CB_MINB
+#define CB_MINB 1
+#endif
 template <typename T, int R>
-__global__ void __launch_bounds__(64) clover_build_kernel(T* __restrict__ clover, T* __restrict__ clover_inv,
-                                                          const T* __restrict__ gauge, Lat L, double kc, double kt, int* flag) {
-  const int gid = blockIdx.x * blockDim.x + threadIdx.x;
-  if (gid >= 2 * L.Vh) return;
-  const int par = gid / L.Vh, idx = gid % L.Vh;
-  const Site s = site_of(L, idx, par);
-  const int x0[4] = {2 * s.xh + s.r, s.y, s.z, s.t};
-  cd F[6][9];  // planes xy, xz, xt, yz, yt, zt
-  {
-    int pl = 0;
-    for (int mu = 0; mu < 4; mu++)
-      for (int nu = mu + 1; nu < 4; nu++) field_strength<T, R>(gauge, L, x0, mu, nu, F[pl++]);
+__global__ void __launch_bounds__(CB_SITES * 6, CB_MINB) clover_build_kernel(T* __restrict__ clover, T* __restrict__ clover_inv,
+                                                                    const T* __restrict__ gauge, Lat L, double kc,
+                                                                    double kt, int* flag) {
+  __shared__ cd Fs[6][9][CB_SITES];  // planes xy, xz, xt, yz, yt, zt
+  const int ls = threadIdx.x, pl = threadIdx.y;
+  const int gid = blockIdx.x * CB_SITES + ls;
+  const bool live = gid < 2 * L.Vh;
+  const int par = live ? gid / L.Vh : 0, idx = live ? gid % L.Vh : 0;
+  if (live) {
+    const Site s = site_of(L, idx, par);
+    const int x0[4] = {2 * s.xh + s.r, s.y, s.z, s.t};
+    const int mu = pl < 3 ? 0 : (pl < 5 ? 1 : 2);
+    const int nu = pl < 3 ? pl + 1 : (pl < 5 ? pl - 1 : 3);
+    cd F[9];
+    field_strength<T, R>(gauge, L, x0, mu, nu, F);
+#pragma unroll
+    for (int e = 0; e < 9; e++) Fs[pl][e][ls] = F[e];
   }
+  __syncthreads();
+  if (!live || pl >= 2) return;
   const size_t half = (size_t)72 * L.Vh;  // reals per parity of a clover field
-  for (int k = 0; k < 2; k++) {
+  {
+    const int k = pl;
     const double sg = k == 0 ? 1.0 : -1.0;
     cd B[6][6];
     for (int i = 0; i < 3; i++)
@@ -173,9 +227,11 @@ __global__ void __launch_bounds__(64) clover_build_kernel(T* __restrict__ clover
         const int e = 3 * i + j;
         // kc = kappa*csw on the spatial planes, kt = kappa*csw_t on the temporal ones (Eq. 5)
         const double st = sg * kt;
-        cd E3 = {kc * F[0][e].re - st * F[5][e].re, kc * F[0][e].im - st * F[5][e].im};  // kc F_xy -/+ kt F_zt
-        cd E2 = {kc * F[1][e].re + st * F[4][e].re, kc * F[1][e].im + st * F[4][e].im};  // kc F_xz +/- kt F_yt
-        cd E1 = {kc * F[3][e].re - st * F[2][e].re, kc * F[3][e].im - st * F[2][e].im};  // kc F_yz -/+ kt F_xt
+        const cd Fxy = Fs[0][e][ls], Fxz = Fs[1][e][ls], Fxt = Fs[2][e][ls], Fyz = Fs[3][e][ls], Fyt = Fs[4][e][ls],
+                 Fzt = Fs[5][e][ls];
+        cd E3 = {kc * Fxy.re - st * Fzt.re, kc * Fxy.im - st * Fzt.im};  // kc F_xy -/+ kt F_zt
+        cd E2 = {kc * Fxz.re + st * Fyt.re, kc * Fxz.im + st * Fyt.im};  // kc F_xz +/- kt F_yt
+        cd E1 = {kc * Fyz.re - st * Fxt.re, kc * Fyz.im - st * Fxt.im};  // kc F_yz -/+ kt F_xt
         const double d = (i == j) ? 1.0 : 0.0;
         B[i][j] = {d - E3.re, -E3.im};
         B[3 + i][3 + j] = {d + E3.re, E3.im};
@@ -193,22 +249,17 @@ __global__ void __launch_bounds__(64) clover_build_kernel(T* __restrict__ clover
       }
     store_block<T>(clover + par * half, L.Vh, idx, k, pk);
     if (clover_inv) {
-      cd a[6][12];
-      for (int i = 0; i < 6; i++)
-        for (int j = 0; j < 6; j++) {
-          a[i][j] = B[i][j];
-          a[i][6 + j] = {i == j ? 1.0 : 0.0, 0.0};
-        }
+      cd (&a)[6][6] = B;  // inverted in place
       if (!invert6(a)) {
         atomicExch(flag, 1);
         for (int i = 0; i < 36; i++) pk[i] = 0;
       } else {
-        for (int i = 0; i < 6; i++) pk[i] = a[i][6 + i].re;
+        for (int i = 0; i < 6; i++) pk[i] = a[i][i].re;
         for (int i = 1; i < 6; i++)
           for (int j = 0; j < i; j++) {
             const int o = 6 + 2 * (i * (i - 1) / 2 + j);
-            pk[o] = 0.5 * (a[i][6 + j].re + a[j][6 + i].re);
-            pk[o + 1] = 0.5 * (a[i][6 + j].im - a[j][6 + i].im);
+            pk[o] = 0.5 * (a[i][j].re + a[j][i].re);
+            pk[o + 1] = 0.5 * (a[i][j].im - a[j][i].im);
           }
       }
       store_block<T>(clover_inv + par * half, L.Vh, idx, k, pk);
@@ -222,7 +273,8 @@ extern "C" int lqcd_clover_build_aniso(lqcd_ctx* c, void* clover, void* clover_i
   if (!lqcd_aligned16(clover) || !lqcd_aligned16(clover_inv) || !lqcd_aligned16(gauge))
     return lqcd_set_error(c, LQCD_ERR_ALIGN, "clover_build: alignment");
   cudaStream_t st = as_stream(stream);
-  const int n = 2 * c->lat.Vh, block = 64, grid = (n + block - 1) / block;
+  const int n = 2 * c->lat.Vh, grid = (n + CB_SITES - 1) / CB_SITES;
+  const dim3 block(CB_SITES, 6);
   const double kc = kappa * csw_s, kt = kappa * csw_t;
   cudaMemsetAsync(c->d_flag, 0, sizeof(int), st);
   c->alg_bytes += (double)lqcd_gauge_bytes(c) + (clover_inv ? 2.0 : 1.0) * (double)lqcd_clover_bytes(c);

@@ -39,18 +39,32 @@ template <typename T> struct DslashArgs {
 #ifndef DSLASH_STAGE_F64
 #define DSLASH_STAGE_F64 0
 #endif
-template <typename T> struct Tune;
-template <> struct Tune<float> { static constexpr int BLOCK = DSLASH_BLOCK_F32, MINB = DSLASH_MINB_F32; static constexpr bool STAGE = DSLASH_STAGE_F32; };
-template <> struct Tune<double> { static constexpr int BLOCK = DSLASH_BLOCK_F64, MINB = DSLASH_MINB_F64; static constexpr bool STAGE = DSLASH_STAGE_F64; };
+#ifndef DSLASH_STAGE_F64_R12
+#define DSLASH_STAGE_F64_R12 1  // cp.async link staging pays for fp64 12-real links only (profiles/r01_tuning.md)
+#endif
+#ifndef DSLASH_MINB_F64_R12
+#define DSLASH_MINB_F64_R12 4
+#endif
+template <typename T, int R> struct Tune;
+#ifndef DSLASH_STAGE_F32_R12
+#define DSLASH_STAGE_F32_R12 0
+#endif
+#ifndef DSLASH_MINB_F32_R12
+#define DSLASH_MINB_F32_R12 DSLASH_MINB_F32
+#endif
+template <> struct Tune<float, 18> { static constexpr int BLOCK = DSLASH_BLOCK_F32, MINB = DSLASH_MINB_F32; static constexpr bool STAGE = DSLASH_STAGE_F32; };
+template <> struct Tune<float, 12> { static constexpr int BLOCK = DSLASH_BLOCK_F32, MINB = DSLASH_MINB_F32_R12; static constexpr bool STAGE = DSLASH_STAGE_F32_R12; };
+template <> struct Tune<double, 18> { static constexpr int BLOCK = DSLASH_BLOCK_F64, MINB = DSLASH_MINB_F64; static constexpr bool STAGE = DSLASH_STAGE_F64; };
+template <> struct Tune<double, 12> { static constexpr int BLOCK = DSLASH_BLOCK_F64, MINB = DSLASH_MINB_F64_R12; static constexpr bool STAGE = DSLASH_STAGE_F64_R12; };
 
 template <typename T, int R, bool DAG, int EPI>
-__global__ void __launch_bounds__(Tune<T>::BLOCK, Tune<T>::MINB) dslash_kernel(const DslashArgs<T> a) {
+__global__ void __launch_bounds__(Tune<T, R>::BLOCK, Tune<T, R>::MINB) dslash_kernel(const DslashArgs<T> a) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= a.lat.Vh) return;
   T acc[24];
-  if (Tune<T>::STAGE) {
+  if (Tune<T, R>::STAGE) {
     extern __shared__ __align__(16) unsigned char dslash_smem[];
-    dslash_site_staged<T, R, DAG, Tune<T>::BLOCK>(acc, a.in, a.gauge, a.lat, idx, a.parity, dslash_smem, a.ws);
+    dslash_site_staged<T, R, DAG, Tune<T, R>::BLOCK>(acc, a.in, a.gauge, a.lat, idx, a.parity, dslash_smem, a.ws);
   } else {
     dslash_site<T, R, DAG>(acc, a.in, a.gauge, a.lat, idx, a.parity, a.ws);
   }
@@ -93,9 +107,9 @@ __global__ void __launch_bounds__(128) clover_apply_kernel(T* __restrict__ out, 
 
 template <typename T, int R, bool DAG>
 static void launch_epi(const DslashArgs<T>& a, int epi, cudaStream_t st) {
-  const int block = Tune<T>::BLOCK;
+  const int block = Tune<T, R>::BLOCK;
   const int grid = (a.lat.Vh + block - 1) / block;
-  const size_t smem = Tune<T>::STAGE ? (size_t)8 * R * sizeof(T) * block : 0;  // eight links per thread
+  const size_t smem = Tune<T, R>::STAGE ? (size_t)8 * R * sizeof(T) * block : 0;  // eight links per thread
   static bool configured = false;  // one flag per (T, R, DAG) instantiation
   if (!configured && smem > 48 * 1024) {
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
