@@ -183,6 +183,38 @@ int lqcd_invert_mixed(lqcd_ctx* ctx, lqcd_ctx* ctx_lo, void* x_public, const voi
                       int matpc, void* workspace, size_t workspace_bytes, void* workspace_lo,
                       size_t workspace_lo_bytes, lqcd_result* res, void* stream);
 
+/* Sources, propagator assembly and per-time-slice contractions of the paper's Listing 1
+ * (SURVEY.md §8(a) a4/a12, §8(f) rank 4).  All arrays are DEVICE arrays in PUBLIC
+ * layout and in the context's precision: phase [2][Lt][Lz][Ly][Lx/2] complex; spinor as above;
+ * propagator [2][Lt][Lz][Ly][Lx/2][4 sink spin j][4 source spin i][3 sink colour b][3 source colour a]
+ * complex; "columns" = 12 consecutive public spinors, column 3*i+a = the solution for
+ * the source of spin i, colour a.
+ *   lqcd_momentum_phase      : phase(x) = exp(2 pi i (n_x x/Lx + n_y y/Ly + n_z z/Lz))
+ *   lqcd_source_wall         : 1 (or phase(x) if phase != NULL) on every site of time-slice t0 in the
+ *                              (spin, colour) component, 0 elsewhere
+ *   lqcd_source_point        : 1 at site x = {x,y,z,t} in the (spin, colour) component
+ *   lqcd_propagator_assemble : columns -> propagator;  lqcd_propagator_split: the inverse (the source
+ *                              columns of invertPropagator)
+ *   lqcd_contract_twopt      : Eq. 6: out[t] = sum_{w,x,y,z,i,j,a,b} conj(phase) conj(S_0) S_p
+ *                              (phase == NULL: 1); out_host: Lt complex as {re, im} doubles
+ *   lqcd_contract_threept    : Eq. 7: out[t] = sum conj(S_p0[j,i,b,a]) Gamma[j][k] S_p[k,i,b,a];
+ *                              gamma: 4x4 complex row-major as 32 doubles (host)
+ *   lqcd_sequential_source   : Eq. 8: X[i,k,a,b] = conj(phase) sum_j Gamma[i][j] S_0[j,k,a,b] on
+ *                              time-slice t, 0 elsewhere; X must not alias S_0
+ * The two contractions accumulate in fp64 with a fixed reduction order (deterministic) and synchronise. */
+int lqcd_momentum_phase(lqcd_ctx* ctx, void* phase_public, const int mom[3], void* stream);
+int lqcd_source_wall(lqcd_ctx* ctx, void* b_public, int t0, int spin, int colour, const void* phase_public,
+                     void* stream);
+int lqcd_source_point(lqcd_ctx* ctx, void* b_public, const int x[4], int spin, int colour, void* stream);
+int lqcd_propagator_assemble(lqcd_ctx* ctx, void* prop_public, const void* columns_public, void* stream);
+int lqcd_propagator_split(lqcd_ctx* ctx, void* columns_public, const void* prop_public, void* stream);
+int lqcd_contract_twopt(lqcd_ctx* ctx, double* out_host, const void* phase_public, const void* S_0,
+                        const void* S_p, void* stream);
+int lqcd_contract_threept(lqcd_ctx* ctx, double* out_host, const void* S_p0, const double gamma[32],
+                          const void* S_p, void* stream);
+int lqcd_sequential_source(lqcd_ctx* ctx, void* X_prop, const void* phase_public, const double gamma[32],
+                           const void* S_0, int t, void* stream);
+
 /* End-to-end variants with HOST buffers (pageable or pinned): the call uploads the public input,
  * packs, computes, unpacks and downloads the public result.  Links/clover stay resident on the
  * device (PAPER.md:225 loadGauge).  scratch: device buffer of >= lqcd_host_scratch_bytes. */

@@ -36,6 +36,8 @@ SYMBOLS = [
     "lqcd_blas_axpy_norm", "lqcd_blas_xpay", "lqcd_blas_cdot", "lqcd_blas_caxpbypz",
     "lqcd_dslash_mrhs", "lqcd_mpc_apply_mrhs", "lqcd_invert_multi_workspace_bytes", "lqcd_invert_multi",
     "lqcd_invert_mixed", "lqcd_set_anisotropy", "lqcd_clover_build_aniso",
+    "lqcd_momentum_phase", "lqcd_source_wall", "lqcd_source_point", "lqcd_propagator_assemble",
+    "lqcd_propagator_split", "lqcd_contract_twopt", "lqcd_contract_threept", "lqcd_sequential_source",
 ]
 MAX_RHS = 16
 
@@ -76,6 +78,16 @@ def load():
     for f in ("lqcd_gauge_pack", "lqcd_spinor_pack", "lqcd_spinor_unpack", "lqcd_clover_unpack"):
         getattr(L, f).argtypes = [vp, vp, vp, vp]
     L.lqcd_clover_build.argtypes = [vp, vp, vp, vp, cd, cd, vp]
+    ip = ctypes.POINTER(ci)
+    dp = ctypes.POINTER(cd)
+    L.lqcd_momentum_phase.argtypes = [vp, vp, ip, vp]
+    L.lqcd_source_wall.argtypes = [vp, vp, ci, ci, ci, vp, vp]
+    L.lqcd_source_point.argtypes = [vp, vp, ip, ci, ci, vp]
+    L.lqcd_propagator_assemble.argtypes = [vp, vp, vp, vp]
+    L.lqcd_propagator_split.argtypes = [vp, vp, vp, vp]
+    L.lqcd_contract_twopt.argtypes = [vp, dp, vp, vp, vp, vp]
+    L.lqcd_contract_threept.argtypes = [vp, dp, vp, dp, vp, vp]
+    L.lqcd_sequential_source.argtypes = [vp, vp, vp, dp, vp, ci, vp]
     L.lqcd_set_anisotropy.argtypes = [vp, cd]
     L.lqcd_clover_build_aniso.argtypes = [vp, vp, vp, vp, cd, cd, cd, vp]
     L.lqcd_clover_apply.argtypes = [vp, vp, vp, vp, ci, vp]
@@ -319,6 +331,59 @@ class Context:
                                         workspace_lo.numel() * lo.prec, ctypes.byref(res), _stream())
         self._check(rc, allow_not_converged=True)
         return x, res
+
+    # ---- sources, propagators, contractions ----------------------------------
+    def _gamma(self, g):
+        g = np.ascontiguousarray(g, dtype=np.complex128).reshape(16)
+        return (ctypes.c_double * 32)(*np.stack([g.real, g.imag], axis=1).ravel())
+
+    def momentum_phase(self, mom):
+        ph = torch.empty(self.site_shape, dtype=self.cdtype, device=self.dev)
+        self._check(self.lib.lqcd_momentum_phase(self.h, _p(ph), (ctypes.c_int * 3)(*mom), _stream()))
+        return ph
+
+    def source_wall(self, t0, spin, colour, phase=None):
+        b = torch.empty(self.site_shape + (4, 3), dtype=self.cdtype, device=self.dev)
+        self._check(self.lib.lqcd_source_wall(self.h, _p(b), t0, spin, colour, _p(phase), _stream()))
+        return b
+
+    def source_point(self, x, spin, colour):
+        b = torch.empty(self.site_shape + (4, 3), dtype=self.cdtype, device=self.dev)
+        self._check(self.lib.lqcd_source_point(self.h, _p(b), (ctypes.c_int * 4)(*x), spin, colour, _stream()))
+        return b
+
+    def propagator_assemble(self, columns):
+        prop = torch.empty(self.site_shape + (4, 4, 3, 3), dtype=self.cdtype, device=self.dev)
+        self._check(self.lib.lqcd_propagator_assemble(self.h, _p(prop), _p(columns), _stream()))
+        return prop
+
+    def propagator_split(self, prop):
+        cols = torch.empty((12,) + self.site_shape + (4, 3), dtype=self.cdtype, device=self.dev)
+        self._check(self.lib.lqcd_propagator_split(self.h, _p(cols), _p(prop), _stream()))
+        return cols
+
+    def contract_twopt(self, phase, S_0, S_p):
+        out = (ctypes.c_double * (2 * self.dims[3]))()
+        self._check(self.lib.lqcd_contract_twopt(self.h, out, _p(phase), _p(S_0), _p(S_p), _stream()))
+        return np.array(out).reshape(-1, 2) @ np.array([1, 1j])
+
+    def contract_threept(self, S_p0, gamma, S_p):
+        out = (ctypes.c_double * (2 * self.dims[3]))()
+        self._check(self.lib.lqcd_contract_threept(self.h, out, _p(S_p0), self._gamma(gamma), _p(S_p), _stream()))
+        return np.array(out).reshape(-1, 2) @ np.array([1, 1j])
+
+    def sequential_source(self, phase, gamma, S_0, t):
+        X = torch.empty_like(S_0)
+        self._check(self.lib.lqcd_sequential_source(self.h, _p(X), _p(phase), self._gamma(gamma), _p(S_0), t, _stream()))
+        return X
+
+    def propagator(self, sources, gauge, clover, clover_inv, kappa, tol=1e-10, maxiter=1000, solver="cgne",
+                   matpc=0, workspace=None):
+        """The paper's `invert`: 12 source columns [12, site..., 4, 3] -> propagator, by
+        one lqcd_invert_multi call and lqcd_propagator_assemble.  Returns (prop, results, status)."""
+        x, res, rc = self.invert_multi(sources, gauge, clover, clover_inv, kappa, tol, maxiter, solver, matpc,
+                                       workspace)
+        return self.propagator_assemble(x), res, rc
 
     # ---- host-buffer (end-to-end) entry points -----------------------------------------------
     def host_scratch(self, solver="cgne"):
