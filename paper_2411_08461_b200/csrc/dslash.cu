@@ -45,6 +45,16 @@ template <typename T> struct DslashArgs {
 #ifndef DSLASH_MINB_F64_R12
 #define DSLASH_MINB_F64_R12 4
 #endif
+// spinor staging (dslash.cuh): 0 = off, 1 = all eight hops per round, 2 = four and four
+#ifndef DSLASH_SSTAGE_F32
+#define DSLASH_SSTAGE_F32 0
+#endif
+#ifndef DSLASH_SSTAGE_F64
+#define DSLASH_SSTAGE_F64 0
+#endif
+template <typename T> struct SStage;
+template <> struct SStage<float> { static constexpr int ROUNDS = DSLASH_SSTAGE_F32; };
+template <> struct SStage<double> { static constexpr int ROUNDS = DSLASH_SSTAGE_F64; };
 template <typename T, int R> struct Tune;
 #ifndef DSLASH_STAGE_F32_R12
 #define DSLASH_STAGE_F32_R12 0
@@ -62,7 +72,11 @@ __global__ void __launch_bounds__(Tune<T, R>::BLOCK, Tune<T, R>::MINB) dslash_ke
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= a.lat.Vh) return;
   T acc[24];
-  if (Tune<T, R>::STAGE) {
+  if (SStage<T>::ROUNDS > 0) {
+    extern __shared__ __align__(16) unsigned char dslash_smem[];
+    dslash_site_sstaged<T, R, DAG, Tune<T, R>::BLOCK, (SStage<T>::ROUNDS > 0 ? SStage<T>::ROUNDS : 1)>(
+        acc, a.in, a.gauge, a.lat, idx, a.parity, dslash_smem, a.ws);
+  } else if (Tune<T, R>::STAGE) {
     extern __shared__ __align__(16) unsigned char dslash_smem[];
     dslash_site_staged<T, R, DAG, Tune<T, R>::BLOCK>(acc, a.in, a.gauge, a.lat, idx, a.parity, dslash_smem, a.ws);
   } else {
@@ -109,7 +123,8 @@ template <typename T, int R, bool DAG>
 static void launch_epi(const DslashArgs<T>& a, int epi, cudaStream_t st) {
   const int block = Tune<T, R>::BLOCK;
   const int grid = (a.lat.Vh + block - 1) / block;
-  const size_t smem = Tune<T, R>::STAGE ? (size_t)8 * R * sizeof(T) * block : 0;  // eight links per thread
+  const size_t smem = SStage<T>::ROUNDS > 0 ? (size_t)(8 / SStage<T>::ROUNDS) * 24 * sizeof(T) * block  // spinors
+                      : Tune<T, R>::STAGE ? (size_t)8 * R * sizeof(T) * block : 0;                      // eight links per thread
   static bool configured = false;  // one flag per (T, R, DAG) instantiation
   if (!configured && smem > 48 * 1024) {
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

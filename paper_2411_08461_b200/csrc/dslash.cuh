@@ -40,35 +40,37 @@ __device__ __forceinline__ void project(const T* psi, T* h) {
   }
 }
 
-// acc_u += chi ; acc_l += S * B_mu^dag chi
+// acc_u += w chi ; acc_l += w S B_mu^dag chi.  w = hop weight (boundary sign on t-hops, nu/xi_0 on
+// spatial hops, Eq. 5): folded into the accumulation, every line is one FFMA/DFMA.
 template <typename T, int MU, int S>
-__device__ __forceinline__ void reconstruct(T* acc, const T* chi) {
+__device__ __forceinline__ void reconstruct(T* acc, const T* chi, T w) {
+  const T ws = S * w;
 #pragma unroll
   for (int c = 0; c < 3; c++) {
-    acc[RE(0, c)] += chi[RE(0, c)];
-    acc[IM(0, c)] += chi[IM(0, c)];
-    acc[RE(1, c)] += chi[RE(1, c)];
-    acc[IM(1, c)] += chi[IM(1, c)];
+    acc[RE(0, c)] += w * chi[RE(0, c)];
+    acc[IM(0, c)] += w * chi[IM(0, c)];
+    acc[RE(1, c)] += w * chi[RE(1, c)];
+    acc[IM(1, c)] += w * chi[IM(1, c)];
     if (MU == 0) {  // B^dag chi = (-i chi_1, -i chi_0)
-      acc[RE(2, c)] += S * chi[IM(1, c)];
-      acc[IM(2, c)] -= S * chi[RE(1, c)];
-      acc[RE(3, c)] += S * chi[IM(0, c)];
-      acc[IM(3, c)] -= S * chi[RE(0, c)];
+      acc[RE(2, c)] += ws * chi[IM(1, c)];
+      acc[IM(2, c)] -= ws * chi[RE(1, c)];
+      acc[RE(3, c)] += ws * chi[IM(0, c)];
+      acc[IM(3, c)] -= ws * chi[RE(0, c)];
     } else if (MU == 1) {  // B^dag chi = (chi_1, -chi_0)
-      acc[RE(2, c)] += S * chi[RE(1, c)];
-      acc[IM(2, c)] += S * chi[IM(1, c)];
-      acc[RE(3, c)] -= S * chi[RE(0, c)];
-      acc[IM(3, c)] -= S * chi[IM(0, c)];
+      acc[RE(2, c)] += ws * chi[RE(1, c)];
+      acc[IM(2, c)] += ws * chi[IM(1, c)];
+      acc[RE(3, c)] -= ws * chi[RE(0, c)];
+      acc[IM(3, c)] -= ws * chi[IM(0, c)];
     } else if (MU == 2) {  // B^dag chi = (-i chi_0, i chi_1)
-      acc[RE(2, c)] += S * chi[IM(0, c)];
-      acc[IM(2, c)] -= S * chi[RE(0, c)];
-      acc[RE(3, c)] -= S * chi[IM(1, c)];
-      acc[IM(3, c)] += S * chi[RE(1, c)];
+      acc[RE(2, c)] += ws * chi[IM(0, c)];
+      acc[IM(2, c)] -= ws * chi[RE(0, c)];
+      acc[RE(3, c)] -= ws * chi[IM(1, c)];
+      acc[IM(3, c)] += ws * chi[RE(1, c)];
     } else {
-      acc[RE(2, c)] += S * chi[RE(0, c)];
-      acc[IM(2, c)] += S * chi[IM(0, c)];
-      acc[RE(3, c)] += S * chi[RE(1, c)];
-      acc[IM(3, c)] += S * chi[IM(1, c)];
+      acc[RE(2, c)] += ws * chi[RE(0, c)];
+      acc[IM(2, c)] += ws * chi[IM(0, c)];
+      acc[RE(3, c)] += ws * chi[RE(1, c)];
+      acc[IM(3, c)] += ws * chi[IM(1, c)];
     }
   }
 }
@@ -85,8 +87,12 @@ __device__ __forceinline__ void su3_mul(const T* U, const T* h, T* chi) {
       for (int b = 0; b < 3; b++) {
         const T ur = DAGGER_U ? U[2 * (3 * b + a)] : U[2 * (3 * a + b)];
         const T ui = DAGGER_U ? -U[2 * (3 * b + a) + 1] : U[2 * (3 * a + b) + 1];
-        re += ur * h[RE(s, b)] - ui * h[IM(s, b)];
-        im += ur * h[IM(s, b)] + ui * h[RE(s, b)];
+        // one multiply-add per statement: each contracts to a single FFMA/DFMA (a*b - c*d + re would cost
+        // FMUL + FFMA + FADD without reassociation)
+        re += ur * h[RE(s, b)];
+        re -= ui * h[IM(s, b)];
+        im += ur * h[IM(s, b)];
+        im += ui * h[RE(s, b)];
       }
       chi[RE(s, a)] = re;
       chi[IM(s, a)] = im;
@@ -103,10 +109,8 @@ __device__ __forceinline__ void hop(T* acc, const T* __restrict__ in, const T* _
   load_spinor<T>(in, Vh, nidx, psi);
   load_link<T, R>(links, Vh, lidx, U);
   project<T, MU, S>(psi, h);
-#pragma unroll
-  for (int e = 0; e < 12; e++) h[e] *= bsign;  // t: boundary sign; x,y,z: hop weight nu/xi_0 (1 if isotropic)
   su3_mul<T, !FWD>(U, h, chi);
-  reconstruct<T, MU, S>(acc, chi);
+  reconstruct<T, MU, S>(acc, chi, bsign);
 }
 
 // all eight hops for output site idx of parity par.  gauge = native links [mu][parity][NGV][Vh].
@@ -197,12 +201,10 @@ __device__ __forceinline__ void hop_staged(T* acc, const T* __restrict__ in, con
   T psi[24], U[18], h[12], chi[12];
   load_spinor<T>(in, Vh, nidx, psi);
   project<T, MU, S>(psi, h);
-#pragma unroll
-  for (int e = 0; e < 12; e++) h[e] *= bsign;
   cp_async_wait<7 - SLOT>();
   fetch_link<T, R, BLOCK>(smem, SLOT, U);
   su3_mul<T, !FWD>(U, h, chi);
-  reconstruct<T, MU, S>(acc, chi);
+  reconstruct<T, MU, S>(acc, chi, bsign);
 }
 
 template <typename T, int R, bool DAG, int BLOCK>
@@ -238,6 +240,87 @@ __device__ __forceinline__ void dslash_site_staged(T* acc, const T* __restrict__
   hop_staged<T, R, 3, false, DAG, BLOCK, 7>(acc, in, smem, Vh, n7, sb);
 }
 
+// ---------------------------------------------------------------------------------------------
+// Spinor staging through shared memory with cp.async: each thread copies the neighbour spinors of
+// ITS OWN site global->shared asynchronously (16-byte copies, one commit group per hop), HOPS hops
+// per round, so all spinor bytes of a round are in flight without holding registers; the links are
+// ordinary streaming loads, for which the whole register file is then free.  Layout in shared
+// memory: [hop of the round][vector][thread] (conflict free); a thread only reads what it copied.
+// ---------------------------------------------------------------------------------------------
+template <typename T, int BLOCK>
+__device__ __forceinline__ void stage_spinor(void* smem, int slot, const T* __restrict__ in, int Vh, int nidx) {
+  typedef typename V16<T>::vec vec;
+  vec* sl = reinterpret_cast<vec*>(smem) + (size_t)slot * Lay<T>::NSV * BLOCK + threadIdx.x;
+  const vec* g = reinterpret_cast<const vec*>(in) + nidx;
+#pragma unroll
+  for (int v = 0; v < Lay<T>::NSV; v++) cp_async<16>(sl + v * BLOCK, g + (size_t)v * Vh);
+  cp_async_commit();
+}
+template <typename T, int R, int MU, bool FWD, bool DAG, int BLOCK, int SLOT, int PENDING>
+__device__ __forceinline__ void hop_sstaged(T* acc, const void* smem, const T* __restrict__ links, int Vh, int lidx, T bsign) {
+  typedef typename V16<T>::vec vec;
+  constexpr int S = (FWD != DAG) ? -1 : +1;
+  T psi[24], U[18], h[12], chi[12];
+  load_link<T, R>(links, Vh, lidx, U);
+  cp_async_wait<PENDING>();
+  const vec* sl = reinterpret_cast<const vec*>(smem) + (size_t)SLOT * Lay<T>::NSV * BLOCK + threadIdx.x;
+#pragma unroll
+  for (int v = 0; v < Lay<T>::NSV; v++) {
+    vec q = sl[v * BLOCK];
+    vec_get(q, psi + v * V16<T>::N);
+  }
+  project<T, MU, S>(psi, h);
+  su3_mul<T, !FWD>(U, h, chi);
+  reconstruct<T, MU, S>(acc, chi, bsign);
+}
+// ROUNDS = 1: all eight hops staged at once; ROUNDS = 2: four and four (half the shared memory)
+template <typename T, int R, bool DAG, int BLOCK, int ROUNDS>
+__device__ __forceinline__ void dslash_site_sstaged(T* acc, const T* __restrict__ in, const T* __restrict__ gauge,
+                                                    const Lat& L, int idx, int par, void* smem, T ws) {
+  const Site s = site_of(L, idx, par);
+  const int Vh = L.Vh;
+  const size_t blk = (size_t)R * Vh;
+  const int n0 = neighbour<0, +1>(L, idx, s), n1 = neighbour<0, -1>(L, idx, s);
+  const int n2 = neighbour<1, +1>(L, idx, s), n3 = neighbour<1, -1>(L, idx, s);
+  const int n4 = neighbour<2, +1>(L, idx, s), n5 = neighbour<2, -1>(L, idx, s);
+  const int n6 = neighbour<3, +1>(L, idx, s), n7 = neighbour<3, -1>(L, idx, s);
+  const T sf = (L.tb < 0 && s.t == L.Lt - 1) ? (T)-1 : (T)1;
+  const T sb = (L.tb < 0 && s.t == 0) ? (T)-1 : (T)1;
+#pragma unroll
+  for (int e = 0; e < 24; e++) acc[e] = 0;
+  stage_spinor<T, BLOCK>(smem, 0, in, Vh, n0);
+  stage_spinor<T, BLOCK>(smem, 1, in, Vh, n1);
+  stage_spinor<T, BLOCK>(smem, 2, in, Vh, n2);
+  stage_spinor<T, BLOCK>(smem, 3, in, Vh, n3);
+  if (ROUNDS == 1) {
+    stage_spinor<T, BLOCK>(smem, 4, in, Vh, n4);
+    stage_spinor<T, BLOCK>(smem, 5, in, Vh, n5);
+    stage_spinor<T, BLOCK>(smem, 6, in, Vh, n6);
+    stage_spinor<T, BLOCK>(smem, 7, in, Vh, n7);
+    hop_sstaged<T, R, 0, true, DAG, BLOCK, 0, 7>(acc, smem, gauge + (0 * 2 + par) * blk, Vh, idx, ws);
+    hop_sstaged<T, R, 0, false, DAG, BLOCK, 1, 6>(acc, smem, gauge + (0 * 2 + 1 - par) * blk, Vh, n1, ws);
+    hop_sstaged<T, R, 1, true, DAG, BLOCK, 2, 5>(acc, smem, gauge + (1 * 2 + par) * blk, Vh, idx, ws);
+    hop_sstaged<T, R, 1, false, DAG, BLOCK, 3, 4>(acc, smem, gauge + (1 * 2 + 1 - par) * blk, Vh, n3, ws);
+    hop_sstaged<T, R, 2, true, DAG, BLOCK, 4, 3>(acc, smem, gauge + (2 * 2 + par) * blk, Vh, idx, ws);
+    hop_sstaged<T, R, 2, false, DAG, BLOCK, 5, 2>(acc, smem, gauge + (2 * 2 + 1 - par) * blk, Vh, n5, ws);
+    hop_sstaged<T, R, 3, true, DAG, BLOCK, 6, 1>(acc, smem, gauge + (3 * 2 + par) * blk, Vh, idx, sf);
+    hop_sstaged<T, R, 3, false, DAG, BLOCK, 7, 0>(acc, smem, gauge + (3 * 2 + 1 - par) * blk, Vh, n7, sb);
+  } else {
+    hop_sstaged<T, R, 0, true, DAG, BLOCK, 0, 3>(acc, smem, gauge + (0 * 2 + par) * blk, Vh, idx, ws);
+    stage_spinor<T, BLOCK>(smem, 0, in, Vh, n4);  // slot 0 is free again: refill it while hops 1-3 run
+    hop_sstaged<T, R, 0, false, DAG, BLOCK, 1, 3>(acc, smem, gauge + (0 * 2 + 1 - par) * blk, Vh, n1, ws);
+    stage_spinor<T, BLOCK>(smem, 1, in, Vh, n5);
+    hop_sstaged<T, R, 1, true, DAG, BLOCK, 2, 3>(acc, smem, gauge + (1 * 2 + par) * blk, Vh, idx, ws);
+    stage_spinor<T, BLOCK>(smem, 2, in, Vh, n6);
+    hop_sstaged<T, R, 1, false, DAG, BLOCK, 3, 3>(acc, smem, gauge + (1 * 2 + 1 - par) * blk, Vh, n3, ws);
+    stage_spinor<T, BLOCK>(smem, 3, in, Vh, n7);
+    hop_sstaged<T, R, 2, true, DAG, BLOCK, 0, 3>(acc, smem, gauge + (2 * 2 + par) * blk, Vh, idx, ws);
+    hop_sstaged<T, R, 2, false, DAG, BLOCK, 1, 2>(acc, smem, gauge + (2 * 2 + 1 - par) * blk, Vh, n5, ws);
+    hop_sstaged<T, R, 3, true, DAG, BLOCK, 2, 1>(acc, smem, gauge + (3 * 2 + par) * blk, Vh, idx, sf);
+    hop_sstaged<T, R, 3, false, DAG, BLOCK, 3, 0>(acc, smem, gauge + (3 * 2 + 1 - par) * blk, Vh, n7, sb);
+  }
+}
+
 // out = C v for the two Hermitian 6x6 chiral blocks of one site.  cl = one-parity clover field
 // [NCV][Vh]; packed order per block: 6 real diagonal, then 15 complex lower entries row-major.
 // v and out are 24-real spinors (block k acts on reals 12k..12k+11); they must not alias.
@@ -263,12 +346,16 @@ __device__ __forceinline__ void clover_mul(const T* __restrict__ cl, int Vh, int
       for (int j = 0; j < 6; j++) {
         if (j < i) {  // L_ij x_j
           const int o = 6 + 2 * (i * (i - 1) / 2 + j);
-          re += a[o] * x[2 * j] - a[o + 1] * x[2 * j + 1];
-          im += a[o] * x[2 * j + 1] + a[o + 1] * x[2 * j];
+          re += a[o] * x[2 * j];
+          re -= a[o + 1] * x[2 * j + 1];
+          im += a[o] * x[2 * j + 1];
+          im += a[o + 1] * x[2 * j];
         } else if (j > i) {  // conj(L_ji) x_j
           const int o = 6 + 2 * (j * (j - 1) / 2 + i);
-          re += a[o] * x[2 * j] + a[o + 1] * x[2 * j + 1];
-          im += a[o] * x[2 * j + 1] - a[o + 1] * x[2 * j];
+          re += a[o] * x[2 * j];
+          re += a[o + 1] * x[2 * j + 1];
+          im += a[o] * x[2 * j + 1];
+          im -= a[o + 1] * x[2 * j];
         }
       }
       y[2 * i] = re;

@@ -23,7 +23,7 @@
 #define MRHS_SITES 32
 #endif
 #ifndef MRHS_MINB_F32
-#define MRHS_MINB_F32 4
+#define MRHS_MINB_F32 5
 #endif
 #ifndef MRHS_MINB_F64
 #define MRHS_MINB_F64 3
@@ -78,18 +78,15 @@ __device__ __forceinline__ void hop_mrhs(T (*acc)[24], const T* __restrict__ in,
   constexpr int S = (FWD != DAG) ? -1 : +1;
   T U[18];
   load_link_l1<T, R>(links, Vh, lidx, U);
-  {  // t: antiperiodic seam; x,y,z: hop weight.  Scale the link once for all NB columns (after the row-3 rebuild)
-    const T sg = (MU == 3) ? (seam ? (T)-1 : (T)1) : bsign;
-#pragma unroll
-    for (int e = 0; e < 18; e++) U[e] *= sg;
-  }
+  // t: antiperiodic seam; x,y,z: hop weight; folded into the accumulation (reconstruct)
+  const T sg = (MU == 3) ? (seam ? (T)-1 : (T)1) : bsign;
 #pragma unroll
   for (int r = 0; r < NB; r++) {
     T psi[24], h[12], chi[12];
     load_spinor<T>(in + r * stride, Vh, nidx, psi);
     project<T, MU, S>(psi, h);
     su3_mul<T, !FWD>(U, h, chi);
-    reconstruct<T, MU, S>(acc[r], chi);
+    reconstruct<T, MU, S>(acc[r], chi, sg);
   }
 }
 
@@ -118,12 +115,16 @@ __device__ __forceinline__ void clover_mul_mrhs(const T* __restrict__ cl, int Vh
         for (int j = 0; j < 6; j++) {
           if (j < i) {
             const int o = 6 + 2 * (i * (i - 1) / 2 + j);
-            re += a[o] * x[2 * j] - a[o + 1] * x[2 * j + 1];
-            im += a[o] * x[2 * j + 1] + a[o + 1] * x[2 * j];
+            re += a[o] * x[2 * j];
+            re -= a[o + 1] * x[2 * j + 1];
+            im += a[o] * x[2 * j + 1];
+            im += a[o + 1] * x[2 * j];
           } else if (j > i) {
             const int o = 6 + 2 * (j * (j - 1) / 2 + i);
-            re += a[o] * x[2 * j] + a[o + 1] * x[2 * j + 1];
-            im += a[o] * x[2 * j + 1] - a[o + 1] * x[2 * j];
+            re += a[o] * x[2 * j];
+            re += a[o + 1] * x[2 * j + 1];
+            im += a[o] * x[2 * j + 1];
+            im -= a[o + 1] * x[2 * j];
           }
         }
         y[2 * i] = re;
