@@ -198,6 +198,18 @@ template <typename T> struct OpCgUpdate {
     acc[0] += (double)w[2][0] * w[2][0] + (double)w[2][1] * w[2][1];
   }
 };
+// x += (s[num]/s[den]) t                            v0 = x, v1 = t
+template <typename T> struct OpAxpyRatio {
+  static constexpr int NV = 2, NR = 0;
+  static constexpr unsigned LOAD = 3, STORE = 1;
+  int num, den;
+  T alpha;
+  __device__ void init(const double* s) { alpha = (T)(s[num] / s[den]); }
+  __device__ void elem(T (*w)[2], double*) {
+    w[0][0] += alpha * w[1][0];
+    w[0][1] += alpha * w[1][1];
+  }
+};
 // r -= (s[num]/s[den]) q ; out0 = |r|^2            v0 = r, v1 = q
 template <typename T> struct OpAxmyNormRatio {
   static constexpr int NV = 2, NR = 1;

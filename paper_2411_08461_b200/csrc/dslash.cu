@@ -6,6 +6,10 @@
 //   1: out = scale * C d                 (e.g. A_oo^-1 D_oe x)
 //   2: out = C x + scale * d             (asymmetric Mhat:  A_ee x - k^2 D_eo t)
 //   3: out = x + scale * C d             (symmetric  Mhat:  x - k^2 A_ee^-1 D_eo t)
+// Epilogues fused with the CG recurrences (single right-hand side; fp64 reduction, deterministic:
+// per-block partials summed in block order by the last block to finish):
+//   4: out = C x + scale * d ; s[out_slot] = |out|^2                          (t = Mhat^dag p, <p, A p>)
+//   5: q   = C x + scale * d ; r -= (s[num]/s[den]) q ; s[out_slot] = |r|^2   (q never stored)
 template <typename T> struct DslashArgs {
   T* out;
   const T* in;
@@ -16,6 +20,11 @@ template <typename T> struct DslashArgs {
   int parity;
   T scale;
   T ws;  // weight of the spatial hops (anisotropy nu/xi_0; 1 = isotropic)
+  // EPI 4, 5 only
+  T* r;
+  double* partial;
+  double* scalars;
+  int num, den;
 };
 
 // Launch shape per precision (threads per block, minimum resident blocks per SM = register budget).
@@ -67,43 +76,108 @@ template <> struct Tune<float, 12> { static constexpr int BLOCK = DSLASH_BLOCK_F
 template <> struct Tune<double, 18> { static constexpr int BLOCK = DSLASH_BLOCK_F64, MINB = DSLASH_MINB_F64; static constexpr bool STAGE = DSLASH_STAGE_F64; };
 template <> struct Tune<double, 12> { static constexpr int BLOCK = DSLASH_BLOCK_F64, MINB = DSLASH_MINB_F64_R12; static constexpr bool STAGE = DSLASH_STAGE_F64_R12; };
 
+// Deterministic fp64 grid reduction of the fused epilogues: block sum -> partial[block] (no fence, no
+// atomic: a ticket scheme inside the stencil kernel cost 25 us per launch in block-retirement latency),
+// then one small kernel sums the partials in a fixed order -> scalars[out_slot].
+template <int BLOCK>
+__device__ __forceinline__ void dslash_reduce(double v, double* partial) {
+  __shared__ double sm[BLOCK / 32];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  if (lane == 0) sm[warp] = v;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0;
+#pragma unroll
+    for (int w = 0; w < BLOCK / 32; w++) t += sm[w];
+    partial[blockIdx.x] = t;
+  }
+}
+constexpr int PSUM_BLOCK = 1024;
+__global__ void __launch_bounds__(PSUM_BLOCK) partial_sum_kernel(const double* __restrict__ partial, int n, double* out) {
+  __shared__ double sm[PSUM_BLOCK / 32];
+  double t0 = 0, t1 = 0, t2 = 0, t3 = 0;  // four independent chains, fixed assignment: deterministic
+  int b = threadIdx.x;
+  for (; b + 3 * PSUM_BLOCK < n; b += 4 * PSUM_BLOCK) {
+    t0 += partial[b];
+    t1 += partial[b + PSUM_BLOCK];
+    t2 += partial[b + 2 * PSUM_BLOCK];
+    t3 += partial[b + 3 * PSUM_BLOCK];
+  }
+  for (; b < n; b += PSUM_BLOCK) t0 += partial[b];
+  double v = (t0 + t1) + (t2 + t3);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  if (lane == 0) sm[warp] = v;
+  __syncthreads();
+  if (warp == 0) {
+    v = sm[lane];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if (lane == 0) *out = v;
+  }
+}
+
 template <typename T, int R, bool DAG, int EPI>
 __global__ void __launch_bounds__(Tune<T, R>::BLOCK, Tune<T, R>::MINB) dslash_kernel(const DslashArgs<T> a) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= a.lat.Vh) return;
-  T acc[24];
-  if (SStage<T>::ROUNDS > 0) {
-    extern __shared__ __align__(16) unsigned char dslash_smem[];
-    dslash_site_sstaged<T, R, DAG, Tune<T, R>::BLOCK, (SStage<T>::ROUNDS > 0 ? SStage<T>::ROUNDS : 1)>(
-        acc, a.in, a.gauge, a.lat, idx, a.parity, dslash_smem, a.ws);
-  } else if (Tune<T, R>::STAGE) {
-    extern __shared__ __align__(16) unsigned char dslash_smem[];
-    dslash_site_staged<T, R, DAG, Tune<T, R>::BLOCK>(acc, a.in, a.gauge, a.lat, idx, a.parity, dslash_smem, a.ws);
-  } else {
-    dslash_site<T, R, DAG>(acc, a.in, a.gauge, a.lat, idx, a.parity, a.ws);
+  const bool live = idx < a.lat.Vh;
+  if (EPI < 4 && !live) return;
+  double local = 0;
+  if (live) {
+    T acc[24];
+    if (SStage<T>::ROUNDS > 0) {
+      extern __shared__ __align__(16) unsigned char dslash_smem[];
+      dslash_site_sstaged<T, R, DAG, Tune<T, R>::BLOCK, (SStage<T>::ROUNDS > 0 ? SStage<T>::ROUNDS : 1)>(
+          acc, a.in, a.gauge, a.lat, idx, a.parity, dslash_smem, a.ws);
+    } else if (Tune<T, R>::STAGE) {
+      extern __shared__ __align__(16) unsigned char dslash_smem[];
+      dslash_site_staged<T, R, DAG, Tune<T, R>::BLOCK>(acc, a.in, a.gauge, a.lat, idx, a.parity, dslash_smem, a.ws);
+    } else {
+      dslash_site<T, R, DAG>(acc, a.in, a.gauge, a.lat, idx, a.parity, a.ws);
+    }
+    T res[24];
+    if (EPI == 0) {
+#pragma unroll
+      for (int e = 0; e < 24; e++) res[e] = a.scale * acc[e];
+    } else if (EPI == 1) {
+      clover_mul<T>(a.cl, a.lat.Vh, idx, acc, res);
+#pragma unroll
+      for (int e = 0; e < 24; e++) res[e] *= a.scale;
+    } else if (EPI == 2 || EPI == 4 || EPI == 5) {
+      T xv[24];
+      load_spinor<T>(a.x, a.lat.Vh, idx, xv);
+      clover_mul<T>(a.cl, a.lat.Vh, idx, xv, res);
+#pragma unroll
+      for (int e = 0; e < 24; e++) res[e] += a.scale * acc[e];
+    } else {
+      T xv[24];
+      load_spinor<T>(a.x, a.lat.Vh, idx, xv);
+      clover_mul<T>(a.cl, a.lat.Vh, idx, acc, res);
+#pragma unroll
+      for (int e = 0; e < 24; e++) res[e] = xv[e] + a.scale * res[e];
+    }
+    if (EPI == 5) {
+      const T alpha = (T)(a.scalars[a.num] / a.scalars[a.den]);
+      T rv[24];
+      load_spinor<T>(a.r, a.lat.Vh, idx, rv);
+#pragma unroll
+      for (int e = 0; e < 24; e++) {
+        rv[e] -= alpha * res[e];
+        local += (double)rv[e] * rv[e];
+      }
+      store_spinor<T>(a.r, a.lat.Vh, idx, rv);
+    } else {
+      if (EPI == 4) {
+#pragma unroll
+        for (int e = 0; e < 24; e++) local += (double)res[e] * res[e];
+      }
+      store_spinor<T>(a.out, a.lat.Vh, idx, res);
+    }
   }
-  T res[24];
-  if (EPI == 0) {
-#pragma unroll
-    for (int e = 0; e < 24; e++) res[e] = a.scale * acc[e];
-  } else if (EPI == 1) {
-    clover_mul<T>(a.cl, a.lat.Vh, idx, acc, res);
-#pragma unroll
-    for (int e = 0; e < 24; e++) res[e] *= a.scale;
-  } else if (EPI == 2) {
-    T xv[24];
-    load_spinor<T>(a.x, a.lat.Vh, idx, xv);
-    clover_mul<T>(a.cl, a.lat.Vh, idx, xv, res);
-#pragma unroll
-    for (int e = 0; e < 24; e++) res[e] += a.scale * acc[e];
-  } else {
-    T xv[24];
-    load_spinor<T>(a.x, a.lat.Vh, idx, xv);
-    clover_mul<T>(a.cl, a.lat.Vh, idx, acc, res);
-#pragma unroll
-    for (int e = 0; e < 24; e++) res[e] = xv[e] + a.scale * res[e];
-  }
-  store_spinor<T>(a.out, a.lat.Vh, idx, res);
+  if (EPI >= 4) dslash_reduce<Tune<T, R>::BLOCK>(local, a.partial);
 }
 
 template <typename T>
@@ -131,20 +205,29 @@ static void launch_epi(const DslashArgs<T>& a, int epi, cudaStream_t st) {
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   }
   configured = true;
   switch (epi) {
     case 0: dslash_kernel<T, R, DAG, 0><<<grid, block, smem, st>>>(a); break;
     case 1: dslash_kernel<T, R, DAG, 1><<<grid, block, smem, st>>>(a); break;
     case 2: dslash_kernel<T, R, DAG, 2><<<grid, block, smem, st>>>(a); break;
-    default: dslash_kernel<T, R, DAG, 3><<<grid, block, smem, st>>>(a); break;
+    case 3: dslash_kernel<T, R, DAG, 3><<<grid, block, smem, st>>>(a); break;
+    case 4: dslash_kernel<T, R, DAG, 4><<<grid, block, smem, st>>>(a); break;
+    default: dslash_kernel<T, R, DAG, 5><<<grid, block, smem, st>>>(a); break;
   }
 }
 
 template <typename T>
 static void launch_typed(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
-                         int parity, double scale, int dagger, int epi, cudaStream_t st) {
+                         int parity, double scale, int dagger, int epi, const DslashFuse* f, cudaStream_t st) {
   DslashArgs<T> a;
+  a.r = f ? (T*)f->r : nullptr;
+  a.partial = c->d_partial;
+  a.scalars = c->d_scalars;
+  a.num = f ? f->num : 0;
+  a.den = f ? f->den : 0;
   a.out = (T*)out;
   a.in = (const T*)in;
   a.gauge = (const T*)gauge;
@@ -175,14 +258,43 @@ int lqcd_dslash_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge
   c->alg_bytes += bytes;
   const bool rec = c->prof_on && c->prof_n < c->prof_cap;
   if (rec) cudaEventRecord(c->prof_ev[2 * c->prof_n], st);
-  if (c->prec == 4) launch_typed<float>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, st);
-  else launch_typed<double>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, st);
+  if (c->prec == 4) launch_typed<float>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nullptr, st);
+  else launch_typed<double>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nullptr, st);
   if (rec) {
     cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], st);
     c->prof_n++;
     c->prof_bytes += bytes;
   }
   LQCD_LAUNCH_CHECK(c, "dslash");
+  return LQCD_OK;
+}
+
+// CG-fused epilogues (4, 5) are available when the per-block partials fit the context's scratch
+bool lqcd_dslash_fuse_ok(const lqcd_ctx* c) {
+  const int block = c->prec == 4 ? DSLASH_BLOCK_F32 : DSLASH_BLOCK_F64;
+  return (long)(c->lat.Vh + block - 1) / block <= 4L * c->max_red_blocks * LQCD_MAX_RHS;
+}
+
+int lqcd_dslash_fused_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
+                             int parity, double scale, int dagger, int epi, const DslashFuse* f, cudaStream_t st) {
+  // epi 4: as epi 2.  epi 5: no output store, r read and written instead
+  const double bytes = (double)c->lat.Vh * c->prec * (8.0 * c->recon + 48.0 + 72.0 + 24.0 + (epi == 5 ? 24.0 : 0.0));
+  c->alg_bytes += bytes;
+  const bool rec = c->prof_on && c->prof_n < c->prof_cap;
+  if (rec) cudaEventRecord(c->prof_ev[2 * c->prof_n], st);
+  if (c->prec == 4) launch_typed<float>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, f, st);
+  else launch_typed<double>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, f, st);
+  {
+    const int block = c->prec == 4 ? DSLASH_BLOCK_F32 : DSLASH_BLOCK_F64;
+    partial_sum_kernel<<<1, PSUM_BLOCK, 0, st>>>(c->d_partial, (c->lat.Vh + block - 1) / block, c->d_scalars + f->out_slot);
+    c->launches++;
+  }
+  if (rec) {
+    cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], st);
+    c->prof_n++;
+    c->prof_bytes += bytes;
+  }
+  LQCD_LAUNCH_CHECK(c, "dslash_fused");
   return LQCD_OK;
 }
 

@@ -179,6 +179,15 @@ static inline cudaStream_t as_stream(void* s) { return reinterpret_cast<cudaStre
 // internal launchers shared between translation units
 int lqcd_dslash_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
                        int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st);
+// CG recurrences fused into the dslash epilogue (dslash.cu, epilogues 4 and 5; single right-hand side)
+struct DslashFuse {
+  void* r;       // epi 5: residual updated in place, r -= (s[num]/s[den]) q
+  int out_slot;  // reduction result: |out|^2 (epi 4) or |r|^2 (epi 5) -> d_scalars[out_slot]
+  int num, den;
+};
+bool lqcd_dslash_fuse_ok(const lqcd_ctx* c);
+int lqcd_dslash_fused_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
+                             int parity, double scale, int dagger, int epi, const DslashFuse* f, cudaStream_t st);
 int lqcd_dslash_mrhs_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
                             int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st);
 int lqcd_clover_apply_launch(lqcd_ctx* c, void* out, const void* in, const void* cl_parity, int nrhs, cudaStream_t st);

@@ -171,11 +171,24 @@ static int solve_cg(lqcd_ctx* c, const Work& w, const void* gauge, const void* A
     cols.rr[j] = hs(c, j, S_RES);
     if (!(cols.rr[j] > cols.stop2[j])) freeze(c, cols, j, st);
   }
+  const bool fused = n == 1 && matpc == LQCD_MATPC_ASYMMETRIC && lqcd_dslash_fuse_ok(c);
   int it = 0;
   while (it < maxiter && cols.nactive() > 0) {
     const int cur = (it & 1) ? S_RR1 : S_RR0, nxt = (it & 1) ? S_RR0 : S_RR1;
     int outs[4] = {S_TT, 0, 0, 0};
-    if (!normal_residual) {
+    if (!normal_residual && fused) {
+      // CGNE with the recurrences fused into the dslash epilogues (dslash.cu EPI 4, 5):
+      //   t = Mhat^dag p and |t|^2 in one launch; q = Mhat t is never stored: r -= alpha q, |r|^2 in its launch
+      const size_t half = lqcd_clover_bytes(c) / 2;
+      const double k2 = -kappa * kappa;
+      DslashFuse f4 = {nullptr, S_TT, 0, 0}, f5 = {r, nxt, cur, S_TT};
+      if ((rc = lqcd_dslash_launch(c, tmp, p, gauge, off(Ai, half), nullptr, 1, 1.0, 1, 1, 1, st))) return rc;
+      if ((rc = lqcd_dslash_fused_launch(c, t, tmp, gauge, A, p, 0, k2, 1, 4, &f4, st))) return rc;
+      if ((rc = lqcd_dslash_launch(c, tmp, t, gauge, off(Ai, half), nullptr, 1, 1.0, 0, 1, 1, st))) return rc;
+      if ((rc = lqcd_dslash_fused_launch(c, nullptr, tmp, gauge, A, t, 0, k2, 0, 5, &f5, st))) return rc;
+      void* u[2] = {x, t};
+      if ((rc = BLAS_CALL(c, OpAxpyRatio, (op.num = cur, op.den = S_TT), u, nullptr, n, 0, st))) return rc;  // x += a t
+    } else if (!normal_residual) {
       if ((rc = mpc_apply(c, t, p, gauge, A, Ai, kappa, matpc, 1, tmp, n, st))) return rc;   // t = Mhat^dag p
       void* v[1] = {t};
       if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v, outs, n, 0, st))) return rc;              // <p, Mhat Mhat^dag p>
