@@ -381,7 +381,7 @@ def run_gpu(args):
         "roofline": {"bound": "hbm", "achieved": ds_bytes / (ds_ms * 1e-3) / 1e9 if ds_ms > 0 else None,
                      "peak": peak, "unit": "GB/s",
                      "frac": (ds_bytes / (ds_ms * 1e-3) / 1e9 / peak) if ds_ms > 0 else None,
-                     "traffic": traffic_from_profile(), "kernel": "dslash_kernel<double,18,*,EPI 1|2> (fused clover epilogues)",
+                     "traffic": traffic_from_profile(), "kernel": "dslash_kernel<double,18,*,EPI 1|4|5> (fused clover and CG epilogues)",
                      "launches_timed": n_ds, "avg_launch_us": ds_ms * 1e3 / max(n_ds, 1),
                      "alg_bytes_per_launch": ds_bytes / max(n_ds, 1), "peak_source": peak_src,
                      "frac_of_8TBps": (ds_bytes / (ds_ms * 1e-3) / 8e12) if ds_ms > 0 else None},
