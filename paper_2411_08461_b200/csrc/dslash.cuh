@@ -12,8 +12,35 @@
 #define IM(s, c) (2 * (3 * (s) + (c)) + 1)
 
 // h = psi_u + S * B_mu psi_l          (S = -1: (1 - gamma_mu), S = +1: (1 + gamma_mu))
+#define CPK(a, s, c) pk2((a)[RE(s, c)], (a)[IM(s, c)])   // (re, im)
+#define CSW(a, s, c) pk2((a)[IM(s, c)], (a)[RE(s, c)])   // (im, re): an operand swizzle, no instruction
+#define CST(a, s, c, v) upk2((v), (a)[RE(s, c)], (a)[IM(s, c)])
+template <int MU, int S>
+__device__ __forceinline__ void project_packed(const float* psi, float* h) {
+  const float p = (float)S, m = (float)-S;
+#pragma unroll
+  for (int c = 0; c < 3; c++) {
+    if (MU == 0) {  // h0 = psi0 + S i psi3, h1 = psi1 + S i psi2;  S i (re, im) = (-S im, S re)
+      CST(h, 0, c, fma2(pk2(m, p), CSW(psi, 3, c), CPK(psi, 0, c)));
+      CST(h, 1, c, fma2(pk2(m, p), CSW(psi, 2, c), CPK(psi, 1, c)));
+    } else if (MU == 1) {  // h0 = psi0 - S psi3, h1 = psi1 + S psi2
+      CST(h, 0, c, fma2(pk2(m, m), CPK(psi, 3, c), CPK(psi, 0, c)));
+      CST(h, 1, c, fma2(pk2(p, p), CPK(psi, 2, c), CPK(psi, 1, c)));
+    } else if (MU == 2) {  // h0 = psi0 + S i psi2, h1 = psi1 - S i psi3
+      CST(h, 0, c, fma2(pk2(m, p), CSW(psi, 2, c), CPK(psi, 0, c)));
+      CST(h, 1, c, fma2(pk2(p, m), CSW(psi, 3, c), CPK(psi, 1, c)));
+    } else {  // h0 = psi0 + S psi2, h1 = psi1 + S psi3
+      CST(h, 0, c, fma2(pk2(p, p), CPK(psi, 2, c), CPK(psi, 0, c)));
+      CST(h, 1, c, fma2(pk2(p, p), CPK(psi, 3, c), CPK(psi, 1, c)));
+    }
+  }
+}
+
 template <typename T, int MU, int S>
 __device__ __forceinline__ void project(const T* psi, T* h) {
+  if constexpr (UsePacked<T>::value) {
+    project_packed<MU, S>(psi, h);
+  } else {
 #pragma unroll
   for (int c = 0; c < 3; c++) {
     if (MU == 0) {  // B psi_l = (i psi_3, i psi_2)
@@ -38,12 +65,39 @@ __device__ __forceinline__ void project(const T* psi, T* h) {
       h[IM(1, c)] = psi[IM(1, c)] + S * psi[IM(3, c)];
     }
   }
+  }
 }
 
 // acc_u += w chi ; acc_l += w S B_mu^dag chi.  w = hop weight (boundary sign on t-hops, nu/xi_0 on
 // spatial hops, Eq. 5): folded into the accumulation, every line is one FFMA/DFMA.
+template <int MU, int S>
+__device__ __forceinline__ void reconstruct_packed(float* acc, const float* chi, float w) {
+  const float ws = S * w, wn = -ws;
+#pragma unroll
+  for (int c = 0; c < 3; c++) {
+    CST(acc, 0, c, fma2(pk2(w, w), CPK(chi, 0, c), CPK(acc, 0, c)));
+    CST(acc, 1, c, fma2(pk2(w, w), CPK(chi, 1, c), CPK(acc, 1, c)));
+    if (MU == 0) {  // acc2 += ws (-i chi1) = (ws, -ws) o (im1, re1); acc3 likewise with chi0
+      CST(acc, 2, c, fma2(pk2(ws, wn), CSW(chi, 1, c), CPK(acc, 2, c)));
+      CST(acc, 3, c, fma2(pk2(ws, wn), CSW(chi, 0, c), CPK(acc, 3, c)));
+    } else if (MU == 1) {  // acc2 += ws chi1; acc3 -= ws chi0
+      CST(acc, 2, c, fma2(pk2(ws, ws), CPK(chi, 1, c), CPK(acc, 2, c)));
+      CST(acc, 3, c, fma2(pk2(wn, wn), CPK(chi, 0, c), CPK(acc, 3, c)));
+    } else if (MU == 2) {  // acc2 += ws (-i chi0); acc3 += ws (i chi1)
+      CST(acc, 2, c, fma2(pk2(ws, wn), CSW(chi, 0, c), CPK(acc, 2, c)));
+      CST(acc, 3, c, fma2(pk2(wn, ws), CSW(chi, 1, c), CPK(acc, 3, c)));
+    } else {
+      CST(acc, 2, c, fma2(pk2(ws, ws), CPK(chi, 0, c), CPK(acc, 2, c)));
+      CST(acc, 3, c, fma2(pk2(ws, ws), CPK(chi, 1, c), CPK(acc, 3, c)));
+    }
+  }
+}
+
 template <typename T, int MU, int S>
 __device__ __forceinline__ void reconstruct(T* acc, const T* chi, T w) {
+  if constexpr (UsePacked<T>::value) {
+    reconstruct_packed<MU, S>(acc, chi, w);
+  } else {
   const T ws = S * w;
 #pragma unroll
   for (int c = 0; c < 3; c++) {
@@ -73,11 +127,35 @@ __device__ __forceinline__ void reconstruct(T* acc, const T* chi, T w) {
       acc[IM(3, c)] += ws * chi[IM(1, c)];
     }
   }
+  }
 }
 
 // chi = U h (DAGGER_U = false) or U^dag h (true), for the two spin components of h
+template <bool DAGGER_U>
+__device__ __forceinline__ void su3_mul_packed(const float* U, const float* h, float* chi) {
+  // chi_a = sum_b ur_ab (hr, hi)_b  +  (-1, 1) o sum_b ui_ab (hi, hr)_b : the swizzled operand is free, the
+  // sign of the imaginary-part products is applied once per output (7 FFMA2 per complex output)
+#pragma unroll
+  for (int s = 0; s < 2; s++)
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+      u64 accr, acci;
+#pragma unroll
+      for (int b = 0; b < 3; b++) {
+        const float ur = DAGGER_U ? U[2 * (3 * b + a)] : U[2 * (3 * a + b)];
+        const float ui = DAGGER_U ? U[2 * (3 * b + a) + 1] : U[2 * (3 * a + b) + 1];
+        accr = (b == 0) ? mul2(pk2(ur, ur), CPK(h, s, b)) : fma2(pk2(ur, ur), CPK(h, s, b), accr);
+        acci = (b == 0) ? mul2(pk2(ui, ui), CSW(h, s, b)) : fma2(pk2(ui, ui), CSW(h, s, b), acci);
+      }
+      CST(chi, s, a, fma2(DAGGER_U ? pk2(1.f, -1.f) : pk2(-1.f, 1.f), acci, accr));
+    }
+}
+
 template <typename T, bool DAGGER_U>
 __device__ __forceinline__ void su3_mul(const T* U, const T* h, T* chi) {
+  if constexpr (UsePacked<T>::value) {
+    su3_mul_packed<DAGGER_U>(U, h, chi);
+  } else {
 #pragma unroll
   for (int s = 0; s < 2; s++)
 #pragma unroll
@@ -97,6 +175,7 @@ __device__ __forceinline__ void su3_mul(const T* U, const T* h, T* chi) {
       chi[RE(s, a)] = re;
       chi[IM(s, a)] = im;
     }
+  }
 }
 
 // one of the eight hops.  FWD: U_mu(x) psi(x+mu) with link block of the output parity at idx;
@@ -181,18 +260,7 @@ __device__ __forceinline__ void fetch_link(const void* smem, int slot, T* U) {
     vec q = sl[v * BLOCK];
     vec_get(q, U + v * N);
   }
-  if (R == 12) {
-#pragma unroll
-    for (int c = 0; c < 3; c++) {
-      const int a = (c + 1) % 3, b = (c + 2) % 3;
-      T re = U[2 * a] * U[6 + 2 * b] - U[2 * a + 1] * U[6 + 2 * b + 1] - U[2 * b] * U[6 + 2 * a] +
-             U[2 * b + 1] * U[6 + 2 * a + 1];
-      T im = U[2 * a] * U[6 + 2 * b + 1] + U[2 * a + 1] * U[6 + 2 * b] - U[2 * b] * U[6 + 2 * a + 1] -
-             U[2 * b + 1] * U[6 + 2 * a];
-      U[12 + 2 * c] = re;
-      U[12 + 2 * c + 1] = -im;
-    }
-  }
+  if (R == 12) recon_row2<T>(U);
 }
 
 template <typename T, int R, int MU, bool FWD, bool DAG, int BLOCK, int SLOT>
@@ -321,6 +389,28 @@ __device__ __forceinline__ void dslash_site_sstaged(T* acc, const T* __restrict_
   }
 }
 
+// y = B x for one packed Hermitian 6x6 block (6 real diagonals, 15 complex lower entries), packed fp32:
+// y_i = sum_j ar_ij (xr, xi)_j + (-1, 1) o sum_j (+-ai_ij) (xi, xr)_j  (lower triangle +, conjugated upper -)
+__device__ __forceinline__ void clover_block_packed(const float* a, const float* x, float* y) {
+#pragma unroll
+  for (int i = 0; i < 6; i++) {
+    u64 accr = mul2(pk2(a[i], a[i]), pk2(x[2 * i], x[2 * i + 1]));
+    u64 acci;
+    bool first = true;
+#pragma unroll
+    for (int j = 0; j < 6; j++) {
+      if (j == i) continue;
+      const int o = j < i ? 6 + 2 * (i * (i - 1) / 2 + j) : 6 + 2 * (j * (j - 1) / 2 + i);
+      const float ar = a[o], ai = j < i ? a[o + 1] : -a[o + 1];
+      const u64 X = pk2(x[2 * j], x[2 * j + 1]), Xs = pk2(x[2 * j + 1], x[2 * j]);
+      accr = fma2(pk2(ar, ar), X, accr);
+      acci = first ? mul2(pk2(ai, ai), Xs) : fma2(pk2(ai, ai), Xs, acci);
+      first = false;
+    }
+    upk2(fma2(pk2(-1.f, 1.f), acci, accr), y[2 * i], y[2 * i + 1]);
+  }
+}
+
 // out = C v for the two Hermitian 6x6 chiral blocks of one site.  cl = one-parity clover field
 // [NCV][Vh]; packed order per block: 6 real diagonal, then 15 complex lower entries row-major.
 // v and out are 24-real spinors (block k acts on reals 12k..12k+11); they must not alias.
@@ -339,6 +429,9 @@ __device__ __forceinline__ void clover_mul(const T* __restrict__ cl, int Vh, int
     }
     const T* x = v + 12 * k;
     T* y = out + 12 * k;
+    if constexpr (UsePacked<T>::value) {
+      clover_block_packed(a, x, y);
+    } else {
 #pragma unroll
     for (int i = 0; i < 6; i++) {
       T re = a[i] * x[2 * i], im = a[i] * x[2 * i + 1];
@@ -360,6 +453,7 @@ __device__ __forceinline__ void clover_mul(const T* __restrict__ cl, int Vh, int
       }
       y[2 * i] = re;
       y[2 * i + 1] = im;
+    }
     }
   }
 }

