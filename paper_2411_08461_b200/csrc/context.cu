@@ -1,6 +1,7 @@
 // Context, error reporting and size queries of liblqcd (include/lqcd.h).
 #include <stdarg.h>
 #include <string.h>
+#include <stdlib.h>
 #include "lqcd_internal.cuh"
 
 int lqcd_set_error(lqcd_ctx* ctx, int code, const char* fmt, ...) {
@@ -72,6 +73,12 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], int prec, int recon, int t_bo
   c->lat.tb = t_boundary;
   c->prec = prec;
   c->ws = 1.0;
+  {
+    // shared-memory tiled dslash (dslash_tiled.cuh): parity-tested, measured slower than the one-thread-per-site
+    // kernel at every tile shape tried (profiles/r01d_tuning.md), so it is opt-in: LQCD_DSLASH_TILED=1
+    const char* e = getenv("LQCD_DSLASH_TILED");
+    c->tiled = (e && e[0] == '1') ? 1 : 0;
+  }
   c->recon = recon;
   c->device = device;
   c->sm_count = prop.multiProcessorCount;

@@ -1,5 +1,6 @@
 // K2 dslash kernel with fused epilogues and K3 clover apply.
 #include "dslash.cuh"
+#include "dslash_tiled.cuh"
 
 // Epilogues (EPI), with d = D_{p,1-p} in  and C = the clover-like field passed in `cl`:
 //   0: out = scale * d
@@ -120,6 +121,50 @@ __global__ void __launch_bounds__(PSUM_BLOCK) partial_sum_kernel(const double* _
   }
 }
 
+// epilogue of one output site (EPI as listed at the top); `local` collects the fp64 reduction term of EPI 4, 5
+template <typename T, int EPI>
+__device__ __forceinline__ void dslash_epilogue(const DslashArgs<T>& a, int idx, const T* acc, double& local) {
+  const int Vh = a.lat.Vh;
+  T res[24];
+  if (EPI == 0) {
+#pragma unroll
+    for (int e = 0; e < 24; e++) res[e] = a.scale * acc[e];
+  } else if (EPI == 1) {
+    clover_mul<T>(a.cl, Vh, idx, acc, res);
+#pragma unroll
+    for (int e = 0; e < 24; e++) res[e] *= a.scale;
+  } else if (EPI == 2 || EPI == 4 || EPI == 5) {
+    T xv[24];
+    load_spinor<T>(a.x, Vh, idx, xv);
+    clover_mul<T>(a.cl, Vh, idx, xv, res);
+#pragma unroll
+    for (int e = 0; e < 24; e++) res[e] += a.scale * acc[e];
+  } else {
+    T xv[24];
+    load_spinor<T>(a.x, Vh, idx, xv);
+    clover_mul<T>(a.cl, Vh, idx, acc, res);
+#pragma unroll
+    for (int e = 0; e < 24; e++) res[e] = xv[e] + a.scale * res[e];
+  }
+  if (EPI == 5) {
+    const T alpha = (T)(a.scalars[a.num] / a.scalars[a.den]);
+    T rv[24];
+    load_spinor<T>(a.r, Vh, idx, rv);
+#pragma unroll
+    for (int e = 0; e < 24; e++) {
+      rv[e] -= alpha * res[e];
+      local += (double)rv[e] * rv[e];
+    }
+    store_spinor<T>(a.r, Vh, idx, rv);
+  } else {
+    if (EPI == 4) {
+#pragma unroll
+      for (int e = 0; e < 24; e++) local += (double)res[e] * res[e];
+    }
+    store_spinor<T>(a.out, Vh, idx, res);
+  }
+}
+
 template <typename T, int R, bool DAG, int EPI>
 __global__ void __launch_bounds__(Tune<T, R>::BLOCK, Tune<T, R>::MINB) dslash_kernel(const DslashArgs<T> a) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
@@ -138,44 +183,7 @@ __global__ void __launch_bounds__(Tune<T, R>::BLOCK, Tune<T, R>::MINB) dslash_ke
     } else {
       dslash_site<T, R, DAG>(acc, a.in, a.gauge, a.lat, idx, a.parity, a.ws);
     }
-    T res[24];
-    if (EPI == 0) {
-#pragma unroll
-      for (int e = 0; e < 24; e++) res[e] = a.scale * acc[e];
-    } else if (EPI == 1) {
-      clover_mul<T>(a.cl, a.lat.Vh, idx, acc, res);
-#pragma unroll
-      for (int e = 0; e < 24; e++) res[e] *= a.scale;
-    } else if (EPI == 2 || EPI == 4 || EPI == 5) {
-      T xv[24];
-      load_spinor<T>(a.x, a.lat.Vh, idx, xv);
-      clover_mul<T>(a.cl, a.lat.Vh, idx, xv, res);
-#pragma unroll
-      for (int e = 0; e < 24; e++) res[e] += a.scale * acc[e];
-    } else {
-      T xv[24];
-      load_spinor<T>(a.x, a.lat.Vh, idx, xv);
-      clover_mul<T>(a.cl, a.lat.Vh, idx, acc, res);
-#pragma unroll
-      for (int e = 0; e < 24; e++) res[e] = xv[e] + a.scale * res[e];
-    }
-    if (EPI == 5) {
-      const T alpha = (T)(a.scalars[a.num] / a.scalars[a.den]);
-      T rv[24];
-      load_spinor<T>(a.r, a.lat.Vh, idx, rv);
-#pragma unroll
-      for (int e = 0; e < 24; e++) {
-        rv[e] -= alpha * res[e];
-        local += (double)rv[e] * rv[e];
-      }
-      store_spinor<T>(a.r, a.lat.Vh, idx, rv);
-    } else {
-      if (EPI == 4) {
-#pragma unroll
-        for (int e = 0; e < 24; e++) local += (double)res[e] * res[e];
-      }
-      store_spinor<T>(a.out, a.lat.Vh, idx, res);
-    }
+    dslash_epilogue<T, EPI>(a, idx, acc, local);
   }
   if (EPI >= 4) dslash_reduce<Tune<T, R>::BLOCK>(local, a.partial);
 }
@@ -191,6 +199,110 @@ __global__ void __launch_bounds__(128) clover_apply_kernel(T* __restrict__ out, 
   load_spinor<T>(in, Vh, idx, v);
   clover_mul<T>(cl, Vh, idx, v, r);
   store_spinor<T>(out, Vh, idx, r);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Tiled kernel (dslash_tiled.cuh): block = one 4-D tile of output sites, neighbour spinors staged through
+// shared memory.  Tile shape and resident blocks per precision (sweep in profiles/r01d_tuning.md).
+// ---------------------------------------------------------------------------------------------
+// output sites per tile: XH (checkerboard sites in x), Y, Z, T
+#ifndef TILE_F32_XH
+#define TILE_F32_XH 4
+#define TILE_F32_Y 4
+#define TILE_F32_Z 4
+#define TILE_F32_T 4
+#endif
+#ifndef TILE_F64_XH
+#define TILE_F64_XH 4
+#define TILE_F64_Y 4
+#define TILE_F64_Z 4
+#define TILE_F64_T 2
+#endif
+#define TILE_F32 TILE_F32_XH, TILE_F32_Y, TILE_F32_Z, TILE_F32_T
+#define TILE_F64 TILE_F64_XH, TILE_F64_Y, TILE_F64_Z, TILE_F64_T
+#ifndef TILE_MINB_F32
+#define TILE_MINB_F32 2
+#endif
+#ifndef TILE_MINB_F64
+#define TILE_MINB_F64 2
+#endif
+template <typename T> struct TileOf;
+template <> struct TileOf<float> { typedef TileShape<TILE_F32> TS; static constexpr int MINB = TILE_MINB_F32, NOUT = TS::NOUT; };
+template <> struct TileOf<double> { typedef TileShape<TILE_F64> TS; static constexpr int MINB = TILE_MINB_F64, NOUT = TS::NOUT; };
+
+template <typename T, int R, bool DAG, int EPI>
+__global__ void __launch_bounds__(TileOf<T>::NOUT, TileOf<T>::MINB) dslash_tiled_kernel(const DslashArgs<T> a) {
+  typedef typename TileOf<T>::TS TS;
+  extern __shared__ __align__(16) unsigned char dslash_smem[];
+  const Lat& L = a.lat;
+  const int ntx = L.Lxh / TS::TXH, nty = L.Ly / TS::TY, ntz = L.Lz / TS::TZ;
+  int b = blockIdx.x;
+  const int x0 = 2 * TS::TXH * (b % ntx);
+  b /= ntx;
+  const int y0 = TS::TY * (b % nty);
+  b /= nty;
+  const int z0 = TS::TZ * (b % ntz);
+  const int t0 = TS::TT * (b / ntz);
+  tile_stage<T, TS>(dslash_smem, a.in, L, x0, y0, z0, t0, 1 - a.parity);
+  int q = threadIdx.x;
+  const int lxh = q % TS::TXH;
+  q /= TS::TXH;
+  const int ly = q % TS::TY;
+  q /= TS::TY;
+  const int lz = q % TS::TZ, lt = q / TS::TZ;
+  Site s;
+  s.xh = (x0 >> 1) + lxh;
+  s.y = y0 + ly;
+  s.z = z0 + lz;
+  s.t = t0 + lt;
+  s.r = (a.parity + s.y + s.z + s.t) & 1;
+  const int idx = s.xh + L.Lxh * (s.y + L.Ly * (s.z + L.Lz * s.t));
+  cp_async_wait<0>();
+  __syncthreads();
+  T acc[24];
+  dslash_site_tiled<T, TS, R, DAG>(acc, dslash_smem, a.gauge, L, idx, a.parity, lxh, ly, lz, lt, s, a.ws);
+  double local = 0;
+  dslash_epilogue<T, EPI>(a, idx, acc, local);
+  if (EPI >= 4) dslash_reduce<TS::NOUT>(local, a.partial);
+}
+
+template <typename T> static bool tile_fits(const Lat& L) {
+  typedef typename TileOf<T>::TS TS;
+  return L.Lxh % TS::TXH == 0 && L.Ly % TS::TY == 0 && L.Lz % TS::TZ == 0 && L.Lt % TS::TT == 0;
+}
+bool lqcd_dslash_tiled(const lqcd_ctx* c) {
+  return c->tiled && (c->prec == 4 ? tile_fits<float>(c->lat) : tile_fits<double>(c->lat));
+}
+// blocks of a single-RHS dslash launch (= per-block partials of the fused epilogues 4, 5)
+int lqcd_dslash_grid(const lqcd_ctx* c) {
+  if (lqcd_dslash_tiled(c)) return c->lat.Vh / (c->prec == 4 ? TileOf<float>::TS::NOUT : TileOf<double>::TS::NOUT);
+  const int block = c->prec == 4 ? DSLASH_BLOCK_F32 : DSLASH_BLOCK_F64;
+  return (c->lat.Vh + block - 1) / block;
+}
+
+template <typename T, int R, bool DAG>
+static void launch_tiled(const DslashArgs<T>& a, int epi, cudaStream_t st) {
+  typedef typename TileOf<T>::TS TS;
+  const int grid = a.lat.Vh / TS::NOUT;
+  const size_t smem = (size_t)TS::NSLOT * 24 * sizeof(T);
+  static bool configured = false;  // one flag per (T, R, DAG) instantiation
+  if (!configured) {
+    cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    configured = true;
+  }
+  switch (epi) {
+    case 0: dslash_tiled_kernel<T, R, DAG, 0><<<grid, TS::NOUT, smem, st>>>(a); break;
+    case 1: dslash_tiled_kernel<T, R, DAG, 1><<<grid, TS::NOUT, smem, st>>>(a); break;
+    case 2: dslash_tiled_kernel<T, R, DAG, 2><<<grid, TS::NOUT, smem, st>>>(a); break;
+    case 3: dslash_tiled_kernel<T, R, DAG, 3><<<grid, TS::NOUT, smem, st>>>(a); break;
+    case 4: dslash_tiled_kernel<T, R, DAG, 4><<<grid, TS::NOUT, smem, st>>>(a); break;
+    default: dslash_tiled_kernel<T, R, DAG, 5><<<grid, TS::NOUT, smem, st>>>(a); break;
+  }
 }
 
 template <typename T, int R, bool DAG>
@@ -237,6 +349,16 @@ static void launch_typed(lqcd_ctx* c, void* out, const void* in, const void* gau
   a.parity = parity;
   a.scale = (T)scale;
   a.ws = (T)c->ws;
+  if (lqcd_dslash_tiled(c)) {
+    if (c->recon == 18) {
+      if (dagger) launch_tiled<T, 18, true>(a, epi, st);
+      else launch_tiled<T, 18, false>(a, epi, st);
+    } else {
+      if (dagger) launch_tiled<T, 12, true>(a, epi, st);
+      else launch_tiled<T, 12, false>(a, epi, st);
+    }
+    return;
+  }
   if (c->recon == 18) {
     if (dagger) launch_epi<T, 18, true>(a, epi, st);
     else launch_epi<T, 18, false>(a, epi, st);
@@ -271,8 +393,7 @@ int lqcd_dslash_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge
 
 // CG-fused epilogues (4, 5) are available when the per-block partials fit the context's scratch
 bool lqcd_dslash_fuse_ok(const lqcd_ctx* c) {
-  const int block = c->prec == 4 ? DSLASH_BLOCK_F32 : DSLASH_BLOCK_F64;
-  return (long)(c->lat.Vh + block - 1) / block <= 4L * c->max_red_blocks * LQCD_MAX_RHS;
+  return (long)lqcd_dslash_grid(c) <= 4L * c->max_red_blocks * LQCD_MAX_RHS;
 }
 
 int lqcd_dslash_fused_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
@@ -284,11 +405,8 @@ int lqcd_dslash_fused_launch(lqcd_ctx* c, void* out, const void* in, const void*
   if (rec) cudaEventRecord(c->prof_ev[2 * c->prof_n], st);
   if (c->prec == 4) launch_typed<float>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, f, st);
   else launch_typed<double>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, f, st);
-  {
-    const int block = c->prec == 4 ? DSLASH_BLOCK_F32 : DSLASH_BLOCK_F64;
-    partial_sum_kernel<<<1, PSUM_BLOCK, 0, st>>>(c->d_partial, (c->lat.Vh + block - 1) / block, c->d_scalars + f->out_slot);
-    c->launches++;
-  }
+  partial_sum_kernel<<<1, PSUM_BLOCK, 0, st>>>(c->d_partial, lqcd_dslash_grid(c), c->d_scalars + f->out_slot);
+  c->launches++;
   if (rec) {
     cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], st);
     c->prof_n++;

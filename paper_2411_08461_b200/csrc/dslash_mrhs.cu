@@ -218,6 +218,175 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kern
   }  // column groups
 }
 
+// ---------------------------------------------------------------------------------------------
+// Staged form (one column per thread): the neighbour spinors of a thread's (site, column) are copied
+// global -> shared memory with per-thread asynchronous 16-byte copies (cp.async.cg), HPR hops per round,
+// two rounds of buffers: while round k is multiplied, round k+1 (the next hops, or the first hops of the
+// thread's NEXT column) is in flight without holding a register.  The one-thread-per-site kernel above
+// is latency bound (ncu: issue slots 43 % busy, DRAM 45 %, 6.5 warps per issue waiting on the long
+// scoreboard, and removing 24 % of its instructions changed nothing): here every thread keeps
+// HPR * 24 reals in flight at all times.  A thread reads only what it copied itself: cp.async.wait_group
+// is the only synchronisation.  Shared memory per thread: 2 * HPR * 24 reals.
+// ---------------------------------------------------------------------------------------------
+// Measured at 32^3x64, 12 columns (profiles/r01d_tuning.md): fp32 12-real links 1003 -> 886 us with one hop per
+// round and 5 blocks/SM; 18-real links and fp64 lose 4-25 % (more shared memory per thread, fewer warps), so the
+// staged kernel runs for <float, 12> only.  HPR = hops per round; 0 = off.
+#ifndef MRHS_HPR_F32_R12
+#define MRHS_HPR_F32_R12 1
+#endif
+#ifndef MRHS_HPR_F32_R18
+#define MRHS_HPR_F32_R18 0
+#endif
+#ifndef MRHS_HPR_F64
+#define MRHS_HPR_F64 0
+#endif
+#ifndef MRHS_SMINB_F32
+#define MRHS_SMINB_F32 5
+#endif
+#ifndef MRHS_SMINB_F64
+#define MRHS_SMINB_F64 3
+#endif
+template <typename T, int R> struct MrhsStage;
+template <> struct MrhsStage<float, 12> { static constexpr int HPR = MRHS_HPR_F32_R12, MINB = MRHS_SMINB_F32; };
+template <> struct MrhsStage<float, 18> { static constexpr int HPR = MRHS_HPR_F32_R18, MINB = MRHS_SMINB_F32; };
+template <> struct MrhsStage<double, 12> { static constexpr int HPR = MRHS_HPR_F64, MINB = MRHS_SMINB_F64; };
+template <> struct MrhsStage<double, 18> { static constexpr int HPR = MRHS_HPR_F64, MINB = MRHS_SMINB_F64; };
+
+template <typename T, int R, int MU, bool FWD, bool DAG>
+__device__ __forceinline__ void hop_mrhs_staged(T* acc, const typename V16<T>::vec* sm, const T* __restrict__ links, int Vh,
+                                                int lidx, T w) {
+  typedef typename V16<T>::vec vec;
+  constexpr int S = (FWD != DAG) ? -1 : +1;
+  T U[18], psi[24], h[12], chi[12];
+  load_link_l1<T, R>(links, Vh, lidx, U);
+#pragma unroll
+  for (int v = 0; v < Lay<T>::NSV; v++) {
+    vec q = sm[v * MRHS_MAXT];
+    vec_get(q, psi + v * V16<T>::N);
+  }
+  project<T, MU, S>(psi, h);
+  su3_mul<T, !FWD>(U, h, chi);
+  reconstruct<T, MU, S>(acc, chi, w);
+}
+
+template <typename T, int R, bool DAG, int EPI>
+__global__ void __launch_bounds__(MRHS_MAXT, MrhsStage<T, R>::MINB) dslash_mrhs_staged_kernel(const MrhsArgs<T> a) {
+  typedef typename V16<T>::vec vec;
+  constexpr int HPR = MrhsStage<T, R>::HPR > 0 ? MrhsStage<T, R>::HPR : 1, NR = 8 / HPR, NSV = Lay<T>::NSV;
+  extern __shared__ __align__(16) unsigned char mrhs_smem[];
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= a.lat.Vh) return;
+  const Lat& L = a.lat;
+  const int Vh = L.Vh, par = a.parity;
+  const size_t stride = a.stride;
+  const Site s = site_of(L, idx, par);
+  const size_t blk = (size_t)R * Vh;
+  // shared memory [buffer][hop of the round][vector][thread]
+  vec* sm = reinterpret_cast<vec*>(mrhs_smem) + threadIdx.y * MRHS_SITES + threadIdx.x;
+  int n[8];
+  n[0] = neighbour<0, +1>(L, idx, s);
+  n[1] = neighbour<0, -1>(L, idx, s);
+  n[2] = neighbour<1, +1>(L, idx, s);
+  n[3] = neighbour<1, -1>(L, idx, s);
+  n[4] = neighbour<2, +1>(L, idx, s);
+  n[5] = neighbour<2, -1>(L, idx, s);
+  n[6] = neighbour<3, +1>(L, idx, s);
+  n[7] = neighbour<3, -1>(L, idx, s);
+  const bool anti = L.tb < 0;
+  const T wf = (anti && s.t == L.Lt - 1) ? (T)-1 : (T)1, wb = (anti && s.t == 0) ? (T)-1 : (T)1;
+  // copies of round rnd (hops rnd*HPR ...) of column `col` into buffer rnd & 1
+  auto issue = [&](const T* __restrict__ col, int rnd) {
+#pragma unroll
+    for (int k = 0; k < HPR; k++) {
+      const vec* g = reinterpret_cast<const vec*>(col) + n[rnd * HPR + k];
+      vec* d = sm + (size_t)((rnd & 1) * HPR + k) * NSV * MRHS_MAXT;
+#pragma unroll
+      for (int v = 0; v < NSV; v++) cp_async<16>(d + v * MRHS_MAXT, g + (size_t)v * Vh);
+    }
+  };
+  int g = threadIdx.y;
+  if (g < a.ngroups) issue(a.in + (size_t)g * stride, 0);
+  cp_async_commit();
+  for (; g < a.ngroups; g += blockDim.y) {
+    const size_t first = (size_t)g * stride;
+    const T* in = a.in + first;
+    const bool more = g + (int)blockDim.y < a.ngroups;
+    T acc[1][24];
+#pragma unroll
+    for (int e = 0; e < 24; e++) acc[0][e] = 0;
+#pragma unroll
+    for (int rnd = 0; rnd < NR; rnd++) {
+      if (rnd + 1 < NR) issue(in, rnd + 1);
+      else if (more) issue(in + (size_t)blockDim.y * stride, 0);
+      cp_async_commit();
+      cp_async_wait<1>();
+#pragma unroll
+      for (int k = 0; k < HPR; k++) {
+        const int H = rnd * HPR + k;
+        const vec* b = sm + (size_t)((rnd & 1) * HPR + k) * NSV * MRHS_MAXT;
+        switch (H) {
+          case 0: hop_mrhs_staged<T, R, 0, true, DAG>(acc[0], b, a.gauge + (0 * 2 + par) * blk, Vh, idx, a.ws); break;
+          case 1: hop_mrhs_staged<T, R, 0, false, DAG>(acc[0], b, a.gauge + (0 * 2 + 1 - par) * blk, Vh, n[1], a.ws); break;
+          case 2: hop_mrhs_staged<T, R, 1, true, DAG>(acc[0], b, a.gauge + (1 * 2 + par) * blk, Vh, idx, a.ws); break;
+          case 3: hop_mrhs_staged<T, R, 1, false, DAG>(acc[0], b, a.gauge + (1 * 2 + 1 - par) * blk, Vh, n[3], a.ws); break;
+          case 4: hop_mrhs_staged<T, R, 2, true, DAG>(acc[0], b, a.gauge + (2 * 2 + par) * blk, Vh, idx, a.ws); break;
+          case 5: hop_mrhs_staged<T, R, 2, false, DAG>(acc[0], b, a.gauge + (2 * 2 + 1 - par) * blk, Vh, n[5], a.ws); break;
+          case 6: hop_mrhs_staged<T, R, 3, true, DAG>(acc[0], b, a.gauge + (3 * 2 + par) * blk, Vh, idx, wf); break;
+          default: hop_mrhs_staged<T, R, 3, false, DAG>(acc[0], b, a.gauge + (3 * 2 + 1 - par) * blk, Vh, n[7], wb); break;
+        }
+      }
+    }
+    T* out = a.out + first;
+    if (EPI == 0) {
+#pragma unroll
+      for (int e = 0; e < 24; e++) acc[0][e] *= a.scale;
+      store_spinor<T>(out, Vh, idx, acc[0]);
+    } else if (EPI == 1) {
+      T res[1][24];
+      clover_mul_mrhs<T, 1>(a.cl, Vh, idx, acc, res);
+#pragma unroll
+      for (int e = 0; e < 24; e++) res[0][e] *= a.scale;
+      store_spinor<T>(out, Vh, idx, res[0]);
+    } else if (EPI == 2) {
+      T xv[1][24], res[1][24];
+      load_spinor<T>(a.x + first, Vh, idx, xv[0]);
+      clover_mul_mrhs<T, 1>(a.cl, Vh, idx, xv, res);
+#pragma unroll
+      for (int e = 0; e < 24; e++) res[0][e] += a.scale * acc[0][e];
+      store_spinor<T>(out, Vh, idx, res[0]);
+    } else {
+      T res[1][24], xv[24];
+      clover_mul_mrhs<T, 1>(a.cl, Vh, idx, acc, res);
+      load_spinor<T>(a.x + first, Vh, idx, xv);
+#pragma unroll
+      for (int e = 0; e < 24; e++) res[0][e] = xv[e] + a.scale * res[0][e];
+      store_spinor<T>(out, Vh, idx, res[0]);
+    }
+  }
+}
+
+template <typename T, int R, bool DAG>
+static void launch_mrhs_staged(MrhsArgs<T> a, int epi, int nrhs, cudaStream_t st) {
+  a.ngroups = nrhs;
+  const dim3 block(MRHS_SITES, a.ngroups < MRHS_GMAX ? a.ngroups : MRHS_GMAX);
+  const int grid = (a.lat.Vh + MRHS_SITES - 1) / MRHS_SITES;
+  const size_t smem = (size_t)2 * MrhsStage<T, R>::HPR * 24 * sizeof(T) * MRHS_MAXT;
+  static bool configured = false;  // one flag per (T, R, DAG) instantiation
+  if (!configured && smem > 48 * 1024) {
+    cudaFuncSetAttribute(dslash_mrhs_staged_kernel<T, R, DAG, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_mrhs_staged_kernel<T, R, DAG, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_mrhs_staged_kernel<T, R, DAG, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_mrhs_staged_kernel<T, R, DAG, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  }
+  configured = true;
+  switch (epi) {
+    case 0: dslash_mrhs_staged_kernel<T, R, DAG, 0><<<grid, block, smem, st>>>(a); break;
+    case 1: dslash_mrhs_staged_kernel<T, R, DAG, 1><<<grid, block, smem, st>>>(a); break;
+    case 2: dslash_mrhs_staged_kernel<T, R, DAG, 2><<<grid, block, smem, st>>>(a); break;
+    default: dslash_mrhs_staged_kernel<T, R, DAG, 3><<<grid, block, smem, st>>>(a); break;
+  }
+}
+
 template <typename T, int R, bool DAG, int NB>
 static void launch_mrhs_epi(MrhsArgs<T> a, int epi, int nrhs, cudaStream_t st) {
   a.ngroups = nrhs / NB;
@@ -233,6 +402,10 @@ static void launch_mrhs_epi(MrhsArgs<T> a, int epi, int nrhs, cudaStream_t st) {
 
 template <typename T, int R, bool DAG>
 static void launch_mrhs_nb(const MrhsArgs<T>& a, int epi, int nrhs, cudaStream_t st) {
+  if (MrhsStage<T, R>::HPR > 0) {
+    launch_mrhs_staged<T, R, DAG>(a, epi, nrhs, st);
+    return;
+  }
   // columns per thread: the tuned NB when it divides nrhs, else one per thread
   if (nrhs % MrhsTune<T>::NB == 0) launch_mrhs_epi<T, R, DAG, MrhsTune<T>::NB>(a, epi, nrhs, st);
   else launch_mrhs_epi<T, R, DAG, 1>(a, epi, nrhs, st);

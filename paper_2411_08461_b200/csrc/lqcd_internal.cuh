@@ -23,6 +23,7 @@ struct lqcd_ctx {
   long V;
   int prec, recon, device, sm_count;
   double ws;  // weight of the spatial hops: nu/xi_0 of Eq. 5; 1 = isotropic
+  int tiled;  // 1: shared-memory tiled dslash where the tile divides the lattice (opt-in: LQCD_DSLASH_TILED=1)
   long launches;
   char err[256];
   // reduction scratch (device): per-block partials, ticket counter, result slots; pinned host mirror

@@ -61,7 +61,10 @@ def test_pack_unpack_roundtrip():
 
 
 @pytest.mark.parametrize("prec,recon", [(8, 18), (8, 12), (4, 18), (4, 12)])
-@pytest.mark.parametrize("dims,tb", [((4, 4, 4, 8), -1), ((4, 6, 8, 10), -1), ((8, 8, 8, 16), 1), ((12, 4, 6, 4), -1)])
+@pytest.mark.parametrize("dims,tb", [((4, 4, 4, 8), -1), ((4, 6, 8, 10), -1), ((8, 8, 8, 16), 1), ((12, 4, 6, 4), -1),
+                                     # shared-memory tiled kernel (csrc/dslash_tiled.cuh): several tiles in every
+                                     # direction, and tiles that span a whole extent (halo wraps onto the tile itself)
+                                     ((16, 8, 4, 8), -1), ((8, 4, 8, 4), -1), ((24, 12, 8, 6), 1)])
 def test_dslash_matches_oracle(prec, recon, dims, tb):
     s = Setup(dims, 0.5, 2, 0.124, 1.2, prec, recon, tb, with_clover=False)
     psi = s.spinor("gaussian", 102)
@@ -178,3 +181,36 @@ def test_blas_kernels():
         assert rel_err(s.down(full)[0], ze) < 10 * tol
         # deterministic: the same reduction twice gives the same bits
         assert ctx.blas_cdot(x, y) == ctx.blas_cdot(x, y)
+
+
+@pytest.mark.parametrize("prec,recon", [(8, 18), (8, 12), (4, 18), (4, 12)])
+@pytest.mark.parametrize("dims,tb", [((16, 8, 4, 8), -1), ((8, 8, 8, 16), -1), ((8, 4, 8, 4), 1)])
+def test_tiled_dslash_matches_oracle(prec, recon, dims, tb, monkeypatch):
+    """The opt-in shared-memory tiled kernel (csrc/dslash_tiled.cuh, LQCD_DSLASH_TILED=1 at context creation):
+    several tiles per direction, tiles spanning a whole extent (the halo wraps onto the tile itself), the seam in t,
+    every epilogue through M and M-hat, and the CG-fused epilogues 4 and 5 through a CGNE solve."""
+    monkeypatch.setenv("LQCD_DSLASH_TILED", "1")
+    s = Setup(dims, 0.5, 2, 0.124, 1.2, prec, recon, tb)
+    psi = s.spinor("gaussian", 102)
+    nat = s.up(psi)
+    out = s.ctx.new_spinor(2)
+    for dagger in (False, True):
+        want = s.orc.dslash(psi, dagger=dagger)
+        for p in (0, 1):
+            s.ctx.dslash(s.ctx.parity(out, p), s.ctx.parity(nat, 1 - p), s.gauge, p, 1.0, dagger)
+        got = s.down(out)
+        for p in (0, 1):
+            assert rel_err(got[p], want[p]) < TOL[prec], (dagger, p)
+        s.ctx.mat_apply(out, nat, s.gauge, s.A, s.kappa, dagger)
+        assert rel_err(s.down(out), s.orc.mat(psi, dagger)) < TOL[prec]
+    pe = psi.copy()
+    pe[1] = 0
+    for matpc in (0, 1):
+        for dagger in (False, True):
+            out.zero_()
+            s.ctx.mpc_apply(s.ctx.parity(out, 0), s.ctx.parity(nat, 0), s.gauge, s.A, s.Ai, s.kappa, matpc, dagger)
+            assert rel_err(s.down(out), s.orc.mpc(pe, matpc, dagger)) < TOL[prec], (matpc, dagger)
+    tol = 1e-10 if prec == 8 else 1e-6
+    x, res = s.ctx.invert(s.ctx.to_device(psi), s.gauge, s.A, s.Ai, s.kappa, tol=tol, maxiter=2000, solver="cgne", matpc=0)
+    assert res.status == 0
+    assert s.orc.true_residual(psi, x.cpu().numpy().astype(np.complex128)) < (tol if prec == 8 else 2e-6)
