@@ -236,6 +236,30 @@ def extras(torch, lqcd, synth, U, b, ctx, gauge, device):
                          "mixed_true_resid": rmx.true_resid, "fp64_true_resid": r64.true_resid,
                          "speedup": r64.seconds / rmx.seconds}
     out["mixed_precision_32x64"] = mixed
+    # 12-column point-source propagator at the headline size to the fp64 tolerance: 12 mixed
+    # solves one after the other vs one batched mixed solve (lqcd_invert_multi_mixed), BiCGStab
+    dims = cfg["dims"]
+    cols = np.stack([synth.source(dims, "point", spin=sp, colour=c) for sp in range(4) for c in range(3)])
+    B = ctx.to_device(cols)
+    ws, _ = ctx.workspace_multi(12, "bicgstab")
+    ws_lo, _ = lo.workspace_multi(12, "bicgstab")
+    for _ in range(2):
+        e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        e0.record()
+        r1 = [ctx.invert_mixed(lo, B[j], gauge, A, Ai, g_lo, A_lo, Ai_lo, kappa, tol=1e-10, inner_tol=1e-5,
+                               maxiter=2000, solver="bicgstab", workspace=ws, workspace_lo=ws_lo)[1] for j in range(12)]
+        e1.record()
+        _, rs, rc = ctx.invert_multi_mixed(lo, B, gauge, A, Ai, g_lo, A_lo, Ai_lo, kappa, tol=1e-10, inner_tol=1e-5,
+                                           maxiter=2000, solver="bicgstab", workspace=ws, workspace_lo=ws_lo)
+        e2.record()
+        torch.cuda.synchronize()
+    out["propagator_32x64_mixed_bicgstab"] = {
+        "single_solves_ms": e0.elapsed_time(e1), "batched_ms": e1.elapsed_time(e2),
+        "speedup": e0.elapsed_time(e1) / e1.elapsed_time(e2),
+        "inner_iterations_single": [r.iterations for r in r1], "inner_iterations_batched": [r.iterations for r in rs],
+        "status": rc, "worst_true_resid_single": max(r.true_resid for r in r1),
+        "worst_true_resid_batched": max(r.true_resid for r in rs)}
+    del B, ws, ws_lo
     lo.close()
     del A, Ai, g_lo, A_lo, Ai_lo
     c3 = synth.CONFIGS[3]

@@ -176,7 +176,17 @@ int lqcd_invert_multi(lqcd_ctx* ctx, void* x_public, const void* b_public, const
  * clover_inv, workspace (as lqcd_invert); ctx_lo: fp32 context of the same lattice/boundary/device
  * owning gauge_lo, clover_lo, clover_inv_lo (its own pack/clover_build of the same links; the
  * reconstructions may differ) and workspace_lo (>= lqcd_invert_workspace_bytes(ctx_lo)).
- * res->iterations counts inner iterations; true_resid is recomputed in fp64.  Host-synchronous. */
+ * res->iterations counts inner iterations; true_resid is recomputed in fp64.  Host-synchronous.
+ * lqcd_invert_multi_mixed: the same for nrhs columns (x_public/b_public: nrhs consecutive public spinors,
+ * res: nrhs results, as lqcd_invert_multi): every outer step is ONE batched fp32 solve (multi-RHS kernels:
+ * links loaded once per site for all columns) over the columns still above their fp64 stopping test;
+ * workspace >= lqcd_invert_multi_workspace_bytes(ctx, solver, nrhs), workspace_lo likewise for ctx_lo.
+ * Returns the worst status over the columns (as lqcd_invert_multi). */
+int lqcd_invert_multi_mixed(lqcd_ctx* ctx, lqcd_ctx* ctx_lo, void* x_public, const void* b_public, const void* gauge,
+                            const void* clover, const void* clover_inv, const void* gauge_lo, const void* clover_lo,
+                            const void* clover_inv_lo, double kappa, double tol, double inner_tol, int maxiter,
+                            int solver, int matpc, int nrhs, void* workspace, size_t workspace_bytes,
+                            void* workspace_lo, size_t workspace_lo_bytes, lqcd_result* res, void* stream);
 int lqcd_invert_mixed(lqcd_ctx* ctx, lqcd_ctx* ctx_lo, void* x_public, const void* b_public, const void* gauge,
                       const void* clover, const void* clover_inv, const void* gauge_lo, const void* clover_lo,
                       const void* clover_inv_lo, double kappa, double tol, double inner_tol, int maxiter, int solver,

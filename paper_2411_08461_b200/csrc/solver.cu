@@ -363,72 +363,107 @@ static int solve_cg(lqcd_ctx* c, const Work& w, const void* gauge, const void* A
 static int solve_bicgstab(lqcd_ctx* c, const Work& w, const void* gauge, const void* A, const void* Ai, double kappa,
                           int matpc, Cols& cols, int maxiter, lqcd_result* res, cudaStream_t st);
 
-// single right-hand side; bhat in w.v[0], x_e (zeroed) in w.x; fills cols.rr[0], res->iterations
+// bhat in w.v[0], x_e (zeroed) in w.x, w.nrhs columns in lock step: every outer step runs ONE batched fp32 solve
+// over the columns still above their fp64 stopping test (the others are frozen in the inner solve and skipped
+// in the fp64 update); fills cols.rr[j], res[j].iterations (inner iterations that column took part in).
 static int solve_mixed(lqcd_ctx* c, const Work& w, const void* gauge, const void* A, const void* Ai, double kappa,
                        int matpc, int solver, Cols& cols, int maxiter, lqcd_result* res, Mixed& m, cudaStream_t st) {
   lqcd_ctx* ci = m.ci;
   char *bh = w.v[0], *r = w.v[1], *mx = w.v[2], *tmp = w.v[5], *x = w.x;
-  const size_t sp = lqcd_spinor_bytes(c);
+  const int n = w.nrhs;
+  const size_t sp = lqcd_spinor_bytes(c), spi = lqcd_spinor_bytes(ci);
   const int Vh = c->lat.Vh, grid = (Vh + 255) / 256;
   int rc;
-  cudaMemcpyAsync(r, bh, sp, cudaMemcpyDeviceToDevice, st);
-  double rr = 0;
+  cudaMemcpyAsync(r, bh, sp * n, cudaMemcpyDeviceToDevice, st);
+  double rr[LQCD_MAX_RHS];
+  bool live[LQCD_MAX_RHS];
+  int iters[LQCD_MAX_RHS];
   {
     void* v[1] = {r};
     int o[4] = {S_RES, 0, 0, 0};
-    if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v, o, 1, 0, st))) return rc;
-    if ((rc = read_scalars(c, 1, st))) return rc;
-    rr = hs(c, 0, S_RES);
+    if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v, o, n, 0, st))) return rc;
+    if ((rc = read_scalars(c, n, st))) return rc;
+  }
+  int nlive = 0;
+  for (int j = 0; j < n; j++) {
+    rr[j] = cols.active[j] ? hs(c, j, S_RES) : 0.0;
+    live[j] = cols.active[j] && rr[j] > cols.stop2[j];
+    iters[j] = 0;
+    nlive += live[j];
   }
   int total = 0, outer = 0;
-  while (rr > cols.stop2[0] && total < maxiter && outer < 64) {
-    const double rn = sqrt(rr);
-    spinor_down_kernel<<<grid, 256, 0, st>>>((float4*)m.wi.v[0], (const double2*)r, Vh, 1.0 / rn);
-    c->alg_bytes += (double)Vh * 24 * 12;
-    LQCD_LAUNCH_CHECK(c, "spinor_down");
-    // inner fp32 solve of Mhat e = r/|r|, relative tolerance tol_k
-    const double need = 0.25 * sqrt(cols.stop2[0] / rr);
-    const double tol_k = need > m.inner_tol ? need : m.inner_tol;
+  while (nlive > 0 && total < maxiter && outer < 64) {
     Cols ic;
-    ic.n = 1;
-    ic.active[0] = true;
-    ic.bb[0] = 1.0;
-    ic.stop2[0] = tol_k * tol_k;
-    ic.rr[0] = 1.0;
-    cudaMemsetAsync(ci->d_scalars, 0, sizeof(double) * SC_STRIDE, st);
-    lqcd_result ri;
-    memset(&ri, 0, sizeof(ri));
+    ic.n = n;
+    cudaMemsetAsync(ci->d_scalars, 0, sizeof(double) * SC_STRIDE * n, st);
+    double rn[LQCD_MAX_RHS];
+    for (int j = 0; j < n; j++) {
+      ic.active[j] = live[j];
+      ic.bb[j] = 1.0;
+      ic.rr[j] = 1.0;
+      ic.stop2[j] = 1.0;
+      if (!live[j]) {
+        set_slot(ci, j, S_DONE, true, st);
+        continue;
+      }
+      rn[j] = sqrt(rr[j]);
+      spinor_down_kernel<<<grid, 256, 0, st>>>((float4*)(m.wi.v[0] + j * spi), (const double2*)(r + j * sp), Vh, 1.0 / rn[j]);
+      c->alg_bytes += (double)Vh * 24 * 12;
+      LQCD_LAUNCH_CHECK(c, "spinor_down");
+      // inner fp32 solve of Mhat e = r/|r|, relative tolerance tol_k
+      const double need = 0.25 * sqrt(cols.stop2[j] / rr[j]);
+      const double tol_k = need > m.inner_tol ? need : m.inner_tol;
+      ic.stop2[j] = tol_k * tol_k;
+    }
+    lqcd_result ri[LQCD_MAX_RHS];
+    memset(ri, 0, sizeof(ri));
+    ci->acct_rhs = nlive;
+    if (solver == LQCD_SOLVER_BICGSTAB) rc = solve_bicgstab(ci, m.wi, m.gauge, m.A, m.Ai, kappa, matpc, ic, maxiter - total, ri, st);
+    else rc = solve_cg(ci, m.wi, m.gauge, m.A, m.Ai, kappa, matpc, solver == LQCD_SOLVER_CGNR, ic, maxiter - total, ri, st);
     ci->acct_rhs = 0;
-    if (solver == LQCD_SOLVER_BICGSTAB) rc = solve_bicgstab(ci, m.wi, m.gauge, m.A, m.Ai, kappa, matpc, ic, maxiter - total, &ri, st);
-    else rc = solve_cg(ci, m.wi, m.gauge, m.A, m.Ai, kappa, matpc, solver == LQCD_SOLVER_CGNR, ic, maxiter - total, &ri, st);
     if (rc) return lqcd_set_error(c, rc, "invert_mixed: inner solve: %s", ci->err);
-    total += ri.iterations;
-    res->dslash_count += ri.dslash_count;
-    if (ri.status < 0) { res->status = ri.status; break; }
-    // x += |r| e ; r = bhat - Mhat x (fp64)
-    spinor_up_axpy_kernel<<<grid, 256, 0, st>>>((double2*)x, (const float4*)m.wi.x, Vh, rn);
-    c->alg_bytes += (double)Vh * 24 * 20;
-    LQCD_LAUNCH_CHECK(c, "spinor_up_axpy");
-    if ((rc = mpc_apply(c, mx, x, gauge, A, Ai, kappa, matpc, 0, tmp, 1, st))) return rc;
-    res->dslash_count += 2;
+    int step = 0;
+    bool broke = false;
+    for (int j = 0; j < n; j++) {
+      if (!live[j]) continue;
+      iters[j] += ri[j].iterations;
+      step = ri[j].iterations > step ? ri[j].iterations : step;
+      res[j].dslash_count += ri[j].dslash_count;
+      if (ri[j].status < 0) { res[j].status = ri[j].status; live[j] = false; nlive--; broke = true; continue; }
+      // x += |r| e
+      spinor_up_axpy_kernel<<<grid, 256, 0, st>>>((double2*)(x + j * sp), (const float4*)(m.wi.x + j * spi), Vh, rn[j]);
+      c->alg_bytes += (double)Vh * 24 * 20;
+      LQCD_LAUNCH_CHECK(c, "spinor_up_axpy");
+    }
+    total += step;
+    if (broke && n == 1) break;
+    // r = bhat - Mhat x in fp64, all columns (a frozen column reproduces its residual)
+    if ((rc = mpc_apply(c, mx, x, gauge, A, Ai, kappa, matpc, 0, tmp, n, st))) return rc;
+    for (int j = 0; j < n; j++) res[j].dslash_count += 2;
     {
       void* v[2] = {bh, mx};
-      if ((rc = BLAS_CALL(c, OpXpay, op.a = -1.0, v, nullptr, 1, 0, st))) return rc;  // mx = bhat - Mhat x
+      if ((rc = BLAS_CALL(c, OpXpay, op.a = -1.0, v, nullptr, n, 0, st))) return rc;  // mx = bhat - Mhat x
       void* v2[1] = {mx};
       int o[4] = {S_RES, 0, 0, 0};
-      if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v2, o, 1, 0, st))) return rc;
-      if ((rc = read_scalars(c, 1, st))) return rc;
+      if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v2, o, n, 0, st))) return rc;
+      if ((rc = read_scalars(c, n, st))) return rc;
     }
     char* sw = r; r = mx; mx = sw;
-    const double rr_new = hs(c, 0, S_RES);
     outer++;
-    if (!(rr_new == rr_new)) { res->status = LQCD_ERR_BREAKDOWN; rr = rr_new; break; }
-    if (rr_new > 0.81 * rr) { rr = rr_new; break; }  // fp32 inner solves no longer reduce the fp64 residual
-    rr = rr_new;
+    for (int j = 0; j < n; j++) {
+      if (!live[j]) continue;
+      const double rr_new = hs(c, j, S_RES);
+      const bool nan = !(rr_new == rr_new), stalled = rr_new > 0.81 * rr[j];  // fp32 solves no longer reduce the fp64 residual
+      rr[j] = rr_new;
+      if (nan) res[j].status = LQCD_ERR_BREAKDOWN;
+      if (nan || stalled || !(rr_new > cols.stop2[j])) { live[j] = false; nlive--; }
+    }
   }
-  cols.rr[0] = rr;
-  res->iterations = total;
-  c->launches += 0;
+  for (int j = 0; j < n; j++) {
+    if (!cols.active[j]) continue;
+    cols.rr[j] = rr[j];
+    res[j].iterations = iters[j];
+  }
   return LQCD_OK;
 }
 
@@ -585,29 +620,40 @@ int lqcd_invert_multi(lqcd_ctx* c, void* x_public, const void* b_public, const v
                        workspace, workspace_bytes, res, as_stream(stream));
 }
 
-int lqcd_invert_mixed(lqcd_ctx* c, lqcd_ctx* ci, void* x_public, const void* b_public, const void* gauge,
-                      const void* clover, const void* clover_inv, const void* gauge_lo, const void* clover_lo,
-                      const void* clover_inv_lo, double kappa, double tol, double inner_tol, int maxiter, int solver,
-                      int matpc, void* workspace, size_t workspace_bytes, void* workspace_lo, size_t workspace_lo_bytes,
-                      lqcd_result* res, void* stream) {
+int lqcd_invert_multi_mixed(lqcd_ctx* c, lqcd_ctx* ci, void* x_public, const void* b_public, const void* gauge,
+                            const void* clover, const void* clover_inv, const void* gauge_lo, const void* clover_lo,
+                            const void* clover_inv_lo, double kappa, double tol, double inner_tol, int maxiter, int solver,
+                            int matpc, int nrhs, void* workspace, size_t workspace_bytes, void* workspace_lo,
+                            size_t workspace_lo_bytes, lqcd_result* res, void* stream) {
   if (!c || !ci || !clover || !clover_inv || !gauge_lo || !clover_lo || !clover_inv_lo || !workspace_lo)
     return LQCD_ERR_INVALID_ARG;
   if (c->prec != 8 || ci->prec != 4 || c->device != ci->device || c->lat.tb != ci->lat.tb || c->L[0] != ci->L[0] ||
-      c->L[1] != ci->L[1] || c->L[2] != ci->L[2] || c->L[3] != ci->L[3] || !(inner_tol > 0) || !(inner_tol < 1))
+      c->L[1] != ci->L[1] || c->L[2] != ci->L[2] || c->L[3] != ci->L[3] || !(inner_tol > 0) || !(inner_tol < 1) ||
+      nrhs < 1 || nrhs > LQCD_MAX_RHS)
     return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "invert_mixed: needs an fp64 and an fp32 context of the same lattice");
-  if (workspace_lo_bytes < lqcd_invert_workspace_bytes(ci, solver))
+  if (workspace_lo_bytes < lqcd_invert_multi_workspace_bytes(ci, solver, nrhs))
     return lqcd_set_error(c, LQCD_ERR_WORKSPACE, "invert_mixed: low-precision workspace too small");
   const void* p[4] = {gauge_lo, clover_lo, clover_inv_lo, workspace_lo};
   if (!check_ptrs(c, p, 4, "invert_mixed")) return LQCD_ERR_ALIGN;
   Mixed m;
   m.ci = ci;
-  carve(ci, workspace_lo, m.wi, 1, false);
+  carve(ci, workspace_lo, m.wi, nrhs, false);
   m.gauge = gauge_lo;
   m.A = clover_lo;
   m.Ai = clover_inv_lo;
   m.inner_tol = inner_tol;
-  return invert_common(c, x_public, b_public, gauge, clover, clover_inv, kappa, 0.0, tol, maxiter, solver, matpc, 1,
+  return invert_common(c, x_public, b_public, gauge, clover, clover_inv, kappa, 0.0, tol, maxiter, solver, matpc, nrhs,
                        workspace, workspace_bytes, res, as_stream(stream), &m);
+}
+
+int lqcd_invert_mixed(lqcd_ctx* c, lqcd_ctx* ci, void* x_public, const void* b_public, const void* gauge,
+                      const void* clover, const void* clover_inv, const void* gauge_lo, const void* clover_lo,
+                      const void* clover_inv_lo, double kappa, double tol, double inner_tol, int maxiter, int solver,
+                      int matpc, void* workspace, size_t workspace_bytes, void* workspace_lo, size_t workspace_lo_bytes,
+                      lqcd_result* res, void* stream) {
+  return lqcd_invert_multi_mixed(c, ci, x_public, b_public, gauge, clover, clover_inv, gauge_lo, clover_lo, clover_inv_lo,
+                                 kappa, tol, inner_tol, maxiter, solver, matpc, 1, workspace, workspace_bytes, workspace_lo,
+                                 workspace_lo_bytes, res, stream);
 }
 
 size_t lqcd_host_scratch_bytes(const lqcd_ctx* c, int solver) {

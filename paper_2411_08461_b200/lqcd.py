@@ -35,7 +35,7 @@ SYMBOLS = [
     "lqcd_invert", "lqcd_host_scratch_bytes", "lqcd_dslash_host", "lqcd_invert_host",
     "lqcd_blas_axpy_norm", "lqcd_blas_xpay", "lqcd_blas_cdot", "lqcd_blas_caxpbypz",
     "lqcd_dslash_mrhs", "lqcd_mpc_apply_mrhs", "lqcd_invert_multi_workspace_bytes", "lqcd_invert_multi",
-    "lqcd_invert_mixed", "lqcd_set_anisotropy", "lqcd_clover_build_aniso",
+    "lqcd_invert_mixed", "lqcd_invert_multi_mixed", "lqcd_set_anisotropy", "lqcd_clover_build_aniso",
     "lqcd_momentum_phase", "lqcd_source_wall", "lqcd_source_point", "lqcd_propagator_assemble",
     "lqcd_propagator_split", "lqcd_contract_twopt", "lqcd_contract_threept", "lqcd_sequential_source",
 ]
@@ -104,6 +104,8 @@ def load():
                                     ctypes.POINTER(Result), vp]
     L.lqcd_invert_mixed.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, cd, cd, cd, ci, ci, ci, vp, sz, vp, sz,
                                     ctypes.POINTER(Result), vp]
+    L.lqcd_invert_multi_mixed.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, cd, cd, cd, ci, ci, ci, ci, vp, sz,
+                                          vp, sz, ctypes.POINTER(Result), vp]
     L.lqcd_dslash_host.argtypes = [vp, vp, vp, vp, ci, cd, ci, vp, vp]
     L.lqcd_invert_host.argtypes = [vp, vp, vp, vp, vp, vp, cd, cd, ci, ci, ci, vp, sz,
                                    ctypes.POINTER(Result), vp]
@@ -331,6 +333,27 @@ class Context:
                                         workspace_lo.numel() * lo.prec, ctypes.byref(res), _stream())
         self._check(rc, allow_not_converged=True)
         return x, res
+
+    def invert_multi_mixed(self, lo, b_public, gauge, clover, clover_inv, gauge_lo, clover_lo, clover_inv_lo, kappa,
+                           tol=1e-10, inner_tol=1e-4, maxiter=1000, solver="cgne", matpc=0, workspace=None,
+                           workspace_lo=None):
+        """Batched mixed-precision solve.  b_public: [nrhs, 2, Lt, Lz, Ly, Lx/2, 4, 3] fp64 device tensor;
+        returns (x, [Result]*nrhs, status)."""
+        nrhs = b_public.shape[0]
+        if workspace is None:
+            workspace, _ = self.workspace_multi(nrhs, solver)
+        if workspace_lo is None:
+            workspace_lo, _ = lo.workspace_multi(nrhs, solver)
+        x = torch.empty_like(b_public)
+        res = (Result * nrhs)()
+        rc = self.lib.lqcd_invert_multi_mixed(self.h, lo.h, _p(x), _p(b_public), _p(gauge), _p(clover), _p(clover_inv),
+                                              _p(gauge_lo), _p(clover_lo), _p(clover_inv_lo), kappa, tol, inner_tol,
+                                              maxiter, SOLVERS[solver], matpc, nrhs, _p(workspace),
+                                              workspace.numel() * self.prec, _p(workspace_lo),
+                                              workspace_lo.numel() * lo.prec, res, _stream())
+        if rc < 0 and rc != -7:
+            self._check(rc)
+        return x, list(res), rc
 
     # ---- sources, propagators, contractions (PAPER.md:151-262) ----------------------------------
     def _gamma(self, g):

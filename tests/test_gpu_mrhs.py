@@ -133,3 +133,39 @@ def test_config3_propagator_12_columns_batched_fp32_recon12():
     S00 = prop[0, 0, 0, 0, 0].transpose(0, 2, 1, 3).reshape(12, 12)
     g5 = np.repeat([1, 1, -1, -1.0], 3)
     assert np.abs(g5[:, None] * S00 * g5[None, :] - S00.conj().T).max() < 1e-5 * np.abs(S00).max()
+
+
+@pytest.mark.parametrize("solver", ["cgne", "bicgstab"])
+def test_invert_multi_mixed_fp64_tolerance_config2(solver):
+    """Batched mixed precision (SURVEY.md §8(f) ranks 1+2): fp64 defect correction around ONE batched fp32
+    reconstruct-12 solve per outer step.  Every column (point, Z2, Gaussian, zero, point) must meet the bar of
+    its own pure fp64 solve (reading A17): oracle solution within 10*tol, oracle-evaluated true residual < tol."""
+    s, c = from_cfg(2, 8, 18)
+    dims = c["dims"]
+    lo = lq().Context(dims, 4, 12, -1)
+    g_lo = lo.gauge_pack(lo.to_device(s.U))
+    A_lo, Ai_lo = lo.clover_build(g_lo, c["csw"], c["kappa"])
+    bs = [synth.source(dims, "point", spin=1, colour=2), synth.source(dims, "z2", 102),
+          synth.source(dims, "gaussian", 5), np.zeros_like(synth.source(dims, "point")),
+          synth.source(dims, "point", spin=3, colour=0)]
+    B = s.ctx.to_device(np.stack(bs))
+    x, res, rc = s.ctx.invert_multi_mixed(lo, B, s.gauge, s.A, s.Ai, g_lo, A_lo, Ai_lo, s.kappa, tol=1e-10,
+                                          inner_tol=1e-4, maxiter=2000, solver=solver)
+    assert rc == 0, [r.as_dict() for r in res]
+    xs = x.cpu().numpy()
+    for r, b in enumerate(bs):
+        assert res[r].status == 0
+        if not b.any():
+            assert res[r].iterations == 0 and not xs[r].any()
+            continue
+        true = s.orc.true_residual(b, xs[r])
+        assert true < 1e-10 and abs(true - res[r].true_resid) < 5e-11, (r, true, res[r].as_dict())
+        xo, ro = s.orc.invert(b, 1e-12, 2000, "bicgstab", 0)
+        assert rel_err(xs[r], xo) < 1e-9, r
+    # one column through the batched entry point = lqcd_invert_mixed
+    x1, res1, rc1 = s.ctx.invert_multi_mixed(lo, B[1:2], s.gauge, s.A, s.Ai, g_lo, A_lo, Ai_lo, s.kappa, tol=1e-10,
+                                             inner_tol=1e-4, maxiter=2000, solver=solver)
+    x2, res2 = s.ctx.invert_mixed(lo, B[1], s.gauge, s.A, s.Ai, g_lo, A_lo, Ai_lo, s.kappa, tol=1e-10,
+                                  inner_tol=1e-4, maxiter=2000, solver=solver)
+    assert rc1 == 0 and res1[0].iterations == res2.iterations
+    assert np.array_equal(x1[0].cpu().numpy(), x2.cpu().numpy())
