@@ -26,6 +26,7 @@ template <typename T> struct DslashArgs {
   double* partial;
   double* scalars;
   int num, den;
+  int remap;  // 0: block = consecutive sites; 4 / 8: block = 2 x 2 (x 2) brick of x-rows (dslash_kernel)
 };
 
 // Launch shape per precision (threads per block, minimum resident blocks per SM = register budget).
@@ -167,7 +168,21 @@ __device__ __forceinline__ void dslash_epilogue(const DslashArgs<T>& a, int idx,
 
 template <typename T, int R, bool DAG, int EPI>
 __global__ void __launch_bounds__(Tune<T, R>::BLOCK, Tune<T, R>::MINB) dslash_kernel(const DslashArgs<T> a) {
-  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (a.remap) {
+    // compact block: the block's x-rows form a 2 x 2 (x 2) brick in (y, z, t) instead of 4 (8) consecutive y-rows,
+    // so more of the +-y, +-z, +-t neighbour rows are shared inside the block (L1); a warp still reads whole x-rows
+    const Lat& L = a.lat;
+    const int xh = threadIdx.x % L.Lxh, r = threadIdx.x / L.Lxh;
+    const int nby = L.Ly >> 1, nbz = L.Lz >> 1;
+    int b = blockIdx.x;
+    const int y = 2 * (b % nby) + (r & 1);
+    b /= nby;
+    const int z = 2 * (b % nbz) + ((r >> 1) & 1);
+    b /= nbz;
+    const int t = a.remap == 8 ? 2 * b + (r >> 2) : b;
+    idx = xh + L.Lxh * (y + L.Ly * (z + L.Lz * t));
+  }
   const bool live = idx < a.lat.Vh;
   if (EPI < 4 && !live) return;
   double local = 0;
@@ -305,9 +320,16 @@ static void launch_tiled(const DslashArgs<T>& a, int epi, cudaStream_t st) {
   }
 }
 
+#ifndef DSLASH_REMAP
+#define DSLASH_REMAP 0
+#endif
 template <typename T, int R, bool DAG>
-static void launch_epi(const DslashArgs<T>& a, int epi, cudaStream_t st) {
+static void launch_epi(DslashArgs<T> a, int epi, cudaStream_t st) {
   const int block = Tune<T, R>::BLOCK;
+  {
+    const int rows = block % a.lat.Lxh == 0 ? block / a.lat.Lxh : 0;
+    a.remap = (DSLASH_REMAP && (rows == 4 || rows == 8) && a.lat.Vh % block == 0) ? rows : 0;
+  }
   const int grid = (a.lat.Vh + block - 1) / block;
   const size_t smem = SStage<T>::ROUNDS > 0 ? (size_t)(8 / SStage<T>::ROUNDS) * 24 * sizeof(T) * block  // spinors
                       : Tune<T, R>::STAGE ? (size_t)8 * R * sizeof(T) * block : 0;                      // eight links per thread
@@ -340,6 +362,7 @@ static void launch_typed(lqcd_ctx* c, void* out, const void* in, const void* gau
   a.scalars = c->d_scalars;
   a.num = f ? f->num : 0;
   a.den = f ? f->den : 0;
+  a.remap = 0;
   a.out = (T*)out;
   a.in = (const T*)in;
   a.gauge = (const T*)gauge;
