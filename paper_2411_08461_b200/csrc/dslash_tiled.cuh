@@ -100,13 +100,31 @@ __device__ __forceinline__ void tile_stage(void* smem, const T* __restrict__ in,
   cp_async_commit();
 }
 
-template <typename T, typename TS, int R, int MU, bool FWD, bool DAG>
+// link through the streaming path (single RHS: read once) or the L1-allocating path (multi-RHS: re-read per column)
+template <typename T, int R, bool L1>
+__device__ __forceinline__ void load_link_sel(const T* __restrict__ block, int Vh, int idx, T* U) {
+  if (!L1) {
+    load_link<T, R>(block, Vh, idx, U);
+  } else {
+    typedef typename GV<T, R>::vec vec;
+    constexpr int N = GV<T, R>::N;
+    const vec* p = reinterpret_cast<const vec*>(block) + idx;
+#pragma unroll
+    for (int v = 0; v < R / N; v++) {
+      vec q = ld_cached(p + (size_t)v * Vh);
+      vec_get(q, U + v * N);
+    }
+    if (R == 12) recon_row2<T>(U);
+  }
+}
+
+template <typename T, typename TS, int R, int MU, bool FWD, bool DAG, bool L1LINKS>
 __device__ __forceinline__ void hop_tiled(T* acc, const void* smem, int slot, const T* __restrict__ links, int Vh,
                                           int lidx, T w) {
   typedef typename V16<T>::vec vec;
   constexpr int S = (FWD != DAG) ? -1 : +1;
   T psi[24], U[18], h[12], chi[12];
-  load_link<T, R>(links, Vh, lidx, U);
+  load_link_sel<T, R, L1LINKS>(links, Vh, lidx, U);
   const vec* sm = reinterpret_cast<const vec*>(smem) + slot;
 #pragma unroll
   for (int v = 0; v < Lay<T>::NSV; v++) {
@@ -119,7 +137,7 @@ __device__ __forceinline__ void hop_tiled(T* acc, const void* smem, int slot, co
 }
 
 // all eight hops of the output site (lxh,ly,lz,lt) of the tile; idx = its global checkerboard index
-template <typename T, typename TS, int R, bool DAG>
+template <typename T, typename TS, int R, bool DAG, bool L1LINKS = false>
 __device__ __forceinline__ void dslash_site_tiled(T* acc, const void* smem, const T* __restrict__ gauge, const Lat& L,
                                                   int idx, int par, int lxh, int ly, int lz, int lt, const Site& s, T ws) {
   const int Vh = L.Vh;
@@ -134,26 +152,26 @@ __device__ __forceinline__ void dslash_site_tiled(T* acc, const void* smem, cons
   int n, slot;
   // x
   slot = row * W + lxh + 1;
-  hop_tiled<T, TS, R, 0, true, DAG>(acc, smem, slot, gauge + (0 * 2 + par) * blk, Vh, idx, ws);
+  hop_tiled<T, TS, R, 0, true, DAG, L1LINKS>(acc, smem, slot, gauge + (0 * 2 + par) * blk, Vh, idx, ws);
   n = neighbour<0, -1>(L, idx, s);
   slot = row * W + lxh;
-  hop_tiled<T, TS, R, 0, false, DAG>(acc, smem, slot, gauge + (0 * 2 + 1 - par) * blk, Vh, n, ws);
+  hop_tiled<T, TS, R, 0, false, DAG, L1LINKS>(acc, smem, slot, gauge + (0 * 2 + 1 - par) * blk, Vh, n, ws);
   // y
   slot = ly + 1 < TS::TY ? (row + 1) * W + jq : TS::OFF_Y + ((1 * TS::TT + lt) * TS::TZ + lz) * TS::TXH + lxh;
-  hop_tiled<T, TS, R, 1, true, DAG>(acc, smem, slot, gauge + (1 * 2 + par) * blk, Vh, idx, ws);
+  hop_tiled<T, TS, R, 1, true, DAG, L1LINKS>(acc, smem, slot, gauge + (1 * 2 + par) * blk, Vh, idx, ws);
   n = neighbour<1, -1>(L, idx, s);
   slot = ly > 0 ? (row - 1) * W + jq : TS::OFF_Y + ((0 * TS::TT + lt) * TS::TZ + lz) * TS::TXH + lxh;
-  hop_tiled<T, TS, R, 1, false, DAG>(acc, smem, slot, gauge + (1 * 2 + 1 - par) * blk, Vh, n, ws);
+  hop_tiled<T, TS, R, 1, false, DAG, L1LINKS>(acc, smem, slot, gauge + (1 * 2 + 1 - par) * blk, Vh, n, ws);
   // z
   slot = lz + 1 < TS::TZ ? (row + TS::TY) * W + jq : TS::OFF_Z + ((1 * TS::TT + lt) * TS::TY + ly) * TS::TXH + lxh;
-  hop_tiled<T, TS, R, 2, true, DAG>(acc, smem, slot, gauge + (2 * 2 + par) * blk, Vh, idx, ws);
+  hop_tiled<T, TS, R, 2, true, DAG, L1LINKS>(acc, smem, slot, gauge + (2 * 2 + par) * blk, Vh, idx, ws);
   n = neighbour<2, -1>(L, idx, s);
   slot = lz > 0 ? (row - TS::TY) * W + jq : TS::OFF_Z + ((0 * TS::TT + lt) * TS::TY + ly) * TS::TXH + lxh;
-  hop_tiled<T, TS, R, 2, false, DAG>(acc, smem, slot, gauge + (2 * 2 + 1 - par) * blk, Vh, n, ws);
+  hop_tiled<T, TS, R, 2, false, DAG, L1LINKS>(acc, smem, slot, gauge + (2 * 2 + 1 - par) * blk, Vh, n, ws);
   // t
   slot = lt + 1 < TS::TT ? (row + TS::TY * TS::TZ) * W + jq : TS::OFF_T + ((1 * TS::TZ + lz) * TS::TY + ly) * TS::TXH + lxh;
-  hop_tiled<T, TS, R, 3, true, DAG>(acc, smem, slot, gauge + (3 * 2 + par) * blk, Vh, idx, sf);
+  hop_tiled<T, TS, R, 3, true, DAG, L1LINKS>(acc, smem, slot, gauge + (3 * 2 + par) * blk, Vh, idx, sf);
   n = neighbour<3, -1>(L, idx, s);
   slot = lt > 0 ? (row - TS::TY * TS::TZ) * W + jq : TS::OFF_T + ((0 * TS::TZ + lz) * TS::TY + ly) * TS::TXH + lxh;
-  hop_tiled<T, TS, R, 3, false, DAG>(acc, smem, slot, gauge + (3 * 2 + 1 - par) * blk, Vh, n, sb);
+  hop_tiled<T, TS, R, 3, false, DAG, L1LINKS>(acc, smem, slot, gauge + (3 * 2 + 1 - par) * blk, Vh, n, sb);
 }

@@ -169,3 +169,29 @@ def test_invert_multi_mixed_fp64_tolerance_config2(solver):
                                   inner_tol=1e-4, maxiter=2000, solver=solver)
     assert rc1 == 0 and res1[0].iterations == res2.iterations
     assert np.array_equal(x1[0].cpu().numpy(), x2.cpu().numpy())
+
+
+@pytest.mark.parametrize("recon", [18, 12])
+def test_tiled_mrhs_kernel_matches_oracle(recon, monkeypatch):
+    """The opt-in tiled multi-RHS kernel (csrc/dslash_mrhs_tiled.cu, LQCD_MRHS_TILED=1 at context creation; fp32):
+    odd and even column counts (the column slots finish at different times), dagger, both parities, M-hat."""
+    monkeypatch.setenv("LQCD_MRHS_TILED", "1")
+    s = Setup((8, 8, 8, 16), 0.5, 2, 0.124, 1.2, 4, recon, -1)
+    for nrhs in (12, 5, 2):
+        psis = [s.spinor("gaussian", 200 + r) for r in range(nrhs)]
+        for dagger in (False, True):
+            wants = [s.orc.dslash(p, dagger=dagger) for p in psis]
+            for par in (0, 1):
+                out = s.ctx.new_spinor(nrhs)
+                s.ctx.dslash_mrhs(out, pack_block(s, psis, 1 - par), s.gauge, par, nrhs, 1.0, dagger)
+                gots = unpack_block(s, out, nrhs, par)
+                for r in range(nrhs):
+                    assert rel_err(gots[r], wants[r][par]) < TOL[4], (nrhs, dagger, par, r)
+        for matpc in (0, 1):
+            out = s.ctx.new_spinor(nrhs)
+            s.ctx.mpc_apply_mrhs(out, pack_block(s, psis, 0), s.gauge, s.A, s.Ai, s.kappa, nrhs, matpc, False)
+            gots = unpack_block(s, out, nrhs, 0)
+            for r in range(nrhs):
+                pe = psis[r].copy()
+                pe[1] = 0
+                assert rel_err(gots[r], s.orc.mpc(pe, matpc, False)[0]) < TOL[4], (nrhs, matpc, r)
