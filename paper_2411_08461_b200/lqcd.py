@@ -129,6 +129,47 @@ def _p(t):
     return ctypes.c_void_p(t.data_ptr()) if t is not None else ctypes.c_void_p(0)
 
 
+def shard_columns(n, rank, world):
+    """Contiguous block [lo, hi) of n independent right-hand sides owned by `rank` of `world` (sizes differ by at
+    most one; the first n % world ranks take the extra column)."""
+    base, extra = divmod(n, world)
+    lo = rank * base + min(rank, extra)
+    return lo, lo + base + (1 if rank < extra else 0)
+
+
+def sharded_solve(sources, solve, group=None):
+    """The n independent columns of `sources` ([n, ...]) sharded over the ranks of a torch.distributed group
+    (the 12 spin-colour columns of a propagator): links and clover are
+    replicated, rank r solves the contiguous block shard_columns(n, r, world) with ONE batched call
+    `solve(block) -> (x, results, status)`, and one all-reduce of a buffer in which every column is owned by
+    exactly one rank (zero elsewhere) brings the solutions to every rank.  No collective on the data path of
+    the solves.  Returns (x [n, ...], iterations per column, worst status over the ranks)."""
+    import torch.distributed as dist
+    on = dist.is_available() and dist.is_initialized()
+    world = dist.get_world_size(group) if on else 1
+    rank = dist.get_rank(group) if on else 0
+    n = sources.shape[0]
+    lo, hi = shard_columns(n, rank, world)
+    x_full = torch.zeros_like(sources)
+    iters = torch.zeros(n, dtype=torch.int64, device=sources.device)
+    rc = 0
+    if hi > lo:
+        x, res, rc = solve(sources[lo:hi])
+        x_full[lo:hi] = x
+        iters[lo:hi] = torch.tensor([r.iterations for r in res], dtype=torch.int64, device=sources.device)
+    worst = torch.tensor([min(rc, 0), max(rc, 0)], dtype=torch.int64, device=sources.device)
+    if world > 1:
+        flat = torch.view_as_real(x_full) if x_full.is_complex() else x_full
+        dist.all_reduce(flat, op=dist.ReduceOp.SUM, group=group)
+        dist.all_reduce(iters, op=dist.ReduceOp.SUM, group=group)
+        neg, pos = worst[:1].clone(), worst[1:].clone()
+        dist.all_reduce(neg, op=dist.ReduceOp.MIN, group=group)
+        dist.all_reduce(pos, op=dist.ReduceOp.MAX, group=group)
+        worst = torch.cat([neg, pos])
+    neg, pos = int(worst[0]), int(worst[1])
+    return x_full, iters.tolist(), (neg if neg < 0 else pos)
+
+
 class Context:
     """One lattice, precision and link reconstruction (init + LatticeInfo)."""
 
@@ -407,6 +448,14 @@ class Context:
         x, res, rc = self.invert_multi(sources, gauge, clover, clover_inv, kappa, tol, maxiter, solver, matpc,
                                        workspace)
         return self.propagator_assemble(x), res, rc
+
+    def propagator_sharded(self, sources, gauge, clover, clover_inv, kappa, tol=1e-10, maxiter=1000, solver="cgne",
+                           matpc=0, group=None):
+        """The paper's `invert` over several GPUs: see sharded_solve.
+        Returns (prop, iterations per column, status)."""
+        solve = lambda blk: self.invert_multi(blk, gauge, clover, clover_inv, kappa, tol, maxiter, solver, matpc)
+        x, iters, rc = sharded_solve(sources, solve, group)
+        return self.propagator_assemble(x), iters, rc
 
     # ---- host-buffer (end-to-end) entry points -----------------------------------------------
     def host_scratch(self, solver="cgne"):

@@ -44,3 +44,56 @@ def test_reference_arm_nonzero_rank_prints_nothing():
     p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2"],
                        env=env, capture_output=True, text=True, timeout=120)
     assert p.returncode == 0 and p.stdout.strip() == ""
+
+
+# ---- column-sharded propagator: host logic on gloo, world size 2 and 3 -------------
+class _Res:
+    def __init__(self, it):
+        self.iterations = it
+
+
+def _shard_worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    from paper_2411_08461_b200 import lqcd
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    g = torch.Generator().manual_seed(5)
+    src = torch.complex(torch.randn(12, 2, 3, 4, generator=g, dtype=torch.float64),
+                        torch.randn(12, 2, 3, 4, generator=g, dtype=torch.float64))
+    lo, hi = lqcd.shard_columns(12, rank, world)
+    calls = []
+
+    def solve(blk):  # stands for the batched GPU solve: x = (2 + i) b, column c "takes" 10 + c iterations
+        calls.append(blk.shape[0])
+        return (2 + 1j) * blk, [_Res(10 + lo + k) for k in range(blk.shape[0])], (1 if rank == world - 1 else 0)
+
+    x, iters, rc = lqcd.sharded_solve(src, solve)
+    ok = bool(torch.equal(x, (2 + 1j) * src)) and iters == [10 + c for c in range(12)] and calls == [hi - lo]
+    dist.barrier()
+    dist.destroy_process_group()
+    json.dump({"ok": ok, "rc": rc, "lo": lo, "hi": hi}, open(out % rank, "w"))
+
+
+def test_sharded_solve_gloo(tmp_path):
+    for world, port in ((2, 29641), (3, 29651)):
+        out = str(tmp_path / ("w%d_" % world + "r%d.json"))
+        mp.spawn(_shard_worker, args=(world, port, out), nprocs=world, join=True)
+        got = [json.load(open(out % r)) for r in range(world)]
+        assert all(d["ok"] for d in got)
+        assert all(d["rc"] == 1 for d in got)                      # NOT_CONVERGED on one rank is everybody's status
+        assert [d["lo"] for d in got] == [r * 12 // world for r in range(world)]
+        assert got[-1]["hi"] == 12
+
+
+def test_shard_columns_covers_every_column_once():
+    sys.path.insert(0, ROOT)
+    from paper_2411_08461_b200 import lqcd
+    for n in (1, 5, 12, 16):
+        for world in (1, 2, 3, 5, 8, 16):
+            blocks = [lqcd.shard_columns(n, r, world) for r in range(world)]
+            cover = [c for lo, hi in blocks for c in range(lo, hi)]
+            assert cover == list(range(n))
+            sizes = [hi - lo for lo, hi in blocks]
+            assert max(sizes) - min(sizes) <= 1 and sizes == sorted(sizes, reverse=True)
+    x, iters, rc = lqcd.sharded_solve(torch.ones(3, 2), lambda b: (b * 3, [_Res(7)] * 3, -7))   # no process group
+    assert torch.equal(x, torch.full((3, 2), 3.0)) and iters == [7, 7, 7] and rc == -7

@@ -195,3 +195,15 @@ def test_tiled_mrhs_kernel_matches_oracle(recon, monkeypatch):
                 pe = psis[r].copy()
                 pe[1] = 0
                 assert rel_err(gots[r], s.orc.mpc(pe, matpc, False)[0]) < TOL[4], (nrhs, matpc, r)
+
+
+def test_propagator_sharded_single_rank_equals_propagator():
+    """Without a process group the column-sharded propagator is the batched one."""
+    s, c = from_cfg(2, 8, 18)
+    dims = c["dims"]
+    cols = np.stack([synth.source(dims, "point", spin=sp, colour=co) for sp in range(4) for co in range(3)])
+    B = s.ctx.to_device(cols)
+    p1, res, rc1 = s.ctx.propagator(B, s.gauge, s.A, s.Ai, s.kappa, tol=1e-10, solver="bicgstab")
+    p2, iters, rc2 = s.ctx.propagator_sharded(B, s.gauge, s.A, s.Ai, s.kappa, tol=1e-10, solver="bicgstab")
+    assert rc1 == 0 and rc2 == 0 and iters == [r.iterations for r in res]
+    assert torch.equal(p1, p2)
