@@ -61,7 +61,10 @@ typedef struct lqcd_result {
  * prec = 4 (fp32) or 8 (fp64): the real type of every native AND public buffer of this context;
  * recon = 18 (full links) or 12 (two rows stored, third recomputed); t_boundary = +1 or -1
  * (antiperiodic in t, applied in-kernel to raw periodic links); device = CUDA
- * ordinal (must be compute capability 10.x). */
+ * ordinal (must be compute capability 10.x).
+ * Measurement switches read from the environment at creation (results are identical, only the kernel differs):
+ * LQCD_DSLASH_TILED=1 runs the shared-memory tiled single-RHS dslash, LQCD_MRHS_TILED=1 the tiled multi-RHS
+ * kernel (fp32), wherever their tile divides the lattice; both are slower than the defaults. */
 int lqcd_create(lqcd_ctx** ctx, const int dims[4], int prec, int recon, int t_boundary, int device);
 int lqcd_destroy(lqcd_ctx* ctx);
 const char* lqcd_strerror(int code);
