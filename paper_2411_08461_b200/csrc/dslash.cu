@@ -11,17 +11,21 @@
 // per-block partials summed in block order by the last block to finish):
 //   4: out = C x + scale * d ; s[out_slot] = |out|^2                          (t = Mhat^dag p, <p, A p>)
 //   5: q   = C x + scale * d ; r -= (s[num]/s[den]) q ; s[out_slot] = |r|^2   (q never stored)
+// Symmetric form (Mhat_s = 1 - k^2 A_ee^-1 D_eo A_oo^-1 D_oe; its adjoint ends in a hop with no clover factor):
+//   6: out = x + scale * d               (Mhat_s^dag y = y - k^2 D^dag_eo A_oo^-1 D^dag_oe A_ee^-1 y)
+//   7: as 6 ; s[out_slot] = |out|^2
+//   8: q   = x + scale * C d ; r -= (s[num]/s[den]) q ; s[out_slot] = |r|^2   (3 fused with the recurrence)
 template <typename T> struct DslashArgs {
   T* out;
   const T* in;
   const T* gauge;
-  const T* cl;  // one-parity clover field of the OUTPUT parity (EPI 1..3)
-  const T* x;   // one-parity spinor of the OUTPUT parity (EPI 2, 3)
+  const T* cl;  // one-parity clover field of the OUTPUT parity (every EPI but 0, 6, 7)
+  const T* x;   // one-parity spinor of the OUTPUT parity (EPI >= 2)
   Lat lat;
   int parity;
   T scale;
   T ws;  // weight of the spatial hops (anisotropy nu/xi_0; 1 = isotropic)
-  // EPI 4, 5 only
+  // EPI 4, 5, 7, 8 only
   T* r;
   double* partial;
   double* scalars;
@@ -122,7 +126,9 @@ __global__ void __launch_bounds__(PSUM_BLOCK) partial_sum_kernel(const double* _
   }
 }
 
-// epilogue of one output site (EPI as listed at the top); `local` collects the fp64 reduction term of EPI 4, 5
+__host__ __device__ constexpr bool epi_reduces(int epi) { return epi == 4 || epi == 5 || epi == 7 || epi == 8; }
+
+// epilogue of one output site (EPI as listed at the top); `local` collects the fp64 reduction term
 template <typename T, int EPI>
 __device__ __forceinline__ void dslash_epilogue(const DslashArgs<T>& a, int idx, const T* acc, double& local) {
   const int Vh = a.lat.Vh;
@@ -140,6 +146,10 @@ __device__ __forceinline__ void dslash_epilogue(const DslashArgs<T>& a, int idx,
     clover_mul<T>(a.cl, Vh, idx, xv, res);
 #pragma unroll
     for (int e = 0; e < 24; e++) res[e] += a.scale * acc[e];
+  } else if (EPI == 6 || EPI == 7) {
+    load_spinor<T>(a.x, Vh, idx, res);
+#pragma unroll
+    for (int e = 0; e < 24; e++) res[e] += a.scale * acc[e];
   } else {
     T xv[24];
     load_spinor<T>(a.x, Vh, idx, xv);
@@ -147,7 +157,7 @@ __device__ __forceinline__ void dslash_epilogue(const DslashArgs<T>& a, int idx,
 #pragma unroll
     for (int e = 0; e < 24; e++) res[e] = xv[e] + a.scale * res[e];
   }
-  if (EPI == 5) {
+  if (EPI == 5 || EPI == 8) {
     const T alpha = (T)(a.scalars[a.num] / a.scalars[a.den]);
     T rv[24];
     load_spinor<T>(a.r, Vh, idx, rv);
@@ -158,7 +168,7 @@ __device__ __forceinline__ void dslash_epilogue(const DslashArgs<T>& a, int idx,
     }
     store_spinor<T>(a.r, Vh, idx, rv);
   } else {
-    if (EPI == 4) {
+    if (EPI == 4 || EPI == 7) {
 #pragma unroll
       for (int e = 0; e < 24; e++) local += (double)res[e] * res[e];
     }
@@ -184,7 +194,7 @@ __global__ void __launch_bounds__(Tune<T, R>::BLOCK, Tune<T, R>::MINB) dslash_ke
     idx = xh + L.Lxh * (y + L.Ly * (z + L.Lz * t));
   }
   const bool live = idx < a.lat.Vh;
-  if (EPI < 4 && !live) return;
+  if (!epi_reduces(EPI) && !live) return;
   double local = 0;
   if (live) {
     T acc[24];
@@ -200,7 +210,7 @@ __global__ void __launch_bounds__(Tune<T, R>::BLOCK, Tune<T, R>::MINB) dslash_ke
     }
     dslash_epilogue<T, EPI>(a, idx, acc, local);
   }
-  if (EPI >= 4) dslash_reduce<Tune<T, R>::BLOCK>(local, a.partial);
+  if (epi_reduces(EPI)) dslash_reduce<Tune<T, R>::BLOCK>(local, a.partial);
 }
 
 template <typename T>
@@ -278,7 +288,7 @@ __global__ void __launch_bounds__(TileOf<T>::NOUT, TileOf<T>::MINB) dslash_tiled
   dslash_site_tiled<T, TS, R, DAG>(acc, dslash_smem, a.gauge, L, idx, a.parity, lxh, ly, lz, lt, s, a.ws);
   double local = 0;
   dslash_epilogue<T, EPI>(a, idx, acc, local);
-  if (EPI >= 4) dslash_reduce<TS::NOUT>(local, a.partial);
+  if (epi_reduces(EPI)) dslash_reduce<TS::NOUT>(local, a.partial);
 }
 
 template <typename T> static bool tile_fits(const Lat& L) {
@@ -308,6 +318,9 @@ static void launch_tiled(const DslashArgs<T>& a, int epi, cudaStream_t st) {
     cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 7>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     configured = true;
   }
   switch (epi) {
@@ -316,7 +329,10 @@ static void launch_tiled(const DslashArgs<T>& a, int epi, cudaStream_t st) {
     case 2: dslash_tiled_kernel<T, R, DAG, 2><<<grid, TS::NOUT, smem, st>>>(a); break;
     case 3: dslash_tiled_kernel<T, R, DAG, 3><<<grid, TS::NOUT, smem, st>>>(a); break;
     case 4: dslash_tiled_kernel<T, R, DAG, 4><<<grid, TS::NOUT, smem, st>>>(a); break;
-    default: dslash_tiled_kernel<T, R, DAG, 5><<<grid, TS::NOUT, smem, st>>>(a); break;
+    case 5: dslash_tiled_kernel<T, R, DAG, 5><<<grid, TS::NOUT, smem, st>>>(a); break;
+    case 6: dslash_tiled_kernel<T, R, DAG, 6><<<grid, TS::NOUT, smem, st>>>(a); break;
+    case 7: dslash_tiled_kernel<T, R, DAG, 7><<<grid, TS::NOUT, smem, st>>>(a); break;
+    default: dslash_tiled_kernel<T, R, DAG, 8><<<grid, TS::NOUT, smem, st>>>(a); break;
   }
 }
 
@@ -341,6 +357,9 @@ static void launch_epi(DslashArgs<T> a, int epi, cudaStream_t st) {
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 7>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   }
   configured = true;
   switch (epi) {
@@ -349,7 +368,10 @@ static void launch_epi(DslashArgs<T> a, int epi, cudaStream_t st) {
     case 2: dslash_kernel<T, R, DAG, 2><<<grid, block, smem, st>>>(a); break;
     case 3: dslash_kernel<T, R, DAG, 3><<<grid, block, smem, st>>>(a); break;
     case 4: dslash_kernel<T, R, DAG, 4><<<grid, block, smem, st>>>(a); break;
-    default: dslash_kernel<T, R, DAG, 5><<<grid, block, smem, st>>>(a); break;
+    case 5: dslash_kernel<T, R, DAG, 5><<<grid, block, smem, st>>>(a); break;
+    case 6: dslash_kernel<T, R, DAG, 6><<<grid, block, smem, st>>>(a); break;
+    case 7: dslash_kernel<T, R, DAG, 7><<<grid, block, smem, st>>>(a); break;
+    default: dslash_kernel<T, R, DAG, 8><<<grid, block, smem, st>>>(a); break;
   }
 }
 
@@ -399,7 +421,7 @@ int lqcd_dslash_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge
   if (nrhs > 1) return lqcd_dslash_mrhs_launch(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st);
   // algorithmic bytes: every link once, input spinor once, output once (+ clover, + x)
   const double bytes = (double)c->lat.Vh * c->prec *
-                       (8.0 * c->recon + 48.0 + (epi >= 1 ? 72.0 : 0.0) + (epi >= 2 ? 24.0 : 0.0));
+                       (8.0 * c->recon + 48.0 + (epi >= 1 && epi != 6 ? 72.0 : 0.0) + (epi >= 2 ? 24.0 : 0.0));
   c->alg_bytes += bytes;
   const bool rec = c->prof_on && c->prof_n < c->prof_cap;
   if (rec) cudaEventRecord(c->prof_ev[2 * c->prof_n], st);
@@ -421,8 +443,9 @@ bool lqcd_dslash_fuse_ok(const lqcd_ctx* c) {
 
 int lqcd_dslash_fused_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
                              int parity, double scale, int dagger, int epi, const DslashFuse* f, cudaStream_t st) {
-  // epi 4: as epi 2.  epi 5: no output store, r read and written instead
-  const double bytes = (double)c->lat.Vh * c->prec * (8.0 * c->recon + 48.0 + 72.0 + 24.0 + (epi == 5 ? 24.0 : 0.0));
+  // epi 4: as epi 2; epi 7: as epi 6 (no clover).  epi 5, 8: no output store, r read and written instead
+  const double bytes = (double)c->lat.Vh * c->prec *
+                       (8.0 * c->recon + 48.0 + (epi == 7 ? 0.0 : 72.0) + 24.0 + (epi == 5 || epi == 8 ? 24.0 : 0.0));
   c->alg_bytes += bytes;
   const bool rec = c->prof_on && c->prof_n < c->prof_cap;
   if (rec) cudaEventRecord(c->prof_ev[2 * c->prof_n], st);

@@ -54,7 +54,8 @@ static int mpc_apply(lqcd_ctx* c, void* out, const void* in, const void* gauge, 
   }
   if ((rc = lqcd_clover_apply_launch(c, out, in, Ai_e, nrhs, st))) return rc;
   if ((rc = lqcd_dslash_launch(c, tmp, out, gauge, Ai_o, nullptr, 1, 1.0, 1, 1, nrhs, st))) return rc;
-  // out = in + k2 * D^dag_eo tmp : plain dslash into `out` followed by an xpay
+  if (nrhs == 1) return lqcd_dslash_launch(c, out, tmp, gauge, nullptr, in, 0, k2, 1, 6, 1, st);  // out = in + k2 D^dag_eo tmp
+  // multi-RHS kernels have no epilogue 6: plain dslash into `out` followed by an xpay
   if ((rc = lqcd_dslash_launch(c, out, tmp, gauge, nullptr, nullptr, 0, k2, 1, 0, nrhs, st))) return rc;
   void* v[2] = {(void*)in, out};
   return BLAS_CALL(c, OpXpay, op.a = 1.0, v, nullptr, nrhs, 0, st);  // out = in + 1*out
@@ -171,12 +172,27 @@ static int solve_cg(lqcd_ctx* c, const Work& w, const void* gauge, const void* A
     cols.rr[j] = hs(c, j, S_RES);
     if (!(cols.rr[j] > cols.stop2[j])) freeze(c, cols, j, st);
   }
-  const bool fused = n == 1 && matpc == LQCD_MATPC_ASYMMETRIC && lqcd_dslash_fuse_ok(c);
+  const bool fused = n == 1 && lqcd_dslash_fuse_ok(c);
   int it = 0;
   while (it < maxiter && cols.nactive() > 0) {
     const int cur = (it & 1) ? S_RR1 : S_RR0, nxt = (it & 1) ? S_RR0 : S_RR1;
     int outs[4] = {S_TT, 0, 0, 0};
-    if (!normal_residual && fused) {
+    if (!normal_residual && fused && matpc == LQCD_MATPC_SYMMETRIC) {
+      // symmetric form, recurrences fused into the epilogues (dslash.cu EPI 7, 8):
+      //   pa = A_ee^-1 p ; tmp = A_oo^-1 D^dag_oe pa ; t = p - k^2 D^dag_eo tmp and |t|^2 in one launch ;
+      //   tmp = A_oo^-1 D_oe t ; q = t - k^2 A_ee^-1 D_eo tmp is never stored: r -= alpha q, |r|^2 in its launch
+      const size_t half = lqcd_clover_bytes(c) / 2;
+      const double k2 = -kappa * kappa;
+      char* pa = q;  // q is not stored in this path
+      DslashFuse f7 = {nullptr, S_TT, 0, 0}, f8 = {r, nxt, cur, S_TT};
+      if ((rc = lqcd_clover_apply_launch(c, pa, p, Ai, 1, st))) return rc;
+      if ((rc = lqcd_dslash_launch(c, tmp, pa, gauge, off(Ai, half), nullptr, 1, 1.0, 1, 1, 1, st))) return rc;
+      if ((rc = lqcd_dslash_fused_launch(c, t, tmp, gauge, nullptr, p, 0, k2, 1, 7, &f7, st))) return rc;
+      if ((rc = lqcd_dslash_launch(c, tmp, t, gauge, off(Ai, half), nullptr, 1, 1.0, 0, 1, 1, st))) return rc;
+      if ((rc = lqcd_dslash_fused_launch(c, nullptr, tmp, gauge, Ai, t, 0, k2, 0, 8, &f8, st))) return rc;
+      void* u[2] = {x, t};
+      if ((rc = BLAS_CALL(c, OpAxpyRatio, (op.num = cur, op.den = S_TT), u, nullptr, n, 0, st))) return rc;  // x += a t
+    } else if (!normal_residual && fused) {
       // CGNE with the recurrences fused into the dslash epilogues (dslash.cu EPI 4, 5):
       //   t = Mhat^dag p and |t|^2 in one launch; q = Mhat t is never stored: r -= alpha q, |r|^2 in its launch
       const size_t half = lqcd_clover_bytes(c) / 2;
