@@ -44,7 +44,7 @@ enum {
   LQCD_ERR_BREAKDOWN = -7
 };
 enum { LQCD_SOLVER_CGNE = 0, LQCD_SOLVER_CGNR = 1, LQCD_SOLVER_BICGSTAB = 2 };
-enum { LQCD_MATPC_ASYMMETRIC = 0, LQCD_MATPC_SYMMETRIC = 1 };
+enum { LQCD_MATPC_ASYMMETRIC = 0, LQCD_MATPC_SYMMETRIC = 1, LQCD_MATPC_SYMMETRIC_RIGHT = 2 };
 #define LQCD_MAX_RHS 16 /* right-hand sides per multi-RHS call (a propagator has 12 columns) */
 
 typedef struct lqcd_result {
@@ -129,8 +129,11 @@ int lqcd_dslash(lqcd_ctx* ctx, void* out, const void* in, const void* gauge, int
 
 /* Even-even Schur complement on one-parity native spinors:
  *   matpc 0: out = A_ee in - kappa^2 D_eo A_oo^-1 D_oe in
- *   matpc 1: out = in - kappa^2 A_ee^-1 D_eo A_oo^-1 D_oe in      (dagger: the adjoint of either)
- * tmp_o: one-parity scratch spinor. */
+ *   matpc 1: out = in - kappa^2 A_ee^-1 D_eo A_oo^-1 D_oe in      (symmetric, preconditioned from the left)
+ *   matpc 2: out = in - kappa^2 D_eo A_oo^-1 D_oe A_ee^-1 in      (symmetric, preconditioned from the right:
+ *            = (matpc 0) A_ee^-1; in a solve the Krylov unknown is y = A_ee x_e and the recurrence residual is
+ *            that of matpc 0, i.e. the even half of the true residual, with the conditioning of matpc 1)
+ * dagger: the adjoint of any of them.  tmp_o: one-parity scratch spinor. */
 int lqcd_mpc_apply(lqcd_ctx* ctx, void* out_e, const void* in_e, const void* gauge, const void* clover,
                    const void* clover_inv, double kappa, int matpc, int dagger, void* tmp_o, void* stream);
 

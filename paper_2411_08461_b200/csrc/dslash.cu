@@ -15,6 +15,9 @@
 //   6: out = x + scale * d               (Mhat_s^dag y = y - k^2 D^dag_eo A_oo^-1 D^dag_oe A_ee^-1 y)
 //   7: as 6 ; s[out_slot] = |out|^2
 //   8: q   = x + scale * C d ; r -= (s[num]/s[den]) q ; s[out_slot] = |r|^2   (3 fused with the recurrence)
+// Right-preconditioned symmetric form (Mhat_r = 1 - k^2 D_eo A_oo^-1 D_oe A_ee^-1, unknown y = A_ee x_e):
+//   9: out = x + scale * C d ; out2 = C out ; s[out_slot] = |out|^2           (t = Mhat_r^dag p and A_ee^-1 t)
+//  10: q   = x + scale * d   ; r -= (s[num]/s[den]) q ; s[out_slot] = |r|^2   (q = Mhat_r t never stored)
 template <typename T> struct DslashArgs {
   T* out;
   const T* in;
@@ -25,8 +28,9 @@ template <typename T> struct DslashArgs {
   int parity;
   T scale;
   T ws;  // weight of the spatial hops (anisotropy nu/xi_0; 1 = isotropic)
-  // EPI 4, 5, 7, 8 only
+  // EPI 4, 5, 7, 8, 9, 10 only
   T* r;
+  T* out2;  // EPI 9: second output, C * out
   double* partial;
   double* scalars;
   int num, den;
@@ -126,7 +130,7 @@ __global__ void __launch_bounds__(PSUM_BLOCK) partial_sum_kernel(const double* _
   }
 }
 
-__host__ __device__ constexpr bool epi_reduces(int epi) { return epi == 4 || epi == 5 || epi == 7 || epi == 8; }
+__host__ __device__ constexpr bool epi_reduces(int epi) { return epi == 4 || epi == 5 || epi >= 7; }
 
 // epilogue of one output site (EPI as listed at the top); `local` collects the fp64 reduction term
 template <typename T, int EPI>
@@ -146,10 +150,15 @@ __device__ __forceinline__ void dslash_epilogue(const DslashArgs<T>& a, int idx,
     clover_mul<T>(a.cl, Vh, idx, xv, res);
 #pragma unroll
     for (int e = 0; e < 24; e++) res[e] += a.scale * acc[e];
-  } else if (EPI == 6 || EPI == 7) {
+  } else if (EPI == 6 || EPI == 7 || EPI == 10) {
     load_spinor<T>(a.x, Vh, idx, res);
 #pragma unroll
     for (int e = 0; e < 24; e++) res[e] += a.scale * acc[e];
+  } else if (EPI == 9) {
+    T xv[24], res2[24];
+    load_spinor<T>(a.x, Vh, idx, xv);
+    clover_mul_twice<T>(a.cl, Vh, idx, acc, xv, a.scale, res, res2);
+    store_spinor<T>(a.out2, Vh, idx, res2);
   } else {
     T xv[24];
     load_spinor<T>(a.x, Vh, idx, xv);
@@ -157,7 +166,7 @@ __device__ __forceinline__ void dslash_epilogue(const DslashArgs<T>& a, int idx,
 #pragma unroll
     for (int e = 0; e < 24; e++) res[e] = xv[e] + a.scale * res[e];
   }
-  if (EPI == 5 || EPI == 8) {
+  if (EPI == 5 || EPI == 8 || EPI == 10) {
     const T alpha = (T)(a.scalars[a.num] / a.scalars[a.den]);
     T rv[24];
     load_spinor<T>(a.r, Vh, idx, rv);
@@ -168,7 +177,7 @@ __device__ __forceinline__ void dslash_epilogue(const DslashArgs<T>& a, int idx,
     }
     store_spinor<T>(a.r, Vh, idx, rv);
   } else {
-    if (EPI == 4 || EPI == 7) {
+    if (EPI == 4 || EPI == 7 || EPI == 9) {
 #pragma unroll
       for (int e = 0; e < 24; e++) local += (double)res[e] * res[e];
     }
@@ -321,6 +330,8 @@ static void launch_tiled(const DslashArgs<T>& a, int epi, cudaStream_t st) {
     cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 7>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 9>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 10>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     configured = true;
   }
   switch (epi) {
@@ -332,7 +343,9 @@ static void launch_tiled(const DslashArgs<T>& a, int epi, cudaStream_t st) {
     case 5: dslash_tiled_kernel<T, R, DAG, 5><<<grid, TS::NOUT, smem, st>>>(a); break;
     case 6: dslash_tiled_kernel<T, R, DAG, 6><<<grid, TS::NOUT, smem, st>>>(a); break;
     case 7: dslash_tiled_kernel<T, R, DAG, 7><<<grid, TS::NOUT, smem, st>>>(a); break;
-    default: dslash_tiled_kernel<T, R, DAG, 8><<<grid, TS::NOUT, smem, st>>>(a); break;
+    case 8: dslash_tiled_kernel<T, R, DAG, 8><<<grid, TS::NOUT, smem, st>>>(a); break;
+    case 9: dslash_tiled_kernel<T, R, DAG, 9><<<grid, TS::NOUT, smem, st>>>(a); break;
+    default: dslash_tiled_kernel<T, R, DAG, 10><<<grid, TS::NOUT, smem, st>>>(a); break;
   }
 }
 
@@ -360,6 +373,8 @@ static void launch_epi(DslashArgs<T> a, int epi, cudaStream_t st) {
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 7>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 9>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 10>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   }
   configured = true;
   switch (epi) {
@@ -371,7 +386,9 @@ static void launch_epi(DslashArgs<T> a, int epi, cudaStream_t st) {
     case 5: dslash_kernel<T, R, DAG, 5><<<grid, block, smem, st>>>(a); break;
     case 6: dslash_kernel<T, R, DAG, 6><<<grid, block, smem, st>>>(a); break;
     case 7: dslash_kernel<T, R, DAG, 7><<<grid, block, smem, st>>>(a); break;
-    default: dslash_kernel<T, R, DAG, 8><<<grid, block, smem, st>>>(a); break;
+    case 8: dslash_kernel<T, R, DAG, 8><<<grid, block, smem, st>>>(a); break;
+    case 9: dslash_kernel<T, R, DAG, 9><<<grid, block, smem, st>>>(a); break;
+    default: dslash_kernel<T, R, DAG, 10><<<grid, block, smem, st>>>(a); break;
   }
 }
 
@@ -380,6 +397,7 @@ static void launch_typed(lqcd_ctx* c, void* out, const void* in, const void* gau
                          int parity, double scale, int dagger, int epi, const DslashFuse* f, cudaStream_t st) {
   DslashArgs<T> a;
   a.r = f ? (T*)f->r : nullptr;
+  a.out2 = f ? (T*)f->out2 : nullptr;
   a.partial = c->d_partial;
   a.scalars = c->d_scalars;
   a.num = f ? f->num : 0;
@@ -443,9 +461,11 @@ bool lqcd_dslash_fuse_ok(const lqcd_ctx* c) {
 
 int lqcd_dslash_fused_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
                              int parity, double scale, int dagger, int epi, const DslashFuse* f, cudaStream_t st) {
-  // epi 4: as epi 2; epi 7: as epi 6 (no clover).  epi 5, 8: no output store, r read and written instead
+  // epi 4: as epi 2; epi 7: as epi 6 (no clover); epi 9: as epi 3 + a second output.  epi 5, 8, 10: no output
+  // store, r read and written instead
   const double bytes = (double)c->lat.Vh * c->prec *
-                       (8.0 * c->recon + 48.0 + (epi == 7 ? 0.0 : 72.0) + 24.0 + (epi == 5 || epi == 8 ? 24.0 : 0.0));
+                       (8.0 * c->recon + 48.0 + (epi == 7 || epi == 10 ? 0.0 : 72.0) + 24.0 +
+                        (epi == 5 || epi == 8 || epi == 9 || epi == 10 ? 24.0 : 0.0));
   c->alg_bytes += bytes;
   const bool rec = c->prof_on && c->prof_n < c->prof_cap;
   if (rec) cudaEventRecord(c->prof_ev[2 * c->prof_n], st);

@@ -457,3 +457,60 @@ __device__ __forceinline__ void clover_mul(const T* __restrict__ cl, int Vh, int
     }
   }
 }
+
+// res = x + scale * C v  and  res2 = C res  with ONE pass over the clover field: each 6x6 chiral block is loaded
+// once and used for both products (dslash.cu epilogue 9).  v, x, res, res2 are 24-real spinors; no aliasing.
+template <typename T>
+__device__ __forceinline__ void clover_mul_twice(const T* __restrict__ cl, int Vh, int idx, const T* v, const T* x, T scale,
+                                                 T* res, T* res2) {
+  typedef typename V16<T>::vec vec;
+  constexpr int N = V16<T>::N;
+  const vec* p = reinterpret_cast<const vec*>(cl) + idx;
+#pragma unroll
+  for (int k = 0; k < 2; k++) {
+    T a[36];
+#pragma unroll
+    for (int q = 0; q < 36 / N; q++) {
+      vec w = ld_stream(p + (size_t)(k * (36 / N) + q) * Vh);
+      vec_get(w, a + q * N);
+    }
+#pragma unroll
+    for (int pass = 0; pass < 2; pass++) {
+      const T* in = pass == 0 ? v + 12 * k : res + 12 * k;
+      T y[12];
+      if constexpr (UsePacked<T>::value) {
+        clover_block_packed(a, in, y);
+      } else {
+#pragma unroll
+        for (int i = 0; i < 6; i++) {
+          T re = a[i] * in[2 * i], im = a[i] * in[2 * i + 1];
+#pragma unroll
+          for (int j = 0; j < 6; j++) {
+            if (j < i) {
+              const int o = 6 + 2 * (i * (i - 1) / 2 + j);
+              re += a[o] * in[2 * j];
+              re -= a[o + 1] * in[2 * j + 1];
+              im += a[o] * in[2 * j + 1];
+              im += a[o + 1] * in[2 * j];
+            } else if (j > i) {
+              const int o = 6 + 2 * (j * (j - 1) / 2 + i);
+              re += a[o] * in[2 * j];
+              re += a[o + 1] * in[2 * j + 1];
+              im += a[o] * in[2 * j + 1];
+              im -= a[o + 1] * in[2 * j];
+            }
+          }
+          y[2 * i] = re;
+          y[2 * i + 1] = im;
+        }
+      }
+      if (pass == 0) {
+#pragma unroll
+        for (int e = 0; e < 12; e++) res[12 * k + e] = x[12 * k + e] + scale * y[e];
+      } else {
+#pragma unroll
+        for (int e = 0; e < 12; e++) res2[12 * k + e] = y[e];
+      }
+    }
+  }
+}

@@ -232,8 +232,9 @@ int lqcd_dslash_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge
 // CG recurrences fused into the dslash epilogue (dslash.cu, epilogues 4 and 5; single right-hand side)
 struct DslashFuse {
   void* r;       // epi 5: residual updated in place, r -= (s[num]/s[den]) q
-  int out_slot;  // reduction result: |out|^2 (epi 4) or |r|^2 (epi 5) -> d_scalars[out_slot]
+  int out_slot;  // reduction result: |out|^2 (epi 4, 7, 9) or |r|^2 (epi 5, 8, 10) -> d_scalars[out_slot]
   int num, den;
+  void* out2;    // epi 9: second output, C * out
 };
 bool lqcd_dslash_fuse_ok(const lqcd_ctx* c);
 int lqcd_dslash_fused_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,

@@ -48,6 +48,20 @@ static int mpc_apply(lqcd_ctx* c, void* out, const void* in, const void* gauge, 
     if ((rc = lqcd_dslash_launch(c, tmp, in, gauge, Ai_o, nullptr, 1, 1.0, dagger, 1, nrhs, st))) return rc;
     return lqcd_dslash_launch(c, out, tmp, gauge, A_e, in, 0, k2, dagger, 2, nrhs, st);
   }
+  if (matpc == LQCD_MATPC_SYMMETRIC_RIGHT) {
+    //   right:        out(scratch) = A_ee^-1 in ; tmp = A_oo^-1 D_oe out ; out = in - k^2 D_eo tmp
+    //   right dagger: tmp = A_oo^-1 D^dag_oe in ; out = in - k^2 A_ee^-1 D^dag_eo tmp
+    if (dagger) {
+      if ((rc = lqcd_dslash_launch(c, tmp, in, gauge, Ai_o, nullptr, 1, 1.0, 1, 1, nrhs, st))) return rc;
+      return lqcd_dslash_launch(c, out, tmp, gauge, Ai_e, in, 0, k2, 1, 3, nrhs, st);
+    }
+    if ((rc = lqcd_clover_apply_launch(c, out, in, Ai_e, nrhs, st))) return rc;
+    if ((rc = lqcd_dslash_launch(c, tmp, out, gauge, Ai_o, nullptr, 1, 1.0, 0, 1, nrhs, st))) return rc;
+    if (nrhs == 1) return lqcd_dslash_launch(c, out, tmp, gauge, nullptr, in, 0, k2, 0, 6, 1, st);
+    if ((rc = lqcd_dslash_launch(c, out, tmp, gauge, nullptr, nullptr, 0, k2, 0, 0, nrhs, st))) return rc;
+    void* v[2] = {(void*)in, out};
+    return BLAS_CALL(c, OpXpay, op.a = 1.0, v, nullptr, nrhs, 0, st);  // out = in + 1*out
+  }
   if (!dagger) {
     if ((rc = lqcd_dslash_launch(c, tmp, in, gauge, Ai_o, nullptr, 1, 1.0, 0, 1, nrhs, st))) return rc;
     return lqcd_dslash_launch(c, out, tmp, gauge, Ai_e, in, 0, k2, 0, 3, nrhs, st);
@@ -83,7 +97,7 @@ extern "C" {
 
 int lqcd_mpc_apply_mrhs(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* clover,
                         const void* clover_inv, double kappa, int matpc, int dagger, void* tmp, int nrhs, void* stream) {
-  if (!c || !out || !in || !gauge || !clover || !clover_inv || !tmp || (matpc != 0 && matpc != 1) || nrhs < 1 ||
+  if (!c || !out || !in || !gauge || !clover || !clover_inv || !tmp || matpc < 0 || matpc > 2 || nrhs < 1 ||
       nrhs > LQCD_MAX_RHS)
     return LQCD_ERR_INVALID_ARG;
   if (out == in || tmp == in || tmp == out) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "mpc_apply: aliasing");
@@ -177,14 +191,28 @@ static int solve_cg(lqcd_ctx* c, const Work& w, const void* gauge, const void* A
   while (it < maxiter && cols.nactive() > 0) {
     const int cur = (it & 1) ? S_RR1 : S_RR0, nxt = (it & 1) ? S_RR0 : S_RR1;
     int outs[4] = {S_TT, 0, 0, 0};
-    if (!normal_residual && fused && matpc == LQCD_MATPC_SYMMETRIC) {
+    if (!normal_residual && fused && matpc == LQCD_MATPC_SYMMETRIC_RIGHT) {
+      // right-preconditioned symmetric form, recurrences fused into the epilogues (dslash.cu EPI 9, 10):
+      //   tmp = A_oo^-1 D^dag_oe p ; t = p - k^2 A_ee^-1 D^dag_eo tmp, ta = A_ee^-1 t and |t|^2 in one launch ;
+      //   tmp = A_oo^-1 D_oe ta ; q = t - k^2 D_eo tmp is never stored: r -= alpha q, |r|^2 in its launch
+      const size_t half = lqcd_clover_bytes(c) / 2;
+      const double k2 = -kappa * kappa;
+      char* ta = q;  // q is not stored in this path
+      DslashFuse f9 = {nullptr, S_TT, 0, 0, ta}, f10 = {r, nxt, cur, S_TT, nullptr};
+      if ((rc = lqcd_dslash_launch(c, tmp, p, gauge, off(Ai, half), nullptr, 1, 1.0, 1, 1, 1, st))) return rc;
+      if ((rc = lqcd_dslash_fused_launch(c, t, tmp, gauge, Ai, p, 0, k2, 1, 9, &f9, st))) return rc;
+      if ((rc = lqcd_dslash_launch(c, tmp, ta, gauge, off(Ai, half), nullptr, 1, 1.0, 0, 1, 1, st))) return rc;
+      if ((rc = lqcd_dslash_fused_launch(c, nullptr, tmp, gauge, nullptr, t, 0, k2, 0, 10, &f10, st))) return rc;
+      void* u[2] = {x, t};
+      if ((rc = BLAS_CALL(c, OpAxpyRatio, (op.num = cur, op.den = S_TT), u, nullptr, n, 0, st))) return rc;  // y += a t
+    } else if (!normal_residual && fused && matpc == LQCD_MATPC_SYMMETRIC) {
       // symmetric form, recurrences fused into the epilogues (dslash.cu EPI 7, 8):
       //   pa = A_ee^-1 p ; tmp = A_oo^-1 D^dag_oe pa ; t = p - k^2 D^dag_eo tmp and |t|^2 in one launch ;
       //   tmp = A_oo^-1 D_oe t ; q = t - k^2 A_ee^-1 D_eo tmp is never stored: r -= alpha q, |r|^2 in its launch
       const size_t half = lqcd_clover_bytes(c) / 2;
       const double k2 = -kappa * kappa;
       char* pa = q;  // q is not stored in this path
-      DslashFuse f7 = {nullptr, S_TT, 0, 0}, f8 = {r, nxt, cur, S_TT};
+      DslashFuse f7 = {nullptr, S_TT, 0, 0, nullptr}, f8 = {r, nxt, cur, S_TT, nullptr};
       if ((rc = lqcd_clover_apply_launch(c, pa, p, Ai, 1, st))) return rc;
       if ((rc = lqcd_dslash_launch(c, tmp, pa, gauge, off(Ai, half), nullptr, 1, 1.0, 1, 1, 1, st))) return rc;
       if ((rc = lqcd_dslash_fused_launch(c, t, tmp, gauge, nullptr, p, 0, k2, 1, 7, &f7, st))) return rc;
@@ -197,7 +225,7 @@ static int solve_cg(lqcd_ctx* c, const Work& w, const void* gauge, const void* A
       //   t = Mhat^dag p and |t|^2 in one launch; q = Mhat t is never stored: r -= alpha q, |r|^2 in its launch
       const size_t half = lqcd_clover_bytes(c) / 2;
       const double k2 = -kappa * kappa;
-      DslashFuse f4 = {nullptr, S_TT, 0, 0}, f5 = {r, nxt, cur, S_TT};
+      DslashFuse f4 = {nullptr, S_TT, 0, 0, nullptr}, f5 = {r, nxt, cur, S_TT, nullptr};
       if ((rc = lqcd_dslash_launch(c, tmp, p, gauge, off(Ai, half), nullptr, 1, 1.0, 1, 1, 1, st))) return rc;
       if ((rc = lqcd_dslash_fused_launch(c, t, tmp, gauge, A, p, 0, k2, 1, 4, &f4, st))) return rc;
       if ((rc = lqcd_dslash_launch(c, tmp, t, gauge, off(Ai, half), nullptr, 1, 1.0, 0, 1, 1, st))) return rc;
@@ -535,6 +563,8 @@ static int invert_native(lqcd_ctx* c, Work& w, const void* gauge, const void* A,
     c->acct_rhs = 0;
     if (rc) return rc;
     set_slot_all(c, n, S_DONE, false, st);  // the closing steps below update every column
+    if (matpc == LQCD_MATPC_SYMMETRIC_RIGHT)     // the Krylov unknown was y = A_ee x_e
+      if ((rc = lqcd_clover_apply_launch(c, x_e, x_e, Ai_e, n, st))) return rc;
     // a10: x_o = A_oo^-1 (b_o + kappa D_oe x_e)
     if ((rc = lqcd_dslash_launch(c, w.v[5], x_e, gauge, nullptr, nullptr, 1, kappa, 0, 0, n, st))) return rc;
     {
@@ -578,7 +608,7 @@ static int invert_common(lqcd_ctx* c, void* x_public, const void* b_public, cons
                          int matpc, int nrhs, void* workspace, size_t workspace_bytes, lqcd_result* res, cudaStream_t st,
                          Mixed* mixed = nullptr) {
   if (!c || !x_public || !b_public || !gauge || !workspace || !res) return LQCD_ERR_INVALID_ARG;
-  if (solver < 0 || solver > 2 || (matpc != 0 && matpc != 1) || maxiter < 0 || !(tol >= 0) || (clover && !clover_inv) ||
+  if (solver < 0 || solver > 2 || matpc < 0 || matpc > 2 || maxiter < 0 || !(tol >= 0) || (clover && !clover_inv) ||
       nrhs < 1 || nrhs > LQCD_MAX_RHS)
     return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "invert: bad solver/matpc/maxiter/tol/nrhs");
   if (workspace_bytes < lqcd_invert_multi_workspace_bytes(c, solver, nrhs))

@@ -97,10 +97,10 @@ def test_config4_operators_every_site_fp64(recon):
     check_operators(Dev(4, 8, recon))
 
 
-@pytest.mark.parametrize("matpc", [0, 1])
+@pytest.mark.parametrize("matpc", [0, 1, 2])
 def test_config4_cgne_fp64_true_residual(matpc):
     """BASELINE config 4: mixed-precision-free fp64 CG (CGNE) to 1e-10, with the asymmetric and the symmetric
-    Schur complement (bench.py times the symmetric one: fused epilogues 7 and 8); the oracle's own operator
+    Schur complements (left: fused epilogues 7 and 8; right: 9 and 10, the one bench.py times); the oracle's own operator
     evaluates the true residual of the GPU's solution, and the two solutions are the same x."""
     d = Dev(4, 8, 18)
     x, res = d.ctx.invert(d.ctx.to_device(d.b), d.gauge, d.A, d.Ai, d.c["kappa"], tol=1e-10, solver="cgne", matpc=matpc)
@@ -108,7 +108,7 @@ def test_config4_cgne_fp64_true_residual(matpc):
     xg = x.cpu().numpy()
     true = d.orc.true_residual(d.b, xg)
     assert true < 1e-10 and abs(true - res.true_resid) < 1e-11, (true, res.as_dict())
-    if matpc == 1:
+    if matpc >= 1:
         x0, res0 = d.ctx.invert(d.ctx.to_device(d.b), d.gauge, d.A, d.Ai, d.c["kappa"], tol=1e-10, solver="cgne", matpc=0)
         assert res.iterations < res0.iterations
         assert rel_err(xg, x0.cpu().numpy()) < 1e-9

@@ -158,6 +158,23 @@ def test_mat_and_mpc_apply(prec, recon):
             assert rel_err(s.down(out), s.orc.mpc(pe, matpc, dagger)) < TOL[prec], (matpc, dagger)
 
 
+@pytest.mark.parametrize("prec,recon", [(8, 18), (4, 12)])
+def test_mpc_apply_right_preconditioned(prec, recon):
+    """matpc 2 (include/lqcd.h): Mhat_r = 1 - k^2 D_eo A_oo^-1 D_oe A_ee^-1 = (asymmetric Mhat) A_ee^-1 by definition;
+    expected values compose the oracle's clover-inverse apply and its asymmetric Schur complement."""
+    s, c = from_cfg(2, prec, recon)
+    psi = s.spinor("gaussian", 31)
+    psi[1] = 0
+    nat = s.up(psi)
+    out = s.ctx.new_spinor(2)
+    want = s.orc.mpc(s.orc.clover_apply(psi, inverse=True, only_parity=0), 0, False)
+    want_dag = s.orc.clover_apply(s.orc.mpc(psi, 0, True), inverse=True, only_parity=0)
+    for dagger, w in ((False, want), (True, want_dag)):
+        out.zero_()
+        s.ctx.mpc_apply(s.ctx.parity(out, 0), s.ctx.parity(nat, 0), s.gauge, s.A, s.Ai, s.kappa, 2, dagger)
+        assert rel_err(s.down(out)[0], w[0]) < TOL[prec], dagger
+
+
 def test_blas_kernels():
     for prec in (8, 4):
         s = Setup((4, 6, 4, 8), 0.4, 3, 0.12, 1.0, prec, 18, with_clover=False)

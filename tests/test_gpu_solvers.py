@@ -39,7 +39,7 @@ def test_config1_point_source_cgne_fp64():
 
 
 @pytest.mark.parametrize("solver", ["cgne", "cgnr", "bicgstab"])
-@pytest.mark.parametrize("matpc", [0, 1])
+@pytest.mark.parametrize("matpc", [0, 1, 2])
 def test_config2_z2_source_fp64(solver, matpc):
     s, c = from_cfg(2, 8, 18)
     b = synth.source(c["dims"], "z2", c["src_seed"])
