@@ -230,9 +230,12 @@ def extras(torch, lqcd, synth, U, b, ctx, gauge, device):
     mixed = {}
     for solver in ("cgne", "bicgstab"):
         for _ in range(2):
-            _, r64 = ctx.invert(b_dev, gauge, A, Ai, kappa, tol=1e-10, maxiter=2000, solver=solver, matpc=MATPC)
+            # CGNE: right-preconditioned symmetric form (no clover apply per iteration); BiCGStab applies only
+            # Mhat, never its adjoint, and the left form is two fused launches
+            mp = MATPC if solver == "cgne" else 1
+            _, r64 = ctx.invert(b_dev, gauge, A, Ai, kappa, tol=1e-10, maxiter=2000, solver=solver, matpc=mp)
             _, rmx = ctx.invert_mixed(lo, b_dev, gauge, A, Ai, g_lo, A_lo, Ai_lo, kappa, tol=1e-10,
-                                      inner_tol=1e-5, maxiter=2000, solver=solver, matpc=MATPC)
+                                      inner_tol=1e-5, maxiter=2000, solver=solver, matpc=mp)
         mixed[solver] = {"fp64_seconds": r64.seconds, "fp64_iterations": r64.iterations,
                          "mixed_seconds": rmx.seconds, "mixed_inner_iterations": rmx.iterations,
                          "mixed_true_resid": rmx.true_resid, "fp64_true_resid": r64.true_resid,
@@ -249,11 +252,11 @@ def extras(torch, lqcd, synth, U, b, ctx, gauge, device):
         e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
         e0.record()
         r1 = [ctx.invert_mixed(lo, B[j], gauge, A, Ai, g_lo, A_lo, Ai_lo, kappa, tol=1e-10, inner_tol=1e-5,
-                               maxiter=2000, solver="bicgstab", matpc=MATPC, workspace=ws, workspace_lo=ws_lo)[1]
+                               maxiter=2000, solver="bicgstab", matpc=1, workspace=ws, workspace_lo=ws_lo)[1]
               for j in range(12)]
         e1.record()
         _, rs, rc = ctx.invert_multi_mixed(lo, B, gauge, A, Ai, g_lo, A_lo, Ai_lo, kappa, tol=1e-10, inner_tol=1e-5,
-                                           maxiter=2000, solver="bicgstab", matpc=MATPC, workspace=ws,
+                                           maxiter=2000, solver="bicgstab", matpc=1, workspace=ws,
                                            workspace_lo=ws_lo)
         e2.record()
         torch.cuda.synchronize()
