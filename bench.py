@@ -280,9 +280,10 @@ def extras(torch, lqcd, synth, U, b, ctx, gauge, device):
     for _ in range(2):
         e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
         e0.record()
-        its = [p.invert(B[j], g3, A3, Ai3, c3["kappa"], tol=1e-6, solver="cgne")[1].iterations for j in range(12)]
+        its = [p.invert(B[j], g3, A3, Ai3, c3["kappa"], tol=1e-6, solver="cgne", matpc=MATPC)[1].iterations
+               for j in range(12)]
         e1.record()
-        _, rs, rc = p.invert_multi(B, g3, A3, Ai3, c3["kappa"], tol=1e-6, solver="cgne")
+        _, rs, rc = p.invert_multi(B, g3, A3, Ai3, c3["kappa"], tol=1e-6, solver="cgne", matpc=MATPC)
         e2.record()
         torch.cuda.synchronize()
     out["propagator_16x32_fp32_recon12"] = {
