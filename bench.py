@@ -379,10 +379,10 @@ def run_gpu(args):
     A, Ai = ctx.empty(ctx.clover_bytes), ctx.empty(ctx.clover_bytes)
 
     def step_e2e():
-        ctx.gauge_pack_host(gauge, U_h, g_scr)
-        ctx._check(lib.lqcd_clover_build(ctx.h, P(A), P(Ai), P(gauge), csw, kappa, S()))
-        return ctx.invert_host(x_h, b_h, gauge, A, Ai, kappa, h_scr, tol=tol, maxiter=2000, solver="cgne",
-                               matpc=MATPC)[1]
+        # one C-ABI call from host buffers: uploads on the context's copy stream (the source goes up while the
+        # links are packed and the clover field is built), solve, download
+        return ctx.solve_host(x_h, b_h, U_h, gauge, A, Ai, csw, kappa, g_scr, h_scr, tol=tol, maxiter=2000,
+                              solver="cgne", matpc=MATPC)[1]
 
     step_e2e()
     barrier()

@@ -244,6 +244,17 @@ int lqcd_invert_host(lqcd_ctx* ctx, void* x_public_host, const void* b_public_ho
                      int solver, int matpc, void* scratch, size_t scratch_bytes, lqcd_result* res,
                      void* stream);
 
+/* The whole path from HOST buffers in one call (loadGauge, clover creation, invert): uploads the
+ * public links and source, packs, builds clover and inverse, solves, downloads the public solution.  The uploads
+ * run on a copy stream owned by the context, so the source upload overlaps the link pack and the clover build.
+ * gauge, clover, clover_inv: device buffers (lqcd_*_bytes) that receive the native fields and stay valid for later
+ * calls; g_scratch: device, >= 4*V*18*prec bytes; scratch: device, >= lqcd_host_scratch_bytes.  Host-synchronous;
+ * returns res->status. */
+int lqcd_solve_host(lqcd_ctx* ctx, void* x_public_host, const void* b_public_host, const void* gauge_public_host,
+                    void* gauge, void* clover, void* clover_inv, double csw, double kappa, double tol, int maxiter,
+                    int solver, int matpc, void* g_scratch, void* scratch, size_t scratch_bytes, lqcd_result* res,
+                    void* stream);
+
 /* Fused BLAS-1 kernels of the solvers, exposed for parity tests and bandwidth measurement
  * (SURVEY.md §8(a) a9).  Vectors are one-parity native spinors; results are fp64 on the host;
  * these calls synchronise.  a, b are complex given as {re, im}.

@@ -93,7 +93,11 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], int prec, int recon, int t_bo
             cudaMallocHost(&c->h_scalars, sizeof(double) * 64 * LQCD_MAX_RHS) == cudaSuccess &&
             cudaMallocHost(&c->h_consts, sizeof(double) * 2) == cudaSuccess &&
             cudaMallocHost(&c->h_flag, sizeof(int) * 4) == cudaSuccess &&
-            cudaEventCreate(&c->ev0) == cudaSuccess && cudaEventCreate(&c->ev1) == cudaSuccess;
+            cudaEventCreate(&c->ev0) == cudaSuccess && cudaEventCreate(&c->ev1) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaEventCreateWithFlags(&c->ev_copy[0], cudaEventDisableTiming) == cudaSuccess &&
+            cudaEventCreateWithFlags(&c->ev_copy[1], cudaEventDisableTiming) == cudaSuccess &&
+            cudaEventCreateWithFlags(&c->ev_copy[2], cudaEventDisableTiming) == cudaSuccess;
   if (ok) {
     c->h_consts[0] = 0.0;
     c->h_consts[1] = 1.0;
@@ -122,6 +126,9 @@ int lqcd_destroy(lqcd_ctx* c) {
   if (c->h_flag) cudaFreeHost(c->h_flag);
   if (c->ev0) cudaEventDestroy(c->ev0);
   if (c->ev1) cudaEventDestroy(c->ev1);
+  for (int i = 0; i < 3; i++)
+    if (c->ev_copy[i]) cudaEventDestroy(c->ev_copy[i]);
+  if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   if (c->prof_ev) {
     for (int i = 0; i < 2 * c->prof_cap; i++) cudaEventDestroy(c->prof_ev[i]);
     delete[] c->prof_ev;

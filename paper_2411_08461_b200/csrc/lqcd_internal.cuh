@@ -37,6 +37,8 @@ struct lqcd_ctx {
   int* h_flag;
   int max_red_blocks;
   cudaEvent_t ev0, ev1;
+  cudaStream_t copy_stream;      // lqcd_solve_host: uploads run here, beside the kernels of the caller's stream
+  cudaEvent_t ev_copy[3];        // entry fence, links uploaded, source uploaded
   // accounting: algorithmic bytes of every launch; optional per-launch event timing of dslash
   double alg_bytes;
   int acct_rhs;  // active right-hand sides of a batched solve (byte accounting of frozen columns)

@@ -748,6 +748,37 @@ int lqcd_invert_host(lqcd_ctx* c, void* x_host, const void* b_host, const void* 
   return rc;
 }
 
+// The whole path from host buffers in one call: links and source go up on the context's copy stream while the
+// caller's stream packs the links and builds the clover field (the source upload hides behind pack + build), then
+// the solve, then the solution goes down.  g_scratch: >= 4*V*18*prec bytes; scratch: as lqcd_invert_host.
+int lqcd_solve_host(lqcd_ctx* c, void* x_host, const void* b_host, const void* gauge_public_host, void* gauge,
+                    void* clover, void* clover_inv, double csw, double kappa, double tol, int maxiter, int solver,
+                    int matpc, void* g_scratch, void* scratch, size_t scratch_bytes, lqcd_result* res, void* stream) {
+  if (!c || !x_host || !b_host || !gauge_public_host || !gauge || !clover || !clover_inv || !g_scratch || !scratch || !res)
+    return LQCD_ERR_INVALID_ARG;
+  if (scratch_bytes < lqcd_host_scratch_bytes(c, solver)) return lqcd_set_error(c, LQCD_ERR_WORKSPACE, "solve_host: scratch too small");
+  cudaStream_t st = as_stream(stream), cp = c->copy_stream;
+  const size_t sp = lqcd_spinor_bytes(c);
+  char* s = (char*)scratch;
+  int rc;
+  cudaEventRecord(c->ev_copy[0], st);        // the scratch buffers may still be in use by earlier work on `stream`
+  cudaStreamWaitEvent(cp, c->ev_copy[0], 0);
+  cudaMemcpyAsync(g_scratch, gauge_public_host, (size_t)4 * c->V * 18 * c->prec, cudaMemcpyHostToDevice, cp);
+  cudaEventRecord(c->ev_copy[1], cp);
+  cudaMemcpyAsync(s, b_host, 2 * sp, cudaMemcpyHostToDevice, cp);
+  cudaEventRecord(c->ev_copy[2], cp);
+  cudaStreamWaitEvent(st, c->ev_copy[1], 0);
+  if ((rc = lqcd_gauge_pack(c, gauge, g_scratch, stream))) return rc;
+  if ((rc = lqcd_clover_build(c, clover, clover_inv, gauge, csw, kappa, stream))) return rc;
+  cudaStreamWaitEvent(st, c->ev_copy[2], 0);
+  rc = invert_common(c, s + 2 * sp, s, gauge, clover, clover_inv, kappa, 0.0, tol, maxiter, solver, matpc, 1, s + 4 * sp,
+                     scratch_bytes - 4 * sp, res, st);
+  if (rc < 0) return rc;
+  cudaMemcpyAsync(x_host, s + 2 * sp, 2 * sp, cudaMemcpyDeviceToHost, st);
+  if (cudaStreamSynchronize(st) != cudaSuccess) return lqcd_check_cuda(c, "solve_host sync");
+  return rc;
+}
+
 // BLAS-1 entry points: single right-hand side, slot S_DONE of column 0 cleared by every solve's end
 int lqcd_blas_axpy_norm(lqcd_ctx* c, double a, const void* x, void* y, double* norm2_host, void* stream) {
   if (!c || !x || !y || !norm2_host) return LQCD_ERR_INVALID_ARG;

@@ -35,7 +35,7 @@ SYMBOLS = [
     "lqcd_invert", "lqcd_host_scratch_bytes", "lqcd_dslash_host", "lqcd_invert_host",
     "lqcd_blas_axpy_norm", "lqcd_blas_xpay", "lqcd_blas_cdot", "lqcd_blas_caxpbypz",
     "lqcd_dslash_mrhs", "lqcd_mpc_apply_mrhs", "lqcd_invert_multi_workspace_bytes", "lqcd_invert_multi",
-    "lqcd_invert_mixed", "lqcd_invert_multi_mixed", "lqcd_set_anisotropy", "lqcd_clover_build_aniso",
+    "lqcd_invert_mixed", "lqcd_invert_multi_mixed", "lqcd_solve_host", "lqcd_set_anisotropy", "lqcd_clover_build_aniso",
     "lqcd_momentum_phase", "lqcd_source_wall", "lqcd_source_point", "lqcd_propagator_assemble",
     "lqcd_propagator_split", "lqcd_contract_twopt", "lqcd_contract_threept", "lqcd_sequential_source",
 ]
@@ -109,6 +109,8 @@ def load():
     L.lqcd_dslash_host.argtypes = [vp, vp, vp, vp, ci, cd, ci, vp, vp]
     L.lqcd_invert_host.argtypes = [vp, vp, vp, vp, vp, vp, cd, cd, ci, ci, ci, vp, sz,
                                    ctypes.POINTER(Result), vp]
+    L.lqcd_solve_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, cd, cd, cd, ci, ci, ci, vp, vp, sz,
+                                  ctypes.POINTER(Result), vp]
     L.lqcd_blas_axpy_norm.argtypes = [vp, cd, vp, vp, ctypes.POINTER(cd), vp]
     L.lqcd_blas_xpay.argtypes = [vp, vp, cd, vp, vp]
     L.lqcd_blas_cdot.argtypes = [vp, vp, vp, ctypes.POINTER(cd), vp]
@@ -475,6 +477,17 @@ class Context:
                                        _p(clover_inv), kappa, tol, maxiter, SOLVERS[solver], matpc,
                                        _p(scratch), scratch.numel() * self.prec, ctypes.byref(res),
                                        _stream())
+        self._check(rc, allow_not_converged=True)
+        return x_host, res
+
+    def solve_host(self, x_host, b_host, U_host, gauge, clover, clover_inv, csw, kappa, g_scratch, scratch,
+                   tol=1e-10, maxiter=1000, solver="cgne", matpc=0):
+        """Host links + host source -> host solution in one call (uploads overlap the pack and the clover build)."""
+        res = Result()
+        rc = self.lib.lqcd_solve_host(self.h, _p(x_host), _p(b_host), _p(U_host), _p(gauge), _p(clover),
+                                      _p(clover_inv), csw, kappa, tol, maxiter, SOLVERS[solver], matpc,
+                                      _p(g_scratch), _p(scratch), scratch.numel() * self.prec, ctypes.byref(res),
+                                      _stream())
         self._check(rc, allow_not_converged=True)
         return x_host, res
 

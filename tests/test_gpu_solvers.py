@@ -91,6 +91,18 @@ def test_host_entry_points():
     for p in (0, 1):
         s.ctx.dslash_host(oh, bh, s.gauge, p, scratch)
     assert rel_err(oh.numpy(), s.orc.dslash(b)) < 1e-13
+    # the whole path from host buffers in one call: host links + host source -> host solution, native fields left
+    # behind for later calls
+    Uh = torch.from_numpy(s.U).pin_memory()
+    gauge, g_scr = s.ctx.empty(s.ctx.gauge_bytes), s.ctx.empty(Uh.numel() * 16)
+    A, Ai = s.ctx.empty(s.ctx.clover_bytes), s.ctx.empty(s.ctx.clover_bytes)
+    for matpc in (0, 2):
+        x2 = torch.zeros_like(bh).pin_memory()
+        _, r2 = s.ctx.solve_host(x2, bh, Uh, gauge, A, Ai, s.csw, s.kappa, g_scr, scratch, tol=1e-10, solver="cgne",
+                                 matpc=matpc)
+        assert r2.status == 0 and s.orc.true_residual(b, x2.numpy()) < 1e-10
+        assert rel_err(x2.numpy(), xh.numpy()) < 1e-9
+    assert torch.equal(gauge, s.gauge) and torch.equal(A, s.A) and torch.equal(Ai, s.Ai)
 
 
 def test_config3_propagator_12_columns_fp32_recon12():
