@@ -148,6 +148,25 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # GPU arm
 # ------------------------------------------------------------------------------------------------
+def time_batched(torch, fn, n=20, reps=7, warm=6):
+    """Median over `reps` of (device time of n back-to-back asynchronous launches) / n, CUDA events on the launching
+    stream.  The host runs ahead of the device, so no launch gap is inside the interval (an event pair around ONE
+    launch issued from Python contains 10-30 us of host latency: 10 % of a 140 us kernel)."""
+    for i in range(warm):
+        fn(i)
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for i in range(n):
+            fn(i)
+        e1.record()
+        e1.synchronize()
+        ts.append(e0.elapsed_time(e1) * 1e-3 / n)
+    return float(np.median(ts))
+
+
 def dslash_sweep(torch, lqcd, U, psi, dims, device, peak):
     """Standalone dslash (bare hopping term, scale 1) at the workload size for the four
     (precision, reconstruction) variants.  Inputs (links 0.4-1.2 GB) exceed L2 (126 MB)."""
@@ -157,18 +176,7 @@ def dslash_sweep(torch, lqcd, U, psi, dims, device, peak):
         g = ctx.gauge_pack(ctx.to_device(U))
         nat = ctx.spinor_pack(ctx.to_device(psi))
         dst = ctx.new_spinor(2)
-        for i in range(10):
-            ctx.dslash(ctx.parity(dst, i & 1), ctx.parity(nat, 1 - (i & 1)), g, i & 1)
-        torch.cuda.synchronize()
-        ts = []
-        for i in range(40):
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-            ctx.dslash(ctx.parity(dst, i & 1), ctx.parity(nat, 1 - (i & 1)), g, i & 1)
-            e1.record()
-            e1.synchronize()
-            ts.append(e0.elapsed_time(e1) * 1e-3)
-        t = float(np.median(ts))
+        t = time_batched(torch, lambda i: ctx.dslash(ctx.parity(dst, i & 1), ctx.parity(nat, 1 - (i & 1)), g, i & 1))
         by = dslash_alg_bytes(recon, prec, ctx.Vh)
         out["fp%d_recon%d" % (8 * prec, recon)] = {
             "us": t * 1e6, "GBps": by / t / 1e9, "frac_of_measured_peak": by / t / 1e9 / peak,
@@ -176,6 +184,42 @@ def dslash_sweep(torch, lqcd, U, psi, dims, device, peak):
             "bytes_per_site": by // ctx.Vh}
         ctx.close()
         del g, nat, dst
+    return out
+
+
+def kernel_sweep(torch, lqcd, synth, U, psi, dims, device, peak):
+    """The other bandwidth-bound kernels of the path at the workload size (north_star: HBM GB/s for clover apply and
+    the BLAS-1 kernels beside dslash): clover / clover-inverse apply (120 w B/site) and the fused BLAS-1 entry points
+    (vectors streamed x 24 w B/site).  One-parity fields of 100-600 MB: larger than L2 together.  The two reduction
+    kernels return their scalars to the host, so their time includes that read-back."""
+    cfg = synth.CONFIGS[WORKLOAD]
+    out = {}
+    for prec in (4, 8):
+        ctx = lqcd.Context(dims, prec, 18, -1, device)
+        g = ctx.gauge_pack(ctx.to_device(U))
+        A, Ai = ctx.clover_build(g, cfg["csw"], cfg["kappa"])
+        nat = ctx.spinor_pack(ctx.to_device(psi))
+        x, y = ctx.parity(nat, 0), ctx.parity(nat, 1)
+        z, w = ctx.new_spinor(1), ctx.new_spinor(1)
+        z.copy_(x)
+        w.copy_(y)
+        site = ctx.Vh * prec
+        runs = (("clover_apply", lambda i: ctx.clover_apply(z if i & 1 else w, x if i & 1 else y, A, i & 1), 120),
+                ("clover_inverse_apply", lambda i: ctx.clover_apply(z if i & 1 else w, x if i & 1 else y, Ai, i & 1), 120),
+                ("blas_xpay", lambda i: ctx.blas_xpay(x if i & 1 else y, 0.5, z if i & 1 else w), 72),
+                ("blas_caxpbypz", lambda i: ctx.blas_caxpbypz(0.5 + 0.1j, x, 0.25 - 0.2j, y, z if i & 1 else w), 96),
+                ("blas_axpy_norm", lambda i: ctx.blas_axpy_norm(1e-3, x if i & 1 else y, z if i & 1 else w), 72),
+                ("blas_cdot", lambda i: ctx.blas_cdot(x if i & 1 else z, y if i & 1 else w), 48))
+        row = {}
+        for name, fn, reals in runs:
+            t = time_batched(torch, fn)
+            row[name] = {"us": t * 1e6, "GBps": reals * site / t / 1e9, "frac_of_measured_peak": reals * site / t / 1e9 / peak,
+                         "bytes_per_site": reals * prec}
+            if name in ("blas_axpy_norm", "blas_cdot"):
+                row[name]["includes_host_readback"] = True  # the call returns its scalars: stream sync inside
+        out["fp%d" % (8 * prec)] = row
+        ctx.close()
+        del g, A, Ai, nat, z, w
     return out
 
 
@@ -191,18 +235,7 @@ def mrhs_sweep(torch, lqcd, U, psi, dims, device, peak, nrhs=12):
         n = ctx.spinor_bytes // prec
         src = [torch.cat([ctx.parity(nat, p)] * nrhs) for p in (0, 1)]
         dst = ctx.new_spinor(nrhs)
-        for i in range(4):
-            ctx.dslash_mrhs(dst, src[1 - (i & 1)], g, i & 1, nrhs)
-        torch.cuda.synchronize()
-        ts = []
-        for i in range(20):
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-            ctx.dslash_mrhs(dst, src[1 - (i & 1)], g, i & 1, nrhs)
-            e1.record()
-            e1.synchronize()
-            ts.append(e0.elapsed_time(e1) * 1e-3)
-        t = float(np.median(ts))
+        t = time_batched(torch, lambda i: ctx.dslash_mrhs(dst, src[1 - (i & 1)], g, i & 1, nrhs), n=6, reps=5, warm=4)
         by = (8 * recon + nrhs * 48) * prec * ctx.Vh
         out["fp%d_recon%d" % (8 * prec, recon)] = {
             "nrhs": nrhs, "us": t * 1e6, "us_per_column": t * 1e6 / nrhs, "GBps": by / t / 1e9,
@@ -427,6 +460,7 @@ def run_gpu(args):
     }
     if rank == 0 and not args.no_sweep:
         line["dslash"] = dslash_sweep(torch, lqcd, U, b, dims, local, peak)
+        line["kernels"] = kernel_sweep(torch, lqcd, synth, U, b, dims, local, peak)
     if rank == 0 and world == 1 and not args.no_extras:
         line["next_rows"] = extras(torch, lqcd, synth, U, b, ctx, gauge, local)
         line["next_rows"]["dslash_mrhs_32x64"] = mrhs_sweep(torch, lqcd, U, b, dims, local, peak)

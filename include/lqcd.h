@@ -257,12 +257,12 @@ int lqcd_solve_host(lqcd_ctx* ctx, void* x_public_host, const void* b_public_hos
 
 /* Fused BLAS-1 kernels of the solvers, exposed for parity tests and bandwidth measurement
  * (SURVEY.md §8(a) a9).  Vectors are one-parity native spinors; results are fp64 on the host;
- * these calls synchronise.  a, b are complex given as {re, im}.
+ * the two that return a scalar (axpy_norm, cdot) synchronise, the other two are asynchronous.  a, b are complex
+ * given as {re, im}.
  *   lqcd_blas_axpy_norm : y += a*x (a real),  returns |y|^2
  *   lqcd_blas_xpay      : y  = x + a*y (a real)
  *   lqcd_blas_cdot      : returns <x,y> = sum conj(x_i) y_i  and |x|^2 in out[0..2]
- *   lqcd_blas_caxpbypz  : z += a*x + b*y (a, b complex)
- *   lqcd_blas_cxpaypbz  : y  = x + a*y + b*z ... see DESIGN.md for the BiCGStab updates */
+ *   lqcd_blas_caxpbypz  : z += a*x + b*y (a, b complex) */
 int lqcd_blas_axpy_norm(lqcd_ctx* ctx, double a, const void* x, void* y, double* norm2_host, void* stream);
 int lqcd_blas_xpay(lqcd_ctx* ctx, const void* x, double a, void* y, void* stream);
 int lqcd_blas_cdot(lqcd_ctx* ctx, const void* x, const void* y, double out_host[3], void* stream);

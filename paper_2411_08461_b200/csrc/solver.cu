@@ -798,7 +798,6 @@ int lqcd_blas_xpay(lqcd_ctx* c, const void* x, double a, void* y, void* stream) 
   void* v[2] = {(void*)x, y};
   int rc;
   if ((rc = BLAS_CALL(c, OpXpay, op.a = a, v, nullptr, 1, 0, st))) return rc;
-  if (cudaStreamSynchronize(st) != cudaSuccess) return lqcd_check_cuda(c, "blas_xpay sync");
   return LQCD_OK;
 }
 
@@ -821,7 +820,6 @@ int lqcd_blas_caxpbypz(lqcd_ctx* c, const double a[2], const void* x, const doub
   void* v[3] = {(void*)x, (void*)y, z};
   int rc;
   if ((rc = BLAS_CALL(c, OpCaxpbypz, (op.a = {a[0], a[1]}, op.b = {b[0], b[1]}), v, nullptr, 1, 0, st))) return rc;
-  if (cudaStreamSynchronize(st) != cudaSuccess) return lqcd_check_cuda(c, "blas_caxpbypz sync");
   return LQCD_OK;
 }
 
