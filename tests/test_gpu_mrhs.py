@@ -207,3 +207,50 @@ def test_propagator_sharded_single_rank_equals_propagator():
     p2, iters, rc2 = s.ctx.propagator_sharded(B, s.gauge, s.A, s.Ai, s.kappa, tol=1e-10, solver="bicgstab")
     assert rc1 == 0 and rc2 == 0 and iters == [r.iterations for r in res]
     assert torch.equal(p1, p2)
+
+
+@pytest.mark.parametrize("solver", ["cgne", "bicgstab"])
+@pytest.mark.parametrize("matpc", [1, 2])
+def test_invert_multi_symmetric_forms_config2(solver, matpc):
+    """Batched solves on the symmetric Schur complements (left and right; the multi-RHS kernels have no epilogue 6, so
+    the clover-first products go through the generic path): every column meets reading A17 and equals the column's
+    own single solve."""
+    s, c = from_cfg(2, 8, 18)
+    dims = c["dims"]
+    bs = [synth.source(dims, "point", spin=1, colour=2), synth.source(dims, "z2", 102), synth.source(dims, "gaussian", 5)]
+    B = s.ctx.to_device(np.stack(bs))
+    x, res, rc = s.ctx.invert_multi(B, s.gauge, s.A, s.Ai, s.kappa, tol=1e-10, maxiter=2000, solver=solver, matpc=matpc)
+    assert rc == 0
+    xs = x.cpu().numpy()
+    for r, b in enumerate(bs):
+        true = s.orc.true_residual(b, xs[r])
+        assert res[r].status == 0 and true < 1e-10 and abs(true - res[r].true_resid) < 5e-11, (r, true, res[r].as_dict())
+        xo, ro = s.orc.invert(b, 1e-12, 2000, "bicgstab", 0)
+        assert rel_err(xs[r], xo) < 1e-9, r
+        x1, r1 = s.ctx.invert(s.ctx.to_device(b), s.gauge, s.A, s.Ai, s.kappa, tol=1e-10, maxiter=2000, solver=solver,
+                              matpc=matpc)
+        assert r1.iterations == res[r].iterations and rel_err(xs[r], x1.cpu().numpy()) < 1e-11
+
+
+@pytest.mark.parametrize("solver,matpc", [("cgne", 2), ("bicgstab", 1)])
+def test_invert_multi_mixed_symmetric_forms_config2(solver, matpc):
+    """The forms bench.py times for the mixed-precision rows (CGNE: right, BiCGStab: left), batched, against the oracle."""
+    s, c = from_cfg(2, 8, 18)
+    dims = c["dims"]
+    lo = lq().Context(dims, 4, 12, -1)
+    g_lo = lo.gauge_pack(lo.to_device(s.U))
+    A_lo, Ai_lo = lo.clover_build(g_lo, c["csw"], c["kappa"])
+    bs = [synth.source(dims, "point", spin=0, colour=1), synth.source(dims, "gaussian", 6), synth.source(dims, "z2", 103)]
+    B = s.ctx.to_device(np.stack(bs))
+    x, res, rc = s.ctx.invert_multi_mixed(lo, B, s.gauge, s.A, s.Ai, g_lo, A_lo, Ai_lo, s.kappa, tol=1e-10,
+                                          inner_tol=1e-4, maxiter=2000, solver=solver, matpc=matpc)
+    assert rc == 0, [r.as_dict() for r in res]
+    xs = x.cpu().numpy()
+    for r, b in enumerate(bs):
+        true = s.orc.true_residual(b, xs[r])
+        assert true < 1e-10 and abs(true - res[r].true_resid) < 5e-11, (r, true, res[r].as_dict())
+        xo, ro = s.orc.invert(b, 1e-12, 2000, "bicgstab", 0)
+        assert rel_err(xs[r], xo) < 1e-9, r
+    x1, r1 = s.ctx.invert_mixed(lo, B[1], s.gauge, s.A, s.Ai, g_lo, A_lo, Ai_lo, s.kappa, tol=1e-10, inner_tol=1e-4,
+                                maxiter=2000, solver=solver, matpc=matpc)
+    assert r1.status == 0 and s.orc.true_residual(bs[1], x1.cpu().numpy()) < 1e-10
