@@ -307,9 +307,8 @@ template <typename T> static bool tile_fits(const Lat& L) {
 bool lqcd_dslash_tiled(const lqcd_ctx* c) {
   return c->tiled && (c->prec == 4 ? tile_fits<float>(c->lat) : tile_fits<double>(c->lat));
 }
-// blocks of a single-RHS dslash launch (= per-block partials of the fused epilogues 4, 5)
+// blocks of a launch of dslash_kernel (= per-block partials of the epilogues that reduce; those never run tiled)
 int lqcd_dslash_grid(const lqcd_ctx* c) {
-  if (lqcd_dslash_tiled(c)) return c->lat.Vh / (c->prec == 4 ? TileOf<float>::TS::NOUT : TileOf<double>::TS::NOUT);
   const int block = c->prec == 4 ? DSLASH_BLOCK_F32 : DSLASH_BLOCK_F64;
   return (c->lat.Vh + block - 1) / block;
 }
@@ -325,13 +324,7 @@ static void launch_tiled(const DslashArgs<T>& a, int epi, cudaStream_t st) {
     cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 7>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 9>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 10>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     configured = true;
   }
   switch (epi) {
@@ -339,13 +332,7 @@ static void launch_tiled(const DslashArgs<T>& a, int epi, cudaStream_t st) {
     case 1: dslash_tiled_kernel<T, R, DAG, 1><<<grid, TS::NOUT, smem, st>>>(a); break;
     case 2: dslash_tiled_kernel<T, R, DAG, 2><<<grid, TS::NOUT, smem, st>>>(a); break;
     case 3: dslash_tiled_kernel<T, R, DAG, 3><<<grid, TS::NOUT, smem, st>>>(a); break;
-    case 4: dslash_tiled_kernel<T, R, DAG, 4><<<grid, TS::NOUT, smem, st>>>(a); break;
-    case 5: dslash_tiled_kernel<T, R, DAG, 5><<<grid, TS::NOUT, smem, st>>>(a); break;
-    case 6: dslash_tiled_kernel<T, R, DAG, 6><<<grid, TS::NOUT, smem, st>>>(a); break;
-    case 7: dslash_tiled_kernel<T, R, DAG, 7><<<grid, TS::NOUT, smem, st>>>(a); break;
-    case 8: dslash_tiled_kernel<T, R, DAG, 8><<<grid, TS::NOUT, smem, st>>>(a); break;
-    case 9: dslash_tiled_kernel<T, R, DAG, 9><<<grid, TS::NOUT, smem, st>>>(a); break;
-    default: dslash_tiled_kernel<T, R, DAG, 10><<<grid, TS::NOUT, smem, st>>>(a); break;
+    default: dslash_tiled_kernel<T, R, DAG, 6><<<grid, TS::NOUT, smem, st>>>(a); break;
   }
 }
 
@@ -363,7 +350,7 @@ static void launch_epi(DslashArgs<T> a, int epi, cudaStream_t st) {
   const size_t smem = SStage<T>::ROUNDS > 0 ? (size_t)(8 / SStage<T>::ROUNDS) * 24 * sizeof(T) * block  // spinors
                       : Tune<T, R>::STAGE ? (size_t)8 * R * sizeof(T) * block : 0;                      // eight links per thread
   static bool configured = false;  // one flag per (T, R, DAG) instantiation
-  if (!configured && smem > 48 * 1024) {
+  if (!configured && smem > 40 * 1024) {  // the epilogues that reduce add static shared memory on top of `smem`
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -412,7 +399,7 @@ static void launch_typed(lqcd_ctx* c, void* out, const void* in, const void* gau
   a.parity = parity;
   a.scale = (T)scale;
   a.ws = (T)c->ws;
-  if (lqcd_dslash_tiled(c)) {
+  if (lqcd_dslash_tiled(c) && (epi <= 3 || epi == 6)) {  // the tiled form exists for the epilogues without a reduction
     if (c->recon == 18) {
       if (dagger) launch_tiled<T, 18, true>(a, epi, st);
       else launch_tiled<T, 18, false>(a, epi, st);

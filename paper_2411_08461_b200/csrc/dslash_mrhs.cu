@@ -372,7 +372,7 @@ static void launch_mrhs_staged(MrhsArgs<T> a, int epi, int nrhs, cudaStream_t st
   const int grid = (a.lat.Vh + MRHS_SITES - 1) / MRHS_SITES;
   const size_t smem = (size_t)2 * MrhsStage<T, R>::HPR * 24 * sizeof(T) * MRHS_MAXT;
   static bool configured = false;  // one flag per (T, R, DAG) instantiation
-  if (!configured && smem > 48 * 1024) {
+  if (!configured && smem > 40 * 1024) {
     cudaFuncSetAttribute(dslash_mrhs_staged_kernel<T, R, DAG, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_mrhs_staged_kernel<T, R, DAG, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_mrhs_staged_kernel<T, R, DAG, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

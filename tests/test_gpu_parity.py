@@ -205,7 +205,8 @@ def test_blas_kernels():
 def test_tiled_dslash_matches_oracle(prec, recon, dims, tb, monkeypatch):
     """The opt-in shared-memory tiled kernel (csrc/dslash_tiled.cuh, LQCD_DSLASH_TILED=1 at context creation):
     several tiles per direction, tiles spanning a whole extent (the halo wraps onto the tile itself), the seam in t,
-    every epilogue through M and M-hat, and the CG-fused epilogues 4 and 5 through a CGNE solve."""
+    every epilogue without a reduction through M and M-hat (both forms, adjoints: 0-3 and 6), and a CGNE solve in which
+    the tiled kernel does the A^-1 D hops and the default kernel the epilogues that reduce."""
     monkeypatch.setenv("LQCD_DSLASH_TILED", "1")
     s = Setup(dims, 0.5, 2, 0.124, 1.2, prec, recon, tb)
     psi = s.spinor("gaussian", 102)

@@ -157,3 +157,13 @@ def test_config2_mixed_precision_reaches_fp64_tolerance(solver, recon_lo):
     # argument checks: contexts swapped / same precision
     with pytest.raises(lq().LqcdError):
         s.ctx.invert_mixed(s.ctx, s.ctx.to_device(b), s.gauge, s.A, s.Ai, s.gauge, s.A, s.Ai, s.kappa)
+
+
+@pytest.mark.parametrize("matpc", [0, 1, 2])
+def test_config2_cgne_fp64_recon12(matpc):
+    """fp64 with reconstruct-12 links: the kernel variant that stages its links through shared memory with cp.async
+    (exactly 48 KB of dynamic shared memory) under the CG-fused epilogues, which add static shared memory of their own."""
+    s, c = from_cfg(2, 8, 12)
+    b = synth.source(c["dims"], "z2", c["src_seed"])
+    xo, ro = s.orc.invert(b, 1e-10, 2000, "bicgstab", 0)
+    solve_and_check(s, b, "cgne", matpc, 1e-10, xo)
