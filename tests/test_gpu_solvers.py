@@ -56,6 +56,10 @@ def test_config2_bicgstab_fp32(recon):
     # allowing the fp32 rounding floor of the recurrence (2x)
     solve_and_check(s, b, "bicgstab", 0, 1e-6, xo, resid_bound=2e-6)
     solve_and_check(s, b, "cgne", 0, 1e-6, xo, resid_bound=2e-6)
+    # the symmetric forms in fp32 (packed FFMA2 epilogues 6-10, clover_mul_twice)
+    for matpc in (1, 2):
+        solve_and_check(s, b, "cgne", matpc, 1e-6, xo, resid_bound=2e-6)
+        solve_and_check(s, b, "bicgstab", matpc, 1e-6, xo, resid_bound=2e-6)
 
 
 def test_invert_builds_clover_when_absent_and_edge_cases():
