@@ -325,6 +325,33 @@ def extras(torch, lqcd, synth, U, b, ctx, gauge, device):
         "iterations_batched": [r.iterations for r in rs], "status": rc,
         "worst_true_resid": max(r.true_resid for r in rs)}
     p.close()
+    del g3, A3, Ai3, B
+    # BASELINE configs[4] (48^3x96, 10.6M sites, fp32 reconstruct-12): capacity and bandwidth of dslash and
+    # clover-inverse apply, and a BiCGStab solve to 1e-6 (symmetric form from the left: BiCGStab never applies the adjoint)
+    c5 = synth.CONFIGS[5]
+    dims = c5["dims"]
+    U5 = synth.gauge(dims, c5["eps"], c5["seed"])
+    b5 = synth.source(dims, c5["source"], c5["src_seed"])
+    q = lqcd.Context(dims, 4, 12, -1, device)
+    g5 = q.gauge_pack(q.to_device(U5))
+    del U5
+    A5, Ai5 = q.clover_build(g5, c5["csw"], c5["kappa"])
+    nat = q.spinor_pack(q.to_device(b5))
+    dst = q.new_spinor(2)
+    peak = measured_peaks()[0]
+    td = time_batched(torch, lambda i: q.dslash(q.parity(dst, i & 1), q.parity(nat, 1 - (i & 1)), g5, i & 1), n=10, reps=5)
+    tc = time_batched(torch, lambda i: q.clover_apply(q.parity(dst, i & 1), q.parity(nat, i & 1), Ai5, i & 1), n=10, reps=5)
+    bd, bc = dslash_alg_bytes(12, 4, q.Vh), 120 * 4 * q.Vh
+    for _ in range(2):
+        _, r5 = q.invert(q.to_device(b5), g5, A5, Ai5, c5["kappa"], tol=1e-6, maxiter=2000, solver="bicgstab", matpc=1)
+    out["capacity_48x96_fp32_recon12"] = {
+        "device_bytes_fields": int(q.gauge_bytes + 2 * q.clover_bytes + 2 * 2 * q.spinor_bytes),
+        "dslash": {"us": td * 1e6, "GBps": bd / td / 1e9, "frac_of_measured_peak": bd / td / 1e9 / peak,
+                   "frac_of_8TBps": bd / td / 8e12, "GFLOPs": FLOPS_PER_SITE * q.Vh / td / 1e9},
+        "clover_inverse_apply": {"us": tc * 1e6, "GBps": bc / tc / 1e9, "frac_of_measured_peak": bc / tc / 1e9 / peak},
+        "bicgstab_1e-6": {"seconds": r5.seconds, "iterations": r5.iterations, "true_resid": r5.true_resid,
+                          "status": r5.status}}
+    q.close()
     return out
 
 
