@@ -206,6 +206,9 @@ __device__ __forceinline__ void store_block(T* __restrict__ field, int Vh, int i
 // planes of a site run in parallel and no thread holds more than one F.  Phase 2: threads (s, k < 2)
 // assemble chiral block k, pack it, invert it by Gauss-Jordan and store both.
 constexpr int CB_SITES = 32;
+#ifndef CB_ZC
+#define CB_ZC 4  // z-planes per slab of the traversal order
+#endif
 #ifndef CB_MINB
 #define CB_MINB 2  // 170 registers, 12 warps/SM: 5.84 -> 4.59 ms at 32^3x64 fp64 (3 blocks/SM spill: 9.1 ms)
 #endif
@@ -215,9 +218,26 @@ __global__ void __launch_bounds__(CB_SITES * 6, CB_MINB) clover_build_kernel(T* 
                                                                     double kt, int* flag) {
   __shared__ cd Fs[6][9][CB_SITES];  // planes xy, xz, xt, yz, yt, zt
   const int ls = threadIdx.x, pl = threadIdx.y;
-  const int gid = blockIdx.x * CB_SITES + ls;
-  const bool live = gid < 2 * L.Vh;
-  const int par = live ? gid / L.Vh : 0, idx = live ? gid % L.Vh : 0;
+  // Traversal order.  Every link is needed by the 14 sites of its two-hop neighbourhood, of both parities; in plain
+  // checkerboard order (all even sites, then all odd; t slowest) the reuse window is three whole time slices of all
+  // links, twice over.  Here a block pair = the even and the odd sites of the same 32 checkerboard indices, and the
+  // index runs (x, y, z within a slab of CB_ZC planes, t, slab): the window is three time slices of ONE z-slab
+  // (7 MB at 32^3x64).  Measured (ncu, 32^3x64 fp64): DRAM reads 10.8 -> 7.1 GB, L2 hit rate 42 -> 55 %, time
+  // unchanged (4.5 ms; any CB_ZC from 2 to 16): the kernel waits on its 12 warps per SM, not on DRAM.
+  const int par = blockIdx.x & 1;
+  const int k = (blockIdx.x >> 1) * CB_SITES + ls;
+  const bool live = k < L.Vh;
+  int idx = 0;
+  if (live) {
+    const int zc = (L.Lz % CB_ZC == 0) ? CB_ZC : 2;  // every extent is even
+    const int plane = L.Lxh * L.Ly;
+    const int xy = k % plane;
+    int q = k / plane;
+    const int zl = q % zc;
+    q /= zc;
+    const int t = q % L.Lt, slab = q / L.Lt;
+    idx = xy + plane * ((slab * zc + zl) + L.Lz * t);
+  }
   if (live) {
     const Site s = site_of(L, idx, par);
     const int x0[4] = {2 * s.xh + s.r, s.y, s.z, s.t};
@@ -286,7 +306,7 @@ extern "C" int lqcd_clover_build_aniso(lqcd_ctx* c, void* clover, void* clover_i
   if (!lqcd_aligned16(clover) || !lqcd_aligned16(clover_inv) || !lqcd_aligned16(gauge))
     return lqcd_set_error(c, LQCD_ERR_ALIGN, "clover_build: alignment");
   cudaStream_t st = as_stream(stream);
-  const int n = 2 * c->lat.Vh, grid = (n + CB_SITES - 1) / CB_SITES;
+  const int grid = 2 * ((c->lat.Vh + CB_SITES - 1) / CB_SITES);
   const dim3 block(CB_SITES, 6);
   const double kc = kappa * csw_s, kt = kappa * csw_t;
   cudaMemsetAsync(c->d_flag, 0, sizeof(int), st);
