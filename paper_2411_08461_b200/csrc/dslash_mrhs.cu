@@ -85,18 +85,32 @@ __device__ __forceinline__ void hop_mrhs(T (*acc)[24], const T* __restrict__ in,
   }
 }
 
-// out[r] = C v[r] for NB vectors with one load of the clover block
+// The clover rows of a block's MRHS_SITES sites, copied to shared memory once per block ([vector][site]): every
+// column of every column group multiplies by the same 72 reals per site, and reloading them per column from
+// L1/L2 put 288 B x nrhs per site on the L2->SM crossbar (ncu: +3.6 GB per 12-column launch, +250-300 us).
+template <typename T>
+__device__ __forceinline__ void stage_clover_block(typename V16<T>::vec* sm, const T* __restrict__ cl, int Vh, int site0) {
+  typedef typename V16<T>::vec vec;
+  const vec* g = reinterpret_cast<const vec*>(cl);
+  const int nthr = blockDim.x * blockDim.y, tid = threadIdx.y * blockDim.x + threadIdx.x;
+  for (int e = tid; e < Lay<T>::NCV * MRHS_SITES; e += nthr) {
+    const int q = e / MRHS_SITES, sl = e % MRHS_SITES;
+    if (site0 + sl < Vh) sm[e] = ld_stream(g + (size_t)q * Vh + site0 + sl);
+  }
+}
+
+// out[r] = C v[r] for NB vectors; C from the block's shared-memory copy (stage_clover_block), site = threadIdx.x
 template <typename T, int NB>
-__device__ __forceinline__ void clover_mul_mrhs(const T* __restrict__ cl, int Vh, int idx, const T (*v)[24], T (*out)[24]) {
+__device__ __forceinline__ void clover_mul_mrhs(const typename V16<T>::vec* sm, const T (*v)[24], T (*out)[24]) {
   typedef typename V16<T>::vec vec;
   constexpr int N = V16<T>::N;
-  const vec* p = reinterpret_cast<const vec*>(cl) + idx;
+  const vec* p = sm + threadIdx.x;
 #pragma unroll
   for (int k = 0; k < 2; k++) {
     T a[36];
 #pragma unroll
     for (int q = 0; q < 36 / N; q++) {
-      vec w = ld_cached(p + (size_t)(k * (36 / N) + q) * Vh);
+      vec w = p[(k * (36 / N) + q) * MRHS_SITES];
       vec_get(w, a + q * N);
     }
 #pragma unroll
@@ -140,6 +154,11 @@ template <> struct MrhsTune<double> { static constexpr int MINB = MRHS_MINB_F64,
 template <typename T, int R, bool DAG, int EPI, int NB>
 __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kernel(const MrhsArgs<T> a) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  __shared__ typename V16<T>::vec cl_sm[EPI >= 1 ? Lay<T>::NCV * MRHS_SITES : 1];
+  if (EPI >= 1) {
+    stage_clover_block<T>(cl_sm, a.cl, a.lat.Vh, blockIdx.x * blockDim.x);
+    __syncthreads();
+  }
   if (idx >= a.lat.Vh) return;
   const Lat& L = a.lat;
   const int Vh = L.Vh, par = a.parity;
@@ -185,7 +204,7 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kern
     }
   } else if (EPI == 1) {
     T res[NB][24];
-    clover_mul_mrhs<T, NB>(a.cl, Vh, idx, acc, res);
+    clover_mul_mrhs<T, NB>(cl_sm, acc, res);
 #pragma unroll
     for (int r = 0; r < NB; r++) {
 #pragma unroll
@@ -196,7 +215,7 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kern
     T xv[NB][24], res[NB][24];
 #pragma unroll
     for (int r = 0; r < NB; r++) load_spinor<T>(a.x + first + r * stride, Vh, idx, xv[r]);
-    clover_mul_mrhs<T, NB>(a.cl, Vh, idx, xv, res);
+    clover_mul_mrhs<T, NB>(cl_sm, xv, res);
 #pragma unroll
     for (int r = 0; r < NB; r++) {
 #pragma unroll
@@ -205,7 +224,7 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kern
     }
   } else {
     T res[NB][24];
-    clover_mul_mrhs<T, NB>(a.cl, Vh, idx, acc, res);
+    clover_mul_mrhs<T, NB>(cl_sm, acc, res);
 #pragma unroll
     for (int r = 0; r < NB; r++) {
       T xv[24];
@@ -275,6 +294,11 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsStage<T, R>::MINB) dslash_mrhs_
   constexpr int HPR = MrhsStage<T, R>::HPR > 0 ? MrhsStage<T, R>::HPR : 1, NR = 8 / HPR, NSV = Lay<T>::NSV;
   extern __shared__ __align__(16) unsigned char mrhs_smem[];
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  __shared__ vec cl_sm[EPI >= 1 ? Lay<T>::NCV * MRHS_SITES : 1];
+  if (EPI >= 1) {
+    stage_clover_block<T>(cl_sm, a.cl, a.lat.Vh, blockIdx.x * blockDim.x);
+    __syncthreads();
+  }
   if (idx >= a.lat.Vh) return;
   const Lat& L = a.lat;
   const int Vh = L.Vh, par = a.parity;
@@ -343,20 +367,20 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsStage<T, R>::MINB) dslash_mrhs_
       store_spinor<T>(out, Vh, idx, acc[0]);
     } else if (EPI == 1) {
       T res[1][24];
-      clover_mul_mrhs<T, 1>(a.cl, Vh, idx, acc, res);
+      clover_mul_mrhs<T, 1>(cl_sm, acc, res);
 #pragma unroll
       for (int e = 0; e < 24; e++) res[0][e] *= a.scale;
       store_spinor<T>(out, Vh, idx, res[0]);
     } else if (EPI == 2) {
       T xv[1][24], res[1][24];
       load_spinor<T>(a.x + first, Vh, idx, xv[0]);
-      clover_mul_mrhs<T, 1>(a.cl, Vh, idx, xv, res);
+      clover_mul_mrhs<T, 1>(cl_sm, xv, res);
 #pragma unroll
       for (int e = 0; e < 24; e++) res[0][e] += a.scale * acc[0][e];
       store_spinor<T>(out, Vh, idx, res[0]);
     } else {
       T res[1][24], xv[24];
-      clover_mul_mrhs<T, 1>(a.cl, Vh, idx, acc, res);
+      clover_mul_mrhs<T, 1>(cl_sm, acc, res);
       load_spinor<T>(a.x + first, Vh, idx, xv);
 #pragma unroll
       for (int e = 0; e < 24; e++) res[0][e] = xv[e] + a.scale * res[0][e];
