@@ -6,11 +6,11 @@
 // Field layout: NRHS consecutive one-parity native spinors, [rhs][NSV][Vh] vec16.
 // Thread layout: blockDim = (SITES, G).  threadIdx.x = site of the block (a warp = 32 consecutive
 // sites: coalesced 512 B rows), threadIdx.y = group of NB columns kept in registers (NB x 24
-// accumulators), NRHS = G * NB.  A thread loads a link once into registers and applies it to its NB
-// half-spinors; the G warps of a block that share the same sites read the same link rows, so only
-// the first touches L2/HBM and the others hit L1 (links are loaded with the L1-allocating path
-// here, unlike the streaming single-RHS kernel).  Epilogues are those of dslash.cu; the clover
-// block is loaded once per thread for its NB columns.
+// accumulators), NRHS = G * NB.  The eight links and the clover rows of the block's sites are copied to
+// shared memory ONCE per block (streaming loads, the column groups share the copying) and every column
+// of every group reads them from there: re-reading them per column through L1 put up to (8R+72)w bytes
+// per site and column on the L2->SM crossbar, which is what bounds this kernel (12 columns at 32^3x64, fp32
+// 18-real links: 1037 -> 850 us, M-hat 2884 -> 2130 us).  Epilogues are those of dslash.cu.
 // packed FFMA2 arithmetic (lqcd_internal.cuh) is off here: measured at 32^3x64, 12 columns, it changes nothing
 // for 12-real links (1015 vs 1008 us) and the paired registers push the 18-real kernel into spills
 #ifndef MRHS_FFMA2
@@ -53,26 +53,19 @@ template <typename T> struct MrhsArgs {
   int ngroups;    // nrhs / NB column groups; group g is handled by threadIdx.y = g mod blockDim.y
 };
 
-template <typename T, int R>
-__device__ __forceinline__ void load_link_l1(const T* __restrict__ block, int Vh, int idx, T* U) {
-  typedef typename GV<T, R>::vec vec;
-  constexpr int N = GV<T, R>::N;
-  const vec* p = reinterpret_cast<const vec*>(block) + idx;
-#pragma unroll
-  for (int v = 0; v < R / N; v++) {
-    vec q = ld_cached(p + (size_t)v * Vh);
-    vec_get(q, U + v * N);
-  }
-  if (R == 12) recon_row2<T>(U);
-}
-
 template <typename T, int R, int MU, bool FWD, bool DAG, int NB>
 __device__ __forceinline__ void hop_mrhs(T (*acc)[24], const T* __restrict__ in, size_t stride,
-                                         const T* __restrict__ links, int Vh, int nidx, int lidx, T bsign,
-                                         bool seam) {
+                                         const typename GV<T, R>::vec* lk, int Vh, int nidx, T bsign, bool seam) {
   constexpr int S = (FWD != DAG) ? -1 : +1;
+  constexpr int GN = GV<T, R>::N;
   T U[18];
-  load_link_l1<T, R>(links, Vh, lidx, U);
+  // this site's link of this hop, from the block's shared-memory copy [vector][site] (stage_links_block)
+#pragma unroll
+  for (int v = 0; v < R / GN; v++) {
+    typename GV<T, R>::vec q = lk[v * MRHS_SITES];
+    vec_get(q, U + v * GN);
+  }
+  if (R == 12) recon_row2<T>(U);
   // t: antiperiodic seam; x,y,z: hop weight; folded into the accumulation (reconstruct)
   const T sg = (MU == 3) ? (seam ? (T)-1 : (T)1) : bsign;
 #pragma unroll
@@ -153,18 +146,41 @@ template <> struct MrhsTune<double> { static constexpr int MINB = MRHS_MINB_F64,
 
 template <typename T, int R, bool DAG, int EPI, int NB>
 __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kernel(const MrhsArgs<T> a) {
+  typedef typename GV<T, R>::vec gvec;
+  constexpr int NGV = R / GV<T, R>::N;
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   __shared__ typename V16<T>::vec cl_sm[EPI >= 1 ? Lay<T>::NCV * MRHS_SITES : 1];
-  if (EPI >= 1) {
-    stage_clover_block<T>(cl_sm, a.cl, a.lat.Vh, blockIdx.x * blockDim.x);
-    __syncthreads();
-  }
-  if (idx >= a.lat.Vh) return;
+  extern __shared__ __align__(16) unsigned char mrhs_lk_smem[];  // the eight links of the block's sites: [hop][vector][site]
+  gvec* lk_sm = reinterpret_cast<gvec*>(mrhs_lk_smem);
   const Lat& L = a.lat;
   const int Vh = L.Vh, par = a.parity;
+  const bool live = idx < Vh;
   const size_t stride = a.stride;
-  const Site s = site_of(L, idx, par);
+  const Site s = site_of(L, live ? idx : 0, par);
   const size_t blk = (size_t)R * Vh;
+  int nb[8];
+  {
+    const int i0 = live ? idx : 0;
+    nb[0] = neighbour<0, +1>(L, i0, s);
+    nb[1] = neighbour<0, -1>(L, i0, s);
+    nb[2] = neighbour<1, +1>(L, i0, s);
+    nb[3] = neighbour<1, -1>(L, i0, s);
+    nb[4] = neighbour<2, +1>(L, i0, s);
+    nb[5] = neighbour<2, -1>(L, i0, s);
+    nb[6] = neighbour<3, +1>(L, i0, s);
+    nb[7] = neighbour<3, -1>(L, i0, s);
+  }
+  // links and clover rows are the same for every column: copied once per block (column group y copies hops y, y+G, ...)
+  if (live) {
+    for (int h = threadIdx.y; h < 8; h += blockDim.y) {
+      const gvec* gp = reinterpret_cast<const gvec*>(a.gauge + ((h >> 1) * 2 + ((h & 1) ? 1 - par : par)) * blk) + ((h & 1) ? nb[h] : idx);
+#pragma unroll
+      for (int v = 0; v < NGV; v++) lk_sm[(h * NGV + v) * MRHS_SITES + threadIdx.x] = ld_stream(gp + (size_t)v * Vh);
+    }
+  }
+  if (EPI >= 1) stage_clover_block<T>(cl_sm, a.cl, Vh, blockIdx.x * blockDim.x);
+  __syncthreads();
+  if (!live) return;
   for (int g = threadIdx.y; g < a.ngroups; g += blockDim.y) {
   const size_t first = (size_t)g * NB * stride;  // first column of this thread's group
   const T* in = a.in + first;
@@ -176,23 +192,14 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kern
   const T one = a.ws;
   const bool anti = L.tb < 0;
   const bool seam_f = anti && s.t == L.Lt - 1, seam_b = anti && s.t == 0;
-  int n;
-  n = neighbour<0, +1>(L, idx, s);
-  hop_mrhs<T, R, 0, true, DAG, NB>(acc, in, stride, a.gauge + (0 * 2 + par) * blk, Vh, n, idx, one, false);
-  n = neighbour<0, -1>(L, idx, s);
-  hop_mrhs<T, R, 0, false, DAG, NB>(acc, in, stride, a.gauge + (0 * 2 + 1 - par) * blk, Vh, n, n, one, false);
-  n = neighbour<1, +1>(L, idx, s);
-  hop_mrhs<T, R, 1, true, DAG, NB>(acc, in, stride, a.gauge + (1 * 2 + par) * blk, Vh, n, idx, one, false);
-  n = neighbour<1, -1>(L, idx, s);
-  hop_mrhs<T, R, 1, false, DAG, NB>(acc, in, stride, a.gauge + (1 * 2 + 1 - par) * blk, Vh, n, n, one, false);
-  n = neighbour<2, +1>(L, idx, s);
-  hop_mrhs<T, R, 2, true, DAG, NB>(acc, in, stride, a.gauge + (2 * 2 + par) * blk, Vh, n, idx, one, false);
-  n = neighbour<2, -1>(L, idx, s);
-  hop_mrhs<T, R, 2, false, DAG, NB>(acc, in, stride, a.gauge + (2 * 2 + 1 - par) * blk, Vh, n, n, one, false);
-  n = neighbour<3, +1>(L, idx, s);
-  hop_mrhs<T, R, 3, true, DAG, NB>(acc, in, stride, a.gauge + (3 * 2 + par) * blk, Vh, n, idx, -one, seam_f);
-  n = neighbour<3, -1>(L, idx, s);
-  hop_mrhs<T, R, 3, false, DAG, NB>(acc, in, stride, a.gauge + (3 * 2 + 1 - par) * blk, Vh, n, n, -one, seam_b);
+  hop_mrhs<T, R, 0, true, DAG, NB>(acc, in, stride, lk_sm + 0 * NGV * MRHS_SITES + threadIdx.x, Vh, nb[0], one, false);
+  hop_mrhs<T, R, 0, false, DAG, NB>(acc, in, stride, lk_sm + 1 * NGV * MRHS_SITES + threadIdx.x, Vh, nb[1], one, false);
+  hop_mrhs<T, R, 1, true, DAG, NB>(acc, in, stride, lk_sm + 2 * NGV * MRHS_SITES + threadIdx.x, Vh, nb[2], one, false);
+  hop_mrhs<T, R, 1, false, DAG, NB>(acc, in, stride, lk_sm + 3 * NGV * MRHS_SITES + threadIdx.x, Vh, nb[3], one, false);
+  hop_mrhs<T, R, 2, true, DAG, NB>(acc, in, stride, lk_sm + 4 * NGV * MRHS_SITES + threadIdx.x, Vh, nb[4], one, false);
+  hop_mrhs<T, R, 2, false, DAG, NB>(acc, in, stride, lk_sm + 5 * NGV * MRHS_SITES + threadIdx.x, Vh, nb[5], one, false);
+  hop_mrhs<T, R, 3, true, DAG, NB>(acc, in, stride, lk_sm + 6 * NGV * MRHS_SITES + threadIdx.x, Vh, nb[6], -one, seam_f);
+  hop_mrhs<T, R, 3, false, DAG, NB>(acc, in, stride, lk_sm + 7 * NGV * MRHS_SITES + threadIdx.x, Vh, nb[7], -one, seam_b);
 
   T* out = a.out + first;
   if (EPI == 0) {
@@ -272,12 +279,18 @@ template <> struct MrhsStage<double, 12> { static constexpr int HPR = MRHS_HPR_F
 template <> struct MrhsStage<double, 18> { static constexpr int HPR = MRHS_HPR_F64, MINB = MRHS_SMINB_F64; };
 
 template <typename T, int R, int MU, bool FWD, bool DAG>
-__device__ __forceinline__ void hop_mrhs_staged(T* acc, const typename V16<T>::vec* sm, const T* __restrict__ links, int Vh,
-                                                int lidx, T w) {
+__device__ __forceinline__ void hop_mrhs_staged(T* acc, const typename V16<T>::vec* sm, const typename GV<T, R>::vec* lk, T w) {
   typedef typename V16<T>::vec vec;
   constexpr int S = (FWD != DAG) ? -1 : +1;
+  constexpr int GN = GV<T, R>::N;
   T U[18], psi[24], h[12], chi[12];
-  load_link_l1<T, R>(links, Vh, lidx, U);
+  // this site's link of this hop, from the block's shared-memory copy [vector][site]
+#pragma unroll
+  for (int v = 0; v < R / GN; v++) {
+    typename GV<T, R>::vec q = lk[v * MRHS_SITES];
+    vec_get(q, U + v * GN);
+  }
+  if (R == 12) recon_row2<T>(U);
 #pragma unroll
   for (int v = 0; v < Lay<T>::NSV; v++) {
     vec q = sm[v * MRHS_MAXT];
@@ -294,28 +307,42 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsStage<T, R>::MINB) dslash_mrhs_
   constexpr int HPR = MrhsStage<T, R>::HPR > 0 ? MrhsStage<T, R>::HPR : 1, NR = 8 / HPR, NSV = Lay<T>::NSV;
   extern __shared__ __align__(16) unsigned char mrhs_smem[];
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  typedef typename GV<T, R>::vec gvec;
+  constexpr int NGV = R / GV<T, R>::N;
   __shared__ vec cl_sm[EPI >= 1 ? Lay<T>::NCV * MRHS_SITES : 1];
-  if (EPI >= 1) {
-    stage_clover_block<T>(cl_sm, a.cl, a.lat.Vh, blockIdx.x * blockDim.x);
-    __syncthreads();
-  }
-  if (idx >= a.lat.Vh) return;
+  __shared__ gvec lk_sm[8 * NGV * MRHS_SITES];  // the eight links of the block's sites: [hop][vector][site]
   const Lat& L = a.lat;
   const int Vh = L.Vh, par = a.parity;
+  const bool live = idx < Vh;
   const size_t stride = a.stride;
-  const Site s = site_of(L, idx, par);
+  const Site s = site_of(L, live ? idx : 0, par);
   const size_t blk = (size_t)R * Vh;
+  int n[8];
+  {
+    const int i0 = live ? idx : 0;
+    n[0] = neighbour<0, +1>(L, i0, s);
+    n[1] = neighbour<0, -1>(L, i0, s);
+    n[2] = neighbour<1, +1>(L, i0, s);
+    n[3] = neighbour<1, -1>(L, i0, s);
+    n[4] = neighbour<2, +1>(L, i0, s);
+    n[5] = neighbour<2, -1>(L, i0, s);
+    n[6] = neighbour<3, +1>(L, i0, s);
+    n[7] = neighbour<3, -1>(L, i0, s);
+  }
+  // every column of every column group multiplies by the same eight links per site: copied once per block (the column
+  // groups share the work: group y copies hops y, y + G, ...), instead of one L1/L2 read per column
+  if (live) {
+    for (int h = threadIdx.y; h < 8; h += blockDim.y) {
+      const gvec* gp = reinterpret_cast<const gvec*>(a.gauge + ((h >> 1) * 2 + ((h & 1) ? 1 - par : par)) * blk) + ((h & 1) ? n[h] : idx);
+#pragma unroll
+      for (int v = 0; v < NGV; v++) lk_sm[(h * NGV + v) * MRHS_SITES + threadIdx.x] = ld_stream(gp + (size_t)v * Vh);
+    }
+  }
+  if (EPI >= 1) stage_clover_block<T>(cl_sm, a.cl, Vh, blockIdx.x * blockDim.x);
+  __syncthreads();
+  if (!live) return;
   // shared memory [buffer][hop of the round][vector][thread]
   vec* sm = reinterpret_cast<vec*>(mrhs_smem) + threadIdx.y * MRHS_SITES + threadIdx.x;
-  int n[8];
-  n[0] = neighbour<0, +1>(L, idx, s);
-  n[1] = neighbour<0, -1>(L, idx, s);
-  n[2] = neighbour<1, +1>(L, idx, s);
-  n[3] = neighbour<1, -1>(L, idx, s);
-  n[4] = neighbour<2, +1>(L, idx, s);
-  n[5] = neighbour<2, -1>(L, idx, s);
-  n[6] = neighbour<3, +1>(L, idx, s);
-  n[7] = neighbour<3, -1>(L, idx, s);
   const bool anti = L.tb < 0;
   const T wf = (anti && s.t == L.Lt - 1) ? (T)-1 : (T)1, wb = (anti && s.t == 0) ? (T)-1 : (T)1;
   // copies of round rnd (hops rnd*HPR ...) of column `col` into buffer rnd & 1
@@ -349,14 +376,14 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsStage<T, R>::MINB) dslash_mrhs_
         const int H = rnd * HPR + k;
         const vec* b = sm + (size_t)((rnd & 1) * HPR + k) * NSV * MRHS_MAXT;
         switch (H) {
-          case 0: hop_mrhs_staged<T, R, 0, true, DAG>(acc[0], b, a.gauge + (0 * 2 + par) * blk, Vh, idx, a.ws); break;
-          case 1: hop_mrhs_staged<T, R, 0, false, DAG>(acc[0], b, a.gauge + (0 * 2 + 1 - par) * blk, Vh, n[1], a.ws); break;
-          case 2: hop_mrhs_staged<T, R, 1, true, DAG>(acc[0], b, a.gauge + (1 * 2 + par) * blk, Vh, idx, a.ws); break;
-          case 3: hop_mrhs_staged<T, R, 1, false, DAG>(acc[0], b, a.gauge + (1 * 2 + 1 - par) * blk, Vh, n[3], a.ws); break;
-          case 4: hop_mrhs_staged<T, R, 2, true, DAG>(acc[0], b, a.gauge + (2 * 2 + par) * blk, Vh, idx, a.ws); break;
-          case 5: hop_mrhs_staged<T, R, 2, false, DAG>(acc[0], b, a.gauge + (2 * 2 + 1 - par) * blk, Vh, n[5], a.ws); break;
-          case 6: hop_mrhs_staged<T, R, 3, true, DAG>(acc[0], b, a.gauge + (3 * 2 + par) * blk, Vh, idx, wf); break;
-          default: hop_mrhs_staged<T, R, 3, false, DAG>(acc[0], b, a.gauge + (3 * 2 + 1 - par) * blk, Vh, n[7], wb); break;
+          case 0: hop_mrhs_staged<T, R, 0, true, DAG>(acc[0], b, lk_sm + 0 * NGV * MRHS_SITES + threadIdx.x, a.ws); break;
+          case 1: hop_mrhs_staged<T, R, 0, false, DAG>(acc[0], b, lk_sm + 1 * NGV * MRHS_SITES + threadIdx.x, a.ws); break;
+          case 2: hop_mrhs_staged<T, R, 1, true, DAG>(acc[0], b, lk_sm + 2 * NGV * MRHS_SITES + threadIdx.x, a.ws); break;
+          case 3: hop_mrhs_staged<T, R, 1, false, DAG>(acc[0], b, lk_sm + 3 * NGV * MRHS_SITES + threadIdx.x, a.ws); break;
+          case 4: hop_mrhs_staged<T, R, 2, true, DAG>(acc[0], b, lk_sm + 4 * NGV * MRHS_SITES + threadIdx.x, a.ws); break;
+          case 5: hop_mrhs_staged<T, R, 2, false, DAG>(acc[0], b, lk_sm + 5 * NGV * MRHS_SITES + threadIdx.x, a.ws); break;
+          case 6: hop_mrhs_staged<T, R, 3, true, DAG>(acc[0], b, lk_sm + 6 * NGV * MRHS_SITES + threadIdx.x, wf); break;
+          default: hop_mrhs_staged<T, R, 3, false, DAG>(acc[0], b, lk_sm + 7 * NGV * MRHS_SITES + threadIdx.x, wb); break;
         }
       }
     }
@@ -416,17 +443,26 @@ static void launch_mrhs_epi(MrhsArgs<T> a, int epi, int nrhs, cudaStream_t st) {
   a.ngroups = nrhs / NB;
   const dim3 block(MRHS_SITES, a.ngroups < MRHS_GMAX ? a.ngroups : MRHS_GMAX);
   const int grid = (a.lat.Vh + MRHS_SITES - 1) / MRHS_SITES;
+  const size_t smem = (size_t)8 * R * sizeof(T) * MRHS_SITES;  // the block's links
+  static bool configured = false;  // one flag per (T, R, DAG, NB) instantiation; the clover rows are static shared memory on top
+  if (!configured && smem + 72 * sizeof(T) * MRHS_SITES > 40 * 1024) {
+    cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 0, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 1, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 2, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 3, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  }
+  configured = true;
   switch (epi) {
-    case 0: dslash_mrhs_kernel<T, R, DAG, 0, NB><<<grid, block, 0, st>>>(a); break;
-    case 1: dslash_mrhs_kernel<T, R, DAG, 1, NB><<<grid, block, 0, st>>>(a); break;
-    case 2: dslash_mrhs_kernel<T, R, DAG, 2, NB><<<grid, block, 0, st>>>(a); break;
-    default: dslash_mrhs_kernel<T, R, DAG, 3, NB><<<grid, block, 0, st>>>(a); break;
+    case 0: dslash_mrhs_kernel<T, R, DAG, 0, NB><<<grid, block, smem, st>>>(a); break;
+    case 1: dslash_mrhs_kernel<T, R, DAG, 1, NB><<<grid, block, smem, st>>>(a); break;
+    case 2: dslash_mrhs_kernel<T, R, DAG, 2, NB><<<grid, block, smem, st>>>(a); break;
+    default: dslash_mrhs_kernel<T, R, DAG, 3, NB><<<grid, block, smem, st>>>(a); break;
   }
 }
 
 template <typename T, int R, bool DAG>
 static void launch_mrhs_nb(const MrhsArgs<T>& a, int epi, int nrhs, cudaStream_t st) {
-  if (MrhsStage<T, R>::HPR > 0) {
+  if constexpr (MrhsStage<T, R>::HPR > 0) {
     launch_mrhs_staged<T, R, DAG>(a, epi, nrhs, st);
     return;
   }
