@@ -149,7 +149,7 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kern
   typedef typename GV<T, R>::vec gvec;
   constexpr int NGV = R / GV<T, R>::N;
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  __shared__ typename V16<T>::vec cl_sm[EPI >= 1 ? Lay<T>::NCV * MRHS_SITES : 1];
+  __shared__ typename V16<T>::vec cl_sm[(EPI >= 1 && EPI != 6) ? Lay<T>::NCV * MRHS_SITES : 1];
   extern __shared__ __align__(16) unsigned char mrhs_lk_smem[];  // the eight links of the block's sites: [hop][vector][site]
   gvec* lk_sm = reinterpret_cast<gvec*>(mrhs_lk_smem);
   const Lat& L = a.lat;
@@ -178,7 +178,7 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kern
       for (int v = 0; v < NGV; v++) lk_sm[(h * NGV + v) * MRHS_SITES + threadIdx.x] = ld_stream(gp + (size_t)v * Vh);
     }
   }
-  if (EPI >= 1) stage_clover_block<T>(cl_sm, a.cl, Vh, blockIdx.x * blockDim.x);
+  if (EPI >= 1 && EPI != 6) stage_clover_block<T>(cl_sm, a.cl, Vh, blockIdx.x * blockDim.x);
   __syncthreads();
   if (!live) return;
   for (int g = threadIdx.y; g < a.ngroups; g += blockDim.y) {
@@ -208,6 +208,15 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kern
 #pragma unroll
       for (int e = 0; e < 24; e++) acc[r][e] *= a.scale;
       store_spinor<T>(out + r * stride, Vh, idx, acc[r]);
+    }
+  } else if (EPI == 6) {  // out = x + scale * d (dslash.cu epilogue 6: the hop without a clover factor of the symmetric forms)
+#pragma unroll
+    for (int r = 0; r < NB; r++) {
+      T xv[24];
+      load_spinor<T>(a.x + first + r * stride, Vh, idx, xv);
+#pragma unroll
+      for (int e = 0; e < 24; e++) xv[e] += a.scale * acc[r][e];
+      store_spinor<T>(out + r * stride, Vh, idx, xv);
     }
   } else if (EPI == 1) {
     T res[NB][24];
@@ -309,7 +318,7 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsStage<T, R>::MINB) dslash_mrhs_
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   typedef typename GV<T, R>::vec gvec;
   constexpr int NGV = R / GV<T, R>::N;
-  __shared__ vec cl_sm[EPI >= 1 ? Lay<T>::NCV * MRHS_SITES : 1];
+  __shared__ vec cl_sm[(EPI >= 1 && EPI != 6) ? Lay<T>::NCV * MRHS_SITES : 1];
   __shared__ gvec lk_sm[8 * NGV * MRHS_SITES];  // the eight links of the block's sites: [hop][vector][site]
   const Lat& L = a.lat;
   const int Vh = L.Vh, par = a.parity;
@@ -338,7 +347,7 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsStage<T, R>::MINB) dslash_mrhs_
       for (int v = 0; v < NGV; v++) lk_sm[(h * NGV + v) * MRHS_SITES + threadIdx.x] = ld_stream(gp + (size_t)v * Vh);
     }
   }
-  if (EPI >= 1) stage_clover_block<T>(cl_sm, a.cl, Vh, blockIdx.x * blockDim.x);
+  if (EPI >= 1 && EPI != 6) stage_clover_block<T>(cl_sm, a.cl, Vh, blockIdx.x * blockDim.x);
   __syncthreads();
   if (!live) return;
   // shared memory [buffer][hop of the round][vector][thread]
@@ -392,6 +401,12 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsStage<T, R>::MINB) dslash_mrhs_
 #pragma unroll
       for (int e = 0; e < 24; e++) acc[0][e] *= a.scale;
       store_spinor<T>(out, Vh, idx, acc[0]);
+    } else if (EPI == 6) {
+      T xv[24];
+      load_spinor<T>(a.x + first, Vh, idx, xv);
+#pragma unroll
+      for (int e = 0; e < 24; e++) xv[e] += a.scale * acc[0][e];
+      store_spinor<T>(out, Vh, idx, xv);
     } else if (EPI == 1) {
       T res[1][24];
       clover_mul_mrhs<T, 1>(cl_sm, acc, res);
@@ -428,13 +443,15 @@ static void launch_mrhs_staged(MrhsArgs<T> a, int epi, int nrhs, cudaStream_t st
     cudaFuncSetAttribute(dslash_mrhs_staged_kernel<T, R, DAG, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_mrhs_staged_kernel<T, R, DAG, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_mrhs_staged_kernel<T, R, DAG, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_mrhs_staged_kernel<T, R, DAG, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   }
   configured = true;
   switch (epi) {
     case 0: dslash_mrhs_staged_kernel<T, R, DAG, 0><<<grid, block, smem, st>>>(a); break;
     case 1: dslash_mrhs_staged_kernel<T, R, DAG, 1><<<grid, block, smem, st>>>(a); break;
     case 2: dslash_mrhs_staged_kernel<T, R, DAG, 2><<<grid, block, smem, st>>>(a); break;
-    default: dslash_mrhs_staged_kernel<T, R, DAG, 3><<<grid, block, smem, st>>>(a); break;
+    case 3: dslash_mrhs_staged_kernel<T, R, DAG, 3><<<grid, block, smem, st>>>(a); break;
+    default: dslash_mrhs_staged_kernel<T, R, DAG, 6><<<grid, block, smem, st>>>(a); break;
   }
 }
 
@@ -450,13 +467,15 @@ static void launch_mrhs_epi(MrhsArgs<T> a, int epi, int nrhs, cudaStream_t st) {
     cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 1, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 2, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 3, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 6, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   }
   configured = true;
   switch (epi) {
     case 0: dslash_mrhs_kernel<T, R, DAG, 0, NB><<<grid, block, smem, st>>>(a); break;
     case 1: dslash_mrhs_kernel<T, R, DAG, 1, NB><<<grid, block, smem, st>>>(a); break;
     case 2: dslash_mrhs_kernel<T, R, DAG, 2, NB><<<grid, block, smem, st>>>(a); break;
-    default: dslash_mrhs_kernel<T, R, DAG, 3, NB><<<grid, block, smem, st>>>(a); break;
+    case 3: dslash_mrhs_kernel<T, R, DAG, 3, NB><<<grid, block, smem, st>>>(a); break;
+    default: dslash_mrhs_kernel<T, R, DAG, 6, NB><<<grid, block, smem, st>>>(a); break;
   }
 }
 
@@ -499,11 +518,11 @@ static void launch_mrhs_typed(lqcd_ctx* c, void* out, const void* in, const void
 int lqcd_dslash_mrhs_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
                             int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st) {
   const double bytes = (double)c->lat.Vh * c->prec *
-                       (8.0 * c->recon + nrhs * 48.0 + (epi >= 1 ? 72.0 : 0.0) + (epi >= 2 ? nrhs * 24.0 : 0.0));
+                       (8.0 * c->recon + nrhs * 48.0 + (epi >= 1 && epi != 6 ? 72.0 : 0.0) + (epi >= 2 ? nrhs * 24.0 : 0.0));
   c->alg_bytes += bytes;
   const bool rec = c->prof_on && c->prof_n < c->prof_cap;
   if (rec) cudaEventRecord(c->prof_ev[2 * c->prof_n], st);
-  if (lqcd_mrhs_tiled_ok(c)) lqcd_dslash_mrhs_tiled_launch(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st);
+  if (lqcd_mrhs_tiled_ok(c) && epi <= 3) lqcd_dslash_mrhs_tiled_launch(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st);
   else if (c->prec == 4) launch_mrhs_typed<float>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st);
   else launch_mrhs_typed<double>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st);
   if (rec) {

@@ -57,10 +57,7 @@ static int mpc_apply(lqcd_ctx* c, void* out, const void* in, const void* gauge, 
     }
     if ((rc = lqcd_clover_apply_launch(c, out, in, Ai_e, nrhs, st))) return rc;
     if ((rc = lqcd_dslash_launch(c, tmp, out, gauge, Ai_o, nullptr, 1, 1.0, 0, 1, nrhs, st))) return rc;
-    if (nrhs == 1) return lqcd_dslash_launch(c, out, tmp, gauge, nullptr, in, 0, k2, 0, 6, 1, st);
-    if ((rc = lqcd_dslash_launch(c, out, tmp, gauge, nullptr, nullptr, 0, k2, 0, 0, nrhs, st))) return rc;
-    void* v[2] = {(void*)in, out};
-    return BLAS_CALL(c, OpXpay, op.a = 1.0, v, nullptr, nrhs, 0, st);  // out = in + 1*out
+    return lqcd_dslash_launch(c, out, tmp, gauge, nullptr, in, 0, k2, 0, 6, nrhs, st);
   }
   if (!dagger) {
     if ((rc = lqcd_dslash_launch(c, tmp, in, gauge, Ai_o, nullptr, 1, 1.0, 0, 1, nrhs, st))) return rc;
@@ -68,11 +65,7 @@ static int mpc_apply(lqcd_ctx* c, void* out, const void* in, const void* gauge, 
   }
   if ((rc = lqcd_clover_apply_launch(c, out, in, Ai_e, nrhs, st))) return rc;
   if ((rc = lqcd_dslash_launch(c, tmp, out, gauge, Ai_o, nullptr, 1, 1.0, 1, 1, nrhs, st))) return rc;
-  if (nrhs == 1) return lqcd_dslash_launch(c, out, tmp, gauge, nullptr, in, 0, k2, 1, 6, 1, st);  // out = in + k2 D^dag_eo tmp
-  // multi-RHS kernels have no epilogue 6: plain dslash into `out` followed by an xpay
-  if ((rc = lqcd_dslash_launch(c, out, tmp, gauge, nullptr, nullptr, 0, k2, 1, 0, nrhs, st))) return rc;
-  void* v[2] = {(void*)in, out};
-  return BLAS_CALL(c, OpXpay, op.a = 1.0, v, nullptr, nrhs, 0, st);  // out = in + 1*out
+  return lqcd_dslash_launch(c, out, tmp, gauge, nullptr, in, 0, k2, 1, 6, nrhs, st);  // out = in + k2 D^dag_eo tmp
 }
 
 // full M (O7): out_p = A_pp in_p - kappa D_{p,1-p} in_{1-p}; fields are [parity][nrhs][one-parity]

@@ -212,9 +212,8 @@ def test_propagator_sharded_single_rank_equals_propagator():
 @pytest.mark.parametrize("solver", ["cgne", "bicgstab"])
 @pytest.mark.parametrize("matpc", [1, 2])
 def test_invert_multi_symmetric_forms_config2(solver, matpc):
-    """Batched solves on the symmetric Schur complements (left and right; the multi-RHS kernels have no epilogue 6, so
-    the clover-first products go through the generic path): every column meets reading A17 and equals the column's
-    own single solve."""
+    """Batched solves on the symmetric Schur complements (left and right; multi-RHS epilogue 6 and the batched clover
+    apply for the clover-first products): every column meets reading A17 and equals the column's own single solve."""
     s, c = from_cfg(2, 8, 18)
     dims = c["dims"]
     bs = [synth.source(dims, "point", spin=1, colour=2), synth.source(dims, "z2", 102), synth.source(dims, "gaussian", 5)]
