@@ -51,9 +51,7 @@ def lib():
         L.orc_clover_defect.restype = cd
         L.orc_clover_defect.argtypes = [vp]
         L.orc_get_clover.argtypes = [vp, vp, vp]
-        L.orc_put_clover.argtypes = [vp, cd, vp, vp]
         L.orc_clover_dense.argtypes = [vp, cd, cd, vp]
-        L.orc_clover_dense_site.argtypes = [vp, cd, cd, cl, vp]
         L.orc_fmunu.argtypes = [vp, ci, ci, vp]
         L.orc_dslash.argtypes = [vp, vp, vp, ci, ci]
         L.orc_dslash_site.argtypes = [vp, vp, cl, ci, vp]
@@ -143,20 +141,9 @@ class Oracle:
         lib().orc_get_clover(self._h, A.ctypes.data, Ai.ctypes.data)
         return A, Ai
 
-    def put_clover(self, kappa, A, Ainv):
-        A = np.ascontiguousarray(A, dtype=np.float64)
-        Ainv = np.ascontiguousarray(Ainv, dtype=np.float64)
-        lib().orc_put_clover(self._h, float(kappa), A.ctypes.data, Ainv.ctypes.data)
-
     def clover_dense(self, kappa, csw):
         out = np.empty(self.site_shape + (12, 12), dtype=np.complex128)
         lib().orc_clover_dense(self._h, float(kappa), float(csw), out.ctypes.data)
-        return out
-
-    def clover_dense_site(self, kappa, csw, public_index):
-        out = np.empty((12, 12), dtype=np.complex128)
-        lib().orc_clover_dense_site(self._h, float(kappa), float(csw), int(public_index),
-                                    out.ctypes.data)
         return out
 
     def fmunu(self, mu, nu):

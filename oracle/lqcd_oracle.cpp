@@ -703,19 +703,6 @@ void orc_get_clover(void* h, double* A_public, double* Ainv_public) {
     if (Ainv_public) std::memcpy(Ainv_public + c * 72, P.Ainv.data() + l * 72, sizeof(double) * 72);
   }
 }
-// load packed clover fields (e.g. produced elsewhere) instead of building them
-void orc_put_clover(void* h, double kappa, const double* A_public, const double* Ainv_public) {
-  Problem& P = *static_cast<Problem*>(h);
-  P.kappa = kappa;
-  P.A.resize((size_t)P.g.V * 72);
-  P.Ainv.resize((size_t)P.g.V * 72);
-  for (long l = 0; l < P.g.V; l++) {
-    long c = P.g.cb(l);
-    std::memcpy(P.A.data() + l * 72, A_public + c * 72, sizeof(double) * 72);
-    std::memcpy(P.Ainv.data() + l * 72, Ainv_public + c * 72, sizeof(double) * 72);
-  }
-}
-
 // dense 12x12 clover matrices for every site, public site order: [2][Vh][12][12] complex
 void orc_clover_dense(void* h, double kappa, double csw, double* out) {
   Problem& P = *static_cast<Problem*>(h);
@@ -723,14 +710,6 @@ void orc_clover_dense(void* h, double kappa, double csw, double* out) {
 #pragma omp parallel for schedule(static)
   for (long l = 0; l < P.g.V; l++) clover_dense_site(P.g, P.U.data(), l, kappa, csw, csw, o + P.g.cb(l) * 144);
 }
-// dense clover at ONE site given by its public index (parity*Vh + cb); for sampled checks at size
-void orc_clover_dense_site(void* h, double kappa, double csw, long public_index, double* out) {
-  Problem& P = *static_cast<Problem*>(h);
-  long par = public_index / P.g.Vh, c = public_index % P.g.Vh;
-  for (long l = 2 * c; l < 2 * c + 2; l++)
-    if (P.g.parity(l) == par) clover_dense_site(P.g, P.U.data(), l, kappa, csw, csw, reinterpret_cast<cplx*>(out));
-}
-
 // F_{mu nu}(x) for all sites: [2][Vh][3][3] complex
 void orc_fmunu(void* h, int mu, int nu, double* out) {
   Problem& P = *static_cast<Problem*>(h);

@@ -32,6 +32,14 @@ __device__ __forceinline__ cplxd cdiv(cplxd a, cplxd b) {
   return {(a.re * b.re + a.im * b.im) / d, (a.im * b.re - a.re * b.im) / d};
 }
 
+// omega = <t,s>/<t,t> of BiCGStab from slots ts..ts+2; t = 0 happens when the half step s = r - alpha v already
+// solved the system (s = 0, "lucky breakdown"): omega = 0 then, so x += alpha p and r = s = 0, not 0/0
+__device__ __forceinline__ cplxd bicg_omega(const double* s, int ts) {
+  const double tt = s[ts + 2];
+  if (!(tt > 0.0)) return {0.0, 0.0};
+  return {s[ts] / tt, s[ts + 1] / tt};
+}
+
 template <int NR>
 __device__ __forceinline__ void block_reduce_finish(double* acc, double* partial, int max_blocks, unsigned int* ticket,
                                                     double* scalars, const int* out_slots) {
@@ -172,6 +180,17 @@ template <typename T> struct OpXpay {  // v0 = x, v1 = y ; y = x + a y (a real, 
     w[1][1] = w[0][1] + (T)a * w[1][1];
   }
 };
+template <typename T> struct OpXpayNorm {  // v0 = x, v1 = y ; y = x + a y (a real, host) ; out0 = |y|^2
+  static constexpr int NV = 2, NR = 1;
+  static constexpr unsigned LOAD = 3, STORE = 2;
+  double a;
+  __device__ void init(const double*) {}
+  __device__ void elem(T (*w)[2], double* acc) {
+    w[1][0] = w[0][0] + (T)a * w[1][0];
+    w[1][1] = w[0][1] + (T)a * w[1][1];
+    acc[0] += (double)w[1][0] * w[1][0] + (double)w[1][1] * w[1][1];
+  }
+};
 template <typename T> struct OpCaxpbypz {  // v0 = x, v1 = y, v2 = z ; z += a x + b y (complex, host)
   static constexpr int NV = 3, NR = 0;
   static constexpr unsigned LOAD = 7, STORE = 4;
@@ -247,7 +266,7 @@ template <typename T> struct OpBicgP {
   __device__ void init(const double* s) {
     first = s[S_FIRST] != 0.0;
     if (first) { beta = {0, 0}; omega = {0, 0}; return; }
-    omega = {s[ts] / s[ts + 2], s[ts + 1] / s[ts + 2]};
+    omega = bicg_omega(s, ts);
     beta = cdiv(cdiv({s[rho], s[rho + 1]}, {s[r0v], s[r0v + 1]}), omega);
   }
   __device__ void elem(T (*w)[2], double*) {
@@ -284,7 +303,7 @@ template <typename T> struct OpBicgXR {
   cplxd alpha, omega;
   __device__ void init(const double* s) {
     alpha = cdiv({s[rho], s[rho + 1]}, {s[r0v], s[r0v + 1]});
-    omega = {s[ts] / s[ts + 2], s[ts + 1] / s[ts + 2]};
+    omega = bicg_omega(s, ts);
   }
   __device__ void elem(T (*w)[2], double* acc) {
     const T ar = (T)alpha.re, ai = (T)alpha.im, orr = (T)omega.re, oi = (T)omega.im;

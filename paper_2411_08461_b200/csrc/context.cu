@@ -52,7 +52,7 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], int prec, int recon, int t_bo
   }
   if (V / 2 > 0x3fffffffL) return LQCD_ERR_DIMS;  // 32-bit site indices inside kernels
   int ndev = 0;
-  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev || device >= LQCD_MAX_DEVICES) {
     cudaGetLastError();
     return LQCD_ERR_CUDA;  // no CPU fallback: without a device the library does nothing
   }

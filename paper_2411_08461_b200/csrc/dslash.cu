@@ -34,7 +34,6 @@ template <typename T> struct DslashArgs {
   double* partial;
   double* scalars;
   int num, den;
-  int remap;  // 0: block = consecutive sites; 4 / 8: block = 2 x 2 (x 2) brick of x-rows (dslash_kernel)
 };
 
 // Launch shape per precision (threads per block, minimum resident blocks per SM = register budget).
@@ -52,38 +51,16 @@ template <typename T> struct DslashArgs {
 #ifndef DSLASH_MINB_F64
 #define DSLASH_MINB_F64 5
 #endif
-#ifndef DSLASH_STAGE_F32
-#define DSLASH_STAGE_F32 0
-#endif
-#ifndef DSLASH_STAGE_F64
-#define DSLASH_STAGE_F64 0
-#endif
 #ifndef DSLASH_STAGE_F64_R12
 #define DSLASH_STAGE_F64_R12 1  // cp.async link staging pays for fp64 12-real links only (profiles/r01_tuning.md)
 #endif
 #ifndef DSLASH_MINB_F64_R12
 #define DSLASH_MINB_F64_R12 4
 #endif
-// spinor staging (dslash.cuh): 0 = off, 1 = all eight hops per round, 2 = four and four
-#ifndef DSLASH_SSTAGE_F32
-#define DSLASH_SSTAGE_F32 0
-#endif
-#ifndef DSLASH_SSTAGE_F64
-#define DSLASH_SSTAGE_F64 0
-#endif
-template <typename T> struct SStage;
-template <> struct SStage<float> { static constexpr int ROUNDS = DSLASH_SSTAGE_F32; };
-template <> struct SStage<double> { static constexpr int ROUNDS = DSLASH_SSTAGE_F64; };
 template <typename T, int R> struct Tune;
-#ifndef DSLASH_STAGE_F32_R12
-#define DSLASH_STAGE_F32_R12 0
-#endif
-#ifndef DSLASH_MINB_F32_R12
-#define DSLASH_MINB_F32_R12 DSLASH_MINB_F32
-#endif
-template <> struct Tune<float, 18> { static constexpr int BLOCK = DSLASH_BLOCK_F32, MINB = DSLASH_MINB_F32; static constexpr bool STAGE = DSLASH_STAGE_F32; };
-template <> struct Tune<float, 12> { static constexpr int BLOCK = DSLASH_BLOCK_F32, MINB = DSLASH_MINB_F32_R12; static constexpr bool STAGE = DSLASH_STAGE_F32_R12; };
-template <> struct Tune<double, 18> { static constexpr int BLOCK = DSLASH_BLOCK_F64, MINB = DSLASH_MINB_F64; static constexpr bool STAGE = DSLASH_STAGE_F64; };
+template <> struct Tune<float, 18> { static constexpr int BLOCK = DSLASH_BLOCK_F32, MINB = DSLASH_MINB_F32; static constexpr bool STAGE = false; };
+template <> struct Tune<float, 12> { static constexpr int BLOCK = DSLASH_BLOCK_F32, MINB = DSLASH_MINB_F32; static constexpr bool STAGE = false; };
+template <> struct Tune<double, 18> { static constexpr int BLOCK = DSLASH_BLOCK_F64, MINB = DSLASH_MINB_F64; static constexpr bool STAGE = false; };
 template <> struct Tune<double, 12> { static constexpr int BLOCK = DSLASH_BLOCK_F64, MINB = DSLASH_MINB_F64_R12; static constexpr bool STAGE = DSLASH_STAGE_F64_R12; };
 
 // Deterministic fp64 grid reduction of the fused epilogues: block sum -> partial[block] (no fence, no
@@ -187,31 +164,13 @@ __device__ __forceinline__ void dslash_epilogue(const DslashArgs<T>& a, int idx,
 
 template <typename T, int R, bool DAG, int EPI>
 __global__ void __launch_bounds__(Tune<T, R>::BLOCK, Tune<T, R>::MINB) dslash_kernel(const DslashArgs<T> a) {
-  int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  if (a.remap) {
-    // compact block: the block's x-rows form a 2 x 2 (x 2) brick in (y, z, t) instead of 4 (8) consecutive y-rows,
-    // so more of the +-y, +-z, +-t neighbour rows are shared inside the block (L1); a warp still reads whole x-rows
-    const Lat& L = a.lat;
-    const int xh = threadIdx.x % L.Lxh, r = threadIdx.x / L.Lxh;
-    const int nby = L.Ly >> 1, nbz = L.Lz >> 1;
-    int b = blockIdx.x;
-    const int y = 2 * (b % nby) + (r & 1);
-    b /= nby;
-    const int z = 2 * (b % nbz) + ((r >> 1) & 1);
-    b /= nbz;
-    const int t = a.remap == 8 ? 2 * b + (r >> 2) : b;
-    idx = xh + L.Lxh * (y + L.Ly * (z + L.Lz * t));
-  }
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   const bool live = idx < a.lat.Vh;
   if (!epi_reduces(EPI) && !live) return;
   double local = 0;
   if (live) {
     T acc[24];
-    if (SStage<T>::ROUNDS > 0) {
-      extern __shared__ __align__(16) unsigned char dslash_smem[];
-      dslash_site_sstaged<T, R, DAG, Tune<T, R>::BLOCK, (SStage<T>::ROUNDS > 0 ? SStage<T>::ROUNDS : 1)>(
-          acc, a.in, a.gauge, a.lat, idx, a.parity, dslash_smem, a.ws);
-    } else if (Tune<T, R>::STAGE) {
+    if (Tune<T, R>::STAGE) {
       extern __shared__ __align__(16) unsigned char dslash_smem[];
       dslash_site_staged<T, R, DAG, Tune<T, R>::BLOCK>(acc, a.in, a.gauge, a.lat, idx, a.parity, dslash_smem, a.ws);
     } else {
@@ -222,15 +181,22 @@ __global__ void __launch_bounds__(Tune<T, R>::BLOCK, Tune<T, R>::MINB) dslash_ke
   if (epi_reduces(EPI)) dslash_reduce<Tune<T, R>::BLOCK>(local, a.partial);
 }
 
+// in and out may alias (lqcd.h: lqcd_clover_apply; the solvers apply A_ee^-1 in place): no __restrict__ and plain
+// (coherent) loads on `in`; a thread reads its whole site before it stores
 template <typename T>
-__global__ void __launch_bounds__(128) clover_apply_kernel(T* __restrict__ out, const T* __restrict__ in,
-                                                           const T* __restrict__ cl, int Vh) {
+__global__ void __launch_bounds__(128) clover_apply_kernel(T* out, const T* in, const T* __restrict__ cl, int Vh) {
+  typedef typename V16<T>::vec vec;
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= Vh) return;
   out += (size_t)blockIdx.y * 24 * Vh;  // right-hand side
   in += (size_t)blockIdx.y * 24 * Vh;
   T v[24], r[24];
-  load_spinor<T>(in, Vh, idx, v);
+  const vec* p = reinterpret_cast<const vec*>(in) + idx;
+#pragma unroll
+  for (int q = 0; q < Lay<T>::NSV; q++) {
+    const vec w = p[(size_t)q * Vh];
+    vec_get(w, v + q * V16<T>::N);
+  }
   clover_mul<T>(cl, Vh, idx, v, r);
   store_spinor<T>(out, Vh, idx, r);
 }
@@ -314,18 +280,18 @@ int lqcd_dslash_grid(const lqcd_ctx* c) {
 }
 
 template <typename T, int R, bool DAG>
-static void launch_tiled(const DslashArgs<T>& a, int epi, cudaStream_t st) {
+static void launch_tiled(const DslashArgs<T>& a, int epi, int device, cudaStream_t st) {
   typedef typename TileOf<T>::TS TS;
   const int grid = a.lat.Vh / TS::NOUT;
   const size_t smem = (size_t)TS::NSLOT * 24 * sizeof(T);
-  static bool configured = false;  // one flag per (T, R, DAG) instantiation
-  if (!configured) {
+  static bool configured[LQCD_MAX_DEVICES] = {};  // per (T, R, DAG) instantiation and device
+  if (!configured[device]) {
     cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_tiled_kernel<T, R, DAG, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    configured = true;
+    configured[device] = true;
   }
   switch (epi) {
     case 0: dslash_tiled_kernel<T, R, DAG, 0><<<grid, TS::NOUT, smem, st>>>(a); break;
@@ -336,21 +302,13 @@ static void launch_tiled(const DslashArgs<T>& a, int epi, cudaStream_t st) {
   }
 }
 
-#ifndef DSLASH_REMAP
-#define DSLASH_REMAP 0
-#endif
 template <typename T, int R, bool DAG>
-static void launch_epi(DslashArgs<T> a, int epi, cudaStream_t st) {
+static void launch_epi(const DslashArgs<T>& a, int epi, int device, cudaStream_t st) {
   const int block = Tune<T, R>::BLOCK;
-  {
-    const int rows = block % a.lat.Lxh == 0 ? block / a.lat.Lxh : 0;
-    a.remap = (DSLASH_REMAP && (rows == 4 || rows == 8) && a.lat.Vh % block == 0) ? rows : 0;
-  }
   const int grid = (a.lat.Vh + block - 1) / block;
-  const size_t smem = SStage<T>::ROUNDS > 0 ? (size_t)(8 / SStage<T>::ROUNDS) * 24 * sizeof(T) * block  // spinors
-                      : Tune<T, R>::STAGE ? (size_t)8 * R * sizeof(T) * block : 0;                      // eight links per thread
-  static bool configured = false;  // one flag per (T, R, DAG) instantiation
-  if (!configured && smem > 40 * 1024) {  // the epilogues that reduce add static shared memory on top of `smem`
+  const size_t smem = Tune<T, R>::STAGE ? (size_t)8 * R * sizeof(T) * block : 0;  // eight links per thread
+  static bool configured[LQCD_MAX_DEVICES] = {};  // per (T, R, DAG) instantiation and device: the attribute is per device
+  if (!configured[device] && smem > 40 * 1024) {  // the epilogues that reduce add static shared memory on top of `smem`
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -363,7 +321,7 @@ static void launch_epi(DslashArgs<T> a, int epi, cudaStream_t st) {
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 9>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 10>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   }
-  configured = true;
+  configured[device] = true;
   switch (epi) {
     case 0: dslash_kernel<T, R, DAG, 0><<<grid, block, smem, st>>>(a); break;
     case 1: dslash_kernel<T, R, DAG, 1><<<grid, block, smem, st>>>(a); break;
@@ -389,7 +347,6 @@ static void launch_typed(lqcd_ctx* c, void* out, const void* in, const void* gau
   a.scalars = c->d_scalars;
   a.num = f ? f->num : 0;
   a.den = f ? f->den : 0;
-  a.remap = 0;
   a.out = (T*)out;
   a.in = (const T*)in;
   a.gauge = (const T*)gauge;
@@ -401,20 +358,20 @@ static void launch_typed(lqcd_ctx* c, void* out, const void* in, const void* gau
   a.ws = (T)c->ws;
   if (lqcd_dslash_tiled(c) && (epi <= 3 || epi == 6)) {  // the tiled form exists for the epilogues without a reduction
     if (c->recon == 18) {
-      if (dagger) launch_tiled<T, 18, true>(a, epi, st);
-      else launch_tiled<T, 18, false>(a, epi, st);
+      if (dagger) launch_tiled<T, 18, true>(a, epi, c->device, st);
+      else launch_tiled<T, 18, false>(a, epi, c->device, st);
     } else {
-      if (dagger) launch_tiled<T, 12, true>(a, epi, st);
-      else launch_tiled<T, 12, false>(a, epi, st);
+      if (dagger) launch_tiled<T, 12, true>(a, epi, c->device, st);
+      else launch_tiled<T, 12, false>(a, epi, c->device, st);
     }
     return;
   }
   if (c->recon == 18) {
-    if (dagger) launch_epi<T, 18, true>(a, epi, st);
-    else launch_epi<T, 18, false>(a, epi, st);
+    if (dagger) launch_epi<T, 18, true>(a, epi, c->device, st);
+    else launch_epi<T, 18, false>(a, epi, c->device, st);
   } else {
-    if (dagger) launch_epi<T, 12, true>(a, epi, st);
-    else launch_epi<T, 12, false>(a, epi, st);
+    if (dagger) launch_epi<T, 12, true>(a, epi, c->device, st);
+    else launch_epi<T, 12, false>(a, epi, c->device, st);
   }
 }
 

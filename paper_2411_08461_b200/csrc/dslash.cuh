@@ -308,87 +308,6 @@ __device__ __forceinline__ void dslash_site_staged(T* acc, const T* __restrict__
   hop_staged<T, R, 3, false, DAG, BLOCK, 7>(acc, in, smem, Vh, n7, sb);
 }
 
-// ---------------------------------------------------------------------------------------------
-// Spinor staging through shared memory with cp.async: each thread copies the neighbour spinors of
-// ITS OWN site global->shared asynchronously (16-byte copies, one commit group per hop), HOPS hops
-// per round, so all spinor bytes of a round are in flight without holding registers; the links are
-// ordinary streaming loads, for which the whole register file is then free.  Layout in shared
-// memory: [hop of the round][vector][thread] (conflict free); a thread only reads what it copied.
-// ---------------------------------------------------------------------------------------------
-template <typename T, int BLOCK>
-__device__ __forceinline__ void stage_spinor(void* smem, int slot, const T* __restrict__ in, int Vh, int nidx) {
-  typedef typename V16<T>::vec vec;
-  vec* sl = reinterpret_cast<vec*>(smem) + (size_t)slot * Lay<T>::NSV * BLOCK + threadIdx.x;
-  const vec* g = reinterpret_cast<const vec*>(in) + nidx;
-#pragma unroll
-  for (int v = 0; v < Lay<T>::NSV; v++) cp_async<16>(sl + v * BLOCK, g + (size_t)v * Vh);
-  cp_async_commit();
-}
-template <typename T, int R, int MU, bool FWD, bool DAG, int BLOCK, int SLOT, int PENDING>
-__device__ __forceinline__ void hop_sstaged(T* acc, const void* smem, const T* __restrict__ links, int Vh, int lidx, T bsign) {
-  typedef typename V16<T>::vec vec;
-  constexpr int S = (FWD != DAG) ? -1 : +1;
-  T psi[24], U[18], h[12], chi[12];
-  load_link<T, R>(links, Vh, lidx, U);
-  cp_async_wait<PENDING>();
-  const vec* sl = reinterpret_cast<const vec*>(smem) + (size_t)SLOT * Lay<T>::NSV * BLOCK + threadIdx.x;
-#pragma unroll
-  for (int v = 0; v < Lay<T>::NSV; v++) {
-    vec q = sl[v * BLOCK];
-    vec_get(q, psi + v * V16<T>::N);
-  }
-  project<T, MU, S>(psi, h);
-  su3_mul<T, !FWD>(U, h, chi);
-  reconstruct<T, MU, S>(acc, chi, bsign);
-}
-// ROUNDS = 1: all eight hops staged at once; ROUNDS = 2: four and four (half the shared memory)
-template <typename T, int R, bool DAG, int BLOCK, int ROUNDS>
-__device__ __forceinline__ void dslash_site_sstaged(T* acc, const T* __restrict__ in, const T* __restrict__ gauge,
-                                                    const Lat& L, int idx, int par, void* smem, T ws) {
-  const Site s = site_of(L, idx, par);
-  const int Vh = L.Vh;
-  const size_t blk = (size_t)R * Vh;
-  const int n0 = neighbour<0, +1>(L, idx, s), n1 = neighbour<0, -1>(L, idx, s);
-  const int n2 = neighbour<1, +1>(L, idx, s), n3 = neighbour<1, -1>(L, idx, s);
-  const int n4 = neighbour<2, +1>(L, idx, s), n5 = neighbour<2, -1>(L, idx, s);
-  const int n6 = neighbour<3, +1>(L, idx, s), n7 = neighbour<3, -1>(L, idx, s);
-  const T sf = (L.tb < 0 && s.t == L.Lt - 1) ? (T)-1 : (T)1;
-  const T sb = (L.tb < 0 && s.t == 0) ? (T)-1 : (T)1;
-#pragma unroll
-  for (int e = 0; e < 24; e++) acc[e] = 0;
-  stage_spinor<T, BLOCK>(smem, 0, in, Vh, n0);
-  stage_spinor<T, BLOCK>(smem, 1, in, Vh, n1);
-  stage_spinor<T, BLOCK>(smem, 2, in, Vh, n2);
-  stage_spinor<T, BLOCK>(smem, 3, in, Vh, n3);
-  if (ROUNDS == 1) {
-    stage_spinor<T, BLOCK>(smem, 4, in, Vh, n4);
-    stage_spinor<T, BLOCK>(smem, 5, in, Vh, n5);
-    stage_spinor<T, BLOCK>(smem, 6, in, Vh, n6);
-    stage_spinor<T, BLOCK>(smem, 7, in, Vh, n7);
-    hop_sstaged<T, R, 0, true, DAG, BLOCK, 0, 7>(acc, smem, gauge + (0 * 2 + par) * blk, Vh, idx, ws);
-    hop_sstaged<T, R, 0, false, DAG, BLOCK, 1, 6>(acc, smem, gauge + (0 * 2 + 1 - par) * blk, Vh, n1, ws);
-    hop_sstaged<T, R, 1, true, DAG, BLOCK, 2, 5>(acc, smem, gauge + (1 * 2 + par) * blk, Vh, idx, ws);
-    hop_sstaged<T, R, 1, false, DAG, BLOCK, 3, 4>(acc, smem, gauge + (1 * 2 + 1 - par) * blk, Vh, n3, ws);
-    hop_sstaged<T, R, 2, true, DAG, BLOCK, 4, 3>(acc, smem, gauge + (2 * 2 + par) * blk, Vh, idx, ws);
-    hop_sstaged<T, R, 2, false, DAG, BLOCK, 5, 2>(acc, smem, gauge + (2 * 2 + 1 - par) * blk, Vh, n5, ws);
-    hop_sstaged<T, R, 3, true, DAG, BLOCK, 6, 1>(acc, smem, gauge + (3 * 2 + par) * blk, Vh, idx, sf);
-    hop_sstaged<T, R, 3, false, DAG, BLOCK, 7, 0>(acc, smem, gauge + (3 * 2 + 1 - par) * blk, Vh, n7, sb);
-  } else {
-    hop_sstaged<T, R, 0, true, DAG, BLOCK, 0, 3>(acc, smem, gauge + (0 * 2 + par) * blk, Vh, idx, ws);
-    stage_spinor<T, BLOCK>(smem, 0, in, Vh, n4);  // slot 0 is free again: refill it while hops 1-3 run
-    hop_sstaged<T, R, 0, false, DAG, BLOCK, 1, 3>(acc, smem, gauge + (0 * 2 + 1 - par) * blk, Vh, n1, ws);
-    stage_spinor<T, BLOCK>(smem, 1, in, Vh, n5);
-    hop_sstaged<T, R, 1, true, DAG, BLOCK, 2, 3>(acc, smem, gauge + (1 * 2 + par) * blk, Vh, idx, ws);
-    stage_spinor<T, BLOCK>(smem, 2, in, Vh, n6);
-    hop_sstaged<T, R, 1, false, DAG, BLOCK, 3, 3>(acc, smem, gauge + (1 * 2 + 1 - par) * blk, Vh, n3, ws);
-    stage_spinor<T, BLOCK>(smem, 3, in, Vh, n7);
-    hop_sstaged<T, R, 2, true, DAG, BLOCK, 0, 3>(acc, smem, gauge + (2 * 2 + par) * blk, Vh, idx, ws);
-    hop_sstaged<T, R, 2, false, DAG, BLOCK, 1, 2>(acc, smem, gauge + (2 * 2 + 1 - par) * blk, Vh, n5, ws);
-    hop_sstaged<T, R, 3, true, DAG, BLOCK, 2, 1>(acc, smem, gauge + (3 * 2 + par) * blk, Vh, idx, sf);
-    hop_sstaged<T, R, 3, false, DAG, BLOCK, 3, 0>(acc, smem, gauge + (3 * 2 + 1 - par) * blk, Vh, n7, sb);
-  }
-}
-
 // y = B x for one packed Hermitian 6x6 block (6 real diagonals, 15 complex lower entries), packed fp32:
 // y_i = sum_j ar_ij (xr, xi)_j + (-1, 1) o sum_j (+-ai_ij) (xi, xr)_j  (lower triangle +, conjugated upper -)
 __device__ __forceinline__ void clover_block_packed(const float* a, const float* x, float* y) {
@@ -411,27 +330,13 @@ __device__ __forceinline__ void clover_block_packed(const float* a, const float*
   }
 }
 
-// out = C v for the two Hermitian 6x6 chiral blocks of one site.  cl = one-parity clover field
-// [NCV][Vh]; packed order per block: 6 real diagonal, then 15 complex lower entries row-major.
-// v and out are 24-real spinors (block k acts on reals 12k..12k+11); they must not alias.
+// y = B x for one packed Hermitian 6x6 block a[36] (6 real diagonals, then the 15 complex lower entries row-major);
+// the ONE block multiply of the library: clover apply, every fused epilogue, single and multi right-hand side
 template <typename T>
-__device__ __forceinline__ void clover_mul(const T* __restrict__ cl, int Vh, int idx, const T* v, T* out) {
-  typedef typename V16<T>::vec vec;
-  constexpr int N = V16<T>::N;
-  const vec* p = reinterpret_cast<const vec*>(cl) + idx;
-#pragma unroll
-  for (int k = 0; k < 2; k++) {
-    T a[36];
-#pragma unroll
-    for (int q = 0; q < 36 / N; q++) {
-      vec w = ld_stream(p + (size_t)(k * (36 / N) + q) * Vh);
-      vec_get(w, a + q * N);
-    }
-    const T* x = v + 12 * k;
-    T* y = out + 12 * k;
-    if constexpr (UsePacked<T>::value) {
-      clover_block_packed(a, x, y);
-    } else {
+__device__ __forceinline__ void clover_block(const T* a, const T* x, T* y) {
+  if constexpr (UsePacked<T>::value) {
+    clover_block_packed(a, x, y);
+  } else {
 #pragma unroll
     for (int i = 0; i < 6; i++) {
       T re = a[i] * x[2 * i], im = a[i] * x[2 * i + 1];
@@ -454,7 +359,32 @@ __device__ __forceinline__ void clover_mul(const T* __restrict__ cl, int Vh, int
       y[2 * i] = re;
       y[2 * i + 1] = im;
     }
-    }
+  }
+}
+
+// one chiral block (k = 0 upper, 1 lower) of site idx from a one-parity clover field [NCV][Vh]
+template <typename T>
+__device__ __forceinline__ void load_clover_block(const T* __restrict__ cl, int Vh, int idx, int k, T* a) {
+  typedef typename V16<T>::vec vec;
+  constexpr int N = V16<T>::N;
+  const vec* p = reinterpret_cast<const vec*>(cl) + idx;
+#pragma unroll
+  for (int q = 0; q < 36 / N; q++) {
+    vec w = ld_stream(p + (size_t)(k * (36 / N) + q) * Vh);
+    vec_get(w, a + q * N);
+  }
+}
+
+// out = C v for the two Hermitian 6x6 chiral blocks of one site.  cl = one-parity clover field
+// [NCV][Vh]; packed order per block: 6 real diagonal, then 15 complex lower entries row-major.
+// v and out are 24-real spinors (block k acts on reals 12k..12k+11); they must not alias.
+template <typename T>
+__device__ __forceinline__ void clover_mul(const T* __restrict__ cl, int Vh, int idx, const T* v, T* out) {
+#pragma unroll
+  for (int k = 0; k < 2; k++) {
+    T a[36];
+    load_clover_block<T>(cl, Vh, idx, k, a);
+    clover_block<T>(a, v + 12 * k, out + 12 * k);
   }
 }
 
@@ -463,54 +393,13 @@ __device__ __forceinline__ void clover_mul(const T* __restrict__ cl, int Vh, int
 template <typename T>
 __device__ __forceinline__ void clover_mul_twice(const T* __restrict__ cl, int Vh, int idx, const T* v, const T* x, T scale,
                                                  T* res, T* res2) {
-  typedef typename V16<T>::vec vec;
-  constexpr int N = V16<T>::N;
-  const vec* p = reinterpret_cast<const vec*>(cl) + idx;
 #pragma unroll
   for (int k = 0; k < 2; k++) {
-    T a[36];
+    T a[36], y[12];
+    load_clover_block<T>(cl, Vh, idx, k, a);
+    clover_block<T>(a, v + 12 * k, y);
 #pragma unroll
-    for (int q = 0; q < 36 / N; q++) {
-      vec w = ld_stream(p + (size_t)(k * (36 / N) + q) * Vh);
-      vec_get(w, a + q * N);
-    }
-#pragma unroll
-    for (int pass = 0; pass < 2; pass++) {
-      const T* in = pass == 0 ? v + 12 * k : res + 12 * k;
-      T y[12];
-      if constexpr (UsePacked<T>::value) {
-        clover_block_packed(a, in, y);
-      } else {
-#pragma unroll
-        for (int i = 0; i < 6; i++) {
-          T re = a[i] * in[2 * i], im = a[i] * in[2 * i + 1];
-#pragma unroll
-          for (int j = 0; j < 6; j++) {
-            if (j < i) {
-              const int o = 6 + 2 * (i * (i - 1) / 2 + j);
-              re += a[o] * in[2 * j];
-              re -= a[o + 1] * in[2 * j + 1];
-              im += a[o] * in[2 * j + 1];
-              im += a[o + 1] * in[2 * j];
-            } else if (j > i) {
-              const int o = 6 + 2 * (j * (j - 1) / 2 + i);
-              re += a[o] * in[2 * j];
-              re += a[o + 1] * in[2 * j + 1];
-              im += a[o] * in[2 * j + 1];
-              im -= a[o + 1] * in[2 * j];
-            }
-          }
-          y[2 * i] = re;
-          y[2 * i + 1] = im;
-        }
-      }
-      if (pass == 0) {
-#pragma unroll
-        for (int e = 0; e < 12; e++) res[12 * k + e] = x[12 * k + e] + scale * y[e];
-      } else {
-#pragma unroll
-        for (int e = 0; e < 12; e++) res2[12 * k + e] = y[e];
-      }
-    }
+    for (int e = 0; e < 12; e++) res[12 * k + e] = x[12 * k + e] + scale * y[e];
+    clover_block<T>(a, res + 12 * k, res2 + 12 * k);
   }
 }

@@ -110,32 +110,7 @@ __device__ __forceinline__ void clover_mul_mrhs(const typename V16<T>::vec* sm, 
     for (int r = 0; r < NB; r++) {
       const T* x = v[r] + 12 * k;
       T* y = out[r] + 12 * k;
-      if constexpr (UsePacked<T>::value) {
-        clover_block_packed(a, x, y);
-      } else {
-#pragma unroll
-      for (int i = 0; i < 6; i++) {
-        T re = a[i] * x[2 * i], im = a[i] * x[2 * i + 1];
-#pragma unroll
-        for (int j = 0; j < 6; j++) {
-          if (j < i) {
-            const int o = 6 + 2 * (i * (i - 1) / 2 + j);
-            re += a[o] * x[2 * j];
-            re -= a[o + 1] * x[2 * j + 1];
-            im += a[o] * x[2 * j + 1];
-            im += a[o + 1] * x[2 * j];
-          } else if (j > i) {
-            const int o = 6 + 2 * (j * (j - 1) / 2 + i);
-            re += a[o] * x[2 * j];
-            re += a[o + 1] * x[2 * j + 1];
-            im += a[o] * x[2 * j + 1];
-            im -= a[o + 1] * x[2 * j];
-          }
-        }
-        y[2 * i] = re;
-        y[2 * i + 1] = im;
-      }
-      }
+      clover_block<T>(a, x, y);
     }
   }
 }

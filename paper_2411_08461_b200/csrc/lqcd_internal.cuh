@@ -17,6 +17,8 @@ struct Lat {
   int tb;  // +1 periodic, -1 antiperiodic in t
 };
 
+constexpr int LQCD_MAX_DEVICES = 64;  // lqcd_create refuses a larger ordinal (per-device launch configuration flags)
+
 struct lqcd_ctx {
   int L[4];
   Lat lat;

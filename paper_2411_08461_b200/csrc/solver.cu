@@ -137,6 +137,8 @@ struct Cols {
   int n;
   bool active[LQCD_MAX_RHS];
   double stop2[LQCD_MAX_RHS], bb[LQCD_MAX_RHS], rr[LQCD_MAX_RHS];
+  int base_it[LQCD_MAX_RHS];  // iterations of earlier passes (residual-replacement restarts, invert_native)
+  bool warm;                  // start from the x already in w.x (r = bhat - Mhat x by the operator), not from x = 0
   int nactive() const { int k = 0; for (int j = 0; j < n; j++) k += active[j]; return k; }
 };
 // freeze column j: its BLAS blocks exit from now on, so x_j, r_j keep the values of this iteration
@@ -156,11 +158,18 @@ static int solve_cg(lqcd_ctx* c, const Work& w, const void* gauge, const void* A
   char* x = w.x;
   int rc;
   long dslashes = 0;
-  cudaMemsetAsync(x, 0, blk, st);
-  if (!normal_residual) {
-    cudaMemcpyAsync(r, w.v[0], blk, cudaMemcpyDeviceToDevice, st);
+  // residual of the start vector: x = 0 -> bhat; warm start (residual replacement) -> bhat - Mhat x by the operator
+  char* res0 = normal_residual ? resv : r;
+  if (!cols.warm) {
+    cudaMemsetAsync(x, 0, blk, st);
+    cudaMemcpyAsync(res0, w.v[0], blk, cudaMemcpyDeviceToDevice, st);
   } else {
-    cudaMemcpyAsync(resv, w.v[0], blk, cudaMemcpyDeviceToDevice, st);
+    if ((rc = mpc_apply(c, res0, x, gauge, A, Ai, kappa, matpc, 0, tmp, n, st))) return rc;
+    dslashes += 2;
+    void* u[2] = {w.v[0], res0};
+    if ((rc = BLAS_CALL(c, OpXpay, op.a = -1.0, u, nullptr, n, 0, st))) return rc;  // res0 = bhat - Mhat x
+  }
+  if (normal_residual) {
     if ((rc = mpc_apply(c, r, resv, gauge, A, Ai, kappa, matpc, 1, tmp, n, st))) return rc;
     dslashes += 2;
   }
@@ -254,7 +263,7 @@ static int solve_cg(lqcd_ctx* c, const Work& w, const void* gauge, const void* A
       if (!cols.active[j]) continue;
       const double resn = normal_residual ? hs(c, j, S_RES) : hs(c, j, nxt);
       cols.rr[j] = resn;
-      res[j].iterations = it;
+      res[j].iterations = cols.base_it[j] + it;
       if (!(resn == resn)) { res[j].status = LQCD_ERR_BREAKDOWN; freeze(c, cols, j, st); }
       else if (!(resn > cols.stop2[j])) freeze(c, cols, j, st);
     }
@@ -272,9 +281,16 @@ static int solve_bicgstab(lqcd_ctx* c, const Work& w, const void* gauge, const v
   int rc;
   long dslashes = 0;
   bool restarted[LQCD_MAX_RHS] = {false};
-  cudaMemsetAsync(x, 0, blk, st);
-  cudaMemcpyAsync(r, w.v[0], blk, cudaMemcpyDeviceToDevice, st);
-  cudaMemcpyAsync(r0, w.v[0], blk, cudaMemcpyDeviceToDevice, st);
+  if (!cols.warm) {
+    cudaMemsetAsync(x, 0, blk, st);
+    cudaMemcpyAsync(r, w.v[0], blk, cudaMemcpyDeviceToDevice, st);
+  } else {  // residual replacement: r = bhat - Mhat x by the operator
+    if ((rc = mpc_apply(c, r, x, gauge, A, Ai, kappa, matpc, 0, tmp, n, st))) return rc;
+    dslashes += 2;
+    void* u[2] = {w.v[0], r};
+    if ((rc = BLAS_CALL(c, OpXpay, op.a = -1.0, u, nullptr, n, 0, st))) return rc;
+  }
+  cudaMemcpyAsync(r0, r, blk, cudaMemcpyDeviceToDevice, st);
   {
     // rho_0 = <r0,r> = |r|^2
     void* u[2] = {r0, r};
@@ -324,7 +340,7 @@ static int solve_bicgstab(lqcd_ctx* c, const Work& w, const void* gauge, const v
       if (!cols.active[j]) continue;
       const double rr = hs(c, j, S_RR);
       cols.rr[j] = rr;
-      res[j].iterations = it;
+      res[j].iterations = cols.base_it[j] + it;
       const double rho_mag = hs(c, j, rho_next) * hs(c, j, rho_next) + hs(c, j, rho_next + 1) * hs(c, j, rho_next + 1);
       const double om_mag = hs(c, j, S_TS) * hs(c, j, S_TS) + hs(c, j, S_TS + 1) * hs(c, j, S_TS + 1);
       if (!(rr == rr)) { res[j].status = LQCD_ERR_BREAKDOWN; freeze(c, cols, j, st); continue; }
@@ -432,10 +448,12 @@ static int solve_mixed(lqcd_ctx* c, const Work& w, const void* gauge, const void
   while (nlive > 0 && total < maxiter && outer < 64) {
     Cols ic;
     ic.n = n;
+    ic.warm = false;
     cudaMemsetAsync(ci->d_scalars, 0, sizeof(double) * SC_STRIDE * n, st);
     double rn[LQCD_MAX_RHS];
     for (int j = 0; j < n; j++) {
       ic.active[j] = live[j];
+      ic.base_it[j] = 0;
       ic.bb[j] = 1.0;
       ic.rr[j] = 1.0;
       ic.stop2[j] = 1.0;
@@ -504,12 +522,21 @@ static int solve_mixed(lqcd_ctx* c, const Work& w, const void* gauge, const void
   return LQCD_OK;
 }
 
-// the whole solve on native fields already in w.b; result in w.x (both parities)
-static int invert_native(lqcd_ctx* c, Work& w, const void* gauge, const void* A, const void* Ai, double kappa,
-                         double tol, int maxiter, int solver, int matpc, lqcd_result* res, cudaStream_t st,
-                         Mixed* mixed = nullptr) {
+// the whole solve on native fields already in w.b; result in w.x (both parities).
+// Residual replacement (SURVEY.md §7 "add a reliable-update restart if the true residual misses"): the Krylov loops
+// stop on the recurrence residual; the solve then closes with x_o (a10) and the true residual |b - M x| of the full
+// operator (a11), which costs nothing extra.  A column whose recurrence converged but whose TRUE residual is still
+// above tol |b| (an fp32 recurrence drifts from the true residual near 2e-7; the left-symmetric form stops on
+// |A_ee^-1 r_hat|) is restarted from its x: r = bhat - Mhat x recomputed with the operator replaces the recurrence
+// residual and the iteration goes on to a target tightened by 1/2 per pass, the other columns frozen.  At most
+// MAX_PASSES passes; a column that no longer improves stops.  status = NOT_CONVERGED if the true residual stays
+// above tol |b| (the precision floor of the storage type).
+static int invert_native_body(lqcd_ctx* c, Work& w, const void* gauge, const void* A, const void* Ai, double kappa,
+                              double tol, int maxiter, int solver, int matpc, lqcd_result* res, cudaStream_t st,
+                              Mixed* mixed) {
+  constexpr int MAX_PASSES = 4;
   const int n = w.nrhs;
-  const size_t blk = lqcd_spinor_bytes(c) * n, half = lqcd_clover_bytes(c) / 2;
+  const size_t sp = lqcd_spinor_bytes(c), blk = sp * n, half = lqcd_clover_bytes(c) / 2;
   const void* Ai_e = Ai;
   const void* Ai_o = off(Ai, half);
   char *b_e = w.b, *b_o = w.b + blk, *x_e = w.x, *x_o = w.x + blk;
@@ -528,31 +555,43 @@ static int invert_native(lqcd_ctx* c, Work& w, const void* gauge, const void* A,
   if ((rc = read_scalars(c, n, st))) return rc;
   Cols cols;
   cols.n = n;
+  cols.warm = false;
+  double stop2[LQCD_MAX_RHS], true_rr[LQCD_MAX_RHS];
+  bool solvable[LQCD_MAX_RHS];
   for (int j = 0; j < n; j++) {
     cols.bb[j] = hs(c, j, S_BB) + hs(c, j, S_BB + 1);
-    cols.stop2[j] = tol * tol * cols.bb[j];
+    const bool finite = cols.bb[j] == cols.bb[j] && cols.bb[j] <= 1.7e308;
+    stop2[j] = cols.stop2[j] = tol * tol * cols.bb[j];
     cols.rr[j] = 0;
-    cols.active[j] = cols.bb[j] > 0.0;  // a zero source has the zero solution: nothing to iterate
-    res[j].status = LQCD_OK;
+    cols.base_it[j] = 0;
+    true_rr[j] = 0;
+    // a zero source has the zero solution: nothing to iterate; a non-finite source cannot be solved
+    solvable[j] = cols.active[j] = finite && cols.bb[j] > 0.0;
+    res[j].status = finite ? LQCD_OK : LQCD_ERR_BREAKDOWN;
   }
   cudaMemsetAsync(w.x, 0, 2 * blk, st);
-  if (cols.nactive() > 0) {
-    // a5: bhat = b_e + kappa D_eo A_oo^-1 b_o   (sym: bhat_s = A_ee^-1 bhat)
-    char* bh = w.v[0];
-    if ((rc = lqcd_clover_apply_launch(c, w.v[5], b_o, Ai_o, n, st))) return rc;
-    if ((rc = lqcd_dslash_launch(c, bh, w.v[5], gauge, nullptr, nullptr, 0, kappa, 0, 0, n, st))) return rc;
-    {
-      void* v[2] = {b_e, bh};
-      if ((rc = BLAS_CALL(c, OpXpay, op.a = 1.0, v, nullptr, n, 0, st))) return rc;
-    }
-    if (matpc == LQCD_MATPC_SYMMETRIC)
-      if ((rc = lqcd_clover_apply_launch(c, bh, bh, Ai_e, n, st))) return rc;
+  if (cols.nactive() == 0) return LQCD_OK;
+  // a5: bhat = b_e + kappa D_eo A_oo^-1 b_o   (sym: bhat_s = A_ee^-1 bhat)
+  char* bh = w.v[0];
+  if ((rc = lqcd_clover_apply_launch(c, w.v[5], b_o, Ai_o, n, st))) return rc;
+  if ((rc = lqcd_dslash_launch(c, bh, w.v[5], gauge, nullptr, nullptr, 0, kappa, 0, 0, n, st))) return rc;
+  {
+    void* v[2] = {b_e, bh};
+    if ((rc = BLAS_CALL(c, OpXpay, op.a = 1.0, v, nullptr, n, 0, st))) return rc;
+  }
+  if (matpc == LQCD_MATPC_SYMMETRIC)
+    if ((rc = lqcd_clover_apply_launch(c, bh, bh, Ai_e, n, st))) return rc;
+  for (int pass = 0;; pass++) {
     for (int j = 0; j < n; j++)
       if (!cols.active[j]) set_slot(c, j, S_DONE, true, st);
     c->acct_rhs = cols.nactive();
-    if (mixed) rc = solve_mixed(c, w, gauge, A, Ai, kappa, matpc, solver, cols, maxiter, res, *mixed, st);
-    else if (solver == LQCD_SOLVER_BICGSTAB) rc = solve_bicgstab(c, w, gauge, A, Ai, kappa, matpc, cols, maxiter, res, st);
-    else rc = solve_cg(c, w, gauge, A, Ai, kappa, matpc, solver == LQCD_SOLVER_CGNR, cols, maxiter, res, st);
+    int done = 0;
+    for (int j = 0; j < n; j++)
+      if (cols.active[j] && cols.base_it[j] > done) done = cols.base_it[j];
+    const int left = maxiter - done;
+    if (mixed) rc = solve_mixed(c, w, gauge, A, Ai, kappa, matpc, solver, cols, left, res, *mixed, st);
+    else if (solver == LQCD_SOLVER_BICGSTAB) rc = solve_bicgstab(c, w, gauge, A, Ai, kappa, matpc, cols, left, res, st);
+    else rc = solve_cg(c, w, gauge, A, Ai, kappa, matpc, solver == LQCD_SOLVER_CGNR, cols, left, res, st);
     c->acct_rhs = 0;
     if (rc) return rc;
     set_slot_all(c, n, S_DONE, false, st);  // the closing steps below update every column
@@ -576,15 +615,55 @@ static int invert_native(lqcd_ctx* c, Work& w, const void* gauge, const void* A,
       if ((rc = BLAS_CALL(c, OpAxpyNorm, op.a = -1.0, v2, o2, n, 0, st))) return rc;
     }
     if ((rc = read_scalars(c, n, st))) return rc;
+    for (int j = 0; j < n; j++) res[j].dslash_count += pass == 0 ? 4 : 3;  // (first pass: prepare,) reconstruct, two for the true residual
+    // which columns go on: recurrence converged, true residual above the bar and still falling
+    int again = 0;
+    for (int j = 0; j < n; j++) {
+      const bool was = cols.active[j];
+      cols.active[j] = false;
+      if (!solvable[j] || !was) continue;
+      const double t2 = hs(c, j, S_TRUE) + hs(c, j, S_TRUE + 1), before = true_rr[j];
+      true_rr[j] = t2;
+      cols.base_it[j] = res[j].iterations;
+      const bool improving = pass == 0 || t2 < 0.5 * before;
+      if (mixed || res[j].status != LQCD_OK || cols.rr[j] > cols.stop2[j] || !(t2 > stop2[j]) || !improving ||
+          pass + 1 >= MAX_PASSES || res[j].iterations >= maxiter)
+        continue;
+      cols.active[j] = true;
+      cols.stop2[j] *= 0.25;
+      again++;
+    }
+    if (again == 0) break;
+    cols.warm = true;
+    if (matpc == LQCD_MATPC_SYMMETRIC_RIGHT)  // back to the Krylov unknown y = A_ee x_e, restarted columns only
+      for (int j = 0; j < n; j++)
+        if (cols.active[j])
+          if ((rc = lqcd_clover_apply_launch(c, x_e + j * sp, x_e + j * sp, A, 1, st))) return rc;
   }
   for (int j = 0; j < n; j++) {
-    if (!(cols.bb[j] > 0.0)) continue;
-    res[j].dslash_count += 4;  // prepare, reconstruct, two for the true residual
+    if (!solvable[j]) continue;
     res[j].iter_resid = sqrt(cols.rr[j] / cols.bb[j]);
-    if (res[j].status == LQCD_OK && cols.rr[j] > cols.stop2[j]) res[j].status = LQCD_NOT_CONVERGED;
-    res[j].true_resid = sqrt((hs(c, j, S_TRUE) + hs(c, j, S_TRUE + 1)) / cols.bb[j]);
+    res[j].true_resid = sqrt(true_rr[j] / cols.bb[j]);
+    if (res[j].status == LQCD_OK && (cols.rr[j] > stop2[j] || true_rr[j] > stop2[j])) res[j].status = LQCD_NOT_CONVERGED;
   }
   return LQCD_OK;
+}
+
+// freeze flags and the first-iteration flag never outlive a solve, whatever path it returned by: the public
+// lqcd_blas_* calls and the next solve on this context (or on the inner context of a mixed solve) start clean
+static int invert_native(lqcd_ctx* c, Work& w, const void* gauge, const void* A, const void* Ai, double kappa,
+                         double tol, int maxiter, int solver, int matpc, lqcd_result* res, cudaStream_t st,
+                         Mixed* mixed = nullptr) {
+  const int rc = invert_native_body(c, w, gauge, A, Ai, kappa, tol, maxiter, solver, matpc, res, st, mixed);
+  c->acct_rhs = 0;
+  set_slot_all(c, w.nrhs, S_DONE, false, st);
+  set_slot_all(c, w.nrhs, S_FIRST, false, st);
+  if (mixed) {
+    mixed->ci->acct_rhs = 0;
+    set_slot_all(mixed->ci, w.nrhs, S_DONE, false, st);
+    set_slot_all(mixed->ci, w.nrhs, S_FIRST, false, st);
+  }
+  return rc;
 }
 
 static int worst_status(const lqcd_result* res, int n) {

@@ -122,10 +122,11 @@ def test_config3_propagator_12_columns_batched_fp32_recon12():
     x, res, rc = s.ctx.invert_multi(B, s.gauge, s.A, s.Ai, s.kappa, tol=1e-6, solver="cgne")
     assert rc == 0
     xs = x.cpu().numpy().astype(np.complex128)
-    for r in (0, 5, 11):
-        assert s.orc.true_residual(bs[r], xs[r]) < 2e-6
-    xo, ro = s.orc.invert(bs[0], 1e-9, 2000, "cgne", 0)
-    assert rel_err(xs[0], xo) < 1e-5
+    for r in range(12):  # every column, oracle-evaluated, below the tolerance asked for (reading A17)
+        assert s.orc.true_residual(bs[r], xs[r]) < 1e-6, (r, res[r].as_dict())
+    for r in (0, 5, 10):
+        xo, ro = s.orc.invert(bs[r], 1e-9, 2000, "cgne", 0)
+        assert rel_err(xs[r], xo) < 1e-5, r
     # sink-source assembly [.., s_sink, s_src, c_sink, c_src] and gamma5-hermiticity at the source
     prop = np.zeros(s.orc.site_shape + (4, 4, 3, 3), dtype=np.complex128)
     for r in range(12):

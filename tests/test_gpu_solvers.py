@@ -52,14 +52,14 @@ def test_config2_bicgstab_fp32(recon):
     s, c = from_cfg(2, 4, recon)
     b = synth.source(c["dims"], "z2", c["src_seed"])
     xo, ro = s.orc.invert(b, 1e-10, 2000, "bicgstab", 0)
-    # north_star: fp32 solve to 1e-6; the oracle-evaluated true residual must be < 1e-6 as well,
-    # allowing the fp32 rounding floor of the recurrence (2x)
-    solve_and_check(s, b, "bicgstab", 0, 1e-6, xo, resid_bound=2e-6)
-    solve_and_check(s, b, "cgne", 0, 1e-6, xo, resid_bound=2e-6)
+    # north_star: fp32 solve to 1e-6; the oracle-evaluated true residual must be < 1e-6 as well (reading A17):
+    # a column whose true residual misses is restarted from its x with the recomputed residual (solver.cu)
+    solve_and_check(s, b, "bicgstab", 0, 1e-6, xo)
+    solve_and_check(s, b, "cgne", 0, 1e-6, xo)
     # the symmetric forms in fp32 (packed FFMA2 epilogues 6-10, clover_mul_twice)
     for matpc in (1, 2):
-        solve_and_check(s, b, "cgne", matpc, 1e-6, xo, resid_bound=2e-6)
-        solve_and_check(s, b, "bicgstab", matpc, 1e-6, xo, resid_bound=2e-6)
+        solve_and_check(s, b, "cgne", matpc, 1e-6, xo)
+        solve_and_check(s, b, "bicgstab", matpc, 1e-6, xo)
 
 
 def test_invert_builds_clover_when_absent_and_edge_cases():
@@ -111,8 +111,8 @@ def test_host_entry_points():
 
 def test_config3_propagator_12_columns_fp32_recon12():
     """BASELINE config 3: 16^3x32, fp32, reconstruct-12, point source, all 12 spin-colour columns by
-    CGNE, assembled sink-source.  Each column's true residual is checked with the
-    oracle's operator; one column is compared with the oracle's own solve."""
+    CGNE, assembled sink-source.  Every column's true residual is checked with the
+    oracle's operator (< tol, reading A17); three columns are compared with the oracle's own solve."""
     s, c = from_cfg(3, 4, 12)
     dims = c["dims"]
     prop = np.zeros(s.orc.site_shape + (4, 4, 3, 3), dtype=np.complex128)
@@ -125,9 +125,8 @@ def test_config3_propagator_12_columns_fp32_recon12():
             assert res.status == 0
             xg = x.cpu().numpy().astype(np.complex128)
             prop[..., :, spin, :, col] = xg
-            if (spin, col) in ((0, 0), (3, 2)):
-                assert s.orc.true_residual(b, xg) < 2e-6
-            if (spin, col) == (0, 0):
+            assert s.orc.true_residual(b, xg) < 1e-6, (spin, col, res.as_dict())
+            if (spin, col) in ((0, 0), (1, 2), (3, 1)):
                 xo, ro = s.orc.invert(b, 1e-9, 2000, "cgne", 0)
                 assert rel_err(xg, xo) < 1e-5
     # gamma5-hermiticity of the point-to-point propagator at the source: g5 S(0,0) g5 = S(0,0)^dag
@@ -171,3 +170,69 @@ def test_config2_cgne_fp64_recon12(matpc):
     b = synth.source(c["dims"], "z2", c["src_seed"])
     xo, ro = s.orc.invert(b, 1e-10, 2000, "bicgstab", 0)
     solve_and_check(s, b, "cgne", matpc, 1e-10, xo)
+
+
+@pytest.mark.parametrize("solver", ["cgne", "bicgstab"])
+def test_fp32_status_is_honest_about_the_true_residual(solver):
+    """PAPER.md:158, 221 (tol is the solver's tolerance): status OK means the TRUE residual, evaluated by the oracle,
+    is below tol -- the recurrence residual of an fp32 solve drifts from it near 2e-7, so a column that misses is
+    restarted with the recomputed residual (solver.cu, invert_native).  Below the fp32 floor the call must say
+    NOT_CONVERGED, not OK."""
+    s, c = from_cfg(2, 4, 18)
+    b = synth.source(c["dims"], "z2", c["src_seed"])
+    ok = 0
+    for tol in (1e-6, 5e-7, 3e-7, 1e-7, 1e-8):
+        for matpc in (0, 1, 2):
+            x, res = s.ctx.invert(s.ctx.to_device(b), s.gauge, s.A, s.Ai, s.kappa, tol=tol, maxiter=500, solver=solver,
+                                  matpc=matpc)
+            true = s.orc.true_residual(b, x.cpu().numpy().astype(np.complex128))
+            assert res.status in (0, 1), res.as_dict()
+            if res.status == 0:
+                assert true < tol, (tol, matpc, true, res.as_dict())
+                ok += 1
+            else:
+                assert res.true_resid > tol or res.iter_resid > tol
+            if tol >= 5e-7:
+                assert res.status == 0, (tol, matpc, res.as_dict())
+    assert ok >= 6
+
+
+def test_freeze_flags_do_not_outlive_a_solve():
+    """a mixed solve freezes the converged columns of its fp32 context; the flags must be cleared at exit
+    (also on the stalled / not-converged paths), or the public BLAS-1 calls on that context silently do nothing."""
+    s, c = from_cfg(1, 8, 18)
+    lo = lq().Context(c["dims"], 4, 18, -1)
+    g_lo = lo.gauge_pack(lo.to_device(s.U))
+    A_lo, Ai_lo = lo.clover_build(g_lo, c["csw"], c["kappa"])
+    b = synth.source(c["dims"], "gaussian", 3)
+    for tol, want in ((1e-10, 0), (1e-18, 1)):  # 1e-18 is below the fp64 floor: the outer loop stalls -> NOT_CONVERGED
+        x, res = s.ctx.invert_mixed(lo, s.ctx.to_device(b), s.gauge, s.A, s.Ai, g_lo, A_lo, Ai_lo, s.kappa, tol=tol,
+                                    inner_tol=1e-4, maxiter=3000, solver="bicgstab")
+        assert res.status == want, res.as_dict()
+        assert s.orc.true_residual(b, x.cpu().numpy()) < 1e-10
+        for ctx in (lo, s.ctx):
+            u = torch.randn(ctx.spinor_bytes // ctx.prec, dtype=ctx.rdtype, device=ctx.dev)
+            v = torch.randn_like(u)
+            dot, nrm = ctx.blas_cdot(u, v)
+            assert abs(nrm - float((u.double() ** 2).sum())) < 1e-5 * nrm
+            w = v.clone()
+            ctx.blas_xpay(u, 2.0, w)
+            assert torch.allclose(w, u + 2.0 * v)
+
+
+def test_degenerate_sources_and_lucky_breakdown():
+    s, c = from_cfg(1, 8, 18)
+    b = synth.source(c["dims"], "gaussian", 5)
+    # a non-finite source is an error of that column, not a successful solve (ADVICE r1)
+    bad = b.copy()
+    bad[0, 0, 0, 0, 0, 0, 0] = np.nan
+    B = s.ctx.to_device(np.stack([b, bad]))
+    x, res, rc = s.ctx.invert_multi(B, s.gauge, s.A, s.Ai, s.kappa, tol=1e-10, solver="cgne")
+    assert res[0].status == 0 and res[1].status == -7 and rc == -7
+    assert s.orc.true_residual(b, x[0].cpu().numpy()) < 1e-10
+    # kappa = 0: M = 1, the first BiCGStab half step already solves the system (s = 0, t = 0, omega = 0/0 guarded)
+    A1, Ai1 = s.ctx.clover_build(s.gauge, c["csw"], 0.0)
+    for solver in ("bicgstab", "cgne"):
+        x1, r1 = s.ctx.invert(s.ctx.to_device(b), s.gauge, A1, Ai1, 0.0, tol=1e-12, solver=solver)
+        assert r1.status == 0 and r1.iterations <= 1, r1.as_dict()
+        assert rel_err(x1.cpu().numpy(), b) < 1e-14
