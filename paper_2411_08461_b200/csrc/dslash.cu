@@ -38,7 +38,7 @@ template <typename T> struct DslashArgs {
 
 // Launch shape per precision (threads per block, minimum resident blocks per SM = register budget).
 // The kernel is latency bound: what matters is how many independent loads ptxas can hoist per
-// thread, which the register budget controls; values chosen by the sweep in profiles/r01_tuning.md.
+// thread, which the register budget controls; values chosen by the round-1 sweep (profiles/r01d_tuning.md; the first sweep is in the git history).
 #ifndef DSLASH_BLOCK_F32
 #define DSLASH_BLOCK_F32 128
 #endif
@@ -52,7 +52,7 @@ template <typename T> struct DslashArgs {
 #define DSLASH_MINB_F64 5
 #endif
 #ifndef DSLASH_STAGE_F64_R12
-#define DSLASH_STAGE_F64_R12 1  // cp.async link staging pays for fp64 12-real links only (profiles/r01_tuning.md)
+#define DSLASH_STAGE_F64_R12 1  // cp.async link staging pays for fp64 12-real links only (round-1 sweep, profiles/r01d_tuning.md)
 #endif
 #ifndef DSLASH_MINB_F64_R12
 #define DSLASH_MINB_F64_R12 4

@@ -582,8 +582,11 @@ static int invert_native_body(lqcd_ctx* c, Work& w, const void* gauge, const voi
   if (matpc == LQCD_MATPC_SYMMETRIC)
     if ((rc = lqcd_clover_apply_launch(c, bh, bh, Ai_e, n, st))) return rc;
   for (int pass = 0;; pass++) {
-    for (int j = 0; j < n; j++)
+    bool in_pass[LQCD_MAX_RHS];  // the Krylov loop clears cols.active[j] when column j stops
+    for (int j = 0; j < n; j++) {
+      in_pass[j] = cols.active[j];
       if (!cols.active[j]) set_slot(c, j, S_DONE, true, st);
+    }
     c->acct_rhs = cols.nactive();
     int done = 0;
     for (int j = 0; j < n; j++)
@@ -619,9 +622,8 @@ static int invert_native_body(lqcd_ctx* c, Work& w, const void* gauge, const voi
     // which columns go on: recurrence converged, true residual above the bar and still falling
     int again = 0;
     for (int j = 0; j < n; j++) {
-      const bool was = cols.active[j];
       cols.active[j] = false;
-      if (!solvable[j] || !was) continue;
+      if (!solvable[j] || !in_pass[j]) continue;
       const double t2 = hs(c, j, S_TRUE) + hs(c, j, S_TRUE + 1), before = true_rr[j];
       true_rr[j] = t2;
       cols.base_it[j] = res[j].iterations;
