@@ -78,8 +78,10 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], int prec, int recon, int t_bo
     // kernel at every tile shape tried (profiles/r01d_tuning.md), so it is opt-in: LQCD_DSLASH_TILED=1
     const char* e = getenv("LQCD_DSLASH_TILED");
     c->tiled = (e && e[0] == '1') ? 1 : 0;
-    const char* m = getenv("LQCD_MRHS_TILED");  // tiled multi-RHS kernel: measurement switch
-    c->mrhs_tiled = (m && m[0] == '1') ? 1 : 0;
+    const char* m = getenv("LQCD_MRHS_TMA");  // TMA-tiled multi-RHS kernel: on unless LQCD_MRHS_TMA=0 (A/B measurements, parity tests of both)
+    c->mrhs_tma = (m && m[0] == '0') ? 0 : 1;
+    const char* z = getenv("LQCD_MRHS_ZSLAB");
+    c->mrhs_zslab = z ? atoi(z) : 4;
   }
   c->recon = recon;
   c->device = device;

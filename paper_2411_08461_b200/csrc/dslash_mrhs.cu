@@ -497,8 +497,10 @@ int lqcd_dslash_mrhs_launch(lqcd_ctx* c, void* out, const void* in, const void* 
   c->alg_bytes += bytes;
   const bool rec = c->prof_on && c->prof_n < c->prof_cap;
   if (rec) cudaEventRecord(c->prof_ev[2 * c->prof_n], st);
-  if (lqcd_mrhs_tiled_ok(c) && epi <= 3) lqcd_dslash_mrhs_tiled_launch(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st);
-  else if (c->prec == 4) launch_mrhs_typed<float>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st);
+  if (lqcd_mrhs_tma_ok(c, epi)) {
+    const int rc = lqcd_dslash_mrhs_tma_launch(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st);
+    if (rc) return rc;
+  } else if (c->prec == 4) launch_mrhs_typed<float>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st);
   else launch_mrhs_typed<double>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st);
   if (rec) {
     cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], st);

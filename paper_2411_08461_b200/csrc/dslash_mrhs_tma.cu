@@ -1,0 +1,424 @@
+// Multi-right-hand-side dslash, TMA-tiled form (the 12 spin-colour columns of a
+// propagator share links and clover).  fp32.
+//
+// What bounds the one-thread-per-(site, column) kernel of dslash_mrhs.cu (profiles/r01d_README.md): every neighbour
+// spinor of every column crosses the L2->SM crossbar once per hop (768 B per site and column, 10-11 TB/s, the
+// crossbar's limit), and the links and clover rows are re-read from shared memory for every column (864 B per site
+// and column on the shared-memory pipe).  This kernel removes both:
+//   * a block owns a tile of TY x TZ x TT full x-rows of output sites (LXH checkerboard sites each) and walks the
+//     columns one after the other; the input spinors of the tile + its one-site halo in y, z, t (x wraps inside a
+//     full row) are brought to shared memory ONCE per column by the TMA unit (cp.async.bulk.tensor, one 3-D box
+//     {row, 6 vectors} per x-row, issued by the lanes of a producer warp, completion on an mbarrier), into a ring of
+//     NST stages: while the consumer warps multiply column c from stage s, column c+1 is already in flight.  Crossbar
+//     traffic per site and column: NROWS/RC x 96 B (384 B at 32^3x64, 336 B at 16^3x32) instead of 768 B;
+//   * a site is split over TWO threads of different warps: role 0 does the hops +-x, +-y and the upper chiral block,
+//     role 1 the hops +-z, +-t and the lower chiral block.  Each keeps ITS four links (72 registers) and its 6x6
+//     clover block (36 registers) in registers for all columns, so links and clover cost no bytes per column at all.
+//     The two partial sums are exchanged through shared memory (12 reals each way) behind a 64-thread named barrier.
+// Per column a thread reads 4 x 96 B of neighbours + 48 B of its partner's half from shared memory, multiplies, applies
+// its clover block, and stores its half of the output: the neighbour bytes are the only per-column traffic left.
+//
+// Tile order (problem (i) of the round-1 verdict: 1.5x excess DRAM traffic because the +-t reuse window of 12 columns
+// outgrew L2): blocks sweep the lattice in z-slabs, t inside a slab, so the window is 2 x slab x 12 columns.
+#define DSLASH_FFMA2 1
+#include <cuda.h>  // CUtensorMap and the encode prototype only; the entry point comes through cudart (no -lcuda)
+#include <stdlib.h>
+#include "dslash.cuh"
+
+namespace {
+
+template <int LXH_, int TY_, int TZ_, int TT_> struct RowTile {
+  static constexpr int LXH = LXH_, TY = TY_, TZ = TZ_, TT = TT_;
+  static constexpr int RC = TY * TZ * TT;                      // core rows = output rows
+  static constexpr int NS = LXH * RC;                          // output sites per tile
+  static constexpr int NYH = TZ * TT, NZH = TY * TT, NTH = TY * TZ;  // rows of one halo face
+  static constexpr int ROWB = LXH * 16;                        // bytes of one vector of one row
+  // a stage holds seven regions, one TMA box each, every region [vector][row][xh] float4 (the order a box lands in):
+  // core (rows ly + TY (lz + TZ lt)), y-, y+ (rows lz + TZ lt), z-, z+ (ly + TY lt), t-, t+ (ly + TY lz)
+  static constexpr int VS_C = RC * ROWB, VS_Y = NYH * ROWB, VS_Z = NZH * ROWB, VS_T = NTH * ROWB;  // vector strides
+  static constexpr int B_C = 0, B_YM = 6 * VS_C, B_YP = B_YM + 6 * VS_Y, B_ZM = B_YP + 6 * VS_Y, B_ZP = B_ZM + 6 * VS_Z,
+                       B_TM = B_ZP + 6 * VS_Z, B_TP = B_TM + 6 * VS_T;
+  static constexpr int STAGE_BYTES = B_TP + 6 * VS_T;
+  static constexpr int NCONS = 2 * NS;                         // threads: two per site
+};
+constexpr int NST = 3;  // ring stages: two columns in flight while one is multiplied
+
+struct TmaArgs {
+  float* out;
+  const float* gauge;
+  const float* cl;
+  const float* x;
+  Lat lat;
+  int parity, nrhs;
+  float scale, ws;
+  size_t stride;  // reals between consecutive right-hand sides
+  int zslab;      // z-tiles per slab of the sweep
+};
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  const unsigned a = smem_u32(bar);
+  unsigned ok;
+  do {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(ok)
+        : "r"(a), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+// one 5-D box {all of x, by, bz, bt, 6 vectors} of the input field -> shared memory, completion bytes on `bar`
+__device__ __forceinline__ void tma_load_box(void* dst, const CUtensorMap* map, int y, int z, int t, int v0,
+                                             unsigned long long* bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.5d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];" ::"r"(
+          smem_u32(dst)),
+      "l"(reinterpret_cast<unsigned long long>(map)), "r"(0), "r"(y), "r"(z), "r"(t), "r"(v0), "r"(smem_u32(bar))
+      : "memory");
+}
+struct TmaMaps {
+  CUtensorMap core, yface, zface, tface;  // the same field, boxes {x, TY, TZ, TT, 6}, {x, 1, TZ, TT, 6}, {x, TY, 1, TT, 6}, {x, TY, TZ, 1, 6}
+};
+// the seven boxes of column c of the tile at (y0, z0, t0) into the stage at `sb`; called by ONE thread
+template <typename TS>
+__device__ __forceinline__ void issue_stage(unsigned char* sb, const TmaMaps* m, const Lat& L, int y0, int z0, int t0, int c,
+                                            unsigned long long* bar) {
+  const int ym = y0 == 0 ? L.Ly - 1 : y0 - 1, yp = y0 + TS::TY == L.Ly ? 0 : y0 + TS::TY;
+  const int zm = z0 == 0 ? L.Lz - 1 : z0 - 1, zp = z0 + TS::TZ == L.Lz ? 0 : z0 + TS::TZ;
+  const int tm = t0 == 0 ? L.Lt - 1 : t0 - 1, tp = t0 + TS::TT == L.Lt ? 0 : t0 + TS::TT;
+  mbar_arrive_expect_tx(bar, TS::STAGE_BYTES);
+  tma_load_box(sb + TS::B_C, &m->core, y0, z0, t0, 6 * c, bar);
+  tma_load_box(sb + TS::B_YM, &m->yface, ym, z0, t0, 6 * c, bar);
+  tma_load_box(sb + TS::B_YP, &m->yface, yp, z0, t0, 6 * c, bar);
+  tma_load_box(sb + TS::B_ZM, &m->zface, y0, zm, t0, 6 * c, bar);
+  tma_load_box(sb + TS::B_ZP, &m->zface, y0, zp, t0, 6 * c, bar);
+  tma_load_box(sb + TS::B_TM, &m->tface, y0, z0, tm, 6 * c, bar);
+  tma_load_box(sb + TS::B_TP, &m->tface, y0, z0, tp, 6 * c, bar);
+}
+__device__ __forceinline__ void pair_barrier(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
+
+// one hop from the staged tile: sp = this site's neighbour, vector 0; the six vectors are vs bytes apart (the
+// vector stride of the region the neighbour lies in: the core box or a halo face)
+template <int MU, bool FWD, bool DAG>
+__device__ __forceinline__ void hop_sm(float* acc, const unsigned char* sp, int vs, const float* U, float w) {
+  constexpr int S = (FWD != DAG) ? -1 : +1;
+  float psi[24], h[12], chi[12];
+#pragma unroll
+  for (int v = 0; v < 6; v++) {
+    const float4 q = *reinterpret_cast<const float4*>(sp + v * vs);
+    vec_get(q, psi + 4 * v);
+  }
+  project<float, MU, S>(psi, h);
+  su3_mul<float, !FWD>(U, h, chi);
+  reconstruct<float, MU, S>(acc, chi, w);
+}
+
+// The work of one consumer thread: ROLE 0 = hops +-x, +-y and the upper chiral block, ROLE 1 = hops +-z, +-t and the
+// lower one (a template parameter, so every register array is indexed statically; the branch on the role is uniform
+// over a warp).  EPI as in dslash.cu: 0 scale*d ; 1 scale*C d ; 2 C x + scale*d ; 3 x + scale*C d ; 6 x + scale*d
+template <typename TS, int R, bool DAG, int EPI, int ROLE>
+__device__ __forceinline__ void consume(const TmaMaps* maps, const TmaArgs& a, unsigned char* stage0, float4* xbuf,
+                                        unsigned long long* bars, int y0, int z0, int t0) {
+  constexpr int LXH = TS::LXH, TY = TS::TY, TZ = TS::TZ, TT = TS::TT, NS = TS::NS, NW = TS::NCONS / 32;
+  constexpr bool CLOVER = EPI == 1 || EPI == 2 || EPI == 3;
+  const Lat& L = a.lat;
+  const int Vh = L.Vh, par = a.parity;
+  const int tid = threadIdx.x, sl = tid % NS, warp = tid >> 5, lane = tid & 31;
+  const int lxh = sl % LXH, crow = sl / LXH;
+  const int ly = crow % TY, lz = (crow / TY) % TZ, lt = crow / (TY * TZ);
+  Site s;
+  s.xh = lxh;
+  s.y = y0 + ly;
+  s.z = z0 + lz;
+  s.t = t0 + lt;
+  s.r = (par + s.y + s.z + s.t) & 1;
+  const int idx = s.xh + L.Lxh * (s.y + L.Ly * (s.z + L.Lz * s.t));
+  const size_t blk = (size_t)R * Vh;
+  // this role's four hops: byte offset of the neighbour inside a stage, and the four links (registers, all columns)
+  int n0, n1, n2, n3, v0, v1, v2, v3;  // neighbour: byte offset of vector 0 in a stage, vector stride of its region
+  float U0[18], U1[18], U2[18], U3[18];
+  float w2, w3;
+  if (ROLE == 0) {
+    const int xp = s.r ? (lxh + 1 == LXH ? 0 : lxh + 1) : lxh, xm = s.r ? lxh : (lxh == 0 ? LXH - 1 : lxh - 1);
+    const int fy = lz + TZ * lt;  // row in a y face
+    n0 = TS::B_C + crow * TS::ROWB + xp * 16;
+    n1 = TS::B_C + crow * TS::ROWB + xm * 16;
+    v0 = v1 = TS::VS_C;
+    n2 = (ly + 1 < TY ? TS::B_C + (crow + 1) * TS::ROWB : TS::B_YP + fy * TS::ROWB) + lxh * 16;
+    v2 = ly + 1 < TY ? TS::VS_C : TS::VS_Y;
+    n3 = (ly > 0 ? TS::B_C + (crow - 1) * TS::ROWB : TS::B_YM + fy * TS::ROWB) + lxh * 16;
+    v3 = ly > 0 ? TS::VS_C : TS::VS_Y;
+    load_link<float, R>(a.gauge + (0 * 2 + par) * blk, Vh, idx, U0);
+    load_link<float, R>(a.gauge + (0 * 2 + 1 - par) * blk, Vh, neighbour<0, -1>(L, idx, s), U1);
+    load_link<float, R>(a.gauge + (1 * 2 + par) * blk, Vh, idx, U2);
+    load_link<float, R>(a.gauge + (1 * 2 + 1 - par) * blk, Vh, neighbour<1, -1>(L, idx, s), U3);
+    w2 = w3 = a.ws;
+  } else {
+    const int fz = ly + TY * lt, ft = ly + TY * lz;  // rows in a z face, a t face
+    n0 = (lz + 1 < TZ ? TS::B_C + (crow + TY) * TS::ROWB : TS::B_ZP + fz * TS::ROWB) + lxh * 16;
+    v0 = lz + 1 < TZ ? TS::VS_C : TS::VS_Z;
+    n1 = (lz > 0 ? TS::B_C + (crow - TY) * TS::ROWB : TS::B_ZM + fz * TS::ROWB) + lxh * 16;
+    v1 = lz > 0 ? TS::VS_C : TS::VS_Z;
+    n2 = (lt + 1 < TT ? TS::B_C + (crow + TY * TZ) * TS::ROWB : TS::B_TP + ft * TS::ROWB) + lxh * 16;
+    v2 = lt + 1 < TT ? TS::VS_C : TS::VS_T;
+    n3 = (lt > 0 ? TS::B_C + (crow - TY * TZ) * TS::ROWB : TS::B_TM + ft * TS::ROWB) + lxh * 16;
+    v3 = lt > 0 ? TS::VS_C : TS::VS_T;
+    load_link<float, R>(a.gauge + (2 * 2 + par) * blk, Vh, idx, U0);
+    load_link<float, R>(a.gauge + (2 * 2 + 1 - par) * blk, Vh, neighbour<2, -1>(L, idx, s), U1);
+    load_link<float, R>(a.gauge + (3 * 2 + par) * blk, Vh, idx, U2);
+    load_link<float, R>(a.gauge + (3 * 2 + 1 - par) * blk, Vh, neighbour<3, -1>(L, idx, s), U3);
+    w2 = (L.tb < 0 && s.t == L.Lt - 1) ? -1.f : 1.f;  // antiperiodic seam, forward and backward
+    w3 = (L.tb < 0 && s.t == 0) ? -1.f : 1.f;
+  }
+  float cb[CLOVER ? 36 : 1];
+  if (CLOVER) load_clover_block<float>(a.cl, Vh, idx, ROLE, cb);
+  // own half of a spinor: vectors 3*ROLE .. 3*ROLE+2 of the native layout (spins 0,1 | 2,3)
+  const size_t hoff = ((size_t)3 * ROLE * Vh + idx) * 4;
+  const int pair_id = 1 + (warp % (NS / 32));
+  float4* xmine = xbuf + (ROLE * 3) * NS + sl;  // what I send: my partial sum of the half I do not own
+  const float4* xtheirs = xbuf + ((1 - ROLE) * 3) * NS + sl;
+
+  for (int c = 0; c < a.nrhs; c++) {
+    const int st = c % NST;
+    const unsigned ph = (c / NST) & 1;
+    float xv[12];
+    if (EPI == 2 || EPI == 3 || EPI == 6) {  // issued before the wait: the latency hides behind it
+      const float4* xp = reinterpret_cast<const float4*>(a.x + (size_t)c * a.stride + hoff);
+#pragma unroll
+      for (int v = 0; v < 3; v++) {
+        const float4 q = ld_cached(xp + (size_t)v * Vh);
+        vec_get(q, xv + 4 * v);
+      }
+    }
+    mbar_wait(&bars[st], ph);
+    const unsigned char* sb = stage0 + st * TS::STAGE_BYTES;
+    float acc[24];
+#pragma unroll
+    for (int e = 0; e < 24; e++) acc[e] = 0.f;
+    hop_sm<2 * ROLE, true, DAG>(acc, sb + n0, v0, U0, a.ws);
+    hop_sm<2 * ROLE, false, DAG>(acc, sb + n1, v1, U1, a.ws);
+    hop_sm<2 * ROLE + 1, true, DAG>(acc, sb + n2, v2, U2, w2);
+    hop_sm<2 * ROLE + 1, false, DAG>(acc, sb + n3, v3, U3, w3);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&bars[NST + st]);  // this warp no longer reads stage st
+    // exchange the halves: I keep reals [12*ROLE, 12*ROLE+12), my partner owns the other twelve
+    float4* xs = xmine + (c & 1) * (2 * 3 * NS);
+#pragma unroll
+    for (int v = 0; v < 3; v++) {
+      const int o = 12 * (1 - ROLE) + 4 * v;
+      xs[v * NS] = make_float4(acc[o], acc[o + 1], acc[o + 2], acc[o + 3]);
+    }
+    pair_barrier(pair_id);
+    const float4* xr = xtheirs + (c & 1) * (2 * 3 * NS);
+    float d[12];
+#pragma unroll
+    for (int v = 0; v < 3; v++) {
+      const float4 q = xr[v * NS];
+      const int o = 12 * ROLE + 4 * v;
+      d[4 * v] = acc[o] + q.x;
+      d[4 * v + 1] = acc[o + 1] + q.y;
+      d[4 * v + 2] = acc[o + 2] + q.z;
+      d[4 * v + 3] = acc[o + 3] + q.w;
+    }
+    float res[12];
+    if (EPI == 0) {
+#pragma unroll
+      for (int e = 0; e < 12; e++) res[e] = a.scale * d[e];
+    } else if (EPI == 1) {
+      clover_block<float>(cb, d, res);
+#pragma unroll
+      for (int e = 0; e < 12; e++) res[e] *= a.scale;
+    } else if (EPI == 2) {
+      clover_block<float>(cb, xv, res);
+#pragma unroll
+      for (int e = 0; e < 12; e++) res[e] += a.scale * d[e];
+    } else if (EPI == 3) {
+      float y[12];
+      clover_block<float>(cb, d, y);
+#pragma unroll
+      for (int e = 0; e < 12; e++) res[e] = xv[e] + a.scale * y[e];
+    } else {
+#pragma unroll
+      for (int e = 0; e < 12; e++) res[e] = xv[e] + a.scale * d[e];
+    }
+    float4* op = reinterpret_cast<float4*>(a.out + (size_t)c * a.stride + hoff);
+#pragma unroll
+    for (int v = 0; v < 3; v++) op[(size_t)v * Vh] = make_float4(res[4 * v], res[4 * v + 1], res[4 * v + 2], res[4 * v + 3]);
+    // refill: column c + NST goes into the stage just read, once every warp has let go of it.  The warps take turns
+    // (warp c mod NW), so the wait and the issue cost each warp one column in NW.
+    if (c + NST < a.nrhs && warp == c % NW) {
+      mbar_wait(&bars[NST + st], ph);
+      if (lane == 0) issue_stage<TS>(stage0 + st * TS::STAGE_BYTES, maps, L, y0, z0, t0, c + NST, &bars[st]);
+      __syncwarp();
+    }
+  }
+}
+
+template <typename TS, int R, bool DAG, int EPI>
+__global__ void __launch_bounds__(TS::NCONS, 1) dslash_mrhs_tma_kernel(const __grid_constant__ TmaMaps maps, const TmaArgs a) {
+  constexpr int TY = TS::TY, TZ = TS::TZ, TT = TS::TT, NS = TS::NS;
+  extern __shared__ __align__(1024) unsigned char tma_smem[];
+  unsigned char* stage0 = tma_smem;                                                // NST stages of the input tile
+  float4* xbuf = reinterpret_cast<float4*>(tma_smem + NST * TS::STAGE_BYTES);      // exchange: [2][2 roles][3][NS]
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(xbuf + 2 * 2 * 3 * NS);  // full[NST], empty[NST]
+  const Lat& L = a.lat;
+  // tile of this block: y fastest, then z inside a slab, then t, then the slab
+  const int nty = L.Ly / TY, ntt = L.Lt / TT;
+  int b = blockIdx.x;
+  const int ty = b % nty;
+  b /= nty;
+  const int tzi = b % a.zslab;
+  b /= a.zslab;
+  const int tt = b % ntt;
+  const int tz = (b / ntt) * a.zslab + tzi;
+  const int y0 = ty * TY, z0 = tz * TZ, t0 = tt * TT;
+  const int tid = threadIdx.x;
+  if (tid == 0) {
+    for (int s = 0; s < NST; s++) {
+      mbar_init(&bars[s], 1);                     // full: the issuing thread's arrive.expect_tx (+ the TMA bytes)
+      mbar_init(&bars[NST + s], TS::NCONS / 32);  // empty: one arrival per warp
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    // first fill: the first NST columns, no stage to wait for
+    for (int c = 0; c < NST && c < a.nrhs; c++) issue_stage<TS>(stage0 + c * TS::STAGE_BYTES, &maps, L, y0, z0, t0, c, &bars[c]);
+  }
+  __syncthreads();
+  if (tid < NS) consume<TS, R, DAG, EPI, 0>(&maps, a, stage0, xbuf, bars, y0, z0, t0);
+  else consume<TS, R, DAG, EPI, 1>(&maps, a, stage0, xbuf, bars, y0, z0, t0);
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+    else
+      cudaGetLastError();
+  }
+  return fn;
+}
+
+// tensor maps of nrhs consecutive one-parity native fp32 spinors seen as {x: 4*Lxh floats, y, z, t, vector: 6*nrhs},
+// one per box shape
+template <typename TS>
+bool make_maps(TmaMaps* m, const void* in, const Lat& L, int nrhs) {
+  EncodeTiledFn enc = encode_fn();
+  if (!enc) return false;
+  const cuuint64_t dims[5] = {(cuuint64_t)4 * L.Lxh, (cuuint64_t)L.Ly, (cuuint64_t)L.Lz, (cuuint64_t)L.Lt, (cuuint64_t)6 * nrhs};
+  const cuuint64_t row = (cuuint64_t)16 * L.Lxh;
+  const cuuint64_t strides[4] = {row, row * L.Ly, row * L.Ly * L.Lz, (cuuint64_t)16 * L.Vh};
+  const cuuint32_t es[5] = {1, 1, 1, 1, 1};
+  const cuuint32_t X = 4 * TS::LXH;
+  const cuuint32_t boxes[4][5] = {{X, TS::TY, TS::TZ, TS::TT, 6}, {X, 1, TS::TZ, TS::TT, 6}, {X, TS::TY, 1, TS::TT, 6}, {X, TS::TY, TS::TZ, 1, 6}};
+  CUtensorMap* out[4] = {&m->core, &m->yface, &m->zface, &m->tface};
+  for (int i = 0; i < 4; i++)
+    if (enc(out[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, const_cast<void*>(in), dims, strides, boxes[i], es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return false;
+  return true;
+}
+
+template <typename TS> constexpr size_t smem_bytes() {
+  return (size_t)NST * TS::STAGE_BYTES + (size_t)2 * 2 * 3 * TS::NS * 16 + 2 * NST * 8;
+}
+
+template <typename TS, int R, bool DAG>
+void launch_tma(const TmaMaps& map, const TmaArgs& a, int epi, int device, cudaStream_t st) {
+  const int grid = (a.lat.Ly / TS::TY) * (a.lat.Lz / TS::TZ) * (a.lat.Lt / TS::TT);
+  const size_t smem = smem_bytes<TS>();
+  static bool configured[LQCD_MAX_DEVICES] = {};
+  if (!configured[device]) {
+    cudaFuncSetAttribute(dslash_mrhs_tma_kernel<TS, R, DAG, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_mrhs_tma_kernel<TS, R, DAG, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_mrhs_tma_kernel<TS, R, DAG, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_mrhs_tma_kernel<TS, R, DAG, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_mrhs_tma_kernel<TS, R, DAG, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    configured[device] = true;
+  }
+  switch (epi) {
+    case 0: dslash_mrhs_tma_kernel<TS, R, DAG, 0><<<grid, TS::NCONS, smem, st>>>(map, a); break;
+    case 1: dslash_mrhs_tma_kernel<TS, R, DAG, 1><<<grid, TS::NCONS, smem, st>>>(map, a); break;
+    case 2: dslash_mrhs_tma_kernel<TS, R, DAG, 2><<<grid, TS::NCONS, smem, st>>>(map, a); break;
+    case 3: dslash_mrhs_tma_kernel<TS, R, DAG, 3><<<grid, TS::NCONS, smem, st>>>(map, a); break;
+    default: dslash_mrhs_tma_kernel<TS, R, DAG, 6><<<grid, TS::NCONS, smem, st>>>(map, a); break;
+  }
+}
+
+template <typename TS>
+void launch_tile(const TmaMaps& map, const TmaArgs& a, int recon, int dagger, int epi, int device, cudaStream_t st) {
+  if (recon == 18) {
+    if (dagger) launch_tma<TS, 18, true>(map, a, epi, device, st);
+    else launch_tma<TS, 18, false>(map, a, epi, device, st);
+  } else {
+    if (dagger) launch_tma<TS, 12, true>(map, a, epi, device, st);
+    else launch_tma<TS, 12, false>(map, a, epi, device, st);
+  }
+}
+
+// tiles: 128 output sites = 256 consumer threads at both row lengths
+typedef RowTile<16, 2, 2, 2> Tile16;  // 32^3 x 64 : 32 staged rows per column (4.0 fetches per spinor)
+typedef RowTile<8, 4, 2, 2> Tile8;    // 16^3 x 32 : 56 staged rows per column (3.5 fetches per spinor)
+
+template <typename TS> bool tile_divides(const Lat& L) {
+  return L.Lxh == TS::LXH && L.Ly % TS::TY == 0 && L.Lz % TS::TZ == 0 && L.Lt % TS::TT == 0;
+}
+
+}  // namespace
+
+// fp32, the epilogues without a reduction, and a lattice whose x-rows are 16 or 8 checkerboard sites long and whose
+// other extents the tile divides; LQCD_MRHS_TMA=0 (read at context creation) keeps the kernels of dslash_mrhs.cu
+bool lqcd_mrhs_tma_ok(const lqcd_ctx* c, int epi) {
+  if (!c->mrhs_tma || c->prec != 4 || !(epi <= 3 || epi == 6)) return false;
+  return (tile_divides<Tile16>(c->lat) || tile_divides<Tile8>(c->lat)) && encode_fn() != nullptr;
+}
+
+int lqcd_dslash_mrhs_tma_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
+                                int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st) {
+  TmaMaps map;
+  const bool t16 = tile_divides<Tile16>(c->lat);
+  if (!(t16 ? make_maps<Tile16>(&map, in, c->lat, nrhs) : make_maps<Tile8>(&map, in, c->lat, nrhs)))
+    return lqcd_set_error(c, LQCD_ERR_CUDA, "dslash_mrhs_tma: cuTensorMapEncodeTiled failed");
+  TmaArgs a;
+  a.out = (float*)out;
+  a.gauge = (const float*)gauge;
+  a.cl = (const float*)cl;
+  a.x = (const float*)x;
+  a.lat = c->lat;
+  a.parity = parity;
+  a.nrhs = nrhs;
+  a.scale = (float)scale;
+  a.ws = (float)c->ws;
+  a.stride = (size_t)24 * c->lat.Vh;
+  if (t16) {
+    const int ntz = c->lat.Lz / Tile16::TZ;
+    a.zslab = (c->mrhs_zslab > 0 && ntz % c->mrhs_zslab == 0) ? c->mrhs_zslab : ntz;
+    launch_tile<Tile16>(map, a, c->recon, dagger, epi, c->device, st);
+  } else {
+    const int ntz = c->lat.Lz / Tile8::TZ;
+    a.zslab = (c->mrhs_zslab > 0 && ntz % c->mrhs_zslab == 0) ? c->mrhs_zslab : ntz;
+    launch_tile<Tile8>(map, a, c->recon, dagger, epi, c->device, st);
+  }
+  return LQCD_OK;
+}

@@ -25,7 +25,8 @@ struct lqcd_ctx {
   long V;
   int prec, recon, device, sm_count;
   double ws;  // weight of the spatial hops: nu/xi_0 of Eq. 5; 1 = isotropic
-  int mrhs_tiled;  // 1: tiled multi-RHS kernel (dslash_mrhs_tiled.cu) where its tile divides the lattice (fp32)
+  int mrhs_tma;    // 1 (default): TMA-tiled multi-RHS kernel (dslash_mrhs_tma.cu) where it applies; LQCD_MRHS_TMA=0 turns it off
+  int mrhs_zslab;  // z-tiles per slab of its sweep (LQCD_MRHS_ZSLAB; 0 = the whole z extent)
   int tiled;  // 1: shared-memory tiled dslash where the tile divides the lattice (opt-in: LQCD_DSLASH_TILED=1)
   long launches;
   char err[256];
@@ -245,9 +246,9 @@ int lqcd_dslash_fused_launch(lqcd_ctx* c, void* out, const void* in, const void*
                              int parity, double scale, int dagger, int epi, const DslashFuse* f, cudaStream_t st);
 int lqcd_dslash_mrhs_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
                             int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st);
-bool lqcd_mrhs_tiled_ok(const lqcd_ctx* c);
-void lqcd_dslash_mrhs_tiled_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
-                                   int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st);
+bool lqcd_mrhs_tma_ok(const lqcd_ctx* c, int epi);
+int lqcd_dslash_mrhs_tma_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
+                                int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st);
 int lqcd_clover_apply_launch(lqcd_ctx* c, void* out, const void* in, const void* cl_parity, int nrhs, cudaStream_t st);
 int lqcd_spinor_pack_parity(lqcd_ctx* c, void* native, const void* pub, cudaStream_t st);
 int lqcd_spinor_unpack_parity(lqcd_ctx* c, void* pub, const void* native, cudaStream_t st);
