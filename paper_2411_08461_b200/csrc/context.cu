@@ -79,7 +79,7 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], int prec, int recon, int t_bo
     const char* e = getenv("LQCD_DSLASH_TILED");
     c->tiled = (e && e[0] == '1') ? 1 : 0;
     const char* m = getenv("LQCD_MRHS_TMA");  // TMA-tiled multi-RHS kernel: on unless LQCD_MRHS_TMA=0 (A/B measurements, parity tests of both)
-    c->mrhs_tma = (m && m[0] == '0') ? 0 : 1;
+    c->mrhs_tma = (m && m[0] == '0') ? 0 : ((m && m[0] == '2') ? 2 : 1);
     const char* z = getenv("LQCD_MRHS_ZSLAB");
     c->mrhs_zslab = z ? atoi(z) : 4;
   }

@@ -7,10 +7,12 @@
 // and column on the shared-memory pipe).  This kernel removes both:
 //   * a block owns a tile of TY x TZ x TT full x-rows of output sites (LXH checkerboard sites each) and walks the
 //     columns one after the other; the input spinors of the tile + its one-site halo in y, z, t (x wraps inside a
-//     full row) are brought to shared memory ONCE per column by the TMA unit (cp.async.bulk.tensor, one 3-D box
-//     {row, 6 vectors} per x-row, issued by the lanes of a producer warp, completion on an mbarrier), into a ring of
-//     NST stages: while the consumer warps multiply column c from stage s, column c+1 is already in flight.  Crossbar
-//     traffic per site and column: NROWS/RC x 96 B (384 B at 32^3x64, 336 B at 16^3x32) instead of 768 B;
+//     full row) are brought to shared memory ONCE per column by the TMA unit (cp.async.bulk.tensor: seven 5-D boxes
+//     {x, y, z, t, 6 vectors} per column -- the core and the six faces -- issued by one thread, completion on an
+//     mbarrier), into a ring of NST stages: while the warps multiply column c from stage s, the next columns are in
+//     flight; the warps take turns at refilling.  (One box per x-row, 32 per column, cost the issuing warp 3200 cycles
+//     a column: the TMA instruction takes uniform registers, so a warp issues its lanes' boxes one by one.)  Crossbar
+//     traffic per site and column: staged rows / output rows x 96 B (384-480 B at 32^3x64) instead of 768 B;
 //   * a site is split over TWO threads of different warps: role 0 does the hops +-x, +-y and the upper chiral block,
 //     role 1 the hops +-z, +-t and the lower chiral block.  Each keeps ITS four links (72 registers) and its 6x6
 //     clover block (36 registers) in registers for all columns, so links and clover cost no bytes per column at all.
@@ -27,8 +29,10 @@
 
 namespace {
 
-template <int LXH_, int TY_, int TZ_, int TT_> struct RowTile {
+template <int LXH_, int TY_, int TZ_, int TT_, int NST_, int MINB_> struct RowTile {
   static constexpr int LXH = LXH_, TY = TY_, TZ = TZ_, TT = TT_;
+  static constexpr int NST = NST_;    // ring stages: NST - 1 columns in flight while one is multiplied
+  static constexpr int MINB = MINB_;  // resident blocks per SM the register budget is cut for
   static constexpr int RC = TY * TZ * TT;                      // core rows = output rows
   static constexpr int NS = LXH * RC;                          // output sites per tile
   static constexpr int NYH = TZ * TT, NZH = TY * TT, NTH = TY * TZ;  // rows of one halo face
@@ -41,7 +45,6 @@ template <int LXH_, int TY_, int TZ_, int TT_> struct RowTile {
   static constexpr int STAGE_BYTES = B_TP + 6 * VS_T;
   static constexpr int NCONS = 2 * NS;                         // threads: two per site
 };
-constexpr int NST = 3;  // ring stages: two columns in flight while one is multiplied
 
 struct TmaArgs {
   float* out;
@@ -132,7 +135,7 @@ __device__ __forceinline__ void hop_sm(float* acc, const unsigned char* sp, int 
 template <typename TS, int R, bool DAG, int EPI, int ROLE>
 __device__ __forceinline__ void consume(const TmaMaps* maps, const TmaArgs& a, unsigned char* stage0, float4* xbuf,
                                         unsigned long long* bars, int y0, int z0, int t0) {
-  constexpr int LXH = TS::LXH, TY = TS::TY, TZ = TS::TZ, TT = TS::TT, NS = TS::NS, NW = TS::NCONS / 32;
+  constexpr int LXH = TS::LXH, TY = TS::TY, TZ = TS::TZ, TT = TS::TT, NS = TS::NS, NW = TS::NCONS / 32, NST = TS::NST;
   constexpr bool CLOVER = EPI == 1 || EPI == 2 || EPI == 3;
   const Lat& L = a.lat;
   const int Vh = L.Vh, par = a.parity;
@@ -268,8 +271,8 @@ __device__ __forceinline__ void consume(const TmaMaps* maps, const TmaArgs& a, u
 }
 
 template <typename TS, int R, bool DAG, int EPI>
-__global__ void __launch_bounds__(TS::NCONS, 1) dslash_mrhs_tma_kernel(const __grid_constant__ TmaMaps maps, const TmaArgs a) {
-  constexpr int TY = TS::TY, TZ = TS::TZ, TT = TS::TT, NS = TS::NS;
+__global__ void __launch_bounds__(TS::NCONS, TS::MINB) dslash_mrhs_tma_kernel(const __grid_constant__ TmaMaps maps, const TmaArgs a) {
+  constexpr int TY = TS::TY, TZ = TS::TZ, TT = TS::TT, NS = TS::NS, NST = TS::NST;
   extern __shared__ __align__(1024) unsigned char tma_smem[];
   unsigned char* stage0 = tma_smem;                                                // NST stages of the input tile
   float4* xbuf = reinterpret_cast<float4*>(tma_smem + NST * TS::STAGE_BYTES);      // exchange: [2][2 roles][3][NS]
@@ -341,65 +344,97 @@ bool make_maps(TmaMaps* m, const void* in, const Lat& L, int nrhs) {
 }
 
 template <typename TS> constexpr size_t smem_bytes() {
-  return (size_t)NST * TS::STAGE_BYTES + (size_t)2 * 2 * 3 * TS::NS * 16 + 2 * NST * 8;
+  return (size_t)TS::NST * TS::STAGE_BYTES + (size_t)2 * 2 * 3 * TS::NS * 16 + 2 * TS::NST * 8;
 }
 
-template <typename TS, int R, bool DAG>
-void launch_tma(const TmaMaps& map, const TmaArgs& a, int epi, int device, cudaStream_t st) {
+template <typename TS, int R, bool DAG, int EPI>
+void launch_one(const TmaMaps& map, const TmaArgs& a, int device, cudaStream_t st) {
   const int grid = (a.lat.Ly / TS::TY) * (a.lat.Lz / TS::TZ) * (a.lat.Lt / TS::TT);
   const size_t smem = smem_bytes<TS>();
-  static bool configured[LQCD_MAX_DEVICES] = {};
+  static bool configured[LQCD_MAX_DEVICES] = {};  // per instantiation and device
   if (!configured[device]) {
-    cudaFuncSetAttribute(dslash_mrhs_tma_kernel<TS, R, DAG, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaFuncSetAttribute(dslash_mrhs_tma_kernel<TS, R, DAG, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaFuncSetAttribute(dslash_mrhs_tma_kernel<TS, R, DAG, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaFuncSetAttribute(dslash_mrhs_tma_kernel<TS, R, DAG, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaFuncSetAttribute(dslash_mrhs_tma_kernel<TS, R, DAG, 6>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_mrhs_tma_kernel<TS, R, DAG, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     configured[device] = true;
   }
-  switch (epi) {
-    case 0: dslash_mrhs_tma_kernel<TS, R, DAG, 0><<<grid, TS::NCONS, smem, st>>>(map, a); break;
-    case 1: dslash_mrhs_tma_kernel<TS, R, DAG, 1><<<grid, TS::NCONS, smem, st>>>(map, a); break;
-    case 2: dslash_mrhs_tma_kernel<TS, R, DAG, 2><<<grid, TS::NCONS, smem, st>>>(map, a); break;
-    case 3: dslash_mrhs_tma_kernel<TS, R, DAG, 3><<<grid, TS::NCONS, smem, st>>>(map, a); break;
-    default: dslash_mrhs_tma_kernel<TS, R, DAG, 6><<<grid, TS::NCONS, smem, st>>>(map, a); break;
-  }
+  dslash_mrhs_tma_kernel<TS, R, DAG, EPI><<<grid, TS::NCONS, smem, st>>>(map, a);
 }
 
-template <typename TS>
-void launch_tile(const TmaMaps& map, const TmaArgs& a, int recon, int dagger, int epi, int device, cudaStream_t st) {
+template <typename TS, int EPI>
+void launch_tile(const TmaMaps& map, const TmaArgs& a, int recon, int dagger, int device, cudaStream_t st) {
   if (recon == 18) {
-    if (dagger) launch_tma<TS, 18, true>(map, a, epi, device, st);
-    else launch_tma<TS, 18, false>(map, a, epi, device, st);
+    if (dagger) launch_one<TS, 18, true, EPI>(map, a, device, st);
+    else launch_one<TS, 18, false, EPI>(map, a, device, st);
   } else {
-    if (dagger) launch_tma<TS, 12, true>(map, a, epi, device, st);
-    else launch_tma<TS, 12, false>(map, a, epi, device, st);
+    if (dagger) launch_one<TS, 12, true, EPI>(map, a, device, st);
+    else launch_one<TS, 12, false, EPI>(map, a, device, st);
   }
 }
 
-// tiles: 128 output sites = 256 consumer threads at both row lengths
-typedef RowTile<16, 2, 2, 2> Tile16;  // 32^3 x 64 : 32 staged rows per column (4.0 fetches per spinor)
-typedef RowTile<8, 4, 2, 2> Tile8;    // 16^3 x 32 : 56 staged rows per column (3.5 fetches per spinor)
+// Tile shapes (sweep at 32^3x64, 12 columns, profiles/r02_mrhs_README.md).  Without a clover block a thread fits 168
+// registers, so three 64-site blocks share an SM (12 warps; 2 stages each): 707 us against 812 us for one 128-site
+// block (8 warps).  With the clover block in registers (210-216) only 8 warps fit; one 128-site block, 3 stages.
+typedef RowTile<16, 2, 2, 1, 2, 3> Tile16;   // epilogues 0, 6: 20 staged rows per 4 output rows
+#ifndef TMA_C_TILE
+#define TMA_C_TILE 16, 2, 2, 2, 3, 1
+#endif
+typedef RowTile<TMA_C_TILE> Tile16C;  // epilogues 1, 2, 3: 32 staged rows per 8 output rows
+typedef RowTile<8, 4, 2, 2, 3, 1> Tile8;     // x-rows of 8 (16^3x32): 56 staged rows per 16; opt-in, see lqcd_mrhs_tma_ok
 
 template <typename TS> bool tile_divides(const Lat& L) {
   return L.Lxh == TS::LXH && L.Ly % TS::TY == 0 && L.Lz % TS::TZ == 0 && L.Lt % TS::TT == 0;
 }
 
+template <typename TS>
+int launch_any(lqcd_ctx* c, TmaArgs& a, const void* in, int dagger, int epi, int nrhs, cudaStream_t st) {
+  TmaMaps map;
+  if (!make_maps<TS>(&map, in, c->lat, nrhs)) return lqcd_set_error(c, LQCD_ERR_CUDA, "dslash_mrhs_tma: cuTensorMapEncodeTiled failed");
+  const int ntz = c->lat.Lz / TS::TZ;
+  a.zslab = (c->mrhs_zslab > 0 && ntz % c->mrhs_zslab == 0) ? c->mrhs_zslab : ntz;
+  switch (epi) {
+    case 0: launch_tile<TS, 0>(map, a, c->recon, dagger, c->device, st); break;
+    case 1: launch_tile<TS, 1>(map, a, c->recon, dagger, c->device, st); break;
+    case 2: launch_tile<TS, 2>(map, a, c->recon, dagger, c->device, st); break;
+    case 3: launch_tile<TS, 3>(map, a, c->recon, dagger, c->device, st); break;
+    default: launch_tile<TS, 6>(map, a, c->recon, dagger, c->device, st); break;
+  }
+  return LQCD_OK;
+}
+// the tile types are instantiated for the epilogues they serve only
+template <typename TS>
+int launch_noclover(lqcd_ctx* c, TmaArgs& a, const void* in, int dagger, int epi, int nrhs, cudaStream_t st) {
+  TmaMaps map;
+  if (!make_maps<TS>(&map, in, c->lat, nrhs)) return lqcd_set_error(c, LQCD_ERR_CUDA, "dslash_mrhs_tma: cuTensorMapEncodeTiled failed");
+  const int ntz = c->lat.Lz / TS::TZ;
+  a.zslab = (c->mrhs_zslab > 0 && ntz % c->mrhs_zslab == 0) ? c->mrhs_zslab : ntz;
+  if (epi == 0) launch_tile<TS, 0>(map, a, c->recon, dagger, c->device, st);
+  else launch_tile<TS, 6>(map, a, c->recon, dagger, c->device, st);
+  return LQCD_OK;
+}
+template <typename TS>
+int launch_clover(lqcd_ctx* c, TmaArgs& a, const void* in, int dagger, int epi, int nrhs, cudaStream_t st) {
+  TmaMaps map;
+  if (!make_maps<TS>(&map, in, c->lat, nrhs)) return lqcd_set_error(c, LQCD_ERR_CUDA, "dslash_mrhs_tma: cuTensorMapEncodeTiled failed");
+  const int ntz = c->lat.Lz / TS::TZ;
+  a.zslab = (c->mrhs_zslab > 0 && ntz % c->mrhs_zslab == 0) ? c->mrhs_zslab : ntz;
+  if (epi == 1) launch_tile<TS, 1>(map, a, c->recon, dagger, c->device, st);
+  else if (epi == 2) launch_tile<TS, 2>(map, a, c->recon, dagger, c->device, st);
+  else launch_tile<TS, 3>(map, a, c->recon, dagger, c->device, st);
+  return LQCD_OK;
+}
+
 }  // namespace
 
-// fp32, the epilogues without a reduction, and a lattice whose x-rows are 16 or 8 checkerboard sites long and whose
-// other extents the tile divides; LQCD_MRHS_TMA=0 (read at context creation) keeps the kernels of dslash_mrhs.cu
+// fp32 and the epilogues without a reduction.  LQCD_MRHS_TMA (read at context creation): 1 (default) = where it was
+// measured faster than the kernels of dslash_mrhs.cu, i.e. x-rows of 16 checkerboard sites (32^3x64; at 16^3x32 the
+// two are within 5 % and the older kernel wins); 2 = wherever a tile divides the lattice (parity tests); 0 = never.
 bool lqcd_mrhs_tma_ok(const lqcd_ctx* c, int epi) {
-  if (!c->mrhs_tma || c->prec != 4 || !(epi <= 3 || epi == 6)) return false;
-  return (tile_divides<Tile16>(c->lat) || tile_divides<Tile8>(c->lat)) && encode_fn() != nullptr;
+  if (!c->mrhs_tma || c->prec != 4 || !(epi <= 3 || epi == 6) || encode_fn() == nullptr) return false;
+  if (tile_divides<Tile16>(c->lat) && tile_divides<Tile16C>(c->lat)) return true;
+  return c->mrhs_tma == 2 && tile_divides<Tile8>(c->lat);
 }
 
 int lqcd_dslash_mrhs_tma_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
                                 int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st) {
-  TmaMaps map;
-  const bool t16 = tile_divides<Tile16>(c->lat);
-  if (!(t16 ? make_maps<Tile16>(&map, in, c->lat, nrhs) : make_maps<Tile8>(&map, in, c->lat, nrhs)))
-    return lqcd_set_error(c, LQCD_ERR_CUDA, "dslash_mrhs_tma: cuTensorMapEncodeTiled failed");
   TmaArgs a;
   a.out = (float*)out;
   a.gauge = (const float*)gauge;
@@ -411,14 +446,10 @@ int lqcd_dslash_mrhs_tma_launch(lqcd_ctx* c, void* out, const void* in, const vo
   a.scale = (float)scale;
   a.ws = (float)c->ws;
   a.stride = (size_t)24 * c->lat.Vh;
-  if (t16) {
-    const int ntz = c->lat.Lz / Tile16::TZ;
-    a.zslab = (c->mrhs_zslab > 0 && ntz % c->mrhs_zslab == 0) ? c->mrhs_zslab : ntz;
-    launch_tile<Tile16>(map, a, c->recon, dagger, epi, c->device, st);
-  } else {
-    const int ntz = c->lat.Lz / Tile8::TZ;
-    a.zslab = (c->mrhs_zslab > 0 && ntz % c->mrhs_zslab == 0) ? c->mrhs_zslab : ntz;
-    launch_tile<Tile8>(map, a, c->recon, dagger, epi, c->device, st);
+  a.zslab = 1;
+  if (tile_divides<Tile16>(c->lat) && tile_divides<Tile16C>(c->lat)) {
+    if (epi == 0 || epi == 6) return launch_noclover<Tile16>(c, a, in, dagger, epi, nrhs, st);
+    return launch_clover<Tile16C>(c, a, in, dagger, epi, nrhs, st);
   }
-  return LQCD_OK;
+  return launch_any<Tile8>(c, a, in, dagger, epi, nrhs, st);
 }

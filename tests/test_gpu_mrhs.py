@@ -180,6 +180,7 @@ def test_tma_mrhs_kernel_matches_oracle(dims, zslab, recon, monkeypatch):
     change roles), dagger, both parities, every epilogue through the three Schur forms -- against the oracle, and
     against the kernels of dslash_mrhs.cu (LQCD_MRHS_TMA=0) which must give the same field to rounding."""
     monkeypatch.setenv("LQCD_MRHS_ZSLAB", zslab)
+    monkeypatch.setenv("LQCD_MRHS_TMA", "2")  # also where it is not the default (x-rows of 8)
     s = Setup(dims, 0.5, 2, 0.124, 1.2, 4, recon, -1)
     monkeypatch.setenv("LQCD_MRHS_TMA", "0")
     ref = lq().Context(dims, 4, recon, -1)
