@@ -125,6 +125,60 @@ def oracle_sample(steps, warmup):
     return gbs, dt * 1e3, oracle.threads()
 
 
+def oracle_legs(config, n_apply, iters):
+    """The oracle as it stands on the host cores (SURVEY.md §8(d) "CPU baseline"; invert is where the
+    time goes): clover build, hopping term, clover apply and the even-odd CGNE solve (asymmetric Schur complement,
+    the oracle's own) at BASELINE config `config`.  The solve is timed for iters[0] and iters[1] iterations; the
+    difference gives seconds per iteration (prepare, reconstruction and true residual cancel)."""
+    import oracle
+    from paper_2411_08461_b200 import synth
+    cfg = synth.CONFIGS[config]
+    dims = cfg["dims"]
+    U = synth.gauge(dims, cfg["eps"], cfg["seed"])
+    psi = synth.source(dims, "gaussian", cfg["src_seed"])
+    orc = oracle.Oracle(dims, U, -1)
+    del U
+    t0 = time.perf_counter()
+    orc.set_clover(cfg["kappa"], cfg["csw"])
+    t_build = time.perf_counter() - t0
+    orc.dslash(psi)
+    t0 = time.perf_counter()
+    for _ in range(n_apply):
+        orc.dslash(psi)
+    t_d = (time.perf_counter() - t0) / n_apply
+    t0 = time.perf_counter()
+    for _ in range(n_apply):
+        orc.clover_apply(psi)
+    t_c = (time.perf_counter() - t0) / n_apply
+    ts = []
+    for n in iters:
+        t0 = time.perf_counter()
+        orc.invert(psi, 1e-10, n, "cgne", 0)
+        ts.append(time.perf_counter() - t0)
+    V = int(np.prod(dims))
+    per_it = (ts[1] - ts[0]) / (iters[1] - iters[0])
+    return {"config": config, "dims": list(dims), "threads": oracle.threads(),
+            "clover_build_s": t_build,
+            "dslash_full_lattice_ms": t_d * 1e3, "dslash_GBps": 2 * dslash_alg_bytes(18, 8, V // 2) / t_d / 1e9,
+            "clover_apply_full_lattice_ms": t_c * 1e3, "clover_apply_GBps": 120 * 8 * V / t_c / 1e9,
+            "cgne_seconds_per_iteration": per_it, "cgne_timed_iterations": list(iters),
+            "cgne_fixed_seconds": ts[0] - iters[0] * per_it}
+
+
+def oracle_leg_subprocess(config, n_apply, iters, threads=None):
+    """oracle_legs in a child process (OMP_NUM_THREADS must be set before the oracle library loads)."""
+    env = dict(os.environ)
+    if threads is not None:
+        env["OMP_NUM_THREADS"] = str(threads)
+    cmd = [sys.executable, os.path.abspath(__file__), "--impl", "cpu-leg", "--cpu-leg",
+           "%d,%d,%d,%d" % (config, n_apply, iters[0], iters[1])]
+    out = subprocess.run(cmd, env=env, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True, timeout=900)
+    for ln in reversed(out.stdout.strip().splitlines()):
+        if ln.startswith("{"):
+            return json.loads(ln)
+    return {"error": (out.stderr or out.stdout)[-300:]}
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -355,6 +409,34 @@ def extras(torch, lqcd, synth, U, b, ctx, gauge, device):
     return out
 
 
+def small_solves(torch, lqcd, synth, device):
+    """Solve wall time at BASELINE configs 1-3 (the lattices that fit in L2, where the host's share of an iteration
+    shows): device seconds of the whole lqcd_invert call (CUDA events inside the library), iterations, launches."""
+    out = {}
+    runs = ((1, 8, 18, "point", "cgne", 0, 1e-10), (2, 8, 18, "z2", "bicgstab", 1, 1e-10), (2, 4, 18, "z2", "bicgstab", 1, 1e-6),
+            (3, 4, 12, "gaussian", "cgne", MATPC, 1e-6), (3, 4, 12, "gaussian", "bicgstab", 1, 1e-6))
+    for n, prec, recon, kind, solver, matpc, tol in runs:
+        c = synth.CONFIGS[n]
+        U = synth.gauge(c["dims"], c["eps"], c["seed"])
+        b = synth.source(c["dims"], kind, c["src_seed"])
+        ctx = lqcd.Context(c["dims"], prec, recon, -1, device)
+        g = ctx.gauge_pack(ctx.to_device(U))
+        A, Ai = ctx.clover_build(g, c["csw"], c["kappa"])
+        bd = ctx.to_device(b)
+        ws, _ = ctx.workspace(solver)
+        best = None
+        for _ in range(5):
+            _, r = ctx.invert(bd, g, A, Ai, c["kappa"], tol=tol, maxiter=2000, solver=solver, matpc=matpc, workspace=ws)
+            if best is None or r.seconds < best.seconds:
+                best = r
+        out["config%d_fp%d_recon%d_%s" % (n, 8 * prec, recon, solver)] = {
+            "dims": list(c["dims"]), "tol": tol, "matpc": matpc, "us": best.seconds * 1e6, "iterations": best.iterations,
+            "us_per_iteration": best.seconds * 1e6 / max(best.iterations, 1), "kernel_launches": best.kernel_launches,
+            "true_resid": best.true_resid, "status": best.status}
+        ctx.close()
+    return out
+
+
 def reduce_over_ranks(dist, dt, sums, device):
     """Multi-replica aggregation: MAX of the device time over ranks, SUM of the work counters.
     dist = torch.distributed (initialised) or None for a single process."""
@@ -461,7 +543,57 @@ def run_gpu(args):
            "d2h_bytes_per_step": int(x_h.numel() * 16), "ms_per_step": dt2 / n_e2e * 1e3,
            "true_resid": r2.true_resid}
 
-    line = {
+    # The driver keeps the standard keys (roofline, cpu_baseline, e2e, config, clocks) and only the NAMES of the others,
+    # and it stores the tail of stdout: the large blocks come first in the line, and the figures the targets are stated
+    # on are repeated, compact, inside `roofline` and `cpu_baseline`.
+    line = {}
+    roofline = {"bound": "hbm", "achieved": ds_bytes / (ds_ms * 1e-3) / 1e9 if ds_ms > 0 else None,
+                "peak": peak, "unit": "GB/s",
+                "frac": (ds_bytes / (ds_ms * 1e-3) / 1e9 / peak) if ds_ms > 0 else None,
+                "traffic": traffic_from_profile(), "traffic_source": "committed ncu --set full capture under profiles/ (not this run)",
+                "kernel": "dslash_kernel<double,18,*,EPI 1|9|10> (fused clover and CG epilogues)",
+                "launches_timed": n_ds, "avg_launch_us": ds_ms * 1e3 / max(n_ds, 1),
+                "alg_bytes_per_launch": ds_bytes / max(n_ds, 1), "peak_source": peak_src,
+                "frac_of_8TBps": (ds_bytes / (ds_ms * 1e-3) / 8e12) if ds_ms > 0 else None,
+                "solve_32x64_fp64_cgne": {"seconds": res.seconds, "iterations": res.iterations, "true_resid": res.true_resid}}
+    cpu = None
+    if rank == 0 and not args.no_sweep:
+        line["dslash"] = dslash_sweep(torch, lqcd, U, b, dims, local, peak)
+        line["kernels"] = kernel_sweep(torch, lqcd, synth, U, b, dims, local, peak)
+        # north_star's target: Wilson-clover dslash at 32^3x64 in fp32 >= 70 % of HBM bandwidth
+        roofline["headline_dslash_fp32"] = {
+            k: {f: line["dslash"]["fp32_" + k][f] for f in ("us", "GBps", "frac_of_measured_peak", "frac_of_8TBps", "GFLOPs")}
+            for k in ("recon18", "recon12")}
+        roofline["clover_apply_frac"] = {k: line["kernels"][k]["clover_apply"]["frac_of_measured_peak"] for k in ("fp32", "fp64")}
+    if rank == 0 and world == 1 and not args.no_extras:
+        nr = extras(torch, lqcd, synth, U, b, ctx, gauge, local)
+        nr["dslash_mrhs_32x64"] = mrhs_sweep(torch, lqcd, U, b, dims, local, peak)
+        nr["small_lattice_solves"] = small_solves(torch, lqcd, synth, local)
+        line["next_rows"] = nr
+        roofline["dslash_mrhs_32x64_frac"] = {k: v["frac_of_measured_peak"] for k, v in nr["dslash_mrhs_32x64"].items()}
+        roofline["propagator_32x64_mixed_bicgstab_ms"] = nr["propagator_32x64_mixed_bicgstab"]["batched_ms"]
+        roofline["propagator_16x32_fp32_cgne_ms"] = nr["propagator_16x32_fp32_recon12"]["batched_ms"]
+        roofline["worst_true_resid_fp32_1e-6"] = max(nr["propagator_16x32_fp32_recon12"]["worst_true_resid"],
+                                                      nr["capacity_48x96_fp32_recon12"]["bicgstab_1e-6"]["true_resid"])
+    if rank == 0 and world == 1 and not args.no_cpu:
+        # the oracle on the host cores: all threads at the workload size, one thread at 16^3x32 (1/16 of the volume)
+        full = oracle_leg_subprocess(WORKLOAD, 3, (2, 5))
+        one = oracle_leg_subprocess(3, 2, (2, 4), threads=1)
+        # iterations of the oracle's own solve (asymmetric CGNE) = those of the GPU's (equal to +-1, tests/test_gpu_solvers.py)
+        ctx._check(lib.lqcd_gauge_pack(ctx.h, P(gauge), P(U_dev), S()))
+        _, ra = ctx.invert(b_dev, gauge, None, None, kappa, csw=csw, tol=tol, maxiter=2000, solver="cgne", matpc=0, workspace=ws)
+        est = None
+        if "error" not in full:
+            est = full["cgne_fixed_seconds"] + ra.iterations * full["cgne_seconds_per_iteration"]
+        cpu = {"value": full.get("dslash_GBps"), "unit": "GB/s", "cores": full.get("threads"), "kind": "oracle",
+               "sample": "32^3x64 fp64 on all host threads: clover build, 3 full-lattice hopping-term applications, 3 clover "
+                         "applies, even-odd CGNE (asymmetric) timed at 2 and 5 iterations; value = dslash algorithmic bytes / time",
+               "all_threads_32x64": full,
+               "cgne_solve_seconds_estimated": est,
+               "cgne_solve_estimate": "fixed + seconds/iteration x %d iterations (the GPU's count for the same asymmetric CGNE to 1e-10; "
+                                      "GPU: %.4f s)" % (ra.iterations, ra.seconds),
+               "one_thread_16x32": one}
+    line.update({
         "metric": METRIC, "value": value, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -473,29 +605,14 @@ def run_gpu(args):
                    "l2": "inputs larger than L2 (links 1.2 GB, clover 2x1.2 GB, spinors 0.2 GB each)",
                    "parallelism": "replicas only (one independent solve per GPU)",
                    "value_definition": "sum over all kernels of the step of their algorithmic HBM bytes / step time"},
-        "roofline": {"bound": "hbm", "achieved": ds_bytes / (ds_ms * 1e-3) / 1e9 if ds_ms > 0 else None,
-                     "peak": peak, "unit": "GB/s",
-                     "frac": (ds_bytes / (ds_ms * 1e-3) / 1e9 / peak) if ds_ms > 0 else None,
-                     "traffic": traffic_from_profile(), "kernel": "dslash_kernel<double,18,*,EPI 1|9|10> (fused clover and CG epilogues)",
-                     "launches_timed": n_ds, "avg_launch_us": ds_ms * 1e3 / max(n_ds, 1),
-                     "alg_bytes_per_launch": ds_bytes / max(n_ds, 1), "peak_source": peak_src,
-                     "frac_of_8TBps": (ds_bytes / (ds_ms * 1e-3) / 8e12) if ds_ms > 0 else None},
+        "roofline": roofline,
         "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "solve": {"solver": "cgne", "tol": tol, "iterations": res.iterations, "seconds": res.seconds,
                   "iter_resid": res.iter_resid, "true_resid": res.true_resid, "status": res.status,
                   "dslash_count": res.dslash_count, "kernel_launches": res.kernel_launches},
-    }
-    if rank == 0 and not args.no_sweep:
-        line["dslash"] = dslash_sweep(torch, lqcd, U, b, dims, local, peak)
-        line["kernels"] = kernel_sweep(torch, lqcd, synth, U, b, dims, local, peak)
-    if rank == 0 and world == 1 and not args.no_extras:
-        line["next_rows"] = extras(torch, lqcd, synth, U, b, ctx, gauge, local)
-        line["next_rows"]["dslash_mrhs_32x64"] = mrhs_sweep(torch, lqcd, U, b, dims, local, peak)
-    if rank == 0 and world == 1 and not args.no_cpu:
-        gbs, ms, cores = oracle_sample(12, 0)
-        line["cpu_baseline"] = {"value": gbs, "unit": "GB/s", "cores": cores, "kind": "oracle",
-                                "sample": "12 full-lattice fp64 hopping-term applications (24 parity sweeps) at 32^3x64; "
-                                          "algorithmic dslash bytes / time", "ms_per_application": ms}
+    })
+    if cpu is not None:
+        line["cpu_baseline"] = cpu
     if rank == 0:
         print(json.dumps(line))
     if dist is not None:
@@ -524,16 +641,58 @@ def traffic_from_profile():
     return None
 
 
+def spawn_command(args, port=None):
+    """`python bench.py --gpus N` outside torchrun: the same command line under torch.distributed.run, one rank per GPU."""
+    import socket
+    if port is None:
+        with socket.socket() as so:
+            so.bind(("127.0.0.1", 0))
+            port = so.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__),
+           "--gpus", str(args.gpus), "--steps", str(args.steps), "--warmup", str(args.warmup), "--impl", args.impl]
+    for flag, on in (("--no-sweep", args.no_sweep), ("--no-extras", args.no_extras), ("--no-cpu", args.no_cpu)):
+        if on:
+            cmd.append(flag)
+    return cmd
+
+
+def run_selftest(args):
+    """Launch plumbing only (tests/test_bench_dist.py): every rank joins a gloo group, rank 0 prints the world size."""
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        dist.init_process_group("gloo")
+        t = torch.ones(1)
+        dist.all_reduce(t)
+        world = int(t.item())
+    if int(os.environ.get("RANK", "0")) == 0:
+        print(json.dumps({"impl": "selftest", "n_gpus": world}))
+    if dist.is_initialized():
+        dist.destroy_process_group()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference", "cpu-leg", "selftest"])
+    ap.add_argument("--cpu-leg", default="", help="internal: config,applications,iters0,iters1 of one oracle leg")
     ap.add_argument("--no-sweep", action="store_true", help="skip the standalone dslash sweep")
     ap.add_argument("--no-extras", action="store_true", help="skip the SURVEY 8(f) rows (mixed precision, batched propagator)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the CPU-oracle baseline leg")
     args = ap.parse_args()
+    if args.impl == "cpu-leg":
+        c, n, i0, i1 = (int(v) for v in args.cpu_leg.split(","))
+        print(json.dumps(oracle_legs(c, n, (i0, i1))))
+        return 0
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return subprocess.call(spawn_command(args))  # N ranks, one per GPU; rank 0 prints the line with n_gpus = N
+    if args.impl == "selftest":
+        return run_selftest(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_gpu(args)

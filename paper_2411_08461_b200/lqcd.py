@@ -143,33 +143,44 @@ def sharded_solve(sources, solve, group=None):
     """The n independent columns of `sources` ([n, ...]) sharded over the ranks of a torch.distributed group
     (the 12 spin-colour columns of a propagator): links and clover are
     replicated, rank r solves the contiguous block shard_columns(n, r, world) with ONE batched call
-    `solve(block) -> (x, results, status)`, and one all-reduce of a buffer in which every column is owned by
-    exactly one rank (zero elsewhere) brings the solutions to every rank.  No collective on the data path of
-    the solves.  Returns (x [n, ...], iterations per column, worst status over the ranks)."""
+    `solve(block) -> (x, results, status)`, and one all-gather of the ranks' blocks (padded to the largest block, so
+    every rank sends ceil(n / world) columns, not n) brings the solutions to every rank.  No collective on the data
+    path of the solves.  Returns (x [n, ...], iterations per column, worst status over the ranks)."""
     import torch.distributed as dist
     on = dist.is_available() and dist.is_initialized()
     world = dist.get_world_size(group) if on else 1
     rank = dist.get_rank(group) if on else 0
     n = sources.shape[0]
     lo, hi = shard_columns(n, rank, world)
-    x_full = torch.zeros_like(sources)
-    iters = torch.zeros(n, dtype=torch.int64, device=sources.device)
+    width = -(-n // world)  # columns of the largest block
+    mine = torch.zeros((width,) + tuple(sources.shape[1:]), dtype=sources.dtype, device=sources.device)
+    my_it = torch.zeros(width, dtype=torch.int64, device=sources.device)
     rc = 0
     if hi > lo:
         x, res, rc = solve(sources[lo:hi])
-        x_full[lo:hi] = x
-        iters[lo:hi] = torch.tensor([r.iterations for r in res], dtype=torch.int64, device=sources.device)
+        mine[:hi - lo] = x
+        my_it[:hi - lo] = torch.tensor([r.iterations for r in res], dtype=torch.int64, device=sources.device)
+    if world == 1:
+        return mine[:n], my_it[:n].tolist(), rc
+    flat = torch.view_as_real(mine) if mine.is_complex() else mine
+    blocks = [torch.empty_like(flat) for _ in range(world)]
+    its = [torch.empty_like(my_it) for _ in range(world)]
+    dist.all_gather(blocks, flat.contiguous(), group=group)
+    dist.all_gather(its, my_it, group=group)
     worst = torch.tensor([min(rc, 0), max(rc, 0)], dtype=torch.int64, device=sources.device)
-    if world > 1:
-        flat = torch.view_as_real(x_full) if x_full.is_complex() else x_full
-        dist.all_reduce(flat, op=dist.ReduceOp.SUM, group=group)
-        dist.all_reduce(iters, op=dist.ReduceOp.SUM, group=group)
-        neg, pos = worst[:1].clone(), worst[1:].clone()
-        dist.all_reduce(neg, op=dist.ReduceOp.MIN, group=group)
-        dist.all_reduce(pos, op=dist.ReduceOp.MAX, group=group)
-        worst = torch.cat([neg, pos])
-    neg, pos = int(worst[0]), int(worst[1])
-    return x_full, iters.tolist(), (neg if neg < 0 else pos)
+    neg, pos = worst[:1].clone(), worst[1:].clone()
+    dist.all_reduce(neg, op=dist.ReduceOp.MIN, group=group)
+    dist.all_reduce(pos, op=dist.ReduceOp.MAX, group=group)
+    x_full = torch.empty_like(sources)
+    iters = []
+    for r in range(world):
+        l, h = shard_columns(n, r, world)
+        if h > l:
+            blk = torch.view_as_complex(blocks[r]) if sources.is_complex() else blocks[r]
+            x_full[l:h] = blk[:h - l]
+            iters += its[r][:h - l].tolist()
+    neg, pos = int(neg), int(pos)
+    return x_full, iters, (neg if neg < 0 else pos)
 
 
 class Context:

@@ -46,6 +46,24 @@ def test_reference_arm_nonzero_rank_prints_nothing():
     assert p.returncode == 0 and p.stdout.strip() == ""
 
 
+def test_gpus_n_without_torchrun_spawns_n_ranks():
+    """`python bench.py --gpus N` with no WORLD_SIZE in the environment must launch N ranks itself
+    and the line must say n_gpus = N (launch plumbing only: the selftest arm joins a gloo group and does no work)."""
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "selftest", "--gpus", "2"],
+                       env=env, capture_output=True, text=True, timeout=300)
+    assert p.returncode == 0, p.stderr[-500:]
+    lines = [ln for ln in p.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1 and json.loads(lines[0])["n_gpus"] == 2
+    sys.path.insert(0, ROOT)
+    import argparse
+    import bench
+    a = argparse.Namespace(gpus=4, steps=7, warmup=3, impl="ours", no_sweep=True, no_extras=False, no_cpu=True)
+    cmd = bench.spawn_command(a, port=12345)
+    assert cmd[1:4] == ["-m", "torch.distributed.run", "--nnodes=1"] and "--nproc-per-node" in cmd and "4" in cmd
+    assert cmd[-2:] == ["--no-sweep", "--no-cpu"] and "127.0.0.1" in cmd
+
+
 # ---- column-sharded propagator (SURVEY.md §8(e)(1)): host logic on gloo, world size 2 and 3 -------------
 class _Res:
     def __init__(self, it):
