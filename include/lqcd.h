@@ -58,7 +58,8 @@ typedef struct lqcd_result {
 } lqcd_result;
 
 /* Context (init + LatticeInfo).  dims = {Lx,Ly,Lz,Lt}, each even and >= 4;
- * prec = 4 (fp32) or 8 (fp64): the real type of every native AND public buffer of this context;
+ * prec = 4 (fp32) or 8 (fp64): the real type of every native AND public buffer of this context; prec = 2: 16-bit
+ * fixed-point NATIVE fields with fp32 arithmetic and fp32 (complex64) public arrays (see "16-bit storage" below);
  * recon = 18 (full links) or 12 (two rows stored, third recomputed); t_boundary = +1 or -1
  * (antiperiodic in t, applied in-kernel to raw periodic links); device = CUDA
  * ordinal (must be compute capability 10.x).
@@ -198,6 +199,19 @@ int lqcd_invert_mixed(lqcd_ctx* ctx, lqcd_ctx* ctx_lo, void* x_public, const voi
                       const void* clover_inv_lo, double kappa, double tol, double inner_tol, int maxiter, int solver,
                       int matpc, void* workspace, size_t workspace_bytes, void* workspace_lo,
                       size_t workspace_lo_bytes, lqcd_result* res, void* stream);
+
+/* 16-bit storage (second half; PAPER.md:423 ref. [1], mixed-precision solvers on GPUs).  A context
+ * created with prec = 2 stores spinors as 24 int16 + one fp32 norm per site (52 B), links as R int16 (|U_ij| <= 1) and
+ * the clover field as 72 int16 + one fp32 norm per chiral block (152 B per site); every kernel computes in fp32
+ * registers.  Sizes come from lqcd_*_bytes as usual; public arrays are complex64.  Available in such a context:
+ * lqcd_gauge_pack, lqcd_spinor_pack / _unpack, lqcd_dslash, lqcd_clover_apply, lqcd_mpc_apply, lqcd_mat_apply,
+ * lqcd_invert (clover fields required), lqcd_blas_*, the sources / contractions (public arrays), and its use as
+ * ctx_lo of lqcd_invert_mixed (one column), which is what it is for: the inner iterations move half the bytes of an
+ * fp32 context and the fp64 defect correction outside restores the tolerance.  Not available (LQCD_ERR_INVALID_ARG):
+ * lqcd_clover_build* (build in an fp32 context of the same lattice, then lqcd_clover_to_half), lqcd_clover_unpack, the
+ * multi-RHS and *_host calls.
+ *   lqcd_clover_to_half : clover_fp32_native (both parities, from an fp32 context of the same lattice) -> 16-bit native */
+int lqcd_clover_to_half(lqcd_ctx* ctx_half, void* clover_half, const void* clover_fp32_native, void* stream);
 
 /* Sources, propagator assembly and per-time-slice contractions of the paper's Listing 1
  * (SURVEY.md §8(a) a4/a12, §8(f) rank 4).  All arrays are DEVICE arrays in PUBLIC

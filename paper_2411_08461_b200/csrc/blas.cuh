@@ -8,6 +8,7 @@
 // deterministic for a fixed grid.  Accumulation is fp64 in both precisions.
 #pragma once
 #include "lqcd_internal.cuh"
+#include "half.cuh"
 
 constexpr int BLAS_BLOCK = 256;
 constexpr int BLAS_MAXV = 6;
@@ -339,5 +340,60 @@ static inline int blas_launch(lqcd_ctx* c, const Op& op, void* const* v, const i
   c->alg_bytes += (double)(__builtin_popcount(Op::LOAD) + __builtin_popcount(Op::STORE)) * 24.0 * sizeof(T) * c->lat.Vh * acct;
   blas_kernel<T, Op><<<dim3(grid, nrhs), BLAS_BLOCK, 0, st>>>(op, vecs, nvec, red);
   LQCD_LAUNCH_CHECK(c, "blas");
+  return LQCD_OK;
+}
+
+// --------------------------------------------------------------------------------------------
+// 16-bit storage (half.cuh): the same ops, one thread per SITE, because a stored vector needs the site's norm
+// (the largest of its 24 components) before its first component can be written.  Single right-hand side.
+// --------------------------------------------------------------------------------------------
+template <typename Op>
+__global__ void __launch_bounds__(BLAS_BLOCK) blas_half_kernel(Op op, BlasVecs<void> vecs, int Vh, RedArgs red) {
+  if (red.scalars[S_DONE] != 0.0) return;
+  op.init(red.scalars);
+  double acc[Op::NR > 0 ? Op::NR : 1];
+#pragma unroll
+  for (int k = 0; k < (Op::NR > 0 ? Op::NR : 1); k++) acc[k] = 0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < Vh; i += gridDim.x * blockDim.x) {
+    float z[Op::NV][24];
+#pragma unroll
+    for (int a = 0; a < Op::NV; a++)
+      if (Op::LOAD & (1u << a)) load_spinor_h_plain(vecs.v[a], Vh, i, z[a]);
+#pragma unroll
+    for (int e = 0; e < 24; e += 2) {
+      float w[Op::NV][2];
+#pragma unroll
+      for (int a = 0; a < Op::NV; a++) { w[a][0] = z[a][e]; w[a][1] = z[a][e + 1]; }
+      op.elem(w, acc);
+#pragma unroll
+      for (int a = 0; a < Op::NV; a++) { z[a][e] = w[a][0]; z[a][e + 1] = w[a][1]; }
+    }
+#pragma unroll
+    for (int a = 0; a < Op::NV; a++)
+      if (Op::STORE & (1u << a)) store_spinor_h(vecs.v[a], Vh, i, z[a]);
+  }
+  if (Op::NR > 0) block_reduce_finish<(Op::NR > 0 ? Op::NR : 1)>(acc, red.partial, red.max_blocks, red.ticket, red.scalars, red.out);
+}
+
+template <typename Op>
+static inline int blas_half_launch(lqcd_ctx* c, const Op& op, void* const* v, const int* out_slots, int nrhs, int rhs0,
+                                   cudaStream_t st) {
+  if (nrhs != 1 || rhs0 != 0) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "16-bit context: one right-hand side only");
+  BlasVecs<void> vecs;
+  for (int a = 0; a < BLAS_MAXV; a++) vecs.v[a] = a < Op::NV ? v[a] : nullptr;
+  const int Vh = c->lat.Vh;
+  const long want = (Vh + BLAS_BLOCK - 1) / BLAS_BLOCK;
+  const int grid = (int)(want < c->max_red_blocks ? want : c->max_red_blocks);
+  RedArgs red;
+  red.partial = c->d_partial;
+  red.scalars = c->d_scalars;
+  red.ticket = c->d_ticket;
+  red.max_blocks = c->max_red_blocks;
+  red.rhs0 = 0;
+  red.stride = 0;
+  for (int k = 0; k < 4; k++) red.out[k] = out_slots ? out_slots[k] : 0;
+  c->alg_bytes += (double)(__builtin_popcount(Op::LOAD) + __builtin_popcount(Op::STORE)) * 52.0 * Vh;
+  blas_half_kernel<Op><<<grid, BLAS_BLOCK, 0, st>>>(op, vecs, Vh, red);
+  LQCD_LAUNCH_CHECK(c, "blas_half");
   return LQCD_OK;
 }

@@ -303,6 +303,7 @@ __global__ void __launch_bounds__(CB_SITES * 6, CB_MINB) clover_build_kernel(T* 
 extern "C" int lqcd_clover_build_aniso(lqcd_ctx* c, void* clover, void* clover_inv, const void* gauge, double csw_s,
                                        double csw_t, double kappa, void* stream) {
   if (!c || !clover || !gauge) return LQCD_ERR_INVALID_ARG;
+  if (c->half) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "clover_build: not available in a 16-bit context; build in an fp32 context and convert (lqcd_clover_to_half)");
   if (!lqcd_aligned16(clover) || !lqcd_aligned16(clover_inv) || !lqcd_aligned16(gauge))
     return lqcd_set_error(c, LQCD_ERR_ALIGN, "clover_build: alignment");
   cudaStream_t st = as_stream(stream);

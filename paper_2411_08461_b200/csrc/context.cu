@@ -43,7 +43,7 @@ long lqcd_launch_count(const lqcd_ctx* ctx) { return ctx ? ctx->launches : 0; }
 int lqcd_create(lqcd_ctx** out, const int dims[4], int prec, int recon, int t_boundary, int device) {
   if (!out || !dims) return LQCD_ERR_INVALID_ARG;
   *out = nullptr;
-  if ((prec != 4 && prec != 8) || (recon != 18 && recon != 12) || (t_boundary != 1 && t_boundary != -1))
+  if ((prec != 4 && prec != 8 && prec != 2) || (recon != 18 && recon != 12) || (t_boundary != 1 && t_boundary != -1))
     return LQCD_ERR_INVALID_ARG;
   long V = 1;
   for (int i = 0; i < 4; i++) {
@@ -71,7 +71,8 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], int prec, int recon, int t_bo
   c->lat.Lt = dims[3];
   c->lat.Vh = (int)(V / 2);
   c->lat.tb = t_boundary;
-  c->prec = prec;
+  c->prec = prec == 2 ? 4 : prec;  // 16-bit storage: fp32 arithmetic and public arrays
+  c->half = prec == 2 ? 1 : 0;
   c->ws = 1.0;
   {
     // shared-memory tiled dslash (dslash_tiled.cuh): parity-tested, measured slower than the one-thread-per-site
@@ -176,8 +177,9 @@ int lqcd_profile_read(lqcd_ctx* c, long* launches, double* total_ms, double* tot
   return LQCD_OK;
 }
 
-size_t lqcd_gauge_bytes(const lqcd_ctx* c) { return c ? (size_t)4 * c->V * c->recon * c->prec : 0; }
-size_t lqcd_spinor_bytes(const lqcd_ctx* c) { return c ? (size_t)c->lat.Vh * 24 * c->prec : 0; }
-size_t lqcd_clover_bytes(const lqcd_ctx* c) { return c ? (size_t)c->V * 72 * c->prec : 0; }
+// 16-bit storage (half.cuh): 2 B per real, + one fp32 norm per spinor site, + two per clover site
+size_t lqcd_gauge_bytes(const lqcd_ctx* c) { return c ? (size_t)4 * c->V * c->recon * (c->half ? 2 : c->prec) : 0; }
+size_t lqcd_spinor_bytes(const lqcd_ctx* c) { return c ? (c->half ? (size_t)c->lat.Vh * 52 : (size_t)c->lat.Vh * 24 * c->prec) : 0; }
+size_t lqcd_clover_bytes(const lqcd_ctx* c) { return c ? (c->half ? (size_t)c->V * 152 : (size_t)c->V * 72 * c->prec) : 0; }
 
 }  // extern "C"

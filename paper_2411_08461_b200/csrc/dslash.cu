@@ -380,6 +380,10 @@ static void launch_typed(lqcd_ctx* c, void* out, const void* in, const void* gau
 // consecutive one-parity spinors and the multi-right-hand-side kernel (dslash_mrhs.cu) runs.
 int lqcd_dslash_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
                        int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st) {
+  if (c->half) {
+    if (nrhs > 1) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "16-bit context: one right-hand side only");
+    return lqcd_dslash_half_launch(c, out, in, gauge, cl, x, parity, scale, dagger, epi, st);
+  }
   if (nrhs > 1) return lqcd_dslash_mrhs_launch(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st);
   // algorithmic bytes: every link once, input spinor once, output once (+ clover, + x)
   const double bytes = (double)c->lat.Vh * c->prec *
@@ -400,7 +404,7 @@ int lqcd_dslash_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge
 
 // CG-fused epilogues (4, 5) are available when the per-block partials fit the context's scratch
 bool lqcd_dslash_fuse_ok(const lqcd_ctx* c) {
-  return (long)lqcd_dslash_grid(c) <= 4L * c->max_red_blocks * LQCD_MAX_RHS;
+  return !c->half && (long)lqcd_dslash_grid(c) <= 4L * c->max_red_blocks * LQCD_MAX_RHS;
 }
 
 int lqcd_dslash_fused_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
@@ -427,6 +431,10 @@ int lqcd_dslash_fused_launch(lqcd_ctx* c, void* out, const void* in, const void*
 }
 
 int lqcd_clover_apply_launch(lqcd_ctx* c, void* out, const void* in, const void* cl_parity, int nrhs, cudaStream_t st) {
+  if (c->half) {
+    if (nrhs > 1) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "16-bit context: one right-hand side only");
+    return lqcd_clover_apply_half_launch(c, out, in, cl_parity, st);
+  }
   const int Vh = c->lat.Vh, block = 128;
   const dim3 grid((Vh + block - 1) / block, nrhs);
   c->alg_bytes += (double)Vh * c->prec * (72.0 + 48.0 * nrhs);

@@ -23,7 +23,8 @@ struct lqcd_ctx {
   int L[4];
   Lat lat;
   long V;
-  int prec, recon, device, sm_count;
+  int prec, recon, device, sm_count;  // prec: bytes of a real of the PUBLIC arrays and of the arithmetic (4 | 8)
+  int half;  // 1: native fields in 16-bit fixed point (half.cuh; created with prec = 2: fp32 arithmetic and public arrays)
   double ws;  // weight of the spatial hops: nu/xi_0 of Eq. 5; 1 = isotropic
   int mrhs_tma;    // 1 (default): TMA-tiled multi-RHS kernel (dslash_mrhs_tma.cu) where it applies; LQCD_MRHS_TMA=0 turns it off
   int mrhs_zslab;  // z-tiles per slab of its sweep (LQCD_MRHS_ZSLAB; 0 = the whole z extent)
@@ -249,6 +250,15 @@ int lqcd_dslash_mrhs_launch(lqcd_ctx* c, void* out, const void* in, const void* 
 bool lqcd_mrhs_tma_ok(const lqcd_ctx* c, int epi);
 int lqcd_dslash_mrhs_tma_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
                                 int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st);
+// 16-bit-storage context (half.cu)
+int lqcd_dslash_half_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
+                            int parity, double scale, int dagger, int epi, cudaStream_t st);
+int lqcd_clover_apply_half_launch(lqcd_ctx* c, void* out, const void* in, const void* cl_parity, cudaStream_t st);
+int lqcd_gauge_pack_half(lqcd_ctx* c, void* native, const void* pub, cudaStream_t st);
+int lqcd_spinor_pack_half(lqcd_ctx* c, void* native, const void* pub, int parities, cudaStream_t st);
+int lqcd_spinor_unpack_half(lqcd_ctx* c, void* pub, const void* native, int parities, cudaStream_t st);
+int lqcd_spinor_down_half(lqcd_ctx* c, void* out, const void* in_fp64, double scale, cudaStream_t st);
+int lqcd_spinor_up_axpy_half(lqcd_ctx* c, void* x_fp64, const void* e, double a, cudaStream_t st);
 int lqcd_clover_apply_launch(lqcd_ctx* c, void* out, const void* in, const void* cl_parity, int nrhs, cudaStream_t st);
 int lqcd_spinor_pack_parity(lqcd_ctx* c, void* native, const void* pub, cudaStream_t st);
 int lqcd_spinor_unpack_parity(lqcd_ctx* c, void* pub, const void* native, cudaStream_t st);

@@ -53,6 +53,7 @@ int lqcd_gauge_pack(lqcd_ctx* c, void* native, const void* pub, void* stream) {
   if (!lqcd_aligned16(native) || !lqcd_aligned16(pub)) return lqcd_set_error(c, LQCD_ERR_ALIGN, "gauge_pack: alignment");
   cudaStream_t st = as_stream(stream);
   const int Vh = c->lat.Vh;
+  if (c->half) return lqcd_gauge_pack_half(c, native, pub, st);
   if (c->prec == 4 && c->recon == 18) launch_to_soa<float, float2, 2, 18, 9>(native, pub, Vh, 8, st);
   else if (c->prec == 4) launch_to_soa<float, float4, 4, 18, 3>(native, pub, Vh, 8, st);
   else if (c->recon == 18) launch_to_soa<double, double2, 2, 18, 9>(native, pub, Vh, 8, st);
@@ -66,6 +67,7 @@ int lqcd_spinor_pack(lqcd_ctx* c, void* native, const void* pub, void* stream) {
   if (!c || !native || !pub) return LQCD_ERR_INVALID_ARG;
   if (!lqcd_aligned16(native) || !lqcd_aligned16(pub)) return lqcd_set_error(c, LQCD_ERR_ALIGN, "spinor_pack: alignment");
   cudaStream_t st = as_stream(stream);
+  if (c->half) return lqcd_spinor_pack_half(c, native, pub, 2, st);
   if (c->prec == 4) launch_to_soa<float, float4, 4, 24, 6>(native, pub, c->lat.Vh, 2, st);
   else launch_to_soa<double, double2, 2, 24, 12>(native, pub, c->lat.Vh, 2, st);
   c->alg_bytes += 4.0 * (double)lqcd_spinor_bytes(c);
@@ -77,6 +79,7 @@ int lqcd_spinor_unpack(lqcd_ctx* c, void* pub, const void* native, void* stream)
   if (!c || !native || !pub) return LQCD_ERR_INVALID_ARG;
   if (!lqcd_aligned16(native) || !lqcd_aligned16(pub)) return lqcd_set_error(c, LQCD_ERR_ALIGN, "spinor_unpack: alignment");
   cudaStream_t st = as_stream(stream);
+  if (c->half) return lqcd_spinor_unpack_half(c, pub, native, 2, st);
   if (c->prec == 4) launch_to_aos<float, float4, 4, 24, 6>(pub, native, c->lat.Vh, 2, st);
   else launch_to_aos<double, double2, 2, 24, 12>(pub, native, c->lat.Vh, 2, st);
   c->alg_bytes += 4.0 * (double)lqcd_spinor_bytes(c);
@@ -88,6 +91,7 @@ int lqcd_clover_unpack(lqcd_ctx* c, void* pub, const void* native, void* stream)
   if (!c || !native || !pub) return LQCD_ERR_INVALID_ARG;
   if (!lqcd_aligned16(native) || !lqcd_aligned16(pub)) return lqcd_set_error(c, LQCD_ERR_ALIGN, "clover_unpack: alignment");
   cudaStream_t st = as_stream(stream);
+  if (c->half) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "clover_unpack: not available in a 16-bit context (convert from an fp32 one: lqcd_clover_to_half)");
   if (c->prec == 4) launch_to_aos<float, float4, 4, 72, 18>(pub, native, c->lat.Vh, 2, st);
   else launch_to_aos<double, double2, 2, 72, 36>(pub, native, c->lat.Vh, 2, st);
   c->alg_bytes += 2.0 * (double)lqcd_clover_bytes(c);
@@ -99,6 +103,7 @@ int lqcd_clover_unpack(lqcd_ctx* c, void* pub, const void* native, void* stream)
 
 // one-parity spinor pack/unpack (used by the *_host entry points)
 int lqcd_spinor_pack_parity(lqcd_ctx* c, void* native, const void* pub, cudaStream_t st) {
+  if (c->half) return lqcd_spinor_pack_half(c, native, pub, 1, st);
   if (c->prec == 4) launch_to_soa<float, float4, 4, 24, 6>(native, pub, c->lat.Vh, 1, st);
   else launch_to_soa<double, double2, 2, 24, 12>(native, pub, c->lat.Vh, 1, st);
   c->alg_bytes += 2.0 * (double)lqcd_spinor_bytes(c);
@@ -106,6 +111,7 @@ int lqcd_spinor_pack_parity(lqcd_ctx* c, void* native, const void* pub, cudaStre
   return LQCD_OK;
 }
 int lqcd_spinor_unpack_parity(lqcd_ctx* c, void* pub, const void* native, cudaStream_t st) {
+  if (c->half) return lqcd_spinor_unpack_half(c, pub, native, 1, st);
   if (c->prec == 4) launch_to_aos<float, float4, 4, 24, 6>(pub, native, c->lat.Vh, 1, st);
   else launch_to_aos<double, double2, 2, 24, 12>(pub, native, c->lat.Vh, 1, st);
   c->alg_bytes += 2.0 * (double)lqcd_spinor_bytes(c);

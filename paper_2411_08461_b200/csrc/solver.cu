@@ -13,7 +13,8 @@ static inline char* off(const void* p, size_t bytes) { return (char*)p + bytes; 
 enum { S_BB = 0, S_RR0 = 2, S_RR1 = 3, S_TT = 4, S_RES = 5, S_RHO0 = 8, S_RHO1 = 10, S_R0V = 12, S_TS = 16, S_RR = 20, S_TRUE = 24 };
 
 #define BLAS_CALL(c, OPNAME, SETUP, vecs, outs, nrhs, rhs0, st)                       \
-  ((c)->prec == 4 ? [&]() { OPNAME<float> op; SETUP; return blas_launch<float, OPNAME<float>>((c), op, (vecs), (outs), (nrhs), (rhs0), (st)); }() \
+  ((c)->half ? [&]() { OPNAME<float> op; SETUP; return blas_half_launch<OPNAME<float>>((c), op, (vecs), (outs), (nrhs), (rhs0), (st)); }() \
+   : (c)->prec == 4 ? [&]() { OPNAME<float> op; SETUP; return blas_launch<float, OPNAME<float>>((c), op, (vecs), (outs), (nrhs), (rhs0), (st)); }() \
                   : [&]() { OPNAME<double> op; SETUP; return blas_launch<double, OPNAME<double>>((c), op, (vecs), (outs), (nrhs), (rhs0), (st)); }())
 
 // all slots of the first nrhs right-hand sides -> pinned host mirror; synchronises the stream
@@ -462,9 +463,13 @@ static int solve_mixed(lqcd_ctx* c, const Work& w, const void* gauge, const void
         continue;
       }
       rn[j] = sqrt(rr[j]);
-      spinor_down_kernel<<<grid, 256, 0, st>>>((float4*)(m.wi.v[0] + j * spi), (const double2*)(r + j * sp), Vh, 1.0 / rn[j]);
-      c->alg_bytes += (double)Vh * 24 * 12;
-      LQCD_LAUNCH_CHECK(c, "spinor_down");
+      if (ci->half) {
+        if ((rc = lqcd_spinor_down_half(c, m.wi.v[0] + j * spi, r + j * sp, 1.0 / rn[j], st))) return rc;
+      } else {
+        spinor_down_kernel<<<grid, 256, 0, st>>>((float4*)(m.wi.v[0] + j * spi), (const double2*)(r + j * sp), Vh, 1.0 / rn[j]);
+        c->alg_bytes += (double)Vh * 24 * 12;
+        LQCD_LAUNCH_CHECK(c, "spinor_down");
+      }
       // inner fp32 solve of Mhat e = r/|r|, relative tolerance tol_k
       const double need = 0.25 * sqrt(cols.stop2[j] / rr[j]);
       const double tol_k = need > m.inner_tol ? need : m.inner_tol;
@@ -486,9 +491,13 @@ static int solve_mixed(lqcd_ctx* c, const Work& w, const void* gauge, const void
       res[j].dslash_count += ri[j].dslash_count;
       if (ri[j].status < 0) { res[j].status = ri[j].status; live[j] = false; nlive--; broke = true; continue; }
       // x += |r| e
-      spinor_up_axpy_kernel<<<grid, 256, 0, st>>>((double2*)(x + j * sp), (const float4*)(m.wi.x + j * spi), Vh, rn[j]);
-      c->alg_bytes += (double)Vh * 24 * 20;
-      LQCD_LAUNCH_CHECK(c, "spinor_up_axpy");
+      if (ci->half) {
+        if ((rc = lqcd_spinor_up_axpy_half(c, x + j * sp, m.wi.x + j * spi, rn[j], st))) return rc;
+      } else {
+        spinor_up_axpy_kernel<<<grid, 256, 0, st>>>((double2*)(x + j * sp), (const float4*)(m.wi.x + j * spi), Vh, rn[j]);
+        c->alg_bytes += (double)Vh * 24 * 20;
+        LQCD_LAUNCH_CHECK(c, "spinor_up_axpy");
+      }
     }
     total += step;
     if (broke && n == 1) break;
@@ -683,8 +692,8 @@ static int invert_common(lqcd_ctx* c, void* x_public, const void* b_public, cons
                          Mixed* mixed = nullptr) {
   if (!c || !x_public || !b_public || !gauge || !workspace || !res) return LQCD_ERR_INVALID_ARG;
   if (solver < 0 || solver > 2 || matpc < 0 || matpc > 2 || maxiter < 0 || !(tol >= 0) || (clover && !clover_inv) ||
-      nrhs < 1 || nrhs > LQCD_MAX_RHS)
-    return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "invert: bad solver/matpc/maxiter/tol/nrhs");
+      nrhs < 1 || nrhs > LQCD_MAX_RHS || (c->half && (nrhs > 1 || !clover)))
+    return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "invert: bad solver/matpc/maxiter/tol/nrhs (16-bit context: one column, clover fields required)");
   if (workspace_bytes < lqcd_invert_multi_workspace_bytes(c, solver, nrhs))
     return lqcd_set_error(c, LQCD_ERR_WORKSPACE, "invert: workspace %zu < %zu", workspace_bytes,
                           lqcd_invert_multi_workspace_bytes(c, solver, nrhs));
@@ -693,6 +702,7 @@ static int invert_common(lqcd_ctx* c, void* x_public, const void* b_public, cons
   memset(res, 0, sizeof(*res) * nrhs);
   const long launches0 = c->launches, mixed_launches0 = mixed ? mixed->ci->launches : 0;
   const size_t sp = lqcd_spinor_bytes(c);
+  const size_t psp = (size_t)c->lat.Vh * 24 * c->prec;  // one parity of a PUBLIC spinor (16-bit context: complex64)
   Work w;
   carve(c, workspace, w, nrhs, clover == nullptr);
   int rc;
@@ -706,11 +716,11 @@ static int invert_common(lqcd_ctx* c, void* x_public, const void* b_public, cons
   for (int j = 0; j < nrhs; j++)
     for (int par = 0; par < 2; par++)
       if ((rc = lqcd_spinor_pack_parity(c, w.b + ((size_t)par * nrhs + j) * sp,
-                                        (const char*)b_public + ((size_t)2 * j + par) * sp, st))) return rc;
+                                        (const char*)b_public + ((size_t)2 * j + par) * psp, st))) return rc;
   if ((rc = invert_native(c, w, gauge, clover, clover_inv, kappa, tol, maxiter, solver, matpc, res, st, mixed))) return rc;
   for (int j = 0; j < nrhs; j++)
     for (int par = 0; par < 2; par++)
-      if ((rc = lqcd_spinor_unpack_parity(c, (char*)x_public + ((size_t)2 * j + par) * sp,
+      if ((rc = lqcd_spinor_unpack_parity(c, (char*)x_public + ((size_t)2 * j + par) * psp,
                                           w.x + ((size_t)par * nrhs + j) * sp, st))) return rc;
   cudaEventRecord(c->ev1, st);
   if (cudaStreamSynchronize(st) != cudaSuccess) return lqcd_check_cuda(c, "invert sync");
@@ -749,8 +759,8 @@ int lqcd_invert_multi_mixed(lqcd_ctx* c, lqcd_ctx* ci, void* x_public, const voi
     return LQCD_ERR_INVALID_ARG;
   if (c->prec != 8 || ci->prec != 4 || c->device != ci->device || c->lat.tb != ci->lat.tb || c->L[0] != ci->L[0] ||
       c->L[1] != ci->L[1] || c->L[2] != ci->L[2] || c->L[3] != ci->L[3] || !(inner_tol > 0) || !(inner_tol < 1) ||
-      nrhs < 1 || nrhs > LQCD_MAX_RHS)
-    return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "invert_mixed: needs an fp64 and an fp32 context of the same lattice");
+      nrhs < 1 || nrhs > LQCD_MAX_RHS || c->half || (ci->half && nrhs > 1))
+    return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "invert_mixed: needs an fp64 and an fp32 (or, one column, 16-bit) context of the same lattice");
   if (workspace_lo_bytes < lqcd_invert_multi_workspace_bytes(ci, solver, nrhs))
     return lqcd_set_error(c, LQCD_ERR_WORKSPACE, "invert_mixed: low-precision workspace too small");
   const void* p[4] = {gauge_lo, clover_lo, clover_inv_lo, workspace_lo};
@@ -782,6 +792,7 @@ size_t lqcd_host_scratch_bytes(const lqcd_ctx* c, int solver) {
 
 int lqcd_gauge_pack_host(lqcd_ctx* c, void* native, const void* pub_host, void* scratch, void* stream) {
   if (!c || !native || !pub_host || !scratch) return LQCD_ERR_INVALID_ARG;
+  if (c->half) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "gauge_pack_host: not available in a 16-bit context");
   cudaStream_t st = as_stream(stream);
   cudaMemcpyAsync(scratch, pub_host, (size_t)4 * c->V * 18 * c->prec, cudaMemcpyHostToDevice, st);
   return lqcd_gauge_pack(c, native, scratch, stream);
@@ -791,6 +802,7 @@ int lqcd_gauge_pack_host(lqcd_ctx* c, void* native, const void* pub_host, void* 
 int lqcd_dslash_host(lqcd_ctx* c, void* out_host, const void* in_host, const void* gauge, int parity, double scale,
                      int dagger, void* scratch, void* stream) {
   if (!c || !out_host || !in_host || !gauge || !scratch || (parity != 0 && parity != 1)) return LQCD_ERR_INVALID_ARG;
+  if (c->half) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "dslash_host: not available in a 16-bit context");
   if (!lqcd_aligned16(scratch) || !lqcd_aligned16(gauge)) return lqcd_set_error(c, LQCD_ERR_ALIGN, "dslash_host: alignment");
   cudaStream_t st = as_stream(stream);
   const size_t sp = lqcd_spinor_bytes(c);
@@ -809,6 +821,7 @@ int lqcd_invert_host(lqcd_ctx* c, void* x_host, const void* b_host, const void* 
                      const void* clover_inv, double kappa, double tol, int maxiter, int solver, int matpc,
                      void* scratch, size_t scratch_bytes, lqcd_result* res, void* stream) {
   if (!c || !x_host || !b_host || !scratch || !clover || !clover_inv) return LQCD_ERR_INVALID_ARG;
+  if (c->half) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "invert_host: not available in a 16-bit context");
   if (scratch_bytes < lqcd_host_scratch_bytes(c, solver)) return lqcd_set_error(c, LQCD_ERR_WORKSPACE, "invert_host: scratch too small");
   cudaStream_t st = as_stream(stream);
   const size_t sp = lqcd_spinor_bytes(c);
@@ -830,6 +843,7 @@ int lqcd_solve_host(lqcd_ctx* c, void* x_host, const void* b_host, const void* g
                     int matpc, void* g_scratch, void* scratch, size_t scratch_bytes, lqcd_result* res, void* stream) {
   if (!c || !x_host || !b_host || !gauge_public_host || !gauge || !clover || !clover_inv || !g_scratch || !scratch || !res)
     return LQCD_ERR_INVALID_ARG;
+  if (c->half) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "solve_host: not available in a 16-bit context");
   if (scratch_bytes < lqcd_host_scratch_bytes(c, solver)) return lqcd_set_error(c, LQCD_ERR_WORKSPACE, "solve_host: scratch too small");
   cudaStream_t st = as_stream(stream), cp = c->copy_stream;
   const size_t sp = lqcd_spinor_bytes(c);

@@ -38,6 +38,7 @@ SYMBOLS = [
     "lqcd_invert_mixed", "lqcd_invert_multi_mixed", "lqcd_solve_host", "lqcd_set_anisotropy", "lqcd_clover_build_aniso",
     "lqcd_momentum_phase", "lqcd_source_wall", "lqcd_source_point", "lqcd_propagator_assemble",
     "lqcd_propagator_split", "lqcd_contract_twopt", "lqcd_contract_threept", "lqcd_sequential_source",
+    "lqcd_clover_to_half",
 ]
 MAX_RHS = 16
 
@@ -88,6 +89,7 @@ def load():
     L.lqcd_contract_twopt.argtypes = [vp, dp, vp, vp, vp, vp]
     L.lqcd_contract_threept.argtypes = [vp, dp, vp, dp, vp, vp]
     L.lqcd_sequential_source.argtypes = [vp, vp, vp, dp, vp, ci, vp]
+    L.lqcd_clover_to_half.argtypes = [vp, vp, vp, vp]
     L.lqcd_set_anisotropy.argtypes = [vp, cd]
     L.lqcd_clover_build_aniso.argtypes = [vp, vp, vp, vp, cd, cd, cd, vp]
     L.lqcd_clover_apply.argtypes = [vp, vp, vp, vp, ci, vp]
@@ -198,9 +200,11 @@ class Context:
                             % self.lib.lqcd_strerror(rc).decode())
         self.h = h
         self.dev = torch.device("cuda", device)
-        self.rdtype = torch.float32 if prec == 4 else torch.float64
-        self.cdtype = torch.complex64 if prec == 4 else torch.complex128
-        self.np_cdtype = np.complex64 if prec == 4 else np.complex128
+        # prec = 2: 16-bit native storage (int16 buffers), fp32 arithmetic, complex64 public arrays
+        self.rdtype = {2: torch.int16, 4: torch.float32, 8: torch.float64}[prec]
+        self.pub_rdtype = torch.float64 if prec == 8 else torch.float32
+        self.cdtype = torch.complex128 if prec == 8 else torch.complex64
+        self.np_cdtype = np.complex128 if prec == 8 else np.complex64
         Lx, Ly, Lz, Lt = self.dims
         self.site_shape = (2, Lt, Lz, Ly, Lx // 2)
         self.Vh = Lx * Ly * Lz * Lt // 2
@@ -257,7 +261,7 @@ class Context:
         if t.is_complex():
             t = t.to(self.cdtype)
         else:
-            t = t.to(self.rdtype)
+            t = t.to(self.pub_rdtype)
         return t.to(self.dev).contiguous()
 
     # ---- pack / unpack ---------------------------------------------------------------------
@@ -277,7 +281,7 @@ class Context:
         return out
 
     def clover_unpack(self, cl_native):
-        out = torch.empty(self.site_shape + (2, 36), dtype=self.rdtype, device=self.dev)
+        out = torch.empty(self.site_shape + (2, 36), dtype=self.pub_rdtype, device=self.dev)
         self._check(self.lib.lqcd_clover_unpack(self.h, _p(out), _p(cl_native), _stream()))
         return out
 
@@ -291,6 +295,12 @@ class Context:
         Ai = self.empty(self.clover_bytes) if want_inverse else None
         self._check(self.lib.lqcd_clover_build(self.h, _p(A), _p(Ai), _p(gauge), csw, kappa, _stream()))
         return A, Ai
+
+    def clover_to_half(self, clover_fp32_native):
+        """self: 16-bit context; clover_fp32_native: A or A^-1 of an fp32 context of the same lattice."""
+        out = self.empty(self.clover_bytes)
+        self._check(self.lib.lqcd_clover_to_half(self.h, _p(out), _p(clover_fp32_native), _stream()))
+        return out
 
     def set_anisotropy(self, nu_over_xi0):
         self._check(self.lib.lqcd_set_anisotropy(self.h, nu_over_xi0))
