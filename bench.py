@@ -327,6 +327,28 @@ def extras(torch, lqcd, synth, U, b, ctx, gauge, device):
                          "mixed_seconds": rmx.seconds, "mixed_inner_iterations": rmx.iterations,
                          "mixed_true_resid": rmx.true_resid, "fp64_true_resid": r64.true_resid,
                          "speedup": r64.seconds / rmx.seconds}
+    # the same with a 16-bit-storage inner context (prec = 2: int16 + per-site norms, fp32 arithmetic), and its dslash
+    # against its own roofline: (8R + 48) reals x 2 B + two 4 B spinor norms per output site
+    hf = lqcd.Context(cfg["dims"], 2, 12, -1, device)
+    g_h = hf.gauge_pack(hf.to_device(synth.round_fp32(U)))
+    A_h, Ai_h = hf.clover_to_half(A_lo), hf.clover_to_half(Ai_lo)
+    for solver in ("cgne", "bicgstab"):
+        mp = MATPC if solver == "cgne" else 1
+        for _ in range(2):
+            _, r16 = ctx.invert_mixed(hf, b_dev, gauge, A, Ai, g_h, A_h, Ai_h, kappa, tol=1e-10, inner_tol=2e-3,
+                                      maxiter=4000, solver=solver, matpc=mp)
+        mixed[solver].update({"mixed16_seconds": r16.seconds, "mixed16_inner_iterations": r16.iterations,
+                              "mixed16_true_resid": r16.true_resid, "mixed16_status": r16.status,
+                              "mixed16_speedup_vs_fp64": mixed[solver]["fp64_seconds"] / r16.seconds})
+    peak = measured_peaks()[0]
+    nat_h = hf.spinor_pack(hf.to_device(synth.round_fp32(b)))
+    dst_h = hf.new_spinor(2)
+    th = time_batched(torch, lambda i: hf.dslash(hf.parity(dst_h, i & 1), hf.parity(nat_h, 1 - (i & 1)), g_h, i & 1))
+    by_h = ((8 * 12 + 48) * 2 + 8) * hf.Vh
+    mixed["dslash_16bit_recon12"] = {"us": th * 1e6, "GBps": by_h / th / 1e9, "frac_of_measured_peak": by_h / th / 1e9 / peak,
+                                     "bytes_per_site": by_h // hf.Vh, "GFLOPs": FLOPS_PER_SITE * hf.Vh / th / 1e9}
+    hf.close()
+    del g_h, A_h, Ai_h, nat_h, dst_h
     out["mixed_precision_32x64"] = mixed
     # 12-column point-source propagator at the headline size to the fp64 tolerance: 12 mixed
     # solves one after the other vs one batched mixed solve (lqcd_invert_multi_mixed), BiCGStab
@@ -571,6 +593,9 @@ def run_gpu(args):
         nr["small_lattice_solves"] = small_solves(torch, lqcd, synth, local)
         line["next_rows"] = nr
         roofline["dslash_mrhs_32x64_frac"] = {k: v["frac_of_measured_peak"] for k, v in nr["dslash_mrhs_32x64"].items()}
+        roofline["mixed_precision_32x64_cgne_ms"] = {k: nr["mixed_precision_32x64"]["cgne"][k + "_seconds"] * 1e3
+                                                     for k in ("fp64", "mixed", "mixed16")}
+        roofline["dslash_16bit_recon12_frac"] = nr["mixed_precision_32x64"]["dslash_16bit_recon12"]["frac_of_measured_peak"]
         roofline["propagator_32x64_mixed_bicgstab_ms"] = nr["propagator_32x64_mixed_bicgstab"]["batched_ms"]
         roofline["propagator_16x32_fp32_cgne_ms"] = nr["propagator_16x32_fp32_recon12"]["batched_ms"]
         roofline["worst_true_resid_fp32_1e-6"] = max(nr["propagator_16x32_fp32_recon12"]["worst_true_resid"],

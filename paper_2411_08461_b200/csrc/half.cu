@@ -169,15 +169,14 @@ __global__ void __launch_bounds__(256) gauge_pack_half_kernel(short* __restrict_
   const float* src = pub + ((size_t)b * Vh + idx) * 18;
   short* dst = nat + (size_t)b * R * Vh;
   if (R == 18) {
-    short2* p = reinterpret_cast<short2*>(dst) + idx;
+    unsigned* p = reinterpret_cast<unsigned*>(dst) + idx;
 #pragma unroll
-    for (int v = 0; v < 9; v++) p[(size_t)v * Vh] = make_short2(quant(src[2 * v], HALF_MAX), quant(src[2 * v + 1], HALF_MAX));
+    for (int v = 0; v < 9; v++) p[(size_t)v * Vh] = enc2(src[2 * v], src[2 * v + 1], HALF_MAX);
   } else {
-    short4* p = reinterpret_cast<short4*>(dst) + idx;
+    uint2* p = reinterpret_cast<uint2*>(dst) + idx;
 #pragma unroll
     for (int v = 0; v < 3; v++)
-      p[(size_t)v * Vh] = make_short4(quant(src[4 * v], HALF_MAX), quant(src[4 * v + 1], HALF_MAX), quant(src[4 * v + 2], HALF_MAX),
-                                      quant(src[4 * v + 3], HALF_MAX));
+      p[(size_t)v * Vh] = make_uint2(enc2(src[4 * v], src[4 * v + 1], HALF_MAX), enc2(src[4 * v + 2], src[4 * v + 3], HALF_MAX));
   }
 }
 // public spinor [nblocks parities][Vh][24] floats <-> native, one block per blockIdx.y
@@ -205,8 +204,8 @@ __global__ void __launch_bounds__(256) clover_to_half_kernel(char* __restrict__ 
   if (idx >= Vh) return;
   const float4* s = src + (size_t)par * 18 * Vh + idx;
   char* d = dst + (size_t)par * 152 * Vh;
-  short4* p = reinterpret_cast<short4*>(d) + idx;
-  float* n = reinterpret_cast<float*>(reinterpret_cast<short4*>(d) + (size_t)18 * Vh);
+  uint2* p = reinterpret_cast<uint2*>(d) + idx;
+  float* n = reinterpret_cast<float*>(reinterpret_cast<uint2*>(d) + (size_t)18 * Vh);
 #pragma unroll
   for (int k = 0; k < 2; k++) {
     float4 a[9];
@@ -219,7 +218,7 @@ __global__ void __launch_bounds__(256) clover_to_half_kernel(char* __restrict__ 
     const float inv = m > 0.f ? HALF_MAX / m : 0.f;
 #pragma unroll
     for (int q = 0; q < 9; q++)
-      p[(size_t)(9 * k + q) * Vh] = make_short4(quant(a[q].x, inv), quant(a[q].y, inv), quant(a[q].z, inv), quant(a[q].w, inv));
+      p[(size_t)(9 * k + q) * Vh] = make_uint2(enc2(a[q].x, a[q].y, inv), enc2(a[q].z, a[q].w, inv));
     n[(size_t)k * Vh + idx] = m;
   }
 }

@@ -44,12 +44,12 @@ def test_pack_unpack_is_the_format_bit_for_bit():
     psi[0, 0, 0, 0, 0] = 0
     nat = s.up(psi)
     Vh = s.ctx.Vh
-    raw = nat.cpu().numpy().view(np.int16)
+    raw = nat.cpu().numpy().view(np.uint16)
     q, n = quantise_spinor(psi)                       # [2, T, Z, Y, Xh, 24], [2, T, Z, Y, Xh]
     for par in range(2):
         blk = raw[par * 26 * Vh:(par + 1) * 26 * Vh]  # 52 B per site = 26 int16
-        got_q = blk[:24 * Vh].reshape(6, Vh, 4).transpose(1, 0, 2).reshape(Vh, 24)
-        got_n = blk[24 * Vh:].view(np.float32)
+        got_q = (blk[:24 * Vh].reshape(6, Vh, 4).transpose(1, 0, 2).reshape(Vh, 24).astype(np.int32) - 32768).astype(np.int16)  # offset binary
+        got_n = np.ascontiguousarray(blk[24 * Vh:]).view(np.float32)
         assert np.array_equal(got_q, q[par].reshape(Vh, 24))
         assert np.array_equal(got_n, n[par].reshape(Vh))
     assert np.array_equal(s.down(nat), round_spinor(psi))
