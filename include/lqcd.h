@@ -213,6 +213,34 @@ int lqcd_invert_mixed(lqcd_ctx* ctx, lqcd_ctx* ctx_lo, void* x_public, const voi
  *   lqcd_clover_to_half : clover_fp32_native (both parities, from an fp32 context of the same lattice) -> 16-bit native */
 int lqcd_clover_to_half(lqcd_ctx* ctx_half, void* clover_half, const void* clover_fp32_native, void* stream);
 
+/* 4-D domain decomposition of the hopping term (the lattice is divided
+ * equally over a 4-D Cartesian grid of ranks, the rank index running fastest in t).  Each rank owns a context, links and
+ * spinors of its sub-lattice (every local extent even and >= 4).  In a partitioned direction the hops that leave the
+ * sub-lattice are served by faces of projected half spinors, 12 reals per face site:
+ *   lqcd_set_partition      : partitioned[mu] != 0 marks direction mu as cut (default: none)
+ *   lqcd_face_bytes         : bytes of one face buffer of direction mu ([12][face sites of one parity], context type)
+ *   lqcd_dslash_dd_interior : out_p = scale * (the hops of D_{p,1-p} in that stay inside the sub-lattice); with no
+ *                             direction partitioned this is lqcd_dslash.  The context's t_boundary sign applies to
+ *                             interior hops only: give +1 to a context whose t direction is cut.
+ *   lqcd_face_pack          : dir = +1: the forward ghost of my -mu neighbour = my FIRST slice, h = P psi;
+ *                             dir = -1: the backward ghost of my +mu neighbour = my LAST slice, U_mu^dag P psi (my links).
+ *                             parity_in = parity of `in` (one-parity native spinor); dagger as in lqcd_dslash.
+ *   lqcd_face_unpack        : out_p += scale * weight * (the hop rebuilt from a received face): dir = +1 a forward ghost
+ *                             (received from the +mu neighbour, multiplied by my link U_mu(x) on my last slice), dir = -1
+ *                             a backward ghost (from the -mu neighbour, added on my first slice).  weight = nu/xi_0 for
+ *                             a spatial mu, and for t the boundary sign of THIS hop: -1 where it crosses the
+ *                             antiperiodic seam of the global lattice, +1 elsewhere.
+ * Moving a packed face to the rank that unpacks it is the caller's job (paper_2411_08461_b200/dd.py: device copies
+ * between sub-lattices on one GPU, torch.distributed send / recv between ranks).  fp32 and fp64 contexts. */
+int lqcd_set_partition(lqcd_ctx* ctx, const int partitioned[4]);
+size_t lqcd_face_bytes(const lqcd_ctx* ctx, int mu);
+int lqcd_dslash_dd_interior(lqcd_ctx* ctx, void* out, const void* in, const void* gauge, int parity, double scale,
+                            int dagger, void* stream);
+int lqcd_face_pack(lqcd_ctx* ctx, void* face, const void* in, const void* gauge, int mu, int dir, int parity_in,
+                   int dagger, void* stream);
+int lqcd_face_unpack(lqcd_ctx* ctx, void* out, const void* face, const void* gauge, int mu, int dir, int parity_out,
+                     double scale, double weight, int dagger, void* stream);
+
 /* Sources, propagator assembly and per-time-slice contractions of the paper's Listing 1
  * (SURVEY.md §8(a) a4/a12, §8(f) rank 4).  All arrays are DEVICE arrays in PUBLIC
  * layout and in the context's precision: phase [2][Lt][Lz][Ly][Lx/2] complex; spinor as above;

@@ -25,6 +25,7 @@ struct lqcd_ctx {
   long V;
   int prec, recon, device, sm_count;  // prec: bytes of a real of the PUBLIC arrays and of the arithmetic (4 | 8)
   int half;  // 1: native fields in 16-bit fixed point (half.cuh; created with prec = 2: fp32 arithmetic and public arrays)
+  int part_mask;  // bit mu: direction mu is cut between ranks (lqcd_set_partition; dd.cu)
   double ws;  // weight of the spatial hops: nu/xi_0 of Eq. 5; 1 = isotropic
   int mrhs_tma;    // 1 (default): TMA-tiled multi-RHS kernel (dslash_mrhs_tma.cu) where it applies; LQCD_MRHS_TMA=0 turns it off
   int mrhs_zslab;  // z-tiles per slab of its sweep (LQCD_MRHS_ZSLAB; 0 = the whole z extent)

@@ -38,7 +38,8 @@ SYMBOLS = [
     "lqcd_invert_mixed", "lqcd_invert_multi_mixed", "lqcd_solve_host", "lqcd_set_anisotropy", "lqcd_clover_build_aniso",
     "lqcd_momentum_phase", "lqcd_source_wall", "lqcd_source_point", "lqcd_propagator_assemble",
     "lqcd_propagator_split", "lqcd_contract_twopt", "lqcd_contract_threept", "lqcd_sequential_source",
-    "lqcd_clover_to_half",
+    "lqcd_clover_to_half", "lqcd_set_partition", "lqcd_face_bytes", "lqcd_dslash_dd_interior", "lqcd_face_pack",
+    "lqcd_face_unpack",
 ]
 MAX_RHS = 16
 
@@ -90,6 +91,12 @@ def load():
     L.lqcd_contract_threept.argtypes = [vp, dp, vp, dp, vp, vp]
     L.lqcd_sequential_source.argtypes = [vp, vp, vp, dp, vp, ci, vp]
     L.lqcd_clover_to_half.argtypes = [vp, vp, vp, vp]
+    L.lqcd_set_partition.argtypes = [vp, ctypes.POINTER(ci)]
+    L.lqcd_face_bytes.restype = sz
+    L.lqcd_face_bytes.argtypes = [vp, ci]
+    L.lqcd_dslash_dd_interior.argtypes = [vp, vp, vp, vp, ci, cd, ci, vp]
+    L.lqcd_face_pack.argtypes = [vp, vp, vp, vp, ci, ci, ci, ci, vp]
+    L.lqcd_face_unpack.argtypes = [vp, vp, vp, vp, ci, ci, ci, cd, cd, ci, vp]
     L.lqcd_set_anisotropy.argtypes = [vp, cd]
     L.lqcd_clover_build_aniso.argtypes = [vp, vp, vp, vp, cd, cd, cd, vp]
     L.lqcd_clover_apply.argtypes = [vp, vp, vp, vp, ci, vp]
@@ -300,6 +307,27 @@ class Context:
         """self: 16-bit context; clover_fp32_native: A or A^-1 of an fp32 context of the same lattice."""
         out = self.empty(self.clover_bytes)
         self._check(self.lib.lqcd_clover_to_half(self.h, _p(out), _p(clover_fp32_native), _stream()))
+        return out
+
+    # ---- domain decomposition (include/lqcd.h; the exchange itself is in dd.py) ---------------------
+    def set_partition(self, partitioned):
+        self._check(self.lib.lqcd_set_partition(self.h, (ctypes.c_int * 4)(*[int(bool(v)) for v in partitioned])))
+        return self
+
+    def face_buffer(self, mu):
+        return self.empty(self.lib.lqcd_face_bytes(self.h, mu))
+
+    def dslash_dd_interior(self, out, inp, gauge, parity, scale=1.0, dagger=False):
+        self._check(self.lib.lqcd_dslash_dd_interior(self.h, _p(out), _p(inp), _p(gauge), parity, scale, int(dagger), _stream()))
+        return out
+
+    def face_pack(self, face, inp, gauge, mu, direction, parity_in, dagger=False):
+        self._check(self.lib.lqcd_face_pack(self.h, _p(face), _p(inp), _p(gauge), mu, direction, parity_in, int(dagger), _stream()))
+        return face
+
+    def face_unpack(self, out, face, gauge, mu, direction, parity_out, scale=1.0, weight=1.0, dagger=False):
+        self._check(self.lib.lqcd_face_unpack(self.h, _p(out), _p(face), _p(gauge), mu, direction, parity_out, scale, weight,
+                                              int(dagger), _stream()))
         return out
 
     def set_anisotropy(self, nu_over_xi0):
