@@ -96,6 +96,9 @@ int lqcd_gauge_pack(lqcd_ctx* ctx, void* gauge_native, const void* gauge_public,
 int lqcd_spinor_pack(lqcd_ctx* ctx, void* spinor_native, const void* spinor_public, void* stream);
 int lqcd_spinor_unpack(lqcd_ctx* ctx, void* spinor_public, const void* spinor_native, void* stream);
 int lqcd_clover_unpack(lqcd_ctx* ctx, void* clover_public, const void* clover_native, void* stream);
+/* the inverse: a packed clover field (or inverse) in the public layout -> native, e.g. a sub-lattice's part of a field
+ * built on the whole lattice (domain decomposition) */
+int lqcd_clover_pack(lqcd_ctx* ctx, void* clover_native, const void* clover_public, void* stream);
 
 /* Clover term and its inverse from the links ("the clover field is then created";
  * SURVEY.md §8(c) O4-O6).  kappa is required because A contains kappa*csw (reading A6).  Leaves

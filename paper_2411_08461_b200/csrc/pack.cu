@@ -99,6 +99,20 @@ int lqcd_clover_unpack(lqcd_ctx* c, void* pub, const void* native, void* stream)
   return LQCD_OK;
 }
 
+// public packed clover [2][Vh][2][36] reals -> native (the inverse of lqcd_clover_unpack): a field built elsewhere, e.g.
+// the sub-lattice's part of a clover field built on the whole lattice (domain decomposition, dd.py)
+int lqcd_clover_pack(lqcd_ctx* c, void* native, const void* pub, void* stream) {
+  if (!c || !native || !pub) return LQCD_ERR_INVALID_ARG;
+  if (!lqcd_aligned16(native) || !lqcd_aligned16(pub)) return lqcd_set_error(c, LQCD_ERR_ALIGN, "clover_pack: alignment");
+  if (c->half) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "clover_pack: not available in a 16-bit context (lqcd_clover_to_half)");
+  cudaStream_t st = as_stream(stream);
+  if (c->prec == 4) launch_to_soa<float, float4, 4, 72, 18>(native, pub, c->lat.Vh, 2, st);
+  else launch_to_soa<double, double2, 2, 72, 36>(native, pub, c->lat.Vh, 2, st);
+  c->alg_bytes += 2.0 * (double)lqcd_clover_bytes(c);
+  LQCD_LAUNCH_CHECK(c, "clover_pack");
+  return LQCD_OK;
+}
+
 }  // extern "C"
 
 // one-parity spinor pack/unpack (used by the *_host entry points)

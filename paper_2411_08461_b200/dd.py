@@ -175,3 +175,105 @@ def dslash_dd(part, rank, ctx, out, inp, gauge, parity, scale=1.0, dagger=False,
     received = exchange(part, rank, faces, group)
     _unpack_all(part, rank, ctx, out, gauge, received, parity, scale, dagger, ws)
     return out
+
+
+# ---- M-hat and an even-odd CGNE solve on a decomposed lattice ------------------------------------------------------
+class Decomposed:
+    """The sub-lattices this process holds (all of them on one device: emulation and tests; exactly one, with a
+    torch.distributed group: one process per GPU) with their contexts and native fields, and the three things a Krylov
+    solve needs across them: D with its face exchange, sums over all ranks, and the BLAS-1 calls of the C ABI with
+    host coefficients.  The solve is host-driven (one scalar round trip per reduction): it is the correctness
+    reference of the decomposed path, not a tuned solver.  The clover fields are given (cut from a field built on the
+    whole lattice: a sub-lattice cannot build its edge sites' clover leaves from its own links alone)."""
+
+    def __init__(self, part, ranks, ctxs, gauges, A, Ai, group=None, ws=1.0):
+        self.part, self.ranks, self.ctxs, self.gauges, self.A, self.Ai = part, list(ranks), ctxs, gauges, A, Ai
+        self.group, self.ws = group, ws
+        self.emulated = group is None
+        if self.emulated and len(self.ranks) != part.size:
+            raise ValueError("without a process group this process must hold every sub-lattice")
+        if not self.emulated and len(self.ranks) != 1:
+            raise ValueError("with a process group a process holds one sub-lattice")
+
+    def new(self):
+        return [c.new_spinor(1) for c in self.ctxs]
+
+    def dslash(self, outs, ins, parity, scale=1.0, dagger=False):
+        if self.emulated:
+            return dslash_dd_emulated(self.part, self.ctxs, outs, ins, self.gauges, parity, scale, dagger, self.ws)
+        dslash_dd(self.part, self.ranks[0], self.ctxs[0], outs[0], ins[0], self.gauges[0], parity, scale, dagger, self.ws, self.group)
+        return outs
+
+    def allsum(self, values):
+        """values: one float or complex per held sub-lattice -> the sum over ALL ranks."""
+        s = complex(sum(values))
+        if not self.emulated:
+            import torch.distributed as dist
+            t = torch.tensor([s.real, s.imag], dtype=torch.float64)
+            if dist.get_backend(self.group) == "nccl":
+                t = t.cuda()
+            dist.all_reduce(t, group=self.group)
+            s = complex(float(t[0]), float(t[1]))
+        return s
+
+    def clover(self, outs, ins, field, parity):
+        for c, o, i, f in zip(self.ctxs, outs, ins, field):
+            c.clover_apply(o, i, f, parity)
+        return outs
+
+    def mpc(self, outs, ins, kappa, dagger, tmp, tmp2):
+        """Asymmetric even-even Schur complement: out = A_ee in - kappa^2 D_eo A_oo^-1 D_oe in."""
+        self.dslash(tmp2, ins, 1, 1.0, dagger)
+        self.clover(tmp, tmp2, self.Ai, 1)
+        self.dslash(outs, tmp, 0, -kappa * kappa, dagger)
+        self.clover(tmp2, ins, self.A, 0)
+        for c, o, t2 in zip(self.ctxs, outs, tmp2):
+            c.blas_caxpbypz(1.0, t2, 0.0, t2, o)        # out += A_ee in
+        return outs
+
+    def norm2(self, xs):
+        return self.allsum([c.blas_cdot(x, x)[1] for c, x in zip(self.ctxs, xs)]).real
+
+    def cgne(self, x, bhat, kappa, tol2_abs, maxiter):
+        """CGNE (O9) on Mhat Mhat^dag y = bhat, x = Mhat^dag y; x is zeroed here.  Returns (iterations, |r|^2)."""
+        r, p, t, q, tmp, tmp2 = (self.new() for _ in range(6))
+        for xx, rr, pp, b in zip(x, r, p, bhat):
+            xx.zero_()
+            rr.copy_(b)
+            pp.copy_(b)
+        rr2 = self.norm2(r)
+        it = 0
+        while it < maxiter and rr2 > tol2_abs:
+            self.mpc(t, p, kappa, True, tmp, tmp2)          # t = Mhat^dag p
+            alpha = rr2 / self.norm2(t)
+            self.mpc(q, t, kappa, False, tmp, tmp2)         # q = Mhat t
+            for c, xx, tt, rr, qq in zip(self.ctxs, x, t, r, q):
+                c.blas_caxpbypz(alpha, tt, 0.0, tt, xx)     # x += alpha t
+                c.blas_caxpbypz(-alpha, qq, 0.0, qq, rr)    # r -= alpha q
+            new = self.norm2(r)
+            for c, pp, rr in zip(self.ctxs, p, r):
+                c.blas_xpay(rr, new / rr2, pp)              # p = r + beta p
+            rr2 = new
+            it += 1
+        return it, rr2
+
+    def invert(self, b_natives, kappa, tol=1e-10, maxiter=2000):
+        """M x = b through the even-even system (O8): b_natives / result: two-parity native spinors per held sub-lattice."""
+        cs = self.ctxs
+        b_e = [c.parity(b, 0) for c, b in zip(cs, b_natives)]
+        b_o = [c.parity(b, 1) for c, b in zip(cs, b_natives)]
+        bb = self.norm2(b_e) + self.norm2(b_o)
+        xs = [c.new_spinor(2) for c in cs]
+        x_e = [c.parity(x, 0) for c, x in zip(cs, xs)]
+        x_o = [c.parity(x, 1) for c, x in zip(cs, xs)]
+        bhat, tmp = self.new(), self.new()
+        self.clover(tmp, b_o, self.Ai, 1)
+        self.dslash(bhat, tmp, 0, kappa)                    # kappa D_eo A_oo^-1 b_o
+        for c, bh, be in zip(cs, bhat, b_e):
+            c.blas_caxpbypz(1.0, be, 0.0, be, bh)           # + b_e
+        it, rr2 = self.cgne(x_e, bhat, kappa, tol * tol * bb, maxiter)
+        self.dslash(tmp, x_e, 1, kappa)                     # x_o = A_oo^-1 (b_o + kappa D_oe x_e)
+        for c, t, bo in zip(cs, tmp, b_o):
+            c.blas_caxpbypz(1.0, bo, 0.0, bo, t)
+        self.clover(x_o, tmp, self.Ai, 1)
+        return xs, it, (rr2 / bb) ** 0.5

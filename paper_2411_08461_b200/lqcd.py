@@ -39,7 +39,7 @@ SYMBOLS = [
     "lqcd_momentum_phase", "lqcd_source_wall", "lqcd_source_point", "lqcd_propagator_assemble",
     "lqcd_propagator_split", "lqcd_contract_twopt", "lqcd_contract_threept", "lqcd_sequential_source",
     "lqcd_clover_to_half", "lqcd_set_partition", "lqcd_face_bytes", "lqcd_dslash_dd_interior", "lqcd_face_pack",
-    "lqcd_face_unpack",
+    "lqcd_face_unpack", "lqcd_clover_pack",
 ]
 MAX_RHS = 16
 
@@ -77,7 +77,7 @@ def load():
     for f in ("lqcd_invert_workspace_bytes", "lqcd_host_scratch_bytes"):
         getattr(L, f).restype = sz
         getattr(L, f).argtypes = [vp, ci]
-    for f in ("lqcd_gauge_pack", "lqcd_spinor_pack", "lqcd_spinor_unpack", "lqcd_clover_unpack"):
+    for f in ("lqcd_gauge_pack", "lqcd_spinor_pack", "lqcd_spinor_unpack", "lqcd_clover_unpack", "lqcd_clover_pack"):
         getattr(L, f).argtypes = [vp, vp, vp, vp]
     L.lqcd_clover_build.argtypes = [vp, vp, vp, vp, cd, cd, vp]
     ip = ctypes.POINTER(ci)
@@ -290,6 +290,11 @@ class Context:
     def clover_unpack(self, cl_native):
         out = torch.empty(self.site_shape + (2, 36), dtype=self.pub_rdtype, device=self.dev)
         self._check(self.lib.lqcd_clover_unpack(self.h, _p(out), _p(cl_native), _stream()))
+        return out
+
+    def clover_pack(self, cl_public):
+        out = self.empty(self.clover_bytes)
+        self._check(self.lib.lqcd_clover_pack(self.h, _p(out), _p(cl_public), _stream()))
         return out
 
     def parity(self, s_native, p):

@@ -70,6 +70,9 @@ def _worker(rank, world, port, grid, out):
     ok = True
     for mu, kind, peer, tag in p.messages(rank)[1]:
         ok = ok and bool((got[tag] == 1000.0 * peer + tag).all())
+    # the reductions of a decomposed solve: one value per held sub-lattice, summed over all ranks
+    D = dd.Decomposed(p, [rank], [None], [None], [None], [None], group=dist.group.WORLD)
+    ok = ok and D.allsum([rank + 1 + 2j]) == 3 + 4j
     dist.barrier()
     dist.destroy_process_group()
     open(out % rank, "w").write("ok" if ok and len(got) == 2 * sum(p.partitioned) else "bad")
