@@ -16,8 +16,6 @@ constexpr int BLAS_MAXV = 6;
 // block of nrhs consecutive one-parity spinors, every right-hand side owns SC_STRIDE scalar slots,
 // its own partials and its own ticket.  Slot S_DONE != 0 freezes a right-hand side (its blocks exit
 // at once: a converged column is no longer updated); slot S_FIRST marks BiCGStab's first iteration.
-constexpr int SC_STRIDE = 64;
-constexpr int S_DONE = 60, S_FIRST = 61;
 constexpr int BLAS_MAXR = 4;  // reductions per launch
 
 template <typename T> struct BlasVecs {

@@ -95,6 +95,7 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], int prec, int recon, int t_bo
             cudaMalloc(&c->d_flag, sizeof(int) * 4) == cudaSuccess &&
             cudaMallocHost(&c->h_scalars, sizeof(double) * 64 * LQCD_MAX_RHS) == cudaSuccess &&
             cudaMallocHost(&c->h_consts, sizeof(double) * 2) == cudaSuccess &&
+            cudaMallocHost(&c->h_stop, sizeof(double) * LQCD_MAX_RHS) == cudaSuccess &&
             cudaMallocHost(&c->h_flag, sizeof(int) * 4) == cudaSuccess &&
             cudaEventCreate(&c->ev0) == cudaSuccess && cudaEventCreate(&c->ev1) == cudaSuccess &&
             cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) == cudaSuccess &&
@@ -126,6 +127,7 @@ int lqcd_destroy(lqcd_ctx* c) {
   if (c->d_flag) cudaFree(c->d_flag);
   if (c->h_scalars) cudaFreeHost(c->h_scalars);
   if (c->h_consts) cudaFreeHost(c->h_consts);
+  if (c->h_stop) cudaFreeHost(c->h_stop);
   if (c->h_flag) cudaFreeHost(c->h_flag);
   if (c->ev0) cudaEventDestroy(c->ev0);
   if (c->ev1) cudaEventDestroy(c->ev1);

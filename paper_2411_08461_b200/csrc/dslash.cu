@@ -144,6 +144,7 @@ __device__ __forceinline__ void dslash_epilogue(const DslashArgs<T>& a, int idx,
     for (int e = 0; e < 24; e++) res[e] = xv[e] + a.scale * res[e];
   }
   if (EPI == 5 || EPI == 8 || EPI == 10) {
+    if (a.scalars[S_DONE] != 0.0) return;  // converged (device-side stopping test, solver.cu): r keeps its value
     const T alpha = (T)(a.scalars[a.num] / a.scalars[a.den]);
     T rv[24];
     load_spinor<T>(a.r, Vh, idx, rv);

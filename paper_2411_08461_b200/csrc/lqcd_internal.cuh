@@ -17,7 +17,14 @@ struct Lat {
   int tb;  // +1 periodic, -1 antiperiodic in t
 };
 
-constexpr int LQCD_MAX_DEVICES = 64;  // lqcd_create refuses a larger ordinal (per-device launch configuration flags)
+constexpr int LQCD_MAX_DEVICES = 64;
+// Scalar slots of one right-hand side in ctx->d_scalars (SC_STRIDE doubles each).  The solvers' own reduction slots
+// are in solver.cu; these are shared with the kernels: S_DONE != 0 freezes a right-hand side (its BLAS blocks exit at
+// once, the fused epilogues leave r alone), S_FIRST marks BiCGStab's first iteration, and the device-side stopping
+// test (solver.cu, conv_check_kernel) keeps its threshold, its iteration counter, a flag (1 NaN, 2 rho/omega
+// underflow) and the last live residual in S_STOP, S_ITERS, S_FLAG, S_RRFIN.
+constexpr int SC_STRIDE = 64;
+constexpr int S_STOP = 56, S_ITERS = 57, S_FLAG = 58, S_RRFIN = 59, S_DONE = 60, S_FIRST = 61;  // lqcd_create refuses a larger ordinal (per-device launch configuration flags)
 
 struct lqcd_ctx {
   int L[4];
@@ -39,6 +46,7 @@ struct lqcd_ctx {
   int* d_flag;
   double* h_scalars;
   double* h_consts;  // pinned {0.0, 1.0}: sources of small asynchronous flag writes
+  double* h_stop;    // pinned, one per right-hand side: source of the asynchronous writes of the stopping thresholds
   int* h_flag;
   int max_red_blocks;
   cudaEvent_t ev0, ev1;
