@@ -72,6 +72,10 @@ const char* lqcd_strerror(int code);
 const char* lqcd_last_error(const lqcd_ctx* ctx);
 /* number of kernels this context has launched since creation (bench.py's gpu_launches) */
 long lqcd_launch_count(const lqcd_ctx* ctx);
+/* Small-lattice solves (one-parity volume x columns <= 131072) stop on the device and replay blocks of 4 Krylov
+ * iterations as CUDA graphs (LQCD_GRAPHS=0 at context creation: plain launches, same results bit for bit); this counts
+ * the blocks replayed.  Their kernels are included in lqcd_launch_count. */
+long lqcd_graph_launch_count(const lqcd_ctx* ctx);
 
 /* Algorithmic HBM bytes (compulsory reads + writes of each kernel) summed over
  * every kernel this context has launched since creation (bench.py's whole-step throughput). */

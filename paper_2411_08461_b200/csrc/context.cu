@@ -39,6 +39,7 @@ const char* lqcd_strerror(int code) {
 
 const char* lqcd_last_error(const lqcd_ctx* ctx) { return ctx ? ctx->err : "null context"; }
 long lqcd_launch_count(const lqcd_ctx* ctx) { return ctx ? ctx->launches : 0; }
+long lqcd_graph_launch_count(const lqcd_ctx* ctx) { return ctx ? ctx->graph_launches : 0; }
 
 int lqcd_create(lqcd_ctx** out, const int dims[4], int prec, int recon, int t_boundary, int device) {
   if (!out || !dims) return LQCD_ERR_INVALID_ARG;
@@ -81,6 +82,8 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], int prec, int recon, int t_bo
     c->tiled = (e && e[0] == '1') ? 1 : 0;
     const char* m = getenv("LQCD_MRHS_TMA");  // TMA-tiled multi-RHS kernel: on unless LQCD_MRHS_TMA=0 (A/B measurements, parity tests of both)
     c->mrhs_tma = (m && m[0] == '0') ? 0 : ((m && m[0] == '2') ? 2 : 1);
+    const char* gr = getenv("LQCD_GRAPHS");
+    c->graphs_on = (gr && gr[0] == '0') ? 0 : 1;
     const char* z = getenv("LQCD_MRHS_ZSLAB");
     c->mrhs_zslab = z ? atoi(z) : 4;
   }
@@ -99,6 +102,8 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], int prec, int recon, int t_bo
             cudaMallocHost(&c->h_flag, sizeof(int) * 4) == cudaSuccess &&
             cudaEventCreate(&c->ev0) == cudaSuccess && cudaEventCreate(&c->ev1) == cudaSuccess &&
             cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&c->graph_stream, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaEventCreateWithFlags(&c->ev_graph, cudaEventDisableTiming) == cudaSuccess &&
             cudaEventCreateWithFlags(&c->ev_copy[0], cudaEventDisableTiming) == cudaSuccess &&
             cudaEventCreateWithFlags(&c->ev_copy[1], cudaEventDisableTiming) == cudaSuccess &&
             cudaEventCreateWithFlags(&c->ev_copy[2], cudaEventDisableTiming) == cudaSuccess;
@@ -126,6 +131,8 @@ int lqcd_destroy(lqcd_ctx* c) {
   if (c->d_ticket) cudaFree(c->d_ticket);
   if (c->d_flag) cudaFree(c->d_flag);
   if (c->h_scalars) cudaFreeHost(c->h_scalars);
+  for (int i = 0; i < 4; i++)
+    if (c->graphs[i].exec) cudaGraphExecDestroy(c->graphs[i].exec);
   if (c->h_consts) cudaFreeHost(c->h_consts);
   if (c->h_stop) cudaFreeHost(c->h_stop);
   if (c->h_flag) cudaFreeHost(c->h_flag);
@@ -134,6 +141,8 @@ int lqcd_destroy(lqcd_ctx* c) {
   for (int i = 0; i < 3; i++)
     if (c->ev_copy[i]) cudaEventDestroy(c->ev_copy[i]);
   if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+  if (c->graph_stream) cudaStreamDestroy(c->graph_stream);
+  if (c->ev_graph) cudaEventDestroy(c->ev_graph);
   if (c->prof_ev) {
     for (int i = 0; i < 2 * c->prof_cap; i++) cudaEventDestroy(c->prof_ev[i]);
     delete[] c->prof_ev;

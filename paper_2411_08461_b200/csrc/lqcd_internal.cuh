@@ -26,12 +26,25 @@ constexpr int LQCD_MAX_DEVICES = 64;
 constexpr int SC_STRIDE = 64;
 constexpr int S_STOP = 56, S_ITERS = 57, S_FLAG = 58, S_RRFIN = 59, S_DONE = 60, S_FIRST = 61;  // lqcd_create refuses a larger ordinal (per-device launch configuration flags)
 
+// an instantiated CUDA graph of `stride` Krylov iterations (solver.cu), reused while the solve's buffers stay the same
+struct GraphSlot {
+  unsigned long long key;
+  cudaGraphExec_t exec;
+  long launches, dslashes;  // what one replay adds to the counters
+  double bytes;
+};
+
 struct lqcd_ctx {
   int L[4];
   Lat lat;
   long V;
   int prec, recon, device, sm_count;  // prec: bytes of a real of the PUBLIC arrays and of the arithmetic (4 | 8)
   int half;  // 1: native fields in 16-bit fixed point (half.cuh; created with prec = 2: fp32 arithmetic and public arrays)
+  cudaStream_t graph_stream;  // the legacy default stream cannot be captured: small-lattice solves called on it run here
+  cudaEvent_t ev_graph;
+  GraphSlot graphs[4];
+  long graph_launches;  // blocks replayed so far (lqcd_graph_launch_count)
+  int graph_next, graphs_on;  // LQCD_GRAPHS=0 (at creation) keeps every iteration a sequence of plain launches
   int part_mask;  // bit mu: direction mu is cut between ranks (lqcd_set_partition; dd.cu)
   double ws;  // weight of the spatial hops: nu/xi_0 of Eq. 5; 1 = isotropic
   int mrhs_tma;    // 1 (default): TMA-tiled multi-RHS kernel (dslash_mrhs_tma.cu) where it applies; LQCD_MRHS_TMA=0 turns it off

@@ -193,6 +193,77 @@ static void arm_check(lqcd_ctx* c, const Cols& cols, cudaStream_t st) {
 // host reads every `stride` iterations: 1 where an iteration is long against a read-back, 4 on the small lattices
 static int check_stride(const lqcd_ctx* c, int n) { return (long)c->lat.Vh * n <= 131072 ? 4 : 1; }
 
+// ---- CUDA graphs for the iteration body (SURVEY.md §7 "small-lattice solve time is launch bound: CUDA graphs for the
+// iteration body; check convergence every k iterations").  A block of `stride` iterations (an even number, starting at
+// an even iteration: the reduction slots alternate with the parity of the iteration) is captured once from the very
+// launches the plain path makes, instantiated, and replayed; the instantiated graph is kept in the context and reused
+// by later solves as long as every buffer, coefficient and shape it baked in is the same (key).
+static unsigned long long mix(unsigned long long h, unsigned long long v) {
+  h ^= v + 0x9e3779b97f4a7c15ull + (h << 6) + (h >> 2);
+  return h;
+}
+static unsigned long long graph_key(const lqcd_ctx* c, int tag, const Work& w, const void* gauge, const void* A, const void* Ai,
+                                    double kappa, int matpc, int variant, int stride) {
+  unsigned long long h = 0x12345 + tag;
+  const void* ptrs[] = {w.x, w.v[0], w.v[1], w.v[2], w.v[3], w.v[4], w.v[5], w.v[6], w.v[7], gauge, A, Ai};
+  for (const void* p : ptrs) h = mix(h, (unsigned long long)(uintptr_t)p);
+  unsigned long long kb, wb;
+  memcpy(&kb, &kappa, 8);
+  memcpy(&wb, &c->ws, 8);
+  h = mix(h, kb);
+  h = mix(h, wb);
+  h = mix(h, (unsigned long long)w.nrhs << 32 | (unsigned)matpc << 16 | (unsigned)variant << 8 | (unsigned)stride);
+  h = mix(h, (unsigned long long)c->part_mask << 8 | (unsigned)c->lat.tb + 2);
+  return h | 1;  // never 0: 0 marks an empty slot
+}
+// runs iterations it0 .. it0+stride-1 as one graph launch; `iterate(it)` enqueues one iteration on `st`
+template <typename F>
+static int run_block(lqcd_ctx* c, unsigned long long key, int stride, int it0, F& iterate, long& dslashes, cudaStream_t st) {
+  for (int i = 0; i < 4; i++)
+    if (c->graphs[i].key == key && c->graphs[i].exec) {
+      GraphSlot& g = c->graphs[i];
+      if (cudaGraphLaunch(g.exec, st) != cudaSuccess) return lqcd_check_cuda(c, "graph launch");
+      c->graph_launches++;
+      c->launches += g.launches;
+      c->alg_bytes += g.bytes;
+      dslashes += g.dslashes;
+      return LQCD_OK;
+    }
+  const long l0 = c->launches, d0 = dslashes;
+  const double b0 = c->alg_bytes;
+  if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+    cudaGetLastError();
+    c->graphs_on = 0;
+    return -1000;  // not capturable here: the caller falls back to plain launches
+  }
+  int rc = LQCD_OK;
+  for (int i = 0; i < stride && !rc; i++) rc = iterate(it0 + i);
+  cudaGraph_t graph = nullptr;
+  const cudaError_t e = cudaStreamEndCapture(st, &graph);
+  cudaGraphExec_t exec = nullptr;
+  if (rc || e != cudaSuccess || cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) {
+    if (graph) cudaGraphDestroy(graph);
+    cudaGetLastError();
+    c->graphs_on = 0;
+    c->launches = l0;
+    c->alg_bytes = b0;
+    dslashes = d0;
+    return rc ? rc : -1000;
+  }
+  cudaGraphDestroy(graph);
+  GraphSlot& g = c->graphs[c->graph_next];
+  c->graph_next = (c->graph_next + 1) & 3;
+  if (g.exec) cudaGraphExecDestroy(g.exec);
+  g.key = key;
+  g.exec = exec;
+  g.launches = c->launches - l0;
+  g.bytes = c->alg_bytes - b0;
+  g.dslashes = dslashes - d0;
+  if (cudaGraphLaunch(exec, st) != cudaSuccess) return lqcd_check_cuda(c, "graph launch");
+  c->graph_launches++;
+  return LQCD_OK;
+}
+
 static int solve_cg(lqcd_ctx* c, const Work& w, const void* gauge, const void* A, const void* Ai, double kappa,
                     int matpc, int normal_residual, Cols& cols, int maxiter, lqcd_result* res, cudaStream_t st) {
   // CGNE (normal_residual = 0): Mhat Mhat^dag y = bhat, x = Mhat^dag y.   bhat in v[0], x_e in w.x
@@ -236,8 +307,8 @@ static int solve_cg(lqcd_ctx* c, const Work& w, const void* gauge, const void* A
   const bool fused = n == 1 && lqcd_dslash_fuse_ok(c);
   const int stride = check_stride(c, n);
   arm_check(c, cols, st);
-  int it = 0;
-  while (it < maxiter && cols.nactive() > 0) {
+  // one iteration, enqueued on `st` (plain launches, or recorded into a graph by run_block)
+  auto iterate = [&](int it) -> int {
     const int cur = (it & 1) ? S_RR1 : S_RR0, nxt = (it & 1) ? S_RR0 : S_RR1;
     int outs[4] = {S_TT, 0, 0, 0};
     if (!normal_residual && fused && matpc == LQCD_MATPC_SYMMETRIC_RIGHT) {
@@ -304,9 +375,29 @@ static int solve_cg(lqcd_ctx* c, const Work& w, const void* gauge, const void* A
     dslashes += 4;
     void* u3[2] = {p, r};
     if ((rc = BLAS_CALL(c, OpXpayRatio, (op.num = nxt, op.den = cur), u3, nullptr, n, 0, st))) return rc;  // p = r + beta p
-    it++;
-    if ((rc = conv_check(c, n, normal_residual ? S_RES : nxt, -1, -1, st))) return rc;
-    if (it % stride && it < maxiter) continue;
+    return conv_check(c, n, normal_residual ? S_RES : nxt, -1, -1, st);
+  };
+  const bool graphs = c->graphs_on && stride > 1 && !c->prof_on;
+  const unsigned long long key = graph_key(c, 1 + normal_residual, w, gauge, A, Ai, kappa, matpc, fused, stride);
+  int it = 0, since_read = 0;
+  while (it < maxiter && cols.nactive() > 0) {
+    bool block = graphs && c->graphs_on && it >= 2 && !(it & 1) && it + stride <= maxiter;
+    if (block) {
+      rc = run_block(c, key, stride, it, iterate, dslashes, st);
+      if (rc == -1000) block = false;
+      else if (rc) return rc;
+      else {
+        it += stride;
+        since_read = stride;
+      }
+    }
+    if (!block) {
+      if ((rc = iterate(it))) return rc;
+      it++;
+      since_read++;
+    }
+    if (since_read < stride && it < maxiter) continue;
+    since_read = 0;
     if ((rc = read_scalars(c, n, st))) return rc;
     for (int j = 0; j < n; j++) {
       if (!cols.active[j]) continue;
@@ -357,8 +448,8 @@ static int solve_bicgstab(lqcd_ctx* c, const Work& w, const void* gauge, const v
   }
   const int stride = check_stride(c, n);
   arm_check(c, cols, st);
-  int it = 0;
-  while (it < maxiter && cols.nactive() > 0) {
+  // one iteration, enqueued on `st` (plain launches, or recorded into a graph by run_block)
+  auto iterate = [&](int it) -> int {
     const int rho = (it & 1) ? S_RHO1 : S_RHO0, rho_next = (it & 1) ? S_RHO0 : S_RHO1;
     {
       void* u[3] = {p, r, v};
@@ -386,9 +477,30 @@ static int solve_bicgstab(lqcd_ctx* c, const Work& w, const void* gauge, const v
       if ((rc = BLAS_CALL(c, OpBicgXR, (op.rho = rho, op.r0v = S_R0V, op.ts = S_TS), u2, o2, n, 0, st))) return rc;
     }
     dslashes += 4;
-    it++;
-    if ((rc = conv_check(c, n, S_RR, rho_next, S_TS, st))) return rc;
-    if (it % stride && it < maxiter) continue;
+    return conv_check(c, n, S_RR, rho_next, S_TS, st);
+  };
+  const bool graphs = c->graphs_on && stride > 1 && !c->prof_on;
+  const unsigned long long key = graph_key(c, 3, w, gauge, A, Ai, kappa, matpc, 0, stride);
+  int it = 0, since_read = 0;
+  while (it < maxiter && cols.nactive() > 0) {
+    // a block never contains a first iteration (start, or a restarted column): those clear S_FIRST from the host
+    bool block = graphs && c->graphs_on && !first_pending && it >= 2 && !(it & 1) && it + stride <= maxiter;
+    if (block) {
+      rc = run_block(c, key, stride, it, iterate, dslashes, st);
+      if (rc == -1000) block = false;
+      else if (rc) return rc;
+      else {
+        it += stride;
+        since_read = stride;
+      }
+    }
+    if (!block) {
+      if ((rc = iterate(it))) return rc;
+      it++;
+      since_read++;
+    }
+    if (since_read < stride && it < maxiter) continue;
+    since_read = 0;
     if ((rc = read_scalars(c, n, st))) return rc;
     for (int j = 0; j < n; j++) {
       if (!cols.active[j]) continue;
@@ -757,6 +869,14 @@ static int invert_common(lqcd_ctx* c, void* x_public, const void* b_public, cons
   const void* p[6] = {x_public, b_public, gauge, clover, clover_inv, workspace};
   if (!check_ptrs(c, p, 6, "invert")) return LQCD_ERR_ALIGN;
   memset(res, 0, sizeof(*res) * nrhs);
+  // A small-lattice solve replays its iterations as CUDA graphs, and the legacy default stream (what PyTorch hands out
+  // unless told otherwise) cannot be captured: such a solve runs on a stream of the context, ordered after the work
+  // already queued on the caller's stream; the call synchronises before it returns, as lqcd_invert always does.
+  if (c->graphs_on && (st == nullptr || st == cudaStreamLegacy) && check_stride(c, nrhs) > 1) {
+    cudaEventRecord(c->ev_graph, st);
+    cudaStreamWaitEvent(c->graph_stream, c->ev_graph, 0);
+    st = c->graph_stream;
+  }
   const long launches0 = c->launches, mixed_launches0 = mixed ? mixed->ci->launches : 0;
   const size_t sp = lqcd_spinor_bytes(c);
   const size_t psp = (size_t)c->lat.Vh * 24 * c->prec;  // one parity of a PUBLIC spinor (16-bit context: complex64)

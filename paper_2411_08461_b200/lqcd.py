@@ -39,7 +39,7 @@ SYMBOLS = [
     "lqcd_momentum_phase", "lqcd_source_wall", "lqcd_source_point", "lqcd_propagator_assemble",
     "lqcd_propagator_split", "lqcd_contract_twopt", "lqcd_contract_threept", "lqcd_sequential_source",
     "lqcd_clover_to_half", "lqcd_set_partition", "lqcd_face_bytes", "lqcd_dslash_dd_interior", "lqcd_face_pack",
-    "lqcd_face_unpack", "lqcd_clover_pack",
+    "lqcd_face_unpack", "lqcd_clover_pack", "lqcd_graph_launch_count",
 ]
 MAX_RHS = 16
 
@@ -66,6 +66,8 @@ def load():
     L.lqcd_last_error.argtypes = [vp]
     L.lqcd_launch_count.restype = ctypes.c_long
     L.lqcd_launch_count.argtypes = [vp]
+    L.lqcd_graph_launch_count.restype = ctypes.c_long
+    L.lqcd_graph_launch_count.argtypes = [vp]
     L.lqcd_algorithmic_bytes.restype = cd
     L.lqcd_algorithmic_bytes.argtypes = [vp]
     L.lqcd_profile_enable.argtypes = [vp, ci]
@@ -239,6 +241,9 @@ class Context:
 
     def launch_count(self):
         return self.lib.lqcd_launch_count(self.h)
+
+    def graph_launch_count(self):
+        return self.lib.lqcd_graph_launch_count(self.h)
 
     def algorithmic_bytes(self):
         return self.lib.lqcd_algorithmic_bytes(self.h)

@@ -236,3 +236,28 @@ def test_degenerate_sources_and_lucky_breakdown():
         x1, r1 = s.ctx.invert(s.ctx.to_device(b), s.gauge, A1, Ai1, 0.0, tol=1e-12, solver=solver)
         assert r1.status == 0 and r1.iterations <= 1, r1.as_dict()
         assert rel_err(x1.cpu().numpy(), b) < 1e-14
+
+
+@pytest.mark.parametrize("solver,matpc", [("cgne", 0), ("cgne", 2), ("cgnr", 1), ("bicgstab", 1)])
+def test_graph_replayed_iterations_equal_plain_launches(solver, matpc, monkeypatch):
+    """Small lattices run blocks of 4 iterations as one CUDA graph and stop on the device (solver.cu): the result must
+    be bit for bit that of the plain launch sequence (LQCD_GRAPHS=0), also when the instantiated graph is reused by a
+    second solve with the same workspace and a different source, and for a batch of columns that stop at different
+    iterations."""
+    s, c = from_cfg(2, 8, 18)
+    monkeypatch.setenv("LQCD_GRAPHS", "0")
+    plain = lq().Context(c["dims"], 8, 18, -1)
+    ws, _ = s.ctx.workspace(solver)
+    wp, _ = plain.workspace(solver)
+    for seed in (1, 2):
+        b = s.ctx.to_device(synth.source(c["dims"], "gaussian", seed))
+        x1, r1 = s.ctx.invert(b, s.gauge, s.A, s.Ai, s.kappa, tol=1e-10, solver=solver, matpc=matpc, workspace=ws)
+        x2, r2 = plain.invert(b, s.gauge, s.A, s.Ai, s.kappa, tol=1e-10, solver=solver, matpc=matpc, workspace=wp)
+        assert r1.status == 0 and r1.iterations == r2.iterations and r1.iterations > 6
+        assert torch.equal(x1, x2) and r1.true_resid == r2.true_resid
+    assert s.ctx.graph_launch_count() >= 2 and plain.graph_launch_count() == 0
+    cols = np.stack([synth.source(c["dims"], "gaussian", 3), synth.source(c["dims"], "point"), 1e-3 * synth.source(c["dims"], "z2", 4)])
+    B = s.ctx.to_device(cols)
+    xa, ra, _ = s.ctx.invert_multi(B, s.gauge, s.A, s.Ai, s.kappa, tol=1e-10, solver=solver, matpc=matpc)
+    xb, rb, _ = plain.invert_multi(B, s.gauge, s.A, s.Ai, s.kappa, tol=1e-10, solver=solver, matpc=matpc)
+    assert [r.iterations for r in ra] == [r.iterations for r in rb] and torch.equal(xa, xb)
