@@ -454,7 +454,7 @@ def small_solves(torch, lqcd, synth, device):
         out["config%d_fp%d_recon%d_%s" % (n, 8 * prec, recon, solver)] = {
             "dims": list(c["dims"]), "tol": tol, "matpc": matpc, "us": best.seconds * 1e6, "iterations": best.iterations,
             "us_per_iteration": best.seconds * 1e6 / max(best.iterations, 1), "kernel_launches": best.kernel_launches,
-            "true_resid": best.true_resid, "status": best.status}
+            "true_resid": best.true_resid, "status": best.status, "graph_blocks_replayed": ctx.graph_launch_count()}
         ctx.close()
     return out
 
