@@ -709,6 +709,7 @@ def main():
     ap.add_argument("--no-sweep", action="store_true", help="skip the standalone dslash sweep")
     ap.add_argument("--no-extras", action="store_true", help="skip the SURVEY 8(f) rows (mixed precision, batched propagator)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the CPU-oracle baseline leg")
+    ap.add_argument("--mrhs-only", action="store_true", help="only the standalone multi-RHS dslash sweep (profiling runs)")
     args = ap.parse_args()
     if args.impl == "cpu-leg":
         c, n, i0, i1 = (int(v) for v in args.cpu_leg.split(","))
@@ -718,6 +719,14 @@ def main():
         return subprocess.call(spawn_command(args))  # N ranks, one per GPU; rank 0 prints the line with n_gpus = N
     if args.impl == "selftest":
         return run_selftest(args)
+    if args.mrhs_only:
+        import torch
+        from paper_2411_08461_b200 import lqcd, synth
+        cfg = synth.CONFIGS[WORKLOAD]
+        U = synth.gauge(cfg["dims"], cfg["eps"], cfg["seed"])
+        b = synth.source(cfg["dims"], cfg["source"], cfg["src_seed"])
+        print(json.dumps({"dslash_mrhs_32x64": mrhs_sweep(torch, lqcd, U, b, cfg["dims"], 0, measured_peaks()[0])}))
+        return 0
     if args.impl == "reference":
         return run_reference(args)
     return run_gpu(args)
