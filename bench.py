@@ -710,6 +710,8 @@ def main():
     ap.add_argument("--no-extras", action="store_true", help="skip the SURVEY 8(f) rows (mixed precision, batched propagator)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the CPU-oracle baseline leg")
     ap.add_argument("--mrhs-only", action="store_true", help="only the standalone multi-RHS dslash sweep (profiling runs)")
+    ap.add_argument("--propagator-only", action="store_true",
+                    help="only the batched 12-column mixed-precision BiCGStab propagator at 32^3x64 (profiling runs)")
     args = ap.parse_args()
     if args.impl == "cpu-leg":
         c, n, i0, i1 = (int(v) for v in args.cpu_leg.split(","))
@@ -719,6 +721,24 @@ def main():
         return subprocess.call(spawn_command(args))  # N ranks, one per GPU; rank 0 prints the line with n_gpus = N
     if args.impl == "selftest":
         return run_selftest(args)
+    if args.propagator_only:
+        import torch
+        from paper_2411_08461_b200 import lqcd, synth
+        cfg = synth.CONFIGS[WORKLOAD]
+        dims, kappa, csw = cfg["dims"], cfg["kappa"], cfg["csw"]
+        U = synth.gauge(dims, cfg["eps"], cfg["seed"])
+        ctx, lo = lqcd.Context(dims, 8, 18, -1, 0), lqcd.Context(dims, 4, 12, -1, 0)
+        g, g_lo = ctx.gauge_pack(ctx.to_device(U)), lo.gauge_pack(lo.to_device(U))
+        (A, Ai), (A_lo, Ai_lo) = ctx.clover_build(g, csw, kappa), lo.clover_build(g_lo, csw, kappa)
+        B = ctx.to_device(np.stack([synth.source(dims, "point", spin=sp, colour=c) for sp in range(4) for c in range(3)]))
+        ws, _ = ctx.workspace_multi(12, "bicgstab")
+        ws_lo, _ = lo.workspace_multi(12, "bicgstab")
+        for _ in range(2):
+            _, rs, rc = ctx.invert_multi_mixed(lo, B, g, A, Ai, g_lo, A_lo, Ai_lo, kappa, tol=1e-10, inner_tol=1e-5, maxiter=2000,
+                                               solver="bicgstab", matpc=1, workspace=ws, workspace_lo=ws_lo)
+        print(json.dumps({"propagator_32x64_mixed_bicgstab_batched_ms": rs[0].seconds * 1e3, "status": rc,
+                          "inner_iterations": [r.iterations for r in rs], "launches": rs[0].kernel_launches}))
+        return 0
     if args.mrhs_only:
         import torch
         from paper_2411_08461_b200 import lqcd, synth
