@@ -386,13 +386,15 @@ def extras(torch, lqcd, synth, U, b, ctx, gauge, device):
     A3, Ai3 = p.clover_build(g3, c3["csw"], c3["kappa"])
     cols = np.stack([synth.source(dims, "point", spin=sp, colour=c) for sp in range(4) for c in range(3)])
     B = p.to_device(cols)
+    ws1, _ = p.workspace("cgne")          # one workspace for the single solves, one for the batched call: like for like
+    ws12, _ = p.workspace_multi(12, "cgne")
     for _ in range(2):
         e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
         e0.record()
-        its = [p.invert(B[j], g3, A3, Ai3, c3["kappa"], tol=1e-6, solver="cgne", matpc=MATPC)[1].iterations
+        its = [p.invert(B[j], g3, A3, Ai3, c3["kappa"], tol=1e-6, solver="cgne", matpc=MATPC, workspace=ws1)[1].iterations
                for j in range(12)]
         e1.record()
-        _, rs, rc = p.invert_multi(B, g3, A3, Ai3, c3["kappa"], tol=1e-6, solver="cgne", matpc=MATPC)
+        _, rs, rc = p.invert_multi(B, g3, A3, Ai3, c3["kappa"], tol=1e-6, solver="cgne", matpc=MATPC, workspace=ws12)
         e2.record()
         torch.cuda.synchronize()
     out["propagator_16x32_fp32_recon12"] = {
