@@ -759,66 +759,83 @@ static int invert_native_body(lqcd_ctx* c, Work& w, const void* gauge, const voi
   }
   if (matpc == LQCD_MATPC_SYMMETRIC)
     if ((rc = lqcd_clover_apply_launch(c, bh, bh, Ai_e, n, st))) return rc;
-  for (int pass = 0;; pass++) {
-    bool in_pass[LQCD_MAX_RHS];  // the Krylov loop clears cols.active[j] when column j stops
-    for (int j = 0; j < n; j++) {
-      in_pass[j] = cols.active[j];
-      if (!cols.active[j]) set_slot(c, j, S_DONE, true, st);
-    }
-    c->acct_rhs = cols.nactive();
-    int done = 0;
-    for (int j = 0; j < n; j++)
-      if (cols.active[j] && cols.base_it[j] > done) done = cols.base_it[j];
-    const int left = maxiter - done;
-    if (mixed) rc = solve_mixed(c, w, gauge, A, Ai, kappa, matpc, solver, cols, left, res, *mixed, st);
-    else if (solver == LQCD_SOLVER_BICGSTAB) rc = solve_bicgstab(c, w, gauge, A, Ai, kappa, matpc, cols, left, res, st);
-    else rc = solve_cg(c, w, gauge, A, Ai, kappa, matpc, solver == LQCD_SOLVER_CGNR, cols, left, res, st);
-    c->acct_rhs = 0;
-    if (rc) return rc;
-    set_slot_all(c, n, S_DONE, false, st);  // the closing steps below update every column
+  // closing steps for n columns given by their own pointers (all columns of the batch, or one column of it):
+  // unknown back to x_e (right-preconditioned form), a10: x_o = A_oo^-1 (b_o + kappa D_oe x_e), a11: the true residual
+  // b - M x with the full operator into (r1, r2), its norms into S_TRUE, S_TRUE + 1
+  auto finish = [&](char* be, char* bo, char* xe, char* xo, char* r1, char* r2, char* t5, int m) -> int {
+    int e;
     if (matpc == LQCD_MATPC_SYMMETRIC_RIGHT)     // the Krylov unknown was y = A_ee x_e
-      if ((rc = lqcd_clover_apply_launch(c, x_e, x_e, Ai_e, n, st))) return rc;
-    // a10: x_o = A_oo^-1 (b_o + kappa D_oe x_e)
-    if ((rc = lqcd_dslash_launch(c, w.v[5], x_e, gauge, nullptr, nullptr, 1, kappa, 0, 0, n, st))) return rc;
+      if ((e = lqcd_clover_apply_launch(c, xe, xe, Ai_e, m, st))) return e;
+    if ((e = lqcd_dslash_launch(c, t5, xe, gauge, nullptr, nullptr, 1, kappa, 0, 0, m, st))) return e;
     {
-      void* v[2] = {b_o, w.v[5]};
-      if ((rc = BLAS_CALL(c, OpXpay, op.a = 1.0, v, nullptr, n, 0, st))) return rc;
+      void* v[2] = {bo, t5};
+      if ((e = BLAS_CALL(c, OpXpay, op.a = 1.0, v, nullptr, m, 0, st))) return e;
     }
-    if ((rc = lqcd_clover_apply_launch(c, x_o, w.v[5], Ai_o, n, st))) return rc;
-    // a11: true residual |b - M x| / |b| with the full operator; v[1], v[2] are adjacent blocks
-    if ((rc = mat_apply(c, w.v[1], w.x, gauge, A, kappa, 0, n, st))) return rc;
+    if ((e = lqcd_clover_apply_launch(c, xo, t5, Ai_o, m, st))) return e;
+    if ((e = lqcd_dslash_launch(c, r1, xo, gauge, A, xe, 0, -kappa, 0, 2, m, st))) return e;
+    if ((e = lqcd_dslash_launch(c, r2, xe, gauge, off(A, half), xo, 1, -kappa, 0, 2, m, st))) return e;
     {
-      void* v[2] = {b_e, w.v[1]};
+      void* v[2] = {be, r1};
       int o[4] = {S_TRUE, 0, 0, 0};
-      if ((rc = BLAS_CALL(c, OpAxpyNorm, op.a = -1.0, v, o, n, 0, st))) return rc;
-      void* v2[2] = {b_o, w.v[2]};
+      if ((e = BLAS_CALL(c, OpAxpyNorm, op.a = -1.0, v, o, m, 0, st))) return e;
+      void* v2[2] = {bo, r2};
       int o2[4] = {S_TRUE + 1, 0, 0, 0};
-      if ((rc = BLAS_CALL(c, OpAxpyNorm, op.a = -1.0, v2, o2, n, 0, st))) return rc;
+      if ((e = BLAS_CALL(c, OpAxpyNorm, op.a = -1.0, v2, o2, m, 0, st))) return e;
     }
-    if ((rc = read_scalars(c, n, st))) return rc;
-    for (int j = 0; j < n; j++) res[j].dslash_count += pass == 0 ? 4 : 3;  // (first pass: prepare,) reconstruct, two for the true residual
-    // which columns go on: recurrence converged, true residual above the bar and still falling
-    int again = 0;
-    for (int j = 0; j < n; j++) {
-      cols.active[j] = false;
-      if (!solvable[j] || !in_pass[j]) continue;
-      const double t2 = hs(c, j, S_TRUE) + hs(c, j, S_TRUE + 1), before = true_rr[j];
+    return read_scalars(c, m, st);
+  };
+  // pass 0: all columns in lock step
+  for (int j = 0; j < n; j++)
+    if (!cols.active[j]) set_slot(c, j, S_DONE, true, st);
+  c->acct_rhs = cols.nactive();
+  if (mixed) rc = solve_mixed(c, w, gauge, A, Ai, kappa, matpc, solver, cols, maxiter, res, *mixed, st);
+  else if (solver == LQCD_SOLVER_BICGSTAB) rc = solve_bicgstab(c, w, gauge, A, Ai, kappa, matpc, cols, maxiter, res, st);
+  else rc = solve_cg(c, w, gauge, A, Ai, kappa, matpc, solver == LQCD_SOLVER_CGNR, cols, maxiter, res, st);
+  c->acct_rhs = 0;
+  if (rc) return rc;
+  set_slot_all(c, n, S_DONE, false, st);  // the closing steps update every column
+  if ((rc = finish(b_e, b_o, x_e, x_o, w.v[1], w.v[2], w.v[5], n))) return rc;
+  for (int j = 0; j < n; j++) {
+    res[j].dslash_count += 4;  // prepare, reconstruct, two for the true residual
+    true_rr[j] = solvable[j] ? hs(c, j, S_TRUE) + hs(c, j, S_TRUE + 1) : 0.0;
+  }
+  // residual replacement, column by column (a one-column view of the batch: the single-RHS kernels run, the other
+  // columns are not touched): only where the recurrence converged and the true residual is still above the bar
+  for (int j = 0; j < n && !mixed; j++) {
+    if (!solvable[j] || res[j].status != LQCD_OK) continue;
+    Work w1 = w;
+    w1.nrhs = 1;
+    w1.x = x_e + j * sp;
+    for (int i = 0; i < 9; i++) w1.v[i] = w.v[i] + j * sp;
+    double target = stop2[j];
+    for (int pass = 1; pass < MAX_PASSES; pass++) {
+      if (cols.rr[j] > target || !(true_rr[j] > stop2[j]) || res[j].iterations >= maxiter) break;
+      target *= 0.25;
+      if (matpc == LQCD_MATPC_SYMMETRIC_RIGHT)  // back to the Krylov unknown y = A_ee x_e
+        if ((rc = lqcd_clover_apply_launch(c, w1.x, w1.x, A, 1, st))) return rc;
+      Cols c1;
+      c1.n = 1;
+      c1.warm = true;
+      c1.active[0] = true;
+      c1.stop2[0] = target;
+      c1.bb[0] = cols.bb[j];
+      c1.rr[0] = cols.rr[j];
+      c1.base_it[0] = res[j].iterations;
+      c->acct_rhs = 1;
+      const int left = maxiter - res[j].iterations;
+      if (solver == LQCD_SOLVER_BICGSTAB) rc = solve_bicgstab(c, w1, gauge, A, Ai, kappa, matpc, c1, left, res + j, st);
+      else rc = solve_cg(c, w1, gauge, A, Ai, kappa, matpc, solver == LQCD_SOLVER_CGNR, c1, left, res + j, st);
+      c->acct_rhs = 0;
+      if (rc) return rc;
+      set_slot(c, 0, S_DONE, false, st);
+      if ((rc = finish(b_e + j * sp, b_o + j * sp, w1.x, x_o + j * sp, w1.v[1], w1.v[2], w1.v[5], 1))) return rc;
+      res[j].dslash_count += 3;
+      cols.rr[j] = c1.rr[0];
+      const double t2 = hs(c, 0, S_TRUE) + hs(c, 0, S_TRUE + 1), before = true_rr[j];
       true_rr[j] = t2;
-      cols.base_it[j] = res[j].iterations;
-      const bool improving = pass == 0 || t2 < 0.5 * before;
-      if (mixed || res[j].status != LQCD_OK || cols.rr[j] > cols.stop2[j] || !(t2 > stop2[j]) || !improving ||
-          pass + 1 >= MAX_PASSES || res[j].iterations >= maxiter)
-        continue;
-      cols.active[j] = true;
-      cols.stop2[j] *= 0.25;
-      again++;
+      if (res[j].status != LQCD_OK || !(t2 < 0.5 * before)) break;  // no longer improving: the floor of the storage type
     }
-    if (again == 0) break;
-    cols.warm = true;
-    if (matpc == LQCD_MATPC_SYMMETRIC_RIGHT)  // back to the Krylov unknown y = A_ee x_e, restarted columns only
-      for (int j = 0; j < n; j++)
-        if (cols.active[j])
-          if ((rc = lqcd_clover_apply_launch(c, x_e + j * sp, x_e + j * sp, A, 1, st))) return rc;
+    cols.stop2[j] = target;
   }
   for (int j = 0; j < n; j++) {
     if (!solvable[j]) continue;
