@@ -127,6 +127,7 @@ int lqcd_destroy(lqcd_ctx* c) {
   if (!c) return LQCD_ERR_INVALID_ARG;
   cudaSetDevice(c->device);
   if (c->d_partial) cudaFree(c->d_partial);
+  if (c->d_partial_mrhs) cudaFree(c->d_partial_mrhs);
   if (c->d_scalars) cudaFree(c->d_scalars);
   if (c->d_ticket) cudaFree(c->d_ticket);
   if (c->d_flag) cudaFree(c->d_flag);

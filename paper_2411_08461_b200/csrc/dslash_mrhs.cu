@@ -11,12 +11,9 @@
 // of every group reads them from there: re-reading them per column through L1 put up to (8R+72)w bytes
 // per site and column on the L2->SM crossbar, which is what bounds this kernel (12 columns at 32^3x64, fp32
 // 18-real links: 1037 -> 850 us, M-hat 2884 -> 2130 us).  Epilogues are those of dslash.cu.
-// packed FFMA2 arithmetic (lqcd_internal.cuh) is off here: measured at 32^3x64, 12 columns, it changes nothing
-// for 12-real links (1015 vs 1008 us) and the paired registers push the 18-real kernel into spills
-#ifndef MRHS_FFMA2
-#define MRHS_FFMA2 0
-#endif
-#define DSLASH_FFMA2 MRHS_FFMA2
+// Packed FFMA2 arithmetic (lqcd_internal.cuh) is off in this file: measured at 32^3x64, 12 columns, it changes nothing
+// for 12-real links (1015 vs 1008 us) and the paired registers push the 18-real kernel into spills (round 1).
+#define DSLASH_FFMA2 0
 #include "dslash.cuh"
 
 #ifndef MRHS_NB_F32
@@ -51,7 +48,19 @@ template <typename T> struct MrhsArgs {
   T ws;           // weight of the spatial hops (anisotropy nu/xi_0)
   size_t stride;  // reals between consecutive right-hand sides (24 * Vh)
   int ngroups;    // nrhs / NB column groups; group g is handled by threadIdx.y = g mod blockDim.y
+  // epilogues 9 and 10 (CG recurrences fused per column, as in dslash.cu)
+  T* r;             // epi 10: residual block, r -= (s[num]/s[den]) q, per column
+  T* out2;          // epi 9: second output, C * out
+  double* partial;  // [column][block]: one partial sum per warp (= 32 sites of one column)
+  const double* scalars;
+  int num, den, nblocks;
 };
+__host__ __device__ constexpr bool mrhs_clover(int epi) { return epi == 1 || epi == 2 || epi == 3 || epi == 9; }
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  return v;
+}
 
 template <typename T, int R, int MU, bool FWD, bool DAG, int NB>
 __device__ __forceinline__ void hop_mrhs(T (*acc)[24], const T* __restrict__ in, size_t stride,
@@ -124,7 +133,7 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kern
   typedef typename GV<T, R>::vec gvec;
   constexpr int NGV = R / GV<T, R>::N;
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  __shared__ typename V16<T>::vec cl_sm[(EPI >= 1 && EPI != 6) ? Lay<T>::NCV * MRHS_SITES : 1];
+  __shared__ typename V16<T>::vec cl_sm[mrhs_clover(EPI) ? Lay<T>::NCV * MRHS_SITES : 1];
   extern __shared__ __align__(16) unsigned char mrhs_lk_smem[];  // the eight links of the block's sites: [hop][vector][site]
   gvec* lk_sm = reinterpret_cast<gvec*>(mrhs_lk_smem);
   const Lat& L = a.lat;
@@ -153,7 +162,7 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kern
       for (int v = 0; v < NGV; v++) lk_sm[(h * NGV + v) * MRHS_SITES + threadIdx.x] = ld_stream(gp + (size_t)v * Vh);
     }
   }
-  if (EPI >= 1 && EPI != 6) stage_clover_block<T>(cl_sm, a.cl, Vh, blockIdx.x * blockDim.x);
+  if (mrhs_clover(EPI)) stage_clover_block<T>(cl_sm, a.cl, Vh, blockIdx.x * blockDim.x);
   __syncthreads();
   if (!live) return;
   for (int g = threadIdx.y; g < a.ngroups; g += blockDim.y) {
@@ -213,6 +222,47 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kern
       for (int e = 0; e < 24; e++) res[r][e] += a.scale * acc[r][e];
       store_spinor<T>(out + r * stride, Vh, idx, res[r]);
     }
+  } else if (EPI == 9) {  // t = x + scale * C d ; ta = C t ; |t|^2 per column (Vh a multiple of 32: full warps)
+    T res[NB][24], res2[NB][24];
+    clover_mul_mrhs<T, NB>(cl_sm, acc, res);
+#pragma unroll
+    for (int r = 0; r < NB; r++) {
+      T xv[24];
+      load_spinor<T>(a.x + first + r * stride, Vh, idx, xv);
+#pragma unroll
+      for (int e = 0; e < 24; e++) res[r][e] = xv[e] + a.scale * res[r][e];
+    }
+    clover_mul_mrhs<T, NB>(cl_sm, res, res2);
+#pragma unroll
+    for (int r = 0; r < NB; r++) {
+      double local = 0;
+#pragma unroll
+      for (int e = 0; e < 24; e++) local += (double)res[r][e] * res[r][e];
+      store_spinor<T>(out + r * stride, Vh, idx, res[r]);
+      store_spinor<T>(a.out2 + first + r * stride, Vh, idx, res2[r]);
+      local = warp_sum(local);
+      if (threadIdx.x == 0) a.partial[(size_t)(g * NB + r) * a.nblocks + blockIdx.x] = local;
+    }
+  } else if (EPI == 10) {  // q = x + scale * d not stored ; r -= (s[num]/s[den]) q ; |r|^2 per column
+#pragma unroll
+    for (int r = 0; r < NB; r++) {
+      const double* sc = a.scalars + (size_t)(g * NB + r) * SC_STRIDE;
+      double local = 0;
+      if (sc[S_DONE] == 0.0) {  // a converged column keeps its r
+        const T alpha = (T)(sc[a.num] / sc[a.den]);
+        T xv[24], rv[24];
+        load_spinor<T>(a.x + first + r * stride, Vh, idx, xv);
+        load_spinor<T>(a.r + first + r * stride, Vh, idx, rv);
+#pragma unroll
+        for (int e = 0; e < 24; e++) {
+          rv[e] -= alpha * (xv[e] + a.scale * acc[r][e]);
+          local += (double)rv[e] * rv[e];
+        }
+        store_spinor<T>(a.r + first + r * stride, Vh, idx, rv);
+      }
+      local = warp_sum(local);
+      if (threadIdx.x == 0) a.partial[(size_t)(g * NB + r) * a.nblocks + blockIdx.x] = local;
+    }
   } else {
     T res[NB][24];
     clover_mul_mrhs<T, NB>(cl_sm, acc, res);
@@ -226,6 +276,22 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kern
     }
   }
   }  // column groups
+}
+
+// sums the per-warp partials of one column in a fixed order -> scalars[column][slot] (deterministic)
+__global__ void __launch_bounds__(256) partial_sum_mrhs_kernel(const double* __restrict__ partial, int nblocks, double* scalars, int slot) {
+  __shared__ double sm[8];
+  const double* p = partial + (size_t)blockIdx.x * nblocks;
+  double v = 0;
+  for (int b = threadIdx.x; b < nblocks; b += 256) v += p[b];
+  v = warp_sum(v);
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0;
+    for (int w = 0; w < 8; w++) t += sm[w];
+    scalars[(size_t)blockIdx.x * SC_STRIDE + slot] = t;
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -293,7 +359,7 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsStage<T, R>::MINB) dslash_mrhs_
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   typedef typename GV<T, R>::vec gvec;
   constexpr int NGV = R / GV<T, R>::N;
-  __shared__ vec cl_sm[(EPI >= 1 && EPI != 6) ? Lay<T>::NCV * MRHS_SITES : 1];
+  __shared__ vec cl_sm[mrhs_clover(EPI) ? Lay<T>::NCV * MRHS_SITES : 1];
   __shared__ gvec lk_sm[8 * NGV * MRHS_SITES];  // the eight links of the block's sites: [hop][vector][site]
   const Lat& L = a.lat;
   const int Vh = L.Vh, par = a.parity;
@@ -322,7 +388,7 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsStage<T, R>::MINB) dslash_mrhs_
       for (int v = 0; v < NGV; v++) lk_sm[(h * NGV + v) * MRHS_SITES + threadIdx.x] = ld_stream(gp + (size_t)v * Vh);
     }
   }
-  if (EPI >= 1 && EPI != 6) stage_clover_block<T>(cl_sm, a.cl, Vh, blockIdx.x * blockDim.x);
+  if (mrhs_clover(EPI)) stage_clover_block<T>(cl_sm, a.cl, Vh, blockIdx.x * blockDim.x);
   __syncthreads();
   if (!live) return;
   // shared memory [buffer][hop of the round][vector][thread]
@@ -443,6 +509,8 @@ static void launch_mrhs_epi(MrhsArgs<T> a, int epi, int nrhs, cudaStream_t st) {
     cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 2, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 3, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 6, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 9, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 10, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   }
   configured = true;
   switch (epi) {
@@ -450,6 +518,8 @@ static void launch_mrhs_epi(MrhsArgs<T> a, int epi, int nrhs, cudaStream_t st) {
     case 1: dslash_mrhs_kernel<T, R, DAG, 1, NB><<<grid, block, smem, st>>>(a); break;
     case 2: dslash_mrhs_kernel<T, R, DAG, 2, NB><<<grid, block, smem, st>>>(a); break;
     case 3: dslash_mrhs_kernel<T, R, DAG, 3, NB><<<grid, block, smem, st>>>(a); break;
+    case 9: dslash_mrhs_kernel<T, R, DAG, 9, NB><<<grid, block, smem, st>>>(a); break;
+    case 10: dslash_mrhs_kernel<T, R, DAG, 10, NB><<<grid, block, smem, st>>>(a); break;
     default: dslash_mrhs_kernel<T, R, DAG, 6, NB><<<grid, block, smem, st>>>(a); break;
   }
 }
@@ -457,8 +527,10 @@ static void launch_mrhs_epi(MrhsArgs<T> a, int epi, int nrhs, cudaStream_t st) {
 template <typename T, int R, bool DAG>
 static void launch_mrhs_nb(const MrhsArgs<T>& a, int epi, int nrhs, cudaStream_t st) {
   if constexpr (MrhsStage<T, R>::HPR > 0) {
-    launch_mrhs_staged<T, R, DAG>(a, epi, nrhs, st);
-    return;
+    if (epi <= 6) {  // the epilogues with a reduction (9, 10) exist in the register kernel only
+      launch_mrhs_staged<T, R, DAG>(a, epi, nrhs, st);
+      return;
+    }
   }
   // columns per thread: the tuned NB when it divides nrhs, else one per thread
   if (nrhs % MrhsTune<T>::NB == 0) launch_mrhs_epi<T, R, DAG, MrhsTune<T>::NB>(a, epi, nrhs, st);
@@ -467,8 +539,16 @@ static void launch_mrhs_nb(const MrhsArgs<T>& a, int epi, int nrhs, cudaStream_t
 
 template <typename T>
 static void launch_mrhs_typed(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
-                              int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st) {
+                              int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st,
+                              const DslashFuse* f = nullptr) {
   MrhsArgs<T> a;
+  a.r = f ? (T*)f->r : nullptr;
+  a.out2 = f ? (T*)f->out2 : nullptr;
+  a.partial = c->d_partial_mrhs;
+  a.scalars = c->d_scalars;
+  a.num = f ? f->num : 0;
+  a.den = f ? f->den : 0;
+  a.nblocks = (c->lat.Vh + MRHS_SITES - 1) / MRHS_SITES;
   a.out = (T*)out;
   a.in = (const T*)in;
   a.gauge = (const T*)gauge;
@@ -508,6 +588,34 @@ int lqcd_dslash_mrhs_launch(lqcd_ctx* c, void* out, const void* in, const void* 
     c->prof_bytes += bytes;
   }
   LQCD_LAUNCH_CHECK(c, "dslash_mrhs");
+  return LQCD_OK;
+}
+
+// CG recurrences fused per column into the epilogue (9: t, ta = C t, |t|^2 ; 10: r -= alpha q, |r|^2, as in dslash.cu);
+// the register kernel of this file, whatever the plain epilogues run on.  Needs whole warps: Vh a multiple of 32.
+bool lqcd_mrhs_fuse_ok(const lqcd_ctx* c) { return !c->half && c->lat.Vh % MRHS_SITES == 0; }
+
+int lqcd_dslash_mrhs_fused_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
+                                  int parity, double scale, int dagger, int epi, int nrhs, const DslashFuse* f, cudaStream_t st) {
+  const int nblocks = (c->lat.Vh + MRHS_SITES - 1) / MRHS_SITES;
+  if (!c->d_partial_mrhs) {
+    if (cudaMalloc(&c->d_partial_mrhs, sizeof(double) * LQCD_MAX_RHS * nblocks) != cudaSuccess) return lqcd_check_cuda(c, "mrhs partials");
+  }
+  // epi 9: links, clover, in, x, out, out2 per column ; epi 10: links, in, x, r read and written
+  const double bytes = (double)c->lat.Vh * c->prec * (8.0 * c->recon + (epi == 9 ? 72.0 : 0.0) + nrhs * 96.0);
+  c->alg_bytes += bytes;
+  const bool rec = c->prof_on && c->prof_n < c->prof_cap;
+  if (rec) cudaEventRecord(c->prof_ev[2 * c->prof_n], st);
+  if (c->prec == 4) launch_mrhs_typed<float>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st, f);
+  else launch_mrhs_typed<double>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st, f);
+  partial_sum_mrhs_kernel<<<nrhs, 256, 0, st>>>(c->d_partial_mrhs, nblocks, c->d_scalars, f->out_slot);
+  c->launches++;
+  if (rec) {
+    cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], st);
+    c->prof_n++;
+    c->prof_bytes += bytes;
+  }
+  LQCD_LAUNCH_CHECK(c, "dslash_mrhs_fused");
   return LQCD_OK;
 }
 

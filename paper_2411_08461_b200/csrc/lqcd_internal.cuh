@@ -54,6 +54,7 @@ struct lqcd_ctx {
   char err[256];
   // reduction scratch (device): per-block partials, ticket counter, result slots; pinned host mirror
   double* d_partial;
+  double* d_partial_mrhs;  // [column][32-site warp]: partials of the multi-RHS fused epilogues (allocated on first use)
   double* d_scalars;
   unsigned int* d_ticket;
   int* d_flag;
@@ -269,6 +270,9 @@ int lqcd_dslash_fused_launch(lqcd_ctx* c, void* out, const void* in, const void*
                              int parity, double scale, int dagger, int epi, const DslashFuse* f, cudaStream_t st);
 int lqcd_dslash_mrhs_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
                             int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st);
+bool lqcd_mrhs_fuse_ok(const lqcd_ctx* c);
+int lqcd_dslash_mrhs_fused_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
+                                  int parity, double scale, int dagger, int epi, int nrhs, const DslashFuse* f, cudaStream_t st);
 bool lqcd_mrhs_tma_ok(const lqcd_ctx* c, int epi);
 int lqcd_dslash_mrhs_tma_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
                                 int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st);

@@ -325,6 +325,18 @@ static int solve_cg(lqcd_ctx* c, const Work& w, const void* gauge, const void* A
       if ((rc = lqcd_dslash_fused_launch(c, nullptr, tmp, gauge, nullptr, t, 0, k2, 0, 10, &f10, st))) return rc;
       void* u[2] = {x, t};
       if ((rc = BLAS_CALL(c, OpAxpyRatio, (op.num = cur, op.den = S_TT), u, nullptr, n, 0, st))) return rc;  // y += a t
+    } else if (!normal_residual && n > 1 && matpc == LQCD_MATPC_SYMMETRIC_RIGHT && lqcd_mrhs_fuse_ok(c)) {
+      // the same for a batch of columns: per-column |t|^2 and r -= alpha q, |r|^2 in the multi-RHS epilogues 9, 10
+      const size_t half = lqcd_clover_bytes(c) / 2;
+      const double k2 = -kappa * kappa;
+      char* ta = q;
+      DslashFuse f9 = {nullptr, S_TT, 0, 0, ta}, f10 = {r, nxt, cur, S_TT, nullptr};
+      if ((rc = lqcd_dslash_launch(c, tmp, p, gauge, off(Ai, half), nullptr, 1, 1.0, 1, 1, n, st))) return rc;
+      if ((rc = lqcd_dslash_mrhs_fused_launch(c, t, tmp, gauge, Ai, p, 0, k2, 1, 9, n, &f9, st))) return rc;
+      if ((rc = lqcd_dslash_launch(c, tmp, ta, gauge, off(Ai, half), nullptr, 1, 1.0, 0, 1, n, st))) return rc;
+      if ((rc = lqcd_dslash_mrhs_fused_launch(c, nullptr, tmp, gauge, nullptr, t, 0, k2, 0, 10, n, &f10, st))) return rc;
+      void* u[2] = {x, t};
+      if ((rc = BLAS_CALL(c, OpAxpyRatio, (op.num = cur, op.den = S_TT), u, nullptr, n, 0, st))) return rc;  // y += a t
     } else if (!normal_residual && fused && matpc == LQCD_MATPC_SYMMETRIC) {
       // symmetric form, recurrences fused into the epilogues (dslash.cu EPI 7, 8):
       //   pa = A_ee^-1 p ; tmp = A_oo^-1 D^dag_oe pa ; t = p - k^2 D^dag_eo tmp and |t|^2 in one launch ;
