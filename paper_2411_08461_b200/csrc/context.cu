@@ -82,6 +82,8 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], int prec, int recon, int t_bo
     c->tiled = (e && e[0] == '1') ? 1 : 0;
     const char* m = getenv("LQCD_MRHS_TMA");  // TMA-tiled multi-RHS kernel: on unless LQCD_MRHS_TMA=0 (A/B measurements, parity tests of both)
     c->mrhs_tma = (m && m[0] == '0') ? 0 : ((m && m[0] == '2') ? 2 : 1);
+    const char* fd = getenv("LQCD_MRHS_FUSE_DOTS");
+    c->mrhs_fuse_dots = fd ? (fd[0] == '1') : -1;  // -1: where the register kernel runs the plain epilogues anyway
     const char* gr = getenv("LQCD_GRAPHS");
     c->graphs_on = (gr && gr[0] == '0') ? 0 : 1;
     const char* z = getenv("LQCD_MRHS_ZSLAB");

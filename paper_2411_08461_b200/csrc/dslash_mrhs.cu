@@ -51,11 +51,11 @@ template <typename T> struct MrhsArgs {
   // epilogues 9 and 10 (CG recurrences fused per column, as in dslash.cu)
   T* r;             // epi 10: residual block, r -= (s[num]/s[den]) q, per column
   T* out2;          // epi 9: second output, C * out
-  double* partial;  // [column][block]: one partial sum per warp (= 32 sites of one column)
+  double* partial;  // [sum k][column][block]: one partial per warp (= 32 sites of one column), k < 3
   const double* scalars;
   int num, den, nblocks;
 };
-__host__ __device__ constexpr bool mrhs_clover(int epi) { return epi == 1 || epi == 2 || epi == 3 || epi == 9; }
+__host__ __device__ constexpr bool mrhs_clover(int epi) { return epi == 1 || epi == 2 || epi == 3 || epi == 9 || epi == 11 || epi == 12; }
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
@@ -243,6 +243,39 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kern
       local = warp_sum(local);
       if (threadIdx.x == 0) a.partial[(size_t)(g * NB + r) * a.nblocks + blockIdx.x] = local;
     }
+  } else if (EPI == 11 || EPI == 12) {
+    // BiCGStab: out = x + scale * C d (epilogue 3) with the inner products the next step needs, per column:
+    //   11: Re<out,x>, Im<out,x>, |out|^2   (t = Mhat s: <t,s>, |t|^2)      12: Re<y,out>, Im<y,out>, |y|^2, y = a.r   (<r0,v>)
+    T res[NB][24];
+    clover_mul_mrhs<T, NB>(cl_sm, acc, res);
+#pragma unroll
+    for (int r = 0; r < NB; r++) {
+      T xv[24], yv[24];
+      load_spinor<T>(a.x + first + r * stride, Vh, idx, xv);
+#pragma unroll
+      for (int e = 0; e < 24; e++) res[r][e] = xv[e] + a.scale * res[r][e];
+      store_spinor<T>(out + r * stride, Vh, idx, res[r]);
+      if (EPI == 12) load_spinor<T>(a.r + first + r * stride, Vh, idx, yv);
+      double s0 = 0, s1 = 0, s2 = 0;
+#pragma unroll
+      for (int e = 0; e < 24; e += 2) {
+        // <u,w> = sum conj(u) w with (u, w) = (out, x) for 11, (y, out) for 12
+        const double ur = EPI == 11 ? res[r][e] : yv[e], ui = EPI == 11 ? res[r][e + 1] : yv[e + 1];
+        const double wr = EPI == 11 ? xv[e] : res[r][e], wi = EPI == 11 ? xv[e + 1] : res[r][e + 1];
+        s0 += ur * wr + ui * wi;
+        s1 += ur * wi - ui * wr;
+        s2 += ur * ur + ui * ui;
+      }
+      s0 = warp_sum(s0);
+      s1 = warp_sum(s1);
+      s2 = warp_sum(s2);
+      if (threadIdx.x == 0) {
+        const size_t col = g * NB + r;
+        a.partial[(0 * LQCD_MAX_RHS + col) * a.nblocks + blockIdx.x] = s0;
+        a.partial[(1 * LQCD_MAX_RHS + col) * a.nblocks + blockIdx.x] = s1;
+        a.partial[(2 * LQCD_MAX_RHS + col) * a.nblocks + blockIdx.x] = s2;
+      }
+    }
   } else if (EPI == 10) {  // q = x + scale * d not stored ; r -= (s[num]/s[den]) q ; |r|^2 per column
 #pragma unroll
     for (int r = 0; r < NB; r++) {
@@ -281,7 +314,8 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kern
 // sums the per-warp partials of one column in a fixed order -> scalars[column][slot] (deterministic)
 __global__ void __launch_bounds__(256) partial_sum_mrhs_kernel(const double* __restrict__ partial, int nblocks, double* scalars, int slot) {
   __shared__ double sm[8];
-  const double* p = partial + (size_t)blockIdx.x * nblocks;
+  const double* p = partial + ((size_t)blockIdx.y * LQCD_MAX_RHS + blockIdx.x) * nblocks;  // blockIdx.y: which of up to 3 sums
+  slot += blockIdx.y;
   double v = 0;
   for (int b = threadIdx.x; b < nblocks; b += 256) v += p[b];
   v = warp_sum(v);
@@ -511,6 +545,8 @@ static void launch_mrhs_epi(MrhsArgs<T> a, int epi, int nrhs, cudaStream_t st) {
     cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 6, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 9, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 10, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 11, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 12, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   }
   configured = true;
   switch (epi) {
@@ -520,6 +556,8 @@ static void launch_mrhs_epi(MrhsArgs<T> a, int epi, int nrhs, cudaStream_t st) {
     case 3: dslash_mrhs_kernel<T, R, DAG, 3, NB><<<grid, block, smem, st>>>(a); break;
     case 9: dslash_mrhs_kernel<T, R, DAG, 9, NB><<<grid, block, smem, st>>>(a); break;
     case 10: dslash_mrhs_kernel<T, R, DAG, 10, NB><<<grid, block, smem, st>>>(a); break;
+    case 11: dslash_mrhs_kernel<T, R, DAG, 11, NB><<<grid, block, smem, st>>>(a); break;
+    case 12: dslash_mrhs_kernel<T, R, DAG, 12, NB><<<grid, block, smem, st>>>(a); break;
     default: dslash_mrhs_kernel<T, R, DAG, 6, NB><<<grid, block, smem, st>>>(a); break;
   }
 }
@@ -591,7 +629,8 @@ int lqcd_dslash_mrhs_launch(lqcd_ctx* c, void* out, const void* in, const void* 
   return LQCD_OK;
 }
 
-// CG recurrences fused per column into the epilogue (9: t, ta = C t, |t|^2 ; 10: r -= alpha q, |r|^2, as in dslash.cu);
+// Krylov recurrences fused per column into the epilogue (9: t, ta = C t, |t|^2 ; 10: r -= alpha q, |r|^2, as in dslash.cu;
+// 11, 12: epilogue 3 with BiCGStab's inner products);
 // the register kernel of this file, whatever the plain epilogues run on.  Needs whole warps: Vh a multiple of 32.
 bool lqcd_mrhs_fuse_ok(const lqcd_ctx* c) { return !c->half && c->lat.Vh % MRHS_SITES == 0; }
 
@@ -599,16 +638,18 @@ int lqcd_dslash_mrhs_fused_launch(lqcd_ctx* c, void* out, const void* in, const 
                                   int parity, double scale, int dagger, int epi, int nrhs, const DslashFuse* f, cudaStream_t st) {
   const int nblocks = (c->lat.Vh + MRHS_SITES - 1) / MRHS_SITES;
   if (!c->d_partial_mrhs) {
-    if (cudaMalloc(&c->d_partial_mrhs, sizeof(double) * LQCD_MAX_RHS * nblocks) != cudaSuccess) return lqcd_check_cuda(c, "mrhs partials");
+    if (cudaMalloc(&c->d_partial_mrhs, sizeof(double) * 3 * LQCD_MAX_RHS * nblocks) != cudaSuccess) return lqcd_check_cuda(c, "mrhs partials");
   }
   // epi 9: links, clover, in, x, out, out2 per column ; epi 10: links, in, x, r read and written
-  const double bytes = (double)c->lat.Vh * c->prec * (8.0 * c->recon + (epi == 9 ? 72.0 : 0.0) + nrhs * 96.0);
+  // epi 11: as epi 3 (links, clover, in, x, out) ; epi 12: + y
+  const double bytes = (double)c->lat.Vh * c->prec *
+                       (8.0 * c->recon + (epi == 10 ? 0.0 : 72.0) + nrhs * (epi == 11 ? 72.0 : 96.0));
   c->alg_bytes += bytes;
   const bool rec = c->prof_on && c->prof_n < c->prof_cap;
   if (rec) cudaEventRecord(c->prof_ev[2 * c->prof_n], st);
   if (c->prec == 4) launch_mrhs_typed<float>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st, f);
   else launch_mrhs_typed<double>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st, f);
-  partial_sum_mrhs_kernel<<<nrhs, 256, 0, st>>>(c->d_partial_mrhs, nblocks, c->d_scalars, f->out_slot);
+  partial_sum_mrhs_kernel<<<dim3(nrhs, epi >= 11 ? 3 : 1), 256, 0, st>>>(c->d_partial_mrhs, nblocks, c->d_scalars, f->out_slot);
   c->launches++;
   if (rec) {
     cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], st);

@@ -48,6 +48,7 @@ struct lqcd_ctx {
   int part_mask;  // bit mu: direction mu is cut between ranks (lqcd_set_partition; dd.cu)
   double ws;  // weight of the spatial hops: nu/xi_0 of Eq. 5; 1 = isotropic
   int mrhs_tma;    // 1 (default): TMA-tiled multi-RHS kernel (dslash_mrhs_tma.cu) where it applies; LQCD_MRHS_TMA=0 turns it off
+  int mrhs_fuse_dots;  // batched BiCGStab: inner products in the multi-RHS epilogues (LQCD_MRHS_FUSE_DOTS: 1 on, 0 off; unset = -1: where measured faster)
   int mrhs_zslab;  // z-tiles per slab of its sweep (LQCD_MRHS_ZSLAB; 0 = the whole z extent)
   int tiled;  // 1: shared-memory tiled dslash where the tile divides the lattice (opt-in: LQCD_DSLASH_TILED=1)
   long launches;
