@@ -54,8 +54,23 @@ template <typename T> struct MrhsArgs {
   double* partial;  // [sum k][column][block]: one partial per warp (= 32 sites of one column), k < 3
   const double* scalars;
   int num, den, nblocks;
+  int zslab;  // z-planes per slab of the sweep (0: plain order)
 };
 __host__ __device__ constexpr bool mrhs_clover(int epi) { return epi == 1 || epi == 2 || epi == 3 || epi == 9 || epi == 11 || epi == 12; }
+// Block order of the sweep: 32-site blocks run x, y, then z inside a slab of `zslab` planes, then t, then the slab, so
+// that the +-t reuse window of all columns (2 x slab x nrhs columns) stays in L2 (round 1: 1.5 x the algorithmic DRAM
+// bytes with 12 columns in plain checkerboard order).  zslab = 0, or a plane that is not a whole number of blocks: identity.
+__device__ __forceinline__ int sweep_block(const Lat& L, int b, int zslab) {
+  const int plane = L.Lxh * L.Ly;
+  if (zslab <= 0 || zslab >= L.Lz || plane % MRHS_SITES || L.Lz % zslab) return b;
+  const int pb = plane / MRHS_SITES;
+  const int xy = b % pb;
+  int q = b / pb;
+  const int zl = q % zslab;
+  q /= zslab;
+  const int t = q % L.Lt, slab = q / L.Lt;
+  return xy + pb * ((slab * zslab + zl) + L.Lz * t);
+}
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
@@ -132,7 +147,8 @@ template <typename T, int R, bool DAG, int EPI, int NB>
 __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kernel(const MrhsArgs<T> a) {
   typedef typename GV<T, R>::vec gvec;
   constexpr int NGV = R / GV<T, R>::N;
-  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int blk0 = sweep_block(a.lat, blockIdx.x, a.zslab);  // block of 32 consecutive sites this thread block computes
+  const int idx = blk0 * blockDim.x + threadIdx.x;
   __shared__ typename V16<T>::vec cl_sm[mrhs_clover(EPI) ? Lay<T>::NCV * MRHS_SITES : 1];
   extern __shared__ __align__(16) unsigned char mrhs_lk_smem[];  // the eight links of the block's sites: [hop][vector][site]
   gvec* lk_sm = reinterpret_cast<gvec*>(mrhs_lk_smem);
@@ -162,7 +178,7 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kern
       for (int v = 0; v < NGV; v++) lk_sm[(h * NGV + v) * MRHS_SITES + threadIdx.x] = ld_stream(gp + (size_t)v * Vh);
     }
   }
-  if (mrhs_clover(EPI)) stage_clover_block<T>(cl_sm, a.cl, Vh, blockIdx.x * blockDim.x);
+  if (mrhs_clover(EPI)) stage_clover_block<T>(cl_sm, a.cl, Vh, blk0 * blockDim.x);
   __syncthreads();
   if (!live) return;
   for (int g = threadIdx.y; g < a.ngroups; g += blockDim.y) {
@@ -390,7 +406,8 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsStage<T, R>::MINB) dslash_mrhs_
   typedef typename V16<T>::vec vec;
   constexpr int HPR = MrhsStage<T, R>::HPR > 0 ? MrhsStage<T, R>::HPR : 1, NR = 8 / HPR, NSV = Lay<T>::NSV;
   extern __shared__ __align__(16) unsigned char mrhs_smem[];
-  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int blk0 = sweep_block(a.lat, blockIdx.x, a.zslab);
+  const int idx = blk0 * blockDim.x + threadIdx.x;
   typedef typename GV<T, R>::vec gvec;
   constexpr int NGV = R / GV<T, R>::N;
   __shared__ vec cl_sm[mrhs_clover(EPI) ? Lay<T>::NCV * MRHS_SITES : 1];
@@ -422,7 +439,7 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsStage<T, R>::MINB) dslash_mrhs_
       for (int v = 0; v < NGV; v++) lk_sm[(h * NGV + v) * MRHS_SITES + threadIdx.x] = ld_stream(gp + (size_t)v * Vh);
     }
   }
-  if (mrhs_clover(EPI)) stage_clover_block<T>(cl_sm, a.cl, Vh, blockIdx.x * blockDim.x);
+  if (mrhs_clover(EPI)) stage_clover_block<T>(cl_sm, a.cl, Vh, blk0 * blockDim.x);
   __syncthreads();
   if (!live) return;
   // shared memory [buffer][hop of the round][vector][thread]
@@ -587,6 +604,7 @@ static void launch_mrhs_typed(lqcd_ctx* c, void* out, const void* in, const void
   a.num = f ? f->num : 0;
   a.den = f ? f->den : 0;
   a.nblocks = (c->lat.Vh + MRHS_SITES - 1) / MRHS_SITES;
+  a.zslab = 2 * c->mrhs_zslab;  // LQCD_MRHS_ZSLAB counts pairs of z-planes (the tiles of the TMA kernel)
   a.out = (T*)out;
   a.in = (const T*)in;
   a.gauge = (const T*)gauge;
