@@ -87,7 +87,7 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], int prec, int recon, int t_bo
     const char* gr = getenv("LQCD_GRAPHS");
     c->graphs_on = (gr && gr[0] == '0') ? 0 : 1;
     const char* z = getenv("LQCD_MRHS_ZSLAB");
-    c->mrhs_zslab = z ? atoi(z) : 2;  // pairs of z-planes per slab (sweep at 32^3x64: 2 best for the register kernels, 2-8 alike for the TMA one)
+    c->mrhs_zslab = z ? atoi(z) : -1;  // pairs of z-planes per slab; -1: each kernel's own default (4 TMA-tiled, 2 register kernels)
   }
   c->recon = recon;
   c->device = device;

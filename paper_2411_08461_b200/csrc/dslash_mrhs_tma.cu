@@ -389,7 +389,8 @@ int launch_any(lqcd_ctx* c, TmaArgs& a, const void* in, int dagger, int epi, int
   TmaMaps map;
   if (!make_maps<TS>(&map, in, c->lat, nrhs)) return lqcd_set_error(c, LQCD_ERR_CUDA, "dslash_mrhs_tma: cuTensorMapEncodeTiled failed");
   const int ntz = c->lat.Lz / TS::TZ;
-  a.zslab = (c->mrhs_zslab > 0 && ntz % c->mrhs_zslab == 0) ? c->mrhs_zslab : ntz;
+  const int want = c->mrhs_zslab < 0 ? 8 / TS::TZ : c->mrhs_zslab * 2 / TS::TZ;  // LQCD_MRHS_ZSLAB: pairs of z-planes; default 4
+  a.zslab = (want > 0 && ntz % want == 0) ? want : ntz;
   switch (epi) {
     case 0: launch_tile<TS, 0>(map, a, c->recon, dagger, c->device, st); break;
     case 1: launch_tile<TS, 1>(map, a, c->recon, dagger, c->device, st); break;
@@ -405,7 +406,8 @@ int launch_noclover(lqcd_ctx* c, TmaArgs& a, const void* in, int dagger, int epi
   TmaMaps map;
   if (!make_maps<TS>(&map, in, c->lat, nrhs)) return lqcd_set_error(c, LQCD_ERR_CUDA, "dslash_mrhs_tma: cuTensorMapEncodeTiled failed");
   const int ntz = c->lat.Lz / TS::TZ;
-  a.zslab = (c->mrhs_zslab > 0 && ntz % c->mrhs_zslab == 0) ? c->mrhs_zslab : ntz;
+  const int want = c->mrhs_zslab < 0 ? 8 / TS::TZ : c->mrhs_zslab * 2 / TS::TZ;  // LQCD_MRHS_ZSLAB: pairs of z-planes; default 4
+  a.zslab = (want > 0 && ntz % want == 0) ? want : ntz;
   if (epi == 0) launch_tile<TS, 0>(map, a, c->recon, dagger, c->device, st);
   else launch_tile<TS, 6>(map, a, c->recon, dagger, c->device, st);
   return LQCD_OK;
@@ -415,7 +417,8 @@ int launch_clover(lqcd_ctx* c, TmaArgs& a, const void* in, int dagger, int epi, 
   TmaMaps map;
   if (!make_maps<TS>(&map, in, c->lat, nrhs)) return lqcd_set_error(c, LQCD_ERR_CUDA, "dslash_mrhs_tma: cuTensorMapEncodeTiled failed");
   const int ntz = c->lat.Lz / TS::TZ;
-  a.zslab = (c->mrhs_zslab > 0 && ntz % c->mrhs_zslab == 0) ? c->mrhs_zslab : ntz;
+  const int want = c->mrhs_zslab < 0 ? 8 / TS::TZ : c->mrhs_zslab * 2 / TS::TZ;  // LQCD_MRHS_ZSLAB: pairs of z-planes; default 4
+  a.zslab = (want > 0 && ntz % want == 0) ? want : ntz;
   if (epi == 1) launch_tile<TS, 1>(map, a, c->recon, dagger, c->device, st);
   else if (epi == 2) launch_tile<TS, 2>(map, a, c->recon, dagger, c->device, st);
   else launch_tile<TS, 3>(map, a, c->recon, dagger, c->device, st);
