@@ -408,8 +408,15 @@ bool lqcd_dslash_fuse_ok(const lqcd_ctx* c) {
   return !c->half && (long)lqcd_dslash_grid(c) <= 4L * c->max_red_blocks * LQCD_MAX_RHS;
 }
 
+int lqcd_partial_sum_launch(lqcd_ctx* c, int n, int slot, cudaStream_t st) {
+  partial_sum_kernel<<<1, PSUM_BLOCK, 0, st>>>(c->d_partial, n, c->d_scalars + slot);
+  LQCD_LAUNCH_CHECK(c, "partial_sum");
+  return LQCD_OK;
+}
+
 int lqcd_dslash_fused_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
                              int parity, double scale, int dagger, int epi, const DslashFuse* f, cudaStream_t st) {
+  if (c->half) return lqcd_dslash_half_launch(c, out, in, gauge, cl, x, parity, scale, dagger, epi, st, f);
   // epi 4: as epi 2; epi 7: as epi 6 (no clover); epi 9: as epi 3 + a second output.  epi 5, 8, 10: no output
   // store, r read and written instead
   const double bytes = (double)c->lat.Vh * c->prec *

@@ -14,26 +14,45 @@ struct HalfArgs {
   Lat lat;
   int parity;
   float scale, ws;
+  // epilogues 9 and 10 (CG recurrences of the right-preconditioned form, as in dslash.cu)
+  void* r;
+  void* out2;
+  double* partial;
+  const double* scalars;
+  int num, den;
 };
 
 template <int R, int MU, bool FWD, bool DAG>
 __device__ __forceinline__ void hop_h(float* acc, const void* in, const short* links, int Vh, int nidx, int lidx, float w) {
   constexpr int S = (FWD != DAG) ? -1 : +1;
   float psi[24], U[18], h[12], chi[12];
-  load_spinor_h(in, Vh, nidx, psi);
+  const float s = load_spinor_h_raw(in, Vh, nidx, psi);  // integers; the site's scale goes into the hop weight
   load_link_h<R>(links, Vh, lidx, U);
   project<float, MU, S>(psi, h);
   su3_mul<float, !FWD>(U, h, chi);
-  reconstruct<float, MU, S>(acc, chi, w);
+  reconstruct<float, MU, S>(acc, chi, w * s);
 }
 
 // EPI as in dslash.cu: 0 scale*d ; 1 scale*C d ; 2 C x + scale*d ; 3 x + scale*C d ; 6 x + scale*d
+// block sum -> partial[block] (summed in a fixed order by lqcd_partial_sum_launch: deterministic)
+__device__ __forceinline__ void half_block_sum(double v, double* partial) {
+  __shared__ double sm[4];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+  __syncthreads();
+  if (threadIdx.x == 0) partial[blockIdx.x] = (sm[0] + sm[1]) + (sm[2] + sm[3]);
+}
+
 template <int R, bool DAG, int EPI>
 __global__ void __launch_bounds__(128, 4) dslash_half_kernel(const HalfArgs a) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   const Lat& L = a.lat;
   const int Vh = L.Vh, par = a.parity;
-  if (idx >= Vh) return;
+  if (idx >= Vh) {
+    if (EPI == 9 || EPI == 10) half_block_sum(0.0, a.partial);  // the reduction needs every thread of the block
+    return;
+  }
   const Site s = site_of(L, idx, par);
   const size_t blk = (size_t)R * Vh;  // shorts per (mu, parity) link block
   float acc[24];
@@ -77,12 +96,42 @@ __global__ void __launch_bounds__(128, 4) dslash_half_kernel(const HalfArgs a) {
     clover_mul_h(a.cl, Vh, idx, acc, res);
 #pragma unroll
     for (int e = 0; e < 24; e++) res[e] = xv[e] + a.scale * res[e];
-  } else {
+  } else if (EPI == 9) {  // t = x + scale * C d ; ta = C t ; |t|^2 (of the value kept, i.e. before it is rounded to 16 bits)
+    float xv[24], res2[24];
+    load_spinor_h(a.x, Vh, idx, xv);
+    clover_mul_h(a.cl, Vh, idx, acc, res);
+#pragma unroll
+    for (int e = 0; e < 24; e++) res[e] = xv[e] + a.scale * res[e];
+    clover_mul_h(a.cl, Vh, idx, res, res2);
+    store_spinor_h(a.out2, Vh, idx, res2);
+  } else {  // 6, 10: x + scale * d
     load_spinor_h(a.x, Vh, idx, res);
 #pragma unroll
     for (int e = 0; e < 24; e++) res[e] += a.scale * acc[e];
   }
+  if (EPI == 10) {  // q = res is not stored: r -= (s[num]/s[den]) q, |r|^2
+    double local = 0;
+    if (a.scalars[S_DONE] == 0.0) {
+      const float alpha = (float)(a.scalars[a.num] / a.scalars[a.den]);
+      float rv[24];
+      load_spinor_h_plain(a.r, Vh, idx, rv);
+#pragma unroll
+      for (int e = 0; e < 24; e++) {
+        rv[e] -= alpha * res[e];
+        local += (double)rv[e] * rv[e];
+      }
+      store_spinor_h(a.r, Vh, idx, rv);
+    }
+    half_block_sum(local, a.partial);
+    return;
+  }
   store_spinor_h(a.out, Vh, idx, res);
+  if (EPI == 9) {
+    double local = 0;
+#pragma unroll
+    for (int e = 0; e < 24; e++) local += (double)res[e] * res[e];
+    half_block_sum(local, a.partial);
+  }
 }
 
 // in and out may alias: plain loads, a thread reads its whole site before it stores
@@ -103,6 +152,8 @@ void launch_epi_h(const HalfArgs& a, int epi, cudaStream_t st) {
     case 1: dslash_half_kernel<R, DAG, 1><<<grid, 128, 0, st>>>(a); break;
     case 2: dslash_half_kernel<R, DAG, 2><<<grid, 128, 0, st>>>(a); break;
     case 3: dslash_half_kernel<R, DAG, 3><<<grid, 128, 0, st>>>(a); break;
+    case 9: dslash_half_kernel<R, DAG, 9><<<grid, 128, 0, st>>>(a); break;
+    case 10: dslash_half_kernel<R, DAG, 10><<<grid, 128, 0, st>>>(a); break;
     default: dslash_half_kernel<R, DAG, 6><<<grid, 128, 0, st>>>(a); break;
   }
 }
@@ -116,9 +167,16 @@ double lqcd_half_dslash_bytes(const lqcd_ctx* c, int epi) {
 }
 
 int lqcd_dslash_half_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
-                            int parity, double scale, int dagger, int epi, cudaStream_t st) {
-  if (!(epi <= 3 || epi == 6)) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "16-bit context: epilogue %d not built", epi);
+                            int parity, double scale, int dagger, int epi, cudaStream_t st, const DslashFuse* f) {
+  if (!(epi <= 3 || epi == 6 || ((epi == 9 || epi == 10) && f)))
+    return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "16-bit context: epilogue %d not built", epi);
   HalfArgs a;
+  a.r = f ? f->r : nullptr;
+  a.out2 = f ? f->out2 : nullptr;
+  a.partial = c->d_partial;
+  a.scalars = c->d_scalars;
+  a.num = f ? f->num : 0;
+  a.den = f ? f->den : 0;
   a.out = out;
   a.in = in;
   a.gauge = (const short*)gauge;
@@ -128,7 +186,7 @@ int lqcd_dslash_half_launch(lqcd_ctx* c, void* out, const void* in, const void* 
   a.parity = parity;
   a.scale = (float)scale;
   a.ws = (float)c->ws;
-  const double bytes = lqcd_half_dslash_bytes(c, epi);
+  const double bytes = lqcd_half_dslash_bytes(c, epi == 9 ? 3 : (epi == 10 ? 6 : epi)) + (epi >= 9 ? 52.0 * c->lat.Vh : 0.0);
   c->alg_bytes += bytes;
   const bool rec = c->prof_on && c->prof_n < c->prof_cap;
   if (rec) cudaEventRecord(c->prof_ev[2 * c->prof_n], st);
@@ -145,6 +203,7 @@ int lqcd_dslash_half_launch(lqcd_ctx* c, void* out, const void* in, const void* 
     c->prof_bytes += bytes;
   }
   LQCD_LAUNCH_CHECK(c, "dslash_half");
+  if (epi >= 9) return lqcd_partial_sum_launch(c, (c->lat.Vh + 127) / 128, f->out_slot, st);
   return LQCD_OK;
 }
 

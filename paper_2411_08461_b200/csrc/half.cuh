@@ -24,11 +24,16 @@ constexpr float HALF_MAX = 32767.f;
 //           integer (ties to even, a single rounding) and leaves u in the low 16 bits of the result.
 // A zeroed buffer (u = 0, norm = 0) still reads as zero.
 constexpr float HALF_DEC = 8421376.f, HALF_ENC = 12615680.f;
+// two stored fields -> the two integers q as floats (exact): 2 PRMT + one packed add (fma.rn.f32x2 with multiplicand 1)
+__device__ __forceinline__ void dec2_raw(unsigned w, float& lo, float& hi) {
+  const u64 v = pk2(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610)),   // bytes: w0 w1 00 4B
+                    __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7632)));  // bytes: w2 w3 00 4B
+  upk2(fma2(v, pk2(1.f, 1.f), pk2(-HALF_DEC, -HALF_DEC)), lo, hi);
+}
+// ... and scaled: one packed multiply more
 __device__ __forceinline__ void dec2(unsigned w, float s, float& lo, float& hi) {
-  const float a = __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610));  // bytes: w0 w1 00 4B
-  const float b = __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7632));  // bytes: w2 w3 00 4B
-  lo = (a - HALF_DEC) * s;
-  hi = (b - HALF_DEC) * s;
+  const u64 v = pk2(__uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610)), __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7632)));
+  upk2(mul2(fma2(v, pk2(1.f, 1.f), pk2(-HALF_DEC, -HALF_DEC)), pk2(s, s)), lo, hi);
 }
 __device__ __forceinline__ unsigned enc2(float lo, float hi, float inv) {
   const unsigned a = __float_as_uint(fmaf(lo, inv, HALF_ENC)), b = __float_as_uint(fmaf(hi, inv, HALF_ENC));
@@ -52,6 +57,18 @@ __device__ __forceinline__ void load_spinor_h_impl(const void* base, int Vh, int
   }
 }
 __device__ __forceinline__ void load_spinor_h(const void* base, int Vh, int idx, float* psi) { load_spinor_h_impl<true>(base, Vh, idx, psi); }
+// the 24 stored integers as floats and the site's scale norm / 32767 apart: projection, SU(3) multiply and
+// reconstruction are linear, so a hop multiplies by the scale once, in its weight, instead of 24 times here
+__device__ __forceinline__ float load_spinor_h_raw(const void* base, int Vh, int idx, float* q24) {
+  const uint2* p = reinterpret_cast<const uint2*>(base) + idx;
+#pragma unroll
+  for (int v = 0; v < 6; v++) {
+    const uint2 q = __ldg(p + (size_t)v * Vh);
+    dec2_raw(q.x, q24[4 * v], q24[4 * v + 1]);
+    dec2_raw(q.y, q24[4 * v + 2], q24[4 * v + 3]);
+  }
+  return __ldg(half_spinor_norms(base, Vh) + idx) * (1.f / HALF_MAX);
+}
 // plain (coherent) loads: for kernels whose input may alias their output
 __device__ __forceinline__ void load_spinor_h_plain(const void* base, int Vh, int idx, float* psi) { load_spinor_h_impl<false>(base, Vh, idx, psi); }
 __device__ __forceinline__ void store_spinor_h(void* base, int Vh, int idx, const float* psi) {

@@ -278,8 +278,10 @@ bool lqcd_mrhs_tma_ok(const lqcd_ctx* c, int epi);
 int lqcd_dslash_mrhs_tma_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
                                 int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st);
 // 16-bit-storage context (half.cu)
+struct DslashFuse;
 int lqcd_dslash_half_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
-                            int parity, double scale, int dagger, int epi, cudaStream_t st);
+                            int parity, double scale, int dagger, int epi, cudaStream_t st, const DslashFuse* f = nullptr);
+int lqcd_partial_sum_launch(lqcd_ctx* c, int n, int slot, cudaStream_t st);  // d_partial[0..n) -> d_scalars[slot], fixed order
 int lqcd_clover_apply_half_launch(lqcd_ctx* c, void* out, const void* in, const void* cl_parity, cudaStream_t st);
 int lqcd_gauge_pack_half(lqcd_ctx* c, void* native, const void* pub, cudaStream_t st);
 int lqcd_spinor_pack_half(lqcd_ctx* c, void* native, const void* pub, int parities, cudaStream_t st);

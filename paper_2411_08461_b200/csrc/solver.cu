@@ -305,13 +305,14 @@ static int solve_cg(lqcd_ctx* c, const Work& w, const void* gauge, const void* A
     if (!(cols.rr[j] > cols.stop2[j])) freeze(c, cols, j, st);
   }
   const bool fused = n == 1 && lqcd_dslash_fuse_ok(c);
+  const bool fused_half = n == 1 && c->half && matpc == LQCD_MATPC_SYMMETRIC_RIGHT;  // 16-bit context: epilogues 9, 10 only
   const int stride = check_stride(c, n);
   arm_check(c, cols, st);
   // one iteration, enqueued on `st` (plain launches, or recorded into a graph by run_block)
   auto iterate = [&](int it) -> int {
     const int cur = (it & 1) ? S_RR1 : S_RR0, nxt = (it & 1) ? S_RR0 : S_RR1;
     int outs[4] = {S_TT, 0, 0, 0};
-    if (!normal_residual && fused && matpc == LQCD_MATPC_SYMMETRIC_RIGHT) {
+    if (!normal_residual && (fused || fused_half) && matpc == LQCD_MATPC_SYMMETRIC_RIGHT) {
       // right-preconditioned symmetric form, recurrences fused into the epilogues (dslash.cu EPI 9, 10):
       //   tmp = A_oo^-1 D^dag_oe p ; t = p - k^2 A_ee^-1 D^dag_eo tmp, ta = A_ee^-1 t and |t|^2 in one launch ;
       //   tmp = A_oo^-1 D_oe ta ; q = t - k^2 D_eo tmp is never stored: r -= alpha q, |r|^2 in its launch
