@@ -44,8 +44,11 @@ __device__ __forceinline__ void half_block_sum(double v, double* partial) {
   if (threadIdx.x == 0) partial[blockIdx.x] = (sm[0] + sm[1]) + (sm[2] + sm[3]);
 }
 
+#ifndef HALF_MINB
+#define HALF_MINB 4
+#endif
 template <int R, bool DAG, int EPI>
-__global__ void __launch_bounds__(128, 4) dslash_half_kernel(const HalfArgs a) {
+__global__ void __launch_bounds__(128, HALF_MINB) dslash_half_kernel(const HalfArgs a) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   const Lat& L = a.lat;
   const int Vh = L.Vh, par = a.parity;
