@@ -63,9 +63,14 @@ typedef struct lqcd_result {
  * recon = 18 (full links) or 12 (two rows stored, third recomputed); t_boundary = +1 or -1
  * (antiperiodic in t, applied in-kernel to raw periodic links); device = CUDA
  * ordinal (must be compute capability 10.x).
- * Measurement switches read from the environment at creation (results are identical, only the kernel differs):
- * LQCD_DSLASH_TILED=1 runs the shared-memory tiled single-RHS dslash, LQCD_MRHS_TILED=1 the tiled multi-RHS
- * kernel (fp32), wherever their tile divides the lattice; both are slower than the defaults. */
+ * Measurement switches read from the environment at creation (results agree to rounding order, only the kernel
+ * differs; every default is the measured-best choice):
+ *   LQCD_DSLASH_TILED=1      shared-memory tiled single-RHS dslash where its tile divides the lattice (slower);
+ *   LQCD_MRHS_TMA=0|1|2      TMA-tiled multi-RHS kernel (fp32): off | where measured faster (default) | wherever it runs;
+ *   LQCD_MRHS_ZSLAB=n        z-planes per slab of the multi-RHS block sweep (default per kernel);
+ *   LQCD_MRHS_FUSE_DOTS=0|1  batched BiCGStab dot products in the multi-RHS epilogues: never | always (default: where
+ *                            the register kernel runs the epilogue anyway);
+ *   LQCD_GRAPHS=0            no CUDA-graph replay of Krylov iteration blocks on small lattices. */
 int lqcd_create(lqcd_ctx** ctx, const int dims[4], int prec, int recon, int t_boundary, int device);
 int lqcd_destroy(lqcd_ctx* ctx);
 const char* lqcd_strerror(int code);
