@@ -212,44 +212,33 @@ constexpr int CB_SITES = 32;
 #ifndef CB_MINB
 #define CB_MINB 2  // 170 registers, 12 warps/SM: 5.84 -> 4.59 ms at 32^3x64 fp64 (3 blocks/SM spill: 9.1 ms)
 #endif
-template <typename T, int R>
-__global__ void __launch_bounds__(CB_SITES * 6, CB_MINB) clover_build_kernel(T* __restrict__ clover, T* __restrict__ clover_inv,
-                                                                    const T* __restrict__ gauge, Lat L, double kc,
-                                                                    double kt, int* flag) {
-  __shared__ cd Fs[6][9][CB_SITES];  // planes xy, xz, xt, yz, yt, zt
-  const int ls = threadIdx.x, pl = threadIdx.y;
-  // Traversal order.  Every link is needed by the 14 sites of its two-hop neighbourhood, of both parities; in plain
-  // checkerboard order (all even sites, then all odd; t slowest) the reuse window is three whole time slices of all
-  // links, twice over.  Here a block pair = the even and the odd sites of the same 32 checkerboard indices, and the
-  // index runs (x, y, z within a slab of CB_ZC planes, t, slab): the window is three time slices of ONE z-slab
-  // (7 MB at 32^3x64).  Measured (ncu, 32^3x64 fp64): DRAM reads 10.8 -> 7.1 GB, L2 hit rate 42 -> 55 %, time
-  // unchanged (4.5 ms; any CB_ZC from 2 to 16): the kernel waits on its 12 warps per SM, not on DRAM.
-  const int par = blockIdx.x & 1;
-  const int k = (blockIdx.x >> 1) * CB_SITES + ls;
-  const bool live = k < L.Vh;
-  int idx = 0;
-  if (live) {
-    const int zc = (L.Lz % CB_ZC == 0) ? CB_ZC : 2;  // every extent is even
-    const int plane = L.Lxh * L.Ly;
-    const int xy = k % plane;
-    int q = k / plane;
-    const int zl = q % zc;
-    q /= zc;
-    const int t = q % L.Lt, slab = q / L.Lt;
-    idx = xy + plane * ((slab * zc + zl) + L.Lz * t);
-  }
-  if (live) {
-    const Site s = site_of(L, idx, par);
-    const int x0[4] = {2 * s.xh + s.r, s.y, s.z, s.t};
-    const int mu = pl < 3 ? 0 : (pl < 5 ? 1 : 2);
-    const int nu = pl < 3 ? pl + 1 : (pl < 5 ? pl - 1 : 3);
-    cd F[9];
-    field_strength<T, R>(gauge, L, x0, mu, nu, F);
-#pragma unroll
-    for (int e = 0; e < 9; e++) Fs[pl][e][ls] = F[e];
-  }
-  __syncthreads();
-  if (!live || pl >= 2) return;
+// F of one plane for NS sites in shared memory.  F is Hermitian exactly (both triangles come from the same
+// difference): 3 real diagonals, then (re, im) of F_01, F_02, F_12.
+template <int NS>
+__device__ __forceinline__ cd herm_entry(const double (&F)[9][NS], int i, int j, int ls) {
+  if (i == j) return {F[i][ls], 0.0};
+  const int lo = i < j ? i : j, hi = i < j ? j : i;
+  const int e = 3 + 2 * (lo + hi - 1);  // (0,1) -> 3, (0,2) -> 5, (1,2) -> 7
+  return {F[e][ls], i < j ? F[e + 1][ls] : -F[e + 1][ls]};
+}
+template <int NS>
+__device__ __forceinline__ void herm_store(double (&F)[9][NS], int ls, const cd* f9) {
+  F[0][ls] = f9[0].re;
+  F[1][ls] = f9[4].re;
+  F[2][ls] = f9[8].re;
+  F[3][ls] = f9[1].re;
+  F[4][ls] = f9[1].im;
+  F[5][ls] = f9[2].re;
+  F[6][ls] = f9[2].im;
+  F[7][ls] = f9[5].re;
+  F[8][ls] = f9[5].im;
+}
+// Phase 2 of either build: thread k < 2 of a site assembles chiral block k from the six F in shared memory, packs it,
+// inverts it by Gauss-Jordan and stores both.
+template <typename T, int NS>
+__device__ __forceinline__ void clover_blocks(const double (&Fs)[6][9][NS], int ls, int pl, T* __restrict__ clover,
+                                              T* __restrict__ clover_inv, const Lat& L, int idx, int par, double kc, double kt,
+                                              int* flag) {
   const size_t half = (size_t)72 * L.Vh;  // reals per parity of a clover field
   {
     const int k = pl;
@@ -257,11 +246,10 @@ __global__ void __launch_bounds__(CB_SITES * 6, CB_MINB) clover_build_kernel(T* 
     cd B[6][6];
     for (int i = 0; i < 3; i++)
       for (int j = 0; j < 3; j++) {
-        const int e = 3 * i + j;
         // kc = kappa*csw on the spatial planes, kt = kappa*csw_t on the temporal ones (Eq. 5)
         const double st = sg * kt;
-        const cd Fxy = Fs[0][e][ls], Fxz = Fs[1][e][ls], Fxt = Fs[2][e][ls], Fyz = Fs[3][e][ls], Fyt = Fs[4][e][ls],
-                 Fzt = Fs[5][e][ls];
+        const cd Fxy = herm_entry(Fs[0], i, j, ls), Fxz = herm_entry(Fs[1], i, j, ls), Fxt = herm_entry(Fs[2], i, j, ls),
+                 Fyz = herm_entry(Fs[3], i, j, ls), Fyt = herm_entry(Fs[4], i, j, ls), Fzt = herm_entry(Fs[5], i, j, ls);
         cd E3 = {kc * Fxy.re - st * Fzt.re, kc * Fxy.im - st * Fzt.im};  // kc F_xy -/+ kt F_zt
         cd E2 = {kc * Fxz.re + st * Fyt.re, kc * Fxz.im + st * Fyt.im};  // kc F_xz +/- kt F_yt
         cd E1 = {kc * Fyz.re - st * Fxt.re, kc * Fyz.im - st * Fxt.im};  // kc F_yz -/+ kt F_xt
@@ -300,6 +288,262 @@ __global__ void __launch_bounds__(CB_SITES * 6, CB_MINB) clover_build_kernel(T* 
   }
 }
 
+template <typename T, int R>
+__global__ void __launch_bounds__(CB_SITES * 6, CB_MINB) clover_build_kernel(T* __restrict__ clover, T* __restrict__ clover_inv,
+                                                                    const T* __restrict__ gauge, Lat L, double kc,
+                                                                    double kt, int* flag) {
+  __shared__ double Fs[6][9][CB_SITES];  // planes xy, xz, xt, yz, yt, zt
+  const int ls = threadIdx.x, pl = threadIdx.y;
+  // Traversal order.  Every link is needed by the 14 sites of its two-hop neighbourhood, of both parities; in plain
+  // checkerboard order (all even sites, then all odd; t slowest) the reuse window is three whole time slices of all
+  // links, twice over.  Here a block pair = the even and the odd sites of the same 32 checkerboard indices, and the
+  // index runs (x, y, z within a slab of CB_ZC planes, t, slab): the window is three time slices of ONE z-slab
+  // (7 MB at 32^3x64).  Measured (ncu, 32^3x64 fp64): DRAM reads 10.8 -> 7.1 GB, L2 hit rate 42 -> 55 %, time
+  // unchanged (4.5 ms; any CB_ZC from 2 to 16): the kernel waits on its 12 warps per SM, not on DRAM.
+  const int par = blockIdx.x & 1;
+  const int k = (blockIdx.x >> 1) * CB_SITES + ls;
+  const bool live = k < L.Vh;
+  int idx = 0;
+  if (live) {
+    const int zc = (L.Lz % CB_ZC == 0) ? CB_ZC : 2;  // every extent is even
+    const int plane = L.Lxh * L.Ly;
+    const int xy = k % plane;
+    int q = k / plane;
+    const int zl = q % zc;
+    q /= zc;
+    const int t = q % L.Lt, slab = q / L.Lt;
+    idx = xy + plane * ((slab * zc + zl) + L.Lz * t);
+  }
+  if (live) {
+    const Site s = site_of(L, idx, par);
+    const int x0[4] = {2 * s.xh + s.r, s.y, s.z, s.t};
+    const int mu = pl < 3 ? 0 : (pl < 5 ? 1 : 2);
+    const int nu = pl < 3 ? pl + 1 : (pl < 5 ? pl - 1 : 3);
+    cd F[9];
+    field_strength<T, R>(gauge, L, x0, mu, nu, F);
+    herm_store(Fs[pl], ls, F);
+  }
+  __syncthreads();
+  if (!live || pl >= 2) return;
+  clover_blocks<T, CB_SITES>(Fs, ls, pl, clover, clover_inv, L, idx, par, kc, kt, flag);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Three-pass build (the default).  The one-kernel build above gathers 72 links per site and multiplies 72 times; it
+// waits on its loads (ncu: 52 % long-scoreboard stalls at 9 warps per SM, fp64 pipe 30 % busy).  The four leaves of a
+// plane are the SAME plaquette seen from its four corners, and moving the starting corner is a transport by one link:
+//   P(y)              = U_mu(y) U_nu(y+mu) [U_nu(y) U_mu(y+nu)]^dag                      (the leaf of y itself)
+//   leaf of y at y+nu = U_nu(y)^dag P(y) U_nu(y),   at y+mu = U_mu(y)^dag P(y) U_mu(y),   at y+mu+nu: both in turn.
+// Only Q - Q^dag enters F and the transport is linear, so each pass carries the anti-Hermitian part X = P - P^dag
+// (9 reals: 3 imaginary diagonals, 3 complex entries above the diagonal):
+//   pass 1: X1(x) = P(x) - P(x)^dag                                         3 products, 4 links
+//   pass 2: X2(x) = X1(x) + U_nu(x-nu)^dag X1(x-nu) U_nu(x-nu)              2 products, 1 link
+//   pass 3: X3(x) = X2(x) + U_mu(x-mu)^dag X2(x-mu) U_mu(x-mu) = Q - Q^dag  2 products, 1 link; F = X3/(8i); blocks, inverses
+// 42 products and 36 link loads per site instead of 72 and 72, every pass a streaming kernel.  Scratch: two fields
+// [6 planes][9][2 Vh] doubles (432 B per site each), owned by the context.
+struct AH {
+  double d[3];  // Im X_00, Im X_11, Im X_22
+  cd o[3];      // X_01, X_02, X_12
+};
+__device__ __forceinline__ M3 expand(const AH& a) {
+  M3 m;
+  m.m[0] = {0.0, a.d[0]};
+  m.m[4] = {0.0, a.d[1]};
+  m.m[8] = {0.0, a.d[2]};
+  m.m[1] = a.o[0];
+  m.m[2] = a.o[1];
+  m.m[5] = a.o[2];
+  m.m[3] = {-a.o[0].re, a.o[0].im};  // X_ji = -conj(X_ij)
+  m.m[6] = {-a.o[1].re, a.o[1].im};
+  m.m[7] = {-a.o[2].re, a.o[2].im};
+  return m;
+}
+__device__ __forceinline__ AH load_ah(const double* __restrict__ X, size_t V, int pl, size_t s) {
+  const double* p = X + (size_t)pl * 9 * V + s;
+  AH a;
+  a.d[0] = p[0];
+  a.d[1] = p[V];
+  a.d[2] = p[2 * V];
+#pragma unroll
+  for (int e = 0; e < 3; e++) a.o[e] = {p[(3 + 2 * e) * V], p[(4 + 2 * e) * V]};
+  return a;
+}
+__device__ __forceinline__ void store_ah(double* __restrict__ X, size_t V, int pl, size_t s, const AH& a) {
+  double* p = X + (size_t)pl * 9 * V + s;
+  p[0] = a.d[0];
+  p[V] = a.d[1];
+  p[2 * V] = a.d[2];
+#pragma unroll
+  for (int e = 0; e < 3; e++) {
+    p[(3 + 2 * e) * V] = a.o[e].re;
+    p[(4 + 2 * e) * V] = a.o[e].im;
+  }
+}
+// entry (i, j) of a^dag b
+__device__ __forceinline__ cd dag_mul_entry(const M3& a, const M3& b, int i, int j) {
+  double re = a.m[i].re * b.m[j].re, im = a.m[i].re * b.m[j].im;
+  re = fma(a.m[i].im, b.m[j].im, re);
+  im = fma(-a.m[i].im, b.m[j].re, im);
+#pragma unroll
+  for (int k = 1; k < 3; k++) {
+    re = fma(a.m[3 * k + i].re, b.m[3 * k + j].re, re);
+    re = fma(a.m[3 * k + i].im, b.m[3 * k + j].im, re);
+    im = fma(a.m[3 * k + i].re, b.m[3 * k + j].im, im);
+    im = fma(-a.m[3 * k + i].im, b.m[3 * k + j].re, im);
+  }
+  return {re, im};
+}
+// the slab traversal of the one-kernel build: block pair = even and odd sites of the same 32 checkerboard indices
+template <int NS = CB_SITES>
+__device__ __forceinline__ bool cb_site(const Lat& L, int& idx, int& par) {
+  par = blockIdx.x & 1;
+  const int k = (blockIdx.x >> 1) * NS + threadIdx.x;
+  if (k >= L.Vh) return false;
+  const int zc = (L.Lz % CB_ZC == 0) ? CB_ZC : 2;
+  const int plane = L.Lxh * L.Ly;
+  const int xy = k % plane;
+  int q = k / plane;
+  const int zl = q % zc;
+  q /= zc;
+  const int t = q % L.Lt, slab = q / L.Lt;
+  idx = xy + plane * ((slab * zc + zl) + L.Lz * t);
+  return true;
+}
+__device__ __forceinline__ void plane_dirs(int pl, int& mu, int& nu) {
+  mu = pl < 3 ? 0 : (pl < 5 ? 1 : 2);
+  nu = pl < 3 ? pl + 1 : (pl < 5 ? pl - 1 : 3);
+}
+__device__ __forceinline__ size_t site_slot(const Lat& L, const int* x) {
+  const int par = (x[0] + x[1] + x[2] + x[3]) & 1;
+  return (size_t)par * L.Vh + (x[0] >> 1) + L.Lxh * (x[1] + L.Ly * (x[2] + L.Lz * x[3]));
+}
+
+#ifndef CB3_MINB
+#define CB3_MINB 3
+#endif
+#ifndef CB1_MINB
+#define CB1_MINB 2  // 168 registers: the four links of a leaf in flight at once (3 blocks: 96 registers, +9 %)
+#endif
+template <typename T, int R>
+__global__ void __launch_bounds__(CB_SITES * 6, CB1_MINB) clover_plaquette_kernel(double* __restrict__ X1, const T* __restrict__ gauge, Lat L) {
+  int idx, par;
+  if (!cb_site(L, idx, par)) return;
+  const int pl = threadIdx.y;
+  int mu, nu;
+  plane_dirs(pl, mu, nu);
+  const Site s = site_of(L, idx, par);
+  int x[4] = {2 * s.xh + s.r, s.y, s.z, s.t}, a[4], b[4];
+  for (int i = 0; i < 4; i++) a[i] = b[i] = x[i];
+  step(L, a, mu, +1);
+  step(L, b, nu, +1);
+  const M3 A = mul(link_at<T, R>(gauge, L, mu, x), link_at<T, R>(gauge, L, nu, a));
+  const M3 B = mul(link_at<T, R>(gauge, L, nu, x), link_at<T, R>(gauge, L, mu, b));
+  const M3 P = mul(A, dag(B));
+  AH h;
+#pragma unroll
+  for (int i = 0; i < 3; i++) h.d[i] = 2.0 * P.m[4 * i].im;
+  h.o[0] = P.m[1] - conj(P.m[3]);
+  h.o[1] = P.m[2] - conj(P.m[6]);
+  h.o[2] = P.m[5] - conj(P.m[7]);
+  store_ah(X1, (size_t)2 * L.Vh, pl, (size_t)par * L.Vh + idx, h);
+}
+
+// X(x) + U_d(x-d)^dag X(x-d) U_d(x-d)
+template <typename T, int R>
+__device__ __forceinline__ AH transport_sum(const double* __restrict__ X, const T* __restrict__ gauge, const Lat& L, int pl,
+                                            int d, const int* x0, size_t s0) {
+  int xm[4];
+  for (int i = 0; i < 4; i++) xm[i] = x0[i];
+  step(L, xm, d, -1);
+  const M3 U = link_at<T, R>(gauge, L, d, xm);
+  const M3 Y = mul(expand(load_ah(X, (size_t)2 * L.Vh, pl, site_slot(L, xm))), U);
+  AH r = load_ah(X, (size_t)2 * L.Vh, pl, s0);
+#pragma unroll
+  for (int i = 0; i < 3; i++) r.d[i] += dag_mul_entry(U, Y, i, i).im;
+  r.o[0] = r.o[0] + dag_mul_entry(U, Y, 0, 1);
+  r.o[1] = r.o[1] + dag_mul_entry(U, Y, 0, 2);
+  r.o[2] = r.o[2] + dag_mul_entry(U, Y, 1, 2);
+  return r;
+}
+template <typename T, int R>
+__global__ void __launch_bounds__(CB_SITES * 6, CB3_MINB) clover_transport_kernel(double* __restrict__ X2, const double* __restrict__ X1,
+                                                                           const T* __restrict__ gauge, Lat L) {
+  int idx, par;
+  if (!cb_site(L, idx, par)) return;
+  const int pl = threadIdx.y;
+  int mu, nu;
+  plane_dirs(pl, mu, nu);
+  const Site s = site_of(L, idx, par);
+  const int x0[4] = {2 * s.xh + s.r, s.y, s.z, s.t};
+  const size_t s0 = (size_t)par * L.Vh + idx;
+  store_ah(X2, (size_t)2 * L.Vh, pl, s0, transport_sum<T, R>(X1, gauge, L, pl, nu, x0, s0));
+}
+
+// Pass 3.  Two threads per site in BOTH phases: thread (s, k) transports planes 3k..3k+2, then inverts chiral block k.
+// (With one thread per plane, as in passes 1 and 2, four of a block's six warps idle through the inversions, whose
+// dependent chains -- pivot search, reciprocal, elimination -- then run on 4 warps per SM: 1.4 of the pass's 1.9 ms.)
+#ifndef CBF_SITES
+#define CBF_SITES 64
+#endif
+#ifndef CBF_MINB
+#define CBF_MINB 3
+#endif
+template <typename T, int R>
+__global__ void __launch_bounds__(CBF_SITES * 2, CBF_MINB) clover_finish_kernel(T* __restrict__ clover, T* __restrict__ clover_inv,
+                                                                          const double* __restrict__ X2, const T* __restrict__ gauge,
+                                                                          Lat L, double kc, double kt, int* flag) {
+  __shared__ double Fs[6][9][CBF_SITES];
+  const int ls = threadIdx.x, k = threadIdx.y;
+  int idx = 0, par = 0;
+  const bool live = cb_site<CBF_SITES>(L, idx, par);
+  if (live) {
+    const Site s = site_of(L, idx, par);
+    const int x0[4] = {2 * s.xh + s.r, s.y, s.z, s.t};
+#pragma unroll
+    for (int i = 0; i < 3; i++) {
+      const int pl = 3 * k + i;
+      int mu, nu;
+      plane_dirs(pl, mu, nu);
+      const AH q = transport_sum<T, R>(X2, gauge, L, pl, mu, x0, (size_t)par * L.Vh + idx);  // Q - Q^dag
+      // F = (Q - Q^dag)/(8i): Hermitian
+#pragma unroll
+      for (int d = 0; d < 3; d++) Fs[pl][d][ls] = 0.125 * q.d[d];
+#pragma unroll
+      for (int e = 0; e < 3; e++) {
+        Fs[pl][3 + 2 * e][ls] = 0.125 * q.o[e].im;
+        Fs[pl][4 + 2 * e][ls] = -0.125 * q.o[e].re;
+      }
+    }
+  }
+  __syncthreads();
+  if (!live) return;
+  clover_blocks<T, CBF_SITES>(Fs, ls, k, clover, clover_inv, L, idx, par, kc, kt, flag);
+}
+
+template <typename T, int R>
+static void clover_build_launch(lqcd_ctx* c, void* clover, void* clover_inv, const void* gauge, double kc, double kt, cudaStream_t st) {
+  const int grid = 2 * ((c->lat.Vh + CB_SITES - 1) / CB_SITES);
+  const dim3 block(CB_SITES, 6);
+  if (!c->clover_onepass && !c->d_clover_scratch) {
+    // two fields of 6 planes x 9 doubles per site; if they do not fit, the one-kernel build needs none
+    if (cudaMalloc(&c->d_clover_scratch, sizeof(double) * 2 * 54 * (size_t)2 * c->lat.Vh) != cudaSuccess) {
+      cudaGetLastError();
+      c->d_clover_scratch = nullptr;
+      c->clover_onepass = 1;
+    }
+  }
+  if (c->clover_onepass) {
+    clover_build_kernel<T, R><<<grid, block, 0, st>>>((T*)clover, (T*)clover_inv, (const T*)gauge, c->lat, kc, kt, c->d_flag);
+    return;
+  }
+  double* X1 = c->d_clover_scratch;
+  double* X2 = X1 + 54 * (size_t)2 * c->lat.Vh;
+  clover_plaquette_kernel<T, R><<<grid, block, 0, st>>>(X1, (const T*)gauge, c->lat);
+  clover_transport_kernel<T, R><<<grid, block, 0, st>>>(X2, X1, (const T*)gauge, c->lat);
+  clover_finish_kernel<T, R><<<2 * ((c->lat.Vh + CBF_SITES - 1) / CBF_SITES), dim3(CBF_SITES, 2), 0, st>>>((T*)clover, (T*)clover_inv, X2, (const T*)gauge, c->lat, kc, kt, c->d_flag);
+  c->launches += 2;  // LQCD_LAUNCH_CHECK counts the third
+}
+
 extern "C" int lqcd_clover_build_aniso(lqcd_ctx* c, void* clover, void* clover_inv, const void* gauge, double csw_s,
                                        double csw_t, double kappa, void* stream) {
   if (!c || !clover || !gauge) return LQCD_ERR_INVALID_ARG;
@@ -307,19 +551,17 @@ extern "C" int lqcd_clover_build_aniso(lqcd_ctx* c, void* clover, void* clover_i
   if (!lqcd_aligned16(clover) || !lqcd_aligned16(clover_inv) || !lqcd_aligned16(gauge))
     return lqcd_set_error(c, LQCD_ERR_ALIGN, "clover_build: alignment");
   cudaStream_t st = as_stream(stream);
-  const int grid = 2 * ((c->lat.Vh + CB_SITES - 1) / CB_SITES);
-  const dim3 block(CB_SITES, 6);
   const double kc = kappa * csw_s, kt = kappa * csw_t;
   cudaMemsetAsync(c->d_flag, 0, sizeof(int), st);
   c->alg_bytes += (double)lqcd_gauge_bytes(c) + (clover_inv ? 2.0 : 1.0) * (double)lqcd_clover_bytes(c);
   if (c->prec == 4 && c->recon == 18)
-    clover_build_kernel<float, 18><<<grid, block, 0, st>>>((float*)clover, (float*)clover_inv, (const float*)gauge, c->lat, kc, kt, c->d_flag);
+    clover_build_launch<float, 18>(c, clover, clover_inv, gauge, kc, kt, st);
   else if (c->prec == 4)
-    clover_build_kernel<float, 12><<<grid, block, 0, st>>>((float*)clover, (float*)clover_inv, (const float*)gauge, c->lat, kc, kt, c->d_flag);
+    clover_build_launch<float, 12>(c, clover, clover_inv, gauge, kc, kt, st);
   else if (c->recon == 18)
-    clover_build_kernel<double, 18><<<grid, block, 0, st>>>((double*)clover, (double*)clover_inv, (const double*)gauge, c->lat, kc, kt, c->d_flag);
+    clover_build_launch<double, 18>(c, clover, clover_inv, gauge, kc, kt, st);
   else
-    clover_build_kernel<double, 12><<<grid, block, 0, st>>>((double*)clover, (double*)clover_inv, (const double*)gauge, c->lat, kc, kt, c->d_flag);
+    clover_build_launch<double, 12>(c, clover, clover_inv, gauge, kc, kt, st);
   LQCD_LAUNCH_CHECK(c, "clover_build");
   cudaMemcpyAsync(c->h_flag, c->d_flag, sizeof(int), cudaMemcpyDeviceToHost, st);
   if (cudaStreamSynchronize(st) != cudaSuccess) return lqcd_check_cuda(c, "clover_build sync");

@@ -86,6 +86,8 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], int prec, int recon, int t_bo
     c->mrhs_fuse_dots = fd ? (fd[0] == '1') : -1;  // -1: where the register kernel runs the plain epilogues anyway
     const char* gr = getenv("LQCD_GRAPHS");
     c->graphs_on = (gr && gr[0] == '0') ? 0 : 1;
+    const char* co = getenv("LQCD_CLOVER_ONEPASS");
+    c->clover_onepass = (co && co[0] == '1') ? 1 : 0;
     const char* z = getenv("LQCD_MRHS_ZSLAB");
     c->mrhs_zslab = z ? atoi(z) : -1;  // pairs of z-planes per slab; -1: each kernel's own default (4 TMA-tiled, 2 register kernels)
   }
@@ -130,6 +132,7 @@ int lqcd_destroy(lqcd_ctx* c) {
   cudaSetDevice(c->device);
   if (c->d_partial) cudaFree(c->d_partial);
   if (c->d_partial_mrhs) cudaFree(c->d_partial_mrhs);
+  if (c->d_clover_scratch) cudaFree(c->d_clover_scratch);
   if (c->d_scalars) cudaFree(c->d_scalars);
   if (c->d_ticket) cudaFree(c->d_ticket);
   if (c->d_flag) cudaFree(c->d_flag);
