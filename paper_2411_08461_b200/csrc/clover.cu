@@ -233,58 +233,138 @@ __device__ __forceinline__ void herm_store(double (&F)[9][NS], int ls, const cd*
   F[7][ls] = f9[5].re;
   F[8][ls] = f9[5].im;
 }
-// Phase 2 of either build: thread k < 2 of a site assembles chiral block k from the six F in shared memory, packs it,
-// inverts it by Gauss-Jordan and stores both.
+// Inverse of a Hermitian positive definite 6x6 matrix held as its packed lower triangle (6 real diagonals dg, 15
+// complex entries lo[i(i-1)/2+j], i > j) by the symmetric sweep operator: for k = 0..5
+//   d = a_kk;  a_ij -= a_ik a_kj / d (i, j != k);  a_ik /= d;  a_kk = -1/d        and the result is -A^-1.
+// The pivot of step k is the k-th pivot of the LDL^H factorisation, so "every pivot > thresh" proves positive
+// definiteness, for which elimination without pivoting is stable.  Half the multiply-adds of Gauss-Jordan on the full
+// matrix and no row exchanges (two thirds of invert6's instructions are the selects of its swap networks).  Returns
+// false as soon as a pivot fails the test (the matrix is then left half swept).
+__device__ __forceinline__ bool sweep6(double (&dg)[6], cd (&lo)[15], double thresh) {
+  bool ok = true;
+#pragma unroll
+  for (int k = 0; k < 6; k++) {
+    const double d = dg[k];
+    ok = ok && (d > thresh);
+    const double id = 1.0 / d;
+    cd col[6];  // a_ik, i != k
+#pragma unroll
+    for (int i = 0; i < 6; i++) {
+      if (i == k) continue;
+      col[i] = i > k ? lo[i * (i - 1) / 2 + k] : conj(lo[k * (k - 1) / 2 + i]);
+    }
+#pragma unroll
+    for (int i = 0; i < 6; i++) {
+      if (i == k) continue;
+      const cd bi = {col[i].re * id, col[i].im * id};
+      dg[i] = fma(-bi.re, col[i].re, fma(-bi.im, col[i].im, dg[i]));
+#pragma unroll
+      for (int j = 0; j < i; j++) {
+        if (j == k) continue;
+        cd& a = lo[i * (i - 1) / 2 + j];  // a_ij -= (a_ik / d) conj(a_jk)
+        a.re = fma(-bi.re, col[j].re, fma(-bi.im, col[j].im, a.re));
+        a.im = fma(-bi.im, col[j].re, fma(bi.re, col[j].im, a.im));
+      }
+      if (i > k)
+        lo[i * (i - 1) / 2 + k] = bi;
+      else
+        lo[k * (k - 1) / 2 + i] = conj(bi);
+    }
+    dg[k] = -id;
+  }
+  return ok;
+}
+
+// chiral block k of a site from the six F in shared memory: A_block = 1 - [[E3, E1 - i E2], [E1 + i E2, -E3]] with
+// E3 = kc F_xy -/+ kt F_zt, E2 = kc F_xz +/- kt F_yt, E1 = kc F_yz -/+ kt F_xt (upper sign: k = 0);
+// kc = kappa*csw on the spatial planes, kt = kappa*csw_t on the temporal ones (Eq. 5)
+template <int NS>
+__device__ __forceinline__ void assemble_block(const double (&Fs)[6][9][NS], int ls, int k, double kc, double kt, cd (&B)[6][6]) {
+  const double st = (k == 0 ? 1.0 : -1.0) * kt;
+#pragma unroll
+  for (int i = 0; i < 3; i++)
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+      const cd Fxy = herm_entry(Fs[0], i, j, ls), Fxz = herm_entry(Fs[1], i, j, ls), Fxt = herm_entry(Fs[2], i, j, ls),
+               Fyz = herm_entry(Fs[3], i, j, ls), Fyt = herm_entry(Fs[4], i, j, ls), Fzt = herm_entry(Fs[5], i, j, ls);
+      const cd E3 = {kc * Fxy.re - st * Fzt.re, kc * Fxy.im - st * Fzt.im};
+      const cd E2 = {kc * Fxz.re + st * Fyt.re, kc * Fxz.im + st * Fyt.im};
+      const cd E1 = {kc * Fyz.re - st * Fxt.re, kc * Fyz.im - st * Fxt.im};
+      const double d = (i == j) ? 1.0 : 0.0;
+      B[i][j] = {d - E3.re, -E3.im};
+      B[3 + i][3 + j] = {d + E3.re, E3.im};
+      B[i][3 + j] = {-(E1.re + E2.im), -(E1.im - E2.re)};  // E1 - i E2
+      B[3 + i][j] = {-(E1.re - E2.im), -(E1.im + E2.re)};  // E1 + i E2
+    }
+}
+
+// the rare path of clover_blocks, out of line so that its registers and spills are not the common path's
 template <typename T, int NS>
-__device__ __forceinline__ void clover_blocks(const double (&Fs)[6][9][NS], int ls, int pl, T* __restrict__ clover,
+__device__ __noinline__ void general_inverse_store(const double (&Fs)[6][9][NS], int ls, int k, double kc, double kt,
+                                                   T* __restrict__ field, int Vh, int idx, int* flag) {
+  double pk[36];
+  cd a[6][6];
+  assemble_block(Fs, ls, k, kc, kt, a);
+  if (!invert6(a)) {
+    atomicExch(flag, 1);
+    for (int i = 0; i < 36; i++) pk[i] = 0;
+  } else {
+    for (int i = 0; i < 6; i++) pk[i] = a[i][i].re;
+    for (int i = 1; i < 6; i++)
+      for (int j = 0; j < i; j++) {
+        // average the two triangles so rounding stays symmetric
+        const int o = 6 + 2 * (i * (i - 1) / 2 + j);
+        pk[o] = 0.5 * (a[i][j].re + a[j][i].re);
+        pk[o + 1] = 0.5 * (a[i][j].im - a[j][i].im);
+      }
+  }
+  store_block<T>(field, Vh, idx, k, pk);
+}
+
+// Phase 2 of either build: thread k < 2 of a site assembles chiral block k (exactly Hermitian: the shared-memory F
+// are), packs and stores it, and inverts it: by the sweep above where every pivot exceeds 1e-6 of the largest
+// diagonal entry (every block of a sensible field: at configs 3 and 4 the smallest pivot is 0.6), otherwise -- not
+// positive definite or nearly singular -- by Gauss-Jordan with partial pivoting on the re-assembled block
+// (no positive-definiteness assumed), which also decides LQCD_ERR_SINGULAR_CLOVER.
+template <typename T, int NS>
+__device__ __forceinline__ void clover_blocks(const double (&Fs)[6][9][NS], int ls, int k, T* __restrict__ clover,
                                               T* __restrict__ clover_inv, const Lat& L, int idx, int par, double kc, double kt,
                                               int* flag) {
   const size_t half = (size_t)72 * L.Vh;  // reals per parity of a clover field
+  double pk[36];
+  double dg[6];
+  cd lo[15];
   {
-    const int k = pl;
-    const double sg = k == 0 ? 1.0 : -1.0;
     cd B[6][6];
-    for (int i = 0; i < 3; i++)
-      for (int j = 0; j < 3; j++) {
-        // kc = kappa*csw on the spatial planes, kt = kappa*csw_t on the temporal ones (Eq. 5)
-        const double st = sg * kt;
-        const cd Fxy = herm_entry(Fs[0], i, j, ls), Fxz = herm_entry(Fs[1], i, j, ls), Fxt = herm_entry(Fs[2], i, j, ls),
-                 Fyz = herm_entry(Fs[3], i, j, ls), Fyt = herm_entry(Fs[4], i, j, ls), Fzt = herm_entry(Fs[5], i, j, ls);
-        cd E3 = {kc * Fxy.re - st * Fzt.re, kc * Fxy.im - st * Fzt.im};  // kc F_xy -/+ kt F_zt
-        cd E2 = {kc * Fxz.re + st * Fyt.re, kc * Fxz.im + st * Fyt.im};  // kc F_xz +/- kt F_yt
-        cd E1 = {kc * Fyz.re - st * Fxt.re, kc * Fyz.im - st * Fxt.im};  // kc F_yz -/+ kt F_xt
-        const double d = (i == j) ? 1.0 : 0.0;
-        B[i][j] = {d - E3.re, -E3.im};
-        B[3 + i][3 + j] = {d + E3.re, E3.im};
-        B[i][3 + j] = {-(E1.re + E2.im), -(E1.im - E2.re)};      // E1 - i E2
-        B[3 + i][j] = {-(E1.re - E2.im), -(E1.im + E2.re)};      // E1 + i E2
-      }
-    double pk[36];
-    for (int i = 0; i < 6; i++) pk[i] = B[i][i].re;
+    assemble_block(Fs, ls, k, kc, kt, B);
+#pragma unroll
+    for (int i = 0; i < 6; i++) pk[i] = dg[i] = B[i][i].re;
+#pragma unroll
     for (int i = 1; i < 6; i++)
+#pragma unroll
       for (int j = 0; j < i; j++) {
-        // Hermitian by construction; average the two triangles so rounding stays symmetric
-        const int o = 6 + 2 * (i * (i - 1) / 2 + j);
-        pk[o] = 0.5 * (B[i][j].re + B[j][i].re);
-        pk[o + 1] = 0.5 * (B[i][j].im - B[j][i].im);
+        const int o = i * (i - 1) / 2 + j;
+        lo[o] = B[i][j];
+        pk[6 + 2 * o] = B[i][j].re;
+        pk[7 + 2 * o] = B[i][j].im;
       }
-    store_block<T>(clover + par * half, L.Vh, idx, k, pk);
-    if (clover_inv) {
-      cd (&a)[6][6] = B;  // inverted in place
-      if (!invert6(a)) {
-        atomicExch(flag, 1);
-        for (int i = 0; i < 36; i++) pk[i] = 0;
-      } else {
-        for (int i = 0; i < 6; i++) pk[i] = a[i][i].re;
-        for (int i = 1; i < 6; i++)
-          for (int j = 0; j < i; j++) {
-            const int o = 6 + 2 * (i * (i - 1) / 2 + j);
-            pk[o] = 0.5 * (a[i][j].re + a[j][i].re);
-            pk[o + 1] = 0.5 * (a[i][j].im - a[j][i].im);
-          }
-      }
-      store_block<T>(clover_inv + par * half, L.Vh, idx, k, pk);
+  }
+  store_block<T>(clover + par * half, L.Vh, idx, k, pk);
+  if (!clover_inv) return;
+  double nrm = dg[0];
+#pragma unroll
+  for (int i = 1; i < 6; i++) nrm = fmax(nrm, dg[i]);
+  if (sweep6(dg, lo, fmax(1e-6 * nrm, 0.0))) {
+#pragma unroll
+    for (int i = 0; i < 6; i++) pk[i] = -dg[i];
+#pragma unroll
+    for (int o = 0; o < 15; o++) {
+      pk[6 + 2 * o] = -lo[o].re;
+      pk[7 + 2 * o] = -lo[o].im;
     }
+    store_block<T>(clover_inv + par * half, L.Vh, idx, k, pk);
+  } else {
+    general_inverse_store<T, NS>(Fs, ls, k, kc, kt, clover_inv + par * half, L.Vh, idx, flag);
   }
 }
 

@@ -117,6 +117,27 @@ def test_clover_build_and_apply(prec, recon):
         assert rel_err(s.down(out), s.orc.clover_apply(psi, inverse=inverse)) < TOL[prec]
 
 
+@pytest.mark.parametrize("onepass", ["0", "1"])
+def test_clover_inverse_of_indefinite_blocks_and_both_build_forms(onepass, monkeypatch):
+    """kappa*csw = 1.2 on a rough field makes most 6x6 blocks indefinite: the Hermitian sweep must hand every such block
+    to the pivoted elimination.  Run for the three-pass build and for the one-kernel build (LQCD_CLOVER_ONEPASS=1);
+    both against the oracle, whose inverse is a general pivoted one."""
+    monkeypatch.setenv("LQCD_CLOVER_ONEPASS", onepass)
+    for dims, kappa, csw in (((4, 6, 8, 10), 0.12, 10.0), ((8, 8, 8, 16), 0.124, 1.2)):
+        s = Setup(dims, 0.7, 9, kappa, csw, 8, 18)
+        A_o, Ai_o = s.orc.clover()
+        A_g = s.ctx.clover_unpack(s.A).cpu().numpy()
+        Ai_g = s.ctx.clover_unpack(s.Ai).cpu().numpy()
+        if csw > 5:
+            assert (A_o[..., :6] < 0).any()  # negative diagonal entries: certainly not positive definite
+        assert rel_err(A_g, A_o) < 1e-13
+        # an indefinite block may be badly conditioned; bound the error blockwise by its condition
+        scale = np.abs(Ai_o).max(axis=-1, keepdims=True)
+        assert (np.abs(Ai_g - Ai_o) / scale).max() < 1e-10
+        assert rel_err(Ai_g, Ai_o) < 1e-11
+        s.ctx.close()
+
+
 def test_clover_build_csw_zero_and_singular():
     s = Setup((4, 4, 4, 8), 0.3, 1, 0.12, 0.0, 8, 18)
     A = s.ctx.clover_unpack(s.A).cpu().numpy()
