@@ -17,8 +17,8 @@
  * caller only needs their byte sizes (lqcd_*_bytes) and moves data with pack/unpack.
  *
  * Conventions.  Every pointer is a DEVICE pointer unless the name ends in _host.  The caller owns
- * all buffers; the library keeps none beyond the call (the context owns only a small reduction
- * scratch).  Device pointers must be 16-byte aligned.  All calls are asynchronous on `stream`
+ * all buffers; the library keeps none beyond the call (the context owns a small reduction
+ * scratch and, after a clover build, that build's scratch).  Device pointers must be 16-byte aligned.  All calls are asynchronous on `stream`
  * (a cudaStream_t passed as void*) except lqcd_invert*, lqcd_*_host and lqcd_blas_*, which
  * synchronise the stream before returning.  Return: 0 = OK, <0 = error, +1 = NOT_CONVERGED.
  * No exceptions, no abort, nothing printed.  A context is not thread-safe.
@@ -70,7 +70,8 @@ typedef struct lqcd_result {
  *   LQCD_MRHS_ZSLAB=n        z-planes per slab of the multi-RHS block sweep (default per kernel);
  *   LQCD_MRHS_FUSE_DOTS=0|1  batched BiCGStab dot products in the multi-RHS epilogues: never | always (default: where
  *                            the register kernel runs the epilogue anyway);
- *   LQCD_GRAPHS=0            no CUDA-graph replay of Krylov iteration blocks on small lattices. */
+ *   LQCD_GRAPHS=0            no CUDA-graph replay of Krylov iteration blocks on small lattices;
+ *   LQCD_CLOVER_ONEPASS=1    one-kernel clover build (no scratch) instead of the three-pass one. */
 int lqcd_create(lqcd_ctx** ctx, const int dims[4], int prec, int recon, int t_boundary, int device);
 int lqcd_destroy(lqcd_ctx* ctx);
 const char* lqcd_strerror(int code);
@@ -112,7 +113,10 @@ int lqcd_clover_pack(lqcd_ctx* ctx, void* clover_native, const void* clover_publ
 /* Clover term and its inverse from the links ("the clover field is then created";
  * SURVEY.md §8(c) O4-O6).  kappa is required because A contains kappa*csw (reading A6).  Leaves
  * and the 6x6 inverses are computed in fp64 whatever the storage precision.  clover_inv may be
- * NULL.  Synchronises; returns LQCD_ERR_SINGULAR_CLOVER if some block has a pivot < 1e-12|A|. */
+ * NULL.  Synchronises; returns LQCD_ERR_SINGULAR_CLOVER if some block has a pivot < 1e-12|A|.
+ * Ownership: the first build makes the context allocate a scratch of 864 bytes per lattice site (two fields of
+ * plaquette parts between the passes of the build), kept until lqcd_destroy; if that allocation fails
+ * the build falls back to a one-kernel form that needs none. */
 int lqcd_clover_build(lqcd_ctx* ctx, void* clover, void* clover_inv, const void* gauge, double csw,
                       double kappa, void* stream);
 
