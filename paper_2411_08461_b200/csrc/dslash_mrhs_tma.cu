@@ -37,12 +37,14 @@ template <int LXH_, int TY_, int TZ_, int TT_, int NST_, int MINB_> struct RowTi
   static constexpr int NS = LXH * RC;                          // output sites per tile
   static constexpr int NYH = TZ * TT, NZH = TY * TT, NTH = TY * TZ;  // rows of one halo face
   static constexpr int ROWB = LXH * 16;                        // bytes of one vector of one row
-  // a stage holds seven regions, one TMA box each, every region [vector][row][xh] float4 (the order a box lands in):
+  // a stage holds seven regions, one TMA box each, every region [row][vector][xh] float4 (the order a box lands in:
+  // the tensor map puts the vector index second, so the six vectors of a site are ROWB apart in EVERY region and a
+  // hop's six loads share one address register):
   // core (rows ly + TY (lz + TZ lt)), y-, y+ (rows lz + TZ lt), z-, z+ (ly + TY lt), t-, t+ (ly + TY lz)
-  static constexpr int VS_C = RC * ROWB, VS_Y = NYH * ROWB, VS_Z = NZH * ROWB, VS_T = NTH * ROWB;  // vector strides
-  static constexpr int B_C = 0, B_YM = 6 * VS_C, B_YP = B_YM + 6 * VS_Y, B_ZM = B_YP + 6 * VS_Y, B_ZP = B_ZM + 6 * VS_Z,
-                       B_TM = B_ZP + 6 * VS_Z, B_TP = B_TM + 6 * VS_T;
-  static constexpr int STAGE_BYTES = B_TP + 6 * VS_T;
+  static constexpr int RS = 6 * ROWB;  // row stride
+  static constexpr int B_C = 0, B_YM = RC * RS, B_YP = B_YM + NYH * RS, B_ZM = B_YP + NYH * RS, B_ZP = B_ZM + NZH * RS,
+                       B_TM = B_ZP + NZH * RS, B_TP = B_TM + NTH * RS;
+  static constexpr int STAGE_BYTES = B_TP + NTH * RS;
   static constexpr int NCONS = 2 * NS;                         // threads: two per site
 };
 
@@ -83,17 +85,17 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned pari
         : "memory");
   } while (!ok);
 }
-// one 5-D box {all of x, by, bz, bt, 6 vectors} of the input field -> shared memory, completion bytes on `bar`
+// one 5-D box {all of x, 6 vectors, by, bz, bt} of the input field -> shared memory, completion bytes on `bar`
 __device__ __forceinline__ void tma_load_box(void* dst, const CUtensorMap* map, int y, int z, int t, int v0,
                                              unsigned long long* bar) {
   asm volatile(
       "cp.async.bulk.tensor.5d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5, %6}], [%7];" ::"r"(
           smem_u32(dst)),
-      "l"(reinterpret_cast<unsigned long long>(map)), "r"(0), "r"(y), "r"(z), "r"(t), "r"(v0), "r"(smem_u32(bar))
+      "l"(reinterpret_cast<unsigned long long>(map)), "r"(0), "r"(v0), "r"(y), "r"(z), "r"(t), "r"(smem_u32(bar))
       : "memory");
 }
 struct TmaMaps {
-  CUtensorMap core, yface, zface, tface;  // the same field, boxes {x, TY, TZ, TT, 6}, {x, 1, TZ, TT, 6}, {x, TY, 1, TT, 6}, {x, TY, TZ, 1, 6}
+  CUtensorMap core, yface, zface, tface;  // the same field, boxes {x, 6, TY, TZ, TT}, {x, 6, 1, TZ, TT}, {x, 6, TY, 1, TT}, {x, 6, TY, TZ, 1}
 };
 // the seven boxes of column c of the tile at (y0, z0, t0) into the stage at `sb`; called by ONE thread
 template <typename TS>
@@ -113,15 +115,14 @@ __device__ __forceinline__ void issue_stage(unsigned char* sb, const TmaMaps* m,
 }
 __device__ __forceinline__ void pair_barrier(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
 
-// one hop from the staged tile: sp = this site's neighbour, vector 0; the six vectors are vs bytes apart (the
-// vector stride of the region the neighbour lies in: the core box or a halo face)
-template <int MU, bool FWD, bool DAG>
-__device__ __forceinline__ void hop_sm(float* acc, const unsigned char* sp, int vs, const float* U, float w) {
+// one hop from the staged tile: sp = this site's neighbour, vector 0; the six vectors are VS bytes apart
+template <int MU, bool FWD, bool DAG, int VS>
+__device__ __forceinline__ void hop_sm(float* acc, const unsigned char* sp, const float* U, float w) {
   constexpr int S = (FWD != DAG) ? -1 : +1;
   float psi[24], h[12], chi[12];
 #pragma unroll
   for (int v = 0; v < 6; v++) {
-    const float4 q = *reinterpret_cast<const float4*>(sp + v * vs);
+    const float4 q = *reinterpret_cast<const float4*>(sp + v * VS);
     vec_get(q, psi + 4 * v);
   }
   project<float, MU, S>(psi, h);
@@ -151,19 +152,17 @@ __device__ __forceinline__ void consume(const TmaMaps* maps, const TmaArgs& a, u
   const int idx = s.xh + L.Lxh * (s.y + L.Ly * (s.z + L.Lz * s.t));
   const size_t blk = (size_t)R * Vh;
   // this role's four hops: byte offset of the neighbour inside a stage, and the four links (registers, all columns)
-  int n0, n1, n2, n3, v0, v1, v2, v3;  // neighbour: byte offset of vector 0 in a stage, vector stride of its region
+  int n0, n1, n2, n3;  // neighbour: byte offset of its vector 0 in a stage
   float U0[18], U1[18], U2[18], U3[18];
   float w2, w3;
+  constexpr int RS = TS::RS;
   if (ROLE == 0) {
     const int xp = s.r ? (lxh + 1 == LXH ? 0 : lxh + 1) : lxh, xm = s.r ? lxh : (lxh == 0 ? LXH - 1 : lxh - 1);
     const int fy = lz + TZ * lt;  // row in a y face
-    n0 = TS::B_C + crow * TS::ROWB + xp * 16;
-    n1 = TS::B_C + crow * TS::ROWB + xm * 16;
-    v0 = v1 = TS::VS_C;
-    n2 = (ly + 1 < TY ? TS::B_C + (crow + 1) * TS::ROWB : TS::B_YP + fy * TS::ROWB) + lxh * 16;
-    v2 = ly + 1 < TY ? TS::VS_C : TS::VS_Y;
-    n3 = (ly > 0 ? TS::B_C + (crow - 1) * TS::ROWB : TS::B_YM + fy * TS::ROWB) + lxh * 16;
-    v3 = ly > 0 ? TS::VS_C : TS::VS_Y;
+    n0 = TS::B_C + crow * RS + xp * 16;
+    n1 = TS::B_C + crow * RS + xm * 16;
+    n2 = (ly + 1 < TY ? TS::B_C + (crow + 1) * RS : TS::B_YP + fy * RS) + lxh * 16;
+    n3 = (ly > 0 ? TS::B_C + (crow - 1) * RS : TS::B_YM + fy * RS) + lxh * 16;
     load_link<float, R>(a.gauge + (0 * 2 + par) * blk, Vh, idx, U0);
     load_link<float, R>(a.gauge + (0 * 2 + 1 - par) * blk, Vh, neighbour<0, -1>(L, idx, s), U1);
     load_link<float, R>(a.gauge + (1 * 2 + par) * blk, Vh, idx, U2);
@@ -171,14 +170,10 @@ __device__ __forceinline__ void consume(const TmaMaps* maps, const TmaArgs& a, u
     w2 = w3 = a.ws;
   } else {
     const int fz = ly + TY * lt, ft = ly + TY * lz;  // rows in a z face, a t face
-    n0 = (lz + 1 < TZ ? TS::B_C + (crow + TY) * TS::ROWB : TS::B_ZP + fz * TS::ROWB) + lxh * 16;
-    v0 = lz + 1 < TZ ? TS::VS_C : TS::VS_Z;
-    n1 = (lz > 0 ? TS::B_C + (crow - TY) * TS::ROWB : TS::B_ZM + fz * TS::ROWB) + lxh * 16;
-    v1 = lz > 0 ? TS::VS_C : TS::VS_Z;
-    n2 = (lt + 1 < TT ? TS::B_C + (crow + TY * TZ) * TS::ROWB : TS::B_TP + ft * TS::ROWB) + lxh * 16;
-    v2 = lt + 1 < TT ? TS::VS_C : TS::VS_T;
-    n3 = (lt > 0 ? TS::B_C + (crow - TY * TZ) * TS::ROWB : TS::B_TM + ft * TS::ROWB) + lxh * 16;
-    v3 = lt > 0 ? TS::VS_C : TS::VS_T;
+    n0 = (lz + 1 < TZ ? TS::B_C + (crow + TY) * RS : TS::B_ZP + fz * RS) + lxh * 16;
+    n1 = (lz > 0 ? TS::B_C + (crow - TY) * RS : TS::B_ZM + fz * RS) + lxh * 16;
+    n2 = (lt + 1 < TT ? TS::B_C + (crow + TY * TZ) * RS : TS::B_TP + ft * RS) + lxh * 16;
+    n3 = (lt > 0 ? TS::B_C + (crow - TY * TZ) * RS : TS::B_TM + ft * RS) + lxh * 16;
     load_link<float, R>(a.gauge + (2 * 2 + par) * blk, Vh, idx, U0);
     load_link<float, R>(a.gauge + (2 * 2 + 1 - par) * blk, Vh, neighbour<2, -1>(L, idx, s), U1);
     load_link<float, R>(a.gauge + (3 * 2 + par) * blk, Vh, idx, U2);
@@ -194,12 +189,19 @@ __device__ __forceinline__ void consume(const TmaMaps* maps, const TmaArgs& a, u
   float4* xmine = xbuf + (ROLE * 3) * NS + sl;  // what I send: my partial sum of the half I do not own
   const float4* xtheirs = xbuf + ((1 - ROLE) * 3) * NS + sl;
 
-  for (int c = 0; c < a.nrhs; c++) {
-    const int st = c % NST;
-    const unsigned ph = (c / NST) & 1;
+  // the column loop is unrolled over the ring, so the stage of a column is a compile-time constant and every
+  // shared-memory address is a register of the set-up above plus an immediate
+  const float4* xp = reinterpret_cast<const float4*>(a.x + hoff);
+  float4* op = reinterpret_cast<float4*>(a.out + hoff);
+  const size_t cstride = a.stride / 4;  // float4 between columns
+  unsigned ph = 0;
+  for (int c0 = 0; c0 < a.nrhs; c0 += NST, ph ^= 1) {
+#pragma unroll
+   for (int st = 0; st < NST; st++) {
+    const int c = c0 + st;
+    if (c >= a.nrhs) break;
     float xv[12];
     if (EPI == 2 || EPI == 3 || EPI == 6) {  // issued before the wait: the latency hides behind it
-      const float4* xp = reinterpret_cast<const float4*>(a.x + (size_t)c * a.stride + hoff);
 #pragma unroll
       for (int v = 0; v < 3; v++) {
         const float4 q = ld_cached(xp + (size_t)v * Vh);
@@ -211,10 +213,10 @@ __device__ __forceinline__ void consume(const TmaMaps* maps, const TmaArgs& a, u
     float acc[24];
 #pragma unroll
     for (int e = 0; e < 24; e++) acc[e] = 0.f;
-    hop_sm<2 * ROLE, true, DAG>(acc, sb + n0, v0, U0, a.ws);
-    hop_sm<2 * ROLE, false, DAG>(acc, sb + n1, v1, U1, a.ws);
-    hop_sm<2 * ROLE + 1, true, DAG>(acc, sb + n2, v2, U2, w2);
-    hop_sm<2 * ROLE + 1, false, DAG>(acc, sb + n3, v3, U3, w3);
+    hop_sm<2 * ROLE, true, DAG, TS::ROWB>(acc, sb + n0, U0, a.ws);
+    hop_sm<2 * ROLE, false, DAG, TS::ROWB>(acc, sb + n1, U1, a.ws);
+    hop_sm<2 * ROLE + 1, true, DAG, TS::ROWB>(acc, sb + n2, U2, w2);
+    hop_sm<2 * ROLE + 1, false, DAG, TS::ROWB>(acc, sb + n3, U3, w3);
     __syncwarp();
     if (lane == 0) mbar_arrive(&bars[NST + st]);  // this warp no longer reads stage st
     // exchange the halves: I keep reals [12*ROLE, 12*ROLE+12), my partner owns the other twelve
@@ -257,9 +259,10 @@ __device__ __forceinline__ void consume(const TmaMaps* maps, const TmaArgs& a, u
 #pragma unroll
       for (int e = 0; e < 12; e++) res[e] = xv[e] + a.scale * d[e];
     }
-    float4* op = reinterpret_cast<float4*>(a.out + (size_t)c * a.stride + hoff);
 #pragma unroll
     for (int v = 0; v < 3; v++) op[(size_t)v * Vh] = make_float4(res[4 * v], res[4 * v + 1], res[4 * v + 2], res[4 * v + 3]);
+    op += cstride;
+    xp += cstride;
     // refill: column c + NST goes into the stage just read, once every warp has let go of it.  The warps take turns
     // (warp c mod NW), so the wait and the issue cost each warp one column in NW.
     if (c + NST < a.nrhs && warp == c % NW) {
@@ -267,6 +270,7 @@ __device__ __forceinline__ void consume(const TmaMaps* maps, const TmaArgs& a, u
       if (lane == 0) issue_stage<TS>(stage0 + st * TS::STAGE_BYTES, maps, L, y0, z0, t0, c + NST, &bars[st]);
       __syncwarp();
     }
+   }
   }
 }
 
@@ -323,18 +327,18 @@ EncodeTiledFn encode_fn() {
   return fn;
 }
 
-// tensor maps of nrhs consecutive one-parity native fp32 spinors seen as {x: 4*Lxh floats, y, z, t, vector: 6*nrhs},
+// tensor maps of nrhs consecutive one-parity native fp32 spinors seen as {x: 4*Lxh floats, vector: 6*nrhs, y, z, t},
 // one per box shape
 template <typename TS>
 bool make_maps(TmaMaps* m, const void* in, const Lat& L, int nrhs) {
   EncodeTiledFn enc = encode_fn();
   if (!enc) return false;
-  const cuuint64_t dims[5] = {(cuuint64_t)4 * L.Lxh, (cuuint64_t)L.Ly, (cuuint64_t)L.Lz, (cuuint64_t)L.Lt, (cuuint64_t)6 * nrhs};
+  const cuuint64_t dims[5] = {(cuuint64_t)4 * L.Lxh, (cuuint64_t)6 * nrhs, (cuuint64_t)L.Ly, (cuuint64_t)L.Lz, (cuuint64_t)L.Lt};
   const cuuint64_t row = (cuuint64_t)16 * L.Lxh;
-  const cuuint64_t strides[4] = {row, row * L.Ly, row * L.Ly * L.Lz, (cuuint64_t)16 * L.Vh};
+  const cuuint64_t strides[4] = {(cuuint64_t)16 * L.Vh, row, row * L.Ly, row * L.Ly * L.Lz};
   const cuuint32_t es[5] = {1, 1, 1, 1, 1};
   const cuuint32_t X = 4 * TS::LXH;
-  const cuuint32_t boxes[4][5] = {{X, TS::TY, TS::TZ, TS::TT, 6}, {X, 1, TS::TZ, TS::TT, 6}, {X, TS::TY, 1, TS::TT, 6}, {X, TS::TY, TS::TZ, 1, 6}};
+  const cuuint32_t boxes[4][5] = {{X, 6, TS::TY, TS::TZ, TS::TT}, {X, 6, 1, TS::TZ, TS::TT}, {X, 6, TS::TY, 1, TS::TT}, {X, 6, TS::TY, TS::TZ, 1}};
   CUtensorMap* out[4] = {&m->core, &m->yface, &m->zface, &m->tface};
   for (int i = 0; i < 4; i++)
     if (enc(out[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, const_cast<void*>(in), dims, strides, boxes[i], es, CU_TENSOR_MAP_INTERLEAVE_NONE,
