@@ -665,9 +665,16 @@ int lqcd_dslash_mrhs_fused_launch(lqcd_ctx* c, void* out, const void* in, const 
   c->alg_bytes += bytes;
   const bool rec = c->prof_on && c->prof_n < c->prof_cap;
   if (rec) cudaEventRecord(c->prof_ev[2 * c->prof_n], st);
-  if (c->prec == 4) launch_mrhs_typed<float>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st, f);
+  int nsum = nblocks;  // partials per sum and column
+  if (epi >= 11 && lqcd_mrhs_tma_fused_ok(c)) {
+    // where the TMA-tiled kernel serves epilogue 3 it serves 11 and 12 too (one partial per 128-site tile)
+    nsum = lqcd_mrhs_tma_fused_blocks(c);
+    const int rc = lqcd_dslash_mrhs_tma_fused_launch(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, f->r,
+                                                     c->d_partial_mrhs, st);
+    if (rc) return rc;
+  } else if (c->prec == 4) launch_mrhs_typed<float>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st, f);
   else launch_mrhs_typed<double>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st, f);
-  partial_sum_mrhs_kernel<<<dim3(nrhs, epi >= 11 ? 3 : 1), 256, 0, st>>>(c->d_partial_mrhs, nblocks, c->d_scalars, f->out_slot);
+  partial_sum_mrhs_kernel<<<dim3(nrhs, epi >= 11 ? 3 : 1), 256, 0, st>>>(c->d_partial_mrhs, nsum, c->d_scalars, f->out_slot);
   c->launches++;
   if (rec) {
     cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], st);

@@ -58,6 +58,8 @@ struct TmaArgs {
   float scale, ws;
   size_t stride;  // reals between consecutive right-hand sides
   int zslab;      // z-tiles per slab of the sweep
+  const float* r;   // epilogue 12: y of <y, out>
+  double* partial;  // epilogues 11, 12: [3 sums][LQCD_MAX_RHS][gridDim.x] per-block partials
 };
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -132,12 +134,15 @@ __device__ __forceinline__ void hop_sm(float* acc, const unsigned char* sp, cons
 
 // The work of one consumer thread: ROLE 0 = hops +-x, +-y and the upper chiral block, ROLE 1 = hops +-z, +-t and the
 // lower one (a template parameter, so every register array is indexed statically; the branch on the role is uniform
-// over a warp).  EPI as in dslash.cu: 0 scale*d ; 1 scale*C d ; 2 C x + scale*d ; 3 x + scale*C d ; 6 x + scale*d
+// over a warp).  EPI as in dslash.cu: 0 scale*d ; 1 scale*C d ; 2 C x + scale*d ; 3 x + scale*C d ; 6 x + scale*d ;
+// 11, 12: epilogue 3 with BiCGStab's inner products per column (dslash_mrhs.cu): Re, Im <out,x>, |out|^2 | Re, Im <y,out>, |y|^2;
+// a thread's twelve products are summed in fp32, over the warp by shuffles, the warps' sums left in redw
 template <typename TS, int R, bool DAG, int EPI, int ROLE>
 __device__ __forceinline__ void consume(const TmaMaps* maps, const TmaArgs& a, unsigned char* stage0, float4* xbuf,
-                                        unsigned long long* bars, int y0, int z0, int t0) {
+                                        unsigned long long* bars, float* redw, int y0, int z0, int t0) {
   constexpr int LXH = TS::LXH, TY = TS::TY, TZ = TS::TZ, TT = TS::TT, NS = TS::NS, NW = TS::NCONS / 32, NST = TS::NST;
-  constexpr bool CLOVER = EPI == 1 || EPI == 2 || EPI == 3;
+  constexpr bool CLOVER = EPI == 1 || EPI == 2 || EPI == 3 || EPI == 11 || EPI == 12;
+  constexpr bool XIN = EPI == 2 || EPI == 3 || EPI == 6 || EPI == 11 || EPI == 12;
   const Lat& L = a.lat;
   const int Vh = L.Vh, par = a.parity;
   const int tid = threadIdx.x, sl = tid % NS, warp = tid >> 5, lane = tid & 31;
@@ -192,6 +197,7 @@ __device__ __forceinline__ void consume(const TmaMaps* maps, const TmaArgs& a, u
   // the column loop is unrolled over the ring, so the stage of a column is a compile-time constant and every
   // shared-memory address is a register of the set-up above plus an immediate
   const float4* xp = reinterpret_cast<const float4*>(a.x + hoff);
+  const float4* yp = reinterpret_cast<const float4*>(a.r + hoff);
   float4* op = reinterpret_cast<float4*>(a.out + hoff);
   const size_t cstride = a.stride / 4;  // float4 between columns
   unsigned ph = 0;
@@ -200,8 +206,15 @@ __device__ __forceinline__ void consume(const TmaMaps* maps, const TmaArgs& a, u
    for (int st = 0; st < NST; st++) {
     const int c = c0 + st;
     if (c >= a.nrhs) break;
-    float xv[12];
-    if (EPI == 2 || EPI == 3 || EPI == 6) {  // issued before the wait: the latency hides behind it
+    float xv[12], yv[EPI == 12 ? 12 : 1];
+    if (EPI == 12) {
+#pragma unroll
+      for (int v = 0; v < 3; v++) {
+        const float4 q = ld_cached(yp + (size_t)v * Vh);
+        vec_get(q, yv + 4 * v);
+      }
+    }
+    if (XIN) {  // issued before the wait: the latency hides behind it
 #pragma unroll
       for (int v = 0; v < 3; v++) {
         const float4 q = ld_cached(xp + (size_t)v * Vh);
@@ -250,7 +263,7 @@ __device__ __forceinline__ void consume(const TmaMaps* maps, const TmaArgs& a, u
       clover_block<float>(cb, xv, res);
 #pragma unroll
       for (int e = 0; e < 12; e++) res[e] += a.scale * d[e];
-    } else if (EPI == 3) {
+    } else if (EPI == 3 || EPI == 11 || EPI == 12) {
       float y[12];
       clover_block<float>(cb, d, y);
 #pragma unroll
@@ -263,6 +276,30 @@ __device__ __forceinline__ void consume(const TmaMaps* maps, const TmaArgs& a, u
     for (int v = 0; v < 3; v++) op[(size_t)v * Vh] = make_float4(res[4 * v], res[4 * v + 1], res[4 * v + 2], res[4 * v + 3]);
     op += cstride;
     xp += cstride;
+    if (EPI == 11 || EPI == 12) {
+      yp += cstride;
+      float s0 = 0.f, s1 = 0.f, s2 = 0.f;
+#pragma unroll
+      for (int e = 0; e < 12; e += 2) {
+        // <u,w> = sum conj(u) w with (u, w) = (out, x) for 11, (y, out) for 12
+        const float ur = EPI == 11 ? res[e] : yv[e], ui = EPI == 11 ? res[e + 1] : yv[e + 1];
+        const float wr = EPI == 11 ? xv[e] : res[e], wi = EPI == 11 ? xv[e + 1] : res[e + 1];
+        s0 += ur * wr + ui * wi;
+        s1 += ur * wi - ui * wr;
+        s2 += ur * ur + ui * ui;
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        s0 += __shfl_xor_sync(0xffffffffu, s0, o);
+        s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+        s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+      }
+      if (lane == 0) {
+        redw[(0 * LQCD_MAX_RHS + c) * NW + warp] = s0;
+        redw[(1 * LQCD_MAX_RHS + c) * NW + warp] = s1;
+        redw[(2 * LQCD_MAX_RHS + c) * NW + warp] = s2;
+      }
+    }
     // refill: column c + NST goes into the stage just read, once every warp has let go of it.  The warps take turns
     // (warp c mod NW), so the wait and the issue cost each warp one column in NW.
     if (c + NST < a.nrhs && warp == c % NW) {
@@ -281,6 +318,7 @@ __global__ void __launch_bounds__(TS::NCONS, TS::MINB) dslash_mrhs_tma_kernel(co
   unsigned char* stage0 = tma_smem;                                                // NST stages of the input tile
   float4* xbuf = reinterpret_cast<float4*>(tma_smem + NST * TS::STAGE_BYTES);      // exchange: [2][2 roles][3][NS]
   unsigned long long* bars = reinterpret_cast<unsigned long long*>(xbuf + 2 * 2 * 3 * NS);  // full[NST], empty[NST]
+  float* redw = reinterpret_cast<float*>(bars + 2 * NST);  // epilogues 11, 12: [3 sums][LQCD_MAX_RHS][warps]
   const Lat& L = a.lat;
   // tile of this block: y fastest, then z inside a slab, then t, then the slab
   const int nty = L.Ly / TY, ntt = L.Lt / TT;
@@ -304,8 +342,18 @@ __global__ void __launch_bounds__(TS::NCONS, TS::MINB) dslash_mrhs_tma_kernel(co
     for (int c = 0; c < NST && c < a.nrhs; c++) issue_stage<TS>(stage0 + c * TS::STAGE_BYTES, &maps, L, y0, z0, t0, c, &bars[c]);
   }
   __syncthreads();
-  if (tid < NS) consume<TS, R, DAG, EPI, 0>(&maps, a, stage0, xbuf, bars, y0, z0, t0);
-  else consume<TS, R, DAG, EPI, 1>(&maps, a, stage0, xbuf, bars, y0, z0, t0);
+  if (tid < NS) consume<TS, R, DAG, EPI, 0>(&maps, a, stage0, xbuf, bars, redw, y0, z0, t0);
+  else consume<TS, R, DAG, EPI, 1>(&maps, a, stage0, xbuf, bars, redw, y0, z0, t0);
+  if (EPI == 11 || EPI == 12) {  // the block's partial of every sum and column: the warps' sums in warp order, in fp64
+    constexpr int NW = TS::NCONS / 32;
+    __syncthreads();
+    if (tid < 3 * a.nrhs) {
+      const int sum = tid / a.nrhs, col = tid % a.nrhs;
+      double t = 0.0;
+      for (int w = 0; w < NW; w++) t += (double)redw[(sum * LQCD_MAX_RHS + col) * NW + w];
+      a.partial[((size_t)sum * LQCD_MAX_RHS + col) * gridDim.x + blockIdx.x] = t;
+    }
+  }
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -348,7 +396,7 @@ bool make_maps(TmaMaps* m, const void* in, const Lat& L, int nrhs) {
 }
 
 template <typename TS> constexpr size_t smem_bytes() {
-  return (size_t)TS::NST * TS::STAGE_BYTES + (size_t)2 * 2 * 3 * TS::NS * 16 + 2 * TS::NST * 8;
+  return (size_t)TS::NST * TS::STAGE_BYTES + (size_t)2 * 2 * 3 * TS::NS * 16 + 2 * TS::NST * 8 + 3 * LQCD_MAX_RHS * (TS::NCONS / 32) * 4;
 }
 
 template <typename TS, int R, bool DAG, int EPI>
@@ -425,6 +473,8 @@ int launch_clover(lqcd_ctx* c, TmaArgs& a, const void* in, int dagger, int epi, 
   a.zslab = (want > 0 && ntz % want == 0) ? want : ntz;
   if (epi == 1) launch_tile<TS, 1>(map, a, c->recon, dagger, c->device, st);
   else if (epi == 2) launch_tile<TS, 2>(map, a, c->recon, dagger, c->device, st);
+  else if (epi == 11) launch_tile<TS, 11>(map, a, c->recon, dagger, c->device, st);
+  else if (epi == 12) launch_tile<TS, 12>(map, a, c->recon, dagger, c->device, st);
   else launch_tile<TS, 3>(map, a, c->recon, dagger, c->device, st);
   return LQCD_OK;
 }
@@ -444,13 +494,24 @@ bool lqcd_mrhs_tma_ok(const lqcd_ctx* c, int epi) {
   return c->mrhs_tma == 2 && tile_divides<Tile8>(c->lat);
 }
 
-int lqcd_dslash_mrhs_tma_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
-                                int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st) {
+// epilogues 11 and 12 (BiCGStab's inner products fused into epilogue 3) where this kernel serves epilogue 3 with the
+// 128-site tile; *nblocks = per-block partials written per sum and column ([3][LQCD_MAX_RHS][*nblocks] doubles)
+bool lqcd_mrhs_tma_fused_ok(const lqcd_ctx* c) {
+  return lqcd_mrhs_tma_ok(c, 3) && tile_divides<Tile16>(c->lat) && tile_divides<Tile16C>(c->lat);
+}
+int lqcd_mrhs_tma_fused_blocks(const lqcd_ctx* c) {
+  return (c->lat.Ly / Tile16C::TY) * (c->lat.Lz / Tile16C::TZ) * (c->lat.Lt / Tile16C::TT);
+}
+
+static int tma_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x, int parity,
+                      double scale, int dagger, int epi, int nrhs, const void* r, double* partial, cudaStream_t st) {
   TmaArgs a;
   a.out = (float*)out;
   a.gauge = (const float*)gauge;
   a.cl = (const float*)cl;
   a.x = (const float*)x;
+  a.r = (const float*)r;
+  a.partial = partial;
   a.lat = c->lat;
   a.parity = parity;
   a.nrhs = nrhs;
@@ -463,4 +524,14 @@ int lqcd_dslash_mrhs_tma_launch(lqcd_ctx* c, void* out, const void* in, const vo
     return launch_clover<Tile16C>(c, a, in, dagger, epi, nrhs, st);
   }
   return launch_any<Tile8>(c, a, in, dagger, epi, nrhs, st);
+}
+
+int lqcd_dslash_mrhs_tma_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
+                                int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st) {
+  return tma_launch(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, nullptr, nullptr, st);
+}
+int lqcd_dslash_mrhs_tma_fused_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
+                                      int parity, double scale, int dagger, int epi, int nrhs, const void* r, double* partial,
+                                      cudaStream_t st) {
+  return tma_launch(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, r, partial, st);
 }

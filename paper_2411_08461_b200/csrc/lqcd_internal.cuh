@@ -277,6 +277,11 @@ bool lqcd_mrhs_fuse_ok(const lqcd_ctx* c);
 int lqcd_dslash_mrhs_fused_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
                                   int parity, double scale, int dagger, int epi, int nrhs, const DslashFuse* f, cudaStream_t st);
 bool lqcd_mrhs_tma_ok(const lqcd_ctx* c, int epi);
+bool lqcd_mrhs_tma_fused_ok(const lqcd_ctx* c);
+int lqcd_mrhs_tma_fused_blocks(const lqcd_ctx* c);
+int lqcd_dslash_mrhs_tma_fused_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
+                                      int parity, double scale, int dagger, int epi, int nrhs, const void* r, double* partial,
+                                      cudaStream_t st);
 int lqcd_dslash_mrhs_tma_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
                                 int parity, double scale, int dagger, int epi, int nrhs, cudaStream_t st);
 // 16-bit-storage context (half.cu)

@@ -474,10 +474,9 @@ static int solve_bicgstab(lqcd_ctx* c, const Work& w, const void* gauge, const v
     }
     // batch of columns, left-symmetric form: <r0,v> and <t,s>, |t|^2 come out of the epilogue that produces v and t
     // (multi-RHS epilogues 12 and 11), two vector passes fewer each
-    // (measured: 16^3x32 fp32 6.09 -> 5.60 ms, 32^3x64 fp64 195.8 -> 186.0 ms per 12-column solve; where the TMA-tiled kernel
-    // serves epilogue 3 it is 10 % faster than the register kernel that carries 11 and 12, and the fusion loses: 127.6 -> 129.1 ms)
-    const bool fuse_dots = n > 1 && matpc == LQCD_MATPC_SYMMETRIC && lqcd_mrhs_fuse_ok(c) &&
-                           (c->mrhs_fuse_dots == 1 || (c->mrhs_fuse_dots < 0 && !lqcd_mrhs_tma_ok(c, 3)));
+    // (measured: 16^3x32 fp32 6.09 -> 5.60 ms, 32^3x64 fp64 195.8 -> 186.0 ms per 12-column solve); the fused launch runs on
+    // the TMA-tiled kernel where that serves epilogue 3, on the register kernel elsewhere.  LQCD_MRHS_FUSE_DOTS=0: off.
+    const bool fuse_dots = n > 1 && matpc == LQCD_MATPC_SYMMETRIC && lqcd_mrhs_fuse_ok(c) && c->mrhs_fuse_dots != 0;
     const size_t half = lqcd_clover_bytes(c) / 2;
     const double k2 = -kappa * kappa;
     if (fuse_dots) {

@@ -214,6 +214,33 @@ def test_tma_mrhs_kernel_matches_oracle(dims, zslab, recon, monkeypatch):
                     assert rel_err(gots[r], want[0]) < TOL[4], (nrhs, matpc, dagger, r)
 
 
+@pytest.mark.parametrize("nrhs", [12, 5])
+def test_batched_bicgstab_inner_products_in_the_epilogues(nrhs, monkeypatch):
+    """Batched BiCGStab on the left-symmetric form takes <r0,v> and <t,s>, |t|^2 from multi-RHS epilogues 12 and 11: in
+    the TMA-tiled kernel where that serves epilogue 3 (fp32, 12-real links, x-rows of 16), in the register kernel
+    (LQCD_MRHS_TMA=0), or from separate BLAS-1 passes (LQCD_MRHS_FUSE_DOTS=0).  All three must meet reading A17 on every
+    column and agree on the iteration counts to +-1 (the sums differ in rounding order only)."""
+    dims, kappa, csw = (32, 4, 6, 8), 0.124, 1.2
+    bs = [synth.round_fp32(synth.source(dims, "gaussian", 300 + r)) for r in range(nrhs)]
+    iters = {}
+    for name, env in (("tma", {}), ("register", {"LQCD_MRHS_TMA": "0"}), ("blas", {"LQCD_MRHS_FUSE_DOTS": "0"})):
+        for k in ("LQCD_MRHS_TMA", "LQCD_MRHS_FUSE_DOTS"):
+            monkeypatch.delenv(k, raising=False)
+        for k, v in env.items():
+            monkeypatch.setenv(k, v)
+        s = Setup(dims, 0.5, 2, kappa, csw, 4, 12, -1)
+        x, res, rc = s.ctx.invert_multi(s.ctx.to_device(np.stack(bs)), s.gauge, s.A, s.Ai, kappa, tol=1e-6, maxiter=500,
+                                        solver="bicgstab", matpc=1)
+        assert rc == 0, name
+        xs = x.cpu().numpy().astype(np.complex128)
+        for r, b in enumerate(bs):
+            assert res[r].status == 0 and s.orc.true_residual(b, xs[r]) < 1e-6, (name, r, res[r].as_dict())
+        iters[name] = [r.iterations for r in res]
+        s.ctx.close()
+    for name in ("register", "blas"):
+        assert max(abs(a - b) for a, b in zip(iters["tma"], iters[name])) <= 1, iters
+
+
 def test_propagator_sharded_single_rank_equals_propagator():
     """Without a process group the column-sharded propagator is the batched one."""
     s, c = from_cfg(2, 8, 18)
