@@ -71,7 +71,9 @@ typedef struct lqcd_result {
  *   LQCD_MRHS_FUSE_DOTS=0|1  batched BiCGStab dot products in the multi-RHS epilogues: never | always (default: where
  *                            the register kernel runs the epilogue anyway);
  *   LQCD_GRAPHS=0            no CUDA-graph replay of Krylov iteration blocks on small lattices;
- *   LQCD_CLOVER_ONEPASS=1    one-kernel clover build (no scratch) instead of the three-pass one. */
+ *   LQCD_CLOVER_ONEPASS=1    one-kernel clover build (no scratch) instead of the three-pass one;
+ *   LQCD_MIXED_LAST_MARGIN=f mixed solves close (x_o, true residual) without a last fp64 Schur residual when the inner
+ *                            recurrence predicts |r|^2 <= f * (tol |b|)^2 (default 0.9; 0 = never; a wrong guess reopens). */
 int lqcd_create(lqcd_ctx** ctx, const int dims[4], int prec, int recon, int t_boundary, int device);
 int lqcd_destroy(lqcd_ctx* ctx);
 const char* lqcd_strerror(int code);

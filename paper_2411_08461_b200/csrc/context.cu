@@ -86,6 +86,8 @@ int lqcd_create(lqcd_ctx** out, const int dims[4], int prec, int recon, int t_bo
     c->mrhs_fuse_dots = fd ? (fd[0] == '1') : -1;  // -1: where the register kernel runs the plain epilogues anyway
     const char* gr = getenv("LQCD_GRAPHS");
     c->graphs_on = (gr && gr[0] == '0') ? 0 : 1;
+    const char* ml = getenv("LQCD_MIXED_LAST_MARGIN");
+    c->mixed_last_margin = ml ? atof(ml) : 0.9;
     const char* co = getenv("LQCD_CLOVER_ONEPASS");
     c->clover_onepass = (co && co[0] == '1') ? 1 : 0;
     const char* z = getenv("LQCD_MRHS_ZSLAB");

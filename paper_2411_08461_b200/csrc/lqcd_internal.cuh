@@ -57,6 +57,7 @@ struct lqcd_ctx {
   double* d_partial;
   double* d_partial_mrhs;  // [column][32-site warp]: partials of the multi-RHS fused epilogues (allocated on first use)
   double* d_clover_scratch;  // clover build in three passes: two fields of 6 planes x 9 doubles per site (allocated on first use)
+  double mixed_last_margin;   // mixed solves: an outer step is taken for the last when the inner residual estimate is below this x the bar
   int clover_onepass;         // LQCD_CLOVER_ONEPASS=1: the one-kernel build (also the fallback when the scratch cannot be allocated)
   double* d_scalars;
   unsigned int* d_ticket;

@@ -162,6 +162,36 @@ def test_config2_mixed_precision_reaches_fp64_tolerance(solver, recon_lo):
         s.ctx.invert_mixed(s.ctx, s.ctx.to_device(b), s.gauge, s.A, s.Ai, s.gauge, s.A, s.Ai, s.kappa)
 
 
+@pytest.mark.parametrize("margin", ["1e30", "0", None])
+@pytest.mark.parametrize("solver,matpc", [("cgne", 2), ("bicgstab", 1), ("cgne", 0)])
+def test_mixed_last_outer_step_guess(solver, matpc, margin, monkeypatch):
+    """A mixed solve closes (x_o, true residual) as soon as the inner recurrences say the bar is met, without an fp64
+    Schur residual of its own; a wrong guess must reopen the iteration.  LQCD_MIXED_LAST_MARGIN=1e30 makes every outer
+    step a guess (so the early ones are wrong), 0 never guesses, unset is the default: the same bar is met each time,
+    single and batched (the batch freezes columns as they finish)."""
+    if margin is None:
+        monkeypatch.delenv("LQCD_MIXED_LAST_MARGIN", raising=False)
+    else:
+        monkeypatch.setenv("LQCD_MIXED_LAST_MARGIN", margin)
+    s, c = from_cfg(2, 8, 18)
+    lo = lq().Context(c["dims"], 4, 12, -1)
+    g_lo = lo.gauge_pack(lo.to_device(s.U))
+    A_lo, Ai_lo = lo.clover_build(g_lo, c["csw"], c["kappa"])
+    bs = [synth.source(c["dims"], "z2", c["src_seed"]), synth.source(c["dims"], "point", spin=2, colour=1),
+          synth.source(c["dims"], "gaussian", 7)]
+    x, res = s.ctx.invert_mixed(lo, s.ctx.to_device(bs[0]), s.gauge, s.A, s.Ai, g_lo, A_lo, Ai_lo, s.kappa,
+                                tol=1e-10, inner_tol=1e-3, maxiter=2000, solver=solver, matpc=matpc)
+    true = s.orc.true_residual(bs[0], x.cpu().numpy())
+    assert res.status == 0 and true < 1e-10 and abs(true - res.true_resid) < 5e-11, (true, res.as_dict())
+    xm, resm, rc = s.ctx.invert_multi_mixed(lo, s.ctx.to_device(np.stack(bs)), s.gauge, s.A, s.Ai, g_lo, A_lo, Ai_lo,
+                                            s.kappa, tol=1e-10, inner_tol=1e-3, maxiter=2000, solver=solver, matpc=matpc)
+    assert rc == 0
+    xs = xm.cpu().numpy()
+    for r, b in enumerate(bs):
+        true = s.orc.true_residual(b, xs[r])
+        assert resm[r].status == 0 and true < 1e-10 and abs(true - resm[r].true_resid) < 5e-11, (r, true, resm[r].as_dict())
+
+
 @pytest.mark.parametrize("matpc", [0, 1, 2])
 def test_config2_cgne_fp64_recon12(matpc):
     """fp64 with reconstruct-12 links: the kernel variant that stages its links through shared memory with cp.async
