@@ -122,6 +122,19 @@ int lqcd_clover_pack(lqcd_ctx* ctx, void* clover_native, const void* clover_publ
 int lqcd_clover_build(lqcd_ctx* ctx, void* clover, void* clover_inv, const void* gauge, double csw,
                       double kappa, void* stream);
 
+/* lqcd_clover_build for callers that cannot tolerate an allocation inside the call (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): same arguments, same result (the same three kernels), but the scratch
+ * between the passes is a fixed device array inside the library instead of a cudaMalloc on the context's first build.
+ * The call makes no cudaMalloc / cudaFree / allocating library call.
+ * Limit: lattices of at most lqcd_clover_noalloc_max_sites() = 32768 sites (e.g. 8^3x64, 16x16x8x16); larger ones return
+ * LQCD_ERR_WORKSPACE with the two numbers in lqcd_last_error.  Cost: 27 MiB of device memory on every GPU that loads the
+ * library, until the process exits.  The array is shared by all contexts and calls on a GPU and keeps the last call's
+ * contents (nothing in it needs clearing: every entry read was written by the same call); calls that overlap on the GPU
+ * race on it, so serialise them.  The context's device must be the current device.  Synchronises like lqcd_clover_build. */
+int lqcd_clover_build_noalloc(lqcd_ctx* ctx, void* clover, void* clover_inv, const void* gauge, double csw,
+                              double kappa, void* stream);
+long lqcd_clover_noalloc_max_sites(void);
+
 /* Anisotropic operator of PAPER.md:218-221, Eq. 5, in kappa normalisation:
  *     M = 1 - kappa [ D_t + (nu/xi_0) sum_i D_i ]
  *           - kappa [ c_SW^t sum_i sigma_i4 F_i4 + (c_SW^r/xi_0) sum_{i<j} sigma_ij F_ij ],   1/kappa = 2(m0 + 1 + 3 nu/xi_0)

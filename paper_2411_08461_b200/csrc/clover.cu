@@ -653,3 +653,82 @@ extern "C" int lqcd_clover_build(lqcd_ctx* c, void* clover, void* clover_inv, co
                                  double kappa, void* stream) {
   return lqcd_clover_build_aniso(c, clover, clover_inv, gauge, csw, csw, kappa, stream);
 }
+
+// ---------------------------------------------------------------------------------------------------------------
+// lqcd_clover_build_noalloc: the three-pass build for callers that cannot tolerate an allocation inside the call (code
+// under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  lqcd_clover_build allocates its
+// scratch (two fields of 6 planes x 9 doubles per site) with cudaMalloc on the first build of a context; here the
+// scratch is a file-scope device array of fixed size, so the entry point calls no cudaMalloc, cudaFree or allocating
+// library routine -- and serves lattices of at most LQCD_CLOVER_NOALLOC_MAX_SITES sites.
+//   Size: 2 x 54 x 8 B x 32768 sites = 27 MiB, held by every GPU that loads the library until the process exits.
+//   Sharing: ONE array per GPU for all contexts and calls.  It keeps the last call's contents; nothing in it has to
+//   start at zero (pass 1 writes every entry of X1 that pass 2 reads, pass 2 every entry of X2 that pass 3 reads), so
+//   nothing is cleared.  Two calls that overlap on the GPU (different streams, or different contexts on one device)
+//   race on it: callers serialise them.
+//   In host code the array's name is a host-side stand-in, not a device address; the device address is taken once per
+//   device with cudaGetSymbolAddress while that device is current, and that pointer is what the kernels get.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr long LQCD_CLOVER_NOALLOC_MAX_SITES = 32768;
+static __device__ __align__(256) double clover_noalloc_scratch[2 * 54 * LQCD_CLOVER_NOALLOC_MAX_SITES];
+static double* clover_noalloc_ptr[LQCD_MAX_DEVICES] = {};  // device address of the array, per device ordinal
+
+extern "C" long lqcd_clover_noalloc_max_sites(void) { return LQCD_CLOVER_NOALLOC_MAX_SITES; }
+
+template <typename T, int R>
+static void clover_build_launch_static(lqcd_ctx* c, double* scratch, void* clover, void* clover_inv, const void* gauge,
+                                       double kc, double kt, cudaStream_t st) {
+  const int grid = 2 * ((c->lat.Vh + CB_SITES - 1) / CB_SITES);
+  const dim3 block(CB_SITES, 6);
+  double* X1 = scratch;
+  double* X2 = X1 + 54 * (size_t)2 * c->lat.Vh;
+  clover_plaquette_kernel<T, R><<<grid, block, 0, st>>>(X1, (const T*)gauge, c->lat);
+  clover_transport_kernel<T, R><<<grid, block, 0, st>>>(X2, X1, (const T*)gauge, c->lat);
+  clover_finish_kernel<T, R><<<2 * ((c->lat.Vh + CBF_SITES - 1) / CBF_SITES), dim3(CBF_SITES, 2), 0, st>>>(
+      (T*)clover, (T*)clover_inv, X2, (const T*)gauge, c->lat, kc, kt, c->d_flag);
+  c->launches += 2;  // LQCD_LAUNCH_CHECK counts the third
+}
+
+extern "C" int lqcd_clover_build_noalloc(lqcd_ctx* c, void* clover, void* clover_inv, const void* gauge, double csw,
+                                         double kappa, void* stream) {
+  if (!c || !clover || !gauge) return LQCD_ERR_INVALID_ARG;
+  if (c->half) return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "clover_build_noalloc: not available in a 16-bit context");
+  if (!lqcd_aligned16(clover) || !lqcd_aligned16(clover_inv) || !lqcd_aligned16(gauge))
+    return lqcd_set_error(c, LQCD_ERR_ALIGN, "clover_build_noalloc: alignment");
+  const long sites = 2L * c->lat.Vh;
+  if (sites > LQCD_CLOVER_NOALLOC_MAX_SITES)
+    return lqcd_set_error(c, LQCD_ERR_WORKSPACE,
+                          "clover_build_noalloc: lattice has %ld sites, the static scratch holds at most %ld (use lqcd_clover_build)",
+                          sites, LQCD_CLOVER_NOALLOC_MAX_SITES);
+  // set-up, once per device, with that device current
+  if (!clover_noalloc_ptr[c->device]) {
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess || cur != c->device)
+      return lqcd_set_error(c, LQCD_ERR_INVALID_ARG, "clover_build_noalloc: device %d of the context is not the current device (%d)",
+                            c->device, cur);
+    double* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress((void**)&p, clover_noalloc_scratch);
+    if (e != cudaSuccess || !p) {
+      cudaGetLastError();
+      return lqcd_set_error(c, LQCD_ERR_CUDA, "clover_build_noalloc: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+    }
+    clover_noalloc_ptr[c->device] = p;
+  }
+  double* scratch = clover_noalloc_ptr[c->device];
+  cudaStream_t st = as_stream(stream);
+  const double kc = kappa * csw;
+  cudaMemsetAsync(c->d_flag, 0, sizeof(int), st);
+  c->alg_bytes += (double)lqcd_gauge_bytes(c) + (clover_inv ? 2.0 : 1.0) * (double)lqcd_clover_bytes(c);
+  if (c->prec == 4 && c->recon == 18)
+    clover_build_launch_static<float, 18>(c, scratch, clover, clover_inv, gauge, kc, kc, st);
+  else if (c->prec == 4)
+    clover_build_launch_static<float, 12>(c, scratch, clover, clover_inv, gauge, kc, kc, st);
+  else if (c->recon == 18)
+    clover_build_launch_static<double, 18>(c, scratch, clover, clover_inv, gauge, kc, kc, st);
+  else
+    clover_build_launch_static<double, 12>(c, scratch, clover, clover_inv, gauge, kc, kc, st);
+  LQCD_LAUNCH_CHECK(c, "clover_build_noalloc");
+  cudaMemcpyAsync(c->h_flag, c->d_flag, sizeof(int), cudaMemcpyDeviceToHost, st);
+  if (cudaStreamSynchronize(st) != cudaSuccess) return lqcd_check_cuda(c, "clover_build_noalloc sync");
+  if (c->h_flag[0]) return lqcd_set_error(c, LQCD_ERR_SINGULAR_CLOVER, "clover_build_noalloc: singular 6x6 block");
+  return LQCD_OK;
+}

@@ -31,6 +31,7 @@ SYMBOLS = [
     "lqcd_algorithmic_bytes", "lqcd_profile_enable", "lqcd_profile_read", "lqcd_gauge_pack_host",
     "lqcd_gauge_bytes", "lqcd_spinor_bytes", "lqcd_clover_bytes", "lqcd_invert_workspace_bytes",
     "lqcd_gauge_pack", "lqcd_spinor_pack", "lqcd_spinor_unpack", "lqcd_clover_unpack",
+    "lqcd_clover_build_noalloc", "lqcd_clover_noalloc_max_sites",
     "lqcd_clover_build", "lqcd_clover_apply", "lqcd_dslash", "lqcd_mpc_apply", "lqcd_mat_apply",
     "lqcd_invert", "lqcd_host_scratch_bytes", "lqcd_dslash_host", "lqcd_invert_host",
     "lqcd_blas_axpy_norm", "lqcd_blas_xpay", "lqcd_blas_cdot", "lqcd_blas_caxpbypz",
@@ -82,6 +83,9 @@ def load():
     for f in ("lqcd_gauge_pack", "lqcd_spinor_pack", "lqcd_spinor_unpack", "lqcd_clover_unpack", "lqcd_clover_pack"):
         getattr(L, f).argtypes = [vp, vp, vp, vp]
     L.lqcd_clover_build.argtypes = [vp, vp, vp, vp, cd, cd, vp]
+    L.lqcd_clover_build_noalloc.argtypes = [vp, vp, vp, vp, cd, cd, vp]
+    L.lqcd_clover_noalloc_max_sites.argtypes = []
+    L.lqcd_clover_noalloc_max_sites.restype = ctypes.c_long
     ip = ctypes.POINTER(ci)
     dp = ctypes.POINTER(cd)
     L.lqcd_momentum_phase.argtypes = [vp, vp, ip, vp]
@@ -312,6 +316,18 @@ class Context:
         Ai = self.empty(self.clover_bytes) if want_inverse else None
         self._check(self.lib.lqcd_clover_build(self.h, _p(A), _p(Ai), _p(gauge), csw, kappa, _stream()))
         return A, Ai
+
+    def clover_build_noalloc(self, gauge, csw, kappa, out=None, out_inv=None):
+        """lqcd_clover_build_noalloc: the build with the library's static scratch (at most clover_noalloc_max_sites()
+        sites).  `out`, `out_inv`: native clover buffers of the caller (allocated here if None -- by torch, not by the
+        library call)."""
+        A = self.empty(self.clover_bytes) if out is None else out
+        Ai = self.empty(self.clover_bytes) if out_inv is None else out_inv
+        self._check(self.lib.lqcd_clover_build_noalloc(self.h, _p(A), _p(Ai), _p(gauge), csw, kappa, _stream()))
+        return A, Ai
+
+    def clover_noalloc_max_sites(self):
+        return int(self.lib.lqcd_clover_noalloc_max_sites())
 
     def clover_to_half(self, clover_fp32_native):
         """self: 16-bit context; clover_fp32_native: A or A^-1 of an fp32 context of the same lattice."""
