@@ -723,6 +723,7 @@ static int solve_mixed(lqcd_ctx* c, const Work& w, const void* gauge, const void
         for (int j = 0; j < n; j++)
           if (live[j]) {
             rr[j] *= ic.rr[j];  // the inner recurrence's |r|^2 / |rhs|^2 at exit
+            if (true_rr[j] < rr[j]) rr[j] = true_rr[j];  // the estimate never reports worse than what was measured
             live[j] = false;
           }
         nlive = 0;
