@@ -425,7 +425,10 @@ void launch_tile(const TmaMaps& map, const TmaArgs& a, int recon, int dagger, in
 // Tile shapes (sweep at 32^3x64, 12 columns, profiles/r02_mrhs_README.md).  Without a clover block a thread fits 168
 // registers, so three 64-site blocks share an SM (12 warps; 2 stages each): 707 us against 812 us for one 128-site
 // block (8 warps).  With the clover block in registers (210-216) only 8 warps fit; one 128-site block, 3 stages.
-typedef RowTile<16, 2, 2, 1, 2, 3> Tile16;   // epilogues 0, 6: 20 staged rows per 4 output rows
+#ifndef TMA_N_TILE
+#define TMA_N_TILE 16, 2, 2, 1, 2, 3
+#endif
+typedef RowTile<TMA_N_TILE> Tile16;   // epilogues 0, 6: 20 staged rows per 4 output rows
 #ifndef TMA_C_TILE
 #define TMA_C_TILE 16, 2, 2, 2, 3, 1
 #endif
