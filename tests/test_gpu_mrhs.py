@@ -241,6 +241,28 @@ def test_batched_bicgstab_inner_products_in_the_epilogues(nrhs, monkeypatch):
         assert max(abs(a - b) for a, b in zip(iters["tma"], iters[name])) <= 1, iters
 
 
+@pytest.mark.parametrize("solver,matpc", [("bicgstab", 1), ("cgne", 2)])
+@pytest.mark.parametrize("recon", [12, 18])
+def test_batched_solves_are_bitwise_reproducible(solver, matpc, recon):
+    """Every reduction of the batched path is summed in a fixed order (per-warp shuffles, per-block partials, one block
+    per column adding them in block order), so two runs of the same solve give the same bits and the same iteration
+    counts -- in the TMA-tiled kernels (x-rows of 16) as in the register kernels.  A race in the shared-memory stages, the
+    half-sum exchange or the partial buffers would show up here as a difference."""
+    dims = (32, 8, 4, 6)
+    s = Setup(dims, 0.5, 11, 0.124, 1.2, 4, recon, -1)
+    bs = np.stack([synth.round_fp32(synth.source(dims, "gaussian", 400 + r)) for r in range(12)])
+    B = s.ctx.to_device(bs)
+    runs = []
+    for _ in range(3):
+        x, res, rc = s.ctx.invert_multi(B, s.gauge, s.A, s.Ai, s.kappa, tol=1e-6, maxiter=500, solver=solver, matpc=matpc)
+        assert rc == 0
+        runs.append((x.clone(), [r.iterations for r in res], [r.true_resid for r in res]))
+    for x, its, tr in runs[1:]:
+        assert its == runs[0][1] and tr == runs[0][2]
+        assert torch.equal(x, runs[0][0])
+    s.ctx.close()
+
+
 def test_propagator_sharded_single_rank_equals_propagator():
     """Without a process group the column-sharded propagator is the batched one."""
     s, c = from_cfg(2, 8, 18)
