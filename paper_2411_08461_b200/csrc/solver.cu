@@ -814,11 +814,8 @@ static int invert_native_body(lqcd_ctx* c, Work& w, const void* gauge, const voi
   // a5: bhat = b_e + kappa D_eo A_oo^-1 b_o   (sym: bhat_s = A_ee^-1 bhat)
   char* bh = w.v[0];
   if ((rc = lqcd_clover_apply_launch(c, w.v[5], b_o, Ai_o, n, st))) return rc;
-  if ((rc = lqcd_dslash_launch(c, bh, w.v[5], gauge, nullptr, nullptr, 0, kappa, 0, 0, n, st))) return rc;
-  {
-    void* v[2] = {b_e, bh};
-    if ((rc = BLAS_CALL(c, OpXpay, op.a = 1.0, v, nullptr, n, 0, st))) return rc;
-  }
+  // the sum rides on the hop (epilogue 6: x + scale * d), one vector pass less
+  if ((rc = lqcd_dslash_launch(c, bh, w.v[5], gauge, nullptr, b_e, 0, kappa, 0, 6, n, st))) return rc;
   if (matpc == LQCD_MATPC_SYMMETRIC)
     if ((rc = lqcd_clover_apply_launch(c, bh, bh, Ai_e, n, st))) return rc;
   // closing steps for n columns given by their own pointers (all columns of the batch, or one column of it):
@@ -828,11 +825,7 @@ static int invert_native_body(lqcd_ctx* c, Work& w, const void* gauge, const voi
     int e;
     if (matpc == LQCD_MATPC_SYMMETRIC_RIGHT)     // the Krylov unknown was y = A_ee x_e
       if ((e = lqcd_clover_apply_launch(c, xe, xe, Ai_e, m, st))) return e;
-    if ((e = lqcd_dslash_launch(c, t5, xe, gauge, nullptr, nullptr, 1, kappa, 0, 0, m, st))) return e;
-    {
-      void* v[2] = {bo, t5};
-      if ((e = BLAS_CALL(c, OpXpay, op.a = 1.0, v, nullptr, m, 0, st))) return e;
-    }
+    if ((e = lqcd_dslash_launch(c, t5, xe, gauge, nullptr, bo, 1, kappa, 0, 6, m, st))) return e;  // b_o + kappa D_oe x_e
     if ((e = lqcd_clover_apply_launch(c, xo, t5, Ai_o, m, st))) return e;
     if ((e = lqcd_dslash_launch(c, r1, xo, gauge, A, xe, 0, -kappa, 0, 2, m, st))) return e;
     if ((e = lqcd_dslash_launch(c, r2, xe, gauge, off(A, half), xo, 1, -kappa, 0, 2, m, st))) return e;
