@@ -737,10 +737,8 @@ static int solve_mixed(lqcd_ctx* c, const Work& w, const void* gauge, const void
     for (int j = 0; j < n; j++) res[j].dslash_count += 2;
     {
       void* v[2] = {bh, mx};
-      if ((rc = BLAS_CALL(c, OpXpay, op.a = -1.0, v, nullptr, n, 0, st))) return rc;  // mx = bhat - Mhat x
-      void* v2[1] = {mx};
       int o[4] = {S_RES, 0, 0, 0};
-      if ((rc = BLAS_CALL(c, OpNorm2, (void)op, v2, o, n, 0, st))) return rc;
+      if ((rc = BLAS_CALL(c, OpXpayNorm, op.a = -1.0, v, o, n, 0, st))) return rc;  // mx = bhat - Mhat x and its norm, one pass
       if ((rc = read_scalars(c, n, st))) return rc;
     }
     char* sw = r; r = mx; mx = sw;
