@@ -56,7 +56,7 @@ template <typename T> struct MrhsArgs {
   int num, den, nblocks;
   int zslab;  // z-planes per slab of the sweep (0: plain order)
 };
-__host__ __device__ constexpr bool mrhs_clover(int epi) { return epi == 1 || epi == 2 || epi == 3 || epi == 9 || epi == 11 || epi == 12; }
+__host__ __device__ constexpr bool mrhs_clover(int epi) { return epi == 1 || epi == 2 || epi == 3 || epi == 9 || epi == 11 || epi == 12 || epi == 13; }
 // Block order of the sweep: 32-site blocks run x, y, then z inside a slab of `zslab` planes, then t, then the slab, so
 // that the +-t reuse window of all columns (2 x slab x nrhs columns) stays in L2 (round 1: 1.5 x the algorithmic DRAM
 // bytes with 12 columns in plain checkerboard order).  zslab = 0, or a plane that is not a whole number of blocks: identity.
@@ -291,6 +291,26 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kern
         a.partial[(1 * LQCD_MAX_RHS + col) * a.nblocks + blockIdx.x] = s1;
         a.partial[(2 * LQCD_MAX_RHS + col) * a.nblocks + blockIdx.x] = s2;
       }
+    }
+  } else if (EPI == 13) {
+    // closing step of a solve: |y - (C x + scale * d)|^2 per column with y = a.r, nothing stored (one parity of the true
+    // residual b - M x: epilogue 2 whose result goes straight into the norm)
+    T xv[NB][24], res[NB][24];
+#pragma unroll
+    for (int r = 0; r < NB; r++) load_spinor<T>(a.x + first + r * stride, Vh, idx, xv[r]);
+    clover_mul_mrhs<T, NB>(cl_sm, xv, res);
+#pragma unroll
+    for (int r = 0; r < NB; r++) {
+      T yv[24];
+      load_spinor<T>(a.r + first + r * stride, Vh, idx, yv);
+      double local = 0;
+#pragma unroll
+      for (int e = 0; e < 24; e++) {
+        const double dlt = (double)yv[e] - ((double)res[r][e] + (double)a.scale * (double)acc[r][e]);
+        local += dlt * dlt;
+      }
+      local = warp_sum(local);
+      if (threadIdx.x == 0) a.partial[(size_t)(g * NB + r) * a.nblocks + blockIdx.x] = local;
     }
   } else if (EPI == 10) {  // q = x + scale * d not stored ; r -= (s[num]/s[den]) q ; |r|^2 per column
 #pragma unroll
@@ -564,6 +584,7 @@ static void launch_mrhs_epi(MrhsArgs<T> a, int epi, int nrhs, cudaStream_t st) {
     cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 10, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 11, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 12, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 13, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   }
   configured = true;
   switch (epi) {
@@ -575,6 +596,7 @@ static void launch_mrhs_epi(MrhsArgs<T> a, int epi, int nrhs, cudaStream_t st) {
     case 10: dslash_mrhs_kernel<T, R, DAG, 10, NB><<<grid, block, smem, st>>>(a); break;
     case 11: dslash_mrhs_kernel<T, R, DAG, 11, NB><<<grid, block, smem, st>>>(a); break;
     case 12: dslash_mrhs_kernel<T, R, DAG, 12, NB><<<grid, block, smem, st>>>(a); break;
+    case 13: dslash_mrhs_kernel<T, R, DAG, 13, NB><<<grid, block, smem, st>>>(a); break;
     default: dslash_mrhs_kernel<T, R, DAG, 6, NB><<<grid, block, smem, st>>>(a); break;
   }
 }
@@ -659,14 +681,14 @@ int lqcd_dslash_mrhs_fused_launch(lqcd_ctx* c, void* out, const void* in, const 
     if (cudaMalloc(&c->d_partial_mrhs, sizeof(double) * 3 * LQCD_MAX_RHS * nblocks) != cudaSuccess) return lqcd_check_cuda(c, "mrhs partials");
   }
   // epi 9: links, clover, in, x, out, out2 per column ; epi 10: links, in, x, r read and written
-  // epi 11: as epi 3 (links, clover, in, x, out) ; epi 12: + y
+  // epi 11: as epi 3 (links, clover, in, x, out) ; epi 12: + y ; epi 13: links, clover, in, x, y (nothing written)
   const double bytes = (double)c->lat.Vh * c->prec *
-                       (8.0 * c->recon + (epi == 10 ? 0.0 : 72.0) + nrhs * (epi == 11 ? 72.0 : 96.0));
+                       (8.0 * c->recon + (epi == 10 ? 0.0 : 72.0) + nrhs * (epi == 11 || epi == 13 ? 72.0 : 96.0));
   c->alg_bytes += bytes;
   const bool rec = c->prof_on && c->prof_n < c->prof_cap;
   if (rec) cudaEventRecord(c->prof_ev[2 * c->prof_n], st);
   int nsum = nblocks;  // partials per sum and column
-  if (epi >= 11 && lqcd_mrhs_tma_fused_ok(c)) {
+  if ((epi == 11 || epi == 12) && lqcd_mrhs_tma_fused_ok(c)) {
     // where the TMA-tiled kernel serves epilogue 3 it serves 11 and 12 too (one partial per 128-site tile)
     nsum = lqcd_mrhs_tma_fused_blocks(c);
     const int rc = lqcd_dslash_mrhs_tma_fused_launch(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, f->r,
@@ -674,7 +696,7 @@ int lqcd_dslash_mrhs_fused_launch(lqcd_ctx* c, void* out, const void* in, const 
     if (rc) return rc;
   } else if (c->prec == 4) launch_mrhs_typed<float>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st, f);
   else launch_mrhs_typed<double>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, nrhs, st, f);
-  partial_sum_mrhs_kernel<<<dim3(nrhs, epi >= 11 ? 3 : 1), 256, 0, st>>>(c->d_partial_mrhs, nsum, c->d_scalars, f->out_slot);
+  partial_sum_mrhs_kernel<<<dim3(nrhs, epi == 11 || epi == 12 ? 3 : 1), 256, 0, st>>>(c->d_partial_mrhs, nsum, c->d_scalars, f->out_slot);
   c->launches++;
   if (rec) {
     cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], st);

@@ -825,6 +825,13 @@ static int invert_native_body(lqcd_ctx* c, Work& w, const void* gauge, const voi
       if ((e = lqcd_clover_apply_launch(c, xe, xe, Ai_e, m, st))) return e;
     if ((e = lqcd_dslash_launch(c, t5, xe, gauge, nullptr, bo, 1, kappa, 0, 6, m, st))) return e;  // b_o + kappa D_oe x_e
     if ((e = lqcd_clover_apply_launch(c, xo, t5, Ai_o, m, st))) return e;
+    if (m > 1 && lqcd_mrhs_fuse_ok(c)) {
+      // batch: each parity of A x - kappa D x goes straight into |b - (...)|^2 (multi-RHS epilogue 13), nothing is stored
+      DslashFuse fe = {be, S_TRUE, 0, 0, nullptr}, fo = {bo, S_TRUE + 1, 0, 0, nullptr};
+      if ((e = lqcd_dslash_mrhs_fused_launch(c, nullptr, xo, gauge, A, xe, 0, -kappa, 0, 13, m, &fe, st))) return e;
+      if ((e = lqcd_dslash_mrhs_fused_launch(c, nullptr, xe, gauge, off(A, half), xo, 1, -kappa, 0, 13, m, &fo, st))) return e;
+      return read_scalars(c, m, st);
+    }
     if ((e = lqcd_dslash_launch(c, r1, xo, gauge, A, xe, 0, -kappa, 0, 2, m, st))) return e;
     if ((e = lqcd_dslash_launch(c, r2, xe, gauge, off(A, half), xo, 1, -kappa, 0, 2, m, st))) return e;
     {
