@@ -56,7 +56,7 @@ template <typename T> struct MrhsArgs {
   int num, den, nblocks;
   int zslab;  // z-planes per slab of the sweep (0: plain order)
 };
-__host__ __device__ constexpr bool mrhs_clover(int epi) { return epi == 1 || epi == 2 || epi == 3 || epi == 9 || epi == 11 || epi == 12 || epi == 13; }
+__host__ __device__ constexpr bool mrhs_clover(int epi) { return epi == 1 || epi == 2 || epi == 3 || epi == 9 || epi == 11 || epi == 12 || epi == 13 || epi == 14; }
 // Block order of the sweep: 32-site blocks run x, y, then z inside a slab of `zslab` planes, then t, then the slab, so
 // that the +-t reuse window of all columns (2 x slab x nrhs columns) stays in L2 (round 1: 1.5 x the algorithmic DRAM
 // bytes with 12 columns in plain checkerboard order).  zslab = 0, or a plane that is not a whole number of blocks: identity.
@@ -218,6 +218,18 @@ __global__ void __launch_bounds__(MRHS_MAXT, MrhsTune<T>::MINB) dslash_mrhs_kern
       for (int e = 0; e < 24; e++) xv[e] += a.scale * acc[r][e];
       store_spinor<T>(out + r * stride, Vh, idx, xv);
     }
+  } else if (EPI == 14) {  // out = C (x + scale * d): b-hat of the left-symmetric form, x_o = A_oo^-1 (b_o + kappa D_oe x_e)
+    T res[NB][24];
+#pragma unroll
+    for (int r = 0; r < NB; r++) {
+      T xv[24];
+      load_spinor<T>(a.x + first + r * stride, Vh, idx, xv);
+#pragma unroll
+      for (int e = 0; e < 24; e++) acc[r][e] = xv[e] + a.scale * acc[r][e];
+    }
+    clover_mul_mrhs<T, NB>(cl_sm, acc, res);
+#pragma unroll
+    for (int r = 0; r < NB; r++) store_spinor<T>(out + r * stride, Vh, idx, res[r]);
   } else if (EPI == 1) {
     T res[NB][24];
     clover_mul_mrhs<T, NB>(cl_sm, acc, res);
@@ -585,6 +597,7 @@ static void launch_mrhs_epi(MrhsArgs<T> a, int epi, int nrhs, cudaStream_t st) {
     cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 11, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 12, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 13, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_mrhs_kernel<T, R, DAG, 14, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   }
   configured = true;
   switch (epi) {
@@ -597,6 +610,7 @@ static void launch_mrhs_epi(MrhsArgs<T> a, int epi, int nrhs, cudaStream_t st) {
     case 11: dslash_mrhs_kernel<T, R, DAG, 11, NB><<<grid, block, smem, st>>>(a); break;
     case 12: dslash_mrhs_kernel<T, R, DAG, 12, NB><<<grid, block, smem, st>>>(a); break;
     case 13: dslash_mrhs_kernel<T, R, DAG, 13, NB><<<grid, block, smem, st>>>(a); break;
+    case 14: dslash_mrhs_kernel<T, R, DAG, 14, NB><<<grid, block, smem, st>>>(a); break;
     default: dslash_mrhs_kernel<T, R, DAG, 6, NB><<<grid, block, smem, st>>>(a); break;
   }
 }

@@ -812,10 +812,16 @@ static int invert_native_body(lqcd_ctx* c, Work& w, const void* gauge, const voi
   // a5: bhat = b_e + kappa D_eo A_oo^-1 b_o   (sym: bhat_s = A_ee^-1 bhat)
   char* bh = w.v[0];
   if ((rc = lqcd_clover_apply_launch(c, w.v[5], b_o, Ai_o, n, st))) return rc;
-  // the sum rides on the hop (epilogue 6: x + scale * d), one vector pass less
-  if ((rc = lqcd_dslash_launch(c, bh, w.v[5], gauge, nullptr, b_e, 0, kappa, 0, 6, n, st))) return rc;
-  if (matpc == LQCD_MATPC_SYMMETRIC)
-    if ((rc = lqcd_clover_apply_launch(c, bh, bh, Ai_e, n, st))) return rc;
+  // the sum rides on the hop (epilogue 6: x + scale * d), one vector pass less; in a batch the clover factor of the
+  // left-symmetric form rides too (multi-RHS epilogue 14: C (x + scale * d))
+  const bool ride = n > 1 && lqcd_mrhs_fuse_ok(c);
+  if (matpc == LQCD_MATPC_SYMMETRIC && ride) {
+    if ((rc = lqcd_dslash_launch(c, bh, w.v[5], gauge, Ai_e, b_e, 0, kappa, 0, 14, n, st))) return rc;
+  } else {
+    if ((rc = lqcd_dslash_launch(c, bh, w.v[5], gauge, nullptr, b_e, 0, kappa, 0, 6, n, st))) return rc;
+    if (matpc == LQCD_MATPC_SYMMETRIC)
+      if ((rc = lqcd_clover_apply_launch(c, bh, bh, Ai_e, n, st))) return rc;
+  }
   // closing steps for n columns given by their own pointers (all columns of the batch, or one column of it):
   // unknown back to x_e (right-preconditioned form), a10: x_o = A_oo^-1 (b_o + kappa D_oe x_e), a11: the true residual
   // b - M x with the full operator into (r1, r2), its norms into S_TRUE, S_TRUE + 1
@@ -823,8 +829,12 @@ static int invert_native_body(lqcd_ctx* c, Work& w, const void* gauge, const voi
     int e;
     if (matpc == LQCD_MATPC_SYMMETRIC_RIGHT)     // the Krylov unknown was y = A_ee x_e
       if ((e = lqcd_clover_apply_launch(c, xe, xe, Ai_e, m, st))) return e;
-    if ((e = lqcd_dslash_launch(c, t5, xe, gauge, nullptr, bo, 1, kappa, 0, 6, m, st))) return e;  // b_o + kappa D_oe x_e
-    if ((e = lqcd_clover_apply_launch(c, xo, t5, Ai_o, m, st))) return e;
+    if (m > 1 && lqcd_mrhs_fuse_ok(c)) {  // x_o = A_oo^-1 (b_o + kappa D_oe x_e) in one launch
+      if ((e = lqcd_dslash_launch(c, xo, xe, gauge, Ai_o, bo, 1, kappa, 0, 14, m, st))) return e;
+    } else {
+      if ((e = lqcd_dslash_launch(c, t5, xe, gauge, nullptr, bo, 1, kappa, 0, 6, m, st))) return e;  // b_o + kappa D_oe x_e
+      if ((e = lqcd_clover_apply_launch(c, xo, t5, Ai_o, m, st))) return e;
+    }
     if (m > 1 && lqcd_mrhs_fuse_ok(c)) {
       // batch: each parity of A x - kappa D x goes straight into |b - (...)|^2 (multi-RHS epilogue 13), nothing is stored
       DslashFuse fe = {be, S_TRUE, 0, 0, nullptr}, fo = {bo, S_TRUE + 1, 0, 0, nullptr};
