@@ -18,6 +18,9 @@
 // Right-preconditioned symmetric form (Mhat_r = 1 - k^2 D_eo A_oo^-1 D_oe A_ee^-1, unknown y = A_ee x_e):
 //   9: out = x + scale * C d ; out2 = C out ; s[out_slot] = |out|^2           (t = Mhat_r^dag p and A_ee^-1 t)
 //  10: q   = x + scale * d   ; r -= (s[num]/s[den]) q ; s[out_slot] = |r|^2   (q = Mhat_r t never stored)
+// BiCGStab on the left-symmetric form (as in dslash_mrhs.cu): epilogue 3 with the inner products of the next step,
+//  11: out = x + scale * C d ; s[out_slot..+2] = Re<out,x>, Im<out,x>, |out|^2        (t = Mhat s: <t,s>, |t|^2)
+//  12: out = x + scale * C d ; s[out_slot..+2] = Re<y,out>, Im<y,out>, |y|^2, y = r   (v = Mhat p: <r0,v>)
 template <typename T> struct DslashArgs {
   T* out;
   const T* in;
@@ -81,9 +84,31 @@ __device__ __forceinline__ void dslash_reduce(double v, double* partial) {
     partial[blockIdx.x] = t;
   }
 }
+// three sums per block (epilogues 11, 12): partial[k * gridDim.x + block]
+template <int BLOCK>
+__device__ __forceinline__ void dslash_reduce3(const double (&v)[3], double* partial) {
+  __shared__ double sm3[3][BLOCK / 32];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int k = 0; k < 3; k++) {
+    double t = v[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_down_sync(0xffffffffu, t, o);
+    if (lane == 0) sm3[k][warp] = t;
+  }
+  __syncthreads();
+  if (threadIdx.x < 3) {
+    double t = 0;
+#pragma unroll
+    for (int w = 0; w < BLOCK / 32; w++) t += sm3[threadIdx.x][w];
+    partial[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = t;
+  }
+}
 constexpr int PSUM_BLOCK = 1024;
 __global__ void __launch_bounds__(PSUM_BLOCK) partial_sum_kernel(const double* __restrict__ partial, int n, double* out) {
   __shared__ double sm[PSUM_BLOCK / 32];
+  partial += (size_t)blockIdx.x * n;  // block k: the k-th sum of the launch (epilogues 11, 12: three), consecutive slots
+  out += blockIdx.x;
   double t0 = 0, t1 = 0, t2 = 0, t3 = 0;  // four independent chains, fixed assignment: deterministic
   int b = threadIdx.x;
   for (; b + 3 * PSUM_BLOCK < n; b += 4 * PSUM_BLOCK) {
@@ -111,7 +136,8 @@ __host__ __device__ constexpr bool epi_reduces(int epi) { return epi == 4 || epi
 
 // epilogue of one output site (EPI as listed at the top); `local` collects the fp64 reduction term
 template <typename T, int EPI>
-__device__ __forceinline__ void dslash_epilogue(const DslashArgs<T>& a, int idx, const T* acc, double& local) {
+__device__ __forceinline__ void dslash_epilogue(const DslashArgs<T>& a, int idx, const T* acc, double (&loc)[3]) {
+  double& local = loc[0];
   const int Vh = a.lat.Vh;
   T res[24];
   if (EPI == 0) {
@@ -159,6 +185,19 @@ __device__ __forceinline__ void dslash_epilogue(const DslashArgs<T>& a, int idx,
 #pragma unroll
       for (int e = 0; e < 24; e++) local += (double)res[e] * res[e];
     }
+    if (EPI == 11 || EPI == 12) {
+      // <u,w> = sum conj(u) w with (u, w) = (out, x) for 11, (y, out) for 12
+      T wv[24];
+      load_spinor<T>(EPI == 11 ? a.x : a.r, Vh, idx, wv);
+#pragma unroll
+      for (int e = 0; e < 24; e += 2) {
+        const double ur = EPI == 11 ? res[e] : wv[e], ui = EPI == 11 ? res[e + 1] : wv[e + 1];
+        const double wr = EPI == 11 ? wv[e] : res[e], wi = EPI == 11 ? wv[e + 1] : res[e + 1];
+        loc[0] += ur * wr + ui * wi;
+        loc[1] += ur * wi - ui * wr;
+        loc[2] += ur * ur + ui * ui;
+      }
+    }
     store_spinor<T>(a.out, Vh, idx, res);
   }
 }
@@ -168,7 +207,7 @@ __global__ void __launch_bounds__(Tune<T, R>::BLOCK, Tune<T, R>::MINB) dslash_ke
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   const bool live = idx < a.lat.Vh;
   if (!epi_reduces(EPI) && !live) return;
-  double local = 0;
+  double local[3] = {0, 0, 0};
   if (live) {
     T acc[24];
     if (Tune<T, R>::STAGE) {
@@ -179,7 +218,8 @@ __global__ void __launch_bounds__(Tune<T, R>::BLOCK, Tune<T, R>::MINB) dslash_ke
     }
     dslash_epilogue<T, EPI>(a, idx, acc, local);
   }
-  if (epi_reduces(EPI)) dslash_reduce<Tune<T, R>::BLOCK>(local, a.partial);
+  if (EPI == 11 || EPI == 12) dslash_reduce3<Tune<T, R>::BLOCK>(local, a.partial);
+  else if (epi_reduces(EPI)) dslash_reduce<Tune<T, R>::BLOCK>(local[0], a.partial);
 }
 
 // in and out may alias (lqcd.h: lqcd_clover_apply; the solvers apply A_ee^-1 in place): no __restrict__ and plain
@@ -262,9 +302,9 @@ __global__ void __launch_bounds__(TileOf<T>::NOUT, TileOf<T>::MINB) dslash_tiled
   __syncthreads();
   T acc[24];
   dslash_site_tiled<T, TS, R, DAG>(acc, dslash_smem, a.gauge, L, idx, a.parity, lxh, ly, lz, lt, s, a.ws);
-  double local = 0;
+  double local[3] = {0, 0, 0};
   dslash_epilogue<T, EPI>(a, idx, acc, local);
-  if (epi_reduces(EPI)) dslash_reduce<TS::NOUT>(local, a.partial);
+  if (epi_reduces(EPI)) dslash_reduce<TS::NOUT>(local[0], a.partial);
 }
 
 template <typename T> static bool tile_fits(const Lat& L) {
@@ -321,6 +361,8 @@ static void launch_epi(const DslashArgs<T>& a, int epi, int device, cudaStream_t
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 9>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 10>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 11>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 12>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   }
   configured[device] = true;
   switch (epi) {
@@ -334,6 +376,8 @@ static void launch_epi(const DslashArgs<T>& a, int epi, int device, cudaStream_t
     case 7: dslash_kernel<T, R, DAG, 7><<<grid, block, smem, st>>>(a); break;
     case 8: dslash_kernel<T, R, DAG, 8><<<grid, block, smem, st>>>(a); break;
     case 9: dslash_kernel<T, R, DAG, 9><<<grid, block, smem, st>>>(a); break;
+    case 11: dslash_kernel<T, R, DAG, 11><<<grid, block, smem, st>>>(a); break;
+    case 12: dslash_kernel<T, R, DAG, 12><<<grid, block, smem, st>>>(a); break;
     default: dslash_kernel<T, R, DAG, 10><<<grid, block, smem, st>>>(a); break;
   }
 }
@@ -407,6 +451,10 @@ int lqcd_dslash_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge
 bool lqcd_dslash_fuse_ok(const lqcd_ctx* c) {
   return !c->half && (long)lqcd_dslash_grid(c) <= 4L * c->max_red_blocks * LQCD_MAX_RHS;
 }
+// ... and the epilogues with three sums (11, 12) when three times as many do
+bool lqcd_dslash_fuse3_ok(const lqcd_ctx* c) {
+  return !c->half && 3L * lqcd_dslash_grid(c) <= 4L * c->max_red_blocks * LQCD_MAX_RHS;
+}
 
 int lqcd_partial_sum_launch(lqcd_ctx* c, int n, int slot, cudaStream_t st) {
   partial_sum_kernel<<<1, PSUM_BLOCK, 0, st>>>(c->d_partial, n, c->d_scalars + slot);
@@ -419,15 +467,16 @@ int lqcd_dslash_fused_launch(lqcd_ctx* c, void* out, const void* in, const void*
   if (c->half) return lqcd_dslash_half_launch(c, out, in, gauge, cl, x, parity, scale, dagger, epi, st, f);
   // epi 4: as epi 2; epi 7: as epi 6 (no clover); epi 9: as epi 3 + a second output.  epi 5, 8, 10: no output
   // store, r read and written instead
+  // epi 11: as epi 3 ; epi 12: as epi 3 + y read
   const double bytes = (double)c->lat.Vh * c->prec *
                        (8.0 * c->recon + 48.0 + (epi == 7 || epi == 10 ? 0.0 : 72.0) + 24.0 +
-                        (epi == 5 || epi == 8 || epi == 9 || epi == 10 ? 24.0 : 0.0));
+                        (epi == 5 || epi == 8 || epi == 9 || epi == 10 || epi == 12 ? 24.0 : 0.0));
   c->alg_bytes += bytes;
   const bool rec = c->prof_on && c->prof_n < c->prof_cap;
   if (rec) cudaEventRecord(c->prof_ev[2 * c->prof_n], st);
   if (c->prec == 4) launch_typed<float>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, f, st);
   else launch_typed<double>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, f, st);
-  partial_sum_kernel<<<1, PSUM_BLOCK, 0, st>>>(c->d_partial, lqcd_dslash_grid(c), c->d_scalars + f->out_slot);
+  partial_sum_kernel<<<epi >= 11 ? 3 : 1, PSUM_BLOCK, 0, st>>>(c->d_partial, lqcd_dslash_grid(c), c->d_scalars + f->out_slot);
   c->launches++;
   if (rec) {
     cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], st);

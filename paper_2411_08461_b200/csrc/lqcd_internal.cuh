@@ -270,6 +270,7 @@ struct DslashFuse {
   void* out2;    // epi 9: second output, C * out
 };
 bool lqcd_dslash_fuse_ok(const lqcd_ctx* c);
+bool lqcd_dslash_fuse3_ok(const lqcd_ctx* c);
 int lqcd_dslash_fused_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,
                              int parity, double scale, int dagger, int epi, const DslashFuse* f, cudaStream_t st);
 int lqcd_dslash_mrhs_launch(lqcd_ctx* c, void* out, const void* in, const void* gauge, const void* cl, const void* x,

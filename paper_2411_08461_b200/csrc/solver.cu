@@ -477,9 +477,15 @@ static int solve_bicgstab(lqcd_ctx* c, const Work& w, const void* gauge, const v
     // (measured: 16^3x32 fp32 6.09 -> 5.60 ms, 32^3x64 fp64 195.8 -> 186.0 ms per 12-column solve); the fused launch runs on
     // the TMA-tiled kernel where that serves epilogue 3, on the register kernel elsewhere.  LQCD_MRHS_FUSE_DOTS=0: off.
     const bool fuse_dots = n > 1 && matpc == LQCD_MATPC_SYMMETRIC && lqcd_mrhs_fuse_ok(c) && c->mrhs_fuse_dots != 0;
+    // one column: the same two epilogues in the single-RHS kernel (dslash.cu)
+    const bool fuse1 = n == 1 && matpc == LQCD_MATPC_SYMMETRIC && lqcd_dslash_fuse3_ok(c) && c->mrhs_fuse_dots != 0;
     const size_t half = lqcd_clover_bytes(c) / 2;
     const double k2 = -kappa * kappa;
-    if (fuse_dots) {
+    if (fuse1) {
+      DslashFuse f12 = {r0, S_R0V, 0, 0, nullptr};
+      if ((rc = lqcd_dslash_launch(c, tmp, p, gauge, off(Ai, half), nullptr, 1, 1.0, 0, 1, 1, st))) return rc;
+      if ((rc = lqcd_dslash_fused_launch(c, v, tmp, gauge, Ai, p, 0, k2, 0, 12, &f12, st))) return rc;
+    } else if (fuse_dots) {
       DslashFuse f12 = {r0, S_R0V, 0, 0, nullptr};
       if ((rc = lqcd_dslash_launch(c, tmp, p, gauge, off(Ai, half), nullptr, 1, 1.0, 0, 1, n, st))) return rc;
       if ((rc = lqcd_dslash_mrhs_fused_launch(c, v, tmp, gauge, Ai, p, 0, k2, 0, 12, n, &f12, st))) return rc;
@@ -493,7 +499,11 @@ static int solve_bicgstab(lqcd_ctx* c, const Work& w, const void* gauge, const v
       void* u2[3] = {s, r, v};
       if ((rc = BLAS_CALL(c, OpBicgS, (op.rho = rho, op.r0v = S_R0V), u2, nullptr, n, 0, st))) return rc;
     }
-    if (fuse_dots) {
+    if (fuse1) {
+      DslashFuse f11 = {nullptr, S_TS, 0, 0, nullptr};
+      if ((rc = lqcd_dslash_launch(c, tmp, s, gauge, off(Ai, half), nullptr, 1, 1.0, 0, 1, 1, st))) return rc;
+      if ((rc = lqcd_dslash_fused_launch(c, t, tmp, gauge, Ai, s, 0, k2, 0, 11, &f11, st))) return rc;
+    } else if (fuse_dots) {
       DslashFuse f11 = {nullptr, S_TS, 0, 0, nullptr};
       if ((rc = lqcd_dslash_launch(c, tmp, s, gauge, off(Ai, half), nullptr, 1, 1.0, 0, 1, n, st))) return rc;
       if ((rc = lqcd_dslash_mrhs_fused_launch(c, t, tmp, gauge, Ai, s, 0, k2, 0, 11, n, &f11, st))) return rc;

@@ -162,6 +162,34 @@ def test_config2_mixed_precision_reaches_fp64_tolerance(solver, recon_lo):
         s.ctx.invert_mixed(s.ctx, s.ctx.to_device(b), s.gauge, s.A, s.Ai, s.gauge, s.A, s.Ai, s.kappa)
 
 
+@pytest.mark.parametrize("prec,recon,tol", [(8, 18, 1e-10), (8, 12, 1e-10), (4, 12, 1e-6)])
+def test_single_bicgstab_inner_products_in_the_epilogues(prec, recon, tol, monkeypatch):
+    """BiCGStab on the left-symmetric form, one column: <r0,v> and <t,s>, |t|^2 come out of epilogues 12 and 11 of the
+    single-RHS dslash kernel (three per-block partials, fixed-order sums); LQCD_MRHS_FUSE_DOTS=0 takes them from BLAS-1
+    passes instead.  Both meet reading A17, agree on the iteration count to +-1, and the fused solve is reproducible
+    bit for bit."""
+    dims = (8, 6, 8, 12)
+    b = synth.source(dims, "gaussian", 77)
+    out = {}
+    for name, env in (("fused", None), ("blas", "0")):
+        if env is None:
+            monkeypatch.delenv("LQCD_MRHS_FUSE_DOTS", raising=False)
+        else:
+            monkeypatch.setenv("LQCD_MRHS_FUSE_DOTS", env)
+        s = Setup(dims, 0.5, 4, 0.124, 1.2, prec, recon)
+        bb = synth.round_fp32(b) if prec == 4 else b
+        runs = []
+        for _ in range(2):
+            x, res = s.ctx.invert(s.ctx.to_device(bb), s.gauge, s.A, s.Ai, s.kappa, tol=tol, maxiter=500, solver="bicgstab", matpc=1)
+            runs.append(x.clone())
+        assert torch.equal(runs[0], runs[1])
+        true = s.orc.true_residual(bb, x.cpu().numpy().astype(np.complex128))
+        assert res.status == 0 and true < tol, (name, true, res.as_dict())
+        out[name] = res.iterations
+        s.ctx.close()
+    assert abs(out["fused"] - out["blas"]) <= 1, out
+
+
 @pytest.mark.parametrize("margin", ["1e30", "0", None])
 @pytest.mark.parametrize("solver,matpc", [("cgne", 2), ("bicgstab", 1), ("cgne", 0)])
 def test_mixed_last_outer_step_guess(solver, matpc, margin, monkeypatch):
