@@ -21,6 +21,9 @@
 // BiCGStab on the left-symmetric form (as in dslash_mrhs.cu): epilogue 3 with the inner products of the next step,
 //  11: out = x + scale * C d ; s[out_slot..+2] = Re<out,x>, Im<out,x>, |out|^2        (t = Mhat s: <t,s>, |t|^2)
 //  12: out = x + scale * C d ; s[out_slot..+2] = Re<y,out>, Im<y,out>, |y|^2, y = r   (v = Mhat p: <r0,v>)
+// Closing steps of a solve (as in dslash_mrhs.cu):
+//  13: s[out_slot] = |y - (C x + scale * d)|^2, y = r, nothing stored   (one parity of the true residual b - M x)
+//  14: out = C (x + scale * d)                                           (b-hat of the left-symmetric form; x_o)
 template <typename T> struct DslashArgs {
   T* out;
   const T* in;
@@ -132,7 +135,7 @@ __global__ void __launch_bounds__(PSUM_BLOCK) partial_sum_kernel(const double* _
   }
 }
 
-__host__ __device__ constexpr bool epi_reduces(int epi) { return epi == 4 || epi == 5 || epi >= 7; }
+__host__ __device__ constexpr bool epi_reduces(int epi) { return epi == 4 || epi == 5 || (epi >= 7 && epi != 14); }
 
 // epilogue of one output site (EPI as listed at the top); `local` collects the fp64 reduction term
 template <typename T, int EPI>
@@ -147,7 +150,7 @@ __device__ __forceinline__ void dslash_epilogue(const DslashArgs<T>& a, int idx,
     clover_mul<T>(a.cl, Vh, idx, acc, res);
 #pragma unroll
     for (int e = 0; e < 24; e++) res[e] *= a.scale;
-  } else if (EPI == 2 || EPI == 4 || EPI == 5) {
+  } else if (EPI == 2 || EPI == 4 || EPI == 5 || EPI == 13) {
     T xv[24];
     load_spinor<T>(a.x, Vh, idx, xv);
     clover_mul<T>(a.cl, Vh, idx, xv, res);
@@ -157,6 +160,12 @@ __device__ __forceinline__ void dslash_epilogue(const DslashArgs<T>& a, int idx,
     load_spinor<T>(a.x, Vh, idx, res);
 #pragma unroll
     for (int e = 0; e < 24; e++) res[e] += a.scale * acc[e];
+  } else if (EPI == 14) {
+    T xv[24];
+    load_spinor<T>(a.x, Vh, idx, xv);
+#pragma unroll
+    for (int e = 0; e < 24; e++) xv[e] += a.scale * acc[e];
+    clover_mul<T>(a.cl, Vh, idx, xv, res);
   } else if (EPI == 9) {
     T xv[24], res2[24];
     load_spinor<T>(a.x, Vh, idx, xv);
@@ -180,6 +189,14 @@ __device__ __forceinline__ void dslash_epilogue(const DslashArgs<T>& a, int idx,
       local += (double)rv[e] * rv[e];
     }
     store_spinor<T>(a.r, Vh, idx, rv);
+  } else if (EPI == 13) {
+    T yv[24];
+    load_spinor<T>(a.r, Vh, idx, yv);
+#pragma unroll
+    for (int e = 0; e < 24; e++) {
+      const double dlt = (double)yv[e] - (double)res[e];
+      local += dlt * dlt;
+    }
   } else {
     if (EPI == 4 || EPI == 7 || EPI == 9) {
 #pragma unroll
@@ -363,6 +380,8 @@ static void launch_epi(const DslashArgs<T>& a, int epi, int device, cudaStream_t
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 10>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 11>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 12>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 13>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(dslash_kernel<T, R, DAG, 14>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   }
   configured[device] = true;
   switch (epi) {
@@ -378,6 +397,8 @@ static void launch_epi(const DslashArgs<T>& a, int epi, int device, cudaStream_t
     case 9: dslash_kernel<T, R, DAG, 9><<<grid, block, smem, st>>>(a); break;
     case 11: dslash_kernel<T, R, DAG, 11><<<grid, block, smem, st>>>(a); break;
     case 12: dslash_kernel<T, R, DAG, 12><<<grid, block, smem, st>>>(a); break;
+    case 13: dslash_kernel<T, R, DAG, 13><<<grid, block, smem, st>>>(a); break;
+    case 14: dslash_kernel<T, R, DAG, 14><<<grid, block, smem, st>>>(a); break;
     default: dslash_kernel<T, R, DAG, 10><<<grid, block, smem, st>>>(a); break;
   }
 }
@@ -476,7 +497,7 @@ int lqcd_dslash_fused_launch(lqcd_ctx* c, void* out, const void* in, const void*
   if (rec) cudaEventRecord(c->prof_ev[2 * c->prof_n], st);
   if (c->prec == 4) launch_typed<float>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, f, st);
   else launch_typed<double>(c, out, in, gauge, cl, x, parity, scale, dagger, epi, f, st);
-  partial_sum_kernel<<<epi >= 11 ? 3 : 1, PSUM_BLOCK, 0, st>>>(c->d_partial, lqcd_dslash_grid(c), c->d_scalars + f->out_slot);
+  partial_sum_kernel<<<epi == 11 || epi == 12 ? 3 : 1, PSUM_BLOCK, 0, st>>>(c->d_partial, lqcd_dslash_grid(c), c->d_scalars + f->out_slot);
   c->launches++;
   if (rec) {
     cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], st);

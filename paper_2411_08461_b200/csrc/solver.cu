@@ -824,7 +824,7 @@ static int invert_native_body(lqcd_ctx* c, Work& w, const void* gauge, const voi
   if ((rc = lqcd_clover_apply_launch(c, w.v[5], b_o, Ai_o, n, st))) return rc;
   // the sum rides on the hop (epilogue 6: x + scale * d), one vector pass less; in a batch the clover factor of the
   // left-symmetric form rides too (multi-RHS epilogue 14: C (x + scale * d))
-  const bool ride = n > 1 && lqcd_mrhs_fuse_ok(c);
+  const bool ride = n > 1 ? lqcd_mrhs_fuse_ok(c) : (!c->half && lqcd_dslash_fuse_ok(c));
   if (matpc == LQCD_MATPC_SYMMETRIC && ride) {
     if ((rc = lqcd_dslash_launch(c, bh, w.v[5], gauge, Ai_e, b_e, 0, kappa, 0, 14, n, st))) return rc;
   } else {
@@ -839,7 +839,8 @@ static int invert_native_body(lqcd_ctx* c, Work& w, const void* gauge, const voi
     int e;
     if (matpc == LQCD_MATPC_SYMMETRIC_RIGHT)     // the Krylov unknown was y = A_ee x_e
       if ((e = lqcd_clover_apply_launch(c, xe, xe, Ai_e, m, st))) return e;
-    if (m > 1 && lqcd_mrhs_fuse_ok(c)) {  // x_o = A_oo^-1 (b_o + kappa D_oe x_e) in one launch
+    const bool ride1 = m == 1 && !c->half && lqcd_dslash_fuse_ok(c);  // one column: the same epilogues in dslash.cu
+    if ((m > 1 && lqcd_mrhs_fuse_ok(c)) || ride1) {  // x_o = A_oo^-1 (b_o + kappa D_oe x_e) in one launch
       if ((e = lqcd_dslash_launch(c, xo, xe, gauge, Ai_o, bo, 1, kappa, 0, 14, m, st))) return e;
     } else {
       if ((e = lqcd_dslash_launch(c, t5, xe, gauge, nullptr, bo, 1, kappa, 0, 6, m, st))) return e;  // b_o + kappa D_oe x_e
@@ -851,6 +852,12 @@ static int invert_native_body(lqcd_ctx* c, Work& w, const void* gauge, const voi
       if ((e = lqcd_dslash_mrhs_fused_launch(c, nullptr, xo, gauge, A, xe, 0, -kappa, 0, 13, m, &fe, st))) return e;
       if ((e = lqcd_dslash_mrhs_fused_launch(c, nullptr, xe, gauge, off(A, half), xo, 1, -kappa, 0, 13, m, &fo, st))) return e;
       return read_scalars(c, m, st);
+    }
+    if (ride1) {
+      DslashFuse fe = {be, S_TRUE, 0, 0, nullptr}, fo = {bo, S_TRUE + 1, 0, 0, nullptr};
+      if ((e = lqcd_dslash_fused_launch(c, nullptr, xo, gauge, A, xe, 0, -kappa, 0, 13, &fe, st))) return e;
+      if ((e = lqcd_dslash_fused_launch(c, nullptr, xe, gauge, off(A, half), xo, 1, -kappa, 0, 13, &fo, st))) return e;
+      return read_scalars(c, 1, st);
     }
     if ((e = lqcd_dslash_launch(c, r1, xo, gauge, A, xe, 0, -kappa, 0, 2, m, st))) return e;
     if ((e = lqcd_dslash_launch(c, r2, xe, gauge, off(A, half), xo, 1, -kappa, 0, 2, m, st))) return e;
